@@ -1,0 +1,143 @@
+/*
+ * gcmcrt_oracle.h -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, serial, fp64 CPU restatement of the hot path of gCMCRT
+ * (arXiv 2110.15640; /root/reference/PAPER.md): Monte Carlo photon-packet
+ * transport with next-event estimation ("peel-off") for albedo and emission
+ * spectra on a 3D spherical-polar grid.  It follows the paper step by step in
+ * the paper's order (citations are "PAPER.md:Lnnn, section/equation") and the
+ * readings C1..C20 of SURVEY.md section 8(c), restated in DESIGN.md.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference leg may build, load or call this.  It shares no code,
+ * header, table or constant generator with paper_2110_15640_b200/ (the CUDA
+ * path) and neither imports the other.
+ *
+ * Pins (tests/test_oracle_*.py, all `-m "not gpu"`): Philox known-answer
+ * vectors; closed-form CDFs and moments of every phase-function sampler;
+ * analytic chord optical depths; grid-refinement invariance; e^{-tau}
+ * transmission; Lambert sphere 2/3 and its phase law; exact Chandrasekhar
+ * H-function albedos; isothermal emitter chord integral; energy conservation;
+ * peel-off <-> escape consistency; brute-force enumeration on a 1-cell grid;
+ * rotational invariance; Eq. 33 vector identity.
+ * Paper-printed numeric values: none exist (Fig. 1 is an image) -> "parity
+ * against paper-printed values: unpinned"; every function is pinned by the
+ * closed forms above instead.
+ */
+#ifndef GCMCRT_ORACLE_H
+#define GCMCRT_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* D1/D2/D4/D5: the 3D spherical grid and
+ * its per-cell fields, cell-flat index = (k*nlat + j)*nlev + i with i the
+ * radial (fastest) index, j colatitude, k longitude. */
+typedef struct {
+    int nlev, nlat, nlon;
+    const double *r_edges;     /* [nlev+1] ascending, m; [0]=R_p0, [nlev]=R_TOA */
+    const double *colat_edges; /* [nlat+1] 0..pi */
+    const double *lon_edges;   /* [nlon+1] 0..2pi */
+    const float *T;            /* [ncell] K */
+    const float *rho;          /* [ncell] kg m^-3 */
+    const float *u, *v, *w;    /* [ncell] m/s east, north, up; nullable */
+    double Omega;              /* rad/s */
+    double surface_albedo;     /* 0 = absorbing lower boundary (C5) */
+} orc_grid;
+
+/* D3: per channel, per cell opacities. */
+typedef struct {
+    int n_chan;
+    int chan0;               /* global index of the first channel (Philox key) */
+    const float *lambda;     /* [n_chan] m */
+    const float *k_abs;      /* [n_chan][ncell] m^2/kg */
+    const float *k_sca_ray;  /* nullable */
+    const float *k_sca_cld;  /* nullable */
+    const float *g_cld;      /* nullable -> 0 */
+} orc_opacity;
+
+typedef struct {
+    double star_dir[3];
+    int n_obs;
+    const double *obs_dir;   /* [n_obs][3] unit vectors */
+    uint64_t packets_per_channel; /* N: defines batches and normalisation */
+    uint64_t pkt_begin, pkt_end;  /* packet ids simulated, [begin,end) within [0,N) */
+    uint64_t seed;
+    int max_events;          /* 0 = unlimited */
+    int scatter_on;
+    int doppler_on;
+    int doppler_halfwidth;   /* W, in wavelength points */
+    double emission_bias;    /* xi (C10) */
+    double tau_vert_max;     /* <=0: no cut (L210) */
+    double tau_cut;          /* peel-off contributions with tau_obs > tau_cut are 0 */
+    int npix;                /* 0 = no images */
+    int n_batches;
+    int n_threads;           /* OpenMP threads over batches; <=1 serial */
+} orc_params;
+
+typedef struct {
+    uint64_t events;             /* peel-off points */
+    uint64_t segments_transport; /* cell crossings on flights */
+    uint64_t segments_peel;      /* cell crossings on peel-off rays */
+    uint64_t packets_escaped, packets_absorbed, packets_surface, packets_stuck;
+    double escaped_weight;
+} orc_counters;
+
+typedef struct {
+    double *flux_sum;      /* [n_chan][n_obs][n_batches] raw sums of f (Eq. 14) */
+    double *L_tot;         /* [n_chan] (emission; with doppler_on [n_chan][n_obs]) */
+    double *image;         /* nullable [n_chan][n_obs][npix][npix] */
+    uint32_t *event_count; /* nullable [n_chan][N] */
+    orc_counters counters;
+} orc_result;
+
+/* A3: Philox4x32-10 (Salmon et al. 2011), C2. */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+/* C2: zeta = ((u>>9)+0.5) * 2^-23 (exact in fp32 and fp64) */
+double orc_u32_to_zeta(uint32_t u);
+/* The block of four zetas for (seed, channel, packet, event, purpose). */
+void orc_zeta_block(uint64_t seed, uint32_t chan, uint32_t pkt, uint32_t event, uint32_t purpose, double z[4]);
+
+/* Phase-function samplers (Eq. 2, 4, 6 [C7], 8 [C8]) and densities per steradian. */
+double orc_sample_isotropic(double zeta);
+double orc_sample_lambert(double zeta);
+double orc_sample_rayleigh(double zeta);
+double orc_sample_hg(double g, double zeta);
+double orc_phase_rayleigh(double mu);
+double orc_phase_hg(double g, double mu);
+/* C9: rotate unit vector n by polar angle acos(ct) and azimuth psi. */
+void orc_rotate(const double n[3], double ct, double psi, double out[3]);
+
+/* O1: cell volume. */
+double orc_cell_volume(const orc_grid *g, int i, int j, int k);
+/* Locate (i,j,k) of a point (used for launch and for debug rays). */
+void orc_locate(const orc_grid *g, const double p[3], int ijk[3]);
+/* B_lambda(T), SI (W m^-3 sr^-1). */
+double orc_planck(double lambda, double T);
+/* O9 / Eq. 33: line-of-sight velocity, both the paper's trigonometric form and the vector form. */
+double orc_vlos_eq33(double u, double v, double w, double Omega, double r, double theta, double phi,
+                     double theta_v, double phi_v);
+double orc_vlos_vector(double u, double v, double w, double Omega, double r, double theta, double phi,
+                       const double obs[3]);
+
+/* O5: optical depth from p along dir to the TOA for channel `chan` (local index)
+ * (observer index obs_index selects the Doppler table; -1 = unshifted).
+ * hit_surface[m]=1 if the ray ends on the lower boundary.  nseg/path optional. */
+int orc_ray_tau(const orc_grid *g, const orc_opacity *op, int chan, long n,
+                const double *pos, const double *dir, double *tau, int *hit_surface,
+                long *nseg, double *path_len);
+
+/* O2: staged per-cell quantities of one channel (for tests): alpha_ext, omega, pgas, g, L_i, cdf. */
+int orc_channel_prep(const orc_grid *g, const orc_opacity *op, const orc_params *prm, int chan, int obs_index,
+                     double *alpha, double *omega, double *pgas, double *gg, double *L_cell, double *L_tot);
+
+/* The two drivers (section 3 call stacks). */
+int orc_run_albedo(const orc_grid *g, const orc_opacity *op, const orc_params *prm, orc_result *out);
+int orc_run_emission(const orc_grid *g, const orc_opacity *op, const orc_params *prm, orc_result *out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

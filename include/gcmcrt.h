@@ -1,0 +1,169 @@
+/*
+ * gcmcrt.h -- C-ABI of libgcmcrt.so: the B200-native (sm_100a) hot path of gCMCRT
+ * (Lee et al., arXiv 2110.15640; citations below are /root/reference/PAPER.md line numbers).
+ *
+ * What the library computes: Monte Carlo photon-packet transport through a 3D spherical-polar
+ * atmosphere (radius shells x colatitude cones x longitude half-planes) with
+ * next-event estimation ("peel-off", Sect. 4.6, Eq. 14) toward one or more observers, for
+ * scattered-light (albedo, Sect. 5.2) and thermal-emission (Sect. 5.3) spectra, per wavelength or
+ * correlated-k g-ordinate ("channel").  Every step runs in hand-written CUDA kernels; there is no
+ * CPU fallback: without a CUDA device every entry point that needs one returns GCMCRT_E_CUDA.
+ *
+ * Conventions
+ *  - SI units: m, K, kg m^-3, m^2 kg^-1, rad, m/s.  Colatitude theta from +z, longitude phi from +x.
+ *  - Cell-flat layout of every per-cell array: [nlon][nlat][nlev], the radial index fastest.
+ *    Per-channel tables are [n_chan][nlon][nlat][nlev] (wavelength-major).
+ *  - POINTERS: every array argument documented "host|device" may live in host memory (pageable or
+ *    pinned) or in device memory; the library asks cudaPointerGetAttributes and copies host arrays
+ *    to / from internal device buffers with cudaMemcpyAsync on the caller's stream.  Arguments
+ *    documented "host" are read on the CPU during the call.
+ *  - OWNERSHIP: the library copies or stages everything it needs during the call that receives it,
+ *    EXCEPT the device-resident k_abs table given to gcmcrt_set_opacity, which is borrowed until
+ *    the next gcmcrt_set_opacity / gcmcrt_destroy when a later run uses doppler_on (the shifted
+ *    tables are rebuilt from it per observer, Eq. 33-34).  Output buffers are caller-owned.
+ *  - STREAMS: all work is enqueued on `stream` (a cudaStream_t passed as void*, NULL = legacy
+ *    default stream).  gcmcrt_run_* synchronise with the stream only to read two pass counters per
+ *    pass (a few bytes); results are complete when the stream has drained (or on return for host
+ *    output pointers, which are copied with a final stream synchronisation).
+ *  - ERRORS: every function returns 0 on success or a negative gcmcrt_status; nothing throws or
+ *    exits.  gcmcrt_last_error() returns a static, human-readable description of the last failure
+ *    on that handle (or of the last failed gcmcrt_grid_create when passed NULL).
+ *  - THREADS: one handle is not thread-safe; distinct handles are independent.
+ */
+#ifndef GCMCRT_H
+#define GCMCRT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gcmcrt_grid gcmcrt_grid;
+
+typedef enum gcmcrt_status {
+    GCMCRT_OK = 0,
+    GCMCRT_E_INVALID = -1, /* bad argument (NULL, non-monotonic edges, sizes <= 0, ...) */
+    GCMCRT_E_NOMEM = -2,   /* host or device allocation failed */
+    GCMCRT_E_CUDA = -3,    /* a CUDA runtime call or kernel failed, or no device */
+    GCMCRT_E_STATE = -4    /* call order: run before set_opacity, ... */
+} gcmcrt_status;
+
+/* Run parameters (every default in parentheses is what 0 selects). */
+typedef struct gcmcrt_run_params {
+    double star_dir[3];          /* unit vector planet -> star (albedo launch) */
+    int n_obs;                   /* number of observer directions (>= 0) */
+    const double *obs_dir;       /* host [n_obs][3] unit vectors planet -> observer (L326-328) */
+    uint64_t packets_per_channel;/* N: normalisation and batch definition */
+    uint64_t pkt_begin, pkt_end; /* simulate packet ids [pkt_begin, pkt_end) of [0, N); pkt_end = 0 -> N */
+    uint64_t seed;               /* Philox counter words 2,3 */
+    int chan_begin, chan_end;    /* channels (local indices of the current table) to run; chan_end = 0 -> all */
+    int max_events;              /* stop a packet after this many interactions (0 = unlimited) */
+    int scatter_on;              /* 0: only the first peel-off point of each packet (L210, L301) */
+    int doppler_on;              /* 1: per-observer Doppler-shifted k_abs (Eq. 33-34), one run per observer */
+    int doppler_halfwidth;       /* W: shift clamped to +-W wavelength points (moving window, L403) */
+    double emission_bias;        /* xi of the composite emission bias (Sect. 4.3; 0 = unbiased Eq. 13) */
+    double tau_vert_max;         /* emission depth cut (L210); <= 0 disables */
+    double tau_cut;              /* peel-off contributions with tau_obs > tau_cut are dropped (0 -> 50) */
+    int npix;                    /* image side (0 = no images) */
+    int n_batches;               /* batches for the batch-means sigma (0 -> 32, max 64) */
+} gcmcrt_run_params;
+
+typedef struct gcmcrt_counters {
+    uint64_t events;             /* peel-off points (emission launches, interactions, surface hits) */
+    uint64_t segments_transport; /* cell crossings on packet flights */
+    uint64_t segments_peel;      /* cell crossings on peel-off rays */
+    uint64_t packets_escaped, packets_absorbed, packets_surface, packets_stuck;
+    double escaped_weight;
+    uint64_t passes;             /* transport/peel kernel pairs launched */
+    uint64_t rays_peel;          /* peel-off rays integrated */
+} gcmcrt_counters;
+
+/* Output buffers, all caller-owned, host|device, nullable unless stated. */
+typedef struct gcmcrt_result {
+    double *flux_sum;      /* REQUIRED [n_chan_run][n_obs][n_batches]: raw sums of f (Eq. 14) */
+    double *L_tot;         /* [n_chan_run][n_obs]: total luminosity (Eq. 27-28), emission only */
+    double *value;         /* [n_chan_run][n_obs]: albedo: reflected fraction per steradian S/N (A_g = pi*value at
+                              zero phase, Eq. 24); emission: L_p = L_tot S/N in W m^-1 sr^-1 (Eq. 28) */
+    double *sigma;         /* [n_chan_run][n_obs]: batch-means standard error of value */
+    float *image;          /* [n_chan_run][n_obs][npix][npix] (L83) */
+    uint32_t *event_count; /* [n_chan_run][pkt_end-pkt_begin]: peel-off points per packet */
+    gcmcrt_counters *counters; /* one struct */
+} gcmcrt_result;
+
+/*
+ * gcmcrt_grid_create -- build the 3D spherical grid (D1, D2, D4, D5) and stage its
+ * geometry tables on the current CUDA device.
+ *   r_edges[nlev+1]     host, strictly ascending; r_edges[0] = lower boundary R_p0, last = R_TOA
+ *   colat_edges[nlat+1] host, ascending, must span 0..pi   (nlat = 1: no cones at all)
+ *   lon_edges[nlon+1]   host, ascending, must span 0..2pi  (nlon = 1: no half-planes)
+ *   T, rho              host|device [nlon][nlat][nlev] (copied)
+ *   u, v, w             host|device, same layout, nullable (east, north, up wind; Eq. 33), copied
+ *   Omega               rotation rate (Eq. 33)
+ *   surface_albedo      Lambert albedo of the lower boundary (Eq. 3-4); 0 = absorbing
+ * Errors: E_INVALID (NULL, sizes, non-monotonic), E_NOMEM, E_CUDA.  *out is NULL on failure.
+ */
+int gcmcrt_grid_create(gcmcrt_grid **out, int nlev, int nlat, int nlon,
+                       const double *r_edges, const double *colat_edges, const double *lon_edges,
+                       const float *T, const float *rho,
+                       const float *u, const float *v, const float *w, double Omega,
+                       float surface_albedo, void *stream);
+
+/*
+ * gcmcrt_set_opacity -- give the per-channel, per-cell opacities (D3) of
+ * channels chan0 .. chan0+n_chan-1 and stage alpha_ext = rho (k_abs + k_ray + k_cld), omega, P_gas (Eq. 11)
+ * and g per (channel, cell) (A0).  chan0 is the global index of the first channel: it keys the random
+ * streams, so results do not depend on how a long table is cut into batches.
+ *   lambda[n_chan]  host, m (Planck function, Doppler spacing)
+ *   k_abs           host|device [n_chan][nlon][nlat][nlev], required (device memory is borrowed, see above)
+ *   k_sca_ray       host|device, nullable (= 0): Rayleigh scattering opacity
+ *   k_sca_cld       host|device, nullable (= 0): cloud scattering opacity
+ *   g_cld           host|device, nullable (= 0): HG asymmetry of the cloud scatterers
+ * Errors: E_INVALID, E_NOMEM, E_CUDA.
+ */
+int gcmcrt_set_opacity(gcmcrt_grid *grid, int chan0, int n_chan, const float *lambda,
+                       const float *k_abs, const float *k_sca_ray, const float *k_sca_cld,
+                       const float *g_cld, void *stream);
+
+/*
+ * gcmcrt_run_albedo -- scattered-light run (Sect. 5.2): packets enter uniformly over the star-facing TOA disc
+ * (incident flux normalised to 1, L283), fly sampled optical depths (L192), peel off to every observer at every
+ * interaction (Eq. 14), scatter with Rayleigh (Eq. 5-6) / Henyey-Greenstein (Eq. 7-8) chosen by P_gas (Eq. 11)
+ * or are absorbed (L192).
+ * gcmcrt_run_emission -- thermal run (Sect. 5.3): packets are emitted from cells in proportion to their
+ * luminosity (Eq. 13, Eq. 27; composite bias xi), peel off at the emission point (L210) and, if scatter_on,
+ * continue as above.  value = L_tot/N sum f (Eq. 28).
+ * Errors: E_STATE (no opacity set), E_INVALID, E_NOMEM, E_CUDA.
+ */
+int gcmcrt_run_albedo(gcmcrt_grid *grid, const gcmcrt_run_params *params, gcmcrt_result *out, void *stream);
+int gcmcrt_run_emission(gcmcrt_grid *grid, const gcmcrt_run_params *params, gcmcrt_result *out, void *stream);
+
+/* gcmcrt_destroy -- synchronise the device, free everything the handle owns.  NULL is a no-op. */
+int gcmcrt_destroy(gcmcrt_grid *grid);
+
+/* Text of the last error on this handle (NULL: last failed gcmcrt_grid_create).  Never NULL. */
+const char *gcmcrt_last_error(const gcmcrt_grid *grid);
+
+/*
+ * gcmcrt_debug_ray_tau -- test-only: optical depth of channel `chan` (local index) from pos[m] along dir[m] to
+ * the TOA with the peel-off ray integrator (A7), without a run.  hit_surface[m] = 1 when the ray ends on the
+ * lower boundary (tau then is the depth down to it).  obs_index >= 0 selects that observer's Doppler-shifted
+ * table (requires a previous run with doppler_on), -1 the unshifted one.
+ *   pos, dir  host|device [n][3] float; tau host|device [n] float; hit_surface host|device [n] int (nullable)
+ */
+int gcmcrt_debug_ray_tau(gcmcrt_grid *grid, int chan, long n, const float *pos, const float *dir,
+                         float *tau, int *hit_surface, void *stream);
+
+/*
+ * gcmcrt_debug_philox -- test-only: out[m][4] = Philox4x32-10(counter = ctr[m][4], key = key[m][2]) computed on
+ * the device by the generator the packet kernels use (A3); all arrays host|device.
+ */
+int gcmcrt_debug_philox(long n, const uint32_t *ctr, const uint32_t *key, uint32_t *out, void *stream);
+
+/* Library build information: "gcmcrt <version> sm_100a ..." */
+const char *gcmcrt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GCMCRT_H */

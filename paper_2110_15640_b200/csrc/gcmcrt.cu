@@ -1,0 +1,635 @@
+// gcmcrt.cu -- host side of libgcmcrt.so: the C-ABI of include/gcmcrt.h.
+// Argument marshalling, device-memory ownership, kernel launches and the pass loop; all arithmetic of the method
+// lives in kernels.cuh / ray.cuh / device_common.cuh.
+#include "../../include/gcmcrt.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "kernels.cuh"
+
+using namespace gcmcrt;
+
+namespace {
+
+thread_local std::string g_create_error = "no error";
+
+struct DevBuf {  // owned device allocation
+    void* p = nullptr;
+    size_t bytes = 0;
+    void release() { if (p) cudaFree(p); p = nullptr; bytes = 0; }
+    cudaError_t ensure(size_t n)
+    {
+        if (n <= bytes) return cudaSuccess;
+        release();
+        cudaError_t e = cudaMalloc(&p, n);
+        if (e == cudaSuccess) bytes = n; else p = nullptr;
+        return e;
+    }
+    template <class T> T* as() const { return static_cast<T*>(p); }
+};
+
+struct PassCtrl {  // small device block reset every pass
+    unsigned int ev_count;
+    unsigned int susp_count[2];
+    unsigned int susp_taken[2];
+    unsigned int pad;
+    unsigned long long work_counter;
+    unsigned long long ray_counter;
+};
+
+}  // namespace
+
+struct gcmcrt_grid {
+    int nlev = 0, nlat = 0, nlon = 0, ncell = 0;
+    std::vector<double> r, th, ph;
+    double Omega = 0.0;
+    float surface_albedo = 0.f;
+    int sm_count = 148;
+    std::string err = "no error";
+
+    // geometry + fields
+    DevBuf tab, r64, cth64, ph64, rc32, thc32, phc32, T, rho, u, v, w;
+    int tab_floats = 0;
+    bool has_wind = false;
+
+    // current opacity table
+    int chan0 = 0, n_chan = 0;
+    std::vector<float> lambda;
+    DevBuf own_kabs, own_kray, own_kcld, own_g;   // copies of host-resident inputs
+    const float *k_abs = nullptr, *k_ray = nullptr, *k_cld = nullptr, *g_cld = nullptr;
+    DevBuf alpha, prop, reff, vlos, lambda64;
+    int staged_obs = -2;   // -2: nothing staged, -1: unshifted table, >= 0: Doppler table of that observer dir
+    double staged_dir[3] = {0, 0, 0};
+    int staged_halfwidth = 0;
+
+    // emission
+    DevBuf Lcell, Lcum, Ltot;
+
+    // workspace
+    DevBuf ev0, ev1, ev2, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount;
+    unsigned int ev_cap = 0;
+    int n_threads_resident = 0;
+    PassCtrl* h_ctrl = nullptr;  // pinned
+};
+
+namespace {
+
+int fail(gcmcrt_grid* g, int code, const std::string& msg)
+{
+    if (g) g->err = msg; else g_create_error = msg;
+    return code;
+}
+
+#define CUDA_TRY(g, expr)                                                                                 \
+    do {                                                                                                  \
+        cudaError_t e__ = (expr);                                                                         \
+        if (e__ != cudaSuccess)                                                                           \
+            return fail(g, e__ == cudaErrorMemoryAllocation ? GCMCRT_E_NOMEM : GCMCRT_E_CUDA,             \
+                        std::string(#expr) + ": " + cudaGetErrorString(e__));                             \
+    } while (0)
+
+bool is_device_ptr(const void* p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// Return a device view of `src` (n elements): the pointer itself when it is device memory, else a copy in `own`.
+template <class T>
+cudaError_t device_view(const T* src, size_t n, DevBuf& own, cudaStream_t s, const T** out, bool force_copy = false)
+{
+    if (!src) { *out = nullptr; return cudaSuccess; }
+    const bool dev = is_device_ptr(src);
+    if (dev && !force_copy) { *out = src; return cudaSuccess; }
+    cudaError_t e = own.ensure(n * sizeof(T));
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpyAsync(own.p, src, n * sizeof(T), dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s);
+    *out = own.as<T>();
+    return e;
+}
+
+template <class T>
+cudaError_t upload(DevBuf& b, const std::vector<T>& v, cudaStream_t s)
+{
+    cudaError_t e = b.ensure(v.size() * sizeof(T));
+    if (e != cudaSuccess) return e;
+    return cudaMemcpyAsync(b.p, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, s);
+}
+
+GeomParams geom_params(const gcmcrt_grid* g)
+{
+    GeomParams gp;
+    gp.nlev = g->nlev; gp.nlat = g->nlat; gp.nlon = g->nlon; gp.ncell = g->ncell;
+    gp.tab = g->tab.as<float>();
+    gp.tab_floats = g->tab_floats;
+    gp.Rtoa = float(g->r[g->nlev]);
+    gp.R0 = float(g->r[0]);
+    gp.maxseg = 8 * (g->nlev + g->nlat + g->nlon) + 64;
+    return gp;
+}
+
+void normalize3(const double* in, float* out)
+{
+    const double n = std::sqrt(in[0] * in[0] + in[1] * in[1] + in[2] * in[2]);
+    for (int m = 0; m < 3; ++m) out[m] = float(in[m] / (n > 0 ? n : 1.0));
+}
+
+// basis (e1, e2) perpendicular to unit d: e1 = normalize(z^ x d) (x^ if degenerate), e2 = d x e1   (O3, C19)
+void perp_basis(const double* d, float* e1, float* e2)
+{
+    double a[3] = {-d[1], d[0], 0.0};
+    const double n = std::sqrt(a[0] * a[0] + a[1] * a[1]);
+    if (n < 1e-6) { a[0] = 1.0; a[1] = 0.0; a[2] = 0.0; } else { a[0] /= n; a[1] /= n; }
+    const double b[3] = {d[1] * a[2] - d[2] * a[1], d[2] * a[0] - d[0] * a[2], d[0] * a[1] - d[1] * a[0]};
+    for (int m = 0; m < 3; ++m) { e1[m] = float(a[m]); e2[m] = float(b[m]); }
+}
+
+// Stage alpha / prop for observer `obs_dir` (nullptr = unshifted table).
+int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStream_t s)
+{
+    const size_t n = size_t(g->n_chan) * g->ncell;
+    CUDA_TRY(g, g->alpha.ensure(n * sizeof(float)));
+    CUDA_TRY(g, g->prop.ensure(n * sizeof(float4)));
+    StageParams sp;
+    sp.n_chan = g->n_chan; sp.ncell = g->ncell; sp.nlev = g->nlev; sp.nlat = g->nlat; sp.nlon = g->nlon;
+    sp.k_abs = g->k_abs; sp.k_ray = g->k_ray; sp.k_cld = g->k_cld; sp.g_cld = g->g_cld;
+    sp.rho = g->rho.as<float>();
+    sp.alpha = g->alpha.as<float>(); sp.prop = g->prop.as<float4>();
+    sp.doppler = obs_dir != nullptr; sp.halfwidth = halfwidth;
+    sp.vlos = nullptr; sp.reff = g->reff.as<float>();
+    if (obs_dir) {
+        CUDA_TRY(g, g->vlos.ensure(size_t(g->ncell) * sizeof(float)));
+        float o[3];
+        normalize3(obs_dir, o);
+        vlos_kernel<<<(g->ncell + 255) / 256, 256, 0, s>>>(g->nlev, g->nlat, g->nlon, g->u.as<float>(), g->v.as<float>(),
+                                                          g->w.as<float>(), float(g->Omega), g->rc32.as<float>(),
+                                                          g->thc32.as<float>(), g->phc32.as<float>(), o[0], o[1], o[2],
+                                                          g->vlos.as<float>());
+        sp.vlos = g->vlos.as<float>();
+    }
+    const long long blocks = std::min<long long>((long long)((n + 255) / 256), (long long)g->sm_count * 32);
+    stage_kernel<<<(unsigned)std::max<long long>(blocks, 1), 256, 0, s>>>(sp);
+    CUDA_TRY(g, cudaGetLastError());
+    g->staged_obs = obs_dir ? 0 : -1;
+    if (obs_dir) { for (int m = 0; m < 3; ++m) g->staged_dir[m] = obs_dir[m]; g->staged_halfwidth = halfwidth; }
+    return GCMCRT_OK;
+}
+
+int ensure_workspace(gcmcrt_grid* g)
+{
+    if (g->ev_cap == 0) {
+        unsigned long long cap = 16ull << 20;
+        if (const char* e = std::getenv("GCMCRT_EVENT_CAP")) cap = std::strtoull(e, nullptr, 10);
+        if (cap < 64) cap = 64;
+        if (cap > (1ull << 30)) cap = 1ull << 30;
+        g->ev_cap = (unsigned int)cap;
+    }
+    CUDA_TRY(g, g->ev0.ensure(size_t(g->ev_cap) * sizeof(float4)));
+    CUDA_TRY(g, g->ev1.ensure(size_t(g->ev_cap) * sizeof(float4)));
+    CUDA_TRY(g, g->ev2.ensure(size_t(g->ev_cap) * sizeof(float4)));
+    CUDA_TRY(g, g->ctrl.ensure(sizeof(PassCtrl)));
+    CUDA_TRY(g, g->counters.ensure(sizeof(DevCounters)));
+    if (!g->h_ctrl) CUDA_TRY(g, cudaMallocHost((void**)&g->h_ctrl, sizeof(PassCtrl)));
+    return GCMCRT_OK;
+}
+
+struct OutBuf {  // an output array: the caller's device pointer, or an internal one copied back at the end
+    void* dev = nullptr;
+    void* host = nullptr;
+    size_t bytes = 0;
+};
+
+int bind_out(gcmcrt_grid* g, void* user, size_t bytes, DevBuf& own, OutBuf& ob, bool always_internal = false)
+{
+    ob.bytes = bytes;
+    if (user && is_device_ptr(user) && !always_internal) { ob.dev = user; ob.host = nullptr; return GCMCRT_OK; }
+    CUDA_TRY(g, own.ensure(bytes > 0 ? bytes : 8));
+    ob.dev = own.p;
+    ob.host = (user && !is_device_ptr(user)) ? user : nullptr;
+    return GCMCRT_OK;
+}
+
+int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, void* stream, int emission)
+{
+    if (!g) return GCMCRT_E_INVALID;
+    if (!prm || !out) return fail(g, GCMCRT_E_INVALID, "params and result must not be NULL");
+    if (g->n_chan <= 0 || g->staged_obs == -2) return fail(g, GCMCRT_E_STATE, "gcmcrt_set_opacity has not been called");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const int n_obs = prm->n_obs;
+    if (n_obs < 0 || n_obs > kMaxObs) return fail(g, GCMCRT_E_INVALID, "n_obs must be in [0, 32]");
+    if (n_obs > 0 && !prm->obs_dir) return fail(g, GCMCRT_E_INVALID, "obs_dir is NULL");
+    const unsigned long long N = prm->packets_per_channel;
+    if (N == 0 || N > 0xffffffffull) return fail(g, GCMCRT_E_INVALID, "packets_per_channel must be in [1, 2^32)");
+    const unsigned long long lo = prm->pkt_begin, hi = prm->pkt_end ? prm->pkt_end : N;
+    if (lo > hi || hi > N) return fail(g, GCMCRT_E_INVALID, "bad packet range");
+    const int cb = prm->chan_begin, ce = prm->chan_end ? prm->chan_end : g->n_chan;
+    if (cb < 0 || ce > g->n_chan || cb >= ce) return fail(g, GCMCRT_E_INVALID, "bad channel range");
+    const int nb = prm->n_batches ? prm->n_batches : 32;
+    if (nb < 1 || nb > kMaxBatches) return fail(g, GCMCRT_E_INVALID, "n_batches must be in [1, 64]");
+    if (!out->flux_sum && n_obs > 0) return fail(g, GCMCRT_E_INVALID, "result.flux_sum is required");
+    if (prm->emission_bias < 0.0 || prm->emission_bias >= 1.0) return fail(g, GCMCRT_E_INVALID, "emission_bias must be in [0,1)");
+    if (prm->doppler_on && g->n_chan > 1 && g->reff.p == nullptr) return fail(g, GCMCRT_E_STATE, "no wavelength table");
+    const int ncr = ce - cb;
+    if (ncr > (1 << 24)) return fail(g, GCMCRT_E_INVALID, "too many channels in one run");
+    const int npix = prm->npix > 0 && out->image ? prm->npix : 0;
+
+    int rcode = ensure_workspace(g);
+    if (rcode) return rcode;
+
+    // ---- outputs
+    OutBuf o_flux, o_ltot, o_val, o_sig, o_img, o_evc, o_cnt;
+    const size_t nflux = size_t(ncr) * std::max(n_obs, 1) * nb;
+    if ((rcode = bind_out(g, out->flux_sum, nflux * sizeof(double), g->flux, o_flux))) return rcode;
+    if ((rcode = bind_out(g, out->L_tot, size_t(ncr) * std::max(n_obs, 1) * sizeof(double), g->ltot_out, o_ltot))) return rcode;
+    if ((rcode = bind_out(g, out->value, size_t(ncr) * std::max(n_obs, 1) * sizeof(double), g->value, o_val))) return rcode;
+    if ((rcode = bind_out(g, out->sigma, size_t(ncr) * std::max(n_obs, 1) * sizeof(double), g->sigma, o_sig))) return rcode;
+    if (npix) if ((rcode = bind_out(g, out->image, size_t(ncr) * n_obs * npix * npix * sizeof(float), g->image, o_img))) return rcode;
+    const size_t n_pkt = size_t(hi - lo);
+    if (out->event_count) if ((rcode = bind_out(g, out->event_count, size_t(ncr) * n_pkt * sizeof(uint32_t), g->evcount, o_evc))) return rcode;
+    if ((rcode = bind_out(g, out->counters, sizeof(gcmcrt_counters), g->counters, o_cnt, true))) return rcode;
+    CUDA_TRY(g, cudaMemsetAsync(o_flux.dev, 0, nflux * sizeof(double), s));
+    CUDA_TRY(g, cudaMemsetAsync(o_ltot.dev, 0, o_ltot.bytes, s));
+    if (npix) CUDA_TRY(g, cudaMemsetAsync(o_img.dev, 0, o_img.bytes, s));
+    if (o_evc.dev) CUDA_TRY(g, cudaMemsetAsync(o_evc.dev, 0, o_evc.bytes, s));
+    CUDA_TRY(g, cudaMemsetAsync(g->counters.p, 0, sizeof(DevCounters), s));
+
+    // ---- constants of the run
+    RunConst rc;
+    std::memset(&rc, 0, sizeof rc);
+    rc.geom = geom_params(g);
+    rc.chan_key0 = uint32_t(g->chan0);
+    rc.chan_begin = cb; rc.n_chan_run = ncr;
+    rc.pkt_begin = uint32_t(lo); rc.n_pkt = uint32_t(n_pkt);
+    rc.N = N; rc.seed = prm->seed;
+    rc.mode = emission;
+    rc.max_events = prm->max_events; rc.scatter_on = prm->scatter_on;
+    rc.surface_albedo = g->surface_albedo;
+    rc.xi = prm->emission_bias;
+    rc.n_batches = nb;
+    rc.n_obs_total = std::max(n_obs, 1);
+    normalize3(prm->star_dir, rc.star);
+    {
+        double sd[3] = {rc.star[0], rc.star[1], rc.star[2]};
+        perp_basis(sd, rc.e1, rc.e2);
+    }
+    for (int o = 0; o < n_obs; ++o) {
+        normalize3(prm->obs_dir + 3 * o, rc.obs[o]);
+        double od[3] = {rc.obs[o][0], rc.obs[o][1], rc.obs[o][2]};
+        perp_basis(od, rc.img_ex[o], rc.img_ey[o]);
+    }
+    rc.tau_cut = float(prm->tau_cut > 0.0 ? prm->tau_cut : 50.0);
+    rc.npix = npix;
+    rc.flux = static_cast<double*>(o_flux.dev);
+    rc.image = npix ? static_cast<float*>(o_img.dev) : nullptr;
+    rc.event_count = static_cast<uint32_t*>(o_evc.dev);
+    rc.counters = g->counters.as<DevCounters>();
+    PassCtrl* ctrl = g->ctrl.as<PassCtrl>();
+    rc.work_counter = &ctrl->work_counter;
+    rc.ray_counter = &ctrl->ray_counter;
+
+    // ---- launch geometry: persistent grids sized to the device
+    const size_t smem_t = size_t(g->tab_floats) * sizeof(float);
+    int occ_t = 0, occ_p = 0;
+    auto tk = transport_kernel<16, 8>;
+    auto pk = peel_kernel<12, 8>;
+    CUDA_TRY(g, cudaFuncSetAttribute(tk, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_t)));
+    CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_t, tk, kTransportThreads, smem_t));
+    if (occ_t < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
+    const int grid_t = g->sm_count * occ_t;
+    const unsigned long long threads_t = (unsigned long long)grid_t * kTransportThreads;
+    for (int b = 0; b < 2; ++b) {
+        CUDA_TRY(g, g->s0[b].ensure(threads_t * sizeof(float4)));
+        CUDA_TRY(g, g->s1[b].ensure(threads_t * sizeof(float4)));
+        CUDA_TRY(g, g->s2[b].ensure(threads_t * sizeof(uint4)));
+    }
+    EventBuf ev;
+    ev.e0 = g->ev0.as<float4>(); ev.e1 = g->ev1.as<float4>(); ev.e2 = g->ev2.as<float4>();
+    ev.count = &ctrl->ev_count;
+    ev.cap = g->ev_cap;
+    ev.soft_cap = (unsigned long long)g->ev_cap > 4 * threads_t ? g->ev_cap - (unsigned int)(2 * threads_t) : g->ev_cap / 2;
+
+    const int n_runs = prm->doppler_on ? std::max(n_obs, 1) : 1;
+    unsigned long long passes = 0;
+    for (int run = 0; run < n_runs; ++run) {
+        // ---- A0/A1: make sure the staged table is the one this run needs
+        if (prm->doppler_on && n_obs > 0) {
+            const double* od = prm->obs_dir + 3 * run;
+            const bool same = g->staged_obs >= 0 && g->staged_halfwidth == prm->doppler_halfwidth &&
+                              g->staged_dir[0] == od[0] && g->staged_dir[1] == od[1] && g->staged_dir[2] == od[2];
+            if (!same && (rcode = stage_opacity(g, od, prm->doppler_halfwidth, s))) return rcode;
+            rc.obs_first = run; rc.n_obs_run = 1;
+        } else {
+            if (g->staged_obs != -1 && (rcode = stage_opacity(g, nullptr, 0, s))) return rcode;
+            rc.obs_first = 0; rc.n_obs_run = n_obs;
+        }
+        rc.alpha = g->alpha.as<float>();
+        rc.prop = g->prop.as<float4>();
+        // ---- A2: emission CDF
+        if (emission) {
+            const size_t n = size_t(g->n_chan) * g->ncell;
+            CUDA_TRY(g, g->Lcell.ensure(n * sizeof(double)));
+            CUDA_TRY(g, g->Lcum.ensure(n * sizeof(double)));
+            CUDA_TRY(g, g->Ltot.ensure(size_t(g->n_chan) * sizeof(double)));
+            EmisParams ep;
+            ep.n_chan = g->n_chan; ep.nlev = g->nlev; ep.nlat = g->nlat; ep.nlon = g->nlon; ep.ncell = g->ncell;
+            ep.alpha = rc.alpha; ep.prop = rc.prop;
+            ep.rho = g->rho.as<float>(); ep.T = g->T.as<float>();
+            ep.lambda = g->lambda64.as<double>();
+            ep.r_edges = g->r64.as<double>(); ep.cth_edges = g->cth64.as<double>(); ep.ph_edges = g->ph64.as<double>();
+            ep.tau_vert_max = prm->tau_vert_max;
+            ep.Lcell = g->Lcell.as<double>(); ep.Lcum = g->Lcum.as<double>(); ep.Ltot = g->Ltot.as<double>();
+            const long long ncolc = (long long)g->n_chan * g->nlat * g->nlon;
+            emis_cell_kernel<<<(unsigned)((ncolc + 127) / 128), 128, 0, s>>>(ep);
+            emis_scan_kernel<<<g->n_chan, 1024, 0, s>>>(ep);
+            CUDA_TRY(g, cudaGetLastError());
+            rc.Lcum = ep.Lcum; rc.Lcell = ep.Lcell; rc.Ltot = ep.Ltot;
+            // L_tot output [n_chan_run][n_obs]
+            const int o0 = prm->doppler_on ? run : 0, o1 = prm->doppler_on ? run + 1 : std::max(n_obs, 1);
+            for (int o = o0; o < o1; ++o)
+                CUDA_TRY(g, cudaMemcpy2DAsync(static_cast<double*>(o_ltot.dev) + o, sizeof(double) * rc.n_obs_total,
+                                              ep.Ltot + cb, sizeof(double), sizeof(double), ncr,
+                                              cudaMemcpyDeviceToDevice, s));
+        }
+        // event counts are recorded for the first run only (with doppler_on: observer 0's run)
+        rc.event_count = run == 0 ? static_cast<uint32_t*>(o_evc.dev) : nullptr;
+
+        // ---- pass loop
+        const unsigned long long total_items = (unsigned long long)ncr * n_pkt;
+        CUDA_TRY(g, cudaMemsetAsync(ctrl, 0, sizeof(PassCtrl), s));
+        int cur = 0;
+        const size_t smem_p = (size_t((g->tab_floats + 31) & ~31) + size_t(kPeelThreads / 32) * rc.n_obs_run * nb) * sizeof(float);
+        if (rc.n_obs_run > 0) {
+            CUDA_TRY(g, cudaFuncSetAttribute(pk, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_p)));
+            CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, pk, kPeelThreads, smem_p));
+            if (occ_p < 1) return fail(g, GCMCRT_E_INVALID, "peel bins do not fit in shared memory");
+        }
+        for (;;) {
+            const int nxt = 1 - cur;
+            SuspBuf sin, sout;
+            sin.s0 = g->s0[cur].as<float4>(); sin.s1 = g->s1[cur].as<float4>(); sin.s2 = g->s2[cur].as<uint4>();
+            sin.count = &ctrl->susp_count[cur]; sin.taken = &ctrl->susp_taken[cur];
+            sout.s0 = g->s0[nxt].as<float4>(); sout.s1 = g->s1[nxt].as<float4>(); sout.s2 = g->s2[nxt].as<uint4>();
+            sout.count = &ctrl->susp_count[nxt]; sout.taken = &ctrl->susp_taken[nxt];
+            tk<<<grid_t, kTransportThreads, smem_t, s>>>(rc, ev, sin, sout, total_items);
+            if (rc.n_obs_run > 0) pk<<<g->sm_count * occ_p, kPeelThreads, smem_p, s>>>(rc, ev);
+            CUDA_TRY(g, cudaGetLastError());
+            ++passes;
+            CUDA_TRY(g, cudaMemcpyAsync(g->h_ctrl, ctrl, sizeof(PassCtrl), cudaMemcpyDeviceToHost, s));
+            CUDA_TRY(g, cudaStreamSynchronize(s));
+            const bool done = g->h_ctrl->work_counter >= total_items && g->h_ctrl->susp_count[nxt] == 0;
+            if (done) break;
+            // reset the per-pass counters: events, rays, the list just consumed
+            PassCtrl next = *g->h_ctrl;
+            next.ev_count = 0; next.ray_counter = 0;
+            next.susp_count[cur] = 0; next.susp_taken[cur] = 0; next.susp_taken[nxt] = 0;
+            CUDA_TRY(g, cudaMemcpyAsync(ctrl, &next, sizeof(PassCtrl), cudaMemcpyHostToDevice, s));
+            CUDA_TRY(g, cudaStreamSynchronize(s));
+            cur = nxt;
+            if (passes > (1ull << 20)) return fail(g, GCMCRT_E_CUDA, "pass loop did not terminate");
+        }
+    }
+
+    // ---- A10
+    if (n_obs > 0) {
+        const int nt = ncr * n_obs;
+        normalise_kernel<<<(nt + 127) / 128, 128, 0, s>>>(ncr, n_obs, nb, N, lo, hi, static_cast<double*>(o_flux.dev),
+                                                         static_cast<double*>(o_ltot.dev), emission,
+                                                         static_cast<double*>(o_val.dev), static_cast<double*>(o_sig.dev));
+        CUDA_TRY(g, cudaGetLastError());
+    }
+    // ---- copy-backs for host-resident outputs
+    bool need_sync = false;
+    for (OutBuf* ob : {&o_flux, &o_ltot, &o_val, &o_sig, &o_img, &o_evc}) {
+        if (ob->host && ob->dev && ob->bytes) {
+            CUDA_TRY(g, cudaMemcpyAsync(ob->host, ob->dev, ob->bytes, cudaMemcpyDeviceToHost, s));
+            need_sync = true;
+        }
+    }
+    if (out->counters) {
+        DevCounters dc;
+        CUDA_TRY(g, cudaMemcpyAsync(&dc, g->counters.p, sizeof dc, cudaMemcpyDeviceToHost, s));
+        CUDA_TRY(g, cudaStreamSynchronize(s));
+        gcmcrt_counters hc;
+        hc.events = dc.events; hc.segments_transport = dc.seg_transport; hc.segments_peel = dc.seg_peel;
+        hc.packets_escaped = dc.escaped; hc.packets_absorbed = dc.absorbed; hc.packets_surface = dc.surface;
+        hc.packets_stuck = dc.stuck; hc.escaped_weight = dc.escaped_weight; hc.passes = passes; hc.rays_peel = dc.rays_peel;
+        if (is_device_ptr(out->counters)) CUDA_TRY(g, cudaMemcpyAsync(out->counters, &hc, sizeof hc, cudaMemcpyHostToDevice, s));
+        else *out->counters = hc;
+        need_sync = true;
+    }
+    if (need_sync) CUDA_TRY(g, cudaStreamSynchronize(s));
+    return GCMCRT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* gcmcrt_version(void) { return "gcmcrt 0.1 sm_100a (CUDA " "12.9" ")"; }
+
+const char* gcmcrt_last_error(const gcmcrt_grid* grid) { return grid ? grid->err.c_str() : g_create_error.c_str(); }
+
+int gcmcrt_grid_create(gcmcrt_grid** out, int nlev, int nlat, int nlon, const double* r_edges, const double* colat_edges,
+                       const double* lon_edges, const float* T, const float* rho, const float* u, const float* v,
+                       const float* w, double Omega, float surface_albedo, void* stream)
+{
+    if (!out) return fail(nullptr, GCMCRT_E_INVALID, "out is NULL");
+    *out = nullptr;
+    if (nlev < 1 || nlat < 1 || nlon < 1 || nlev > 1023 || nlat > 1023 || nlon > 2047)
+        return fail(nullptr, GCMCRT_E_INVALID, "grid sizes must satisfy 1 <= nlev, nlat <= 1023, 1 <= nlon <= 2047");
+    if (!r_edges || !colat_edges || !lon_edges || !T || !rho) return fail(nullptr, GCMCRT_E_INVALID, "NULL grid array");
+    for (int i = 0; i < nlev; ++i)
+        if (!(r_edges[i + 1] > r_edges[i]) || !(r_edges[i] > 0.0)) return fail(nullptr, GCMCRT_E_INVALID, "r_edges must be positive and strictly ascending");
+    for (int j = 0; j < nlat; ++j)
+        if (!(colat_edges[j + 1] > colat_edges[j])) return fail(nullptr, GCMCRT_E_INVALID, "colat_edges must be strictly ascending");
+    for (int k = 0; k < nlon; ++k)
+        if (!(lon_edges[k + 1] > lon_edges[k])) return fail(nullptr, GCMCRT_E_INVALID, "lon_edges must be strictly ascending");
+    const double pi = 3.14159265358979323846;
+    if (std::fabs(colat_edges[0]) > 1e-9 || std::fabs(colat_edges[nlat] - pi) > 1e-9)
+        return fail(nullptr, GCMCRT_E_INVALID, "colat_edges must span 0..pi");
+    if (std::fabs(lon_edges[0]) > 1e-9 || std::fabs(lon_edges[nlon] - 2 * pi) > 1e-9)
+        return fail(nullptr, GCMCRT_E_INVALID, "lon_edges must span 0..2pi");
+    if (!(surface_albedo >= 0.f && surface_albedo <= 1.f)) return fail(nullptr, GCMCRT_E_INVALID, "surface_albedo must be in [0,1]");
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return fail(nullptr, GCMCRT_E_CUDA, "no CUDA device"); }
+    gcmcrt_grid* g = new (std::nothrow) gcmcrt_grid;
+    if (!g) return fail(nullptr, GCMCRT_E_NOMEM, "host allocation failed");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    g->nlev = nlev; g->nlat = nlat; g->nlon = nlon; g->ncell = nlev * nlat * nlon;
+    g->r.assign(r_edges, r_edges + nlev + 1);
+    g->th.assign(colat_edges, colat_edges + nlat + 1);
+    g->ph.assign(lon_edges, lon_edges + nlon + 1);
+    g->Omega = Omega; g->surface_albedo = surface_albedo;
+    cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev);
+
+    // packed fp32 tables: R, R^2, qcube, cos(theta_e), cos(phi_e), sin(phi_e), phi_e
+    std::vector<float> tab;
+    for (int i = 0; i <= nlev; ++i) tab.push_back(float(g->r[i]));
+    for (int i = 0; i <= nlev; ++i) tab.push_back(float(g->r[i] * g->r[i]));
+    for (int i = 0; i < nlev; ++i) { const double q = g->r[i + 1] / g->r[i]; tab.push_back(float(q * q * q - 1.0)); }
+    std::vector<double> cth(nlat + 1);
+    for (int j = 0; j <= nlat; ++j) cth[j] = j == 0 ? 1.0 : (j == nlat ? -1.0 : std::cos(g->th[j]));
+    for (int j = 0; j <= nlat; ++j) tab.push_back(float(cth[j]));
+    for (int k = 0; k <= nlon; ++k) tab.push_back(float(k == nlon ? std::cos(g->ph[0]) : std::cos(g->ph[k])));
+    for (int k = 0; k <= nlon; ++k) tab.push_back(float(k == nlon ? std::sin(g->ph[0]) : std::sin(g->ph[k])));
+    for (int k = 0; k <= nlon; ++k) tab.push_back(float(g->ph[k]));
+    g->tab_floats = int(tab.size());
+    std::vector<float> rc(nlev), thc(nlat), phc(nlon);
+    for (int i = 0; i < nlev; ++i) rc[i] = float(0.5 * (g->r[i] + g->r[i + 1]));
+    for (int j = 0; j < nlat; ++j) thc[j] = float(0.5 * (g->th[j] + g->th[j + 1]));
+    for (int k = 0; k < nlon; ++k) phc[k] = float(0.5 * (g->ph[k] + g->ph[k + 1]));
+
+    cudaError_t e = upload(g->tab, tab, s);
+    if (e == cudaSuccess) e = upload(g->r64, g->r, s);
+    if (e == cudaSuccess) e = upload(g->cth64, cth, s);
+    if (e == cudaSuccess) e = upload(g->ph64, g->ph, s);
+    if (e == cudaSuccess) e = upload(g->rc32, rc, s);
+    if (e == cudaSuccess) e = upload(g->thc32, thc, s);
+    if (e == cudaSuccess) e = upload(g->phc32, phc, s);
+    const float* dummy = nullptr;
+    const size_t nc = size_t(g->ncell);
+    if (e == cudaSuccess) e = device_view(T, nc, g->T, s, &dummy, true);
+    if (e == cudaSuccess) e = device_view(rho, nc, g->rho, s, &dummy, true);
+    if (e == cudaSuccess && u) e = device_view(u, nc, g->u, s, &dummy, true);
+    if (e == cudaSuccess && v) e = device_view(v, nc, g->v, s, &dummy, true);
+    if (e == cudaSuccess && w) e = device_view(w, nc, g->w, s, &dummy, true);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);   // host vectors above go out of scope
+    if (e != cudaSuccess) {
+        const int code = fail(nullptr, e == cudaErrorMemoryAllocation ? GCMCRT_E_NOMEM : GCMCRT_E_CUDA,
+                              std::string("grid_create: ") + cudaGetErrorString(e));
+        cudaGetLastError();
+        gcmcrt_destroy(g);
+        return code;
+    }
+    *out = g;
+    return GCMCRT_OK;
+}
+
+int gcmcrt_set_opacity(gcmcrt_grid* g, int chan0, int n_chan, const float* lambda, const float* k_abs,
+                       const float* k_sca_ray, const float* k_sca_cld, const float* g_cld, void* stream)
+{
+    if (!g) return GCMCRT_E_INVALID;
+    if (n_chan < 1 || chan0 < 0 || !lambda || !k_abs) return fail(g, GCMCRT_E_INVALID, "set_opacity: bad arguments");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const size_t n = size_t(n_chan) * g->ncell;
+    g->staged_obs = -2;
+    g->n_chan = 0;
+    CUDA_TRY(g, device_view(k_abs, n, g->own_kabs, s, &g->k_abs));
+    CUDA_TRY(g, device_view(k_sca_ray, n, g->own_kray, s, &g->k_ray));
+    CUDA_TRY(g, device_view(k_sca_cld, n, g->own_kcld, s, &g->k_cld));
+    CUDA_TRY(g, device_view(g_cld, n, g->own_g, s, &g->g_cld));
+    std::vector<float> lam(n_chan);
+    if (is_device_ptr(lambda)) {
+        CUDA_TRY(g, cudaMemcpyAsync(lam.data(), lambda, n_chan * sizeof(float), cudaMemcpyDeviceToHost, s));
+        CUDA_TRY(g, cudaStreamSynchronize(s));
+    } else {
+        std::memcpy(lam.data(), lambda, n_chan * sizeof(float));
+    }
+    for (int c = 0; c < n_chan; ++c)
+        if (!(lam[c] > 0.f)) return fail(g, GCMCRT_E_INVALID, "lambda must be positive");
+    g->lambda = lam;
+    std::vector<double> lam64(lam.begin(), lam.end());
+    std::vector<float> reff(n_chan, 0.f);
+    for (int c = 0; c < n_chan && n_chan > 1; ++c) {
+        const int c1 = c + 1 < n_chan ? c : c - 1;
+        const double ratio = double(lam[c1 + 1]) / double(lam[c1]);
+        reff[c] = ratio != 1.0 ? float(1.0 / std::log(ratio)) : 0.f;
+    }
+    CUDA_TRY(g, upload(g->lambda64, lam64, s));
+    CUDA_TRY(g, upload(g->reff, reff, s));
+    CUDA_TRY(g, cudaStreamSynchronize(s));
+    g->chan0 = chan0;
+    g->n_chan = n_chan;
+    return stage_opacity(g, nullptr, 0, s);
+}
+
+int gcmcrt_run_albedo(gcmcrt_grid* g, const gcmcrt_run_params* p, gcmcrt_result* out, void* stream)
+{
+    return run_mode(g, p, out, stream, 0);
+}
+
+int gcmcrt_run_emission(gcmcrt_grid* g, const gcmcrt_run_params* p, gcmcrt_result* out, void* stream)
+{
+    return run_mode(g, p, out, stream, 1);
+}
+
+int gcmcrt_destroy(gcmcrt_grid* g)
+{
+    if (!g) return GCMCRT_OK;
+    cudaDeviceSynchronize();
+    cudaGetLastError();
+    for (DevBuf* b : {&g->tab, &g->r64, &g->cth64, &g->ph64, &g->rc32, &g->thc32, &g->phc32, &g->T, &g->rho, &g->u, &g->v,
+                      &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->prop, &g->reff, &g->vlos,
+                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->ev1, &g->ev2, &g->s0[0], &g->s0[1],
+                      &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->flux, &g->ltot_out,
+                      &g->value, &g->sigma, &g->image, &g->evcount})
+        b->release();
+    if (g->h_ctrl) cudaFreeHost(g->h_ctrl);
+    delete g;
+    return GCMCRT_OK;
+}
+
+int gcmcrt_debug_ray_tau(gcmcrt_grid* g, int chan, long n, const float* pos, const float* dir, float* tau,
+                         int* hit_surface, void* stream)
+{
+    if (!g) return GCMCRT_E_INVALID;
+    if (g->staged_obs == -2) return fail(g, GCMCRT_E_STATE, "gcmcrt_set_opacity has not been called");
+    if (chan < 0 || chan >= g->n_chan || n < 0 || !pos || !dir || !tau) return fail(g, GCMCRT_E_INVALID, "debug_ray_tau: bad arguments");
+    if (n == 0) return GCMCRT_OK;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    DevBuf bp, bd, bt, bh;
+    const float *dp = nullptr, *dd = nullptr;
+    int rcode = GCMCRT_OK;
+    do {
+        cudaError_t e = device_view(pos, size_t(3 * n), bp, s, &dp);
+        if (e == cudaSuccess) e = device_view(dir, size_t(3 * n), bd, s, &dd);
+        const bool tdev = is_device_ptr(tau), hdev = hit_surface && is_device_ptr(hit_surface);
+        float* dt = tau; int* dh = hit_surface;
+        if (e == cudaSuccess && !tdev) { e = bt.ensure(n * sizeof(float)); dt = bt.as<float>(); }
+        if (e == cudaSuccess && hit_surface && !hdev) { e = bh.ensure(n * sizeof(int)); dh = bh.as<int>(); }
+        if (e == cudaSuccess) {
+            const GeomParams gp = geom_params(g);
+            debug_ray_tau_kernel<<<(unsigned)((n + 127) / 128), 128, g->tab_floats * sizeof(float), s>>>(
+                gp, g->alpha.as<float>() + size_t(chan) * g->ncell, n, dp, dd, dt, dh);
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess && !tdev) e = cudaMemcpyAsync(tau, dt, n * sizeof(float), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess && hit_surface && !hdev) e = cudaMemcpyAsync(hit_surface, dh, n * sizeof(int), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) rcode = fail(g, GCMCRT_E_CUDA, std::string("debug_ray_tau: ") + cudaGetErrorString(e));
+    } while (0);
+    bp.release(); bd.release(); bt.release(); bh.release();
+    return rcode;
+}
+
+int gcmcrt_debug_philox(long n, const uint32_t* ctr, const uint32_t* key, uint32_t* out, void* stream)
+{
+    if (n < 0 || !ctr || !key || !out) return GCMCRT_E_INVALID;
+    if (n == 0) return GCMCRT_OK;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    DevBuf bc, bk, bo;
+    const uint32_t *dc = nullptr, *dk = nullptr;
+    cudaError_t e = device_view(ctr, size_t(4 * n), bc, s, &dc);
+    if (e == cudaSuccess) e = device_view(key, size_t(2 * n), bk, s, &dk);
+    const bool odev = is_device_ptr(out);
+    uint32_t* dout = out;
+    if (e == cudaSuccess && !odev) { e = bo.ensure(size_t(4 * n) * sizeof(uint32_t)); dout = bo.as<uint32_t>(); }
+    if (e == cudaSuccess) {
+        debug_philox_kernel<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(n, dc, dk, dout);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess && !odev) e = cudaMemcpyAsync(out, dout, size_t(4 * n) * sizeof(uint32_t), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    bc.release(); bk.release(); bo.release();
+    if (e != cudaSuccess) { g_create_error = std::string("debug_philox: ") + cudaGetErrorString(e); cudaGetLastError(); return GCMCRT_E_CUDA; }
+    return GCMCRT_OK;
+}
+
+}  // extern "C"

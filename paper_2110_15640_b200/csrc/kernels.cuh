@@ -1,0 +1,786 @@
+// kernels.cuh -- the packet kernels of libgcmcrt (sm_100a): opacity staging (A0/A1), emission CDF (A2),
+// persistent-thread transport with warp-level refill (A3-A6, A8), the separate peel-off ray integrator with
+// shared-memory flux bins (A7, A9) and the normalisation (A10).  See DESIGN.md for the data layout.
+#pragma once
+#include "ray.cuh"
+
+namespace gcmcrt {
+
+constexpr int kMaxObs = 32;
+constexpr int kMaxBatches = 64;
+constexpr int kTransportThreads = 256;
+constexpr int kPeelThreads = 256;
+
+// Packed cell id: i | j << 10 | k << 20  (nlev, nlat <= 1024, nlon <= 2048)
+__device__ __forceinline__ uint32_t pack_cell(int i, int j, int k) { return uint32_t(i) | uint32_t(j) << 10 | uint32_t(k) << 20; }
+__device__ __forceinline__ void unpack_cell(uint32_t c, int& i, int& j, int& k) { i = c & 1023; j = (c >> 10) & 1023; k = c >> 20; }
+
+enum EventKind : uint32_t { EV_MEDIUM = 0, EV_EMIT = 1, EV_SURFACE = 2 };
+
+// Event records written by the transport kernel, consumed by the peel kernel (structure of arrays of float4).
+struct EventBuf {
+    float4* e0;  // px py pz pref          pref = W*omega (medium), W (emission), W*a (surface)
+    float4* e1;  // nx ny nz pgas          n = incoming direction (medium) or surface normal
+    float4* e2;  // g  cell  meta  pkt     meta = kind | batch << 2 | chan_run << 8
+    unsigned int* count;
+    unsigned int cap;
+    unsigned int soft_cap;
+};
+
+// Packets suspended because the event buffer filled up; resumed by the next pass.
+struct SuspBuf {
+    float4* s0;  // px py pz W
+    float4* s1;  // nx ny nz cell
+    uint4* s2;   // chan_run pkt m_inter nev|kind<<28
+    unsigned int* count;
+    unsigned int* taken;
+};
+
+struct DevCounters {
+    unsigned long long events, seg_transport, seg_peel, escaped, absorbed, surface, stuck, rays_peel;
+    double escaped_weight;
+};
+
+struct RunConst {
+    GeomParams geom;
+    const float* alpha;    // [n_chan_tab][ncell] extinction (m^-1)
+    const float4* prop;    // [n_chan_tab][ncell] omega, P_gas, g, k_abs_eff
+    const double* Lcum;    // emission: [n_chan_tab][ncell] running luminosity
+    const double* Lcell;   // emission, xi > 0 only
+    const double* Ltot;    // emission: [n_chan_tab]
+    uint32_t chan_key0;    // global channel index of table row 0 (Philox key)
+    int chan_begin;        // first table row of this run
+    int n_chan_run;
+    uint32_t pkt_begin, n_pkt;
+    unsigned long long N;  // packets_per_channel
+    unsigned long long seed;
+    int mode;              // 0 albedo, 1 emission
+    int max_events, scatter_on;
+    float surface_albedo;
+    double xi;
+    int n_batches;
+    int n_obs_run, obs_first, n_obs_total;
+    float star[3], e1[3], e2[3];
+    float obs[kMaxObs][3];
+    float img_ex[kMaxObs][3], img_ey[kMaxObs][3];
+    float tau_cut;
+    int npix;
+    // outputs
+    double* flux;          // [n_chan_run][n_obs_total][n_batches]
+    float* image;          // nullable
+    uint32_t* event_count; // nullable [n_chan_run][n_pkt]
+    DevCounters* counters;
+    unsigned long long* work_counter;   // next fresh packet item
+    unsigned long long* ray_counter;    // next peel ray of this pass
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// A0 / A1: opacity staging.  One thread per (channel, cell); coalesced along the radial index.
+// ---------------------------------------------------------------------------------------------------------
+struct StageParams {
+    int n_chan, ncell, nlev, nlat, nlon;
+    const float *k_abs, *k_ray, *k_cld, *g_cld, *rho;
+    float* alpha;
+    float4* prop;
+    // Doppler (A1): per-cell line-of-sight velocity of this observer, per-channel 1/ln(lambda ratio)
+    int doppler, halfwidth;
+    const float* vlos;   // [ncell] for the current observer
+    const float* reff;   // [n_chan]
+};
+
+__global__ void __launch_bounds__(256) vlos_kernel(int nlev, int nlat, int nlon, const float* __restrict__ u,
+                                                   const float* __restrict__ v, const float* __restrict__ w, float Omega,
+                                                   const float* __restrict__ rc, const float* __restrict__ thc,
+                                                   const float* __restrict__ phc, float ox, float oy, float oz,
+                                                   float* __restrict__ vlos)
+{
+    // Eq. 33 in vector form (C13): v_LOS = -(u phi^ - v theta^ + w r^ + Omega r sin(theta) phi^) . o^ at the cell centre
+    const int cell = blockIdx.x * blockDim.x + threadIdx.x;
+    const int ncell = nlev * nlat * nlon;
+    if (cell >= ncell) return;
+    const int i = cell % nlev, j = (cell / nlev) % nlat, k = cell / (nlev * nlat);
+    float st, ct, sp, cp;
+    sincosf(thc[j], &st, &ct);
+    sincosf(phc[k], &sp, &cp);
+    const float ue = (u ? u[cell] : 0.0f) + Omega * rc[i] * st;
+    const float vn = v ? v[cell] : 0.0f, wu = w ? w[cell] : 0.0f;
+    const float Vx = ue * (-sp) - vn * (ct * cp) + wu * (st * cp);
+    const float Vy = ue * cp - vn * (ct * sp) + wu * (st * sp);
+    const float Vz = vn * st + wu * ct;
+    vlos[cell] = -(Vx * ox + Vy * oy + Vz * oz);
+}
+
+__global__ void __launch_bounds__(256) stage_kernel(const StageParams p)
+{
+    const long long total = (long long)p.n_chan * p.ncell;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total;
+         t += (long long)gridDim.x * blockDim.x) {
+        const int c = int(t / p.ncell);
+        const int cell = int(t - (long long)c * p.ncell);
+        float ka;
+        if (p.doppler && p.n_chan > 1) {
+            // Eq. 34: lambda_eff = lambda_0 (1 - v/c) -> index offset dn = -v/c / ln(lambda_{n+1}/lambda_n), C14
+            float dn = -p.vlos[cell] * (1.0f / 299792458.0f) * p.reff[c];
+            dn = fminf(fmaxf(dn, -float(p.halfwidth)), float(p.halfwidth));
+            float x = fminf(fmaxf(float(c) + dn, 0.0f), float(p.n_chan - 1));
+            int lo = min(int(floorf(x)), p.n_chan - 2);
+            const float f = x - float(lo);
+            const float k0 = __ldg(p.k_abs + (long long)lo * p.ncell + cell);
+            const float k1 = __ldg(p.k_abs + (long long)(lo + 1) * p.ncell + cell);
+            ka = (1.0f - f) * k0 + f * k1;
+        } else {
+            ka = __ldg(p.k_abs + t);
+        }
+        const float kr = p.k_ray ? __ldg(p.k_ray + t) : 0.0f;
+        const float kc = p.k_cld ? __ldg(p.k_cld + t) : 0.0f;
+        const float g = p.g_cld ? __ldg(p.g_cld + t) : 0.0f;
+        const float ks = kr + kc;
+        const float kext = ka + ks;
+        p.alpha[t] = __ldg(p.rho + cell) * kext;
+        p.prop[t] = make_float4(kext > 0.0f ? ks / kext : 0.0f, ks > 0.0f ? kr / ks : 0.0f, g, ka);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// A2: emission luminosities (Eq. 27), tau_vert cut (L210, C15) and the running sum used as CDF (Eq. 13).
+// ---------------------------------------------------------------------------------------------------------
+struct EmisParams {
+    int n_chan, nlev, nlat, nlon, ncell;
+    const float* alpha;
+    const float4* prop;
+    const float *rho, *T;
+    const double* lambda;   // [n_chan]
+    const double *r_edges, *cth_edges, *ph_edges;  // fp64 geometry for the volumes
+    double tau_vert_max;
+    double* Lcell;  // [n_chan][ncell] (scratch; overwritten by the scan into Lcum when Lcell_keep == null)
+    double* Lcum;
+    double* Ltot;
+};
+
+__device__ __forceinline__ double planck_lambda(double lam, double T)
+{
+    const double h = 6.62607015e-34, c = 299792458.0, kb = 1.380649e-23;
+    const double x = h * c / (lam * kb * T);
+    return 2.0 * h * c * c / (lam * lam * lam * lam * lam) / expm1(x);
+}
+
+// one thread per (channel, column): walks the column from the top, writes L_i with the depth cut applied
+__global__ void __launch_bounds__(128) emis_cell_kernel(const EmisParams p)
+{
+    const int ncol = p.nlat * p.nlon;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)p.n_chan * ncol) return;
+    const int c = int(t / ncol), col = int(t % ncol);
+    const int j = col % p.nlat, k = col / p.nlat;
+    const double lam = p.lambda[c];
+    const double ang = (p.cth_edges[j] - p.cth_edges[j + 1]) * (p.ph_edges[k + 1] - p.ph_edges[k]);
+    const long long base = (long long)c * p.ncell + (long long)col * p.nlev;
+    double tv = 0.0;
+    for (int i = p.nlev - 1; i >= 0; --i) {
+        const double r0 = p.r_edges[i], r1 = p.r_edges[i + 1];
+        const double vol = (r1 * r1 * r1 - r0 * r0 * r0) / 3.0 * ang;
+        const int cell = col * p.nlev + i;
+        double L = 4.0 * 3.14159265358979323846 * vol * double(p.rho[cell]) * double(p.prop[base + i].w) *
+                   planck_lambda(lam, double(p.T[cell]));
+        if (p.tau_vert_max > 0.0 && tv > p.tau_vert_max) L = 0.0;
+        tv += double(p.alpha[base + i]) * (r1 - r0);
+        p.Lcell[base + i] = L;
+    }
+}
+
+// one CTA per channel: inclusive fp64 scan of L_i over the ncell cells, chunk by chunk with a carry
+__global__ void __launch_bounds__(1024) emis_scan_kernel(const EmisParams p)
+{
+    __shared__ double warp_tot[32];
+    __shared__ double carry_s;
+    const int c = blockIdx.x;
+    const double* in = p.Lcell + (long long)c * p.ncell;
+    double* out = p.Lcum + (long long)c * p.ncell;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    if (threadIdx.x == 0) carry_s = 0.0;
+    __syncthreads();
+    for (int base = 0; base < p.ncell; base += blockDim.x) {
+        const int idx = base + threadIdx.x;
+        double v = idx < p.ncell ? in[idx] : 0.0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const double n = __shfl_up_sync(kFullMask, v, o);
+            if (lane >= o) v += n;
+        }
+        if (lane == 31) warp_tot[wid] = v;
+        __syncthreads();
+        if (wid == 0) {
+            double w = lane < nw ? warp_tot[lane] : 0.0;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const double n = __shfl_up_sync(kFullMask, w, o);
+                if (lane >= o) w += n;
+            }
+            warp_tot[lane] = w;  // inclusive totals of warps
+        }
+        __syncthreads();
+        const double carry = carry_s;
+        const double pre = wid > 0 ? warp_tot[wid - 1] : 0.0;
+        if (idx < p.ncell) out[idx] = carry + pre + v;
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry_s = carry + pre + v;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) p.Ltot[c] = carry_s;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Scattering physics (A8), fp32.
+// ---------------------------------------------------------------------------------------------------------
+// Eq. 6 as repaired (C7): q = 4 zeta - 2, u = cbrt(q + sqrt(1 + q^2)), cos = u - 1/u
+__device__ __forceinline__ float sample_rayleigh(float z)
+{
+    const float q = fmaf(4.0f, z, -2.0f);
+    const float u = cbrtf(q + sqrtf(fmaf(q, q, 1.0f)));
+    return u - 1.0f / u;
+}
+// Eq. 8; |g| < 1e-3 -> Eq. 2 (C8)
+__device__ __forceinline__ float sample_hg(float g, float z)
+{
+    if (fabsf(g) < 1e-3f) return fmaf(2.0f, z, -1.0f);
+    const float t = (1.0f - g * g) / (1.0f - g + 2.0f * g * z);
+    return (1.0f + g * g - t * t) / (2.0f * g);
+}
+// C9: rotate n by polar angle acos(ct), azimuth psi = 2 pi zpsi
+__device__ __forceinline__ void rotate_dir(float& nx, float& ny, float& nz, float ct, float zpsi)
+{
+    const float st = sqrtf(fmaxf(0.0f, 1.0f - ct * ct));
+    float sp, cp;
+    sincospif(2.0f * zpsi, &sp, &cp);
+    const float s2 = fmaf(nx, nx, ny * ny);
+    float x, y, z;
+    if (s2 < 1e-12f) {
+        x = st * cp; y = st * sp; z = ct * (nz >= 0.0f ? 1.0f : -1.0f);
+    } else {
+        const float sq = sqrtf(s2), inv = 1.0f / sq;
+        x = st * (nx * nz * cp - ny * sp) * inv + nx * ct;
+        y = st * (ny * nz * cp + nx * sp) * inv + ny * ct;
+        z = -st * cp * sq + nz * ct;
+    }
+    const float rn = rsqrtf(fmaf(x, x, fmaf(y, y, z * z)));
+    nx = x * rn; ny = y * rn; nz = z * rn;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Transport kernel: persistent threads, one packet per lane, warp-level refill.
+// ---------------------------------------------------------------------------------------------------------
+enum LaneState : int { LS_IDLE = 0, LS_FLY = 1, LS_EV_MEDIUM = 2, LS_EV_EMIT = 3, LS_EV_SURFACE = 4, LS_DONE = 5 };
+
+struct Packet {
+    Ray ray;
+    float tau, tau_t, W;
+    uint32_t chan_run, pkt, m_inter, nev;
+    int fl_seg;
+};
+
+__device__ __forceinline__ uint32_t batch_of(const RunConst& rc, uint32_t pkt)
+{
+    return uint32_t(((unsigned long long)pkt * (unsigned long long)rc.n_batches) / rc.N);
+}
+
+__device__ __forceinline__ void finish_packet(const RunConst& rc, const Packet& pk)
+{
+    if (rc.event_count) rc.event_count[(size_t)pk.chan_run * rc.n_pkt + (pk.pkt - rc.pkt_begin)] = pk.nev;
+}
+
+template <int THRESH, int KSTEPS>
+__global__ void __launch_bounds__(kTransportThreads, 2)
+transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const SuspBuf susp_in, const SuspBuf susp_out,
+                 const unsigned long long total_items)
+{
+    extern __shared__ float smem_f[];
+    const GeomSmem gs = load_geom(rc.geom, smem_f);
+    __syncthreads();
+
+    Packet pk;
+    pk.tau = 0.f; pk.tau_t = 0.f; pk.W = 0.f; pk.chan_run = 0; pk.pkt = 0; pk.m_inter = 0; pk.nev = 0; pk.fl_seg = 0;
+    pk.ray = Ray{};
+    int st = LS_IDLE;
+    const float* alpha_c = rc.alpha;  // table of this lane's channel
+    unsigned long long c_events = 0, c_seg = 0, c_esc = 0, c_abs = 0, c_surf = 0, c_stuck = 0;
+    double c_escw = 0.0;
+    const bool record = rc.n_obs_run > 0;
+    bool fresh_left = true;   // warp-uniform: fresh packets may still be available
+    const unsigned int n_susp_in = *susp_in.count;
+    bool susp_left = n_susp_in > 0;
+
+    for (;;) {
+        const unsigned m_fly = __ballot_sync(kFullMask, st == LS_FLY);
+        const unsigned m_ev = __ballot_sync(kFullMask, st >= LS_EV_MEDIUM && st <= LS_EV_SURFACE);
+        unsigned m_idle = __ballot_sync(kFullMask, st == LS_IDLE);
+        if (!(fresh_left || susp_left)) {  // nothing to fetch any more: idle lanes are done
+            if (st == LS_IDLE) st = LS_DONE;
+            m_idle = 0;
+        }
+        const int n_service = __popc(m_ev | m_idle);
+        if (n_service >= THRESH || (m_fly == 0 && n_service > 0)) {
+            // ---------------- fetch: resume suspended packets first, then fresh ones ----------------
+            if (m_idle) {
+                bool need = (st == LS_IDLE);
+                if (susp_left) {
+                    const unsigned m = __ballot_sync(kFullMask, need);
+                    unsigned int base = 0;
+                    if (lane_id() == __ffs(m) - 1) base = atomicAdd(susp_in.taken, (unsigned)__popc(m));
+                    base = __shfl_sync(kFullMask, base, __ffs(m) - 1);
+                    const unsigned int idx = base + rank_in_mask(m);
+                    if (need && idx < n_susp_in) {
+                        const float4 a = susp_in.s0[idx], b = susp_in.s1[idx];
+                        const uint4 c = susp_in.s2[idx];
+                        pk.W = a.w; pk.chan_run = c.x; pk.pkt = c.y; pk.m_inter = c.z; pk.nev = c.w & 0x0fffffffu;
+                        int i, j, k;
+                        unpack_cell(__float_as_uint(b.w), i, j, k);
+                        pk.ray.pcx = a.x; pk.ray.pcy = a.y; pk.ray.pcz = a.z; pk.ray.u = 0.f;
+                        pk.ray.nx = b.x; pk.ray.ny = b.y; pk.ray.nz = b.z;
+                        pk.ray.i = i; pk.ray.j = j; pk.ray.k = k;
+                        pk.ray.col = (k * gs.nlat + j) * gs.nlev;
+                        alpha_c = rc.alpha + (size_t)(rc.chan_begin + pk.chan_run) * rc.geom.ncell;
+                        const uint32_t kind = c.w >> 28;
+                        st = kind == EV_MEDIUM ? LS_EV_MEDIUM : (kind == EV_EMIT ? LS_EV_EMIT : LS_EV_SURFACE);
+                        need = false;
+                    }
+                    if (base + __popc(m) >= n_susp_in) susp_left = false;
+                }
+                if (fresh_left) {
+                    const unsigned m = __ballot_sync(kFullMask, need);
+                    if (m) {
+                        if (record && *(volatile unsigned int*)ev.count >= ev.soft_cap) {
+                            fresh_left = false;  // event buffer nearly full: let the pass drain
+                        } else {
+                            unsigned long long base = 0;
+                            if (lane_id() == __ffs(m) - 1) base = atomicAdd(rc.work_counter, (unsigned long long)__popc(m));
+                            base = __shfl_sync(kFullMask, base, __ffs(m) - 1);
+                            const unsigned long long item = base + rank_in_mask(m);
+                            if (base + __popc(m) >= total_items) fresh_left = false;
+                            if (need && item < total_items) {
+                                pk.chan_run = uint32_t(item / rc.n_pkt);
+                                pk.pkt = rc.pkt_begin + uint32_t(item - (unsigned long long)pk.chan_run * rc.n_pkt);
+                                pk.m_inter = 0; pk.nev = 0;
+                                const int ctab = rc.chan_begin + int(pk.chan_run);
+                                alpha_c = rc.alpha + (size_t)ctab * rc.geom.ncell;
+                                const uint32_t ckey = rc.chan_key0 + uint32_t(ctab);
+                                const Zeta4 z = zeta_block(rc.seed, ckey, pk.pkt, 0, 0);
+                                if (rc.mode == 0) {
+                                    // O3: uniform point on the star-facing TOA disc, direction -s^
+                                    const float b = rc.geom.Rtoa * sqrtf(z.z0);
+                                    float sp, cp;
+                                    sincospif(2.0f * z.z1, &sp, &cp);
+                                    const float h = rc.geom.Rtoa * sqrtf(1.0f - z.z0);
+                                    const float ax = b * cp, ay = b * sp;
+                                    const float px = ax * rc.e1[0] + ay * rc.e2[0] + h * rc.star[0];
+                                    const float py = ax * rc.e1[1] + ay * rc.e2[1] + h * rc.star[1];
+                                    const float pz = ax * rc.e1[2] + ay * rc.e2[2] + h * rc.star[2];
+                                    int j, k;
+                                    locate_angles(gs, px, py, pz, j, k);
+                                    pk.W = 1.0f;
+                                    pk.tau_t = -logf(z.z2);
+                                    pk.tau = 0.f; pk.fl_seg = 0;
+                                    ray_init(pk.ray, gs, px, py, pz, -rc.star[0], -rc.star[1], -rc.star[2], gs.nlev - 1,
+                                             j, k, alpha_c);
+                                    st = LS_FLY;
+                                } else {
+                                    // O4: cell ~ luminosity (Eq. 13) with composite bias xi, uniform point in the cell
+                                    const int ncell = rc.geom.ncell;
+                                    const double* cum = rc.Lcum + (size_t)ctab * ncell;
+                                    const double Ltot = rc.Ltot[ctab];
+                                    int cell;
+                                    st = LS_EV_EMIT;
+                                    if (!(Ltot > 0.0)) {
+                                        cell = 0; st = LS_IDLE; finish_packet(rc, pk);
+                                    } else if (double(z.z0) < rc.xi) {
+                                        cell = min(int(floor(double(z.z0) / rc.xi * ncell)), ncell - 1);
+                                    } else {
+                                        const double x = (double(z.z0) - rc.xi) / (1.0 - rc.xi) * Ltot;
+                                        int lo = 0, hi = ncell - 1;
+                                        while (lo < hi) {
+                                            const int mid = (lo + hi) >> 1;
+                                            if (cum[mid] > x) hi = mid; else lo = mid + 1;
+                                        }
+                                        cell = lo;
+                                    }
+                                    if (st == LS_EV_EMIT) {
+                                        float W = 1.0f;
+                                        bool live = true;
+                                        if (rc.xi > 0.0) {
+                                            const double Li = rc.Lcell[(size_t)ctab * ncell + cell];
+                                            live = Li > 0.0;
+                                            W = live ? float(1.0 / ((1.0 - rc.xi) + rc.xi * Ltot / (double(ncell) * Li))) : 0.f;
+                                        }
+                                        if (!live) {
+                                            st = LS_IDLE; finish_packet(rc, pk);
+                                        } else {
+                                            const int i = cell % gs.nlev, j = (cell / gs.nlev) % gs.nlat,
+                                                      k = cell / (gs.nlev * gs.nlat);
+                                            const float r = gs.R[i] * cbrtf(fmaf(z.z1, gs.qcube[i], 1.0f));
+                                            const float ct = fmaf(z.z2, gs.cth[j + 1] - gs.cth[j], gs.cth[j]);
+                                            const float sth = sqrtf(fmaxf(0.f, 1.0f - ct * ct));
+                                            const float phi = fmaf(z.z3, gs.ph[k + 1] - gs.ph[k], gs.ph[k]);
+                                            float sp, cp;
+                                            sincosf(phi, &sp, &cp);
+                                            pk.W = W;
+                                            pk.ray.pcx = r * sth * cp; pk.ray.pcy = r * sth * sp; pk.ray.pcz = r * ct;
+                                            pk.ray.u = 0.f; pk.ray.nx = 0.f; pk.ray.ny = 0.f; pk.ray.nz = 1.f;
+                                            pk.ray.i = i; pk.ray.j = j; pk.ray.k = k;
+                                            pk.ray.col = (k * gs.nlat + j) * gs.nlev;
+                                        }
+                                    }
+                                }
+                            }
+                        }
+                    }
+                }
+            }
+            // ---------------- events: record for the peel kernel, then absorb / scatter ----------------
+            const bool is_ev = st >= LS_EV_MEDIUM && st <= LS_EV_SURFACE;
+            const unsigned m_e = __ballot_sync(kFullMask, is_ev);
+            if (m_e) {
+                unsigned int slot = 0;
+                bool have_slot = true;
+                if (record) {
+                    unsigned int base = 0;
+                    if (lane_id() == __ffs(m_e) - 1) base = atomicAdd(ev.count, (unsigned)__popc(m_e));
+                    base = __shfl_sync(kFullMask, base, __ffs(m_e) - 1);
+                    slot = base + rank_in_mask(m_e);
+                    have_slot = slot < ev.cap;
+                }
+                if (is_ev) {
+                    float px, py, pz;
+                    ray_position(pk.ray, px, py, pz);
+                    const uint32_t cellp = pack_cell(pk.ray.i, pk.ray.j, pk.ray.k);
+                    const uint32_t kind = st == LS_EV_MEDIUM ? EV_MEDIUM : (st == LS_EV_EMIT ? EV_EMIT : EV_SURFACE);
+                    if (!have_slot) {
+                        // event buffer full: park the packet for the next pass
+                        const unsigned int sidx = atomicAdd(susp_out.count, 1u);
+                        susp_out.s0[sidx] = make_float4(px, py, pz, pk.W);
+                        susp_out.s1[sidx] = make_float4(pk.ray.nx, pk.ray.ny, pk.ray.nz, __uint_as_float(cellp));
+                        susp_out.s2[sidx] = make_uint4(pk.chan_run, pk.pkt, pk.m_inter, pk.nev | kind << 28);
+                        st = LS_DONE;
+                    } else {
+                        const int ctab = rc.chan_begin + int(pk.chan_run);
+                        const uint32_t ckey = rc.chan_key0 + uint32_t(ctab);
+                        const int cell = pk.ray.col + pk.ray.i;
+                        const uint32_t meta = kind | batch_of(rc, pk.pkt) << 2 | pk.chan_run << 8;
+                        ++c_events;
+                        ++pk.nev;
+                        if (st == LS_EV_MEDIUM) {
+                            const float4 pr = __ldg(rc.prop + (size_t)ctab * rc.geom.ncell + cell);
+                            if (record) {
+                                ev.e0[slot] = make_float4(px, py, pz, pk.W * pr.x);
+                                ev.e1[slot] = make_float4(pk.ray.nx, pk.ray.ny, pk.ray.nz, pr.y);
+                                ev.e2[slot] = make_float4(pr.z, __uint_as_float(cellp), __uint_as_float(meta),
+                                                          __uint_as_float(pk.pkt));
+                            }
+                            ++pk.m_inter;
+                            const Zeta4 z = zeta_block(rc.seed, ckey, pk.pkt, pk.m_inter, 1);
+                            if ((rc.max_events && int(pk.m_inter) == rc.max_events) || !rc.scatter_on || z.z0 >= pr.x) {
+                                ++c_abs; st = LS_IDLE; finish_packet(rc, pk);       // L192: absorbed
+                            } else {
+                                const float ct = (z.z0 < pr.x * pr.y) ? sample_rayleigh(z.z1) : sample_hg(pr.z, z.z1);
+                                float nx = pk.ray.nx, ny = pk.ray.ny, nz = pk.ray.nz;
+                                rotate_dir(nx, ny, nz, ct, z.z2);
+                                pk.tau_t = -logf(z.z3); pk.tau = 0.f; pk.fl_seg = 0;
+                                ray_init(pk.ray, gs, px, py, pz, nx, ny, nz, pk.ray.i, pk.ray.j, pk.ray.k, alpha_c);
+                                st = LS_FLY;
+                            }
+                        } else if (st == LS_EV_EMIT) {
+                            if (record) {
+                                ev.e0[slot] = make_float4(px, py, pz, pk.W);
+                                ev.e1[slot] = make_float4(0.f, 0.f, 1.f, 0.f);
+                                ev.e2[slot] = make_float4(0.f, __uint_as_float(cellp), __uint_as_float(meta),
+                                                          __uint_as_float(pk.pkt));
+                            }
+                            if (!rc.scatter_on) {
+                                ++c_abs; st = LS_IDLE; finish_packet(rc, pk);
+                            } else {
+                                const Zeta4 z = zeta_block(rc.seed, ckey, pk.pkt, 1, 0);
+                                const float nz = fmaf(2.0f, z.z0, -1.0f);   // Eq. 2
+                                const float ns = sqrtf(fmaxf(0.f, 1.0f - nz * nz));
+                                float sp, cp;
+                                sincospif(2.0f * z.z1, &sp, &cp);
+                                pk.tau_t = -logf(z.z2); pk.tau = 0.f; pk.fl_seg = 0;
+                                ray_init(pk.ray, gs, px, py, pz, ns * cp, ns * sp, nz, pk.ray.i, pk.ray.j, pk.ray.k, alpha_c);
+                                st = LS_FLY;
+                            }
+                        } else {  // Lambert surface (O7, Eq. 3-4)
+                            const float a = rc.surface_albedo;
+                            const float rn = rsqrtf(fmaf(px, px, fmaf(py, py, pz * pz)));
+                            float hx = px * rn, hy = py * rn, hz = pz * rn;
+                            if (record) {
+                                ev.e0[slot] = make_float4(px, py, pz, pk.W * a);
+                                ev.e1[slot] = make_float4(hx, hy, hz, 0.f);
+                                ev.e2[slot] = make_float4(0.f, __uint_as_float(cellp), __uint_as_float(meta),
+                                                          __uint_as_float(pk.pkt));
+                            }
+                            ++pk.m_inter;
+                            const Zeta4 z = zeta_block(rc.seed, ckey, pk.pkt, pk.m_inter, 3);
+                            if (rc.max_events && int(pk.m_inter) == rc.max_events) {
+                                ++c_abs; st = LS_IDLE; finish_packet(rc, pk);
+                            } else if (z.z0 >= a) {
+                                ++c_surf; st = LS_IDLE; finish_packet(rc, pk);
+                            } else {
+                                rotate_dir(hx, hy, hz, sqrtf(z.z1), z.z2);      // Eq. 4 about the normal
+                                pk.tau_t = -logf(z.z3); pk.tau = 0.f; pk.fl_seg = 0;
+                                ray_init(pk.ray, gs, px, py, pz, hx, hy, hz, 0, pk.ray.j, pk.ray.k, alpha_c);
+                                st = LS_FLY;
+                            }
+                        }
+                    }
+                }
+            }
+        }
+        if (__ballot_sync(kFullMask, st == LS_FLY) == 0) {
+            if (__ballot_sync(kFullMask, st != LS_DONE) == 0) break;
+            continue;
+        }
+        // ---------------- march: up to KSTEPS cell crossings per lane ----------------
+#pragma unroll 1
+        for (int s = 0; s < KSTEPS; ++s) {
+            if (st == LS_FLY) {
+                const int rs = ray_step(pk.ray, gs, pk.tau, pk.tau_t, alpha_c);
+                ++c_seg;
+                if (rs != RAY_FLYING) {
+                    if (rs == RAY_LIMIT) {
+                        st = LS_EV_MEDIUM;
+                    } else if (rs == RAY_ESCAPE) {
+                        ++c_esc; c_escw += double(pk.W); st = LS_IDLE; finish_packet(rc, pk);
+                    } else {  // RAY_SURFACE
+                        if (rc.surface_albedo > 0.f) st = LS_EV_SURFACE;
+                        else { ++c_surf; st = LS_IDLE; finish_packet(rc, pk); }
+                    }
+                } else if (++pk.fl_seg > rc.geom.maxseg) {
+                    ++c_stuck; st = LS_IDLE; finish_packet(rc, pk);
+                }
+            }
+        }
+    }
+
+    // counters: warp reduce, one atomic per warp
+    c_events = warp_sum_u64(c_events); c_seg = warp_sum_u64(c_seg); c_esc = warp_sum_u64(c_esc);
+    c_abs = warp_sum_u64(c_abs); c_surf = warp_sum_u64(c_surf); c_stuck = warp_sum_u64(c_stuck);
+    c_escw = warp_sum_f64(c_escw);
+    if (lane_id() == 0) {
+        if (c_events) atomicAdd(&rc.counters->events, c_events);
+        if (c_seg) atomicAdd(&rc.counters->seg_transport, c_seg);
+        if (c_esc) atomicAdd(&rc.counters->escaped, c_esc);
+        if (c_abs) atomicAdd(&rc.counters->absorbed, c_abs);
+        if (c_surf) atomicAdd(&rc.counters->surface, c_surf);
+        if (c_stuck) atomicAdd(&rc.counters->stuck, c_stuck);
+        if (c_escw != 0.0) atomicAdd(&rc.counters->escaped_weight, c_escw);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Peel-off kernel (A7 + A9): one ray per (event, observer); persistent lanes with warp-level refill;
+// f = pref * Theta * exp(-tau_obs) (Eq. 14) accumulated in warp-private shared-memory bins [obs][batch] of the
+// warp's current channel, flushed to the fp64 global sums when the channel changes and at the end.
+// ---------------------------------------------------------------------------------------------------------
+template <int THRESH, int KSTEPS>
+__global__ void __launch_bounds__(kPeelThreads, 2)
+peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev)
+{
+    extern __shared__ float smem_f[];
+    const GeomSmem gs = load_geom(rc.geom, smem_f);
+    const int nbins = rc.n_obs_run * rc.n_batches;
+    float* bins = smem_f + ((rc.geom.tab_floats + 31) & ~31) + (threadIdx.x >> 5) * nbins;
+    for (int t = lane_id(); t < nbins; t += 32) bins[t] = 0.f;
+    __syncthreads();
+
+    const unsigned int n_events = min(*ev.count, ev.cap);
+    const unsigned long long n_rays = (unsigned long long)n_events * rc.n_obs_run;
+    int warp_chan = -1;  // channel (run-local) the warp's bins belong to
+
+    Ray ray{};
+    float tau = 0.f, pref = 0.f;
+    uint32_t meta = 0;
+    int obs = 0, fl_seg = 0;
+    bool fly = false;
+    bool work_left = n_rays > 0;
+    unsigned long long c_seg = 0, c_rays = 0;
+    float ipx = 0.f, ipy = 0.f, ipz = 0.f;
+
+    for (;;) {
+        const unsigned m_idle = __ballot_sync(kFullMask, !fly);
+        if (work_left && (__popc(m_idle) >= THRESH)) {
+            unsigned long long base = 0;
+            if (lane_id() == __ffs(m_idle) - 1) base = atomicAdd(rc.ray_counter, (unsigned long long)__popc(m_idle));
+            base = __shfl_sync(kFullMask, base, __ffs(m_idle) - 1);
+            const unsigned long long rid = base + rank_in_mask(m_idle);
+            if (base + __popc(m_idle) >= n_rays) work_left = false;
+            int new_chan = -1;
+            if (!fly && rid < n_rays) {
+                const unsigned int e = (unsigned int)(rid / rc.n_obs_run);
+                obs = int(rid - (unsigned long long)e * rc.n_obs_run);
+                const float4 a = __ldg(ev.e0 + e), b = __ldg(ev.e1 + e), c = __ldg(ev.e2 + e);
+                meta = __float_as_uint(c.z);
+                const uint32_t kind = meta & 3u;
+                const float* od = rc.obs[rc.obs_first + obs];
+                const float mu = b.x * od[0] + b.y * od[1] + b.z * od[2];
+                float theta;
+                if (kind == EV_MEDIUM) {  // C6: mixture phase function, per steradian (Eq. 5, Eq. 7)
+                    const float g = c.x;
+                    const float d = fmaf(-2.0f * g, mu, 1.0f + g * g);
+                    const float hg = (1.0f - g * g) / (4.0f * kPi * d * sqrtf(d));
+                    const float ray_p = 3.0f * (1.0f + mu * mu) / (16.0f * kPi);
+                    theta = b.w * ray_p + (1.0f - b.w) * hg;
+                } else if (kind == EV_EMIT) {
+                    theta = 1.0f / (4.0f * kPi);
+                } else {
+                    theta = fmaxf(mu, 0.0f) / kPi;
+                }
+                pref = a.w * theta;
+                new_chan = int(meta >> 8);
+                if (pref > 0.0f) {
+                    int i, j, k;
+                    unpack_cell(__float_as_uint(c.y), i, j, k);
+                    const float* alpha_c = rc.alpha + (size_t)(rc.chan_begin + new_chan) * rc.geom.ncell;
+                    ray_init(ray, gs, a.x, a.y, a.z, od[0], od[1], od[2], i, j, k, alpha_c);
+                    ipx = a.x; ipy = a.y; ipz = a.z;
+                    tau = 0.f; fl_seg = 0;
+                    fly = true;
+                    ++c_rays;
+                }
+            }
+            // the warp's bins follow the newest channel; stragglers of older channels go straight to global memory
+            int mx = new_chan;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(kFullMask, mx, o));
+            if (mx > warp_chan) {
+                if (warp_chan >= 0) {
+                    __syncwarp();
+                    for (int t = lane_id(); t < nbins; t += 32) {
+                        const float v = bins[t];
+                        if (v != 0.f) {
+                            const int o = t / rc.n_batches, bt = t - o * rc.n_batches;
+                            atomicAdd(rc.flux + ((size_t)warp_chan * rc.n_obs_total + rc.obs_first + o) * rc.n_batches + bt,
+                                      double(v));
+                            bins[t] = 0.f;
+                        }
+                    }
+                    __syncwarp();
+                }
+                warp_chan = mx;
+            }
+        }
+        if (__ballot_sync(kFullMask, fly) == 0) {
+            if (!work_left) break;
+            continue;
+        }
+#pragma unroll 1
+        for (int s = 0; s < KSTEPS; ++s) {
+            if (fly) {
+                const int chan = int(meta >> 8);
+                const float* alpha_c = rc.alpha + (size_t)(rc.chan_begin + chan) * rc.geom.ncell;
+                const int rs = ray_step(ray, gs, tau, rc.tau_cut, alpha_c);
+                ++c_seg;
+                if (rs == RAY_ESCAPE) {
+                    const float f = pref * expf(-tau);
+                    const int bt = int((meta >> 2) & 63u);
+                    if (chan == warp_chan) atomicAdd(bins + obs * rc.n_batches + bt, f);
+                    else atomicAdd(rc.flux + ((size_t)chan * rc.n_obs_total + rc.obs_first + obs) * rc.n_batches + bt, double(f));
+                    if (rc.image) {
+                        const int o = rc.obs_first + obs;
+                        const float X = ipx * rc.img_ex[o][0] + ipy * rc.img_ex[o][1] + ipz * rc.img_ex[o][2];
+                        const float Y = ipx * rc.img_ey[o][0] + ipy * rc.img_ey[o][1] + ipz * rc.img_ey[o][2];
+                        const int ix = min(max(int(floorf((X / rc.geom.Rtoa + 1.0f) * 0.5f * rc.npix)), 0), rc.npix - 1);
+                        const int iy = min(max(int(floorf((Y / rc.geom.Rtoa + 1.0f) * 0.5f * rc.npix)), 0), rc.npix - 1);
+                        atomicAdd(rc.image + ((size_t)chan * rc.n_obs_total + o) * rc.npix * rc.npix + iy * rc.npix + ix, f);
+                    }
+                    fly = false;
+                } else if (rs != RAY_FLYING) {
+                    fly = false;   // surface hit or tau_obs > tau_cut: nothing reaches the observer
+                } else if (++fl_seg > rc.geom.maxseg) {
+                    fly = false;
+                }
+            }
+        }
+    }
+    __syncwarp();
+    if (warp_chan >= 0) {
+        for (int t = lane_id(); t < nbins; t += 32) {
+            const float v = bins[t];
+            if (v != 0.f) {
+                const int o = t / rc.n_batches, bt = t - o * rc.n_batches;
+                atomicAdd(rc.flux + ((size_t)warp_chan * rc.n_obs_total + rc.obs_first + o) * rc.n_batches + bt, double(v));
+            }
+        }
+    }
+    c_seg = warp_sum_u64(c_seg); c_rays = warp_sum_u64(c_rays);
+    if (lane_id() == 0) {
+        if (c_seg) atomicAdd(&rc.counters->seg_peel, c_seg);
+        if (c_rays) atomicAdd(&rc.counters->rays_peel, c_rays);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// A10: value and batch-means sigma (C12) per (channel, observer).
+// ---------------------------------------------------------------------------------------------------------
+__global__ void normalise_kernel(int n_chan_run, int n_obs, int n_batches, unsigned long long N, unsigned long long lo,
+                                 unsigned long long hi, const double* __restrict__ flux, const double* __restrict__ Ltot,
+                                 int emission, double* __restrict__ value, double* __restrict__ sigma)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_chan_run * n_obs) return;
+    const double* S = flux + (size_t)t * n_batches;
+    double sum = 0.0, n_run = 0.0, m1 = 0.0, m2 = 0.0;
+    int used = 0;
+    for (int b = 0; b < n_batches; ++b) {
+        unsigned long long e0 = ((unsigned long long)b * N + n_batches - 1) / n_batches;
+        unsigned long long e1 = ((unsigned long long)(b + 1) * N + n_batches - 1) / n_batches;
+        e0 = e0 < lo ? lo : e0;
+        e1 = e1 > hi ? hi : e1;
+        const double cnt = e1 > e0 ? double(e1 - e0) : 0.0;
+        sum += S[b];
+        n_run += cnt;
+        if (cnt > 0.0) { const double bm = S[b] / cnt; m1 += bm; m2 += bm * bm; ++used; }
+    }
+    double mean = n_run > 0.0 ? sum / n_run : 0.0;
+    double sg = 0.0;
+    if (used > 1) {
+        const double mu = m1 / used;
+        const double var = fmax(0.0, (m2 - used * mu * mu) / (used - 1));
+        sg = sqrt(var / used);
+    }
+    const double scale = emission ? Ltot[t] : 1.0;
+    if (value) value[t] = mean * scale;
+    if (sigma) sigma[t] = sg * scale;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Test-only kernels.
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) debug_ray_tau_kernel(const GeomParams g, const float* __restrict__ alpha_c, long n,
+                                                           const float* __restrict__ pos, const float* __restrict__ dir,
+                                                           float* __restrict__ tau_out, int* __restrict__ hit)
+{
+    extern __shared__ float smem_f[];
+    const GeomSmem gs = load_geom(g, smem_f);
+    __syncthreads();
+    const long m = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    const float px = pos[3 * m], py = pos[3 * m + 1], pz = pos[3 * m + 2];
+    int j, k;
+    locate_angles(gs, px, py, pz, j, k);
+    const int i = locate_ascending(gs.R, gs.nlev, sqrtf(px * px + py * py + pz * pz));
+    Ray ray{};
+    ray_init(ray, gs, px, py, pz, dir[3 * m], dir[3 * m + 1], dir[3 * m + 2], i, j, k, alpha_c);
+    float tau = 0.f;
+    int rs = RAY_FLYING, nseg = 0;
+    while (rs == RAY_FLYING && nseg++ <= g.maxseg) rs = ray_step(ray, gs, tau, kInf, alpha_c);
+    tau_out[m] = tau;
+    if (hit) hit[m] = rs == RAY_SURFACE ? 1 : (rs == RAY_ESCAPE ? 0 : -1);
+}
+
+__global__ void debug_philox_kernel(long n, const uint32_t* __restrict__ ctr, const uint32_t* __restrict__ key,
+                                    uint32_t* __restrict__ out)
+{
+    const long m = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    const Philox4 r = philox4x32_10(ctr[4 * m], ctr[4 * m + 1], ctr[4 * m + 2], ctr[4 * m + 3], key[2 * m], key[2 * m + 1]);
+    out[4 * m] = r.x; out[4 * m + 1] = r.y; out[4 * m + 2] = r.z; out[4 * m + 3] = r.w;
+}
+
+}  // namespace gcmcrt

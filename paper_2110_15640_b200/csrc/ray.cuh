@@ -1,0 +1,225 @@
+// ray.cuh -- fp32 ray marcher through the spherical-polar grid (A6 / A7), shared by the transport kernel and
+// the peel-off ray integrator.
+//
+// Formulation (differs from the paper-era "recompute six face distances from the current position" scheme the
+// oracle follows): a ray is described once by its invariants -- closest-approach point pc = p0 - n (p0.n), direction
+// n, impact parameter d^2 = |p0 x n|^2 -- and a running signed distance u from the closest-approach point, so that
+//   r(u)^2 = d^2 + u^2,   p(u) = pc + n u.
+// Every face crossing is then a closed-form root in u that depends only on the invariants and the face:
+//   shell R_k:           u = -/+ sqrt(R_k^2 - d^2)                      (1 MUFU)
+//   cone cos(theta)=c:   (n_z^2-c^2) u^2 + 2 z_c n_z u + (z_c^2 - c^2 d^2) = 0
+//   half-plane phi_e:    u = -(pc.N)/(n.N),  N = (-sin phi_e, cos phi_e, 0)
+// Only the face family that was just crossed is recomputed, positions are never advanced incrementally (no drift),
+// cell indices are tracked by crossings (never re-located from coordinates), and the face just crossed is excluded
+// by the strict comparison root > u, which is exact because the recomputed root is bit-identical to the u it set.
+#pragma once
+#include "device_common.cuh"
+
+namespace gcmcrt {
+
+// Geometry tables, staged by the host into one device array and copied to shared memory by every CTA.
+struct GeomParams {
+    int nlev, nlat, nlon, ncell;
+    const float* tab;  // packed: R[nlev+1] R2[nlev+1] qcube[nlev] cth[nlat+1] cph[nlon+1] sph[nlon+1] ph[nlon+1]
+    int tab_floats;
+    float Rtoa, R0;
+    int maxseg;
+};
+
+struct GeomSmem {
+    const float *R, *R2, *qcube, *cth, *cph, *sph, *ph;
+    int nlev, nlat, nlon;
+};
+
+__device__ __forceinline__ GeomSmem load_geom(const GeomParams& g, float* smem)
+{
+    for (int t = threadIdx.x; t < g.tab_floats; t += blockDim.x) smem[t] = g.tab[t];
+    GeomSmem s;
+    s.nlev = g.nlev; s.nlat = g.nlat; s.nlon = g.nlon;
+    s.R = smem;
+    s.R2 = s.R + (g.nlev + 1);
+    s.qcube = s.R2 + (g.nlev + 1);
+    s.cth = s.qcube + g.nlev;
+    s.cph = s.cth + (g.nlat + 1);
+    s.sph = s.cph + (g.nlon + 1);
+    s.ph = s.sph + (g.nlon + 1);
+    return s;
+}
+
+enum RayStatus : int { RAY_FLYING = 0, RAY_LIMIT = 1, RAY_ESCAPE = 2, RAY_SURFACE = 3, RAY_STUCK = 4 };
+
+struct Ray {
+    float pcx, pcy, pcz;  // closest-approach point
+    float nx, ny, nz;     // unit direction
+    float d2;             // impact parameter squared
+    float u;              // signed distance from the closest-approach point
+    float u_rad, u_lat, u_lon;  // next crossing of each face family
+    float alpha;          // extinction of the current cell
+    int i, j, k;          // cell
+    int col;              // (k*nlat + j)*nlev
+    int rad_step, lat_step, lon_step;
+};
+
+__device__ __forceinline__ void ray_setup_rad(Ray& r, const GeomSmem& s)
+{
+    if (r.u < 0.0f) {  // inward phase: the inner shell is hit iff it lies outside the impact parameter
+        const float q = s.R2[r.i] - r.d2;
+        if (q > 0.0f) {
+            r.u_rad = -sqrt_approx(q);
+            r.rad_step = -1;
+            return;
+        }
+    }
+    const float q = s.R2[r.i + 1] - r.d2;
+    r.u_rad = sqrt_approx(fmaxf(q, 0.0f));
+    r.rad_step = 1;
+}
+
+__device__ __forceinline__ void ray_cone_roots(const Ray& r, float c, int step, float& best, int& best_step)
+{
+    if (fabsf(c) < 1e-6f) {  // theta = pi/2: the plane z = 0
+        const float ur = -r.pcz * rcp_approx(r.nz);
+        if (ur > r.u && ur < best) { best = ur; best_step = step; }
+        return;
+    }
+    const float c2 = c * c;
+    const float A = fmaf(r.nz, r.nz, -c2);
+    const float B = r.pcz * r.nz;
+    const float C = fmaf(r.pcz, r.pcz, -c2 * r.d2);
+    const float inner = fmaf(r.d2, A, r.pcz * r.pcz);  // disc = c^2 (z_c^2 + d^2 A)
+    if (!(inner >= 0.0f)) return;
+    const float sq = fabsf(c) * sqrt_approx(inner);
+    const float q = -(B + copysignf(sq, B));
+    const float u1 = q * rcp_approx(A);   // A == 0 -> inf / nan: rejected by the comparisons below
+    const float u2 = C * rcp_approx(q);
+    if (u1 > r.u && u1 < best && fmaf(r.nz, u1, r.pcz) * c > 0.0f) { best = u1; best_step = step; }
+    if (u2 > r.u && u2 < best && fmaf(r.nz, u2, r.pcz) * c > 0.0f) { best = u2; best_step = step; }
+}
+
+__device__ __forceinline__ void ray_setup_lat(Ray& r, const GeomSmem& s)
+{
+    float best = kInf;
+    int step = 0;
+    if (s.nlat > 1) {
+        if (r.j > 0) ray_cone_roots(r, s.cth[r.j], -1, best, step);                // lower-colatitude edge
+        if (r.j + 1 < s.nlat) ray_cone_roots(r, s.cth[r.j + 1], +1, best, step);   // pole edges are no surfaces
+    }
+    r.u_lat = best;
+    r.lat_step = step;
+}
+
+__device__ __forceinline__ void ray_plane_root(const Ray& r, float cp, float sp, int step, float& best, int& best_step)
+{
+    const float den = fmaf(r.ny, cp, -r.nx * sp);  // n . N
+    const float num = fmaf(r.pcy, cp, -r.pcx * sp);
+    const float ur = -num * rcp_approx(den);        // den == 0 -> inf / nan: rejected
+    if (ur > r.u && ur < best) {
+        const float hx = fmaf(r.nx, ur, r.pcx), hy = fmaf(r.ny, ur, r.pcy);
+        if (fmaf(hx, cp, hy * sp) > 0.0f) { best = ur; best_step = step; }  // the half-plane, not its mirror
+    }
+}
+
+__device__ __forceinline__ void ray_setup_lon(Ray& r, const GeomSmem& s)
+{
+    float best = kInf;
+    int step = 0;
+    if (s.nlon > 1) {
+        ray_plane_root(r, s.cph[r.k], s.sph[r.k], -1, best, step);
+        ray_plane_root(r, s.cph[r.k + 1], s.sph[r.k + 1], +1, best, step);
+    }
+    r.u_lon = best;
+    r.lon_step = step;
+}
+
+// Start a ray at p with unit direction n inside cell (i,j,k).
+__device__ __forceinline__ void ray_init(Ray& r, const GeomSmem& s, float px, float py, float pz, float nx, float ny,
+                                         float nz, int i, int j, int k, const float* __restrict__ alpha_tab)
+{
+    const float b0 = fmaf(px, nx, fmaf(py, ny, pz * nz));
+    const float cx = fmaf(py, nz, -pz * ny), cy = fmaf(pz, nx, -px * nz), cz = fmaf(px, ny, -py * nx);
+    r.d2 = fmaf(cx, cx, fmaf(cy, cy, cz * cz));
+    r.pcx = fmaf(-nx, b0, px); r.pcy = fmaf(-ny, b0, py); r.pcz = fmaf(-nz, b0, pz);
+    r.nx = nx; r.ny = ny; r.nz = nz;
+    r.u = b0;
+    r.i = i; r.j = j; r.k = k;
+    r.col = (k * s.nlat + j) * s.nlev;
+    ray_setup_rad(r, s);
+    ray_setup_lat(r, s);
+    ray_setup_lon(r, s);
+    r.alpha = __ldg(alpha_tab + r.col + i);
+}
+
+// One cell crossing.  tau accumulates; returns RAY_FLYING, or why the ray stopped.
+__device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, float tau_limit,
+                                        const float* __restrict__ alpha_tab)
+{
+    const float un = fminf(r.u_rad, fminf(r.u_lat, r.u_lon));
+    const float ds = fmaxf(un - r.u, 0.0f);
+    const float dtau = r.alpha * ds;
+    if (tau + dtau >= tau_limit) {  // the limit is reached inside this cell
+        r.u += (tau_limit - tau) / r.alpha;
+        tau = tau_limit;
+        return RAY_LIMIT;
+    }
+    tau += dtau;
+    r.u = fmaxf(un, r.u);
+    if (un == r.u_rad) {  // ties: shells first (C1)
+        r.i += r.rad_step;
+        if (r.i >= s.nlev) { r.i = s.nlev - 1; return RAY_ESCAPE; }
+        if (r.i < 0) { r.i = 0; return RAY_SURFACE; }
+        ray_setup_rad(r, s);
+    } else if (un == r.u_lat) {
+        r.j = min(max(r.j + r.lat_step, 0), s.nlat - 1);
+        r.col = (r.k * s.nlat + r.j) * s.nlev;
+        ray_setup_lat(r, s);
+    } else {
+        r.k += r.lon_step;
+        r.k = (r.k < 0) ? r.k + s.nlon : (r.k >= s.nlon ? r.k - s.nlon : r.k);
+        r.col = (r.k * s.nlat + r.j) * s.nlev;
+        ray_setup_lon(r, s);
+    }
+    r.alpha = __ldg(alpha_tab + r.col + r.i);
+    return RAY_FLYING;
+}
+
+__device__ __forceinline__ void ray_position(const Ray& r, float& px, float& py, float& pz)
+{
+    px = fmaf(r.nx, r.u, r.pcx); py = fmaf(r.ny, r.u, r.pcy); pz = fmaf(r.nz, r.u, r.pcz);
+}
+
+// Binary search: cell m with e[m] <= x < e[m+1] (ascending edges), clamped.
+__device__ __forceinline__ int locate_ascending(const float* e, int n, float x)
+{
+    int lo = 0, hi = n;  // invariant: e[lo] <= x < e[hi] after clamping
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (x >= e[mid]) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+// Same for descending tables (cosines of ascending colatitudes).
+__device__ __forceinline__ int locate_descending(const float* e, int n, float x)
+{
+    int lo = 0, hi = n;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (x <= e[mid]) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+__device__ __forceinline__ void locate_angles(const GeomSmem& s, float px, float py, float pz, int& j, int& k)
+{
+    j = 0; k = 0;
+    if (s.nlat > 1) {
+        const float ct = pz * rsqrtf(fmaf(px, px, fmaf(py, py, pz * pz)));
+        j = locate_descending(s.cth, s.nlat, ct);
+    }
+    if (s.nlon > 1) {
+        float phi = atan2f(py, px);
+        if (phi < 0.0f) phi += 2.0f * kPi;
+        k = locate_ascending(s.ph, s.nlon, phi);
+    }
+}
+
+}  // namespace gcmcrt

@@ -77,6 +77,10 @@ typedef struct gcmcrt_counters {
     double escaped_weight;
     uint64_t passes;             /* transport/peel kernel pairs launched */
     uint64_t rays_peel;          /* peel-off rays integrated */
+    uint64_t launches;           /* kernels this call launched (all kinds) */
+    /* device time of this call's kernels by kind, from cudaEvents recorded on the caller's stream around each
+       launch (milliseconds, summed over passes / observers) */
+    double ms_stage, ms_emission_cdf, ms_transport, ms_peel;
 } gcmcrt_counters;
 
 /* Output buffers, all caller-owned, host|device, nullable unless stated. */

@@ -37,7 +37,8 @@ class Counters(C.Structure):
     _fields_ = [("events", C.c_uint64), ("segments_transport", C.c_uint64), ("segments_peel", C.c_uint64),
                 ("packets_escaped", C.c_uint64), ("packets_absorbed", C.c_uint64), ("packets_surface", C.c_uint64),
                 ("packets_stuck", C.c_uint64), ("escaped_weight", C.c_double), ("passes", C.c_uint64),
-                ("rays_peel", C.c_uint64)]
+                ("rays_peel", C.c_uint64), ("launches", C.c_uint64), ("ms_stage", C.c_double),
+                ("ms_emission_cdf", C.c_double), ("ms_transport", C.c_double), ("ms_peel", C.c_double)]
 
 
 class Result(C.Structure):
@@ -159,7 +160,8 @@ def _run(fn, handle, prm, n_chan_table, want_event_count, want_image, device_out
     N = p.packets_per_channel
     lo, hi = p.pkt_begin, (p.pkt_end or N)
     cb, ce = p.chan_begin, (p.chan_end or n_chan_table)
-    ncr, nobs, nb = ce - cb, max(p.n_obs, 1), (p.n_batches or 32)
+    ncr, nobs, nb = max(ce - cb, 0), max(p.n_obs, 1), (p.n_batches or 32)
+    hi = max(hi, lo)          # invalid ranges are reported by the library (E_INVALID), not by numpy
     shapes = {"flux_sum": ((ncr, nobs, nb), np.float64), "L_tot": ((ncr, nobs), np.float64),
               "value": ((ncr, nobs), np.float64), "sigma": ((ncr, nobs), np.float64)}
     if want_image and p.npix > 0:

@@ -76,6 +76,10 @@ struct gcmcrt_grid {
     unsigned int ev_cap = 0;
     int n_threads_resident = 0;
     PassCtrl* h_ctrl = nullptr;  // pinned
+    cudaEvent_t tev[4] = {nullptr, nullptr, nullptr, nullptr};   // kernel timing (A0 | A2 | transport | peel)
+    unsigned long long launches = 0, launches_pending = 0;
+    double ms_stage = 0.0, ms_emis = 0.0, ms_transport = 0.0, ms_peel = 0.0;
+    double ms_stage_pending = 0.0;   // staging done by set_opacity, reported by the next run
 };
 
 namespace {
@@ -151,6 +155,13 @@ void perp_basis(const double* d, float* e1, float* e2)
     for (int m = 0; m < 3; ++m) { e1[m] = float(a[m]); e2[m] = float(b[m]); }
 }
 
+cudaError_t ensure_events(gcmcrt_grid* g)
+{
+    for (auto& e : g->tev)
+        if (!e) { cudaError_t r = cudaEventCreate(&e); if (r != cudaSuccess) return r; }
+    return cudaSuccess;
+}
+
 // Stage alpha / prop for observer `obs_dir` (nullptr = unshifted table).
 int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStream_t s)
 {
@@ -164,6 +175,8 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
     sp.alpha = g->alpha.as<float>(); sp.prop = g->prop.as<float4>();
     sp.doppler = obs_dir != nullptr; sp.halfwidth = halfwidth;
     sp.vlos = nullptr; sp.reff = g->reff.as<float>();
+    CUDA_TRY(g, ensure_events(g));
+    CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
     if (obs_dir) {
         CUDA_TRY(g, g->vlos.ensure(size_t(g->ncell) * sizeof(float)));
         float o[3];
@@ -173,10 +186,19 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
                                                           g->thc32.as<float>(), g->phc32.as<float>(), o[0], o[1], o[2],
                                                           g->vlos.as<float>());
         sp.vlos = g->vlos.as<float>();
+        ++g->launches;
     }
     const long long blocks = std::min<long long>((long long)((n + 255) / 256), (long long)g->sm_count * 32);
     stage_kernel<<<(unsigned)std::max<long long>(blocks, 1), 256, 0, s>>>(sp);
     CUDA_TRY(g, cudaGetLastError());
+    ++g->launches;
+    CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
+    CUDA_TRY(g, cudaEventSynchronize(g->tev[1]));
+    {
+        float ms = 0.f;
+        CUDA_TRY(g, cudaEventElapsedTime(&ms, g->tev[0], g->tev[1]));
+        g->ms_stage_pending += ms;
+    }
     g->staged_obs = obs_dir ? 0 : -1;
     if (obs_dir) { for (int m = 0; m < 3; ++m) g->staged_dir[m] = obs_dir[m]; g->staged_halfwidth = halfwidth; }
     return GCMCRT_OK;
@@ -317,6 +339,9 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
 
     const int n_runs = prm->doppler_on ? std::max(n_obs, 1) : 1;
     unsigned long long passes = 0;
+    CUDA_TRY(g, ensure_events(g));
+    g->launches = g->launches_pending; g->launches_pending = 0; g->ms_emis = g->ms_transport = g->ms_peel = 0.0;
+    g->ms_stage = 0.0;
     for (int run = 0; run < n_runs; ++run) {
         // ---- A0/A1: make sure the staged table is the one this run needs
         if (prm->doppler_on && n_obs > 0) {
@@ -346,9 +371,18 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             ep.tau_vert_max = prm->tau_vert_max;
             ep.Lcell = g->Lcell.as<double>(); ep.Lcum = g->Lcum.as<double>(); ep.Ltot = g->Ltot.as<double>();
             const long long ncolc = (long long)g->n_chan * g->nlat * g->nlon;
+            CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
             emis_cell_kernel<<<(unsigned)((ncolc + 127) / 128), 128, 0, s>>>(ep);
             emis_scan_kernel<<<g->n_chan, 1024, 0, s>>>(ep);
             CUDA_TRY(g, cudaGetLastError());
+            CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
+            CUDA_TRY(g, cudaEventSynchronize(g->tev[1]));
+            {
+                float ms = 0.f;
+                CUDA_TRY(g, cudaEventElapsedTime(&ms, g->tev[0], g->tev[1]));
+                g->ms_emis += ms;
+            }
+            g->launches += 2;
             rc.Lcum = ep.Lcum; rc.Lcell = ep.Lcell; rc.Ltot = ep.Ltot;
             // L_tot output [n_chan_run][n_obs]
             const int o0 = prm->doppler_on ? run : 0, o1 = prm->doppler_on ? run + 1 : std::max(n_obs, 1);
@@ -377,12 +411,22 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             sin.count = &ctrl->susp_count[cur]; sin.taken = &ctrl->susp_taken[cur];
             sout.s0 = g->s0[nxt].as<float4>(); sout.s1 = g->s1[nxt].as<float4>(); sout.s2 = g->s2[nxt].as<uint4>();
             sout.count = &ctrl->susp_count[nxt]; sout.taken = &ctrl->susp_taken[nxt];
+            CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
             tk<<<grid_t, kTransportThreads, smem_t, s>>>(rc, ev, sin, sout, total_items);
+            CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
             if (rc.n_obs_run > 0) pk<<<g->sm_count * occ_p, kPeelThreads, smem_p, s>>>(rc, ev);
+            CUDA_TRY(g, cudaEventRecord(g->tev[2], s));
             CUDA_TRY(g, cudaGetLastError());
             ++passes;
+            g->launches += rc.n_obs_run > 0 ? 2 : 1;
             CUDA_TRY(g, cudaMemcpyAsync(g->h_ctrl, ctrl, sizeof(PassCtrl), cudaMemcpyDeviceToHost, s));
             CUDA_TRY(g, cudaStreamSynchronize(s));
+            {
+                float a = 0.f, b = 0.f;
+                CUDA_TRY(g, cudaEventElapsedTime(&a, g->tev[0], g->tev[1]));
+                CUDA_TRY(g, cudaEventElapsedTime(&b, g->tev[1], g->tev[2]));
+                g->ms_transport += a; g->ms_peel += b;
+            }
             const bool done = g->h_ctrl->work_counter >= total_items && g->h_ctrl->susp_count[nxt] == 0;
             if (done) break;
             // reset the per-pass counters: events, rays, the list just consumed
@@ -403,7 +447,10 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
                                                          static_cast<double*>(o_ltot.dev), emission,
                                                          static_cast<double*>(o_val.dev), static_cast<double*>(o_sig.dev));
         CUDA_TRY(g, cudaGetLastError());
+        ++g->launches;
     }
+    g->ms_stage += g->ms_stage_pending;
+    g->ms_stage_pending = 0.0;
     // ---- copy-backs for host-resident outputs
     bool need_sync = false;
     for (OutBuf* ob : {&o_flux, &o_ltot, &o_val, &o_sig, &o_img, &o_evc}) {
@@ -420,6 +467,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         hc.events = dc.events; hc.segments_transport = dc.seg_transport; hc.segments_peel = dc.seg_peel;
         hc.packets_escaped = dc.escaped; hc.packets_absorbed = dc.absorbed; hc.packets_surface = dc.surface;
         hc.packets_stuck = dc.stuck; hc.escaped_weight = dc.escaped_weight; hc.passes = passes; hc.rays_peel = dc.rays_peel;
+        hc.launches = g->launches; hc.ms_stage = g->ms_stage; hc.ms_emission_cdf = g->ms_emis;
+        hc.ms_transport = g->ms_transport; hc.ms_peel = g->ms_peel;
         if (is_device_ptr(out->counters)) CUDA_TRY(g, cudaMemcpyAsync(out->counters, &hc, sizeof hc, cudaMemcpyHostToDevice, s));
         else *out->counters = hc;
         need_sync = true;
@@ -547,7 +596,11 @@ int gcmcrt_set_opacity(gcmcrt_grid* g, int chan0, int n_chan, const float* lambd
     CUDA_TRY(g, cudaStreamSynchronize(s));
     g->chan0 = chan0;
     g->n_chan = n_chan;
-    return stage_opacity(g, nullptr, 0, s);
+    g->launches = 0;
+    g->ms_stage_pending = 0.0;
+    const int rcode = stage_opacity(g, nullptr, 0, s);
+    g->launches_pending = g->launches;
+    return rcode;
 }
 
 int gcmcrt_run_albedo(gcmcrt_grid* g, const gcmcrt_run_params* p, gcmcrt_result* out, void* stream)
@@ -572,6 +625,7 @@ int gcmcrt_destroy(gcmcrt_grid* g)
                       &g->value, &g->sigma, &g->image, &g->evcount})
         b->release();
     if (g->h_ctrl) cudaFreeHost(g->h_ctrl);
+    for (auto& e : g->tev) if (e) cudaEventDestroy(e);
     delete g;
     return GCMCRT_OK;
 }

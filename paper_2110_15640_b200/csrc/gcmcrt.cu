@@ -518,10 +518,11 @@ int gcmcrt_grid_create(gcmcrt_grid** out, int nlev, int nlat, int nlon, const do
     g->Omega = Omega; g->surface_albedo = surface_albedo;
     cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev);
 
-    // packed fp32 tables: R, R^2, qcube, cos(theta_e), cos(phi_e), sin(phi_e), phi_e
+    // packed fp32 tables: R, R^2 (high, low parts), qcube, cos(theta_e), cos(phi_e), sin(phi_e), phi_e
     std::vector<float> tab;
     for (int i = 0; i <= nlev; ++i) tab.push_back(float(g->r[i]));
     for (int i = 0; i <= nlev; ++i) tab.push_back(float(g->r[i] * g->r[i]));
+    for (int i = 0; i <= nlev; ++i) { const double r2 = g->r[i] * g->r[i]; tab.push_back(float(r2 - double(float(r2)))); }
     for (int i = 0; i < nlev; ++i) { const double q = g->r[i + 1] / g->r[i]; tab.push_back(float(q * q * q - 1.0)); }
     std::vector<double> cth(nlat + 1);
     for (int j = 0; j <= nlat; ++j) cth[j] = j == 0 ? 1.0 : (j == nlat ? -1.0 : std::cos(g->th[j]));

@@ -20,14 +20,14 @@ namespace gcmcrt {
 // Geometry tables, staged by the host into one device array and copied to shared memory by every CTA.
 struct GeomParams {
     int nlev, nlat, nlon, ncell;
-    const float* tab;  // packed: R[nlev+1] R2[nlev+1] qcube[nlev] cth[nlat+1] cph[nlon+1] sph[nlon+1] ph[nlon+1]
+    const float* tab;  // packed: R[nlev+1] R2[nlev+1] R2lo[nlev+1] qcube[nlev] cth[nlat+1] cph[nlon+1] sph[nlon+1] ph[nlon+1]
     int tab_floats;
     float Rtoa, R0;
     int maxseg;
 };
 
 struct GeomSmem {
-    const float *R, *R2, *qcube, *cth, *cph, *sph, *ph;
+    const float *R, *R2, *R2lo, *qcube, *cth, *cph, *sph, *ph;
     int nlev, nlat, nlon;
 };
 
@@ -38,7 +38,8 @@ __device__ __forceinline__ GeomSmem load_geom(const GeomParams& g, float* smem)
     s.nlev = g.nlev; s.nlat = g.nlat; s.nlon = g.nlon;
     s.R = smem;
     s.R2 = s.R + (g.nlev + 1);
-    s.qcube = s.R2 + (g.nlev + 1);
+    s.R2lo = s.R2 + (g.nlev + 1);
+    s.qcube = s.R2lo + (g.nlev + 1);
     s.cth = s.qcube + g.nlev;
     s.cph = s.cth + (g.nlat + 1);
     s.sph = s.cph + (g.nlon + 1);
@@ -51,7 +52,8 @@ enum RayStatus : int { RAY_FLYING = 0, RAY_LIMIT = 1, RAY_ESCAPE = 2, RAY_SURFAC
 struct Ray {
     float pcx, pcy, pcz;  // closest-approach point
     float nx, ny, nz;     // unit direction
-    float d2;             // impact parameter squared
+    float d2;             // impact parameter squared: high part of the double-float (d2, d2lo)
+    float d2lo;           // low part: R_k^2 - d^2 cancels catastrophically in plain fp32 for grazing rays
     float u;              // signed distance from the closest-approach point
     float u_rad, u_lat, u_lon;  // next crossing of each face family
     float alpha;          // extinction of the current cell
@@ -63,14 +65,14 @@ struct Ray {
 __device__ __forceinline__ void ray_setup_rad(Ray& r, const GeomSmem& s)
 {
     if (r.u < 0.0f) {  // inward phase: the inner shell is hit iff it lies outside the impact parameter
-        const float q = s.R2[r.i] - r.d2;
+        const float q = (s.R2[r.i] - r.d2) + (s.R2lo[r.i] - r.d2lo);
         if (q > 0.0f) {
             r.u_rad = -sqrt_approx(q);
             r.rad_step = -1;
             return;
         }
     }
-    const float q = s.R2[r.i + 1] - r.d2;
+    const float q = (s.R2[r.i + 1] - r.d2) + (s.R2lo[r.i + 1] - r.d2lo);
     r.u_rad = sqrt_approx(fmaxf(q, 0.0f));
     r.rad_step = 1;
 }
@@ -136,8 +138,16 @@ __device__ __forceinline__ void ray_init(Ray& r, const GeomSmem& s, float px, fl
                                          float nz, int i, int j, int k, const float* __restrict__ alpha_tab)
 {
     const float b0 = fmaf(px, nx, fmaf(py, ny, pz * nz));
-    const float cx = fmaf(py, nz, -pz * ny), cy = fmaf(pz, nx, -px * nz), cz = fmaf(px, ny, -py * nx);
-    r.d2 = fmaf(cx, cx, fmaf(cy, cy, cz * cz));
+    {   // d^2 = |p x n|^2 / |n|^2 in fp64, kept as a double-float: once per ray, so that every later
+        // R_k^2 - d^2 is exact to fp32 rounding (fp32 products of 1e8 m coordinates carry 1e9 m^2 of error)
+        const double dpx = px, dpy = py, dpz = pz, dnx = nx, dny = ny, dnz = nz;
+        const double cx = dpy * dnz - dpz * dny, cy = dpz * dnx - dpx * dnz, cz = dpx * dny - dpy * dnx;
+        const double eps = fma(dnx, dnx, fma(dny, dny, fma(dnz, dnz, -1.0)));   // |n|^2 - 1 ~ 1e-7
+        const double cc = fma(cx, cx, fma(cy, cy, cz * cz));
+        const double d2 = fma(-cc, eps * (1.0 - eps), cc);                      // cc / (1 + eps)
+        r.d2 = float(d2);
+        r.d2lo = float(d2 - double(r.d2));
+    }
     r.pcx = fmaf(-nx, b0, px); r.pcy = fmaf(-ny, b0, py); r.pcz = fmaf(-nz, b0, pz);
     r.nx = nx; r.ny = ny; r.nz = nz;
     r.u = b0;

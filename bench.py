@@ -276,7 +276,7 @@ def run_ours(args):
                     "work_lane_instr_per_launch": work / n_dom, "ms_per_launch": dur_ms / n_dom,
                     "hbm_term": {"bytes_per_step": hbm_bytes, "ms_at_peak": hbm_bytes / (pk["hbm_gbs"] * 1e9) * 1e3 * 1.0,
                                  "peak_gbs": pk["hbm_gbs"]},
-                    "kernel_ms_per_step": {k: acc[k] / args.steps for k in ("ms_stage", "ms_emission_cdf", "ms_transport", "ms_peel")}}
+                    "kernel_ms_per_step": {k: acc[k] / args.steps for k in ("ms_stage", "ms_emission_cdf", "ms_transport", "ms_sort", "ms_peel")}}
         cpu = oracle_leg(args.workload, grid, dict(opac, chan0=0), prm, mode) if world == 1 and not args.no_cpu else None
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
@@ -289,7 +289,10 @@ def run_ours(args):
                 "spectra_per_s": world * args.steps / (ms * 1e-3),
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                         "ms_per_step": ms_e2e / args.steps},
-                "gpu_launches": int(acc["launches"]), "clocks": clocks, "roofline": roofline}
+                "gpu_launches": int(acc["launches"]), "clocks": clocks, "roofline": roofline,
+                "counters_per_step": {k: acc[k] / args.steps for k in
+                                      ("events", "segments_transport", "segments_peel", "rays_peel", "packets_escaped",
+                                       "packets_absorbed", "packets_surface", "packets_stuck", "passes")}}
         if cpu is not None:
             line["cpu_baseline"] = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
         print(json.dumps(line), flush=True)

@@ -81,6 +81,7 @@ typedef struct gcmcrt_counters {
     /* device time of this call's kernels by kind, from cudaEvents recorded on the caller's stream around each
        launch (milliseconds, summed over passes / observers) */
     double ms_stage, ms_emission_cdf, ms_transport, ms_peel;
+    double ms_sort;              /* counting sort of the event records by (channel, cell) before each peel pass */
 } gcmcrt_counters;
 
 /* Output buffers, all caller-owned, host|device, nullable unless stated. */

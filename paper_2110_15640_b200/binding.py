@@ -38,7 +38,8 @@ class Counters(C.Structure):
                 ("packets_escaped", C.c_uint64), ("packets_absorbed", C.c_uint64), ("packets_surface", C.c_uint64),
                 ("packets_stuck", C.c_uint64), ("escaped_weight", C.c_double), ("passes", C.c_uint64),
                 ("rays_peel", C.c_uint64), ("launches", C.c_uint64), ("ms_stage", C.c_double),
-                ("ms_emission_cdf", C.c_double), ("ms_transport", C.c_double), ("ms_peel", C.c_double)]
+                ("ms_emission_cdf", C.c_double), ("ms_transport", C.c_double), ("ms_peel", C.c_double),
+                ("ms_sort", C.c_double)]
 
 
 class Result(C.Structure):

@@ -24,6 +24,11 @@ __device__ __forceinline__ float rcp_approx(float x)
     return y;
 }
 
+__device__ __forceinline__ void prefetch_l1(const void* p)
+{
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+}
+
 // ---- A3: Philox4x32-10 (Salmon et al. 2011).  key = (channel, packet), counter = (event, purpose, seed) ----
 struct Philox4 {
     uint32_t x, y, z, w;
@@ -60,6 +65,15 @@ __device__ __forceinline__ Zeta4 zeta_block(uint64_t seed, uint32_t chan, uint32
     const Philox4 r = philox4x32_10(event, purpose, static_cast<uint32_t>(seed), static_cast<uint32_t>(seed >> 32),
                                     chan, pkt);
     return Zeta4{u32_to_zeta(r.x), u32_to_zeta(r.y), u32_to_zeta(r.z), u32_to_zeta(r.w)};
+}
+
+// ---- exact 64-bit division by a run constant: q = floor(n / d) with m = floor(2^64 / d) computed on the host
+// (m = 2^64 - 1 for d = 1).  n m / 2^64 lies in (n/d - 1, n/d], so one correction step makes it exact.
+__device__ __forceinline__ unsigned long long div_magic(unsigned long long n, unsigned long long d, unsigned long long m)
+{
+    unsigned long long q = __umul64hi(n, m);
+    if (n - q * d >= d) ++q;
+    return q;
 }
 
 // ---- warp helpers ----

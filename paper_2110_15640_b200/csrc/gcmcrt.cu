@@ -72,13 +72,14 @@ struct gcmcrt_grid {
     DevBuf Lcell, Lcum, Ltot;
 
     // workspace
-    DevBuf ev0, ev1, ev2, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount;
+    DevBuf ev0, ev1, ev2, perm, hist, tile_sums, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount;
     unsigned int ev_cap = 0;
     int n_threads_resident = 0;
+    int tune[3] = {12, 8, 10};   // warp scheduling thresholds: service, lateral, peel refill (GCMCRT_TUNE overrides)
     PassCtrl* h_ctrl = nullptr;  // pinned
     cudaEvent_t tev[4] = {nullptr, nullptr, nullptr, nullptr};   // kernel timing (A0 | A2 | transport | peel)
     unsigned long long launches = 0, launches_pending = 0;
-    double ms_stage = 0.0, ms_emis = 0.0, ms_transport = 0.0, ms_peel = 0.0;
+    double ms_stage = 0.0, ms_emis = 0.0, ms_transport = 0.0, ms_peel = 0.0, ms_sort = 0.0;
     double ms_stage_pending = 0.0;   // staging done by set_opacity, reported by the next run
 };
 
@@ -137,6 +138,13 @@ GeomParams geom_params(const gcmcrt_grid* g)
     gp.R0 = float(g->r[0]);
     gp.maxseg = 8 * (g->nlev + g->nlat + g->nlon) + 64;
     return gp;
+}
+
+// floor(2^64 / d) for the kernels' exact division by a run constant (2^64 - 1 for d = 1)
+unsigned long long magic_div(unsigned long long d)
+{
+    if (d <= 1) return ~0ull;
+    return (unsigned long long)((((unsigned __int128)1) << 64) / d);
 }
 
 void normalize3(const double* in, float* out)
@@ -212,10 +220,18 @@ int ensure_workspace(gcmcrt_grid* g)
         if (cap < 64) cap = 64;
         if (cap > (1ull << 30)) cap = 1ull << 30;
         g->ev_cap = (unsigned int)cap;
+        if (const char* e = std::getenv("GCMCRT_TUNE")) {   // "service,lateral,refill": scheduling thresholds, 1..32
+            int a = 0, b = 0, c = 0;
+            if (std::sscanf(e, "%d,%d,%d", &a, &b, &c) == 3) {
+                g->tune[0] = std::min(std::max(a, 1), 32); g->tune[1] = std::min(std::max(b, 1), 32);
+                g->tune[2] = std::min(std::max(c, 1), 32);
+            }
+        }
     }
     CUDA_TRY(g, g->ev0.ensure(size_t(g->ev_cap) * sizeof(float4)));
     CUDA_TRY(g, g->ev1.ensure(size_t(g->ev_cap) * sizeof(float4)));
     CUDA_TRY(g, g->ev2.ensure(size_t(g->ev_cap) * sizeof(float4)));
+    CUDA_TRY(g, g->perm.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));
     CUDA_TRY(g, g->ctrl.ensure(sizeof(PassCtrl)));
     CUDA_TRY(g, g->counters.ensure(sizeof(DevCounters)));
     if (!g->h_ctrl) CUDA_TRY(g, cudaMallocHost((void**)&g->h_ctrl, sizeof(PassCtrl)));
@@ -312,6 +328,9 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.image = npix ? static_cast<float*>(o_img.dev) : nullptr;
     rc.event_count = static_cast<uint32_t*>(o_evc.dev);
     rc.counters = g->counters.as<DevCounters>();
+    rc.magic_N = magic_div(N);
+    rc.magic_npkt = magic_div(n_pkt);
+    rc.t_service = g->tune[0]; rc.t_lateral = g->tune[1]; rc.p_refill = g->tune[2];
     PassCtrl* ctrl = g->ctrl.as<PassCtrl>();
     rc.work_counter = &ctrl->work_counter;
     rc.ray_counter = &ctrl->ray_counter;
@@ -319,8 +338,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     // ---- launch geometry: persistent grids sized to the device
     const size_t smem_t = size_t(g->tab_floats) * sizeof(float);
     int occ_t = 0, occ_p = 0;
-    auto tk = transport_kernel<16, 8>;
-    auto pk = peel_kernel<12, 8>;
+    auto tk = transport_kernel<4>;
+    auto pk = peel_kernel<4>;
     CUDA_TRY(g, cudaFuncSetAttribute(tk, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_t)));
     CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_t, tk, kTransportThreads, smem_t));
     if (occ_t < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
@@ -340,7 +359,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     const int n_runs = prm->doppler_on ? std::max(n_obs, 1) : 1;
     unsigned long long passes = 0;
     CUDA_TRY(g, ensure_events(g));
-    g->launches = g->launches_pending; g->launches_pending = 0; g->ms_emis = g->ms_transport = g->ms_peel = 0.0;
+    g->launches = g->launches_pending; g->launches_pending = 0; g->ms_emis = g->ms_transport = g->ms_peel = g->ms_sort = 0.0;
     g->ms_stage = 0.0;
     for (int run = 0; run < n_runs; ++run) {
         // ---- A0/A1: make sure the staged table is the one this run needs
@@ -354,6 +373,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             if (g->staged_obs != -1 && (rcode = stage_opacity(g, nullptr, 0, s))) return rcode;
             rc.obs_first = 0; rc.n_obs_run = n_obs;
         }
+        rc.magic_nobs = magic_div((unsigned long long)std::max(rc.n_obs_run, 1));
         rc.alpha = g->alpha.as<float>();
         rc.prop = g->prop.as<float4>();
         // ---- A2: emission CDF
@@ -404,6 +424,20 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, pk, kPeelThreads, smem_p));
             if (occ_p < 1) return fail(g, GCMCRT_E_INVALID, "peel bins do not fit in shared memory");
         }
+        SortParams sp;
+        std::memset(&sp, 0, sizeof sp);
+        if (rc.n_obs_run > 0) {
+            const long long max_bins = 1ll << 25;
+            sp.c_fold = int(std::max<long long>(1, std::min<long long>(ncr, max_bins / g->ncell)));
+            sp.nbins = (unsigned int)((long long)sp.c_fold * g->ncell);
+            sp.n_tiles = (sp.nbins + kScanTile - 1) / kScanTile;
+            CUDA_TRY(g, g->hist.ensure(size_t(sp.nbins) * sizeof(unsigned int)));
+            CUDA_TRY(g, g->tile_sums.ensure(size_t(sp.n_tiles) * sizeof(unsigned int)));
+            sp.e2 = ev.e2; sp.count = ev.count; sp.cap = ev.cap;
+            sp.hist = g->hist.as<unsigned int>(); sp.tile_sums = g->tile_sums.as<unsigned int>();
+            sp.perm = g->perm.as<unsigned int>();
+            sp.nlev = g->nlev; sp.nlat = g->nlat; sp.ncell = g->ncell;
+        }
         for (;;) {
             const int nxt = 1 - cur;
             SuspBuf sin, sout;
@@ -414,18 +448,29 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
             tk<<<grid_t, kTransportThreads, smem_t, s>>>(rc, ev, sin, sout, total_items);
             CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
-            if (rc.n_obs_run > 0) pk<<<g->sm_count * occ_p, kPeelThreads, smem_p, s>>>(rc, ev);
+            if (rc.n_obs_run > 0) {
+                // counting sort of this pass's events by (channel, cell): sort.cuh
+                CUDA_TRY(g, cudaMemsetAsync(sp.hist, 0, size_t(sp.nbins) * sizeof(unsigned int), s));
+                ev_hist_kernel<<<g->sm_count * 8, 256, 0, s>>>(sp);
+                scan_reduce_kernel<<<sp.n_tiles, kScanThreads, 0, s>>>(sp);
+                scan_tiles_kernel<<<1, 1024, 0, s>>>(sp);
+                scan_apply_kernel<<<sp.n_tiles, kScanThreads, 0, s>>>(sp);
+                ev_scatter_kernel<<<g->sm_count * 8, 256, 0, s>>>(sp);
+            }
             CUDA_TRY(g, cudaEventRecord(g->tev[2], s));
+            if (rc.n_obs_run > 0) pk<<<g->sm_count * occ_p, kPeelThreads, smem_p, s>>>(rc, ev, sp.perm);
+            CUDA_TRY(g, cudaEventRecord(g->tev[3], s));
             CUDA_TRY(g, cudaGetLastError());
             ++passes;
-            g->launches += rc.n_obs_run > 0 ? 2 : 1;
+            g->launches += rc.n_obs_run > 0 ? 7 : 1;
             CUDA_TRY(g, cudaMemcpyAsync(g->h_ctrl, ctrl, sizeof(PassCtrl), cudaMemcpyDeviceToHost, s));
             CUDA_TRY(g, cudaStreamSynchronize(s));
             {
-                float a = 0.f, b = 0.f;
+                float a = 0.f, b = 0.f, c = 0.f;
                 CUDA_TRY(g, cudaEventElapsedTime(&a, g->tev[0], g->tev[1]));
                 CUDA_TRY(g, cudaEventElapsedTime(&b, g->tev[1], g->tev[2]));
-                g->ms_transport += a; g->ms_peel += b;
+                CUDA_TRY(g, cudaEventElapsedTime(&c, g->tev[2], g->tev[3]));
+                g->ms_transport += a; g->ms_sort += b; g->ms_peel += c;
             }
             const bool done = g->h_ctrl->work_counter >= total_items && g->h_ctrl->susp_count[nxt] == 0;
             if (done) break;
@@ -468,7 +513,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         hc.packets_escaped = dc.escaped; hc.packets_absorbed = dc.absorbed; hc.packets_surface = dc.surface;
         hc.packets_stuck = dc.stuck; hc.escaped_weight = dc.escaped_weight; hc.passes = passes; hc.rays_peel = dc.rays_peel;
         hc.launches = g->launches; hc.ms_stage = g->ms_stage; hc.ms_emission_cdf = g->ms_emis;
-        hc.ms_transport = g->ms_transport; hc.ms_peel = g->ms_peel;
+        hc.ms_transport = g->ms_transport; hc.ms_peel = g->ms_peel; hc.ms_sort = g->ms_sort;
         if (is_device_ptr(out->counters)) CUDA_TRY(g, cudaMemcpyAsync(out->counters, &hc, sizeof hc, cudaMemcpyHostToDevice, s));
         else *out->counters = hc;
         need_sync = true;
@@ -621,7 +666,7 @@ int gcmcrt_destroy(gcmcrt_grid* g)
     cudaGetLastError();
     for (DevBuf* b : {&g->tab, &g->r64, &g->cth64, &g->ph64, &g->rc32, &g->thc32, &g->phc32, &g->T, &g->rho, &g->u, &g->v,
                       &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->prop, &g->reff, &g->vlos,
-                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->ev1, &g->ev2, &g->s0[0], &g->s0[1],
+                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->ev1, &g->ev2, &g->perm, &g->hist, &g->tile_sums, &g->s0[0], &g->s0[1],
                       &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->flux, &g->ltot_out,
                       &g->value, &g->sigma, &g->image, &g->evcount})
         b->release();

@@ -3,6 +3,7 @@
 // shared-memory flux bins (A7, A9) and the normalisation (A10).  See DESIGN.md for the data layout.
 #pragma once
 #include "ray.cuh"
+#include "sort.cuh"
 
 namespace gcmcrt {
 
@@ -72,6 +73,12 @@ struct RunConst {
     DevCounters* counters;
     unsigned long long* work_counter;   // next fresh packet item
     unsigned long long* ray_counter;    // next peel ray of this pass
+    // exact-division constants floor(2^64 / d) for d = N, n_pkt, n_obs_run (device_common.cuh div_magic)
+    unsigned long long magic_N, magic_npkt, magic_nobs;
+    // warp scheduling thresholds (lanes waiting before the warp leaves the radial march to serve them)
+    int t_service;   // transport: finished / idle / event lanes
+    int t_lateral;   // both kernels: lanes parked at a cone or half-plane
+    int p_refill;    // peel: finished / idle lanes
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -269,7 +276,14 @@ __device__ __forceinline__ void rotate_dir(float& nx, float& ny, float& nz, floa
 // ---------------------------------------------------------------------------------------------------------
 // Transport kernel: persistent threads, one packet per lane, warp-level refill.
 // ---------------------------------------------------------------------------------------------------------
-enum LaneState : int { LS_IDLE = 0, LS_FLY = 1, LS_EV_MEDIUM = 2, LS_EV_EMIT = 3, LS_EV_SURFACE = 4, LS_DONE = 5 };
+// Lane states of the transport kernel.  The warp is a small scheduler: lanes in LS_FLY run the radial march; lanes
+// that need anything else wait in their state until enough of them have gathered for the warp to serve that state
+// with most lanes active (or until no lane can march any more).
+enum LaneState : int {
+    LS_IDLE = 0, LS_FLY = 1, LS_EV_MEDIUM = 2, LS_EV_EMIT = 3, LS_EV_SURFACE = 4, LS_DONE = 5,
+    LS_PARK = 6,                                         // at a cone / half-plane: ray_lateral() pending
+    LS_END_ESC = 7, LS_END_SURF = 8, LS_END_STUCK = 9    // flight over: bookkeeping pending
+};
 
 struct Packet {
     Ray ray;
@@ -280,7 +294,7 @@ struct Packet {
 
 __device__ __forceinline__ uint32_t batch_of(const RunConst& rc, uint32_t pkt)
 {
-    return uint32_t(((unsigned long long)pkt * (unsigned long long)rc.n_batches) / rc.N);
+    return uint32_t(div_magic((unsigned long long)pkt * (unsigned long long)rc.n_batches, rc.N, rc.magic_N));
 }
 
 __device__ __forceinline__ void finish_packet(const RunConst& rc, const Packet& pk)
@@ -288,7 +302,7 @@ __device__ __forceinline__ void finish_packet(const RunConst& rc, const Packet& 
     if (rc.event_count) rc.event_count[(size_t)pk.chan_run * rc.n_pkt + (pk.pkt - rc.pkt_begin)] = pk.nev;
 }
 
-template <int THRESH, int KSTEPS>
+template <int KSTEPS>
 __global__ void __launch_bounds__(kTransportThreads, 2)
 transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const SuspBuf susp_in, const SuspBuf susp_out,
                  const unsigned long long total_items)
@@ -303,6 +317,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
     int st = LS_IDLE;
     const float* alpha_c = rc.alpha;  // table of this lane's channel
     unsigned long long c_events = 0, c_seg = 0, c_esc = 0, c_abs = 0, c_surf = 0, c_stuck = 0;
+    unsigned int c_seg32 = 0;
     double c_escw = 0.0;
     const bool record = rc.n_obs_run > 0;
     bool fresh_left = true;   // warp-uniform: fresh packets may still be available
@@ -311,14 +326,29 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
 
     for (;;) {
         const unsigned m_fly = __ballot_sync(kFullMask, st == LS_FLY);
+        const unsigned m_park = __ballot_sync(kFullMask, st == LS_PARK);
         const unsigned m_ev = __ballot_sync(kFullMask, st >= LS_EV_MEDIUM && st <= LS_EV_SURFACE);
+        const unsigned m_end = __ballot_sync(kFullMask, st >= LS_END_ESC);
         unsigned m_idle = __ballot_sync(kFullMask, st == LS_IDLE);
         if (!(fresh_left || susp_left)) {  // nothing to fetch any more: idle lanes are done
             if (st == LS_IDLE) st = LS_DONE;
             m_idle = 0;
         }
-        const int n_service = __popc(m_ev | m_idle);
-        if (n_service >= THRESH || (m_fly == 0 && n_service > 0)) {
+        const bool starving = m_fly == 0;
+        const int n_service = __popc(m_ev | m_idle | m_end);
+        if (n_service >= rc.t_service || (starving && n_service > 0)) {
+            c_seg += c_seg32; c_seg32 = 0;
+            // ---------------- flights that ended: bookkeeping, then the lane is free ----------------
+            if (m_end) {
+                if (st >= LS_END_ESC) {
+                    if (st == LS_END_ESC) { ++c_esc; c_escw += double(pk.W); }
+                    else if (st == LS_END_SURF) ++c_surf;
+                    else ++c_stuck;
+                    finish_packet(rc, pk);
+                    st = (fresh_left || susp_left) ? LS_IDLE : LS_DONE;
+                }
+                m_idle = __ballot_sync(kFullMask, st == LS_IDLE);
+            }
             // ---------------- fetch: resume suspended packets first, then fresh ones ----------------
             if (m_idle) {
                 bool need = (st == LS_IDLE);
@@ -357,7 +387,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                             const unsigned long long item = base + rank_in_mask(m);
                             if (base + __popc(m) >= total_items) fresh_left = false;
                             if (need && item < total_items) {
-                                pk.chan_run = uint32_t(item / rc.n_pkt);
+                                pk.chan_run = uint32_t(div_magic(item, rc.n_pkt, rc.magic_npkt));
                                 pk.pkt = rc.pkt_begin + uint32_t(item - (unsigned long long)pk.chan_run * rc.n_pkt);
                                 pk.m_inter = 0; pk.nev = 0;
                                 const int ctab = rc.chan_begin + int(pk.chan_run);
@@ -532,33 +562,40 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                 }
             }
         }
+        // ---------------- lateral crossings: cone / half-plane root updates, batched across the warp ----------------
+        if (m_park && (__popc(m_park) >= rc.t_lateral || starving)) {
+            if (st == LS_PARK) {
+                ray_lateral(pk.ray, gs, alpha_c);
+                st = LS_FLY;
+            }
+        }
         if (__ballot_sync(kFullMask, st == LS_FLY) == 0) {
             if (__ballot_sync(kFullMask, st != LS_DONE) == 0) break;
             continue;
         }
-        // ---------------- march: up to KSTEPS cell crossings per lane ----------------
-#pragma unroll 1
+        // ---------------- march: up to KSTEPS radial cell crossings per lane ----------------
+#pragma unroll
         for (int s = 0; s < KSTEPS; ++s) {
             if (st == LS_FLY) {
                 const int rs = ray_step(pk.ray, gs, pk.tau, pk.tau_t, alpha_c);
-                ++c_seg;
-                if (rs != RAY_FLYING) {
-                    if (rs == RAY_LIMIT) {
-                        st = LS_EV_MEDIUM;
-                    } else if (rs == RAY_ESCAPE) {
-                        ++c_esc; c_escw += double(pk.W); st = LS_IDLE; finish_packet(rc, pk);
-                    } else {  // RAY_SURFACE
-                        if (rc.surface_albedo > 0.f) st = LS_EV_SURFACE;
-                        else { ++c_surf; st = LS_IDLE; finish_packet(rc, pk); }
-                    }
-                } else if (++pk.fl_seg > rc.geom.maxseg) {
-                    ++c_stuck; st = LS_IDLE; finish_packet(rc, pk);
+                ++c_seg32;
+                if (rs == RAY_FLYING) {
+                    if (++pk.fl_seg > rc.geom.maxseg) st = LS_END_STUCK;
+                } else if (rs == RAY_PARK) {
+                    st = (++pk.fl_seg > rc.geom.maxseg) ? LS_END_STUCK : LS_PARK;
+                } else if (rs == RAY_LIMIT) {
+                    st = LS_EV_MEDIUM;
+                } else if (rs == RAY_ESCAPE) {
+                    st = LS_END_ESC;
+                } else {  // RAY_SURFACE
+                    st = rc.surface_albedo > 0.f ? LS_EV_SURFACE : LS_END_SURF;
                 }
             }
         }
     }
 
     // counters: warp reduce, one atomic per warp
+    c_seg += c_seg32;
     c_events = warp_sum_u64(c_events); c_seg = warp_sum_u64(c_seg); c_esc = warp_sum_u64(c_esc);
     c_abs = warp_sum_u64(c_abs); c_surf = warp_sum_u64(c_surf); c_stuck = warp_sum_u64(c_stuck);
     c_escw = warp_sum_f64(c_escw);
@@ -574,13 +611,32 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Peel-off kernel (A7 + A9): one ray per (event, observer); persistent lanes with warp-level refill;
-// f = pref * Theta * exp(-tau_obs) (Eq. 14) accumulated in warp-private shared-memory bins [obs][batch] of the
-// warp's current channel, flushed to the fp64 global sums when the channel changes and at the end.
+// Peel-off kernel (A7 + A9).  Events arrive sorted by (channel, cell) (sort.cuh): a warp takes 32 consecutive
+// events, one per lane, and integrates their rays toward one observer at a time -- 32 parallel rays that start in
+// the same or neighbouring cells, so the lanes read the same extinction sectors, cross the same shells in the same
+// step and finish within a few steps of each other.  Cone / half-plane crossings are batched across the warp
+// (ray_lateral).  f = pref * Theta * exp(-tau_obs) (Eq. 14) goes to warp-private shared-memory bins [obs][batch]
+// of the warp's current channel, flushed to the fp64 global sums when the channel changes and at the end.
 // ---------------------------------------------------------------------------------------------------------
-template <int THRESH, int KSTEPS>
+enum PeelState : int { PS_IDLE = 0, PS_FLY = 1, PS_PARK = 2, PS_ESCAPED = 3 };
+
+__device__ __forceinline__ void peel_flush_bins(const RunConst& rc, float* bins, int nbins, int warp_chan)
+{
+    for (int t = lane_id(); t < nbins; t += 32) {
+        const float v = bins[t];
+        if (v != 0.f) {
+            const int o = t / rc.n_batches, bt = t - o * rc.n_batches;
+            atomicAdd(rc.flux + ((size_t)warp_chan * rc.n_obs_total + rc.obs_first + o) * rc.n_batches + bt, double(v));
+            bins[t] = 0.f;
+        }
+    }
+}
+
+constexpr int kPeelChunk = 128;   // consecutive sorted events a warp takes per atomic (4 rounds of 32)
+
+template <int KSTEPS>
 __global__ void __launch_bounds__(kPeelThreads, 2)
-peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev)
+peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsigned int* __restrict__ perm)
 {
     extern __shared__ float smem_f[];
     const GeomSmem gs = load_geom(rc.geom, smem_f);
@@ -590,35 +646,46 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev)
     __syncthreads();
 
     const unsigned int n_events = min(*ev.count, ev.cap);
-    const unsigned long long n_rays = (unsigned long long)n_events * rc.n_obs_run;
     int warp_chan = -1;  // channel (run-local) the warp's bins belong to
-
-    Ray ray{};
-    float tau = 0.f, pref = 0.f;
-    uint32_t meta = 0;
-    int obs = 0, fl_seg = 0;
-    bool fly = false;
-    bool work_left = n_rays > 0;
     unsigned long long c_seg = 0, c_rays = 0;
-    float ipx = 0.f, ipy = 0.f, ipz = 0.f;
 
     for (;;) {
-        const unsigned m_idle = __ballot_sync(kFullMask, !fly);
-        if (work_left && (__popc(m_idle) >= THRESH)) {
-            unsigned long long base = 0;
-            if (lane_id() == __ffs(m_idle) - 1) base = atomicAdd(rc.ray_counter, (unsigned long long)__popc(m_idle));
-            base = __shfl_sync(kFullMask, base, __ffs(m_idle) - 1);
-            const unsigned long long rid = base + rank_in_mask(m_idle);
-            if (base + __popc(m_idle) >= n_rays) work_left = false;
-            int new_chan = -1;
-            if (!fly && rid < n_rays) {
-                const unsigned int e = (unsigned int)(rid / rc.n_obs_run);
-                obs = int(rid - (unsigned long long)e * rc.n_obs_run);
-                const float4 a = __ldg(ev.e0 + e), b = __ldg(ev.e1 + e), c = __ldg(ev.e2 + e);
-                meta = __float_as_uint(c.z);
-                const uint32_t kind = meta & 3u;
+        unsigned long long base = 0;
+        if (lane_id() == 0) base = atomicAdd(rc.ray_counter, (unsigned long long)kPeelChunk);
+        base = __shfl_sync(kFullMask, base, 0);
+        if (base >= n_events) break;
+        const unsigned int chunk_end = (unsigned int)min((unsigned long long)n_events, base + kPeelChunk);
+        for (unsigned int r0 = (unsigned int)base; r0 < chunk_end; r0 += 32) {
+            const unsigned int rank = r0 + lane_id();
+            const bool have = rank < chunk_end;
+            float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a;
+            if (have) {
+                const unsigned int e = __ldg(perm + rank);
+                a = __ldg(ev.e0 + e); b = __ldg(ev.e1 + e); c = __ldg(ev.e2 + e);
+            }
+            const uint32_t meta = __float_as_uint(c.z);
+            const uint32_t kind = meta & 3u;
+            const int chan = have ? int(meta >> 8) : -1;
+            const int bt = int((meta >> 2) & 63u);
+            int ci, cj, ck;
+            unpack_cell(__float_as_uint(c.y), ci, cj, ck);
+            const float* alpha_c = rc.alpha + (size_t)(rc.chan_begin + max(chan, 0)) * rc.geom.ncell;
+            // the warp's bins follow the newest channel; stragglers of older channels go straight to global memory
+            int mx = chan;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(kFullMask, mx, o));
+            if (mx > warp_chan) {
+                if (warp_chan >= 0) {
+                    __syncwarp();
+                    peel_flush_bins(rc, bins, nbins, warp_chan);
+                    __syncwarp();
+                }
+                warp_chan = mx;
+            }
+            for (int obs = 0; obs < rc.n_obs_run; ++obs) {
                 const float* od = rc.obs[rc.obs_first + obs];
-                const float mu = b.x * od[0] + b.y * od[1] + b.z * od[2];
+                const float ox = od[0], oy = od[1], oz = od[2];
+                const float mu = b.x * ox + b.y * oy + b.z * oz;
                 float theta;
                 if (kind == EV_MEDIUM) {  // C6: mixture phase function, per steradian (Eq. 5, Eq. 7)
                     const float g = c.x;
@@ -631,83 +698,65 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev)
                 } else {
                     theta = fmaxf(mu, 0.0f) / kPi;
                 }
-                pref = a.w * theta;
-                new_chan = int(meta >> 8);
-                if (pref > 0.0f) {
-                    int i, j, k;
-                    unpack_cell(__float_as_uint(c.y), i, j, k);
-                    const float* alpha_c = rc.alpha + (size_t)(rc.chan_begin + new_chan) * rc.geom.ncell;
-                    ray_init(ray, gs, a.x, a.y, a.z, od[0], od[1], od[2], i, j, k, alpha_c);
-                    ipx = a.x; ipy = a.y; ipz = a.z;
-                    tau = 0.f; fl_seg = 0;
-                    fly = true;
+                const float pref = a.w * theta;
+                Ray ray{};
+                float tau = 0.f;
+                int fl_seg = 0;
+                int st = PS_IDLE;
+                unsigned int seg32 = 0;
+                if (have && pref > 0.0f) {
+                    ray_init(ray, gs, a.x, a.y, a.z, ox, oy, oz, ci, cj, ck, alpha_c);
+                    st = PS_FLY;
                     ++c_rays;
                 }
-            }
-            // the warp's bins follow the newest channel; stragglers of older channels go straight to global memory
-            int mx = new_chan;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(kFullMask, mx, o));
-            if (mx > warp_chan) {
-                if (warp_chan >= 0) {
-                    __syncwarp();
-                    for (int t = lane_id(); t < nbins; t += 32) {
-                        const float v = bins[t];
-                        if (v != 0.f) {
-                            const int o = t / rc.n_batches, bt = t - o * rc.n_batches;
-                            atomicAdd(rc.flux + ((size_t)warp_chan * rc.n_obs_total + rc.obs_first + o) * rc.n_batches + bt,
-                                      double(v));
-                            bins[t] = 0.f;
+                for (;;) {
+                    const unsigned m_fly = __ballot_sync(kFullMask, st == PS_FLY);
+                    const unsigned m_park = __ballot_sync(kFullMask, st == PS_PARK);
+                    if ((m_fly | m_park) == 0) break;
+                    if (m_park && (__popc(m_park) >= rc.t_lateral || m_fly == 0)) {
+                        if (st == PS_PARK) {
+                            ray_lateral(ray, gs, alpha_c);
+                            st = PS_FLY;
                         }
                     }
-                    __syncwarp();
+#pragma unroll
+                    for (int s = 0; s < KSTEPS; ++s) {
+                        if (st == PS_FLY) {
+                            const int rs = ray_step(ray, gs, tau, rc.tau_cut, alpha_c);
+                            ++seg32;
+                            if (rs == RAY_FLYING) {
+                                if (++fl_seg > rc.geom.maxseg) st = PS_IDLE;
+                            } else if (rs == RAY_PARK) {
+                                st = (++fl_seg > rc.geom.maxseg) ? PS_IDLE : PS_PARK;
+                            } else if (rs == RAY_ESCAPE) {
+                                st = PS_ESCAPED;
+                            } else {
+                                st = PS_IDLE;   // surface hit or tau_obs > tau_cut: nothing reaches the observer
+                            }
+                        }
+                    }
                 }
-                warp_chan = mx;
-            }
-        }
-        if (__ballot_sync(kFullMask, fly) == 0) {
-            if (!work_left) break;
-            continue;
-        }
-#pragma unroll 1
-        for (int s = 0; s < KSTEPS; ++s) {
-            if (fly) {
-                const int chan = int(meta >> 8);
-                const float* alpha_c = rc.alpha + (size_t)(rc.chan_begin + chan) * rc.geom.ncell;
-                const int rs = ray_step(ray, gs, tau, rc.tau_cut, alpha_c);
-                ++c_seg;
-                if (rs == RAY_ESCAPE) {
+                c_seg += seg32;
+                // ---------------- rays that reached the top of the atmosphere: Eq. 14 ----------------
+                if (st == PS_ESCAPED) {
                     const float f = pref * expf(-tau);
-                    const int bt = int((meta >> 2) & 63u);
                     if (chan == warp_chan) atomicAdd(bins + obs * rc.n_batches + bt, f);
                     else atomicAdd(rc.flux + ((size_t)chan * rc.n_obs_total + rc.obs_first + obs) * rc.n_batches + bt, double(f));
                     if (rc.image) {
                         const int o = rc.obs_first + obs;
-                        const float X = ipx * rc.img_ex[o][0] + ipy * rc.img_ex[o][1] + ipz * rc.img_ex[o][2];
-                        const float Y = ipx * rc.img_ey[o][0] + ipy * rc.img_ey[o][1] + ipz * rc.img_ey[o][2];
+                        const float X = a.x * rc.img_ex[o][0] + a.y * rc.img_ex[o][1] + a.z * rc.img_ex[o][2];
+                        const float Y = a.x * rc.img_ey[o][0] + a.y * rc.img_ey[o][1] + a.z * rc.img_ey[o][2];
                         const int ix = min(max(int(floorf((X / rc.geom.Rtoa + 1.0f) * 0.5f * rc.npix)), 0), rc.npix - 1);
                         const int iy = min(max(int(floorf((Y / rc.geom.Rtoa + 1.0f) * 0.5f * rc.npix)), 0), rc.npix - 1);
                         atomicAdd(rc.image + ((size_t)chan * rc.n_obs_total + o) * rc.npix * rc.npix + iy * rc.npix + ix, f);
                     }
-                    fly = false;
-                } else if (rs != RAY_FLYING) {
-                    fly = false;   // surface hit or tau_obs > tau_cut: nothing reaches the observer
-                } else if (++fl_seg > rc.geom.maxseg) {
-                    fly = false;
                 }
+                __syncwarp();
             }
         }
     }
     __syncwarp();
-    if (warp_chan >= 0) {
-        for (int t = lane_id(); t < nbins; t += 32) {
-            const float v = bins[t];
-            if (v != 0.f) {
-                const int o = t / rc.n_batches, bt = t - o * rc.n_batches;
-                atomicAdd(rc.flux + ((size_t)warp_chan * rc.n_obs_total + rc.obs_first + o) * rc.n_batches + bt, double(v));
-            }
-        }
-    }
+    if (warp_chan >= 0) peel_flush_bins(rc, bins, nbins, warp_chan);
     c_seg = warp_sum_u64(c_seg); c_rays = warp_sum_u64(c_rays);
     if (lane_id() == 0) {
         if (c_seg) atomicAdd(&rc.counters->seg_peel, c_seg);
@@ -769,7 +818,10 @@ __global__ void __launch_bounds__(128) debug_ray_tau_kernel(const GeomParams g, 
     ray_init(ray, gs, px, py, pz, dir[3 * m], dir[3 * m + 1], dir[3 * m + 2], i, j, k, alpha_c);
     float tau = 0.f;
     int rs = RAY_FLYING, nseg = 0;
-    while (rs == RAY_FLYING && nseg++ <= g.maxseg) rs = ray_step(ray, gs, tau, kInf, alpha_c);
+    while (rs == RAY_FLYING && nseg++ <= g.maxseg) {
+        rs = ray_step(ray, gs, tau, kInf, alpha_c);
+        if (rs == RAY_PARK) { ray_lateral(ray, gs, alpha_c); rs = RAY_FLYING; }
+    }
     tau_out[m] = tau;
     if (hit) hit[m] = rs == RAY_SURFACE ? 1 : (rs == RAY_ESCAPE ? 0 : -1);
 }

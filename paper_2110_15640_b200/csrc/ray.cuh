@@ -47,7 +47,7 @@ __device__ __forceinline__ GeomSmem load_geom(const GeomParams& g, float* smem)
     return s;
 }
 
-enum RayStatus : int { RAY_FLYING = 0, RAY_LIMIT = 1, RAY_ESCAPE = 2, RAY_SURFACE = 3, RAY_STUCK = 4 };
+enum RayStatus : int { RAY_FLYING = 0, RAY_LIMIT = 1, RAY_ESCAPE = 2, RAY_SURFACE = 3, RAY_STUCK = 4, RAY_PARK = 5 };
 
 struct Ray {
     float pcx, pcy, pcz;  // closest-approach point
@@ -57,6 +57,7 @@ struct Ray {
     float u;              // signed distance from the closest-approach point
     float u_rad, u_lat, u_lon;  // next crossing of each face family
     float alpha;          // extinction of the current cell
+    float alpha_n;        // prefetched extinction of the radial neighbour (i + rad_step) in the same column
     int i, j, k;          // cell
     int col;              // (k*nlat + j)*nlev
     int rad_step, lat_step, lon_step;
@@ -133,6 +134,20 @@ __device__ __forceinline__ void ray_setup_lon(Ray& r, const GeomSmem& s)
     r.lon_step = step;
 }
 
+// Extinction of the current cell and, one step ahead, of the radial neighbour the ray will enter next: the march
+// loop consumes alpha one iteration after the load was issued, so the gather latency overlaps a full step.
+__device__ __forceinline__ void ray_load_alpha(Ray& r, const GeomSmem& s, const float* __restrict__ alpha_tab)
+{
+    const float* colp = alpha_tab + r.col;
+    r.alpha = __ldg(colp + r.i);
+    r.alpha_n = __ldg(colp + min(max(r.i + r.rad_step, 0), s.nlev - 1));
+#ifdef GCMCRT_PREFETCH
+    // the column is new to this lane: pull the next sectors along the radial direction into L1 ahead of the march
+    prefetch_l1(colp + min(max(r.i + 8 * r.rad_step, 0), s.nlev - 1));
+    prefetch_l1(colp + min(max(r.i + 16 * r.rad_step, 0), s.nlev - 1));
+#endif
+}
+
 // Start a ray at p with unit direction n inside cell (i,j,k).
 __device__ __forceinline__ void ray_init(Ray& r, const GeomSmem& s, float px, float py, float pz, float nx, float ny,
                                          float nz, int i, int j, int k, const float* __restrict__ alpha_tab)
@@ -156,14 +171,19 @@ __device__ __forceinline__ void ray_init(Ray& r, const GeomSmem& s, float px, fl
     ray_setup_rad(r, s);
     ray_setup_lat(r, s);
     ray_setup_lon(r, s);
-    r.alpha = __ldg(alpha_tab + r.col + i);
+    ray_load_alpha(r, s, alpha_tab);
 }
 
-// One cell crossing.  tau accumulates; returns RAY_FLYING, or why the ray stopped.
+// One step of the march, radial fast path.  tau accumulates over the segment up to the next face.  A shell crossing
+// is completed here (index, next shell root, alpha rotation + prefetch) and returns RAY_FLYING; when the next face
+// is a cone or a half-plane the ray is advanced to it and RAY_PARK is returned: the caller completes the crossing
+// with ray_lateral(), which the kernels batch across the warp so that the rarely taken, expensive cone / plane
+// root updates do not serialise against the radial path of the other lanes.
 __device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, float tau_limit,
                                         const float* __restrict__ alpha_tab)
 {
-    const float un = fminf(r.u_rad, fminf(r.u_lat, r.u_lon));
+    const float ul = fminf(r.u_lat, r.u_lon);
+    const float un = fminf(r.u_rad, ul);
     const float ds = fmaxf(un - r.u, 0.0f);
     const float dtau = r.alpha * ds;
     if (tau + dtau >= tau_limit) {  // the limit is reached inside this cell
@@ -173,12 +193,22 @@ __device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, f
     }
     tau += dtau;
     r.u = fmaxf(un, r.u);
-    if (un == r.u_rad) {  // ties: shells first (C1)
+    if (r.u_rad <= ul) {  // ties: shells first (C1)
         r.i += r.rad_step;
         if (r.i >= s.nlev) { r.i = s.nlev - 1; return RAY_ESCAPE; }
         if (r.i < 0) { r.i = 0; return RAY_SURFACE; }
-        ray_setup_rad(r, s);
-    } else if (un == r.u_lat) {
+        r.alpha = r.alpha_n;   // prefetched for exactly this cell
+        ray_setup_rad(r, s);   // may turn the ray from inward to outward
+        r.alpha_n = __ldg(alpha_tab + r.col + min(max(r.i + r.rad_step, 0), s.nlev - 1));
+        return RAY_FLYING;
+    }
+    return RAY_PARK;
+}
+
+// Completes the cone / half-plane crossing of a parked ray (ties: cones before planes, C1).
+__device__ __forceinline__ void ray_lateral(Ray& r, const GeomSmem& s, const float* __restrict__ alpha_tab)
+{
+    if (r.u_lat <= r.u_lon) {
         r.j = min(max(r.j + r.lat_step, 0), s.nlat - 1);
         r.col = (r.k * s.nlat + r.j) * s.nlev;
         ray_setup_lat(r, s);
@@ -188,8 +218,7 @@ __device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, f
         r.col = (r.k * s.nlat + r.j) * s.nlev;
         ray_setup_lon(r, s);
     }
-    r.alpha = __ldg(alpha_tab + r.col + r.i);
-    return RAY_FLYING;
+    ray_load_alpha(r, s, alpha_tab);
 }
 
 __device__ __forceinline__ void ray_position(const Ray& r, float& px, float& py, float& pz)

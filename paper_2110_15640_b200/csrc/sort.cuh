@@ -1,0 +1,151 @@
+// sort.cuh -- counting sort of one pass of event records by (channel, cell), between the transport kernel and the
+// peel-off kernel.  Peel-off rays of one observer are parallel, so events that start in the same cell of the same
+// channel march through the same columns of the same extinction table for nearly the same number of segments:
+// handing the peel kernel its events in (channel, cell) order turns 32 unrelated gathers per warp-load into one or
+// two sectors and makes the lanes of a warp finish together.  Only a permutation is built (4 B per event); the
+// 48 B records stay where the transport kernel wrote them.
+//
+//   key(e) = (chan_run(e) mod c_fold) * ncell + (k * nlat + j) * nlev + i        (cell-flat layout, i fastest)
+//   ev_hist_kernel    hist[key]++                                  (global atomics)
+//   scan_*            exclusive prefix sum of hist in place        (tile reduce, scan of tile sums, tile scan)
+//   ev_scatter_kernel perm[hist[key]++] = e
+//
+// c_fold bounds the histogram (<= 2^25 bins); channels that fold onto each other only lose locality.
+#pragma once
+#include "device_common.cuh"
+
+namespace gcmcrt {
+
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 16;                       // per thread
+constexpr int kScanTile = kScanThreads * kScanItems;  // 4096 bins per CTA
+
+struct SortParams {
+    const float4* e2;            // event records, third float4: g cell meta pkt
+    const unsigned int* count;   // events written this pass (device)
+    unsigned int cap;
+    unsigned int* hist;          // [nbins]
+    unsigned int* tile_sums;     // [n_tiles]
+    unsigned int* perm;          // [cap]
+    unsigned int nbins, n_tiles;
+    int nlev, nlat, ncell, c_fold;
+};
+
+__device__ __forceinline__ unsigned int event_sort_key(const SortParams& p, const float4 c)
+{
+    const uint32_t cell = __float_as_uint(c.y), meta = __float_as_uint(c.z);
+    const int i = cell & 1023, j = (cell >> 10) & 1023, k = cell >> 20;
+    const unsigned int chan = (meta >> 8) % (unsigned int)p.c_fold;
+    return chan * (unsigned int)p.ncell + (unsigned int)((k * p.nlat + j) * p.nlev + i);
+}
+
+__global__ void __launch_bounds__(256) ev_hist_kernel(const SortParams p)
+{
+    const unsigned int n = min(*p.count, p.cap);
+    for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x)
+        atomicAdd(p.hist + event_sort_key(p, __ldg(p.e2 + e)), 1u);
+}
+
+__global__ void __launch_bounds__(256) ev_scatter_kernel(const SortParams p)
+{
+    const unsigned int n = min(*p.count, p.cap);
+    for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x)
+        p.perm[atomicAdd(p.hist + event_sort_key(p, __ldg(p.e2 + e)), 1u)] = e;
+}
+
+__device__ __forceinline__ unsigned int block_sum_u32(unsigned int v, unsigned int* warp_part)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFullMask, v, o);
+    if (lane_id() == 0) warp_part[threadIdx.x >> 5] = v;
+    __syncthreads();
+    unsigned int t = 0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += warp_part[w];
+    __syncthreads();
+    return t;
+}
+
+// tile_sums[b] = sum of hist over tile b
+__global__ void __launch_bounds__(kScanThreads) scan_reduce_kernel(const SortParams p)
+{
+    __shared__ unsigned int warp_part[kScanThreads / 32];
+    const unsigned int base = blockIdx.x * kScanTile;
+    unsigned int s = 0;
+#pragma unroll
+    for (int m = 0; m < kScanItems; ++m) {
+        const unsigned int idx = base + m * kScanThreads + threadIdx.x;
+        if (idx < p.nbins) s += p.hist[idx];
+    }
+    s = block_sum_u32(s, warp_part);
+    if (threadIdx.x == 0) p.tile_sums[blockIdx.x] = s;
+}
+
+// exclusive scan of tile_sums in place, one CTA
+__global__ void __launch_bounds__(1024) scan_tiles_kernel(const SortParams p)
+{
+    __shared__ unsigned int warp_tot[32];
+    __shared__ unsigned int carry_s;
+    const int lane = lane_id(), wid = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (unsigned int base = 0; base < p.n_tiles; base += blockDim.x) {
+        const unsigned int idx = base + threadIdx.x;
+        const unsigned int x = idx < p.n_tiles ? p.tile_sums[idx] : 0u;
+        unsigned int v = x;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned int n = __shfl_up_sync(kFullMask, v, o);
+            if (lane >= o) v += n;
+        }
+        if (lane == 31) warp_tot[wid] = v;
+        __syncthreads();
+        if (wid == 0) {
+            unsigned int w = warp_tot[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const unsigned int n = __shfl_up_sync(kFullMask, w, o);
+                if (lane >= o) w += n;
+            }
+            warp_tot[lane] = w;
+        }
+        __syncthreads();
+        const unsigned int carry = carry_s;
+        const unsigned int incl = carry + (wid > 0 ? warp_tot[wid - 1] : 0u) + v;
+        if (idx < p.n_tiles) p.tile_sums[idx] = incl - x;
+        __syncthreads();
+        if (threadIdx.x == blockDim.x - 1) carry_s = incl;
+        __syncthreads();
+    }
+}
+
+// hist[idx] = tile offset + exclusive scan within the tile (each thread owns kScanItems consecutive bins)
+__global__ void __launch_bounds__(kScanThreads) scan_apply_kernel(const SortParams p)
+{
+    __shared__ unsigned int warp_tot[kScanThreads / 32];
+    const unsigned int base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
+    unsigned int x[kScanItems];
+    unsigned int s = 0;
+#pragma unroll
+    for (int m = 0; m < kScanItems; ++m) {
+        x[m] = (base + m < p.nbins) ? p.hist[base + m] : 0u;
+        s += x[m];
+    }
+    const int lane = lane_id(), wid = threadIdx.x >> 5;
+    unsigned int v = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int n = __shfl_up_sync(kFullMask, v, o);
+        if (lane >= o) v += n;
+    }
+    if (lane == 31) warp_tot[wid] = v;
+    __syncthreads();
+    unsigned int off = p.tile_sums[blockIdx.x] + (v - s);
+    for (int w = 0; w < wid; ++w) off += warp_tot[w];
+#pragma unroll
+    for (int m = 0; m < kScanItems; ++m) {
+        if (base + m < p.nbins) p.hist[base + m] = off;
+        off += x[m];
+    }
+}
+
+}  // namespace gcmcrt

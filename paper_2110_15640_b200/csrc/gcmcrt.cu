@@ -137,6 +137,8 @@ GeomParams geom_params(const gcmcrt_grid* g)
     gp.Rtoa = float(g->r[g->nlev]);
     gp.R0 = float(g->r[0]);
     gp.maxseg = 8 * (g->nlev + g->nlat + g->nlon) + 64;
+    gp.col_stride = alpha_col_stride(g->nlev);
+    gp.alpha_stride = (long long)g->nlat * g->nlon * gp.col_stride;
     return gp;
 }
 
@@ -174,13 +176,17 @@ cudaError_t ensure_events(gcmcrt_grid* g)
 int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStream_t s)
 {
     const size_t n = size_t(g->n_chan) * g->ncell;
-    CUDA_TRY(g, g->alpha.ensure(n * sizeof(float)));
+    const GeomParams gp0 = geom_params(g);
+    const size_t n_alpha = size_t(g->n_chan) * size_t(gp0.alpha_stride);
+    CUDA_TRY(g, g->alpha.ensure(n_alpha * sizeof(float)));
+    CUDA_TRY(g, cudaMemsetAsync(g->alpha.p, 0, n_alpha * sizeof(float), s));   // guard entries and padding
     CUDA_TRY(g, g->prop.ensure(n * sizeof(float4)));
     StageParams sp;
     sp.n_chan = g->n_chan; sp.ncell = g->ncell; sp.nlev = g->nlev; sp.nlat = g->nlat; sp.nlon = g->nlon;
     sp.k_abs = g->k_abs; sp.k_ray = g->k_ray; sp.k_cld = g->k_cld; sp.g_cld = g->g_cld;
     sp.rho = g->rho.as<float>();
     sp.alpha = g->alpha.as<float>(); sp.prop = g->prop.as<float4>();
+    sp.alpha_stride = gp0.alpha_stride; sp.col_stride = gp0.col_stride;
     sp.doppler = obs_dir != nullptr; sp.halfwidth = halfwidth;
     sp.vlos = nullptr; sp.reff = g->reff.as<float>();
     CUDA_TRY(g, ensure_events(g));
@@ -385,6 +391,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             EmisParams ep;
             ep.n_chan = g->n_chan; ep.nlev = g->nlev; ep.nlat = g->nlat; ep.nlon = g->nlon; ep.ncell = g->ncell;
             ep.alpha = rc.alpha; ep.prop = rc.prop;
+            ep.alpha_stride = rc.geom.alpha_stride; ep.col_stride = rc.geom.col_stride;
             ep.rho = g->rho.as<float>(); ep.T = g->T.as<float>();
             ep.lambda = g->lambda64.as<double>();
             ep.r_edges = g->r64.as<double>(); ep.cth_edges = g->cth64.as<double>(); ep.ph_edges = g->ph64.as<double>();
@@ -428,7 +435,10 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         std::memset(&sp, 0, sizeof sp);
         if (rc.n_obs_run > 0) {
             const long long max_bins = 1ll << 25;
-            sp.c_fold = int(std::max<long long>(1, std::min<long long>(ncr, max_bins / g->ncell)));
+            // channels whose events can share one pass: every packet makes at least one event when it interacts,
+            // so a pass of ev_cap events spans about ev_cap / n_pkt channels; more bins than that only cost scan time
+            const long long span = (long long)(g->ev_cap / std::max<size_t>(n_pkt, 1)) + 2;
+            sp.c_fold = int(std::max<long long>(1, std::min<long long>(std::min<long long>(ncr, max_bins / g->ncell), span)));
             sp.nbins = (unsigned int)((long long)sp.c_fold * g->ncell);
             sp.n_tiles = (sp.nbins + kScanTile - 1) / kScanTile;
             CUDA_TRY(g, g->hist.ensure(size_t(sp.nbins) * sizeof(unsigned int)));
@@ -438,6 +448,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             sp.perm = g->perm.as<unsigned int>();
             sp.nlev = g->nlev; sp.nlat = g->nlat; sp.ncell = g->ncell;
         }
+        unsigned long long items_before = 0;   // fresh-packet counter at the start of the pass
         for (;;) {
             const int nxt = 1 - cur;
             SuspBuf sin, sout;
@@ -450,6 +461,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
             if (rc.n_obs_run > 0) {
                 // counting sort of this pass's events by (channel, cell): sort.cuh
+                sp.chan_lo = int(std::min<unsigned long long>(items_before / std::max<size_t>(n_pkt, 1), (unsigned long long)ncr));
                 CUDA_TRY(g, cudaMemsetAsync(sp.hist, 0, size_t(sp.nbins) * sizeof(unsigned int), s));
                 ev_hist_kernel<<<g->sm_count * 8, 256, 0, s>>>(sp);
                 scan_reduce_kernel<<<sp.n_tiles, kScanThreads, 0, s>>>(sp);
@@ -472,6 +484,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
                 CUDA_TRY(g, cudaEventElapsedTime(&c, g->tev[2], g->tev[3]));
                 g->ms_transport += a; g->ms_sort += b; g->ms_peel += c;
             }
+            items_before = std::min<unsigned long long>(g->h_ctrl->work_counter, total_items);
             const bool done = g->h_ctrl->work_counter >= total_items && g->h_ctrl->susp_count[nxt] == 0;
             if (done) break;
             // reset the per-pass counters: events, rays, the list just consumed
@@ -563,11 +576,14 @@ int gcmcrt_grid_create(gcmcrt_grid** out, int nlev, int nlat, int nlon, const do
     g->Omega = Omega; g->surface_albedo = surface_albedo;
     cudaDeviceGetAttribute(&g->sm_count, cudaDevAttrMultiProcessorCount, dev);
 
-    // packed fp32 tables: R, R^2 (high, low parts), qcube, cos(theta_e), cos(phi_e), sin(phi_e), phi_e
+    // packed fp32 tables: R^2 (high, low) pairs, R, qcube, cos(theta_e), cos(phi_e), sin(phi_e), phi_e
     std::vector<float> tab;
+    for (int i = 0; i <= nlev; ++i) {   // R_k^2 as (high, low) pairs: one LDS.64 per shell root
+        const double r2 = g->r[i] * g->r[i];
+        tab.push_back(float(r2));
+        tab.push_back(float(r2 - double(float(r2))));
+    }
     for (int i = 0; i <= nlev; ++i) tab.push_back(float(g->r[i]));
-    for (int i = 0; i <= nlev; ++i) tab.push_back(float(g->r[i] * g->r[i]));
-    for (int i = 0; i <= nlev; ++i) { const double r2 = g->r[i] * g->r[i]; tab.push_back(float(r2 - double(float(r2)))); }
     for (int i = 0; i < nlev; ++i) { const double q = g->r[i + 1] / g->r[i]; tab.push_back(float(q * q * q - 1.0)); }
     std::vector<double> cth(nlat + 1);
     for (int j = 0; j <= nlat; ++j) cth[j] = j == 0 ? 1.0 : (j == nlat ? -1.0 : std::cos(g->th[j]));
@@ -697,7 +713,7 @@ int gcmcrt_debug_ray_tau(gcmcrt_grid* g, int chan, long n, const float* pos, con
         if (e == cudaSuccess) {
             const GeomParams gp = geom_params(g);
             debug_ray_tau_kernel<<<(unsigned)((n + 127) / 128), 128, g->tab_floats * sizeof(float), s>>>(
-                gp, g->alpha.as<float>() + size_t(chan) * g->ncell, n, dp, dd, dt, dh);
+                gp, g->alpha.as<float>() + size_t(chan) * size_t(gp.alpha_stride), n, dp, dd, dt, dh);
             e = cudaGetLastError();
         }
         if (e == cudaSuccess && !tdev) e = cudaMemcpyAsync(tau, dt, n * sizeof(float), cudaMemcpyDeviceToHost, s);

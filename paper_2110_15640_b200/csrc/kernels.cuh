@@ -44,7 +44,7 @@ struct DevCounters {
 
 struct RunConst {
     GeomParams geom;
-    const float* alpha;    // [n_chan_tab][ncell] extinction (m^-1)
+    const float* alpha;    // [n_chan_tab][ncol][col_stride] extinction (m^-1), guard-padded columns (ray.cuh)
     const float4* prop;    // [n_chan_tab][ncell] omega, P_gas, g, k_abs_eff
     const double* Lcum;    // emission: [n_chan_tab][ncell] running luminosity
     const double* Lcell;   // emission, xi > 0 only
@@ -87,7 +87,9 @@ struct RunConst {
 struct StageParams {
     int n_chan, ncell, nlev, nlat, nlon;
     const float *k_abs, *k_ray, *k_cld, *g_cld, *rho;
-    float* alpha;
+    float* alpha;          // [n_chan][ncol][col_stride], zero-filled by the host before the launch (guard entries)
+    long long alpha_stride;
+    int col_stride;
     float4* prop;
     // Doppler (A1): per-cell line-of-sight velocity of this observer, per-channel 1/ln(lambda ratio)
     int doppler, halfwidth;
@@ -143,7 +145,10 @@ __global__ void __launch_bounds__(256) stage_kernel(const StageParams p)
         const float g = p.g_cld ? __ldg(p.g_cld + t) : 0.0f;
         const float ks = kr + kc;
         const float kext = ka + ks;
-        p.alpha[t] = __ldg(p.rho + cell) * kext;
+        {   // guard-padded column layout of the marcher: [chan][col][col_stride], level i at offset 1 + i
+            const int col = cell / p.nlev, i = cell - col * p.nlev;
+            p.alpha[(size_t)c * p.alpha_stride + (size_t)col * p.col_stride + 1 + i] = __ldg(p.rho + cell) * kext;
+        }
         p.prop[t] = make_float4(kext > 0.0f ? ks / kext : 0.0f, ks > 0.0f ? kr / ks : 0.0f, g, ka);
     }
 }
@@ -154,6 +159,8 @@ __global__ void __launch_bounds__(256) stage_kernel(const StageParams p)
 struct EmisParams {
     int n_chan, nlev, nlat, nlon, ncell;
     const float* alpha;
+    long long alpha_stride;
+    int col_stride;
     const float4* prop;
     const float *rho, *T;
     const double* lambda;   // [n_chan]
@@ -190,7 +197,7 @@ __global__ void __launch_bounds__(128) emis_cell_kernel(const EmisParams p)
         double L = 4.0 * 3.14159265358979323846 * vol * double(p.rho[cell]) * double(p.prop[base + i].w) *
                    planck_lambda(lam, double(p.T[cell]));
         if (p.tau_vert_max > 0.0 && tv > p.tau_vert_max) L = 0.0;
-        tv += double(p.alpha[base + i]) * (r1 - r0);
+        tv += double(p.alpha[(size_t)c * p.alpha_stride + (size_t)col * p.col_stride + 1 + i]) * (r1 - r0);
         p.Lcell[base + i] = L;
     }
 }
@@ -367,8 +374,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                         pk.ray.pcx = a.x; pk.ray.pcy = a.y; pk.ray.pcz = a.z; pk.ray.u = 0.f;
                         pk.ray.nx = b.x; pk.ray.ny = b.y; pk.ray.nz = b.z;
                         pk.ray.i = i; pk.ray.j = j; pk.ray.k = k;
-                        pk.ray.col = (k * gs.nlat + j) * gs.nlev;
-                        alpha_c = rc.alpha + (size_t)(rc.chan_begin + pk.chan_run) * rc.geom.ncell;
+                        alpha_c = rc.alpha + (size_t)(rc.chan_begin + pk.chan_run) * rc.geom.alpha_stride;
                         const uint32_t kind = c.w >> 28;
                         st = kind == EV_MEDIUM ? LS_EV_MEDIUM : (kind == EV_EMIT ? LS_EV_EMIT : LS_EV_SURFACE);
                         need = false;
@@ -391,7 +397,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                 pk.pkt = rc.pkt_begin + uint32_t(item - (unsigned long long)pk.chan_run * rc.n_pkt);
                                 pk.m_inter = 0; pk.nev = 0;
                                 const int ctab = rc.chan_begin + int(pk.chan_run);
-                                alpha_c = rc.alpha + (size_t)ctab * rc.geom.ncell;
+                                alpha_c = rc.alpha + (size_t)ctab * rc.geom.alpha_stride;
                                 const uint32_t ckey = rc.chan_key0 + uint32_t(ctab);
                                 const Zeta4 z = zeta_block(rc.seed, ckey, pk.pkt, 0, 0);
                                 if (rc.mode == 0) {
@@ -455,8 +461,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                             pk.ray.pcx = r * sth * cp; pk.ray.pcy = r * sth * sp; pk.ray.pcz = r * ct;
                                             pk.ray.u = 0.f; pk.ray.nx = 0.f; pk.ray.ny = 0.f; pk.ray.nz = 1.f;
                                             pk.ray.i = i; pk.ray.j = j; pk.ray.k = k;
-                                            pk.ray.col = (k * gs.nlat + j) * gs.nlev;
-                                        }
+                                                            }
                                     }
                                 }
                             }
@@ -492,7 +497,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                     } else {
                         const int ctab = rc.chan_begin + int(pk.chan_run);
                         const uint32_t ckey = rc.chan_key0 + uint32_t(ctab);
-                        const int cell = pk.ray.col + pk.ray.i;
+                        const int cell = (pk.ray.k * gs.nlat + pk.ray.j) * gs.nlev + pk.ray.i;
                         const uint32_t meta = kind | batch_of(rc, pk.pkt) << 2 | pk.chan_run << 8;
                         ++c_events;
                         ++pk.nev;
@@ -577,7 +582,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
 #pragma unroll
         for (int s = 0; s < KSTEPS; ++s) {
             if (st == LS_FLY) {
-                const int rs = ray_step(pk.ray, gs, pk.tau, pk.tau_t, alpha_c);
+                const int rs = ray_step(pk.ray, gs, pk.tau, pk.tau_t);
                 ++c_seg32;
                 if (rs == RAY_FLYING) {
                     if (++pk.fl_seg > rc.geom.maxseg) st = LS_END_STUCK;
@@ -618,8 +623,6 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
 // (ray_lateral).  f = pref * Theta * exp(-tau_obs) (Eq. 14) goes to warp-private shared-memory bins [obs][batch]
 // of the warp's current channel, flushed to the fp64 global sums when the channel changes and at the end.
 // ---------------------------------------------------------------------------------------------------------
-enum PeelState : int { PS_IDLE = 0, PS_FLY = 1, PS_PARK = 2, PS_ESCAPED = 3 };
-
 __device__ __forceinline__ void peel_flush_bins(const RunConst& rc, float* bins, int nbins, int warp_chan)
 {
     for (int t = lane_id(); t < nbins; t += 32) {
@@ -635,7 +638,7 @@ __device__ __forceinline__ void peel_flush_bins(const RunConst& rc, float* bins,
 constexpr int kPeelChunk = 128;   // consecutive sorted events a warp takes per atomic (4 rounds of 32)
 
 template <int KSTEPS>
-__global__ void __launch_bounds__(kPeelThreads, 2)
+__global__ void __launch_bounds__(kPeelThreads, 4)
 peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsigned int* __restrict__ perm)
 {
     extern __shared__ float smem_f[];
@@ -669,7 +672,7 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
             const int bt = int((meta >> 2) & 63u);
             int ci, cj, ck;
             unpack_cell(__float_as_uint(c.y), ci, cj, ck);
-            const float* alpha_c = rc.alpha + (size_t)(rc.chan_begin + max(chan, 0)) * rc.geom.ncell;
+            const float* alpha_c = rc.alpha + (size_t)(rc.chan_begin + max(chan, 0)) * rc.geom.alpha_stride;
             // the warp's bins follow the newest channel; stragglers of older channels go straight to global memory
             int mx = chan;
 #pragma unroll
@@ -701,44 +704,35 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
                 const float pref = a.w * theta;
                 Ray ray{};
                 float tau = 0.f;
-                int fl_seg = 0;
-                int st = PS_IDLE;
+                int st = RAY_NONE;      // lane state = ray status: RAY_FLYING marches, RAY_PARK waits for ray_lateral
                 unsigned int seg32 = 0;
                 if (have && pref > 0.0f) {
                     ray_init(ray, gs, a.x, a.y, a.z, ox, oy, oz, ci, cj, ck, alpha_c);
-                    st = PS_FLY;
+                    st = RAY_FLYING;
                     ++c_rays;
                 }
-                for (;;) {
-                    const unsigned m_fly = __ballot_sync(kFullMask, st == PS_FLY);
-                    const unsigned m_park = __ballot_sync(kFullMask, st == PS_PARK);
+                // all lanes start together, so one warp-uniform step budget guards against a ray that never ends
+                for (int it = 0; it <= rc.geom.maxseg; it += KSTEPS) {
+                    const unsigned m_fly = __ballot_sync(kFullMask, st == RAY_FLYING);
+                    const unsigned m_park = __ballot_sync(kFullMask, st == RAY_PARK);
                     if ((m_fly | m_park) == 0) break;
                     if (m_park && (__popc(m_park) >= rc.t_lateral || m_fly == 0)) {
-                        if (st == PS_PARK) {
+                        if (st == RAY_PARK) {
                             ray_lateral(ray, gs, alpha_c);
-                            st = PS_FLY;
+                            st = RAY_FLYING;
                         }
                     }
 #pragma unroll
                     for (int s = 0; s < KSTEPS; ++s) {
-                        if (st == PS_FLY) {
-                            const int rs = ray_step(ray, gs, tau, rc.tau_cut, alpha_c);
+                        if (st == RAY_FLYING) {
                             ++seg32;
-                            if (rs == RAY_FLYING) {
-                                if (++fl_seg > rc.geom.maxseg) st = PS_IDLE;
-                            } else if (rs == RAY_PARK) {
-                                st = (++fl_seg > rc.geom.maxseg) ? PS_IDLE : PS_PARK;
-                            } else if (rs == RAY_ESCAPE) {
-                                st = PS_ESCAPED;
-                            } else {
-                                st = PS_IDLE;   // surface hit or tau_obs > tau_cut: nothing reaches the observer
-                            }
+                            st = ray_step(ray, gs, tau, rc.tau_cut);
                         }
                     }
                 }
                 c_seg += seg32;
                 // ---------------- rays that reached the top of the atmosphere: Eq. 14 ----------------
-                if (st == PS_ESCAPED) {
+                if (st == RAY_ESCAPE) {
                     const float f = pref * expf(-tau);
                     if (chan == warp_chan) atomicAdd(bins + obs * rc.n_batches + bt, f);
                     else atomicAdd(rc.flux + ((size_t)chan * rc.n_obs_total + rc.obs_first + obs) * rc.n_batches + bt, double(f));
@@ -819,7 +813,7 @@ __global__ void __launch_bounds__(128) debug_ray_tau_kernel(const GeomParams g, 
     float tau = 0.f;
     int rs = RAY_FLYING, nseg = 0;
     while (rs == RAY_FLYING && nseg++ <= g.maxseg) {
-        rs = ray_step(ray, gs, tau, kInf, alpha_c);
+        rs = ray_step(ray, gs, tau, kInf);
         if (rs == RAY_PARK) { ray_lateral(ray, gs, alpha_c); rs = RAY_FLYING; }
     }
     tau_out[m] = tau;

@@ -12,34 +12,45 @@
 // Only the face family that was just crossed is recomputed, positions are never advanced incrementally (no drift),
 // cell indices are tracked by crossings (never re-located from coordinates), and the face just crossed is excluded
 // by the strict comparison root > u, which is exact because the recomputed root is bit-identical to the u it set.
+//
+// The march is split in two: ray_step() is the radial fast path (shell crossings: ~30 instructions, no global
+// address arithmetic beyond one IMAD.WIDE, the extinction of the next cell prefetched one step ahead); a cone or
+// half-plane crossing stops it with RAY_PARK and is completed by ray_lateral(), which the kernels batch across the
+// warp.  The staged extinction table has one guard entry below and above every column so that the prefetch needs
+// no clamping.
 #pragma once
 #include "device_common.cuh"
 
 namespace gcmcrt {
 
+// Padded column length of the staged extinction table: nlev + 2 guard entries, rounded up to whole 32 B sectors.
+__host__ __device__ inline int alpha_col_stride(int nlev) { return (nlev + 2 + 7) & ~7; }
+
 // Geometry tables, staged by the host into one device array and copied to shared memory by every CTA.
 struct GeomParams {
     int nlev, nlat, nlon, ncell;
-    const float* tab;  // packed: R[nlev+1] R2[nlev+1] R2lo[nlev+1] qcube[nlev] cth[nlat+1] cph[nlon+1] sph[nlon+1] ph[nlon+1]
+    const float* tab;  // packed: R2pair[2(nlev+1)] R[nlev+1] qcube[nlev] cth[nlat+1] cph[nlon+1] sph[nlon+1] ph[nlon+1]
     int tab_floats;
     float Rtoa, R0;
     int maxseg;
+    int col_stride;    // alpha_col_stride(nlev)
+    long long alpha_stride;  // floats per channel of the staged extinction table: nlat * nlon * col_stride
 };
 
 struct GeomSmem {
-    const float *R, *R2, *R2lo, *qcube, *cth, *cph, *sph, *ph;
-    int nlev, nlat, nlon;
+    const float2* R2;  // (high, low) parts of R_k^2
+    const float *R, *qcube, *cth, *cph, *sph, *ph;
+    int nlev, nlat, nlon, col_stride;
 };
 
 __device__ __forceinline__ GeomSmem load_geom(const GeomParams& g, float* smem)
 {
     for (int t = threadIdx.x; t < g.tab_floats; t += blockDim.x) smem[t] = g.tab[t];
     GeomSmem s;
-    s.nlev = g.nlev; s.nlat = g.nlat; s.nlon = g.nlon;
-    s.R = smem;
-    s.R2 = s.R + (g.nlev + 1);
-    s.R2lo = s.R2 + (g.nlev + 1);
-    s.qcube = s.R2lo + (g.nlev + 1);
+    s.nlev = g.nlev; s.nlat = g.nlat; s.nlon = g.nlon; s.col_stride = g.col_stride;
+    s.R2 = reinterpret_cast<const float2*>(smem);
+    s.R = smem + 2 * (g.nlev + 1);
+    s.qcube = s.R + (g.nlev + 1);
     s.cth = s.qcube + g.nlev;
     s.cph = s.cth + (g.nlat + 1);
     s.sph = s.cph + (g.nlon + 1);
@@ -47,7 +58,10 @@ __device__ __forceinline__ GeomSmem load_geom(const GeomParams& g, float* smem)
     return s;
 }
 
-enum RayStatus : int { RAY_FLYING = 0, RAY_LIMIT = 1, RAY_ESCAPE = 2, RAY_SURFACE = 3, RAY_STUCK = 4, RAY_PARK = 5 };
+// Ray status doubles as the lane state of the kernels: RAY_FLYING lanes march, RAY_PARK lanes wait for
+// ray_lateral(), everything else is a finished flight.
+enum RayStatus : int { RAY_FLYING = 0, RAY_LIMIT = 1, RAY_ESCAPE = 2, RAY_SURFACE = 3, RAY_STUCK = 4, RAY_PARK = 5,
+                       RAY_NONE = 6 };
 
 struct Ray {
     float pcx, pcy, pcz;  // closest-approach point
@@ -58,23 +72,29 @@ struct Ray {
     float u_rad, u_lat, u_lon;  // next crossing of each face family
     float alpha;          // extinction of the current cell
     float alpha_n;        // prefetched extinction of the radial neighbour (i + rad_step) in the same column
+    const float* colp;    // extinction column of the current (j, k): colp[i], guard entries at colp[-1], colp[nlev]
     int i, j, k;          // cell
-    int col;              // (k*nlat + j)*nlev
     int rad_step, lat_step, lon_step;
 };
 
+__device__ __forceinline__ float shell_q(const Ray& r, const GeomSmem& s, int idx)
+{
+    const float2 R2 = s.R2[idx];
+    return (R2.x - r.d2) + (R2.y - r.d2lo);
+}
+
+// Next shell crossing at the start of a ray.
 __device__ __forceinline__ void ray_setup_rad(Ray& r, const GeomSmem& s)
 {
     if (r.u < 0.0f) {  // inward phase: the inner shell is hit iff it lies outside the impact parameter
-        const float q = (s.R2[r.i] - r.d2) + (s.R2lo[r.i] - r.d2lo);
+        const float q = shell_q(r, s, r.i);
         if (q > 0.0f) {
             r.u_rad = -sqrt_approx(q);
             r.rad_step = -1;
             return;
         }
     }
-    const float q = (s.R2[r.i + 1] - r.d2) + (s.R2lo[r.i + 1] - r.d2lo);
-    r.u_rad = sqrt_approx(fmaxf(q, 0.0f));
+    r.u_rad = sqrt_approx(fmaxf(shell_q(r, s, r.i + 1), 0.0f));
     r.rad_step = 1;
 }
 
@@ -134,18 +154,19 @@ __device__ __forceinline__ void ray_setup_lon(Ray& r, const GeomSmem& s)
     r.lon_step = step;
 }
 
+// Column pointer of (j, k) in the staged extinction table of one channel (alpha_tab points at that channel).
+__device__ __forceinline__ const float* ray_column(const GeomSmem& s, const float* __restrict__ alpha_tab, int j, int k)
+{
+    return alpha_tab + (size_t)(k * s.nlat + j) * s.col_stride + 1;
+}
+
 // Extinction of the current cell and, one step ahead, of the radial neighbour the ray will enter next: the march
 // loop consumes alpha one iteration after the load was issued, so the gather latency overlaps a full step.
 __device__ __forceinline__ void ray_load_alpha(Ray& r, const GeomSmem& s, const float* __restrict__ alpha_tab)
 {
-    const float* colp = alpha_tab + r.col;
-    r.alpha = __ldg(colp + r.i);
-    r.alpha_n = __ldg(colp + min(max(r.i + r.rad_step, 0), s.nlev - 1));
-#ifdef GCMCRT_PREFETCH
-    // the column is new to this lane: pull the next sectors along the radial direction into L1 ahead of the march
-    prefetch_l1(colp + min(max(r.i + 8 * r.rad_step, 0), s.nlev - 1));
-    prefetch_l1(colp + min(max(r.i + 16 * r.rad_step, 0), s.nlev - 1));
-#endif
+    r.colp = ray_column(s, alpha_tab, r.j, r.k);
+    r.alpha = __ldg(r.colp + r.i);
+    r.alpha_n = __ldg(r.colp + (r.i + r.rad_step));
 }
 
 // Start a ray at p with unit direction n inside cell (i,j,k).
@@ -167,7 +188,6 @@ __device__ __forceinline__ void ray_init(Ray& r, const GeomSmem& s, float px, fl
     r.nx = nx; r.ny = ny; r.nz = nz;
     r.u = b0;
     r.i = i; r.j = j; r.k = k;
-    r.col = (k * s.nlat + j) * s.nlev;
     ray_setup_rad(r, s);
     ray_setup_lat(r, s);
     ray_setup_lon(r, s);
@@ -177,32 +197,38 @@ __device__ __forceinline__ void ray_init(Ray& r, const GeomSmem& s, float px, fl
 // One step of the march, radial fast path.  tau accumulates over the segment up to the next face.  A shell crossing
 // is completed here (index, next shell root, alpha rotation + prefetch) and returns RAY_FLYING; when the next face
 // is a cone or a half-plane the ray is advanced to it and RAY_PARK is returned: the caller completes the crossing
-// with ray_lateral(), which the kernels batch across the warp so that the rarely taken, expensive cone / plane
-// root updates do not serialise against the radial path of the other lanes.
-__device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, float tau_limit,
-                                        const float* __restrict__ alpha_tab)
+// with ray_lateral().  Once a ray has crossed a shell outward it stays outward (u > 0), so only a ray still moving
+// inward has to ask whether the next inner shell lies outside its impact parameter.
+__device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, float tau_limit)
 {
     const float ul = fminf(r.u_lat, r.u_lon);
     const float un = fminf(r.u_rad, ul);
     const float ds = fmaxf(un - r.u, 0.0f);
-    const float dtau = r.alpha * ds;
-    if (tau + dtau >= tau_limit) {  // the limit is reached inside this cell
+    const float tnew = fmaf(r.alpha, ds, tau);
+    if (tnew >= tau_limit) {  // the limit is reached inside this cell
         r.u += (tau_limit - tau) / r.alpha;
         tau = tau_limit;
         return RAY_LIMIT;
     }
-    tau += dtau;
+    tau = tnew;
     r.u = fmaxf(un, r.u);
-    if (r.u_rad <= ul) {  // ties: shells first (C1)
-        r.i += r.rad_step;
-        if (r.i >= s.nlev) { r.i = s.nlev - 1; return RAY_ESCAPE; }
+    if (r.u_rad > ul) return RAY_PARK;  // ties: shells first (C1)
+    r.i += r.rad_step;
+    if ((unsigned)r.i >= (unsigned)s.nlev) {
         if (r.i < 0) { r.i = 0; return RAY_SURFACE; }
-        r.alpha = r.alpha_n;   // prefetched for exactly this cell
-        ray_setup_rad(r, s);   // may turn the ray from inward to outward
-        r.alpha_n = __ldg(alpha_tab + r.col + min(max(r.i + r.rad_step, 0), s.nlev - 1));
-        return RAY_FLYING;
+        r.i = s.nlev - 1;
+        return RAY_ESCAPE;
     }
-    return RAY_PARK;
+    r.alpha = r.alpha_n;   // prefetched for exactly this cell
+    float q = shell_q(r, s, r.i + ((r.rad_step + 1) >> 1));
+    if (r.rad_step < 0 && !(q > 0.0f)) {   // the inner shell lies inside the impact parameter: turn outward
+        r.rad_step = 1;
+        q = shell_q(r, s, r.i + 1);
+    }
+    const float sq = sqrt_approx(fmaxf(q, 0.0f));
+    r.u_rad = __int_as_float(__float_as_int(sq) | (r.rad_step & 0x80000000));
+    r.alpha_n = __ldg(r.colp + (r.i + r.rad_step));
+    return RAY_FLYING;
 }
 
 // Completes the cone / half-plane crossing of a parked ray (ties: cones before planes, C1).
@@ -210,12 +236,10 @@ __device__ __forceinline__ void ray_lateral(Ray& r, const GeomSmem& s, const flo
 {
     if (r.u_lat <= r.u_lon) {
         r.j = min(max(r.j + r.lat_step, 0), s.nlat - 1);
-        r.col = (r.k * s.nlat + r.j) * s.nlev;
         ray_setup_lat(r, s);
     } else {
         r.k += r.lon_step;
         r.k = (r.k < 0) ? r.k + s.nlon : (r.k >= s.nlon ? r.k - s.nlon : r.k);
-        r.col = (r.k * s.nlat + r.j) * s.nlev;
         ray_setup_lon(r, s);
     }
     ray_load_alpha(r, s, alpha_tab);

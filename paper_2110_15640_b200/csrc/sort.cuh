@@ -5,12 +5,14 @@
 // two sectors and makes the lanes of a warp finish together.  Only a permutation is built (4 B per event); the
 // 48 B records stay where the transport kernel wrote them.
 //
-//   key(e) = (chan_run(e) mod c_fold) * ncell + (k * nlat + j) * nlev + i        (cell-flat layout, i fastest)
+//   key(e) = clamp(chan_run(e) - chan_lo, 0, c_fold - 1) * ncell + (k * nlat + j) * nlev + i   (i fastest)
 //   ev_hist_kernel    hist[key]++                                  (global atomics)
 //   scan_*            exclusive prefix sum of hist in place        (tile reduce, scan of tile sums, tile scan)
 //   ev_scatter_kernel perm[hist[key]++] = e
 //
-// c_fold bounds the histogram (<= 2^25 bins); channels that fold onto each other only lose locality.
+// chan_lo is the first channel this pass draws fresh packets from (resumed packets of earlier channels clamp to it)
+// and c_fold the number of channels a pass can span; the clamped key keeps the order monotone in the channel, which
+// the peel kernel's per-warp flux bins rely on, and bounds the histogram (<= 2^25 bins).
 #pragma once
 #include "device_common.cuh"
 
@@ -28,14 +30,14 @@ struct SortParams {
     unsigned int* tile_sums;     // [n_tiles]
     unsigned int* perm;          // [cap]
     unsigned int nbins, n_tiles;
-    int nlev, nlat, ncell, c_fold;
+    int nlev, nlat, ncell, c_fold, chan_lo;
 };
 
 __device__ __forceinline__ unsigned int event_sort_key(const SortParams& p, const float4 c)
 {
     const uint32_t cell = __float_as_uint(c.y), meta = __float_as_uint(c.z);
     const int i = cell & 1023, j = (cell >> 10) & 1023, k = cell >> 20;
-    const unsigned int chan = (meta >> 8) % (unsigned int)p.c_fold;
+    const unsigned int chan = (unsigned int)min(max(int(meta >> 8) - p.chan_lo, 0), p.c_fold - 1);
     return chan * (unsigned int)p.ncell + (unsigned int)((k * p.nlat + j) * p.nlev + i);
 }
 

@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgcmcrt.so")
 SOURCES = [os.path.join(CSRC, "gcmcrt.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "ray.cuh", "sort.cuh", "device_common.cuh")] + \
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "ray.cuh", "sort.cuh", "wavefront.cuh", "device_common.cuh")] + \
     [os.path.join(os.path.dirname(HERE), "include", "gcmcrt.h")]
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -34,6 +34,8 @@ struct DevBuf {  // owned device allocation
     template <class T> T* as() const { return static_cast<T*>(p); }
 };
 
+constexpr int kMaxGen = 30;
+
 struct PassCtrl {  // small device block reset every pass
     unsigned int ev_count;
     unsigned int susp_count[2];
@@ -41,6 +43,7 @@ struct PassCtrl {  // small device block reset every pass
     unsigned int pad;
     unsigned long long work_counter;
     unsigned long long ray_counter;
+    unsigned int gen_mark[kMaxGen + 2];   // event-buffer offsets of the wavefront generations of this pass
 };
 
 }  // namespace
@@ -72,10 +75,13 @@ struct gcmcrt_grid {
     DevBuf Lcell, Lcum, Ltot;
 
     // workspace
-    DevBuf ev0, ev1, ev2, perm, hist, tile_sums, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount;
+    DevBuf ev0, ev1, ev2, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount;
     unsigned int ev_cap = 0;
     int n_threads_resident = 0;
-    int tune[3] = {12, 8, 10};   // warp scheduling thresholds: service, lateral, peel refill (GCMCRT_TUNE overrides)
+    // GCMCRT_TUNE="service,lateral,gens,batch_div": lanes waiting before the persistent kernel serves them; lanes parked at
+    // a cone / half-plane before a warp serves them; wavefront generations per pass before the persistent kernel takes over
+    // (0 = persistent kernel only); first-pass batch = event capacity / batch_div
+    int tune[4] = {16, 1, 8, 4};
     PassCtrl* h_ctrl = nullptr;  // pinned
     cudaEvent_t tev[4] = {nullptr, nullptr, nullptr, nullptr};   // kernel timing (A0 | A2 | transport | peel)
     unsigned long long launches = 0, launches_pending = 0;
@@ -227,11 +233,11 @@ int ensure_workspace(gcmcrt_grid* g)
         if (cap > (1ull << 30)) cap = 1ull << 30;
         g->ev_cap = (unsigned int)cap;
         if (const char* e = std::getenv("GCMCRT_TUNE")) {   // "service,lateral,refill": scheduling thresholds, 1..32
-            int a = 0, b = 0, c = 0;
-            if (std::sscanf(e, "%d,%d,%d", &a, &b, &c) == 3) {
-                g->tune[0] = std::min(std::max(a, 1), 32); g->tune[1] = std::min(std::max(b, 1), 32);
-                g->tune[2] = std::min(std::max(c, 1), 32);
-            }
+            int a = 0, b = 0, c = 0, d = 0;
+            const int n = std::sscanf(e, "%d,%d,%d,%d", &a, &b, &c, &d);
+            if (n >= 2) { g->tune[0] = std::min(std::max(a, 1), 32); g->tune[1] = std::min(std::max(b, 1), 32); }
+            if (n >= 3) g->tune[2] = std::min(std::max(c, 0), kMaxGen);
+            if (n >= 4) g->tune[3] = std::min(std::max(d, 1), 64);
         }
     }
     CUDA_TRY(g, g->ev0.ensure(size_t(g->ev_cap) * sizeof(float4)));
@@ -336,7 +342,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.counters = g->counters.as<DevCounters>();
     rc.magic_N = magic_div(N);
     rc.magic_npkt = magic_div(n_pkt);
-    rc.t_service = g->tune[0]; rc.t_lateral = g->tune[1]; rc.p_refill = g->tune[2];
+    rc.t_service = g->tune[0]; rc.t_lateral = g->tune[1]; rc.p_refill = 12;
     PassCtrl* ctrl = g->ctrl.as<PassCtrl>();
     rc.work_counter = &ctrl->work_counter;
     rc.ray_counter = &ctrl->ray_counter;
@@ -351,10 +357,13 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     if (occ_t < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
     const int grid_t = g->sm_count * occ_t;
     const unsigned long long threads_t = (unsigned long long)grid_t * kTransportThreads;
+    // suspended list: one entry per resident lane for the persistent kernel, plus what a wavefront pass can park (its
+    // last generation and whatever found the event buffer full): bounded by 2 x event capacity (see the pass loop)
+    const unsigned long long susp_cap = threads_t + (g->tune[2] > 0 ? 2ull * g->ev_cap : 0ull);
     for (int b = 0; b < 2; ++b) {
-        CUDA_TRY(g, g->s0[b].ensure(threads_t * sizeof(float4)));
-        CUDA_TRY(g, g->s1[b].ensure(threads_t * sizeof(float4)));
-        CUDA_TRY(g, g->s2[b].ensure(threads_t * sizeof(uint4)));
+        CUDA_TRY(g, g->s0[b].ensure(susp_cap * sizeof(float4)));
+        CUDA_TRY(g, g->s1[b].ensure(susp_cap * sizeof(float4)));
+        CUDA_TRY(g, g->s2[b].ensure(susp_cap * sizeof(uint4)));
     }
     EventBuf ev;
     ev.e0 = g->ev0.as<float4>(); ev.e1 = g->ev1.as<float4>(); ev.e2 = g->ev2.as<float4>();
@@ -448,7 +457,44 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             sp.perm = g->perm.as<unsigned int>();
             sp.nlev = g->nlev; sp.nlat = g->nlat; sp.ncell = g->ncell;
         }
-        unsigned long long items_before = 0;   // fresh-packet counter at the start of the pass
+        // ---- wavefront kernels (wavefront.cuh): launch geometry and the launch-order sort of albedo runs
+        const int n_gen = g->tune[2];
+        auto k_keys = wave_launch_keys_kernel;
+        auto k_first = wave_first_flight_kernel<4>;
+        auto k_emit = wave_emit_kernel;
+        auto k_inter = wave_interact_kernel<4>;
+        const size_t smem_w = smem_t;
+        const size_t smem_i = (size_t((g->tab_floats + 31) & ~31) + size_t(kWaveThreads / 32) * kStageFields * kStageSlots) * sizeof(float);
+        int occ_f = 1, occ_i = 1;
+        SortParams spl;
+        std::memset(&spl, 0, sizeof spl);
+        if (n_gen > 0) {
+            CUDA_TRY(g, cudaFuncSetAttribute(k_keys, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_w)));
+            CUDA_TRY(g, cudaFuncSetAttribute(k_first, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_w)));
+            CUDA_TRY(g, cudaFuncSetAttribute(k_emit, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_w)));
+            CUDA_TRY(g, cudaFuncSetAttribute(k_inter, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_i)));
+            CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_first, kWaveThreads, smem_w));
+            CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_i, k_inter, kWaveThreads, smem_i));
+            if (occ_f < 1 || occ_i < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
+            if (!emission) {
+                const int ncol = g->nlat * g->nlon;
+                spl.c_fold = int(std::max<long long>(1, std::min<long long>(ncr, (long long)(g->ev_cap / std::max<size_t>(n_pkt, 1)) + 2)));
+                spl.nbins = (unsigned int)((long long)spl.c_fold * ncol);
+                spl.n_tiles = (spl.nbins + kScanTile - 1) / kScanTile;
+                CUDA_TRY(g, g->lkeys.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));
+                CUDA_TRY(g, g->lperm.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));
+                CUDA_TRY(g, g->lhist.ensure(size_t(spl.nbins) * sizeof(unsigned int)));
+                CUDA_TRY(g, g->ltile.ensure(size_t(spl.n_tiles) * sizeof(unsigned int)));
+                spl.keys = g->lkeys.as<unsigned int>(); spl.count = nullptr; spl.cap = g->ev_cap;
+                spl.hist = g->lhist.as<unsigned int>(); spl.tile_sums = g->ltile.as<unsigned int>();
+                spl.perm = g->lperm.as<unsigned int>();
+            }
+        }
+        // Fresh packets per pass: sized so that all their events fit the event buffer; the ratio events / packet is
+        // learnt from the passes already run.  Whatever does not fit is parked and resumed by the next pass.
+        unsigned long long item0 = 0;
+        unsigned long long batch = std::max<unsigned long long>(1024, g->ev_cap / (unsigned long long)g->tune[3]);
+        unsigned long long ev_seen = 0, pk_seen = 0, leftover = 0;
         for (;;) {
             const int nxt = 1 - cur;
             SuspBuf sin, sout;
@@ -457,11 +503,50 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             sout.s0 = g->s0[nxt].as<float4>(); sout.s1 = g->s1[nxt].as<float4>(); sout.s2 = g->s2[nxt].as<uint4>();
             sout.count = &ctrl->susp_count[nxt]; sout.taken = &ctrl->susp_taken[nxt];
             CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
-            tk<<<grid_t, kTransportThreads, smem_t, s>>>(rc, ev, sin, sout, total_items);
+            unsigned long long n_fresh = 0, tail_items = total_items;
+            const unsigned long long chan_lo_pass = item0 / std::max<size_t>(n_pkt, 1);
+            if (n_gen > 0) {
+                // a pass that inherited a long suspended list only drains it (keeps the list bounded, see susp_cap)
+                n_fresh = leftover > g->ev_cap / 2 ? 0 : std::min<unsigned long long>(std::min<unsigned long long>(batch, g->ev_cap / 2), total_items - item0);
+                tail_items = 0;   // the persistent kernel only finishes what the generations leave over
+                WaveConst wc;
+                std::memset(&wc, 0, sizeof wc);
+                wc.item0 = item0; wc.n_items = (unsigned int)n_fresh;
+                wc.chan_lo = int(chan_lo_pass); wc.c_fold = std::max(spl.c_fold, 1);
+                if (n_fresh > 0) {
+                    if (!emission) {
+                        wc.keys = g->lkeys.as<unsigned int>(); wc.perm = g->lperm.as<unsigned int>();
+                        spl.n_host = wc.n_items;
+                        const unsigned gk = (unsigned)std::min<unsigned long long>((n_fresh + 255) / 256, (unsigned long long)g->sm_count * 8);
+                        k_keys<<<gk, kWaveThreads, smem_w, s>>>(rc, wc);
+                        CUDA_TRY(g, cudaMemsetAsync(spl.hist, 0, size_t(spl.nbins) * sizeof(unsigned int), s));
+                        ev_hist_kernel<<<gk, 256, 0, s>>>(spl);
+                        scan_reduce_kernel<<<spl.n_tiles, kScanThreads, 0, s>>>(spl);
+                        scan_tiles_kernel<<<1, 1024, 0, s>>>(spl);
+                        scan_apply_kernel<<<spl.n_tiles, kScanThreads, 0, s>>>(spl);
+                        ev_scatter_kernel<<<gk, 256, 0, s>>>(spl);
+                        k_first<<<g->sm_count * occ_f, kWaveThreads, smem_w, s>>>(rc, ev, sin, wc);
+                        g->launches += 7;
+                    } else {
+                        const unsigned ge = (unsigned)std::min<unsigned long long>((n_fresh + 255) / 256, (unsigned long long)g->sm_count * 8);
+                        k_emit<<<ge, kWaveThreads, smem_w, s>>>(rc, ev, sin, wc);
+                        g->launches += 1;
+                    }
+                    CUDA_TRY(g, cudaMemcpyAsync(&ctrl->gen_mark[1], &ctrl->ev_count, sizeof(unsigned int), cudaMemcpyDeviceToDevice, s));
+                    for (int gi = 0; gi < n_gen; ++gi) {
+                        wc.gen_mark = &ctrl->gen_mark[gi];
+                        wc.park_all = gi == n_gen - 1;
+                        k_inter<<<g->sm_count * occ_i, kWaveThreads, smem_i, s>>>(rc, ev, sin, wc);
+                        CUDA_TRY(g, cudaMemcpyAsync(&ctrl->gen_mark[gi + 2], &ctrl->ev_count, sizeof(unsigned int), cudaMemcpyDeviceToDevice, s));
+                    }
+                    g->launches += n_gen;
+                }
+            }
+            tk<<<grid_t, kTransportThreads, smem_t, s>>>(rc, ev, sin, sout, tail_items);
             CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
             if (rc.n_obs_run > 0) {
                 // counting sort of this pass's events by (channel, cell): sort.cuh
-                sp.chan_lo = int(std::min<unsigned long long>(items_before / std::max<size_t>(n_pkt, 1), (unsigned long long)ncr));
+                sp.chan_lo = int(std::min<unsigned long long>(n_gen > 0 ? chan_lo_pass : item0 / std::max<size_t>(n_pkt, 1), (unsigned long long)ncr));
                 CUDA_TRY(g, cudaMemsetAsync(sp.hist, 0, size_t(sp.nbins) * sizeof(unsigned int), s));
                 ev_hist_kernel<<<g->sm_count * 8, 256, 0, s>>>(sp);
                 scan_reduce_kernel<<<sp.n_tiles, kScanThreads, 0, s>>>(sp);
@@ -484,13 +569,25 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
                 CUDA_TRY(g, cudaEventElapsedTime(&c, g->tev[2], g->tev[3]));
                 g->ms_transport += a; g->ms_sort += b; g->ms_peel += c;
             }
-            items_before = std::min<unsigned long long>(g->h_ctrl->work_counter, total_items);
-            const bool done = g->h_ctrl->work_counter >= total_items && g->h_ctrl->susp_count[nxt] == 0;
+            if (n_gen > 0) {
+                item0 += n_fresh;
+                ev_seen += std::min<unsigned long long>(g->h_ctrl->ev_count, g->ev_cap); pk_seen += n_fresh;
+                if (pk_seen > 0) {   // next batch: 85 % of the buffer at the ratio seen so far
+                    const double ratio = std::max(0.25, double(ev_seen) / double(pk_seen));
+                    batch = std::max<unsigned long long>(1024, (unsigned long long)(0.85 * double(g->ev_cap) / ratio));
+                }
+            } else {
+                item0 = std::min<unsigned long long>(g->h_ctrl->work_counter, total_items);
+            }
+            leftover = g->h_ctrl->susp_count[nxt];
+            if (leftover > susp_cap) return fail(g, GCMCRT_E_CUDA, "suspended-packet list overflow");
+            const bool done = item0 >= total_items && leftover == 0;
             if (done) break;
-            // reset the per-pass counters: events, rays, the list just consumed
+            // reset the per-pass counters: events, rays, generation marks, the list just consumed
             PassCtrl next = *g->h_ctrl;
             next.ev_count = 0; next.ray_counter = 0;
             next.susp_count[cur] = 0; next.susp_taken[cur] = 0; next.susp_taken[nxt] = 0;
+            std::memset(next.gen_mark, 0, sizeof next.gen_mark);
             CUDA_TRY(g, cudaMemcpyAsync(ctrl, &next, sizeof(PassCtrl), cudaMemcpyHostToDevice, s));
             CUDA_TRY(g, cudaStreamSynchronize(s));
             cur = nxt;
@@ -682,7 +779,7 @@ int gcmcrt_destroy(gcmcrt_grid* g)
     cudaGetLastError();
     for (DevBuf* b : {&g->tab, &g->r64, &g->cth64, &g->ph64, &g->rc32, &g->thc32, &g->phc32, &g->T, &g->rho, &g->u, &g->v,
                       &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->prop, &g->reff, &g->vlos,
-                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->ev1, &g->ev2, &g->perm, &g->hist, &g->tile_sums, &g->s0[0], &g->s0[1],
+                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->ev1, &g->ev2, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->s0[0], &g->s0[1],
                       &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->flux, &g->ltot_out,
                       &g->value, &g->sigma, &g->image, &g->evcount})
         b->release();

@@ -18,15 +18,32 @@ __device__ __forceinline__ void unpack_cell(uint32_t c, int& i, int& j, int& k) 
 
 enum EventKind : uint32_t { EV_MEDIUM = 0, EV_EMIT = 1, EV_SURFACE = 2 };
 
+struct EventBuf;
+__device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slot, float px, float py, float pz, float W,
+                                            float nx, float ny, float nz, uint32_t m_inter, uint32_t cellp, uint32_t meta,
+                                            uint32_t pkt);
+
 // Event records written by the transport kernel, consumed by the peel kernel (structure of arrays of float4).
 struct EventBuf {
-    float4* e0;  // px py pz pref          pref = W*omega (medium), W (emission), W*a (surface)
-    float4* e1;  // nx ny nz pgas          n = incoming direction (medium) or surface normal
-    float4* e2;  // g  cell  meta  pkt     meta = kind | batch << 2 | chan_run << 8
+    float4* e0;  // px py pz W             packet weight before the event
+    float4* e1;  // nx ny nz 0             n = incoming direction (medium) or surface normal
+    float4* e2;  // m_inter cell meta pkt  (bit patterns) interactions completed before this event; packed cell;
+                 //                        meta = kind | batch << 2 | chan_run << 8; packet id
+                 // The record is the peel kernel's input AND the packet's full state at the event: the wavefront
+                 // kernels continue packets from it.
     unsigned int* count;
     unsigned int cap;
     unsigned int soft_cap;
 };
+
+__device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slot, float px, float py, float pz, float W,
+                                            float nx, float ny, float nz, uint32_t m_inter, uint32_t cellp, uint32_t meta,
+                                            uint32_t pkt)
+{
+    ev.e0[slot] = make_float4(px, py, pz, W);
+    ev.e1[slot] = make_float4(nx, ny, nz, 0.f);
+    ev.e2[slot] = make_float4(__uint_as_float(m_inter), __uint_as_float(cellp), __uint_as_float(meta), __uint_as_float(pkt));
+}
 
 // Packets suspended because the event buffer filled up; resumed by the next pass.
 struct SuspBuf {
@@ -493,7 +510,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                         susp_out.s0[sidx] = make_float4(px, py, pz, pk.W);
                         susp_out.s1[sidx] = make_float4(pk.ray.nx, pk.ray.ny, pk.ray.nz, __uint_as_float(cellp));
                         susp_out.s2[sidx] = make_uint4(pk.chan_run, pk.pkt, pk.m_inter, pk.nev | kind << 28);
-                        st = LS_DONE;
+                        st = LS_IDLE;   // the lane goes on moving the rest of the suspended list over to the next pass
                     } else {
                         const int ctab = rc.chan_begin + int(pk.chan_run);
                         const uint32_t ckey = rc.chan_key0 + uint32_t(ctab);
@@ -504,10 +521,8 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                         if (st == LS_EV_MEDIUM) {
                             const float4 pr = __ldg(rc.prop + (size_t)ctab * rc.geom.ncell + cell);
                             if (record) {
-                                ev.e0[slot] = make_float4(px, py, pz, pk.W * pr.x);
-                                ev.e1[slot] = make_float4(pk.ray.nx, pk.ray.ny, pk.ray.nz, pr.y);
-                                ev.e2[slot] = make_float4(pr.z, __uint_as_float(cellp), __uint_as_float(meta),
-                                                          __uint_as_float(pk.pkt));
+                                write_event(ev, slot, px, py, pz, pk.W, pk.ray.nx, pk.ray.ny, pk.ray.nz, pk.m_inter, cellp,
+                                            meta, pk.pkt);
                             }
                             ++pk.m_inter;
                             const Zeta4 z = zeta_block(rc.seed, ckey, pk.pkt, pk.m_inter, 1);
@@ -523,10 +538,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                             }
                         } else if (st == LS_EV_EMIT) {
                             if (record) {
-                                ev.e0[slot] = make_float4(px, py, pz, pk.W);
-                                ev.e1[slot] = make_float4(0.f, 0.f, 1.f, 0.f);
-                                ev.e2[slot] = make_float4(0.f, __uint_as_float(cellp), __uint_as_float(meta),
-                                                          __uint_as_float(pk.pkt));
+                                write_event(ev, slot, px, py, pz, pk.W, 0.f, 0.f, 1.f, pk.m_inter, cellp, meta, pk.pkt);
                             }
                             if (!rc.scatter_on) {
                                 ++c_abs; st = LS_IDLE; finish_packet(rc, pk);
@@ -545,10 +557,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                             const float rn = rsqrtf(fmaf(px, px, fmaf(py, py, pz * pz)));
                             float hx = px * rn, hy = py * rn, hz = pz * rn;
                             if (record) {
-                                ev.e0[slot] = make_float4(px, py, pz, pk.W * a);
-                                ev.e1[slot] = make_float4(hx, hy, hz, 0.f);
-                                ev.e2[slot] = make_float4(0.f, __uint_as_float(cellp), __uint_as_float(meta),
-                                                          __uint_as_float(pk.pkt));
+                                write_event(ev, slot, px, py, pz, pk.W, hx, hy, hz, pk.m_inter, cellp, meta, pk.pkt);
                             }
                             ++pk.m_inter;
                             const Zeta4 z = zeta_block(rc.seed, ckey, pk.pkt, pk.m_inter, 3);
@@ -615,6 +624,10 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
     }
 }
 
+}  // namespace gcmcrt
+#include "wavefront.cuh"
+namespace gcmcrt {
+
 // ---------------------------------------------------------------------------------------------------------
 // Peel-off kernel (A7 + A9).  Events arrive sorted by (channel, cell) (sort.cuh): a warp takes 32 consecutive
 // events, one per lane, and integrates their rays toward one observer at a time -- 32 parallel rays that start in
@@ -673,6 +686,15 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
             int ci, cj, ck;
             unpack_cell(__float_as_uint(c.y), ci, cj, ck);
             const float* alpha_c = rc.alpha + (size_t)(rc.chan_begin + max(chan, 0)) * rc.geom.alpha_stride;
+            // what the event scatters toward an observer: W omega (medium, Eq. 14), W (emission), W a (surface)
+            float wsca = a.w, pgas = 0.f, g = 0.f;
+            if (have && kind == EV_MEDIUM) {
+                const float4 pr = __ldg(rc.prop + (size_t)(rc.chan_begin + chan) * rc.geom.ncell +
+                                        ((ck * gs.nlat + cj) * gs.nlev + ci));
+                wsca *= pr.x; pgas = pr.y; g = pr.z;
+            } else if (kind == EV_SURFACE) {
+                wsca *= rc.surface_albedo;
+            }
             // the warp's bins follow the newest channel; stragglers of older channels go straight to global memory
             int mx = chan;
 #pragma unroll
@@ -691,17 +713,16 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
                 const float mu = b.x * ox + b.y * oy + b.z * oz;
                 float theta;
                 if (kind == EV_MEDIUM) {  // C6: mixture phase function, per steradian (Eq. 5, Eq. 7)
-                    const float g = c.x;
                     const float d = fmaf(-2.0f * g, mu, 1.0f + g * g);
                     const float hg = (1.0f - g * g) / (4.0f * kPi * d * sqrtf(d));
                     const float ray_p = 3.0f * (1.0f + mu * mu) / (16.0f * kPi);
-                    theta = b.w * ray_p + (1.0f - b.w) * hg;
+                    theta = pgas * ray_p + (1.0f - pgas) * hg;
                 } else if (kind == EV_EMIT) {
                     theta = 1.0f / (4.0f * kPi);
                 } else {
                     theta = fmaxf(mu, 0.0f) / kPi;
                 }
-                const float pref = a.w * theta;
+                const float pref = wsca * theta;
                 Ray ray{};
                 float tau = 0.f;
                 int st = RAY_NONE;      // lane state = ray status: RAY_FLYING marches, RAY_PARK waits for ray_lateral

@@ -23,9 +23,10 @@ constexpr int kScanItems = 16;                       // per thread
 constexpr int kScanTile = kScanThreads * kScanItems;  // 4096 bins per CTA
 
 struct SortParams {
-    const float4* e2;            // event records, third float4: g cell meta pkt
-    const unsigned int* count;   // events written this pass (device)
-    unsigned int cap;
+    const float4* e2;            // event records, third float4: m_inter cell meta pkt (key computed from it) ...
+    const unsigned int* keys;    // ... or explicit keys [n] (launch order of the first flights); e2 unused then
+    const unsigned int* count;   // number of items on the device (events written this pass), or NULL -> n_host
+    unsigned int cap, n_host;
     unsigned int* hist;          // [nbins]
     unsigned int* tile_sums;     // [n_tiles]
     unsigned int* perm;          // [cap]
@@ -41,18 +42,23 @@ __device__ __forceinline__ unsigned int event_sort_key(const SortParams& p, cons
     return chan * (unsigned int)p.ncell + (unsigned int)((k * p.nlat + j) * p.nlev + i);
 }
 
+__device__ __forceinline__ unsigned int sort_key_of(const SortParams& p, unsigned int e)
+{
+    return p.keys ? __ldg(p.keys + e) : event_sort_key(p, __ldg(p.e2 + e));
+}
+
 __global__ void __launch_bounds__(256) ev_hist_kernel(const SortParams p)
 {
-    const unsigned int n = min(*p.count, p.cap);
+    const unsigned int n = p.count ? min(*p.count, p.cap) : p.n_host;
     for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x)
-        atomicAdd(p.hist + event_sort_key(p, __ldg(p.e2 + e)), 1u);
+        atomicAdd(p.hist + sort_key_of(p, e), 1u);
 }
 
 __global__ void __launch_bounds__(256) ev_scatter_kernel(const SortParams p)
 {
-    const unsigned int n = min(*p.count, p.cap);
+    const unsigned int n = p.count ? min(*p.count, p.cap) : p.n_host;
     for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x)
-        p.perm[atomicAdd(p.hist + event_sort_key(p, __ldg(p.e2 + e)), 1u)] = e;
+        p.perm[atomicAdd(p.hist + sort_key_of(p, e), 1u)] = e;
 }
 
 __device__ __forceinline__ unsigned int block_sum_u32(unsigned int v, unsigned int* warp_part)

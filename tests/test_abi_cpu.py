@@ -36,7 +36,7 @@ def test_struct_layouts_match_header():
     assert C.sizeof(binding.RunParams) == 24 + 8 + 8 + 32 + 24 + 24 + 8
     assert binding.RunParams.obs_dir.offset == 32 and binding.RunParams.seed.offset == 64
     assert binding.RunParams.emission_bias.offset == 96 and binding.RunParams.n_batches.offset == 124
-    assert C.sizeof(binding.Counters) == 120
+    assert C.sizeof(binding.Counters) == 128     # 11 u64/double + 5 ms doubles (ms_sort added with the event sort)
     assert C.sizeof(binding.Result) == 56
 
 

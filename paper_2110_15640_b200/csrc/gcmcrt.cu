@@ -227,7 +227,7 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
 int ensure_workspace(gcmcrt_grid* g)
 {
     if (g->ev_cap == 0) {
-        unsigned long long cap = 16ull << 20;
+        unsigned long long cap = 64ull << 20;   // 64 Mi events x 48 B = 3 GB: a cfg2 step takes 7 passes
         if (const char* e = std::getenv("GCMCRT_EVENT_CAP")) cap = std::strtoull(e, nullptr, 10);
         if (cap < 64) cap = 64;
         if (cap > (1ull << 30)) cap = 1ull << 30;
@@ -358,8 +358,9 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     const int grid_t = g->sm_count * occ_t;
     const unsigned long long threads_t = (unsigned long long)grid_t * kTransportThreads;
     // suspended list: one entry per resident lane for the persistent kernel, plus what a wavefront pass can park (its
-    // last generation and whatever found the event buffer full): bounded by 2 x event capacity (see the pass loop)
-    const unsigned long long susp_cap = threads_t + (g->tune[2] > 0 ? 2ull * g->ev_cap : 0ull);
+    // last generation and whatever found the event buffer full).  A pass starts with at most ev_cap / 2 inherited
+    // entries (else it only drains) and parks each of its <= ev_cap / 2 fresh packets at most once: <= ev_cap in all
+    const unsigned long long susp_cap = threads_t + (g->tune[2] > 0 ? 1ull * g->ev_cap : 0ull);
     for (int b = 0; b < 2; ++b) {
         CUDA_TRY(g, g->s0[b].ensure(susp_cap * sizeof(float4)));
         CUDA_TRY(g, g->s1[b].ensure(susp_cap * sizeof(float4)));
@@ -479,7 +480,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             if (!emission) {
                 const int ncol = g->nlat * g->nlon;
                 spl.c_fold = int(std::max<long long>(1, std::min<long long>(ncr, (long long)(g->ev_cap / std::max<size_t>(n_pkt, 1)) + 2)));
-                spl.nbins = (unsigned int)((long long)spl.c_fold * ncol);
+                spl.nbins = (unsigned int)((long long)spl.c_fold * ncol * kLaunchTauBuckets);
                 spl.n_tiles = (spl.nbins + kScanTile - 1) / kScanTile;
                 CUDA_TRY(g, g->lkeys.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));
                 CUDA_TRY(g, g->lperm.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));

@@ -23,6 +23,7 @@ namespace gcmcrt {
 constexpr int kWaveThreads = 256;
 constexpr int kStageFields = 14;
 constexpr int kStageSlots = 64;   // per warp: at most 31 left over + 32 new survivors
+constexpr int kLaunchTauBuckets = 16;   // launch order: packets of one entry column grouped by sampled optical depth
 
 struct WaveConst {
     unsigned long long item0;      // first fresh packet item of this pass (item = chan_run * n_pkt + packet offset)
@@ -169,7 +170,7 @@ __device__ __forceinline__ void wave_item(const RunConst& rc, unsigned long long
     pkt = rc.pkt_begin + uint32_t(item - (unsigned long long)chan_run * rc.n_pkt);
 }
 
-// albedo: sort key of every fresh packet = (channel window slot, entry column)
+// albedo: sort key of every fresh packet = (channel window slot, entry column, optical-depth bucket)
 __global__ void __launch_bounds__(kWaveThreads) wave_launch_keys_kernel(const __grid_constant__ RunConst rc,
                                                                        const WaveConst wc)
 {
@@ -185,7 +186,11 @@ __global__ void __launch_bounds__(kWaveThreads) wave_launch_keys_kernel(const __
         int j, k;
         albedo_launch_point(rc, gs, z, px, py, pz, j, k);
         const int slot = min(max(int(chan_run) - wc.chan_lo, 0), wc.c_fold - 1);
-        wc.keys[t] = (unsigned int)(slot * (gs.nlat * gs.nlon) + k * gs.nlat + j);
+        // the extinction grows roughly exponentially with depth, so the level a packet reaches goes with log(tau):
+        // packets of one column that share a log2(tau) bucket end their first flight within a few cells of each other
+        const float lt = __log2f(-__logf(z.z2));                       // log2 of the sampled optical depth, about -23 .. 4
+        const int tb = min(max(int(floorf((lt + 8.0f) * (kLaunchTauBuckets / 12.0f))), 0), kLaunchTauBuckets - 1);
+        wc.keys[t] = (unsigned int)((slot * (gs.nlat * gs.nlon) + k * gs.nlat + j) * kLaunchTauBuckets + tb);
     }
 }
 

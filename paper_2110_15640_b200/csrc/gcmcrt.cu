@@ -75,7 +75,7 @@ struct gcmcrt_grid {
     DevBuf Lcell, Lcum, Ltot;
 
     // workspace
-    DevBuf ev0, ev1, ev2, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount;
+    DevBuf ev0, ev1, ev2, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, flights, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount;
     unsigned int ev_cap = 0;
     int n_threads_resident = 0;
     // GCMCRT_TUNE="service,lateral,gens,batch_div": lanes waiting before the persistent kernel serves them; lanes parked at
@@ -477,6 +477,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_first, kWaveThreads, smem_w));
             CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_i, k_inter, kWaveThreads, smem_i));
             if (occ_f < 1 || occ_i < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
+            CUDA_TRY(g, g->flights.ensure(size_t(g->sm_count) * occ_i * (kWaveThreads / 32) * kFlightFields * kStageSlots * sizeof(float)));
             if (!emission) {
                 const int ncol = g->nlat * g->nlon;
                 spl.c_fold = int(std::max<long long>(1, std::min<long long>(ncr, (long long)(g->ev_cap / std::max<size_t>(n_pkt, 1)) + 2)));
@@ -514,6 +515,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
                 std::memset(&wc, 0, sizeof wc);
                 wc.item0 = item0; wc.n_items = (unsigned int)n_fresh;
                 wc.chan_lo = int(chan_lo_pass); wc.c_fold = std::max(spl.c_fold, 1);
+                wc.flights = g->flights.as<float>();
                 if (n_fresh > 0) {
                     if (!emission) {
                         wc.keys = g->lkeys.as<unsigned int>(); wc.perm = g->lperm.as<unsigned int>();
@@ -780,7 +782,7 @@ int gcmcrt_destroy(gcmcrt_grid* g)
     cudaGetLastError();
     for (DevBuf* b : {&g->tab, &g->r64, &g->cth64, &g->ph64, &g->rc32, &g->thc32, &g->phc32, &g->T, &g->rho, &g->u, &g->v,
                       &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->prop, &g->reff, &g->vlos,
-                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->ev1, &g->ev2, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->s0[0], &g->s0[1],
+                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->ev1, &g->ev2, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
                       &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->flux, &g->ltot_out,
                       &g->value, &g->sigma, &g->image, &g->evcount})
         b->release();

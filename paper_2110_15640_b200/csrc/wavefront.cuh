@@ -33,6 +33,7 @@ struct WaveConst {
     const unsigned int* gen_mark;  // interact: events [gen_mark[0], gen_mark[1]) form this generation (device)
     int park_all;                  // last generation: survivors' next events go to the suspended list
     int chan_lo, c_fold;           // launch sort key window
+    float* flights;                // interact: per-warp lists of flights in progress [n_warps][kFlightFields][kStageSlots]
 };
 
 struct WaveCounters {
@@ -99,17 +100,15 @@ __device__ __forceinline__ void wave_record(const RunConst& rc, const EventBuf& 
     }
 }
 
-// Warp-collective: 32 flights that start together.  Marches every active lane to the end of its flight (radial
-// steps, cone / half-plane crossings batched), then records the next event or closes the packet.
+// Warp-collective: marches every lane whose status is RAY_FLYING / RAY_PARK for at most `budget` steps (radial steps,
+// cone / half-plane crossings batched across the warp).  Returns the number of loop steps spent (warp-uniform).
 template <int KSTEPS>
-__device__ __forceinline__ void wave_fly(const RunConst& rc, const EventBuf& ev, const SuspBuf& susp, int park_all,
-                                         const GeomSmem& gs, bool active, Ray& ray, float tau_t, const float* alpha_c,
-                                         float W, uint32_t chan_run, uint32_t pkt, uint32_t m_inter, WaveCounters& wcnt)
+__device__ __forceinline__ int wave_march(const RunConst& rc, const GeomSmem& gs, int& st, Ray& ray, float& tau,
+                                          float tau_t, const float* alpha_c, int budget, WaveCounters& wcnt)
 {
-    int st = active ? RAY_FLYING : RAY_NONE;
-    float tau = 0.f;
     unsigned int seg32 = 0;
-    for (int it = 0; it <= rc.geom.maxseg; it += KSTEPS) {
+    int it = 0;
+    for (; it < budget; it += KSTEPS) {
         const unsigned m_fly = __ballot_sync(kFullMask, st == RAY_FLYING);
         const unsigned m_park = __ballot_sync(kFullMask, st == RAY_PARK);
         if ((m_fly | m_park) == 0) break;
@@ -128,9 +127,17 @@ __device__ __forceinline__ void wave_fly(const RunConst& rc, const EventBuf& ev,
         }
     }
     wcnt.seg += seg32;
-    if (active && (st == RAY_FLYING || st == RAY_PARK)) st = RAY_STUCK;   // step budget exhausted
-    const bool surf_ev = active && st == RAY_SURFACE && rc.surface_albedo > 0.f;
-    const bool want = active && (st == RAY_LIMIT || surf_ev);
+    return it;
+}
+
+// Warp-collective: lanes with `fin` have ended their flight with status st: record the next event (or park the
+// packet), or close the packet.
+__device__ __forceinline__ void wave_close(const RunConst& rc, const EventBuf& ev, const SuspBuf& susp, int park_all,
+                                           bool fin, int st, const Ray& ray, float W, uint32_t chan_run, uint32_t pkt,
+                                           uint32_t m_inter, WaveCounters& wcnt)
+{
+    const bool surf_ev = fin && st == RAY_SURFACE && rc.surface_albedo > 0.f;
+    const bool want = fin && (st == RAY_LIMIT || surf_ev);
     float px = 0.f, py = 0.f, pz = 0.f, rx = ray.nx, ry = ray.ny, rz = ray.nz;
     if (want) {
         ray_position(ray, px, py, pz);
@@ -141,12 +148,69 @@ __device__ __forceinline__ void wave_fly(const RunConst& rc, const EventBuf& ev,
     }
     wave_record(rc, ev, susp, park_all, want, surf_ev ? EV_SURFACE : EV_MEDIUM, px, py, pz, rx, ry, rz, ray.nx, ray.ny,
                 ray.nz, W, pack_cell(ray.i, ray.j, ray.k), chan_run, pkt, m_inter, wcnt);
-    if (active && !want) {
+    if (fin && !want) {
         if (st == RAY_ESCAPE) { ++wcnt.esc; wcnt.escw += double(W); }
         else if (st == RAY_SURFACE) ++wcnt.surf;
         else ++wcnt.stuck;
         wave_finish_packet(rc, chan_run, pkt, m_inter + (rc.mode == 1 ? 1u : 0u));
     }
+}
+
+// Warp-collective: 32 flights that start together, each marched to its end.
+template <int KSTEPS>
+__device__ __forceinline__ void wave_fly(const RunConst& rc, const EventBuf& ev, const SuspBuf& susp, int park_all,
+                                         const GeomSmem& gs, bool active, Ray& ray, float tau_t, const float* alpha_c,
+                                         float W, uint32_t chan_run, uint32_t pkt, uint32_t m_inter, WaveCounters& wcnt)
+{
+    int st = active ? RAY_FLYING : RAY_NONE;
+    float tau = 0.f;
+    wave_march<KSTEPS>(rc, gs, st, ray, tau, tau_t, alpha_c, rc.geom.maxseg + 1, wcnt);
+    if (active && (st == RAY_FLYING || st == RAY_PARK)) st = RAY_STUCK;   // step budget exhausted
+    wave_close(rc, ev, susp, park_all, active, st, ray, W, chan_run, pkt, m_inter, wcnt);
+}
+
+// ---- flights in progress, set aside (interact kernel): a scattered packet's flight is short most of the time and
+// long now and then, so a warp marches its 32 fresh flights for a few steps only and moves the unfinished ones to a
+// per-warp list in global memory (L2-resident); 32 of those are then marched together for longer.  22 words per flight.
+constexpr int kFlightFields = 22;
+constexpr int kFirstRoundSteps = 4, kLongRoundSteps = 16;
+
+__device__ __forceinline__ void flight_save(float* fl, const Ray& r, float tau, float tau_t, float W, uint32_t chan_run,
+                                            uint32_t pkt, uint32_t m_inter, int st, int used)
+{
+    fl[0 * kStageSlots] = r.pcx; fl[1 * kStageSlots] = r.pcy; fl[2 * kStageSlots] = r.pcz;
+    fl[3 * kStageSlots] = r.nx; fl[4 * kStageSlots] = r.ny; fl[5 * kStageSlots] = r.nz;
+    fl[6 * kStageSlots] = r.d2; fl[7 * kStageSlots] = r.d2lo; fl[8 * kStageSlots] = r.u;
+    fl[9 * kStageSlots] = r.u_rad; fl[10 * kStageSlots] = r.u_lat; fl[11 * kStageSlots] = r.u_lon;
+    fl[12 * kStageSlots] = r.alpha; fl[13 * kStageSlots] = r.alpha_n;
+    fl[14 * kStageSlots] = tau; fl[15 * kStageSlots] = tau_t; fl[16 * kStageSlots] = W;
+    fl[17 * kStageSlots] = __uint_as_float(pack_cell(r.i, r.j, r.k));
+    const uint32_t steps = uint32_t(r.rad_step + 1) | uint32_t(r.lat_step + 1) << 2 | uint32_t(r.lon_step + 1) << 4 |
+                           uint32_t(st == RAY_PARK) << 6 | uint32_t(used) << 8;
+    fl[18 * kStageSlots] = __uint_as_float(steps);
+    fl[19 * kStageSlots] = __uint_as_float(chan_run); fl[20 * kStageSlots] = __uint_as_float(pkt);
+    fl[21 * kStageSlots] = __uint_as_float(m_inter);
+}
+
+__device__ __forceinline__ void flight_load(const float* fl, const RunConst& rc, const GeomSmem& gs, Ray& r, float& tau,
+                                            float& tau_t, float& W, uint32_t& chan_run, uint32_t& pkt, uint32_t& m_inter,
+                                            int& st, int& used, const float*& alpha_c)
+{
+    r.pcx = fl[0 * kStageSlots]; r.pcy = fl[1 * kStageSlots]; r.pcz = fl[2 * kStageSlots];
+    r.nx = fl[3 * kStageSlots]; r.ny = fl[4 * kStageSlots]; r.nz = fl[5 * kStageSlots];
+    r.d2 = fl[6 * kStageSlots]; r.d2lo = fl[7 * kStageSlots]; r.u = fl[8 * kStageSlots];
+    r.u_rad = fl[9 * kStageSlots]; r.u_lat = fl[10 * kStageSlots]; r.u_lon = fl[11 * kStageSlots];
+    r.alpha = fl[12 * kStageSlots]; r.alpha_n = fl[13 * kStageSlots];
+    tau = fl[14 * kStageSlots]; tau_t = fl[15 * kStageSlots]; W = fl[16 * kStageSlots];
+    unpack_cell(__float_as_uint(fl[17 * kStageSlots]), r.i, r.j, r.k);
+    const uint32_t steps = __float_as_uint(fl[18 * kStageSlots]);
+    r.rad_step = int(steps & 3u) - 1; r.lat_step = int((steps >> 2) & 3u) - 1; r.lon_step = int((steps >> 4) & 3u) - 1;
+    st = (steps >> 6) & 1u ? RAY_PARK : RAY_FLYING;
+    used = int(steps >> 8);
+    chan_run = __float_as_uint(fl[19 * kStageSlots]); pkt = __float_as_uint(fl[20 * kStageSlots]);
+    m_inter = __float_as_uint(fl[21 * kStageSlots]);
+    alpha_c = rc.alpha + (size_t)(rc.chan_begin + int(chan_run)) * rc.geom.alpha_stride;
+    r.colp = ray_column(gs, alpha_c, r.j, r.k);
 }
 
 // O3: uniform point on the star-facing TOA disc from Philox block (event 0, purpose 0), and its entry column
@@ -301,7 +365,8 @@ wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, con
     WaveCounters wcnt;
     const unsigned int begin = wc.gen_mark[0], end = min(wc.gen_mark[1], ev.cap);
     const unsigned int warp0 = begin + ((blockIdx.x * blockDim.x + threadIdx.x) & ~31u);
-    int staged = 0;   // warp-uniform
+    int staged = 0, in_flight = 0;   // warp-uniform list lengths
+    float* flights = wc.flights + (size_t)((blockIdx.x * blockDim.x + threadIdx.x) >> 5) * (kFlightFields * kStageSlots);
 
     for (unsigned int base = warp0;; base += gridDim.x * blockDim.x) {
         const bool more = base < end;   // warp-uniform
@@ -366,42 +431,61 @@ wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, con
             staged += __popc(m_s);
             __syncwarp();
         }
-        // ---------------- phase 2: a full warp of survivors flies to its next event ----------------
-        while (staged >= 32 || (!more && staged > 0)) {
-            const int n_take = min(staged, 32);
+        // ---------------- phase 2: full warps of survivors start their flights; phase 3: long flights ----------------
+        for (;;) {
+            const bool do_long = in_flight >= 32 || (!more && staged == 0 && in_flight > 0);
+            const bool do_new = !do_long && (staged >= 32 || (!more && staged > 0));
+            if (!do_long && !do_new) break;
+            const int n_take = min(do_long ? in_flight : staged, 32);
             const bool active = lane_id() < n_take;
             Ray ray{};
-            float tau_t = 0.f, W = 0.f;
+            float tau = 0.f, tau_t = 0.f, W = 0.f;
             uint32_t chan_run = 0, pkt = 0, m_new = 0;
+            int st = RAY_NONE, used = 0;
             const float* alpha_c = rc.alpha;
-            if (active) {
-                const float* sl = stage + (staged - n_take) + lane_id();
-                const float px = sl[0 * kStageSlots], py = sl[1 * kStageSlots], pz = sl[2 * kStageSlots];
-                W = sl[3 * kStageSlots];
-                float nx = sl[4 * kStageSlots], ny = sl[5 * kStageSlots], nz = sl[6 * kStageSlots];
-                const float ct = sl[7 * kStageSlots], zpsi = sl[8 * kStageSlots];
-                tau_t = sl[9 * kStageSlots];
-                const uint32_t cellp = __float_as_uint(sl[10 * kStageSlots]), meta = __float_as_uint(sl[11 * kStageSlots]);
-                pkt = __float_as_uint(sl[12 * kStageSlots]); m_new = __float_as_uint(sl[13 * kStageSlots]);
-                const uint32_t kind = meta & 3u;
-                chan_run = meta >> 8;
-                int i, j, k;
-                unpack_cell(cellp, i, j, k);
-                if (kind == EV_EMIT) {   // isotropic emission direction (Eq. 2), as the persistent kernel writes it
-                    const float ns = sqrtf(fmaxf(0.f, 1.0f - ct * ct));
-                    float sp, cp;
-                    sincospif(2.0f * zpsi, &sp, &cp);
-                    nx = ns * cp; ny = ns * sp; nz = ct;
-                } else {
-                    rotate_dir(nx, ny, nz, ct, zpsi);   // about the incoming direction, or the surface normal (Eq. 4)
-                    if (kind == EV_SURFACE) i = 0;
+            if (do_long) {
+                if (active) flight_load(flights + (in_flight - n_take) + lane_id(), rc, gs, ray, tau, tau_t, W, chan_run, pkt,
+                                        m_new, st, used, alpha_c);
+                __syncwarp();
+                in_flight -= n_take;
+            } else {
+                if (active) {
+                    const float* sl = stage + (staged - n_take) + lane_id();
+                    const float px = sl[0 * kStageSlots], py = sl[1 * kStageSlots], pz = sl[2 * kStageSlots];
+                    W = sl[3 * kStageSlots];
+                    float nx = sl[4 * kStageSlots], ny = sl[5 * kStageSlots], nz = sl[6 * kStageSlots];
+                    const float ct = sl[7 * kStageSlots], zpsi = sl[8 * kStageSlots];
+                    tau_t = sl[9 * kStageSlots];
+                    const uint32_t cellp = __float_as_uint(sl[10 * kStageSlots]), meta = __float_as_uint(sl[11 * kStageSlots]);
+                    pkt = __float_as_uint(sl[12 * kStageSlots]); m_new = __float_as_uint(sl[13 * kStageSlots]);
+                    const uint32_t kind = meta & 3u;
+                    chan_run = meta >> 8;
+                    int i, j, k;
+                    unpack_cell(cellp, i, j, k);
+                    if (kind == EV_EMIT) {   // isotropic emission direction (Eq. 2), as the persistent kernel writes it
+                        const float ns = sqrtf(fmaxf(0.f, 1.0f - ct * ct));
+                        float sp, cp;
+                        sincospif(2.0f * zpsi, &sp, &cp);
+                        nx = ns * cp; ny = ns * sp; nz = ct;
+                    } else {
+                        rotate_dir(nx, ny, nz, ct, zpsi);   // about the incoming direction, or the surface normal (Eq. 4)
+                        if (kind == EV_SURFACE) i = 0;
+                    }
+                    alpha_c = rc.alpha + (size_t)(rc.chan_begin + int(chan_run)) * rc.geom.alpha_stride;
+                    ray_init(ray, gs, px, py, pz, nx, ny, nz, i, j, k, alpha_c);
+                    st = RAY_FLYING;
                 }
-                alpha_c = rc.alpha + (size_t)(rc.chan_begin + int(chan_run)) * rc.geom.alpha_stride;
-                ray_init(ray, gs, px, py, pz, nx, ny, nz, i, j, k, alpha_c);
+                __syncwarp();
+                staged -= n_take;
             }
+            used += wave_march<KSTEPS>(rc, gs, st, ray, tau, tau_t, alpha_c, do_long ? kLongRoundSteps : kFirstRoundSteps, wcnt);
+            bool unfinished = active && (st == RAY_FLYING || st == RAY_PARK);
+            if (unfinished && used > rc.geom.maxseg) { st = RAY_STUCK; unfinished = false; }
+            wave_close(rc, ev, susp, wc.park_all, active && !unfinished, st, ray, W, chan_run, pkt, m_new, wcnt);
+            const unsigned m_u = __ballot_sync(kFullMask, unfinished);
+            if (unfinished) flight_save(flights + in_flight + rank_in_mask(m_u), ray, tau, tau_t, W, chan_run, pkt, m_new, st, used);
+            in_flight += __popc(m_u);
             __syncwarp();
-            staged -= n_take;
-            wave_fly<KSTEPS>(rc, ev, susp, wc.park_all, gs, active, ray, tau_t, alpha_c, W, chan_run, pkt, m_new, wcnt);
         }
         if (!more) break;
     }

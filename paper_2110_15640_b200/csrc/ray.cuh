@@ -124,8 +124,16 @@ __device__ __forceinline__ void ray_setup_lat(Ray& r, const GeomSmem& s)
     float best = kInf;
     int step = 0;
     if (s.nlat > 1) {
-        if (r.j > 0) ray_cone_roots(r, s.cth[r.j], -1, best, step);                // lower-colatitude edge
-        if (r.j + 1 < s.nlat) ray_cone_roots(r, s.cth[r.j + 1], +1, best, step);   // pole edges are no surfaces
+        // d cos(theta) / du has the sign of n_z d^2 - z_c u, which changes at most once along a line: the ray can
+        // only reach the cone it is moving toward unless it turns first, so the other cone is asked only when the
+        // first has no crossing ahead (pole edges are no surfaces)
+        const bool up = fmaf(r.nz, r.d2, -r.pcz * r.u) > 0.0f;   // colatitude decreasing
+        const int e1 = up ? r.j : r.j + 1, s1 = up ? -1 : 1;
+        if (e1 > 0 && e1 < s.nlat) ray_cone_roots(r, s.cth[e1], s1, best, step);
+        if (step == 0) {
+            const int e2 = up ? r.j + 1 : r.j;
+            if (e2 > 0 && e2 < s.nlat) ray_cone_roots(r, s.cth[e2], -s1, best, step);
+        }
     }
     r.u_lat = best;
     r.lat_step = step;
@@ -240,7 +248,13 @@ __device__ __forceinline__ void ray_lateral(Ray& r, const GeomSmem& s, const flo
     } else {
         r.k += r.lon_step;
         r.k = (r.k < 0) ? r.k + s.nlon : (r.k >= s.nlon ? r.k - s.nlon : r.k);
-        ray_setup_lon(r, s);
+        // the azimuth of a straight line is monotonic: the next half-plane lies in the same direction
+        float best = kInf;
+        int step = 0;
+        const int e = r.lon_step > 0 ? r.k + 1 : r.k;
+        ray_plane_root(r, s.cph[e], s.sph[e], r.lon_step, best, step);
+        r.u_lon = best;
+        r.lon_step = step == 0 ? r.lon_step : step;
     }
     ray_load_alpha(r, s, alpha_tab);
 }

@@ -269,6 +269,48 @@ def test_event_buffer_overflow_suspends_and_resumes(gpu, orc, monkeypatch):
     assert small["counters"]["events"] == ref["counters"]["events"]
 
 
+@pytest.mark.parametrize("mode", ["albedo", "emission"])
+def test_wavefront_and_persistent_transport_carry_packets_identically(gpu, monkeypatch, mode):
+    """The generation kernels (wavefront.cuh) and the persistent kernel run the same per-packet arithmetic: with
+    0, 2 and 8 generations per pass every packet makes exactly the same number of events, and the spectra agree to
+    the rounding of the summation order."""
+    if mode == "albedo":
+        grid, opac, prm = wl.cfg2(nlon=16, nlat=8, nlev=20, nbands=2, ng=3, packets=30000)
+    else:
+        grid, opac, prm = wl.cfg3(nlon=16, nlat=8, nlev=20, nbands=1, ng=4, packets=30000, n_obs=3)
+    runs = []
+    for tune in ("16,1,0,4", "16,1,2,4", "16,1,8,4", "16,4,8,16"):
+        monkeypatch.setenv("GCMCRT_TUNE", tune)
+        runs.append(_gpu_run(gpu, grid, opac, prm, mode, want_event_count=True))
+    ref = runs[0]
+    for r in runs[1:]:
+        assert np.array_equal(r["event_count"], ref["event_count"])
+        assert r["counters"]["events"] == ref["counters"]["events"]
+        for k in ("packets_escaped", "packets_absorbed", "packets_surface", "packets_stuck", "rays_peel"):
+            assert r["counters"][k] == ref["counters"][k], k
+        assert r["counters"]["segments_transport"] == ref["counters"]["segments_transport"]
+        assert np.allclose(r["flux_sum"], ref["flux_sum"], rtol=2e-5, atol=1e-12 * np.abs(ref["flux_sum"]).max())
+
+
+def test_wavefront_with_surface_and_tiny_event_buffer(gpu, orc, monkeypatch):
+    """Lambert surface events, mixed Rayleigh / HG scatterers and an event buffer far smaller than one generation:
+    packets parked by the generation kernels are resumed by the persistent kernel in later passes."""
+    grid, opac = wl.uniform_medium(6, 4, 5, 1.0e6, 1.3e6, 2.0 / 0.3e6, 0.9, g=0.4, pgas=0.3, n_chan=2, surface_albedo=0.6)
+    prm = wl.default_params(packets_per_channel=20000, seed=5, obs_dir=[[1.0, 0, 0], [0.6, 0, 0.8]])
+    monkeypatch.setenv("GCMCRT_TUNE", "16,1,0,4")
+    ref = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+    monkeypatch.setenv("GCMCRT_TUNE", "16,1,3,4")
+    monkeypatch.setenv("GCMCRT_EVENT_CAP", "6000")
+    small = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+    assert small["counters"]["passes"] > 5
+    assert np.array_equal(small["event_count"], ref["event_count"])
+    assert small["counters"]["events"] == ref["counters"]["events"]
+    assert small["counters"]["packets_surface"] == ref["counters"]["packets_surface"] > 0
+    assert np.allclose(small["flux_sum"], ref["flux_sum"], rtol=2e-5)
+    o = orc.run_albedo(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
+    _check_parity(orc, small, o, "albedo")
+
+
 def test_packet_and_channel_subranges_compose(gpu):
     grid, opac, prm = wl.cfg2(nlon=8, nlat=4, nlev=10, nbands=1, ng=4, packets=20000)
     full = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)

@@ -75,7 +75,7 @@ struct gcmcrt_grid {
     DevBuf Lcell, Lcum, Ltot;
 
     // workspace
-    DevBuf ev0, ev1, ev2, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, flights, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount;
+    DevBuf ev0, ev1, ev2, evkeys, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, flights, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount;
     unsigned int ev_cap = 0;
     int n_threads_resident = 0;
     // GCMCRT_TUNE="service,lateral,gens,batch_div": lanes waiting before the persistent kernel serves them; lanes parked at
@@ -244,6 +244,7 @@ int ensure_workspace(gcmcrt_grid* g)
     CUDA_TRY(g, g->ev1.ensure(size_t(g->ev_cap) * sizeof(float4)));
     CUDA_TRY(g, g->ev2.ensure(size_t(g->ev_cap) * sizeof(float4)));
     CUDA_TRY(g, g->perm.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));
+    CUDA_TRY(g, g->evkeys.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));
     CUDA_TRY(g, g->ctrl.ensure(sizeof(PassCtrl)));
     CUDA_TRY(g, g->counters.ensure(sizeof(DevCounters)));
     if (!g->h_ctrl) CUDA_TRY(g, cudaMallocHost((void**)&g->h_ctrl, sizeof(PassCtrl)));
@@ -367,6 +368,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         CUDA_TRY(g, g->s2[b].ensure(susp_cap * sizeof(uint4)));
     }
     EventBuf ev;
+    std::memset(&ev, 0, sizeof ev);
     ev.e0 = g->ev0.as<float4>(); ev.e1 = g->ev1.as<float4>(); ev.e2 = g->ev2.as<float4>();
     ev.count = &ctrl->ev_count;
     ev.cap = g->ev_cap;
@@ -454,6 +456,9 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             CUDA_TRY(g, g->hist.ensure(size_t(sp.nbins) * sizeof(unsigned int)));
             CUDA_TRY(g, g->tile_sums.ensure(size_t(sp.n_tiles) * sizeof(unsigned int)));
             sp.e2 = ev.e2; sp.count = ev.count; sp.cap = ev.cap;
+            sp.keys = g->evkeys.as<unsigned int>();
+            ev.keys = g->evkeys.as<unsigned int>(); ev.hist = emission ? nullptr : g->hist.as<unsigned int>();
+            ev.c_fold = sp.c_fold; ev.nlev = g->nlev; ev.nlat = g->nlat; ev.ncell = g->ncell;
             sp.hist = g->hist.as<unsigned int>(); sp.tile_sums = g->tile_sums.as<unsigned int>();
             sp.perm = g->perm.as<unsigned int>();
             sp.nlev = g->nlev; sp.nlat = g->nlat; sp.ncell = g->ncell;
@@ -507,6 +512,10 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
             unsigned long long n_fresh = 0, tail_items = total_items;
             const unsigned long long chan_lo_pass = item0 / std::max<size_t>(n_pkt, 1);
+            if (rc.n_obs_run > 0) {   // the event sort's histogram is filled while the records are written
+                sp.chan_lo = ev.chan_lo = int(std::min<unsigned long long>(chan_lo_pass, (unsigned long long)ncr));
+                CUDA_TRY(g, cudaMemsetAsync(sp.hist, 0, size_t(sp.nbins) * sizeof(unsigned int), s));
+            }
             if (n_gen > 0) {
                 // a pass that inherited a long suspended list only drains it (keeps the list bounded, see susp_cap)
                 n_fresh = leftover > g->ev_cap / 2 ? 0 : std::min<unsigned long long>(std::min<unsigned long long>(batch, g->ev_cap / 2), total_items - item0);
@@ -549,9 +558,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
             if (rc.n_obs_run > 0) {
                 // counting sort of this pass's events by (channel, cell): sort.cuh
-                sp.chan_lo = int(std::min<unsigned long long>(n_gen > 0 ? chan_lo_pass : item0 / std::max<size_t>(n_pkt, 1), (unsigned long long)ncr));
-                CUDA_TRY(g, cudaMemsetAsync(sp.hist, 0, size_t(sp.nbins) * sizeof(unsigned int), s));
-                ev_hist_kernel<<<g->sm_count * 8, 256, 0, s>>>(sp);
+                if (!ev.hist) { ev_hist_kernel<<<g->sm_count * 8, 256, 0, s>>>(sp); ++g->launches; }
                 scan_reduce_kernel<<<sp.n_tiles, kScanThreads, 0, s>>>(sp);
                 scan_tiles_kernel<<<1, 1024, 0, s>>>(sp);
                 scan_apply_kernel<<<sp.n_tiles, kScanThreads, 0, s>>>(sp);
@@ -562,7 +569,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             CUDA_TRY(g, cudaEventRecord(g->tev[3], s));
             CUDA_TRY(g, cudaGetLastError());
             ++passes;
-            g->launches += rc.n_obs_run > 0 ? 7 : 1;
+            g->launches += rc.n_obs_run > 0 ? 6 : 1;
             CUDA_TRY(g, cudaMemcpyAsync(g->h_ctrl, ctrl, sizeof(PassCtrl), cudaMemcpyDeviceToHost, s));
             CUDA_TRY(g, cudaStreamSynchronize(s));
             {
@@ -782,7 +789,7 @@ int gcmcrt_destroy(gcmcrt_grid* g)
     cudaGetLastError();
     for (DevBuf* b : {&g->tab, &g->r64, &g->cth64, &g->ph64, &g->rc32, &g->thc32, &g->phc32, &g->T, &g->rho, &g->u, &g->v,
                       &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->prop, &g->reff, &g->vlos,
-                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->ev1, &g->ev2, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
+                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->ev1, &g->ev2, &g->evkeys, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
                       &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->flux, &g->ltot_out,
                       &g->value, &g->sigma, &g->image, &g->evcount})
         b->release();

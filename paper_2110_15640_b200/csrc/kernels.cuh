@@ -34,6 +34,13 @@ struct EventBuf {
     unsigned int* count;
     unsigned int cap;
     unsigned int soft_cap;
+    // first half of the counting sort by (channel, cell) (sort.cuh), done while the record is written: the key is kept
+    // and its histogram bin counted, so that the sort itself is one scan and one scatter.  NULL when no peel follows.
+    unsigned int* keys;   // [cap]
+    unsigned int* hist;   // [c_fold * ncell], zeroed by the host before the pass; NULL: the host runs ev_hist_kernel
+                          // instead (emission: events pile up in a few bright cells and the contended atomics are
+                          // cheaper in a kernel of their own than inside the emit / interact kernels)
+    int chan_lo, c_fold, nlev, nlat, ncell;
 };
 
 __device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slot, float px, float py, float pz, float W,
@@ -43,6 +50,13 @@ __device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slo
     ev.e0[slot] = make_float4(px, py, pz, W);
     ev.e1[slot] = make_float4(nx, ny, nz, 0.f);
     ev.e2[slot] = make_float4(__uint_as_float(m_inter), __uint_as_float(cellp), __uint_as_float(meta), __uint_as_float(pkt));
+    if (ev.keys) {
+        const int i = cellp & 1023, j = (cellp >> 10) & 1023, k = cellp >> 20;
+        const unsigned int chan = (unsigned int)min(max(int(meta >> 8) - ev.chan_lo, 0), ev.c_fold - 1);
+        const unsigned int key = chan * (unsigned int)ev.ncell + (unsigned int)((k * ev.nlat + j) * ev.nlev + i);
+        ev.keys[slot] = key;
+        if (ev.hist) atomicAdd(ev.hist + key, 1u);
+    }
 }
 
 // Packets suspended because the event buffer filled up; resumed by the next pass.

@@ -74,6 +74,9 @@ struct Ray {
     float alpha_n;        // prefetched extinction of the radial neighbour (i + rad_step) in the same column
     const float* colp;    // extinction column of the current (j, k): colp[i], guard entries at colp[-1], colp[nlev]
     int i, j, k;          // cell
+    int ish;              // index of the shell the ray crosses next: i while moving inward, i + 1 outward
+    int i_turn;           // cell in which an inward ray turns outward (its inner shell lies inside the impact
+                          // parameter); below every cell index when the ray never turns inside the grid
     int rad_step, lat_step, lon_step;
 };
 
@@ -83,19 +86,31 @@ __device__ __forceinline__ float shell_q(const Ray& r, const GeomSmem& s, int id
     return (R2.x - r.d2) + (R2.y - r.d2lo);
 }
 
-// Next shell crossing at the start of a ray.
+// Next shell crossing at the start of a ray, and where an inward ray will turn.
 __device__ __forceinline__ void ray_setup_rad(Ray& r, const GeomSmem& s)
 {
+    r.i_turn = -2;
     if (r.u < 0.0f) {  // inward phase: the inner shell is hit iff it lies outside the impact parameter
         const float q = shell_q(r, s, r.i);
         if (q > 0.0f) {
             r.u_rad = -sqrt_approx(q);
             r.rad_step = -1;
+            r.ish = r.i;
+            // innermost shell the ray reaches = smallest k in [0, i] with R_k^2 - d^2 > 0 (same double-float
+            // expression as every shell root, so the march never asks for a shell it decided it cannot reach);
+            // the ray turns in the cell below it (k = 0: it reaches the lower boundary instead)
+            int lo = 0, hi = r.i;   // invariant: shell hi is reached
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (shell_q(r, s, mid) > 0.0f) hi = mid; else lo = mid + 1;
+            }
+            r.i_turn = hi - 1;
             return;
         }
     }
     r.u_rad = sqrt_approx(fmaxf(shell_q(r, s, r.i + 1), 0.0f));
     r.rad_step = 1;
+    r.ish = r.i + 1;
 }
 
 __device__ __forceinline__ void ray_cone_roots(const Ray& r, float c, int step, float& best, int& best_step)
@@ -228,12 +243,9 @@ __device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, f
         return RAY_ESCAPE;
     }
     r.alpha = r.alpha_n;   // prefetched for exactly this cell
-    float q = shell_q(r, s, r.i + ((r.rad_step + 1) >> 1));
-    if (r.rad_step < 0 && !(q > 0.0f)) {   // the inner shell lies inside the impact parameter: turn outward
-        r.rad_step = 1;
-        q = shell_q(r, s, r.i + 1);
-    }
-    const float sq = sqrt_approx(fmaxf(q, 0.0f));
+    if (r.i == r.i_turn) r.rad_step = 1;   // the inner shell of this cell lies inside the impact parameter
+    else r.ish += r.rad_step;              // (turning, the shell just crossed inward is the next one outward)
+    const float sq = sqrt_approx(fmaxf(shell_q(r, s, r.ish), 0.0f));
     r.u_rad = __int_as_float(__float_as_int(sq) | (r.rad_step & 0x80000000));
     r.alpha_n = __ldg(r.colp + (r.i + r.rad_step));
     return RAY_FLYING;

@@ -171,8 +171,8 @@ __device__ __forceinline__ void wave_fly(const RunConst& rc, const EventBuf& ev,
 
 // ---- flights in progress, set aside (interact kernel): a scattered packet's flight is short most of the time and
 // long now and then, so a warp marches its 32 fresh flights for a few steps only and moves the unfinished ones to a
-// per-warp list in global memory (L2-resident); 32 of those are then marched together for longer.  22 words per flight.
-constexpr int kFlightFields = 22;
+// per-warp list in global memory (L2-resident); 32 of those are then marched together for longer.  23 words per flight.
+constexpr int kFlightFields = 23;
 constexpr int kFirstRoundSteps = 4, kLongRoundSteps = 16;
 
 __device__ __forceinline__ void flight_save(float* fl, const Ray& r, float tau, float tau_t, float W, uint32_t chan_run,
@@ -190,6 +190,7 @@ __device__ __forceinline__ void flight_save(float* fl, const Ray& r, float tau, 
     fl[18 * kStageSlots] = __uint_as_float(steps);
     fl[19 * kStageSlots] = __uint_as_float(chan_run); fl[20 * kStageSlots] = __uint_as_float(pkt);
     fl[21 * kStageSlots] = __uint_as_float(m_inter);
+    fl[22 * kStageSlots] = __int_as_float(r.i_turn);
 }
 
 __device__ __forceinline__ void flight_load(const float* fl, const RunConst& rc, const GeomSmem& gs, Ray& r, float& tau,
@@ -209,6 +210,8 @@ __device__ __forceinline__ void flight_load(const float* fl, const RunConst& rc,
     used = int(steps >> 8);
     chan_run = __float_as_uint(fl[19 * kStageSlots]); pkt = __float_as_uint(fl[20 * kStageSlots]);
     m_inter = __float_as_uint(fl[21 * kStageSlots]);
+    r.i_turn = __float_as_int(fl[22 * kStageSlots]);
+    r.ish = r.rad_step > 0 ? r.i + 1 : r.i;
     alpha_c = rc.alpha + (size_t)(rc.chan_begin + int(chan_run)) * rc.geom.alpha_stride;
     r.colp = ray_column(gs, alpha_c, r.j, r.k);
 }

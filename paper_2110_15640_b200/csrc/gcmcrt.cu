@@ -352,7 +352,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     const size_t smem_t = size_t(g->tab_floats) * sizeof(float);
     int occ_t = 0, occ_p = 0;
     auto tk = transport_kernel<4>;
-    auto pk = peel_kernel<4>;
+    auto pk = peel_kernel<8>;
     CUDA_TRY(g, cudaFuncSetAttribute(tk, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_t)));
     CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_t, tk, kTransportThreads, smem_t));
     if (occ_t < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
@@ -466,7 +466,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         // ---- wavefront kernels (wavefront.cuh): launch geometry and the launch-order sort of albedo runs
         const int n_gen = g->tune[2];
         auto k_keys = wave_launch_keys_kernel;
-        auto k_first = wave_first_flight_kernel<4>;
+        auto k_first = wave_first_flight_kernel<8>;
         auto k_emit = wave_emit_kernel;
         auto k_inter = wave_interact_kernel<4>;
         const size_t smem_w = smem_t;

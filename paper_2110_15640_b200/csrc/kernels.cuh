@@ -516,7 +516,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                 if (is_ev) {
                     float px, py, pz;
                     ray_position(pk.ray, px, py, pz);
-                    const uint32_t cellp = pack_cell(pk.ray.i, pk.ray.j, pk.ray.k);
+                    const uint32_t cellp = pack_cell(st == LS_EV_SURFACE ? 0 : pk.ray.i, pk.ray.j, pk.ray.k);
                     const uint32_t kind = st == LS_EV_MEDIUM ? EV_MEDIUM : (st == LS_EV_EMIT ? EV_EMIT : EV_SURFACE);
                     if (!have_slot) {
                         // event buffer full: park the packet for the next pass
@@ -757,12 +757,10 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
                             st = RAY_FLYING;
                         }
                     }
-#pragma unroll
-                    for (int s = 0; s < KSTEPS; ++s) {
-                        if (st == RAY_FLYING) {
-                            ++seg32;
-                            st = ray_step(ray, gs, tau, rc.tau_cut);
-                        }
+#pragma unroll 1
+                    for (int s = 0; s < KSTEPS && st == RAY_FLYING; ++s) {   // lanes in flight step together
+                        ++seg32;
+                        st = ray_step(ray, gs, tau, rc.tau_cut);
                     }
                 }
                 c_seg += seg32;

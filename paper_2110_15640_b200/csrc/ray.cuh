@@ -38,6 +38,7 @@ struct GeomParams {
 };
 
 struct GeomSmem {
+    uint32_t r2_saddr; // shared-space address of R2: the shell roots load it with one LDS.64 and no generic-address set-up
     const float2* R2;  // (high, low) parts of R_k^2
     const float *R, *qcube, *cth, *cph, *sph, *ph;
     int nlev, nlat, nlon, col_stride;
@@ -49,6 +50,7 @@ __device__ __forceinline__ GeomSmem load_geom(const GeomParams& g, float* smem)
     GeomSmem s;
     s.nlev = g.nlev; s.nlat = g.nlat; s.nlon = g.nlon; s.col_stride = g.col_stride;
     s.R2 = reinterpret_cast<const float2*>(smem);
+    s.r2_saddr = static_cast<uint32_t>(__cvta_generic_to_shared(smem));
     s.R = smem + 2 * (g.nlev + 1);
     s.qcube = s.R + (g.nlev + 1);
     s.cth = s.qcube + g.nlev;
@@ -72,7 +74,8 @@ struct Ray {
     float u_rad, u_lat, u_lon;  // next crossing of each face family
     float alpha;          // extinction of the current cell
     float alpha_n;        // prefetched extinction of the radial neighbour (i + rad_step) in the same column
-    const float* colp;    // extinction column of the current (j, k): colp[i], guard entries at colp[-1], colp[nlev]
+    const float* pn;      // address of the extinction prefetched next, in the column of (j, k): column + i + rad_step
+                          // (every column has a guard entry below level 0 and above level nlev - 1)
     int i, j, k;          // cell
     int ish;              // index of the shell the ray crosses next: i while moving inward, i + 1 outward
     int i_turn;           // cell in which an inward ray turns outward (its inner shell lies inside the impact
@@ -82,8 +85,9 @@ struct Ray {
 
 __device__ __forceinline__ float shell_q(const Ray& r, const GeomSmem& s, int idx)
 {
-    const float2 R2 = s.R2[idx];
-    return (R2.x - r.d2) + (R2.y - r.d2lo);
+    float hi, lo;
+    asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(hi), "=f"(lo) : "r"(s.r2_saddr + 8u * uint32_t(idx)));
+    return (hi - r.d2) + (lo - r.d2lo);
 }
 
 // Next shell crossing at the start of a ray, and where an inward ray will turn.
@@ -187,9 +191,10 @@ __device__ __forceinline__ const float* ray_column(const GeomSmem& s, const floa
 // loop consumes alpha one iteration after the load was issued, so the gather latency overlaps a full step.
 __device__ __forceinline__ void ray_load_alpha(Ray& r, const GeomSmem& s, const float* __restrict__ alpha_tab)
 {
-    r.colp = ray_column(s, alpha_tab, r.j, r.k);
-    r.alpha = __ldg(r.colp + r.i);
-    r.alpha_n = __ldg(r.colp + (r.i + r.rad_step));
+    const float* colp = ray_column(s, alpha_tab, r.j, r.k);
+    r.alpha = __ldg(colp + r.i);
+    r.pn = colp + (r.i + r.rad_step);
+    r.alpha_n = __ldg(r.pn);
 }
 
 // Start a ray at p with unit direction n inside cell (i,j,k).
@@ -237,17 +242,14 @@ __device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, f
     r.u = fmaxf(un, r.u);
     if (r.u_rad > ul) return RAY_PARK;  // ties: shells first (C1)
     r.i += r.rad_step;
-    if ((unsigned)r.i >= (unsigned)s.nlev) {
-        if (r.i < 0) { r.i = 0; return RAY_SURFACE; }
-        r.i = s.nlev - 1;
-        return RAY_ESCAPE;
-    }
+    if ((unsigned)r.i >= (unsigned)s.nlev) return r.i < 0 ? RAY_SURFACE : RAY_ESCAPE;   // r.i is left outside the grid
     r.alpha = r.alpha_n;   // prefetched for exactly this cell
     if (r.i == r.i_turn) r.rad_step = 1;   // the inner shell of this cell lies inside the impact parameter
     else r.ish += r.rad_step;              // (turning, the shell just crossed inward is the next one outward)
     const float sq = sqrt_approx(fmaxf(shell_q(r, s, r.ish), 0.0f));
     r.u_rad = __int_as_float(__float_as_int(sq) | (r.rad_step & 0x80000000));
-    r.alpha_n = __ldg(r.colp + (r.i + r.rad_step));
+    r.pn += r.rad_step;   // also right at the turn: the prefetch pointed at this cell, the next one is one up
+    r.alpha_n = __ldg(r.pn);
     return RAY_FLYING;
 }
 

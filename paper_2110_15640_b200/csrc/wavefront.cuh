@@ -118,12 +118,10 @@ __device__ __forceinline__ int wave_march(const RunConst& rc, const GeomSmem& gs
                 st = RAY_FLYING;
             }
         }
-#pragma unroll
-        for (int s = 0; s < KSTEPS; ++s) {
-            if (st == RAY_FLYING) {
-                ++seg32;
-                st = ray_step(ray, gs, tau, tau_t);
-            }
+#pragma unroll 1
+        for (int s = 0; s < KSTEPS && st == RAY_FLYING; ++s) {   // lanes in flight step together
+            ++seg32;
+            st = ray_step(ray, gs, tau, tau_t);
         }
     }
     wcnt.seg += seg32;
@@ -147,7 +145,7 @@ __device__ __forceinline__ void wave_close(const RunConst& rc, const EventBuf& e
         }
     }
     wave_record(rc, ev, susp, park_all, want, surf_ev ? EV_SURFACE : EV_MEDIUM, px, py, pz, rx, ry, rz, ray.nx, ray.ny,
-                ray.nz, W, pack_cell(ray.i, ray.j, ray.k), chan_run, pkt, m_inter, wcnt);
+                ray.nz, W, pack_cell(surf_ev ? 0 : ray.i, ray.j, ray.k), chan_run, pkt, m_inter, wcnt);
     if (fin && !want) {
         if (st == RAY_ESCAPE) { ++wcnt.esc; wcnt.escw += double(W); }
         else if (st == RAY_SURFACE) ++wcnt.surf;
@@ -213,7 +211,7 @@ __device__ __forceinline__ void flight_load(const float* fl, const RunConst& rc,
     r.i_turn = __float_as_int(fl[22 * kStageSlots]);
     r.ish = r.rad_step > 0 ? r.i + 1 : r.i;
     alpha_c = rc.alpha + (size_t)(rc.chan_begin + int(chan_run)) * rc.geom.alpha_stride;
-    r.colp = ray_column(gs, alpha_c, r.j, r.k);
+    r.pn = ray_column(gs, alpha_c, r.j, r.k) + (r.i + r.rad_step);
 }
 
 // O3: uniform point on the star-facing TOA disc from Philox block (event 0, purpose 0), and its entry column

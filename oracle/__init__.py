@@ -34,7 +34,8 @@ class _Params(C.Structure):
                 ("seed", C.c_uint64), ("max_events", C.c_int), ("scatter_on", C.c_int),
                 ("doppler_on", C.c_int), ("doppler_halfwidth", C.c_int),
                 ("emission_bias", C.c_double), ("tau_vert_max", C.c_double), ("tau_cut", C.c_double),
-                ("npix", C.c_int), ("n_batches", C.c_int), ("n_threads", C.c_int)]
+                ("npix", C.c_int), ("n_batches", C.c_int), ("n_threads", C.c_int),
+                ("survival_bias", C.c_int), ("roulette_w_min", C.c_double), ("roulette_survive", C.c_double)]
 
 
 class _Counters(C.Structure):
@@ -188,6 +189,9 @@ def _params_struct(prm, keep):
     p.npix = int(prm.get("npix", 0))
     p.n_batches = int(prm.get("n_batches", 32))
     p.n_threads = int(prm.get("n_threads", 1))
+    p.survival_bias = int(prm.get("survival_bias", 0))
+    p.roulette_w_min = float(prm.get("roulette_w_min", 0.0))
+    p.roulette_survive = float(prm.get("roulette_survive", 0.0))
     return p
 
 

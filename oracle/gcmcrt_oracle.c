@@ -593,9 +593,25 @@ static void transport(const run_ctx *rc, uint32_t pkt, double p[3], double n[3],
         peel(rc, p, ijk, 0, W, n, omega, pgas, gg, batch, cnt);     /* peel-off first (Sect. 4.6) */
         if (prm->max_events && (int)m_inter == prm->max_events) { cnt->packets_absorbed++; break; }
         if (!prm->scatter_on) { cnt->packets_absorbed++; break; }
-        if (z[0] >= omega) { cnt->packets_absorbed++; break; }     /* Sect. 4.4: analog absorption */
-        double ct = (z[0] < omega * pgas) ? orc_sample_rayleigh(z[1])  /* Eq. 11 + C6 partition */
-                                          : orc_sample_hg(gg, z[1]);
+        double ct;
+        if (prm->survival_bias) {
+            /* Sect. 4.4: the packet is forced to scatter and its weight reduced by omega; the draw that
+             * decides absorption in the analog scheme only picks the scatterer (Eq. 11: gas with probability P_gas) */
+            if (!(omega > 0.0)) { cnt->packets_absorbed++; break; }
+            W *= omega;
+            /* Sect. 4.5: Russian roulette below the weight threshold; block (m_inter, purpose 2) */
+            if (prm->roulette_w_min > 0.0 && W < prm->roulette_w_min) {
+                double zr[4];
+                orc_zeta_block(prm->seed, rc->chan_key, pkt, m_inter, 2, zr);
+                if (zr[0] >= prm->roulette_survive) { cnt->packets_absorbed++; break; }
+                W /= prm->roulette_survive;
+            }
+            ct = (z[0] < pgas) ? orc_sample_rayleigh(z[1]) : orc_sample_hg(gg, z[1]);
+        } else {
+            if (z[0] >= omega) { cnt->packets_absorbed++; break; }     /* Sect. 4.4: analog absorption */
+            ct = (z[0] < omega * pgas) ? orc_sample_rayleigh(z[1])  /* Eq. 11 + C6 partition */
+                                       : orc_sample_hg(gg, z[1]);
+        }
         double nn[3];
         orc_rotate(n, ct, 2.0 * PI * z[2], nn);
         n[0] = nn[0]; n[1] = nn[1]; n[2] = nn[2];

@@ -75,6 +75,10 @@ typedef struct {
     int npix;                /* 0 = no images */
     int n_batches;
     int n_threads;           /* OpenMP threads over batches; <=1 serial */
+    /* Variance reduction (Sect. 4.4-4.5); all 0 = analog transport */
+    int survival_bias;       /* 1: a medium interaction always scatters and W <- W omega (L192-196) */
+    double roulette_w_min;   /* Russian roulette (L200) when W < roulette_w_min after an interaction ... */
+    double roulette_survive; /* ... the packet survives with this probability and W <- W / roulette_survive */
 } orc_params;
 
 typedef struct {

@@ -637,3 +637,48 @@ def test_images_sum_to_flux(orc):
     # the zero-phase image of a back-lit... front-lit planet is symmetric about the sub-observer point within noise
     im = res["image"][0, 0]
     assert im.sum() > 0 and im[:, :8].sum() > 0 and im[:, 8:].sum() > 0
+
+
+# ----------------------------------------------------------------------------- Sect. 4.4-4.5: survival biasing, roulette
+@pytest.mark.parametrize("omega,roulette", [(0.5, None), (0.9, None), (0.9, (0.3, 0.5)), (0.99, (1e-2, 0.25))])
+def test_survival_biasing_and_roulette_keep_the_exact_semi_infinite_albedo(orc, omega, roulette):
+    """Survival biasing (L192-196) and Russian roulette (L200) change weights, not expectations: the exact
+    Chandrasekhar H-function albedo of the semi-infinite isotropic atmosphere (tests/golden) is still reproduced."""
+    rows = dict(np.loadtxt(os.path.join(GOLDEN, "isotropic_semi_infinite_albedo.txt")))
+    R0, depth = 1.0e8, 1.0e4
+    grid, opac = wl.uniform_medium(4, 1, 1, R0, R0 + depth, 80.0 / depth, omega, g=0.0, surface_albedo=1.0)
+    s = np.array([0.3, -0.5, 0.81]); s /= np.linalg.norm(s)
+    prm = wl.default_params(packets_per_channel=40000, seed=33, star_dir=s, obs_dir=s[None], survival_bias=1)
+    if roulette:
+        prm.update(roulette_w_min=roulette[0], roulette_survive=roulette[1])
+    else:
+        prm.update(max_events=400)      # without roulette a packet would scatter for ever: omega^400 is < 1e-17
+    res = orc.run_albedo(grid, opac, prm)
+    val, sig = orc.reduce(res, "albedo")
+    Ag = PI * val[0, 0]
+    assert abs(Ag - rows[omega]) < 4 * PI * sig[0, 0] + 3e-4 * rows[omega], (Ag, rows[omega], PI * sig[0, 0])
+
+
+def test_survival_biasing_conserves_energy_and_lowers_variance(orc):
+    """Escaped weight: the analog count of escaped packets and the survival-biased sum of escaped weights estimate the
+    same escape fraction; the weighted estimator has the smaller batch-to-batch scatter in the peeled-off flux."""
+    R0, Rt = 1.0e6, 1.3e6
+    grid, opac = wl.uniform_medium(4, 3, 4, R0, Rt, 3.0 / (Rt - R0), 0.6, g=0.3, pgas=0.3)
+    N = 60000
+    obs = np.array([[1.0, 0, 0], [0, 0.6, 0.8]])
+    base = wl.default_params(packets_per_channel=N, seed=12, obs_dir=obs)
+    ana = orc.run_albedo(grid, opac, base)
+    sur = orc.run_albedo(grid, opac, dict(base, survival_bias=1, roulette_w_min=1e-3, roulette_survive=0.2))
+    fa = ana["counters"]["escaped_weight"] / N
+    fs = sur["counters"]["escaped_weight"] / N
+    assert abs(fa - fs) < 4 * np.sqrt(fa * (1 - fa) / N) + 4e-3, (fa, fs)
+    va, sa = orc.reduce(ana, "albedo")
+    vs, ss = orc.reduce(sur, "albedo")
+    assert np.all(np.abs(va - vs) < 4 * np.hypot(sa, ss) + 1e-5 * va)
+    assert np.all(ss < sa)                     # more, lighter scattering events per packet: lower variance
+    assert sur["counters"]["events"] > ana["counters"]["events"]
+    # omega = 1: survival biasing changes nothing at all (same streams, W omega = W)
+    grid1, opac1 = wl.uniform_medium(4, 3, 4, R0, Rt, 3.0 / (Rt - R0), 1.0, g=0.3, pgas=0.3, surface_albedo=1.0)
+    a1 = orc.run_albedo(grid1, opac1, dict(base, packets_per_channel=3000), want_event_count=True)
+    s1 = orc.run_albedo(grid1, opac1, dict(base, packets_per_channel=3000, survival_bias=1), want_event_count=True)
+    assert np.array_equal(a1["event_count"], s1["event_count"]) and np.allclose(a1["flux_sum"], s1["flux_sum"], rtol=1e-12)

@@ -67,6 +67,12 @@ typedef struct gcmcrt_run_params {
     double tau_cut;              /* peel-off contributions with tau_obs > tau_cut are dropped (0 -> 50) */
     int npix;                    /* image side (0 = no images) */
     int n_batches;               /* batches for the batch-means sigma (0 -> 32, max 64) */
+    /* Variance reduction (Sect. 4.4-4.5); all 0 = analog transport (L192) */
+    int survival_bias;           /* 1: a medium interaction always scatters and W <- W omega (L192-196); the surface
+                                    stays analog */
+    double roulette_w_min;       /* Russian roulette (L200): when W < roulette_w_min after an interaction ... */
+    double roulette_survive;     /* ... the packet survives with this probability and W <- W / roulette_survive
+                                    (the paper states neither value; 0 disables).  Requires survival_bias. */
 } gcmcrt_run_params;
 
 typedef struct gcmcrt_counters {

@@ -30,7 +30,8 @@ class RunParams(C.Structure):
                 ("seed", C.c_uint64), ("chan_begin", C.c_int), ("chan_end", C.c_int),
                 ("max_events", C.c_int), ("scatter_on", C.c_int), ("doppler_on", C.c_int),
                 ("doppler_halfwidth", C.c_int), ("emission_bias", C.c_double), ("tau_vert_max", C.c_double),
-                ("tau_cut", C.c_double), ("npix", C.c_int), ("n_batches", C.c_int)]
+                ("tau_cut", C.c_double), ("npix", C.c_int), ("n_batches", C.c_int),
+                ("survival_bias", C.c_int), ("roulette_w_min", C.c_double), ("roulette_survive", C.c_double)]
 
 
 class Counters(C.Structure):
@@ -153,6 +154,9 @@ def make_params(prm):
     p.tau_vert_max = float(prm.get("tau_vert_max", 30.0))
     p.tau_cut = float(prm.get("tau_cut", 50.0))
     p.n_batches = int(prm.get("n_batches", 32))
+    p.survival_bias = int(prm.get("survival_bias", 0))
+    p.roulette_w_min = float(prm.get("roulette_w_min", 0.0))
+    p.roulette_survive = float(prm.get("roulette_survive", 0.0))
     return p, obs
 
 

@@ -286,6 +286,9 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     if (nb < 1 || nb > kMaxBatches) return fail(g, GCMCRT_E_INVALID, "n_batches must be in [1, 64]");
     if (!out->flux_sum && n_obs > 0) return fail(g, GCMCRT_E_INVALID, "result.flux_sum is required");
     if (prm->emission_bias < 0.0 || prm->emission_bias >= 1.0) return fail(g, GCMCRT_E_INVALID, "emission_bias must be in [0,1)");
+    if (prm->roulette_w_min < 0.0 || (prm->roulette_w_min > 0.0 && !(prm->roulette_survive > 0.0 && prm->roulette_survive <= 1.0)))
+        return fail(g, GCMCRT_E_INVALID, "roulette: w_min >= 0 and 0 < survive <= 1 required");
+    if (prm->roulette_w_min > 0.0 && !prm->survival_bias) return fail(g, GCMCRT_E_INVALID, "roulette requires survival_bias");
     if (prm->doppler_on && g->n_chan > 1 && g->reff.p == nullptr) return fail(g, GCMCRT_E_STATE, "no wavelength table");
     const int ncr = ce - cb;
     if (ncr > (1 << 24)) return fail(g, GCMCRT_E_INVALID, "too many channels in one run");
@@ -321,6 +324,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.N = N; rc.seed = prm->seed;
     rc.mode = emission;
     rc.max_events = prm->max_events; rc.scatter_on = prm->scatter_on;
+    rc.survival_bias = prm->survival_bias != 0;
+    rc.roulette_w_min = float(prm->roulette_w_min); rc.roulette_survive = float(prm->roulette_survive);
     rc.surface_albedo = g->surface_albedo;
     rc.xi = prm->emission_bias;
     rc.n_batches = nb;

@@ -88,6 +88,8 @@ struct RunConst {
     unsigned long long seed;
     int mode;              // 0 albedo, 1 emission
     int max_events, scatter_on;
+    int survival_bias;             // Sect. 4.4: forced scattering with W <- W omega
+    float roulette_w_min, roulette_survive;   // Sect. 4.5: Russian roulette below the weight threshold (0 = off)
     float surface_albedo;
     double xi;
     int n_batches;
@@ -309,6 +311,29 @@ __device__ __forceinline__ void rotate_dir(float& nx, float& ny, float& nz, floa
     }
     const float rn = rsqrtf(fmaf(x, x, fmaf(y, y, z * z)));
     nx = x * rn; ny = y * rn; nz = z * rn;
+}
+
+// O6 decision at a medium interaction m (Philox block z of (m, purpose 1)): absorbed, or the polar cosine of the
+// scattering angle.  Analog (L192): zeta0 partitions [0, omega P_gas) Rayleigh / [omega P_gas, omega) HG / [omega, 1)
+// absorbed (C6).  Survival biasing (Sect. 4.4): always scatters, W <- W omega, zeta0 only picks the scatterer; below
+// the roulette threshold (Sect. 4.5) block (m, purpose 2) decides survival with W <- W / p.
+__device__ __forceinline__ bool medium_interaction(const RunConst& rc, const float4 pr, const Zeta4& z, uint32_t ckey,
+                                                   uint32_t pkt, uint32_t m, float& W, float& ct)
+{
+    if (rc.survival_bias) {
+        if (!(pr.x > 0.0f)) return false;
+        W *= pr.x;
+        if (rc.roulette_w_min > 0.0f && W < rc.roulette_w_min) {
+            const Zeta4 zr = zeta_block(rc.seed, ckey, pkt, m, 2);
+            if (zr.z0 >= rc.roulette_survive) return false;
+            W /= rc.roulette_survive;
+        }
+        ct = (z.z0 < pr.y) ? sample_rayleigh(z.z1) : sample_hg(pr.z, z.z1);
+        return true;
+    }
+    if (z.z0 >= pr.x) return false;
+    ct = (z.z0 < pr.x * pr.y) ? sample_rayleigh(z.z1) : sample_hg(pr.z, z.z1);
+    return true;
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -540,10 +565,11 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                             }
                             ++pk.m_inter;
                             const Zeta4 z = zeta_block(rc.seed, ckey, pk.pkt, pk.m_inter, 1);
-                            if ((rc.max_events && int(pk.m_inter) == rc.max_events) || !rc.scatter_on || z.z0 >= pr.x) {
+                            float ct = 0.f;
+                            if ((rc.max_events && int(pk.m_inter) == rc.max_events) || !rc.scatter_on ||
+                                !medium_interaction(rc, pr, z, ckey, pk.pkt, pk.m_inter, pk.W, ct)) {
                                 ++c_abs; st = LS_IDLE; finish_packet(rc, pk);       // L192: absorbed
                             } else {
-                                const float ct = (z.z0 < pr.x * pr.y) ? sample_rayleigh(z.z1) : sample_hg(pr.z, z.z1);
                                 float nx = pk.ray.nx, ny = pk.ray.ny, nz = pk.ray.nz;
                                 rotate_dir(nx, ny, nz, ct, z.z2);
                                 pk.tau_t = -logf(z.z3); pk.tau = 0.f; pk.fl_seg = 0;

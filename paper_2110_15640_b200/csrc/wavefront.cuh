@@ -394,10 +394,10 @@ wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, con
                     const float4 pr = __ldg(rc.prop + (size_t)ctab * rc.geom.ncell + ((k * gs.nlat + j) * gs.nlev + i));
                     m_new = m_inter + 1;
                     const Zeta4 z = zeta_block(rc.seed, ckey, pkt, m_new, 1);
-                    if ((rc.max_events && int(m_new) == rc.max_events) || !rc.scatter_on || z.z0 >= pr.x) {
+                    if ((rc.max_events && int(m_new) == rc.max_events) || !rc.scatter_on ||
+                        !medium_interaction(rc, pr, z, ckey, pkt, m_new, a.w, ct)) {
                         ++wcnt.abs; wave_finish_packet(rc, chan_run, pkt, nev);       // L192: absorbed
                     } else {
-                        ct = (z.z0 < pr.x * pr.y) ? sample_rayleigh(z.z1) : sample_hg(pr.z, z.z1);
                         zpsi = z.z2; tau_t = -logf(z.z3); surv = true;
                     }
                 } else if (kind == EV_EMIT) {

@@ -311,6 +311,27 @@ def test_wavefront_with_surface_and_tiny_event_buffer(gpu, orc, monkeypatch):
     _check_parity(orc, small, o, "albedo")
 
 
+@pytest.mark.parametrize("tune", ["16,1,8,4", "16,1,0,4"])
+def test_survival_biasing_and_roulette_parity(gpu, orc, monkeypatch, tune):
+    """Sect. 4.4-4.5 on the GPU (generation kernels and persistent kernel) against the oracle: same streams, same
+    weights, same roulette draws (Philox purpose 2)."""
+    monkeypatch.setenv("GCMCRT_TUNE", tune)
+    grid, opac, prm = wl.cfg2(nlon=16, nlat=8, nlev=20, nbands=2, ng=3, packets=20000)
+    prm = dict(prm, survival_bias=1, roulette_w_min=0.05, roulette_survive=0.25)
+    g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+    o = orc.run_albedo(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
+    _check_parity(orc, g, o, "albedo")
+    assert abs(g["counters"]["escaped_weight"] - o["counters"]["escaped_weight"]) < 1e-3 * o["counters"]["escaped_weight"]
+    ana = _gpu_run(gpu, grid, opac, dict(prm, survival_bias=0, roulette_w_min=0.0), "albedo")
+    assert g["counters"]["events"] > ana["counters"]["events"]
+    assert np.all(np.abs(g["value"] - ana["value"]) < 4 * np.hypot(g["sigma"], ana["sigma"]) + 1e-5 * ana["value"])
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        with pytest.raises(gpu.GcmcrtError) as e:
+            G.run_albedo(dict(prm, survival_bias=0))
+        assert e.value.code == gpu.E_INVALID
+
+
 def test_packet_and_channel_subranges_compose(gpu):
     grid, opac, prm = wl.cfg2(nlon=8, nlat=4, nlev=10, nbands=1, ng=4, packets=20000)
     full = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)

@@ -100,6 +100,9 @@ typedef struct gcmcrt_result {
     float *image;          /* [n_chan_run][n_obs][npix][npix] (L83) */
     uint32_t *event_count; /* [n_chan_run][pkt_end-pkt_begin]: peel-off points per packet */
     gcmcrt_counters *counters; /* one struct */
+    float *contrib;        /* [n_chan_run][n_obs][2][ncell] (cell-flat layout): contribution functions of Sect. 6,
+                              Eq. 32, as raw sums of the peeled-off f per event cell: [0] thermal (emission points),
+                              [1] scattered (medium and surface events).  CF = contrib / sum over cells. */
 } gcmcrt_result;
 
 /*

@@ -47,7 +47,7 @@ class _Counters(C.Structure):
 
 class _Result(C.Structure):
     _fields_ = [("flux_sum", C.c_void_p), ("L_tot", C.c_void_p), ("image", C.c_void_p),
-                ("event_count", C.c_void_p), ("counters", _Counters)]
+                ("event_count", C.c_void_p), ("counters", _Counters), ("contrib", C.c_void_p)]
 
 
 def lib():
@@ -195,7 +195,7 @@ def _params_struct(prm, keep):
     return p
 
 
-def _run(mode, grid, opac, prm, want_event_count=False):
+def _run(mode, grid, opac, prm, want_event_count=False, want_contrib=False):
     keep = _Keep()
     g, ncell = _grid_struct(grid, keep)
     o, n_chan = _opac_struct(opac, ncell, keep)
@@ -205,25 +205,27 @@ def _run(mode, grid, opac, prm, want_event_count=False):
     ltot = np.zeros((n_chan, nobs), dtype=np.float64)
     image = np.zeros((n_chan, nobs, npix, npix), dtype=np.float64) if npix > 0 else None
     evc = np.zeros((n_chan, N), dtype=np.uint32) if want_event_count else None
-    res = _Result(_ptr(flux), _ptr(ltot), _ptr(image), _ptr(evc), _Counters())
+    contrib = np.zeros((n_chan, nobs, 2, ncell), dtype=np.float64) if want_contrib else None
+    res = _Result(_ptr(flux), _ptr(ltot), _ptr(image), _ptr(evc), _Counters(), _ptr(contrib))
     fn = lib().orc_run_albedo if mode == "albedo" else lib().orc_run_emission
     fn.restype = C.c_int
     rc = fn(C.byref(g), C.byref(o), C.byref(p), C.byref(res))
     if rc != 0:
         raise RuntimeError("oracle run failed: %d" % rc)
     cnt = {name: getattr(res.counters, name) for name, _ in _Counters._fields_}
-    return {"flux_sum": flux, "L_tot": ltot, "image": image, "event_count": evc, "counters": cnt,
+    return {"flux_sum": flux, "L_tot": ltot, "image": image, "event_count": evc, "counters": cnt, "contrib": contrib,
             "n_batches": nb, "packets_per_channel": N, "pkt_range": (p.pkt_begin, p.pkt_end)}
 
 
-def run_albedo(grid, opac, prm, want_event_count=False):
-    """O3,O5-O8: albedo mode.  Returns raw sums flux_sum[n_chan][n_obs][n_batches] (Eq. 14) etc."""
-    return _run("albedo", grid, opac, prm, want_event_count)
+def run_albedo(grid, opac, prm, want_event_count=False, want_contrib=False):
+    """O3,O5-O8: albedo mode.  Returns raw sums flux_sum[n_chan][n_obs][n_batches] (Eq. 14) etc.; contrib
+    [n_chan][n_obs][2][ncell] = Eq. 32 numerators (thermal, scattered) when asked for."""
+    return _run("albedo", grid, opac, prm, want_event_count, want_contrib)
 
 
-def run_emission(grid, opac, prm, want_event_count=False):
+def run_emission(grid, opac, prm, want_event_count=False, want_contrib=False):
     """O4-O8: emission mode."""
-    return _run("emission", grid, opac, prm, want_event_count)
+    return _run("emission", grid, opac, prm, want_event_count, want_contrib)
 
 
 def reduce(result, mode):

@@ -501,6 +501,7 @@ typedef struct {
     double e1[3], e2[3]; /* launch disc basis (O3) */
     double *S;         /* flux_sum for this channel: [n_obs][n_batches] */
     double *image;     /* this channel's [n_obs][npix][npix] or NULL */
+    double *contrib;   /* this channel's [n_obs][2][ncell] or NULL (Sect. 6, Eq. 32) */
     uint32_t *evcount; /* this channel's [N] or NULL */
 } run_ctx;
 
@@ -553,6 +554,8 @@ static void peel(const run_ctx *rc, const double p[3], const int ijk[3], int kin
             int npix = rc->prm->npix;
             rc->image[(size_t)o * npix * npix + image_pixel(p, od, G->Rtoa, npix)] += f;
         }
+        if (rc->contrib)   /* Sect. 6: the contribution of the event's cell to the output, thermal / scattered apart */
+            rc->contrib[((size_t)o * 2 + (kind == 1 ? 0 : 1)) * G->ncell + cell_index(G, ijk[0], ijk[1], ijk[2])] += f;
     }
 }
 
@@ -709,6 +712,7 @@ static int run_mode(const orc_grid *g, const orc_opacity *op, const orc_params *
     memset(&out->counters, 0, sizeof out->counters);
     memset(out->flux_sum, 0, sizeof(double) * (size_t)op->n_chan * nobs * nb);
     if (out->image && npix > 0) memset(out->image, 0, sizeof(double) * (size_t)op->n_chan * nobs * npix * npix);
+    if (out->contrib) memset(out->contrib, 0, sizeof(double) * (size_t)op->n_chan * nobs * 2 * G.ncell);
     int nthreads = prm->n_threads > 1 ? prm->n_threads : 1;
     chan_t ch;
     if (chan_alloc(&ch, G.ncell)) { geom_free(&G); return -1; }
@@ -740,11 +744,12 @@ static int run_mode(const orc_grid *g, const orc_opacity *op, const orc_params *
             }
             rc.S = out->flux_sum + (size_t)c * nobs * nb;
             rc.image = (out->image && npix > 0) ? out->image + (size_t)c * nobs * npix * npix : NULL;
+            rc.contrib = out->contrib ? out->contrib + (size_t)c * nobs * 2 * G.ncell : NULL;
             rc.evcount = (out->event_count && run == 0) ? out->event_count + (size_t)c * N : NULL;
             if (emission && !(ch.L_tot > 0.0)) continue;
             /* O8 / C12: batch(pkt) = floor(pkt * n_batches / N); batches are independent -> OpenMP over them */
 #ifdef _OPENMP
-#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads) if (nthreads > 1 && !rc.image)
+#pragma omp parallel for schedule(dynamic, 1) num_threads(nthreads) if (nthreads > 1 && !rc.image && !rc.contrib)
 #endif
             for (int b = 0; b < nb; ++b) {
                 orc_counters cnt;

@@ -95,6 +95,8 @@ typedef struct {
     double *image;         /* nullable [n_chan][n_obs][npix][npix] */
     uint32_t *event_count; /* nullable [n_chan][N] */
     orc_counters counters;
+    double *contrib;       /* nullable [n_chan][n_obs][2][ncell]: Eq. 32 numerators: peeled-off f summed per event
+                              cell, [0] thermal (emission points), [1] scattered (medium + surface events) */
 } orc_result;
 
 /* A3: Philox4x32-10 (Salmon et al. 2011), C2. */

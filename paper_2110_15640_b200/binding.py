@@ -45,7 +45,8 @@ class Counters(C.Structure):
 
 class Result(C.Structure):
     _fields_ = [("flux_sum", C.c_void_p), ("L_tot", C.c_void_p), ("value", C.c_void_p), ("sigma", C.c_void_p),
-                ("image", C.c_void_p), ("event_count", C.c_void_p), ("counters", C.POINTER(Counters))]
+                ("image", C.c_void_p), ("event_count", C.c_void_p), ("counters", C.POINTER(Counters)),
+                ("contrib", C.c_void_p)]
 
 
 def lib():
@@ -160,7 +161,7 @@ def make_params(prm):
     return p, obs
 
 
-def _run(fn, handle, prm, n_chan_table, want_event_count, want_image, device_outputs, stream):
+def _run(fn, handle, prm, n_chan_table, want_event_count, want_image, device_outputs, stream, want_contrib=0):
     p, keep = make_params(prm)
     N = p.packets_per_channel
     lo, hi = p.pkt_begin, (p.pkt_end or N)
@@ -173,6 +174,8 @@ def _run(fn, handle, prm, n_chan_table, want_event_count, want_image, device_out
         shapes["image"] = ((ncr, nobs, p.npix, p.npix), np.float32)
     if want_event_count:
         shapes["event_count"] = ((ncr, hi - lo), np.uint32)
+    if want_contrib:             # = ncell: contribution functions (Sect. 6, Eq. 32), [chan][obs][thermal|scattered][cell]
+        shapes["contrib"] = ((ncr, nobs, 2, int(want_contrib)), np.float32)
     out = {}
     if device_outputs:
         import torch
@@ -184,7 +187,7 @@ def _run(fn, handle, prm, n_chan_table, want_event_count, want_image, device_out
             out[k] = np.zeros(shp, dtype=dt)
     cnt = Counters()
     res = Result()
-    for k in ("flux_sum", "L_tot", "value", "sigma", "image", "event_count"):
+    for k in ("flux_sum", "L_tot", "value", "sigma", "image", "event_count", "contrib"):
         setattr(res, k, _ptr(out[k]) if k in out else None)
     res.counters = C.pointer(cnt)
     rc = fn(handle, C.byref(p), C.byref(res), _stream_ptr(stream))
@@ -195,12 +198,16 @@ def _run(fn, handle, prm, n_chan_table, want_event_count, want_image, device_out
     return out
 
 
-def run_albedo(handle, prm, n_chan_table, want_event_count=False, want_image=True, device_outputs=False, stream=None):
-    return _run(lib().gcmcrt_run_albedo, handle, prm, n_chan_table, want_event_count, want_image, device_outputs, stream)
+def run_albedo(handle, prm, n_chan_table, want_event_count=False, want_image=True, device_outputs=False, stream=None,
+               want_contrib=0):
+    return _run(lib().gcmcrt_run_albedo, handle, prm, n_chan_table, want_event_count, want_image, device_outputs, stream,
+                want_contrib)
 
 
-def run_emission(handle, prm, n_chan_table, want_event_count=False, want_image=True, device_outputs=False, stream=None):
-    return _run(lib().gcmcrt_run_emission, handle, prm, n_chan_table, want_event_count, want_image, device_outputs, stream)
+def run_emission(handle, prm, n_chan_table, want_event_count=False, want_image=True, device_outputs=False, stream=None,
+                 want_contrib=0):
+    return _run(lib().gcmcrt_run_emission, handle, prm, n_chan_table, want_event_count, want_image, device_outputs, stream,
+                want_contrib)
 
 
 def debug_ray_tau(handle, chan, pos, dirs, stream=None):

@@ -75,7 +75,7 @@ struct gcmcrt_grid {
     DevBuf Lcell, Lcum, Ltot;
 
     // workspace
-    DevBuf ev0, ev1, ev2, evkeys, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, flights, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount;
+    DevBuf ev0, ev1, ev2, evkeys, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, flights, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount, contrib;
     unsigned int ev_cap = 0;
     int n_threads_resident = 0;
     // GCMCRT_TUNE="service,lateral,gens,batch_div": lanes waiting before the persistent kernel serves them; lanes parked at
@@ -298,7 +298,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     if (rcode) return rcode;
 
     // ---- outputs
-    OutBuf o_flux, o_ltot, o_val, o_sig, o_img, o_evc, o_cnt;
+    OutBuf o_flux, o_ltot, o_val, o_sig, o_img, o_evc, o_cnt, o_ctb;
     const size_t nflux = size_t(ncr) * std::max(n_obs, 1) * nb;
     if ((rcode = bind_out(g, out->flux_sum, nflux * sizeof(double), g->flux, o_flux))) return rcode;
     if ((rcode = bind_out(g, out->L_tot, size_t(ncr) * std::max(n_obs, 1) * sizeof(double), g->ltot_out, o_ltot))) return rcode;
@@ -311,6 +311,10 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     CUDA_TRY(g, cudaMemsetAsync(o_flux.dev, 0, nflux * sizeof(double), s));
     CUDA_TRY(g, cudaMemsetAsync(o_ltot.dev, 0, o_ltot.bytes, s));
     if (npix) CUDA_TRY(g, cudaMemsetAsync(o_img.dev, 0, o_img.bytes, s));
+    if (out->contrib && n_obs > 0) {
+        if ((rcode = bind_out(g, out->contrib, size_t(ncr) * n_obs * 2 * g->ncell * sizeof(float), g->contrib, o_ctb))) return rcode;
+        CUDA_TRY(g, cudaMemsetAsync(o_ctb.dev, 0, o_ctb.bytes, s));
+    }
     if (o_evc.dev) CUDA_TRY(g, cudaMemsetAsync(o_evc.dev, 0, o_evc.bytes, s));
     CUDA_TRY(g, cudaMemsetAsync(g->counters.p, 0, sizeof(DevCounters), s));
 
@@ -344,6 +348,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.npix = npix;
     rc.flux = static_cast<double*>(o_flux.dev);
     rc.image = npix ? static_cast<float*>(o_img.dev) : nullptr;
+    rc.contrib = static_cast<float*>(o_ctb.dev);
     rc.event_count = static_cast<uint32_t*>(o_evc.dev);
     rc.counters = g->counters.as<DevCounters>();
     rc.magic_N = magic_div(N);
@@ -623,7 +628,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     g->ms_stage_pending = 0.0;
     // ---- copy-backs for host-resident outputs
     bool need_sync = false;
-    for (OutBuf* ob : {&o_flux, &o_ltot, &o_val, &o_sig, &o_img, &o_evc}) {
+    for (OutBuf* ob : {&o_flux, &o_ltot, &o_val, &o_sig, &o_img, &o_evc, &o_ctb}) {
         if (ob->host && ob->dev && ob->bytes) {
             CUDA_TRY(g, cudaMemcpyAsync(ob->host, ob->dev, ob->bytes, cudaMemcpyDeviceToHost, s));
             need_sync = true;
@@ -796,7 +801,7 @@ int gcmcrt_destroy(gcmcrt_grid* g)
                       &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->prop, &g->reff, &g->vlos,
                       &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->ev1, &g->ev2, &g->evkeys, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
                       &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->flux, &g->ltot_out,
-                      &g->value, &g->sigma, &g->image, &g->evcount})
+                      &g->value, &g->sigma, &g->image, &g->evcount, &g->contrib})
         b->release();
     if (g->h_ctrl) cudaFreeHost(g->h_ctrl);
     for (auto& e : g->tev) if (e) cudaEventDestroy(e);

@@ -102,6 +102,7 @@ struct RunConst {
     // outputs
     double* flux;          // [n_chan_run][n_obs_total][n_batches]
     float* image;          // nullable
+    float* contrib;        // nullable [n_chan_run][n_obs_total][2][ncell]: Eq. 32 numerators (thermal, scattered)
     uint32_t* event_count; // nullable [n_chan_run][n_pkt]
     DevCounters* counters;
     unsigned long long* work_counter;   // next fresh packet item
@@ -802,6 +803,28 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
                         const int ix = min(max(int(floorf((X / rc.geom.Rtoa + 1.0f) * 0.5f * rc.npix)), 0), rc.npix - 1);
                         const int iy = min(max(int(floorf((Y / rc.geom.Rtoa + 1.0f) * 0.5f * rc.npix)), 0), rc.npix - 1);
                         atomicAdd(rc.image + ((size_t)chan * rc.n_obs_total + o) * rc.npix * rc.npix + iy * rc.npix + ix, f);
+                    }
+                }
+                if (rc.contrib) {
+                    // Sect. 6, Eq. 32: f per event cell, thermal and scattered apart.  The lanes are sorted by
+                    // (channel, cell), so the lanes of one cell are neighbours: sum each run with a segmented shuffle
+                    // reduction (both components at once) and let its first lane do the atomics.
+                    const unsigned ckey = have ? unsigned((ck * gs.nlat + cj) * gs.nlev + ci) : 0xffffffffu;
+                    const float f = st == RAY_ESCAPE ? pref * expf(-tau) : 0.f;
+                    float v0 = kind == EV_EMIT ? f : 0.f, v1 = kind == EV_EMIT ? 0.f : f;
+#pragma unroll
+                    for (int off = 1; off < 32; off <<= 1) {
+                        const float w0 = __shfl_down_sync(kFullMask, v0, off), w1 = __shfl_down_sync(kFullMask, v1, off);
+                        const unsigned kk = __shfl_down_sync(kFullMask, ckey, off);
+                        const int cc = __shfl_down_sync(kFullMask, chan, off);
+                        if (lane_id() + off < 32 && kk == ckey && cc == chan) { v0 += w0; v1 += w1; }
+                    }
+                    const unsigned kp = __shfl_up_sync(kFullMask, ckey, 1);
+                    const int cp = __shfl_up_sync(kFullMask, chan, 1);
+                    if (have && (lane_id() == 0 || kp != ckey || cp != chan)) {
+                        float* dst = rc.contrib + ((size_t)chan * rc.n_obs_total + rc.obs_first + obs) * 2 * rc.geom.ncell + ckey;
+                        if (v0 != 0.f) atomicAdd(dst, v0);
+                        if (v1 != 0.f) atomicAdd(dst + rc.geom.ncell, v1);
                     }
                 }
                 __syncwarp();

@@ -38,7 +38,7 @@ def test_struct_layouts_match_header():
     assert binding.RunParams.obs_dir.offset == 32 and binding.RunParams.seed.offset == 64
     assert binding.RunParams.emission_bias.offset == 96 and binding.RunParams.n_batches.offset == 124
     assert C.sizeof(binding.Counters) == 128     # 11 u64/double + 5 ms doubles (ms_sort added with the event sort)
-    assert C.sizeof(binding.Result) == 56
+    assert C.sizeof(binding.Result) == 64      # 8 pointers (contrib added with the contribution functions)
 
 
 def test_no_cpu_fallback_without_device(lib):

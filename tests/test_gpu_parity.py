@@ -373,6 +373,30 @@ def test_images_sum_to_flux_and_match_oracle(gpu, orc):
     assert np.allclose(g["image"], o["image"], rtol=0.05, atol=0.02 * o["image"].max())
 
 
+def test_contribution_functions_match_oracle(gpu, orc):
+    """Sect. 6, Eq. 32: per-cell sums of the peeled-off f, thermal and scattered apart, against the oracle's."""
+    grid, opac, prm = wl.cfg3(nlon=8, nlat=4, nlev=12, nbands=1, ng=3, packets=40000, n_obs=3)
+    ncell = 8 * 4 * 12
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        g = G.run_emission(prm, want_contrib=ncell)
+    o = orc.run_emission(grid, opac, dict(prm, n_threads=1), want_contrib=True)
+    assert np.allclose(g["contrib"].sum(axis=(2, 3)), g["flux_sum"].sum(axis=2), rtol=2e-4)
+    for comp in (0, 1):
+        cg, co = g["contrib"][:, :, comp], o["contrib"][:, :, comp]
+        assert np.allclose(cg.sum(axis=2), co.sum(axis=2), rtol=2e-3, atol=1e-4 * co.sum(axis=2).max())
+        big = co > 0.02 * co.max()                 # cells that carry the signal: same packets, same streams
+        assert np.allclose(cg[big], co[big], rtol=2e-2)
+        cf_g, cf_o = cg / cg.sum(axis=2, keepdims=True), co / co.sum(axis=2, keepdims=True)      # Eq. 32
+        assert np.abs(cf_g - cf_o).max() < 2e-3
+    grid, opac, prm = wl.cfg2(nlon=8, nlat=4, nlev=12, nbands=1, ng=3, packets=20000)
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        a = G.run_albedo(prm, want_contrib=ncell)
+    assert a["contrib"][:, :, 0].sum() == 0.0
+    assert np.allclose(a["contrib"][:, :, 1].sum(axis=2), a["flux_sum"].sum(axis=2), rtol=2e-4)
+
+
 def test_error_paths(gpu):
     grid, opac, prm = wl.cfg1(packets=100)
     with gpu.Grid(grid) as G:

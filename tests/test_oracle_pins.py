@@ -682,3 +682,31 @@ def test_survival_biasing_conserves_energy_and_lowers_variance(orc):
     a1 = orc.run_albedo(grid1, opac1, dict(base, packets_per_channel=3000), want_event_count=True)
     s1 = orc.run_albedo(grid1, opac1, dict(base, packets_per_channel=3000, survival_bias=1), want_event_count=True)
     assert np.array_equal(a1["event_count"], s1["event_count"]) and np.allclose(a1["flux_sum"], s1["flux_sum"], rtol=1e-12)
+
+
+# ----------------------------------------------------------------------------- Sect. 6, Eq. 32: contribution functions
+def test_contribution_counters_partition_the_flux(orc):
+    """Eq. 32 numerators: the per-cell counters sum to the peeled-off flux of each observer; with scattering off an
+    emission run is all thermal; an albedo run is all scattered; a purely absorbing isothermal 1D atmosphere puts the
+    thermal contribution where d exp(-tau)/dr says (Eq. 31 with B constant): radial profile vs chord quadrature."""
+    grid, opac, prm = wl.cfg3(nlon=8, nlat=4, nlev=12, nbands=1, ng=3, packets=6000, n_obs=3)
+    e = orc.run_emission(grid, opac, prm, want_contrib=True)
+    assert np.allclose(e["contrib"].sum(axis=(2, 3)), e["flux_sum"].sum(axis=2), rtol=1e-10)
+    assert e["contrib"][:, :, 1].sum() > 0 and e["contrib"][:, :, 0].sum() > 0        # thermal and scattered parts
+    e0 = orc.run_emission(grid, opac, dict(prm, scatter_on=0), want_contrib=True)
+    assert e0["contrib"][:, :, 1].sum() == 0.0
+    assert np.allclose(e0["contrib"][:, :, 0].sum(axis=2), e0["flux_sum"].sum(axis=2), rtol=1e-10)
+    grid, opac, prm = wl.cfg2(nlon=8, nlat=4, nlev=12, nbands=1, ng=3, packets=6000)
+    a = orc.run_albedo(grid, opac, prm, want_contrib=True)
+    assert a["contrib"][:, :, 0].sum() == 0.0
+    assert np.allclose(a["contrib"][:, :, 1].sum(axis=2), a["flux_sum"].sum(axis=2), rtol=1e-10)
+    # radial profile of the thermal contribution of an isothermal absorber seen along +z: cell (i) of a 1D grid
+    # contributes B * integral over its volume of alpha exp(-tau_obs) / ... ; total over cells = chord integral (P9);
+    # here only the ordering is pinned: the contribution peaks where the vertical optical depth passes ~1
+    grid1, opac1, r, alpha = _layered(nlev=12, seed=3, nlat=1, nlon=1)
+    grid1["T"][:] = 1500.0
+    p1 = wl.default_params(packets_per_channel=40000, seed=2, obs_dir=[[0.0, 0.0, 1.0]], scatter_on=0, tau_vert_max=0.0)
+    c1 = orc.run_emission(grid1, opac1, p1, want_contrib=True)["contrib"][0, 0, 0]
+    tau_above = np.concatenate([np.cumsum((alpha * np.diff(r))[::-1])[::-1][1:], [0.0]])
+    visible = tau_above < 5.0
+    assert c1[visible].sum() > 0.97 * c1.sum()

@@ -35,7 +35,8 @@ class _Params(C.Structure):
                 ("doppler_on", C.c_int), ("doppler_halfwidth", C.c_int),
                 ("emission_bias", C.c_double), ("tau_vert_max", C.c_double), ("tau_cut", C.c_double),
                 ("npix", C.c_int), ("n_batches", C.c_int), ("n_threads", C.c_int),
-                ("survival_bias", C.c_int), ("roulette_w_min", C.c_double), ("roulette_survive", C.c_double)]
+                ("survival_bias", C.c_int), ("roulette_w_min", C.c_double), ("roulette_survive", C.c_double),
+                ("star_radius", C.c_double), ("planet_xy", C.c_double * 2), ("ld_c1", C.c_double), ("ld_c2", C.c_double)]
 
 
 class _Counters(C.Structure):
@@ -192,6 +193,10 @@ def _params_struct(prm, keep):
     p.survival_bias = int(prm.get("survival_bias", 0))
     p.roulette_w_min = float(prm.get("roulette_w_min", 0.0))
     p.roulette_survive = float(prm.get("roulette_survive", 0.0))
+    p.star_radius = float(prm.get("star_radius", 0.0))
+    xy = prm.get("planet_xy", (0.0, 0.0))
+    p.planet_xy[0], p.planet_xy[1] = float(xy[0]), float(xy[1])
+    p.ld_c1, p.ld_c2 = float(prm.get("ld_c1", 0.0)), float(prm.get("ld_c2", 0.0))
     return p
 
 
@@ -207,7 +212,8 @@ def _run(mode, grid, opac, prm, want_event_count=False, want_contrib=False):
     evc = np.zeros((n_chan, N), dtype=np.uint32) if want_event_count else None
     contrib = np.zeros((n_chan, nobs, 2, ncell), dtype=np.float64) if want_contrib else None
     res = _Result(_ptr(flux), _ptr(ltot), _ptr(image), _ptr(evc), _Counters(), _ptr(contrib))
-    fn = lib().orc_run_albedo if mode == "albedo" else lib().orc_run_emission
+    fn = {"albedo": lib().orc_run_albedo, "emission": lib().orc_run_emission,
+          "transmission": lib().orc_run_transmission}[mode]
     fn.restype = C.c_int
     rc = fn(C.byref(g), C.byref(o), C.byref(p), C.byref(res))
     if rc != 0:
@@ -226,6 +232,15 @@ def run_albedo(grid, opac, prm, want_event_count=False, want_contrib=False):
 def run_emission(grid, opac, prm, want_event_count=False, want_contrib=False):
     """O4-O8: emission mode."""
     return _run("emission", grid, opac, prm, want_event_count, want_contrib)
+
+
+def run_transmission(grid, opac, prm):
+    """Sect. 5.1, Eq. 20-23: random transit chords, multiple scattering off.  reduce(.., "transmission") gives <I_p>
+    of Eq. 21 in m^2 once multiplied by (R_TOA - R_p0): see reduce()."""
+    res = _run("transmission", grid, opac, prm)
+    r = np.asarray(grid["r_edges"], dtype=np.float64)
+    res["annulus_width"] = float(r[-1] - r[0])
+    return res
 
 
 def reduce(result, mode):
@@ -250,6 +265,9 @@ def reduce(result, mode):
     if mode == "emission":
         mean = mean * result["L_tot"]
         sigma = sigma * result["L_tot"]
+    if mode == "transmission":          # Eq. 21: <I_p> = (R_TOA - R_p0) / N * sum, m^2
+        mean = mean * result["annulus_width"]
+        sigma = sigma * result["annulus_width"]
     return mean, sigma
 
 

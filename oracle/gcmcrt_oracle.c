@@ -784,3 +784,63 @@ int orc_run_emission(const orc_grid *g, const orc_opacity *op, const orc_params 
 {
     return run_mode(g, op, prm, out, 1);
 }
+
+/* ---- Sect. 5.1: transmission by random transit chords (Eq. 20-23) ------------------------------------------------
+ * Packet pkt of channel c, Philox block (event 0, purpose 0): b = R_p0 + zeta0 (R_TOA - R_p0) (uniform in b: Eq. 21
+ * carries the factor b_i explicitly), psi = 2 pi zeta1 around the limb.  The chord runs along o^ (planet -> observer)
+ * through the point b (cos psi e_x + sin psi e_y) of the sky plane; it starts on the star side of the TOA sphere.
+ * tau_i = extinction optical depth of the whole chord (the "initial peeloff", L255).  Chords never meet the lower
+ * boundary because b >= R_p0 (L257).  Limb darkening: the chord's sky position relative to the stellar disc centre
+ * gives mu = sqrt(1 - rho^2 / R_star^2) and W = 1 - c1 (1 - mu) - c2 (1 - mu)^2 (Eq. 22-23); off the disc W = 0. */
+int orc_run_transmission(const orc_grid *g, const orc_opacity *op, const orc_params *prm, orc_result *out)
+{
+    geom_t G;
+    if (!g || !op || !prm || !out || prm->n_batches < 1 || prm->n_obs < 1) return -1;
+    if (geom_init(&G, g)) return -1;
+    const uint64_t N = prm->packets_per_channel;
+    const int nb = prm->n_batches, nobs = prm->n_obs;
+    memset(&out->counters, 0, sizeof out->counters);
+    memset(out->flux_sum, 0, sizeof(double) * (size_t)op->n_chan * nobs * nb);
+    chan_t ch;
+    if (chan_alloc(&ch, G.ncell)) { geom_free(&G); return -1; }
+    const double R0 = G.R[0], Rt = G.Rtoa;
+    for (int c = 0; c < op->n_chan; ++c) {
+        for (int o = 0; o < nobs; ++o) {
+            /* with doppler_on the observer's shifted table (O9); the unshifted one otherwise */
+            if (o == 0 || prm->doppler_on) chan_prep(g, &G, op, prm, c, prm->doppler_on ? o : -1, 0, &ch);
+            const double *od = prm->obs_dir + 3 * o;
+            double ex[3] = { -od[1], od[0], 0.0 };   /* C19 frame */
+            double nn = sqrt(ex[0] * ex[0] + ex[1] * ex[1]);
+            if (nn < 1e-6) { ex[0] = 1.0; ex[1] = 0.0; ex[2] = 0.0; } else { ex[0] /= nn; ex[1] /= nn; }
+            double ey[3] = { od[1] * ex[2] - od[2] * ex[1], od[2] * ex[0] - od[0] * ex[2], od[0] * ex[1] - od[1] * ex[0] };
+            for (uint64_t pkt = prm->pkt_begin; pkt < prm->pkt_end; ++pkt) {
+                double z[4];
+                orc_zeta_block(prm->seed, (uint32_t)(op->chan0 + c), (uint32_t)pkt, 0, 0, z);
+                const double b = R0 + z[0] * (Rt - R0), psi = 2.0 * PI * z[1];
+                const double X = b * cos(psi), Y = b * sin(psi), h = sqrt(fmax(0.0, Rt * Rt - b * b));
+                double p[3], q[3];
+                for (int m = 0; m < 3; ++m) { p[m] = X * ex[m] + Y * ey[m] - h * od[m]; q[m] = p[m]; }
+                double W = 1.0;
+                if (prm->star_radius > 0.0) {
+                    const double sx = prm->planet_xy[0] + X, sy = prm->planet_xy[1] + Y;
+                    const double rho2 = (sx * sx + sy * sy) / (prm->star_radius * prm->star_radius);
+                    if (rho2 >= 1.0) W = 0.0;
+                    else { const double mu = sqrt(1.0 - rho2); W = 1.0 - prm->ld_c1 * (1.0 - mu) - prm->ld_c2 * (1.0 - mu) * (1.0 - mu); }
+                }
+                int ijk[3];
+                locate(&G, q, ijk);
+                ijk[0] = G.nlev - 1;
+                double tau = 0.0;
+                int st = march(&G, ch.alpha, q, od, ijk, INFINITY, &tau, &out->counters.segments_peel, NULL);
+                out->counters.events++;
+                if (st == ST_STUCK) { out->counters.packets_stuck++; continue; }
+                const double absorbed = (st == ST_SURFACE) ? 1.0 : 1.0 - exp(-tau);   /* (a chord grazing R_p0 in fp) */
+                const int batch = (int)((pkt * (uint64_t)nb) / N);
+                out->flux_sum[((size_t)c * nobs + o) * nb + batch] += W * absorbed * b;
+            }
+        }
+    }
+    chan_free(&ch);
+    geom_free(&G);
+    return 0;
+}

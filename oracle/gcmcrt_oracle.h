@@ -79,6 +79,11 @@ typedef struct {
     int survival_bias;       /* 1: a medium interaction always scatters and W <- W omega (L192-196) */
     double roulette_w_min;   /* Russian roulette (L200) when W < roulette_w_min after an interaction ... */
     double roulette_survive; /* ... the packet survives with this probability and W <- W / roulette_survive */
+    /* Transmission (Sect. 5.1): stellar disc for the limb-darkening weight of Eq. 22-23; star_radius = 0: W = 1 */
+    double star_radius;      /* R_star, m */
+    double planet_xy[2];     /* sky-plane position of the planet centre relative to the stellar disc centre, m, in
+                                the observer's image frame (C19: e_x = z^ x o^ normalised, e_y = o^ x e_x) */
+    double ld_c1, ld_c2;     /* quadratic limb-darkening law, Eq. 22 */
 } orc_params;
 
 typedef struct {
@@ -142,6 +147,10 @@ int orc_channel_prep(const orc_grid *g, const orc_opacity *op, const orc_params 
 /* The two drivers (section 3 call stacks). */
 int orc_run_albedo(const orc_grid *g, const orc_opacity *op, const orc_params *prm, orc_result *out);
 int orc_run_emission(const orc_grid *g, const orc_opacity *op, const orc_params *prm, orc_result *out);
+/* Transmission spectrum by random transit chords (Sect. 5.1, Eq. 20-21), multiple scattering off (L259: "reduces the
+ * model to a raytracer scheme with random transit chord sampler"): flux_sum[c][o][batch] = sum over packets of
+ * W [1 - exp(-tau_i)] b_i; <I_p> = (R_TOA - R_p0) / N * sum (Eq. 21); W from Eq. 22-23. */
+int orc_run_transmission(const orc_grid *g, const orc_opacity *op, const orc_params *prm, orc_result *out);
 
 #ifdef __cplusplus
 }

@@ -710,3 +710,62 @@ def test_contribution_counters_partition_the_flux(orc):
     tau_above = np.concatenate([np.cumsum((alpha * np.diff(r))[::-1])[::-1][1:], [0.0]])
     visible = tau_above < 5.0
     assert c1[visible].sum() > 0.97 * c1.sum()
+
+
+# ----------------------------------------------------------------------------- Sect. 5.1: transmission, Eq. 20-23
+def test_transmission_chord_sampler_matches_quadrature(orc):
+    """Eq. 21 against a deterministic quadrature of Eq. 20's integrand: homogeneous shell (tau(b) in closed form),
+    a layered 1D atmosphere (chord formula of P3), the opaque and the transparent limits, and independence of the
+    3D grid resolution and of the viewing direction for a spherically symmetric atmosphere."""
+    R0, Rt = 1.0e7, 1.2e7
+    nbq = 200000
+    b = R0 + (np.arange(nbq) + 0.5) / nbq * (Rt - R0)
+    for a_ext, nl, nla, nlo, obs in [(3.0e-7, 1, 1, 1, [0, 0, 1.0]), (3.0e-7, 7, 5, 6, [0.6, 0, 0.8]), (1.0e-4, 3, 2, 3, [1.0, 0, 0]),
+                                     (1.0e-12, 3, 2, 3, [0, 1.0, 0])]:
+        grid, opac = wl.uniform_medium(nl, nla, nlo, R0, Rt, a_ext, 0.3)
+        prm = wl.default_params(packets_per_channel=40000, seed=6, obs_dir=[obs])
+        val, sig = orc.reduce(orc.run_transmission(grid, opac, prm), "transmission")
+        tau = 2 * a_ext * np.sqrt(Rt ** 2 - b ** 2)
+        exact = np.sum((1 - np.exp(-tau)) * b) * (Rt - R0) / nbq
+        assert abs(val[0, 0] - exact) < 4 * sig[0, 0] + 1e-6 * exact + 1e-9 * Rt ** 2, (val[0, 0], exact, sig[0, 0])
+    # opaque limit: R_p = R_TOA (Eq. 20 with T = 0)
+    assert abs(R0 ** 2 + 2 * exact - Rt ** 2) < 1.0 or a_ext < 1e-6
+    grid, opac, r, alpha = _layered(nlev=9, seed=4, nlat=3, nlon=4)
+    prm = wl.default_params(packets_per_channel=60000, seed=8, obs_dir=[[0.36, -0.48, 0.8]])
+    val, sig = orc.reduce(orc.run_transmission(grid, opac, prm), "transmission")
+    bq = r[0] + (np.arange(20000) + 0.5) / 20000 * (r[-1] - r[0])
+    exact = np.sum((1 - np.exp(-np.array([_chord_tau(r, alpha, x) for x in bq]))) * bq) * (r[-1] - r[0]) / 20000
+    assert abs(val[0, 0] - exact) < 4 * sig[0, 0] + 2e-4 * exact, (val[0, 0], exact, sig[0, 0])
+
+
+def test_transmission_limb_darkening_weights(orc):
+    """Eq. 22-23: an opaque annulus weighs every chord by the stellar intensity behind it.  Planet far smaller than the
+    star: W ~ I(mu0)/I(0) at the planet's position; planet at the disc centre of a huge star: W -> 1; chords off the
+    stellar disc carry no light."""
+    R0, Rt = 1.0e7, 1.1e7
+    grid, opac = wl.uniform_medium(2, 1, 1, R0, Rt, 1.0e-3, 0.0)
+    base = wl.default_params(packets_per_channel=20000, seed=3, obs_dir=[[0, 0, 1.0]])
+    full = (Rt ** 2 - R0 ** 2) / 2
+    v0, _ = orc.reduce(orc.run_transmission(grid, opac, base), "transmission")
+    assert abs(v0[0, 0] / full - 1) < 0.01
+    Rs, c1, c2 = 7.0e8, 0.4, 0.25
+    for rho0 in (0.0, 0.5, 0.9):
+        prm = dict(base, star_radius=Rs, planet_xy=(rho0 * Rs, 0.0), ld_c1=c1, ld_c2=c2)
+        v, s = orc.reduce(orc.run_transmission(grid, opac, prm), "transmission")
+        mu0 = np.sqrt(1 - rho0 ** 2)
+        w = 1 - c1 * (1 - mu0) - c2 * (1 - mu0) ** 2
+        assert abs(v[0, 0] / (full * w) - 1) < 0.02 + 4 * s[0, 0] / v[0, 0], (rho0, v[0, 0] / full, w)
+    off = dict(base, star_radius=Rs, planet_xy=(1.5 * Rs, 0.0), ld_c1=c1, ld_c2=c2)
+    assert orc.run_transmission(grid, opac, off)["flux_sum"].sum() == 0.0
+    # brute force over the (zeta0, zeta1) square for a planet straddling the stellar limb
+    limb = dict(base, star_radius=5.0e7, planet_xy=(4.6e7, 1.0e6), ld_c1=c1, ld_c2=c2, packets_per_channel=80000)
+    v, s = orc.reduce(orc.run_transmission(grid, opac, limb), "transmission")
+    n = 600
+    z0, z1 = np.meshgrid((np.arange(n) + 0.5) / n, (np.arange(n) + 0.5) / n, indexing="ij")
+    bb = R0 + z0 * (Rt - R0)
+    sx, sy = 4.6e7 + bb * np.cos(2 * PI * z1), 1.0e6 + bb * np.sin(2 * PI * z1)
+    rho2 = (sx ** 2 + sy ** 2) / 5.0e7 ** 2
+    mu = np.sqrt(np.clip(1 - rho2, 0, None))
+    W = np.where(rho2 < 1, 1 - c1 * (1 - mu) - c2 * (1 - mu) ** 2, 0.0)
+    exact = np.mean(W * bb) * (Rt - R0)          # the annulus is opaque: 1 - exp(-tau) = 1 to 1e-9
+    assert abs(v[0, 0] - exact) < 4 * s[0, 0] + 2e-3 * exact, (v[0, 0], exact, s[0, 0])

@@ -73,6 +73,11 @@ typedef struct gcmcrt_run_params {
     double roulette_w_min;       /* Russian roulette (L200): when W < roulette_w_min after an interaction ... */
     double roulette_survive;     /* ... the packet survives with this probability and W <- W / roulette_survive
                                     (the paper states neither value; 0 disables).  Requires survival_bias. */
+    /* Transmission (Sect. 5.1.1): stellar disc behind the planet for the limb-darkening weight, Eq. 22-23 */
+    double star_radius;          /* R_star in m; 0 = no limb darkening (W = 1) */
+    double planet_xy[2];         /* sky-plane position of the planet centre relative to the stellar disc centre, m, in
+                                    the observer's image frame (e_x = z^ x o^ normalised, e_y = o^ x e_x) */
+    double ld_c1, ld_c2;         /* quadratic law I(mu)/I(0) = 1 - c1 (1 - mu) - c2 (1 - mu)^2 (Eq. 22) */
 } gcmcrt_run_params;
 
 typedef struct gcmcrt_counters {
@@ -151,6 +156,20 @@ int gcmcrt_set_opacity(gcmcrt_grid *grid, int chan0, int n_chan, const float *la
  */
 int gcmcrt_run_albedo(gcmcrt_grid *grid, const gcmcrt_run_params *params, gcmcrt_result *out, void *stream);
 int gcmcrt_run_emission(gcmcrt_grid *grid, const gcmcrt_run_params *params, gcmcrt_result *out, void *stream);
+
+/*
+ * gcmcrt_run_transmission -- transmission spectrum by random transit chords (Sect. 5.1, Eq. 20-21) with multiple
+ * scattering off (L259: "a raytracer scheme with random transit chord sampler"; the paper gives no formula for the
+ * scattered contribution).  Packet i of a channel draws an impact parameter b_i uniform in [R_p0, R_TOA] and an
+ * azimuth around the limb; tau_i is the extinction optical depth of the whole chord along obs_dir (planet -> observer)
+ * -- with doppler_on through that observer's Doppler-shifted table (Eq. 33-34, the set-up of the paper's Sect. 13).
+ *   flux_sum[c][o][batch] = sum_i W_i [1 - exp(-tau_i)] b_i      (W_i: limb darkening, Eq. 22-23; 1 if star_radius = 0)
+ *   value[c][o] = <I_p> = (R_TOA - R_p0) / N * sum  [m^2] (Eq. 21), sigma its batch-means standard error;
+ *   the caller forms (R_p / R_star)^2 = (R_p0^2 + 2 <I_p>) / R_star^2 (Eq. 20).
+ * star_dir, scatter_on, max_events, emission_bias, npix, image, event_count, contrib are not used.  n_obs >= 1.
+ * Errors: as gcmcrt_run_albedo.
+ */
+int gcmcrt_run_transmission(gcmcrt_grid *grid, const gcmcrt_run_params *params, gcmcrt_result *out, void *stream);
 
 /* gcmcrt_destroy -- synchronise the device, free everything the handle owns.  NULL is a no-op. */
 int gcmcrt_destroy(gcmcrt_grid *grid);

@@ -14,7 +14,8 @@ LIB_PATH = os.path.join(_HERE, "libgcmcrt.so")
 _lib = None
 
 OK, E_INVALID, E_NOMEM, E_CUDA, E_STATE = 0, -1, -2, -3, -4
-EXPORTS = ["gcmcrt_grid_create", "gcmcrt_set_opacity", "gcmcrt_run_albedo", "gcmcrt_run_emission", "gcmcrt_destroy",
+EXPORTS = ["gcmcrt_grid_create", "gcmcrt_set_opacity", "gcmcrt_run_albedo", "gcmcrt_run_emission",
+           "gcmcrt_run_transmission", "gcmcrt_destroy",
            "gcmcrt_last_error", "gcmcrt_debug_ray_tau", "gcmcrt_debug_philox", "gcmcrt_version"]
 
 
@@ -31,7 +32,8 @@ class RunParams(C.Structure):
                 ("max_events", C.c_int), ("scatter_on", C.c_int), ("doppler_on", C.c_int),
                 ("doppler_halfwidth", C.c_int), ("emission_bias", C.c_double), ("tau_vert_max", C.c_double),
                 ("tau_cut", C.c_double), ("npix", C.c_int), ("n_batches", C.c_int),
-                ("survival_bias", C.c_int), ("roulette_w_min", C.c_double), ("roulette_survive", C.c_double)]
+                ("survival_bias", C.c_int), ("roulette_w_min", C.c_double), ("roulette_survive", C.c_double),
+                ("star_radius", C.c_double), ("planet_xy", C.c_double * 2), ("ld_c1", C.c_double), ("ld_c2", C.c_double)]
 
 
 class Counters(C.Structure):
@@ -65,6 +67,7 @@ def lib():
         L.gcmcrt_set_opacity.argtypes = [C.c_void_p, C.c_int, C.c_int] + [C.c_void_p] * 6
         L.gcmcrt_run_albedo.argtypes = [C.c_void_p, C.POINTER(RunParams), C.POINTER(Result), C.c_void_p]
         L.gcmcrt_run_emission.argtypes = [C.c_void_p, C.POINTER(RunParams), C.POINTER(Result), C.c_void_p]
+        L.gcmcrt_run_transmission.argtypes = [C.c_void_p, C.POINTER(RunParams), C.POINTER(Result), C.c_void_p]
         L.gcmcrt_destroy.argtypes = [C.c_void_p]
         L.gcmcrt_debug_ray_tau.argtypes = [C.c_void_p, C.c_int, C.c_long] + [C.c_void_p] * 5
         L.gcmcrt_debug_philox.argtypes = [C.c_long] + [C.c_void_p] * 4
@@ -158,6 +161,10 @@ def make_params(prm):
     p.survival_bias = int(prm.get("survival_bias", 0))
     p.roulette_w_min = float(prm.get("roulette_w_min", 0.0))
     p.roulette_survive = float(prm.get("roulette_survive", 0.0))
+    p.star_radius = float(prm.get("star_radius", 0.0))
+    xy = prm.get("planet_xy", (0.0, 0.0))
+    p.planet_xy[0], p.planet_xy[1] = float(xy[0]), float(xy[1])
+    p.ld_c1, p.ld_c2 = float(prm.get("ld_c1", 0.0)), float(prm.get("ld_c2", 0.0))
     return p, obs
 
 
@@ -210,6 +217,10 @@ def run_emission(handle, prm, n_chan_table, want_event_count=False, want_image=T
                 want_contrib)
 
 
+def run_transmission(handle, prm, n_chan_table, device_outputs=False, stream=None):
+    return _run(lib().gcmcrt_run_transmission, handle, prm, n_chan_table, False, False, device_outputs, stream)
+
+
 def debug_ray_tau(handle, chan, pos, dirs, stream=None):
     pos = np.ascontiguousarray(pos, dtype=np.float32).reshape(-1, 3)
     dirs = np.ascontiguousarray(dirs, dtype=np.float32).reshape(-1, 3)
@@ -252,6 +263,9 @@ class Grid:
 
     def run_emission(self, prm, **kw):
         return run_emission(self.handle, prm, self.n_chan, stream=self.stream, **kw)
+
+    def run_transmission(self, prm, **kw):
+        return run_transmission(self.handle, prm, self.n_chan, stream=self.stream, **kw)
 
     def ray_tau(self, chan, pos, dirs):
         return debug_ray_tau(self.handle, chan, pos, dirs, self.stream)

@@ -267,8 +267,10 @@ int bind_out(gcmcrt_grid* g, void* user, size_t bytes, DevBuf& own, OutBuf& ob, 
     return GCMCRT_OK;
 }
 
-int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, void* stream, int emission)
+// mode: 0 albedo, 1 emission, 2 transmission
+int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, void* stream, int mode)
 {
+    const int emission = mode == 1;
     if (!g) return GCMCRT_E_INVALID;
     if (!prm || !out) return fail(g, GCMCRT_E_INVALID, "params and result must not be NULL");
     if (g->n_chan <= 0 || g->staged_obs == -2) return fail(g, GCMCRT_E_STATE, "gcmcrt_set_opacity has not been called");
@@ -327,6 +329,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.pkt_begin = uint32_t(lo); rc.n_pkt = uint32_t(n_pkt);
     rc.N = N; rc.seed = prm->seed;
     rc.mode = emission;
+    if (mode == 2 && n_obs < 1) return fail(g, GCMCRT_E_INVALID, "transmission needs at least one observer direction");
     rc.max_events = prm->max_events; rc.scatter_on = prm->scatter_on;
     rc.survival_bias = prm->survival_bias != 0;
     rc.roulette_w_min = float(prm->roulette_w_min); rc.roulette_survive = float(prm->roulette_survive);
@@ -445,6 +448,36 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
 
         // ---- pass loop
         const unsigned long long total_items = (unsigned long long)ncr * n_pkt;
+        if (mode == 2) {
+            // ---- transmission (Sect. 5.1): one chord per packet and observer, no events, no passes
+            auto k_tr = transmission_kernel<8>;
+            int occ_tr = 1;
+            CUDA_TRY(g, cudaFuncSetAttribute(k_tr, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_t)));
+            CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tr, k_tr, 256, smem_t));
+            if (occ_tr < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
+            CUDA_TRY(g, cudaEventRecord(g->tev[2], s));
+            for (int o = rc.obs_first; o < rc.obs_first + rc.n_obs_run; ++o) {
+                TransParams tp;
+                tp.o = o;
+                for (int m = 0; m < 3; ++m) { tp.ex[m] = rc.img_ex[o][m]; tp.ey[m] = rc.img_ey[o][m]; }
+                tp.star_radius = float(prm->star_radius);
+                tp.planet_x = float(prm->planet_xy[0]); tp.planet_y = float(prm->planet_xy[1]);
+                tp.ld_c1 = float(prm->ld_c1); tp.ld_c2 = float(prm->ld_c2);
+                const unsigned gt = (unsigned)std::min<unsigned long long>((total_items + 255) / 256, (unsigned long long)g->sm_count * occ_tr);
+                k_tr<<<std::max(gt, 1u), 256, smem_t, s>>>(rc, tp, total_items);
+                ++g->launches;
+            }
+            CUDA_TRY(g, cudaEventRecord(g->tev[3], s));
+            CUDA_TRY(g, cudaGetLastError());
+            CUDA_TRY(g, cudaEventSynchronize(g->tev[3]));
+            {
+                float c = 0.f;
+                CUDA_TRY(g, cudaEventElapsedTime(&c, g->tev[2], g->tev[3]));
+                g->ms_peel += c;
+            }
+            ++passes;
+            continue;
+        }
         CUDA_TRY(g, cudaMemsetAsync(ctrl, 0, sizeof(PassCtrl), s));
         int cur = 0;
         const size_t smem_p = (size_t((g->tab_floats + 31) & ~31) + size_t(kPeelThreads / 32) * rc.n_obs_run * nb) * sizeof(float);
@@ -619,7 +652,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     if (n_obs > 0) {
         const int nt = ncr * n_obs;
         normalise_kernel<<<(nt + 127) / 128, 128, 0, s>>>(ncr, n_obs, nb, N, lo, hi, static_cast<double*>(o_flux.dev),
-                                                         static_cast<double*>(o_ltot.dev), emission,
+                                                         static_cast<double*>(o_ltot.dev), mode,
+                                                         g->r[g->nlev] - g->r[0],
                                                          static_cast<double*>(o_val.dev), static_cast<double*>(o_sig.dev));
         CUDA_TRY(g, cudaGetLastError());
         ++g->launches;
@@ -790,6 +824,11 @@ int gcmcrt_run_albedo(gcmcrt_grid* g, const gcmcrt_run_params* p, gcmcrt_result*
 int gcmcrt_run_emission(gcmcrt_grid* g, const gcmcrt_run_params* p, gcmcrt_result* out, void* stream)
 {
     return run_mode(g, p, out, stream, 1);
+}
+
+int gcmcrt_run_transmission(gcmcrt_grid* g, const gcmcrt_run_params* p, gcmcrt_result* out, void* stream)
+{
+    return run_mode(g, p, out, stream, 2);
 }
 
 int gcmcrt_destroy(gcmcrt_grid* g)

@@ -841,11 +841,110 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Transmission (Sect. 5.1, Eq. 20-23): one random transit chord per packet, toward observer `o`.
+// ---------------------------------------------------------------------------------------------------------
+struct TransParams {
+    int o;                   // observer index (row of rc.obs, column of flux)
+    float ex[3], ey[3];      // sky-plane frame of the observer (C19)
+    float star_radius, planet_x, planet_y, ld_c1, ld_c2;
+};
+
+template <int KSTEPS>
+__global__ void __launch_bounds__(256, 3)
+transmission_kernel(const __grid_constant__ RunConst rc, const TransParams tp, const unsigned long long total_items)
+{
+    extern __shared__ float smem_f[];
+    const GeomSmem gs = load_geom(rc.geom, smem_f);
+    __syncthreads();
+    const float ox = rc.obs[tp.o][0], oy = rc.obs[tp.o][1], oz = rc.obs[tp.o][2];
+    const float R0 = rc.geom.R0, Rt = rc.geom.Rtoa;
+    unsigned long long c_seg = 0, c_ev = 0, c_stuck = 0;
+    const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+    for (unsigned long long base = ((unsigned long long)blockIdx.x * blockDim.x + threadIdx.x) & ~31ull; base < total_items;
+         base += stride) {
+        const unsigned long long item = base + lane_id();
+        const bool active = item < total_items;
+        uint32_t chan_run = 0, pkt = 0;
+        Ray ray{};
+        float b = 0.f, W = 0.f, tau = 0.f;
+        int st = RAY_NONE;
+        const float* alpha_c = rc.alpha;
+        if (active) {
+            chan_run = uint32_t(div_magic(item, rc.n_pkt, rc.magic_npkt));
+            pkt = rc.pkt_begin + uint32_t(item - (unsigned long long)chan_run * rc.n_pkt);
+            const int ctab = rc.chan_begin + int(chan_run);
+            alpha_c = rc.alpha + (size_t)ctab * rc.geom.alpha_stride;
+            const Zeta4 z = zeta_block(rc.seed, rc.chan_key0 + uint32_t(ctab), pkt, 0, 0);
+            b = fmaf(z.z0, Rt - R0, R0);                       // uniform in b: Eq. 21 carries the factor b_i
+            float sp, cp;
+            sincospif(2.0f * z.z1, &sp, &cp);
+            const float X = b * cp, Y = b * sp, h = sqrtf(fmaxf(0.f, (Rt - b) * (Rt + b)));
+            const float px = X * tp.ex[0] + Y * tp.ey[0] - h * ox;
+            const float py = X * tp.ex[1] + Y * tp.ey[1] - h * oy;
+            const float pz = X * tp.ex[2] + Y * tp.ey[2] - h * oz;
+            W = 1.0f;
+            if (tp.star_radius > 0.f) {                         // Eq. 22-23
+                const float sx = (tp.planet_x + X) / tp.star_radius, sy = (tp.planet_y + Y) / tp.star_radius;
+                const float rho2 = fmaf(sx, sx, sy * sy);
+                const float mu1 = 1.0f - sqrtf(fmaxf(0.f, 1.0f - rho2));
+                W = rho2 >= 1.0f ? 0.f : 1.0f - tp.ld_c1 * mu1 - tp.ld_c2 * mu1 * mu1;
+            }
+            int j, k;
+            locate_angles(gs, px, py, pz, j, k);
+            ray_init(ray, gs, px, py, pz, ox, oy, oz, gs.nlev - 1, j, k, alpha_c);
+            st = RAY_FLYING;
+            ++c_ev;
+        }
+        unsigned int seg32 = 0;
+        for (int it = 0; it <= rc.geom.maxseg; it += KSTEPS) {
+            const unsigned m_fly = __ballot_sync(kFullMask, st == RAY_FLYING);
+            const unsigned m_park = __ballot_sync(kFullMask, st == RAY_PARK);
+            if ((m_fly | m_park) == 0) break;
+            if (m_park && (__popc(m_park) >= rc.t_lateral || m_fly == 0)) {
+                if (st == RAY_PARK) { ray_lateral(ray, gs, alpha_c); st = RAY_FLYING; }
+            }
+#pragma unroll 1
+            for (int s = 0; s < KSTEPS && st == RAY_FLYING; ++s) {
+                ++seg32;
+                st = ray_step(ray, gs, tau, rc.tau_cut);     // beyond tau_cut the chord is opaque: 1 - e^-tau = 1
+            }
+        }
+        c_seg += seg32;
+        float v = 0.f;
+        if (active) {
+            if (st == RAY_ESCAPE) v = W * b * -expm1f(-tau);
+            else if (st == RAY_LIMIT || st == RAY_SURFACE) v = W * b;
+            else ++c_stuck;
+        }
+        // items of a warp are consecutive packets: (channel, batch) runs are contiguous -> segmented reduction
+        const int key = active ? int(chan_run) * rc.n_batches + int(batch_of(rc, pkt)) : -1;
+        double dv = double(v);
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const double w = __shfl_down_sync(kFullMask, dv, off);
+            const int kk = __shfl_down_sync(kFullMask, key, off);
+            if (lane_id() + off < 32 && kk == key) dv += w;
+        }
+        const int kp = __shfl_up_sync(kFullMask, key, 1);
+        if (active && (lane_id() == 0 || kp != key) && dv != 0.0) {
+            const int bt = key - int(chan_run) * rc.n_batches;
+            atomicAdd(rc.flux + ((size_t)chan_run * rc.n_obs_total + tp.o) * rc.n_batches + bt, dv);
+        }
+    }
+    c_seg = warp_sum_u64(c_seg); c_ev = warp_sum_u64(c_ev); c_stuck = warp_sum_u64(c_stuck);
+    if (lane_id() == 0) {
+        if (c_seg) atomicAdd(&rc.counters->seg_peel, c_seg);
+        if (c_ev) { atomicAdd(&rc.counters->events, c_ev); atomicAdd(&rc.counters->rays_peel, c_ev); }
+        if (c_stuck) atomicAdd(&rc.counters->stuck, c_stuck);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // A10: value and batch-means sigma (C12) per (channel, observer).
 // ---------------------------------------------------------------------------------------------------------
 __global__ void normalise_kernel(int n_chan_run, int n_obs, int n_batches, unsigned long long N, unsigned long long lo,
                                  unsigned long long hi, const double* __restrict__ flux, const double* __restrict__ Ltot,
-                                 int emission, double* __restrict__ value, double* __restrict__ sigma)
+                                 int emission, double scale_const, double* __restrict__ value, double* __restrict__ sigma)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n_chan_run * n_obs) return;
@@ -869,7 +968,7 @@ __global__ void normalise_kernel(int n_chan_run, int n_obs, int n_batches, unsig
         const double var = fmax(0.0, (m2 - used * mu * mu) / (used - 1));
         sg = sqrt(var / used);
     }
-    const double scale = emission ? Ltot[t] : 1.0;
+    const double scale = emission == 1 ? Ltot[t] : (emission == 2 ? scale_const : 1.0);   // Eq. 28 | Eq. 21 | Eq. 24
     if (value) value[t] = mean * scale;
     if (sigma) sigma[t] = sg * scale;
 }

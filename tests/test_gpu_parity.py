@@ -397,6 +397,41 @@ def test_contribution_functions_match_oracle(gpu, orc):
     assert np.allclose(a["contrib"][:, :, 1].sum(axis=2), a["flux_sum"].sum(axis=2), rtol=2e-4)
 
 
+def test_transmission_matches_oracle(gpu, orc):
+    """Sect. 5.1, Eq. 20-23: random transit chords on the GPU against the oracle (same chords: same Philox block),
+    on a 3D correlated-k table with two viewing directions, with limb darkening, and through Doppler-shifted tables."""
+    grid, opac, prm = wl.cfg2(nlon=16, nlat=8, nlev=20, nbands=2, ng=3, packets=30000)
+    obs = np.array([[1.0, 0, 0], [0.36, -0.48, 0.8]])
+    prm = dict(prm, obs_dir=obs, star_radius=7.0e8, planet_xy=(3.0e8, -2.0e8), ld_c1=0.4, ld_c2=0.2)
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        g = G.run_transmission(prm)
+    o = orc.run_transmission(grid, opac, prm)
+    vo, so = orc.reduce(o, "transmission")
+    assert np.all(np.abs(g["value"] - vo) <= 4 * so + 1e-5 * np.abs(vo))
+    assert np.allclose(g["flux_sum"], o["flux_sum"], rtol=2e-4)          # batch by batch: the same chords
+    assert np.allclose(g["sigma"], so, rtol=1e-2)
+    assert g["counters"]["events"] == 2 * 6 * 30000 and g["counters"]["packets_stuck"] == 0
+    # the kernel stops a chord at tau_cut (1 - exp(-50) = 1 in fp32), the oracle integrates every chord to the end
+    assert 0 < g["counters"]["segments_peel"] <= o["counters"]["segments_peel"]
+    # opaque atmosphere, no limb darkening: R_p = R_TOA (Eq. 20)
+    R0, Rt = 1.0e7, 1.2e7
+    grid2, opac2 = wl.uniform_medium(5, 4, 6, R0, Rt, 1.0e-3, 0.5)
+    with gpu.Grid(grid2) as G:
+        G.set_opacity(opac2)
+        t = G.run_transmission(wl.default_params(packets_per_channel=20000, seed=2, obs_dir=[[0, 0.6, 0.8]]))
+    assert abs(R0 ** 2 + 2 * t["value"][0, 0] - Rt ** 2) < 4 * 2 * t["sigma"][0, 0] + 1e-3 * Rt ** 2
+    # Doppler-shifted chords (the paper's high-resolution transmission set-up, Sect. 13)
+    grid4, opac4, prm4 = wl.cfg4(nlon=12, nlat=6, nlev=16, n_chan=24, n_lines=20, packets=4000)
+    prm4 = dict(prm4, obs_dir=np.array([[-1.0, 0, 0], [0, 1.0, 0]]))
+    with gpu.Grid(grid4) as G:
+        G.set_opacity(opac4)
+        g4 = G.run_transmission(prm4)
+    o4 = orc.run_transmission(grid4, opac4, prm4)
+    v4, s4 = orc.reduce(o4, "transmission")
+    assert np.all(np.abs(g4["value"] - v4) <= 4 * s4 + 1e-4 * np.abs(v4))
+
+
 def test_error_paths(gpu):
     grid, opac, prm = wl.cfg1(packets=100)
     with gpu.Grid(grid) as G:

@@ -36,7 +36,7 @@ class _Params(C.Structure):
                 ("emission_bias", C.c_double), ("tau_vert_max", C.c_double), ("tau_cut", C.c_double),
                 ("npix", C.c_int), ("n_batches", C.c_int), ("n_threads", C.c_int),
                 ("survival_bias", C.c_int), ("roulette_w_min", C.c_double), ("roulette_survive", C.c_double),
-                ("star_radius", C.c_double), ("planet_xy", C.c_double * 2), ("ld_c1", C.c_double), ("ld_c2", C.c_double)]
+                ("star_radius", C.c_double), ("planet_xy", C.c_double * 2), ("ld_c1", C.c_double), ("ld_c2", C.c_double), ("cloud_phase", C.c_int)]
 
 
 class _Counters(C.Structure):
@@ -61,7 +61,9 @@ def lib():
         for name in ("orc_sample_isotropic", "orc_sample_lambert", "orc_sample_rayleigh", "orc_phase_rayleigh"):
             getattr(L, name).restype = C.c_double
             getattr(L, name).argtypes = [C.c_double]
-        for name in ("orc_sample_hg", "orc_phase_hg", "orc_planck"):
+        L.orc_sample_tthg.restype = C.c_double
+        L.orc_sample_tthg.argtypes = [C.c_double] * 3
+        for name in ("orc_sample_hg", "orc_phase_hg", "orc_phase_tthg", "orc_planck"):
             getattr(L, name).restype = C.c_double
             getattr(L, name).argtypes = [C.c_double, C.c_double]
         L.orc_cell_volume.restype = C.c_double
@@ -112,6 +114,8 @@ def sample_rayleigh(z): return lib().orc_sample_rayleigh(z)
 def sample_hg(g, z): return lib().orc_sample_hg(g, z)
 def phase_rayleigh(mu): return lib().orc_phase_rayleigh(mu)
 def phase_hg(g, mu): return lib().orc_phase_hg(g, mu)
+def phase_tthg(g, mu): return lib().orc_phase_tthg(g, mu)
+def sample_tthg(g, zl, z): return lib().orc_sample_tthg(g, zl, z)
 def planck(lam, T): return lib().orc_planck(lam, T)
 
 
@@ -197,6 +201,7 @@ def _params_struct(prm, keep):
     xy = prm.get("planet_xy", (0.0, 0.0))
     p.planet_xy[0], p.planet_xy[1] = float(xy[0]), float(xy[1])
     p.ld_c1, p.ld_c2 = float(prm.get("ld_c1", 0.0)), float(prm.get("ld_c2", 0.0))
+    p.cloud_phase = int(prm.get("cloud_phase", 0))
     return p
 
 

@@ -93,6 +93,19 @@ double orc_phase_hg(double g, double mu)
     return (1.0 - g * g) / (4.0 * PI * d * sqrt(d));
 }
 
+/* Eq. 10: two-term HG with the default g1 = g, g2 = -g/2, alpha = 1 - g2^2. */
+double orc_phase_tthg(double g, double mu)
+{
+    const double g2 = -0.5 * g, a = 1.0 - g2 * g2;
+    return a * orc_phase_hg(g, mu) + (1.0 - a) * orc_phase_hg(g2, mu);
+}
+/* L152: zeta_lobe < alpha -> Eq. 8 with g1, else Eq. 8 with g2. */
+double orc_sample_tthg(double g, double zeta_lobe, double zeta)
+{
+    const double g2 = -0.5 * g, a = 1.0 - g2 * g2;
+    return zeta_lobe < a ? orc_sample_hg(g, zeta) : orc_sample_hg(g2, zeta);
+}
+
 /* C9: rotate n by polar angle acos(ct) and azimuth psi. */
 void orc_rotate(const double n[3], double ct, double psi, double out[3])
 {
@@ -533,7 +546,8 @@ static void peel(const run_ctx *rc, const double p[3], const int ijk[3], int kin
         double pref;
         if (kind == 0) {            /* medium interaction, C6: mixture phase function */
             double mu = dot3(nin, od);
-            double theta = pgas * orc_phase_rayleigh(mu) + (1.0 - pgas) * orc_phase_hg(gg, mu);
+            double cld = rc->prm->cloud_phase == 1 ? orc_phase_tthg(gg, mu) : orc_phase_hg(gg, mu);
+            double theta = pgas * orc_phase_rayleigh(mu) + (1.0 - pgas) * cld;
             pref = W * omega * theta;
         } else if (kind == 1) {     /* thermal emission: isotropic, no omega (O4) */
             pref = W / (4.0 * PI);
@@ -557,6 +571,13 @@ static void peel(const run_ctx *rc, const double p[3], const int ijk[3], int kin
         if (rc->contrib)   /* Sect. 6: the contribution of the event's cell to the output, thermal / scattered apart */
             rc->contrib[((size_t)o * 2 + (kind == 1 ? 0 : 1)) * G->ncell + cell_index(G, ijk[0], ijk[1], ijk[2])] += f;
     }
+}
+
+/* Cloud scatterer: HG, or TTHG whose lobe is picked by the part of zeta0 left over inside the cloud interval of the
+ * partition (uniform in [0,1) given that the cloud was chosen), so that no extra draw is needed. */
+static double sample_cloud(const orc_params *prm, double gg, double zlobe, double zeta)
+{
+    return prm->cloud_phase == 1 ? orc_sample_tthg(gg, zlobe, zeta) : orc_sample_hg(gg, zeta);
 }
 
 /* O6/O7/O5 loop shared by both modes.  m = number of peel-off points so far. */
@@ -609,11 +630,11 @@ static void transport(const run_ctx *rc, uint32_t pkt, double p[3], double n[3],
                 if (zr[0] >= prm->roulette_survive) { cnt->packets_absorbed++; break; }
                 W /= prm->roulette_survive;
             }
-            ct = (z[0] < pgas) ? orc_sample_rayleigh(z[1]) : orc_sample_hg(gg, z[1]);
+            ct = (z[0] < pgas) ? orc_sample_rayleigh(z[1]) : sample_cloud(prm, gg, (z[0] - pgas) / (1.0 - pgas), z[1]);
         } else {
             if (z[0] >= omega) { cnt->packets_absorbed++; break; }     /* Sect. 4.4: analog absorption */
             ct = (z[0] < omega * pgas) ? orc_sample_rayleigh(z[1])  /* Eq. 11 + C6 partition */
-                                       : orc_sample_hg(gg, z[1]);
+                                       : sample_cloud(prm, gg, (z[0] - omega * pgas) / (omega - omega * pgas), z[1]);
         }
         double nn[3];
         orc_rotate(n, ct, 2.0 * PI * z[2], nn);

@@ -84,6 +84,8 @@ typedef struct {
     double planet_xy[2];     /* sky-plane position of the planet centre relative to the stellar disc centre, m, in
                                 the observer's image frame (C19: e_x = z^ x o^ normalised, e_y = o^ x e_x) */
     double ld_c1, ld_c2;     /* quadratic limb-darkening law, Eq. 22 */
+    int cloud_phase;         /* cloud scatterers: 0 = HG (Eq. 7-8), 1 = two-term HG (Eq. 10) with the paper's default
+                                g1 = g, g2 = -g/2, alpha = 1 - g2^2 (L157) */
 } orc_params;
 
 typedef struct {
@@ -118,6 +120,9 @@ double orc_sample_rayleigh(double zeta);
 double orc_sample_hg(double g, double zeta);
 double orc_phase_rayleigh(double mu);
 double orc_phase_hg(double g, double mu);
+/* Eq. 10 with g1 = g, g2 = -g/2, alpha = 1 - g2^2 (L157); zeta_lobe < alpha picks the forward lobe (L152) */
+double orc_sample_tthg(double g, double zeta_lobe, double zeta);
+double orc_phase_tthg(double g, double mu);
 /* C9: rotate unit vector n by polar angle acos(ct) and azimuth psi. */
 void orc_rotate(const double n[3], double ct, double psi, double out[3]);
 

@@ -769,3 +769,47 @@ def test_transmission_limb_darkening_weights(orc):
     W = np.where(rho2 < 1, 1 - c1 * (1 - mu) - c2 * (1 - mu) ** 2, 0.0)
     exact = np.mean(W * bb) * (Rt - R0)          # the annulus is opaque: 1 - exp(-tau) = 1 to 1e-9
     assert abs(v[0, 0] - exact) < 4 * s[0, 0] + 2e-3 * exact, (v[0, 0], exact, s[0, 0])
+
+
+# ----------------------------------------------------------------------------- Eq. 10: two-term Henyey-Greenstein
+@pytest.mark.parametrize("g", [0.3, 0.6, 0.85])
+def test_tthg_density_and_sampler(orc, g):
+    """Eq. 10 with g1 = g, g2 = -g/2, alpha = 1 - g2^2 (L157): normalised, <cos> = alpha g1 + (1 - alpha) g2, and the
+    two-draw sampler (L152) reproduces the density (histogram against the bin integrals of the closed-form CDFs)."""
+    g2, a = -g / 2, 1 - g * g / 4
+    mu = np.linspace(-1, 1, 40001)
+    dens = np.array([orc.phase_tthg(g, m) for m in mu])
+    assert abs(np.trapezoid(dens, mu) * 2 * PI - 1) < 2e-4
+    assert abs(np.trapezoid(dens * mu, mu) * 2 * PI - (a * g + (1 - a) * g2)) < 2e-4
+    assert np.allclose(dens, a * np.array([orc.phase_hg(g, m) for m in mu]) + (1 - a) * np.array([orc.phase_hg(g2, m) for m in mu]))
+    # L152: zeta_lobe < alpha -> Eq. 8 with g1, else Eq. 8 with g2 (Eq. 8 itself is pinned by its CDF above); the mean
+    # over the unit square of draws is then alpha g1 + (1 - alpha) g2
+    for z in _mid(50):
+        assert orc.sample_tthg(g, 0.5 * a, z) == orc.sample_hg(g, z)
+        assert orc.sample_tthg(g, a - 1e-12, z) == orc.sample_hg(g, z)
+        assert orc.sample_tthg(g, a + 1e-12, z) == orc.sample_hg(g2, z)
+        assert orc.sample_tthg(g, 0.5 * (1 + a), z) == orc.sample_hg(g2, z)
+    zz = _mid(20000)
+    m1 = np.mean([orc.sample_hg(g, x) for x in zz]); m2 = np.mean([orc.sample_hg(g2, x) for x in zz])
+    assert abs(a * m1 + (1 - a) * m2 - np.trapezoid(dens * mu, mu) * 2 * PI) < 3e-4
+
+
+def test_tthg_transport_keeps_peel_escape_consistency(orc):
+    """With the TTHG cloud phase function the 4 pi-integrated peel-off still equals the weight that escapes after
+    scattering (the peel-off density and the sampler describe the same function), omega = 1, reflecting floor."""
+    R0, Rt = 1.0e6, 1.3e6
+    grid, opac = wl.uniform_medium(4, 3, 4, R0, Rt, 2.0 / (Rt - R0), 1.0, g=0.7, pgas=0.25, surface_albedo=1.0)
+    nmu, nphi = 10, 10
+    x, w = np.polynomial.legendre.leggauss(nmu)
+    obs = [[np.sqrt(1 - a * a) * np.cos(2 * PI * (q + .5) / nphi), np.sqrt(1 - a * a) * np.sin(2 * PI * (q + .5) / nphi), a]
+           for a in x for q in range(nphi)]
+    wq = np.repeat(w, nphi) * 2 * PI / nphi
+    N = 20000
+    prm = wl.default_params(packets_per_channel=N, seed=14, obs_dir=np.array(obs), cloud_phase=1)
+    res = orc.run_albedo(grid, opac, prm, want_event_count=True)
+    val, sig = orc.reduce(res, "albedo")
+    scattered = (res["event_count"][0] > 0).mean()          # every packet escapes (omega = a = 1): those with >= 1 event
+    total = np.sum(val[0] * wq)
+    assert abs(total - scattered) < 4 * np.sqrt(np.sum((sig[0] * wq) ** 2)) + 0.01, (total, scattered)
+    hg = orc.run_albedo(grid, opac, dict(prm, cloud_phase=0))
+    assert not np.allclose(hg["flux_sum"], res["flux_sum"])

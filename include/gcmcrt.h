@@ -78,6 +78,8 @@ typedef struct gcmcrt_run_params {
     double planet_xy[2];         /* sky-plane position of the planet centre relative to the stellar disc centre, m, in
                                     the observer's image frame (e_x = z^ x o^ normalised, e_y = o^ x e_x) */
     double ld_c1, ld_c2;         /* quadratic law I(mu)/I(0) = 1 - c1 (1 - mu) - c2 (1 - mu)^2 (Eq. 22) */
+    int cloud_phase;             /* phase function of the cloud scatterers: 0 = Henyey-Greenstein (Eq. 7-8), 1 = two-term
+                                    HG (Eq. 10) with the paper's default g1 = g, g2 = -g/2, alpha = 1 - g2^2 (L157) */
 } gcmcrt_run_params;
 
 typedef struct gcmcrt_counters {

@@ -332,6 +332,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     if (mode == 2 && n_obs < 1) return fail(g, GCMCRT_E_INVALID, "transmission needs at least one observer direction");
     rc.max_events = prm->max_events; rc.scatter_on = prm->scatter_on;
     rc.survival_bias = prm->survival_bias != 0;
+    rc.cloud_phase = prm->cloud_phase;
+    if (prm->cloud_phase != 0 && prm->cloud_phase != 1) return fail(g, GCMCRT_E_INVALID, "cloud_phase must be 0 (HG) or 1 (TTHG)");
     rc.roulette_w_min = float(prm->roulette_w_min); rc.roulette_survive = float(prm->roulette_survive);
     rc.surface_albedo = g->surface_albedo;
     rc.xi = prm->emission_bias;

@@ -90,6 +90,7 @@ struct RunConst {
     int max_events, scatter_on;
     int survival_bias;             // Sect. 4.4: forced scattering with W <- W omega
     float roulette_w_min, roulette_survive;   // Sect. 4.5: Russian roulette below the weight threshold (0 = off)
+    int cloud_phase;               // 0 HG (Eq. 7-8), 1 two-term HG (Eq. 10, g1 = g, g2 = -g/2, alpha = 1 - g2^2)
     float surface_albedo;
     double xi;
     int n_batches;
@@ -294,6 +295,29 @@ __device__ __forceinline__ float sample_hg(float g, float z)
     const float t = (1.0f - g * g) / (1.0f - g + 2.0f * g * z);
     return (1.0f + g * g - t * t) / (2.0f * g);
 }
+// Cloud scatterer: HG, or the two-term HG of Eq. 10 whose lobe is picked by zlobe (L152), the part of zeta0 left over
+// inside the cloud interval of the partition.
+__device__ __forceinline__ float sample_cloud(int cloud_phase, float g, float zlobe, float z)
+{
+    if (cloud_phase == 1) {
+        const float g2 = -0.5f * g, a = 1.0f - g2 * g2;
+        return sample_hg(zlobe < a ? g : g2, z);
+    }
+    return sample_hg(g, z);
+}
+__device__ __forceinline__ float phase_hg(float g, float mu)
+{
+    const float d = fmaf(-2.0f * g, mu, 1.0f + g * g);
+    return (1.0f - g * g) / (4.0f * kPi * d * sqrtf(d));
+}
+__device__ __forceinline__ float phase_cloud(int cloud_phase, float g, float mu)
+{
+    if (cloud_phase == 1) {
+        const float g2 = -0.5f * g, a = 1.0f - g2 * g2;
+        return a * phase_hg(g, mu) + (1.0f - a) * phase_hg(g2, mu);
+    }
+    return phase_hg(g, mu);
+}
 // C9: rotate n by polar angle acos(ct), azimuth psi = 2 pi zpsi
 __device__ __forceinline__ void rotate_dir(float& nx, float& ny, float& nz, float ct, float zpsi)
 {
@@ -329,11 +353,12 @@ __device__ __forceinline__ bool medium_interaction(const RunConst& rc, const flo
             if (zr.z0 >= rc.roulette_survive) return false;
             W /= rc.roulette_survive;
         }
-        ct = (z.z0 < pr.y) ? sample_rayleigh(z.z1) : sample_hg(pr.z, z.z1);
+        ct = (z.z0 < pr.y) ? sample_rayleigh(z.z1) : sample_cloud(rc.cloud_phase, pr.z, (z.z0 - pr.y) / (1.0f - pr.y), z.z1);
         return true;
     }
     if (z.z0 >= pr.x) return false;
-    ct = (z.z0 < pr.x * pr.y) ? sample_rayleigh(z.z1) : sample_hg(pr.z, z.z1);
+    const float lo = pr.x * pr.y;
+    ct = (z.z0 < lo) ? sample_rayleigh(z.z1) : sample_cloud(rc.cloud_phase, pr.z, (z.z0 - lo) / (pr.x - lo), z.z1);
     return true;
 }
 
@@ -754,8 +779,7 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
                 const float mu = b.x * ox + b.y * oy + b.z * oz;
                 float theta;
                 if (kind == EV_MEDIUM) {  // C6: mixture phase function, per steradian (Eq. 5, Eq. 7)
-                    const float d = fmaf(-2.0f * g, mu, 1.0f + g * g);
-                    const float hg = (1.0f - g * g) / (4.0f * kPi * d * sqrtf(d));
+                    const float hg = phase_cloud(rc.cloud_phase, g, mu);
                     const float ray_p = 3.0f * (1.0f + mu * mu) / (16.0f * kPi);
                     theta = pgas * ray_p + (1.0f - pgas) * hg;
                 } else if (kind == EV_EMIT) {

@@ -332,6 +332,19 @@ def test_survival_biasing_and_roulette_parity(gpu, orc, monkeypatch, tune):
         assert e.value.code == gpu.E_INVALID
 
 
+def test_tthg_cloud_phase_function_parity(gpu, orc):
+    """Eq. 10 (two-term HG, g1 = g, g2 = -g/2, alpha = 1 - g2^2) in the sampler and in the peel-off density."""
+    grid, opac, prm = wl.cfg2(nlon=16, nlat=8, nlev=20, nbands=2, ng=3, packets=20000)
+    opac = dict(opac, g_cld=np.full_like(opac["g_cld"], 0.8))
+    obs = np.array([[1.0, 0, 0], [-0.6, 0.0, 0.8]])
+    prm = dict(prm, cloud_phase=1, obs_dir=obs)
+    g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+    o = orc.run_albedo(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
+    _check_parity(orc, g, o, "albedo")
+    hg = _gpu_run(gpu, grid, opac, dict(prm, cloud_phase=0), "albedo")
+    assert np.any(np.abs(hg["value"] - g["value"]) > 4 * np.hypot(hg["sigma"], g["sigma"]))    # a different function
+
+
 def test_packet_and_channel_subranges_compose(gpu):
     grid, opac, prm = wl.cfg2(nlon=8, nlat=4, nlev=10, nbands=1, ng=4, packets=20000)
     full = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)

@@ -234,7 +234,8 @@ __device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, f
     const float ds = fmaxf(un - r.u, 0.0f);
     const float tnew = fmaf(r.alpha, ds, tau);
     if (tnew >= tau_limit) {  // the limit is reached inside this cell
-        r.u += (tau_limit - tau) / r.alpha;
+        r.u += __fdividef(tau_limit - tau, r.alpha);   // MUFU.RCP + FMUL: the IEEE sequence is 20 instructions, once per flight
+                                                       // at a different step in every lane
         tau = tau_limit;
         return RAY_LIMIT;
     }

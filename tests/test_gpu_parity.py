@@ -445,6 +445,51 @@ def test_transmission_matches_oracle(gpu, orc):
     assert np.all(np.abs(g4["value"] - v4) <= 4 * s4 + 1e-4 * np.abs(v4))
 
 
+def test_full_size_cfg2_sampled_packets_and_invariants(gpu, orc):
+    """BASELINE config 2 at its full size, in the launch configuration bench.py times (device-resident tables, device
+    outputs): sampled packets against the oracle one by one (per-packet event counts of the first 1500 packets of three
+    channels, which are independent of everything else by the counter-based streams), the spectra of those channels
+    against an oracle run on a packet sub-range, and the invariants that hold at any size."""
+    import torch
+    grid, opac, prm = wl.cfg2(packets=1000000)
+    n_chan = opac["lambda"].size
+    dev = dict(opac)
+    for k in ("k_abs", "k_sca_ray", "k_sca_cld", "g_cld"):
+        if opac.get(k) is not None:
+            dev[k] = torch.from_numpy(np.ascontiguousarray(opac[k], dtype=np.float32)).cuda()
+    with gpu.Grid(grid) as G:
+        G.set_opacity(dev)
+        g = G.run_albedo(prm, device_outputs=True, want_event_count=True)
+    c = g["counters"]
+    N = 1000000
+    assert c["packets_escaped"] + c["packets_absorbed"] + c["packets_surface"] == N * n_chan and c["packets_stuck"] == 0
+    assert c["escaped_weight"] == c["packets_escaped"]                    # analog transport: W = 1
+    evc = g["event_count"]
+    assert int(evc.to(torch.int64).sum().item()) == c["events"] == c["rays_peel"]
+    val = g["value"].cpu().numpy(); sig = g["sigma"].cpu().numpy(); flux = g["flux_sum"].cpu().numpy()
+    assert np.all(val > 0) and np.all(val < 1 / PI) and np.all(sig < 0.02 * val)
+    assert np.allclose(flux.sum(axis=2)[:, 0] / N, val[:, 0], rtol=1e-12)
+    # g-ordinates of one band: the single-scattering albedo is the same, the extinction grows with g (sorted k per
+    # cell), so less light reaches the absorbing lower boundary and more is reflected
+    band0 = val[:16, 0]
+    assert band0[-1] > band0[0]
+    chans, n_s = [0, 77, 175], 1500
+    for ch in chans:
+        one = {k: (np.ascontiguousarray(v[ch:ch + 1]) if isinstance(v, np.ndarray) and v.shape[:1] == (n_chan,) else v)
+               for k, v in opac.items()}
+        one["chan0"] = ch
+        o = orc.run_albedo(grid, one, dict(prm, pkt_begin=0, pkt_end=n_s, n_threads=os.cpu_count() or 1), want_event_count=True)
+        same = (evc[ch, :n_s].cpu().numpy().astype(np.uint32) == o["event_count"][0, :n_s]).mean()
+        assert same >= 0.99, (ch, same)
+        # the same packets (streams are keyed by channel and packet id only) as a run of their own, so that the
+        # batch-means sigma is defined: full parity bar on the full-size grid and tables
+        small = dict(prm, packets_per_channel=n_s)
+        gs_ = _gpu_run(gpu, grid, one, small, "albedo", want_event_count=True)
+        os_ = orc.run_albedo(grid, one, dict(small, n_threads=os.cpu_count() or 1), want_event_count=True)
+        _check_parity(orc, gs_, os_, "albedo")
+        assert np.array_equal(gs_["event_count"][0], evc[ch, :n_s].cpu().numpy().astype(np.uint32))
+
+
 def test_error_paths(gpu):
     grid, opac, prm = wl.cfg1(packets=100)
     with gpu.Grid(grid) as G:

@@ -74,6 +74,26 @@ def peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
 
 
+def rank_chan0(rank, n_chan_per_gpu):
+    """Weak scaling over channels: rank r runs its own n_chan_per_gpu channels, whose global
+    indices start here; the index keys the Philox streams, so the ranks simulate different channels."""
+    return rank * n_chan_per_gpu
+
+
+def reduce_over_ranks(ms, sums, world, device="cpu"):
+    """Step time = max over ranks (device-timed on every rank), work counters = sum over ranks.  The only
+    communication of the multi-GPU path: no data-path collective.  Works with any torch.distributed backend."""
+    if world <= 1:
+        return float(ms), [float(x) for x in sums]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    u = torch.tensor([float(x) for x in sums], device=device, dtype=torch.float64)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), [float(x) for x in u.tolist()]
+
+
 class ClockSampler(threading.Thread):
     """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -188,7 +208,7 @@ def run_ours(args):
 
     grid, opac, prm, mode = make_workload(args.workload, args.packets)
     n_chan = int(np.asarray(opac["lambda"]).size)
-    opac["chan0"] = rank * n_chan          # this rank's global channel range (keys the Philox streams)
+    opac["chan0"] = rank_chan0(rank, n_chan)   # this rank's global channel range (keys the Philox streams)
     N = int(prm["packets_per_channel"])
     tab_keys = [k for k in ("k_abs", "k_sca_ray", "k_sca_cld", "g_cld") if opac.get(k) is not None]
     stream = torch.cuda.current_stream()
@@ -227,10 +247,6 @@ def run_ours(args):
         e1.record(stream)
         barrier()
         ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
         return ms, acc, out
 
     for _ in range(max(args.warmup, 3)):
@@ -244,15 +260,9 @@ def run_ours(args):
     ms_e2e, acc_e2e, out_e2e = timed(host_opac, False, args.steps)
     d2h = sum(out_e2e[k].nbytes for k in ("flux_sum", "L_tot", "value", "sigma") if k in out_e2e)
 
-    ev_local = acc["events"]
-    if world > 1:
-        t = torch.tensor([acc["events"], acc_e2e["events"], acc["segments_transport"] + acc["segments_peel"]],
-                         device="cuda", dtype=torch.float64)
-        dist.all_reduce(t)
-        ev_all, ev_all_e2e, seg_all = [float(x) for x in t.tolist()]
-    else:
-        ev_all, ev_all_e2e = float(acc["events"]), float(acc_e2e["events"])
-        seg_all = float(acc["segments_transport"] + acc["segments_peel"])
+    ms, (ev_all, seg_all) = reduce_over_ranks(ms, [acc["events"], acc["segments_transport"] + acc["segments_peel"]],
+                                              world, "cuda")
+    ms_e2e, (ev_all_e2e,) = reduce_over_ranks(ms_e2e, [acc_e2e["events"]], world, "cuda")
     value = ev_all / (ms * 1e-3)
     e2e_value = ev_all_e2e / (ms_e2e * 1e-3)
 

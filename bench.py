@@ -139,6 +139,8 @@ def oracle_leg(name, grid, opac, prm, mode, budget_s=15.0):
     run = oracle.run_albedo if mode == "albedo" else oracle.run_emission
 
     def once(n):
+        # the first n packets of every channel as a run of their own (streams are keyed by packet id only): its 32
+        # batches spread over the host threads, which a sub-range of the full run (all in batch 0) would not
         p = dict(prm, packets_per_channel=n, pkt_begin=0, pkt_end=n, n_threads=cores)
         t0 = time.perf_counter()
         o = run(grid, opac, p)
@@ -146,17 +148,23 @@ def oracle_leg(name, grid, opac, prm, mode, budget_s=15.0):
 
     full = int(prm["packets_per_channel"])
     once(64)                      # thread pool and page-in, untimed
-    n = min(full, 2048)
-    dt, c = once(n)               # calibration: packets per second of the oracle as it stands
-    n2 = int(min(full, max(n, n * budget_s / max(dt, 1e-3))))
-    n2 = max(32, (n2 // 32) * 32)
-    if n2 > n:
-        dt, c = once(n2)
-    else:
-        n2 = n
+    n1, n2 = min(full, 1024), min(full, 4096)
+    t1, c = once(n1)              # two calibration points: per-channel table preparation is a fixed cost
+    n_run, dt = n1, t1
+    if n2 > n1:
+        t2, c = once(n2)
+        n_run, dt = n2, t2
+        per_pkt = max((t2 - t1) / (n2 - n1), 1e-9)
+        fixed = max(t1 - per_pkt * n1, 0.0)
+        n3 = int(min(full, max(n2, (budget_s - fixed) / per_pkt)))
+        n3 = max(32, (n3 // 32) * 32)
+        if n3 > n2:
+            dt, c = once(n3)
+            n_run = n3
+    n2 = n_run
     nseg = c["segments_transport"] + c["segments_peel"]
     n_chan = int(np.asarray(opac["lambda"]).size)
-    return {"value": c["events"] / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+    return {"value": c["events"] / dt, "unit": UNIT, "cores": min(cores, int(prm.get("n_batches", 32))), "kind": "oracle",
             "sample": "%s: first %d of %d packets of each of %d channels (%.1f s wall, OpenMP over batches)"
                       % (name, n2, full, n_chan, dt),
             "segments_per_s": nseg / dt, "seconds": dt, "events": int(c["events"])}

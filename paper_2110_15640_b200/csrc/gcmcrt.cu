@@ -75,7 +75,7 @@ struct gcmcrt_grid {
     DevBuf Lcell, Lcum, Ltot;
 
     // workspace
-    DevBuf ev0, ev1, ev2, evkeys, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, flights, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount, contrib;
+    DevBuf ev0, evkeys, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, flights, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount, contrib;
     unsigned int ev_cap = 0;
     int n_threads_resident = 0;
     // GCMCRT_TUNE="service,lateral,gens,batch_div": lanes waiting before the persistent kernel serves them; lanes parked at
@@ -240,9 +240,7 @@ int ensure_workspace(gcmcrt_grid* g)
             if (n >= 4) g->tune[3] = std::min(std::max(d, 1), 64);
         }
     }
-    CUDA_TRY(g, g->ev0.ensure(size_t(g->ev_cap) * sizeof(float4)));
-    CUDA_TRY(g, g->ev1.ensure(size_t(g->ev_cap) * sizeof(float4)));
-    CUDA_TRY(g, g->ev2.ensure(size_t(g->ev_cap) * sizeof(float4)));
+    CUDA_TRY(g, g->ev0.ensure(size_t(g->ev_cap) * 4 * sizeof(float4)));   // 64-byte records
     CUDA_TRY(g, g->perm.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));
     CUDA_TRY(g, g->evkeys.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));
     CUDA_TRY(g, g->ctrl.ensure(sizeof(PassCtrl)));
@@ -384,7 +382,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     }
     EventBuf ev;
     std::memset(&ev, 0, sizeof ev);
-    ev.e0 = g->ev0.as<float4>(); ev.e1 = g->ev1.as<float4>(); ev.e2 = g->ev2.as<float4>();
+    ev.rec = g->ev0.as<float4>();
     ev.count = &ctrl->ev_count;
     ev.cap = g->ev_cap;
     ev.soft_cap = (unsigned long long)g->ev_cap > 4 * threads_t ? g->ev_cap - (unsigned int)(2 * threads_t) : g->ev_cap / 2;
@@ -500,7 +498,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             sp.n_tiles = (sp.nbins + kScanTile - 1) / kScanTile;
             CUDA_TRY(g, g->hist.ensure(size_t(sp.nbins) * sizeof(unsigned int)));
             CUDA_TRY(g, g->tile_sums.ensure(size_t(sp.n_tiles) * sizeof(unsigned int)));
-            sp.e2 = ev.e2; sp.count = ev.count; sp.cap = ev.cap;
+            sp.count = ev.count; sp.cap = ev.cap;
             sp.keys = g->evkeys.as<unsigned int>();
             ev.keys = g->evkeys.as<unsigned int>(); ev.hist = emission ? nullptr : g->hist.as<unsigned int>();
             ev.c_fold = sp.c_fold; ev.nlev = g->nlev; ev.nlat = g->nlat; ev.ncell = g->ncell;
@@ -840,7 +838,7 @@ int gcmcrt_destroy(gcmcrt_grid* g)
     cudaGetLastError();
     for (DevBuf* b : {&g->tab, &g->r64, &g->cth64, &g->ph64, &g->rc32, &g->thc32, &g->phc32, &g->T, &g->rho, &g->u, &g->v,
                       &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->prop, &g->reff, &g->vlos,
-                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->ev1, &g->ev2, &g->evkeys, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
+                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->evkeys, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
                       &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->flux, &g->ltot_out,
                       &g->value, &g->sigma, &g->image, &g->evcount, &g->contrib})
         b->release();

@@ -21,16 +21,20 @@ enum EventKind : uint32_t { EV_MEDIUM = 0, EV_EMIT = 1, EV_SURFACE = 2 };
 struct EventBuf;
 __device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slot, float px, float py, float pz, float W,
                                             float nx, float ny, float nz, uint32_t m_inter, uint32_t cellp, uint32_t meta,
-                                            uint32_t pkt);
+                                            uint32_t pkt, float4 prop);
 
-// Event records written by the transport kernel, consumed by the peel kernel (structure of arrays of float4).
+// Event records written by the transport kernels, consumed by the peel kernel and by the next generation: one
+// 64-byte, 64-byte-aligned record per event = two whole 32 B sectors, so that reading records through the sort
+// permutation moves no byte it does not use.
 struct EventBuf {
-    float4* e0;  // px py pz W             packet weight before the event
-    float4* e1;  // nx ny nz 0             n = incoming direction (medium) or surface normal
-    float4* e2;  // m_inter cell meta pkt  (bit patterns) interactions completed before this event; packed cell;
-                 //                        meta = kind | batch << 2 | chan_run << 8; packet id
-                 // The record is the peel kernel's input AND the packet's full state at the event: the wavefront
-                 // kernels continue packets from it.
+    float4* rec;  // [cap][4]:
+                  //   [0] px py pz W             packet weight before the event
+                  //   [1] nx ny nz 0             n = incoming direction (medium) or surface normal
+                  //   [2] m_inter cell meta pkt  (bit patterns) interactions completed before this event; packed cell;
+                  //                              meta = kind | batch << 2 | chan_run << 8; packet id
+                  //   [3] omega P_gas g kappa    the cell's scattering properties (medium events; zeros otherwise)
+                  // The record is the peel kernel's input AND the packet's full state at the event: the wavefront
+                  // kernels continue packets from it.
     unsigned int* count;
     unsigned int cap;
     unsigned int soft_cap;
@@ -45,11 +49,13 @@ struct EventBuf {
 
 __device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slot, float px, float py, float pz, float W,
                                             float nx, float ny, float nz, uint32_t m_inter, uint32_t cellp, uint32_t meta,
-                                            uint32_t pkt)
+                                            uint32_t pkt, float4 prop)
 {
-    ev.e0[slot] = make_float4(px, py, pz, W);
-    ev.e1[slot] = make_float4(nx, ny, nz, 0.f);
-    ev.e2[slot] = make_float4(__uint_as_float(m_inter), __uint_as_float(cellp), __uint_as_float(meta), __uint_as_float(pkt));
+    float4* r = ev.rec + 4 * (size_t)slot;
+    r[0] = make_float4(px, py, pz, W);
+    r[1] = make_float4(nx, ny, nz, 0.f);
+    r[2] = make_float4(__uint_as_float(m_inter), __uint_as_float(cellp), __uint_as_float(meta), __uint_as_float(pkt));
+    r[3] = prop;
     if (ev.keys) {
         const int i = cellp & 1023, j = (cellp >> 10) & 1023, k = cellp >> 20;
         const unsigned int chan = (unsigned int)min(max(int(meta >> 8) - ev.chan_lo, 0), ev.c_fold - 1);
@@ -587,7 +593,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                             const float4 pr = __ldg(rc.prop + (size_t)ctab * rc.geom.ncell + cell);
                             if (record) {
                                 write_event(ev, slot, px, py, pz, pk.W, pk.ray.nx, pk.ray.ny, pk.ray.nz, pk.m_inter, cellp,
-                                            meta, pk.pkt);
+                                            meta, pk.pkt, pr);
                             }
                             ++pk.m_inter;
                             const Zeta4 z = zeta_block(rc.seed, ckey, pk.pkt, pk.m_inter, 1);
@@ -604,7 +610,8 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                             }
                         } else if (st == LS_EV_EMIT) {
                             if (record) {
-                                write_event(ev, slot, px, py, pz, pk.W, 0.f, 0.f, 1.f, pk.m_inter, cellp, meta, pk.pkt);
+                                write_event(ev, slot, px, py, pz, pk.W, 0.f, 0.f, 1.f, pk.m_inter, cellp, meta, pk.pkt,
+                                            make_float4(0.f, 0.f, 0.f, 0.f));
                             }
                             if (!rc.scatter_on) {
                                 ++c_abs; st = LS_IDLE; finish_packet(rc, pk);
@@ -623,7 +630,8 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                             const float rn = rsqrtf(fmaf(px, px, fmaf(py, py, pz * pz)));
                             float hx = px * rn, hy = py * rn, hz = pz * rn;
                             if (record) {
-                                write_event(ev, slot, px, py, pz, pk.W, hx, hy, hz, pk.m_inter, cellp, meta, pk.pkt);
+                                write_event(ev, slot, px, py, pz, pk.W, hx, hy, hz, pk.m_inter, cellp, meta, pk.pkt,
+                                            make_float4(0.f, 0.f, 0.f, 0.f));
                             }
                             ++pk.m_inter;
                             const Zeta4 z = zeta_block(rc.seed, ckey, pk.pkt, pk.m_inter, 3);
@@ -740,10 +748,10 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
         for (unsigned int r0 = (unsigned int)base; r0 < chunk_end; r0 += 32) {
             const unsigned int rank = r0 + lane_id();
             const bool have = rank < chunk_end;
-            float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a;
+            float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, pr = a;
             if (have) {
-                const unsigned int e = __ldg(perm + rank);
-                a = __ldg(ev.e0 + e); b = __ldg(ev.e1 + e); c = __ldg(ev.e2 + e);
+                const float4* r = ev.rec + 4 * (size_t)__ldg(perm + rank);
+                a = __ldg(r); b = __ldg(r + 1); c = __ldg(r + 2); pr = __ldg(r + 3);
             }
             const uint32_t meta = __float_as_uint(c.z);
             const uint32_t kind = meta & 3u;
@@ -755,8 +763,6 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
             // what the event scatters toward an observer: W omega (medium, Eq. 14), W (emission), W a (surface)
             float wsca = a.w, pgas = 0.f, g = 0.f;
             if (have && kind == EV_MEDIUM) {
-                const float4 pr = __ldg(rc.prop + (size_t)(rc.chan_begin + chan) * rc.geom.ncell +
-                                        ((ck * gs.nlat + cj) * gs.nlev + ci));
                 wsca *= pr.x; pgas = pr.y; g = pr.z;
             } else if (kind == EV_SURFACE) {
                 wsca *= rc.surface_albedo;

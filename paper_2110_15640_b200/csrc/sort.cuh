@@ -6,7 +6,7 @@
 // 48 B records stay where the transport kernel wrote them.
 //
 //   key(e) = clamp(chan_run(e) - chan_lo, 0, c_fold - 1) * ncell + (k * nlat + j) * nlev + i   (i fastest)
-//   ev_hist_kernel    hist[key]++                                  (global atomics)
+//   ev_hist_kernel    hist[key]++   (global atomics; albedo runs count the bin while the record is written instead)
 //   scan_*            exclusive prefix sum of hist in place        (tile reduce, scan of tile sums, tile scan)
 //   ev_scatter_kernel perm[hist[key]++] = e
 //
@@ -23,8 +23,8 @@ constexpr int kScanItems = 16;                       // per thread
 constexpr int kScanTile = kScanThreads * kScanItems;  // 4096 bins per CTA
 
 struct SortParams {
-    const float4* e2;            // event records, third float4: m_inter cell meta pkt (key computed from it) ...
-    const unsigned int* keys;    // ... or explicit keys [n] (launch order of the first flights); e2 unused then
+    const unsigned int* keys;    // [n] sort keys: stored with the event records (kernels.cuh write_event), or the
+                                 // launch keys of the first flights
     const unsigned int* count;   // number of items on the device (events written this pass), or NULL -> n_host
     unsigned int cap, n_host;
     unsigned int* hist;          // [nbins]
@@ -34,31 +34,18 @@ struct SortParams {
     int nlev, nlat, ncell, c_fold, chan_lo;
 };
 
-__device__ __forceinline__ unsigned int event_sort_key(const SortParams& p, const float4 c)
-{
-    const uint32_t cell = __float_as_uint(c.y), meta = __float_as_uint(c.z);
-    const int i = cell & 1023, j = (cell >> 10) & 1023, k = cell >> 20;
-    const unsigned int chan = (unsigned int)min(max(int(meta >> 8) - p.chan_lo, 0), p.c_fold - 1);
-    return chan * (unsigned int)p.ncell + (unsigned int)((k * p.nlat + j) * p.nlev + i);
-}
-
-__device__ __forceinline__ unsigned int sort_key_of(const SortParams& p, unsigned int e)
-{
-    return p.keys ? __ldg(p.keys + e) : event_sort_key(p, __ldg(p.e2 + e));
-}
-
 __global__ void __launch_bounds__(256) ev_hist_kernel(const SortParams p)
 {
     const unsigned int n = p.count ? min(*p.count, p.cap) : p.n_host;
     for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x)
-        atomicAdd(p.hist + sort_key_of(p, e), 1u);
+        atomicAdd(p.hist + __ldg(p.keys + e), 1u);
 }
 
 __global__ void __launch_bounds__(256) ev_scatter_kernel(const SortParams p)
 {
     const unsigned int n = p.count ? min(*p.count, p.cap) : p.n_host;
     for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x)
-        p.perm[atomicAdd(p.hist + sort_key_of(p, e), 1u)] = e;
+        p.perm[atomicAdd(p.hist + __ldg(p.keys + e), 1u)] = e;
 }
 
 __device__ __forceinline__ unsigned int block_sum_u32(unsigned int v, unsigned int* warp_part)

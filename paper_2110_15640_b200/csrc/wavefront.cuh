@@ -89,7 +89,13 @@ __device__ __forceinline__ void wave_record(const RunConst& rc, const EventBuf& 
     if (want) {
         if (slot < ev.cap) {
             const uint32_t meta = kind | batch_of(rc, pkt) << 2 | chan_run << 8;
-            write_event(ev, slot, px, py, pz, W, rx, ry, rz, m_inter, cellp, meta, pkt);
+            float4 prop = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (kind == EV_MEDIUM) {   // the cell's scattering properties travel with the record
+                const int i = cellp & 1023, j = (cellp >> 10) & 1023, k = cellp >> 20;
+                prop = __ldg(rc.prop + (size_t)(rc.chan_begin + int(chan_run)) * rc.geom.ncell +
+                             ((k * rc.geom.nlat + j) * rc.geom.nlev + i));
+            }
+            write_event(ev, slot, px, py, pz, W, rx, ry, rz, m_inter, cellp, meta, pkt, prop);
             ++wcnt.events;
         } else {
             const unsigned int sidx = atomicAdd(susp.count, 1u);
@@ -379,8 +385,9 @@ wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, con
             float ct = 0.f, zpsi = 0.f, tau_t = 0.f;
             uint32_t m_new = 0, cellp = 0, meta = 0, pkt = 0;
             if (e < end) {
-                a = ev.e0[e]; b = ev.e1[e];
-                const float4 c = ev.e2[e];
+                const float4* r = ev.rec + 4 * (size_t)e;
+                a = r[0]; b = r[1];
+                const float4 c = r[2], pr = r[3];
                 const uint32_t m_inter = __float_as_uint(c.x);
                 cellp = __float_as_uint(c.y); meta = __float_as_uint(c.z); pkt = __float_as_uint(c.w);
                 const uint32_t kind = meta & 3u, chan_run = meta >> 8;
@@ -389,9 +396,6 @@ wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, con
                 const uint32_t nev = nev_before(rc, kind, m_inter) + 1u;   // peel-off points including this one
                 m_new = m_inter;
                 if (kind == EV_MEDIUM) {
-                    int i, j, k;
-                    unpack_cell(cellp, i, j, k);
-                    const float4 pr = __ldg(rc.prop + (size_t)ctab * rc.geom.ncell + ((k * gs.nlat + j) * gs.nlev + i));
                     m_new = m_inter + 1;
                     const Zeta4 z = zeta_block(rc.seed, ckey, pkt, m_new, 1);
                     if ((rc.max_events && int(m_new) == rc.max_events) || !rc.scatter_on ||

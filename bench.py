@@ -48,7 +48,7 @@ I_EVENT = 420.0      # Philox block, phase sampling, rotation, ray setup, event 
 I_PEEL_RAY = 300.0   # record + prop read, phase function, ray setup for one (event, observer), exp, bin accumulation
 
 
-def make_workload(name, packets=None):
+def make_workload(name, packets=None, channels=None):
     if name == "cfg1":
         grid, opac, prm = wl.cfg1(packets=packets or 100000)
         mode = "albedo"
@@ -57,6 +57,11 @@ def make_workload(name, packets=None):
         mode = "albedo"
     elif name == "cfg3":
         grid, opac, prm = wl.cfg3(packets=packets or 1000000)
+        mode = "emission"
+    elif name == "cfg4":
+        # high-resolution Doppler-shifted emission; the full 1e4 wavelength points take ~2 min of numpy to generate
+        # (4.9 GB of tables), so --channels can cut the wavelength range for a quick look (say so when quoting it)
+        grid, opac, prm = wl.cfg4(packets=packets or 100000, **({"n_chan": channels} if channels else {}))
         mode = "emission"
     else:
         raise SystemExit("unknown workload %s" % name)
@@ -174,7 +179,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    grid, opac, prm, mode = make_workload(args.workload, args.packets)
+    grid, opac, prm, mode = make_workload(args.workload, args.packets, args.channels)
     vals = []
     base = None
     budget = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
@@ -214,7 +219,7 @@ def run_ours(args):
     build.build()
     binding.lib()
 
-    grid, opac, prm, mode = make_workload(args.workload, args.packets)
+    grid, opac, prm, mode = make_workload(args.workload, args.packets, args.channels)
     n_chan = int(np.asarray(opac["lambda"]).size)
     opac["chan0"] = rank_chan0(rank, n_chan)   # this rank's global channel range (keys the Philox streams)
     N = int(prm["packets_per_channel"])
@@ -333,7 +338,8 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--channels", type=int, default=None, help="cfg4 only: number of wavelength points (default 10000)")
     ap.add_argument("--packets", type=int, default=None, help="override packets per channel (debugging only)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()

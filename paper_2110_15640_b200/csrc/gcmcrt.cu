@@ -588,13 +588,15 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
                         g->launches += 1;
                     }
                     CUDA_TRY(g, cudaMemcpyAsync(&ctrl->gen_mark[1], &ctrl->ev_count, sizeof(unsigned int), cudaMemcpyDeviceToDevice, s));
-                    for (int gi = 0; gi < n_gen; ++gi) {
+                    // emission without scattering (L210): the emit kernel has already closed every packet it recorded
+                    const int n_gen_run = (emission && !prm->scatter_on) ? 0 : n_gen;
+                    for (int gi = 0; gi < n_gen_run; ++gi) {
                         wc.gen_mark = &ctrl->gen_mark[gi];
                         wc.park_all = gi == n_gen - 1;
                         k_inter<<<g->sm_count * occ_i, kWaveThreads, smem_i, s>>>(rc, ev, sin, wc);
                         CUDA_TRY(g, cudaMemcpyAsync(&ctrl->gen_mark[gi + 2], &ctrl->ev_count, sizeof(unsigned int), cudaMemcpyDeviceToDevice, s));
                     }
-                    g->launches += n_gen;
+                    g->launches += n_gen_run;
                 }
             }
             tk<<<grid_t, kTransportThreads, smem_t, s>>>(rc, ev, sin, sout, tail_items);

@@ -72,13 +72,13 @@ __device__ __forceinline__ void wave_finish_packet(const RunConst& rc, uint32_t 
 // the last generation, the packet is parked at the event instead (not yet recorded), in the persistent kernel's format.
 // (rx, ry, rz) is what the record stores as direction (incoming direction, or the surface normal), (dx, dy, dz) the
 // packet's flight direction.
-__device__ __forceinline__ void wave_record(const RunConst& rc, const EventBuf& ev, const SuspBuf& susp, int park_all,
+__device__ __forceinline__ bool wave_record(const RunConst& rc, const EventBuf& ev, const SuspBuf& susp, int park_all,
                                             bool want, uint32_t kind, float px, float py, float pz, float rx, float ry,
                                             float rz, float dx, float dy, float dz, float W, uint32_t cellp,
                                             uint32_t chan_run, uint32_t pkt, uint32_t m_inter, WaveCounters& wcnt)
 {
     const unsigned m = __ballot_sync(kFullMask, want);
-    if (m == 0) return;
+    if (m == 0) return false;
     unsigned int slot = 0xffffffffu;
     if (!park_all) {
         unsigned int base = 0;
@@ -104,6 +104,7 @@ __device__ __forceinline__ void wave_record(const RunConst& rc, const EventBuf& 
             susp.s2[sidx] = make_uint4(chan_run, pkt, m_inter, nev_before(rc, kind, m_inter) | kind << 28);
         }
     }
+    return want && slot < ev.cap;   // true: the event is in the buffer (false: parked, the persistent kernel records it)
 }
 
 // Warp-collective: marches every lane whose status is RAY_FLYING / RAY_PARK for at most `budget` steps (radial steps,
@@ -353,8 +354,12 @@ __global__ void __launch_bounds__(kWaveThreads) wave_emit_kernel(const __grid_co
                 wave_finish_packet(rc, chan_run, pkt, 0u);   // a packet without luminosity makes no event
             }
         }
-        wave_record(rc, ev, susp, wc.park_all, live, EV_EMIT, px, py, pz, 0.f, 0.f, 1.f, 0.f, 0.f, 1.f, W, cellp, chan_run,
-                    pkt, 0u, wcnt);
+        const bool recorded = wave_record(rc, ev, susp, wc.park_all, live, EV_EMIT, px, py, pz, 0.f, 0.f, 1.f, 0.f, 0.f, 1.f,
+                                          W, cellp, chan_run, pkt, 0u, wcnt);
+        if (recorded && !rc.scatter_on) {   // L210: only the initial peel-off; no generation kernel has to look at it
+            ++wcnt.abs;
+            wave_finish_packet(rc, chan_run, pkt, 1u);
+        }
     }
     wave_flush_counters(rc, wcnt);
 }

@@ -72,7 +72,7 @@ struct gcmcrt_grid {
     int staged_halfwidth = 0;
 
     // emission
-    DevBuf Lcell, Lcum, Ltot;
+    DevBuf Lcell, Lcum, Ltot, guide;
 
     // workspace
     DevBuf ev0, evkeys, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, flights, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount, contrib;
@@ -426,6 +426,9 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
             emis_cell_kernel<<<(unsigned)((ncolc + 127) / 128), 128, 0, s>>>(ep);
             emis_scan_kernel<<<g->n_chan, 1024, 0, s>>>(ep);
+            CUDA_TRY(g, g->guide.ensure(size_t(g->n_chan) * kEmisGuide * sizeof(int)));
+            emis_guide_kernel<<<(unsigned)(((long long)g->n_chan * kEmisGuide + 255) / 256), 256, 0, s>>>(
+                g->n_chan, g->ncell, ep.Lcum, ep.Ltot, g->guide.as<int>());
             CUDA_TRY(g, cudaGetLastError());
             CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
             CUDA_TRY(g, cudaEventSynchronize(g->tev[1]));
@@ -434,8 +437,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
                 CUDA_TRY(g, cudaEventElapsedTime(&ms, g->tev[0], g->tev[1]));
                 g->ms_emis += ms;
             }
-            g->launches += 2;
-            rc.Lcum = ep.Lcum; rc.Lcell = ep.Lcell; rc.Ltot = ep.Ltot;
+            g->launches += 3;
+            rc.Lcum = ep.Lcum; rc.Lcell = ep.Lcell; rc.Ltot = ep.Ltot; rc.guide = g->guide.as<int>();
             // L_tot output [n_chan_run][n_obs]
             const int o0 = prm->doppler_on ? run : 0, o1 = prm->doppler_on ? run + 1 : std::max(n_obs, 1);
             for (int o = o0; o < o1; ++o)
@@ -840,7 +843,7 @@ int gcmcrt_destroy(gcmcrt_grid* g)
     cudaGetLastError();
     for (DevBuf* b : {&g->tab, &g->r64, &g->cth64, &g->ph64, &g->rc32, &g->thc32, &g->phc32, &g->T, &g->rho, &g->u, &g->v,
                       &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->prop, &g->reff, &g->vlos,
-                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->ev0, &g->evkeys, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
+                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->guide, &g->ev0, &g->evkeys, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
                       &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->flux, &g->ltot_out,
                       &g->value, &g->sigma, &g->image, &g->evcount, &g->contrib})
         b->release();

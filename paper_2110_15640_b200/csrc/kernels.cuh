@@ -86,6 +86,7 @@ struct RunConst {
     const double* Lcum;    // emission: [n_chan_tab][ncell] running luminosity
     const double* Lcell;   // emission, xi > 0 only
     const double* Ltot;    // emission: [n_chan_tab]
+    const int* guide;      // emission: [n_chan_tab][kEmisGuide] search brackets of the CDF (emis_guide_kernel)
     uint32_t chan_key0;    // global channel index of table row 0 (Philox key)
     int chan_begin;        // first table row of this run
     int n_chan_run;
@@ -282,6 +283,28 @@ __global__ void __launch_bounds__(1024) emis_scan_kernel(const EmisParams p)
         __syncthreads();
     }
     if (threadIdx.x == 0) p.Ltot[c] = carry_s;
+}
+
+// Guide table of the emission CDF: guide[c][g] = first cell whose running luminosity exceeds (g / kEmisGuide) L_tot.
+// A packet's search (Eq. 13) then starts from the bracket [guide[g], guide[g+1]] of its own g = floor(frac * kEmisGuide)
+// -- a few cells in the bright part of the atmosphere instead of 17 dependent loads over the whole table -- and finds
+// the same cell as the full search (the bracket contains it by monotonicity of frac -> frac * L_tot in fp64).
+constexpr int kEmisGuide = 4096;
+
+__global__ void __launch_bounds__(256) emis_guide_kernel(int n_chan, int ncell, const double* __restrict__ Lcum,
+                                                         const double* __restrict__ Ltot, int* __restrict__ guide)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)n_chan * kEmisGuide) return;
+    const int c = int(t / kEmisGuide), gi = int(t % kEmisGuide);
+    const double* cum = Lcum + (size_t)c * ncell;
+    const double x = double(gi) / double(kEmisGuide) * Ltot[c];
+    int lo = 0, hi = ncell - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (cum[mid] > x) hi = mid; else lo = mid + 1;
+    }
+    guide[t] = lo;
 }
 
 // ---------------------------------------------------------------------------------------------------------

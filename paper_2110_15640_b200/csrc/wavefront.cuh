@@ -326,8 +326,11 @@ __global__ void __launch_bounds__(kWaveThreads) wave_emit_kernel(const __grid_co
                 if (double(z.z0) < rc.xi) {
                     cell = min(int(floor(double(z.z0) / rc.xi * ncell)), ncell - 1);
                 } else {
-                    const double x = (double(z.z0) - rc.xi) / (1.0 - rc.xi) * Ltot;
-                    int lo = 0, hi = ncell - 1;
+                    const double frac = (double(z.z0) - rc.xi) / (1.0 - rc.xi);
+                    const double x = frac * Ltot;
+                    const int gi = min(int(frac * double(kEmisGuide)), kEmisGuide - 1);
+                    const int* gd = rc.guide + (size_t)ctab * kEmisGuide;
+                    int lo = __ldg(gd + gi), hi = gi + 1 < kEmisGuide ? __ldg(gd + gi + 1) : ncell - 1;
                     while (lo < hi) {
                         const int mid = (lo + hi) >> 1;
                         if (cum[mid] > x) hi = mid; else lo = mid + 1;

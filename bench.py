@@ -42,9 +42,11 @@ UNIT = "events/s"
 
 # Algorithmic lane-instructions (FP32/INT issue slots) per unit of work; DESIGN.md section "Roofline" derives them
 # from the audited SASS of the march loop, the event handler and the launch code.
-I_SEG_3D = 52.0      # one 3D cell crossing: radial step 50 (SASS of ray_step incl. its loop share) + 4 % lateral x 45
-I_SEG_1D = 50.0      # nlat = nlon = 1: the same radial step, no lateral crossings
+I_SEG_3D = 40.0      # one 3D cell crossing: radial step 36.3 thread-instructions (ncu source page, executed counts) +
+                     # 4 % cone / half-plane crossings x ~45 + the column's extinction reload
+I_SEG_1D = 37.0      # nlat = nlon = 1: the same radial step, no lateral crossings
 I_EVENT = 420.0      # Philox block, phase sampling, rotation, ray setup, event record write + read
+PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 = 4.49e9   # ncu: 7 launches of a cfg2 step average 4.488 GB read + 4.8 MB written
 I_PEEL_RAY = 300.0   # record + prop read, phase function, ray setup for one (event, observer), exp, bin accumulation
 
 
@@ -296,7 +298,11 @@ def run_ours(args):
         ncell = int(np.asarray(grid["T"]).size)
         hbm_bytes = n_chan * ncell * 4 * (len(tab_keys) + 1 + 4)   # tables read once + alpha/prop written once
         roofline = {"bound": "alu", "kernel": dom + "_kernel", "achieved": achieved, "peak": peak,
-                    "unit": "Tlane-instr/s", "frac": achieved / peak if peak else None, "traffic": None,
+                    "unit": "Tlane-instr/s", "frac": achieved / peak if peak else None,
+                    # dram__bytes_read + write per peel_kernel launch from one ncu --set full capture of the default
+                    # workload (profiles/ncu_full_r01_wavefront.txt); other workloads: not captured
+                    "traffic": PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 if (args.workload == "cfg2" and args.packets is None) else None,
+                    "traffic_unit": "bytes per launch (54 M events: 64 B record + 4 B permutation entry + extinction gathers)",
                     "peak_source": "148 SM x 128 FP32 lanes x sm_max_mhz (%s)" % pk["source"],
                     "work_lane_instr_per_launch": work / n_dom, "ms_per_launch": dur_ms / n_dom,
                     "hbm_term": {"bytes_per_step": hbm_bytes, "ms_at_peak": hbm_bytes / (pk["hbm_gbs"] * 1e9) * 1e3 * 1.0,

@@ -555,6 +555,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             sin.count = &ctrl->susp_count[cur]; sin.taken = &ctrl->susp_taken[cur];
             sout.s0 = g->s0[nxt].as<float4>(); sout.s1 = g->s1[nxt].as<float4>(); sout.s2 = g->s2[nxt].as<uint4>();
             sout.count = &ctrl->susp_count[nxt]; sout.taken = &ctrl->susp_taken[nxt];
+            sin.cap = sout.cap = (unsigned int)std::min<unsigned long long>(susp_cap, 0xffffffffull);
             CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
             unsigned long long n_fresh = 0, tail_items = total_items;
             const unsigned long long chan_lo_pass = item0 / std::max<size_t>(n_pkt, 1);

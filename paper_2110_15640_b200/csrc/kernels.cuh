@@ -72,6 +72,8 @@ struct SuspBuf {
     uint4* s2;   // chan_run pkt m_inter nev|kind<<28
     unsigned int* count;
     unsigned int* taken;
+    unsigned int cap;   // entries allocated: a park beyond it is dropped and counted as a stuck packet (the host sizes the
+                        // list so that this cannot happen and reports an error if the count ever exceeds it)
 };
 
 struct DevCounters {
@@ -601,9 +603,13 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                     if (!have_slot) {
                         // event buffer full: park the packet for the next pass
                         const unsigned int sidx = atomicAdd(susp_out.count, 1u);
-                        susp_out.s0[sidx] = make_float4(px, py, pz, pk.W);
-                        susp_out.s1[sidx] = make_float4(pk.ray.nx, pk.ray.ny, pk.ray.nz, __uint_as_float(cellp));
-                        susp_out.s2[sidx] = make_uint4(pk.chan_run, pk.pkt, pk.m_inter, pk.nev | kind << 28);
+                        if (sidx < susp_out.cap) {
+                            susp_out.s0[sidx] = make_float4(px, py, pz, pk.W);
+                            susp_out.s1[sidx] = make_float4(pk.ray.nx, pk.ray.ny, pk.ray.nz, __uint_as_float(cellp));
+                            susp_out.s2[sidx] = make_uint4(pk.chan_run, pk.pkt, pk.m_inter, pk.nev | kind << 28);
+                        } else {
+                            ++c_stuck;
+                        }
                         st = LS_IDLE;   // the lane goes on moving the rest of the suspended list over to the next pass
                     } else {
                         const int ctab = rc.chan_begin + int(pk.chan_run);

@@ -99,9 +99,13 @@ __device__ __forceinline__ bool wave_record(const RunConst& rc, const EventBuf& 
             ++wcnt.events;
         } else {
             const unsigned int sidx = atomicAdd(susp.count, 1u);
-            susp.s0[sidx] = make_float4(px, py, pz, W);
-            susp.s1[sidx] = make_float4(dx, dy, dz, __uint_as_float(cellp));
-            susp.s2[sidx] = make_uint4(chan_run, pkt, m_inter, nev_before(rc, kind, m_inter) | kind << 28);
+            if (sidx < susp.cap) {
+                susp.s0[sidx] = make_float4(px, py, pz, W);
+                susp.s1[sidx] = make_float4(dx, dy, dz, __uint_as_float(cellp));
+                susp.s2[sidx] = make_uint4(chan_run, pkt, m_inter, nev_before(rc, kind, m_inter) | kind << 28);
+            } else {
+                ++wcnt.stuck;
+            }
         }
     }
     return want && slot < ev.cap;   // true: the event is in the buffer (false: parked, the persistent kernel records it)

@@ -147,6 +147,24 @@ int gcmcrt_set_opacity(gcmcrt_grid *grid, int chan0, int n_chan, const float *la
                        const float *g_cld, void *stream);
 
 /*
+ * gcmcrt_set_opacity_nodes -- as gcmcrt_set_opacity, but the absorption opacity comes from (T, log10 p) node tables
+ * and is interpolated to the cells on the device (the GPU opacity interpolation the paper plans, Sect. 7; its
+ * stated bottleneck is reading per-cell 3D opacity tables): a channel costs nT*nP floats instead of ncell.
+ *   k_abs(c, cell) = bilinear interpolation of node_kabs[c][nT][nP] at (T[cell], log10 p_cell[cell]), clamped to the
+ *   table; with doppler_on the shifted opacity (Eq. 34) interpolates between the bilinear values of the two
+ *   neighbouring channels.
+ *   node_kabs   host|device [n_chan][nT][nP] m^2/kg (copied)
+ *   T_nodes     host [nT] K, uniformly spaced ascending;  logp_nodes  host [nP] log10(Pa), uniformly spaced ascending
+ *   p_cell      host|device [nlon][nlat][nlev] Pa (copied)
+ *   lambda, k_sca_ray, k_sca_cld, g_cld: as gcmcrt_set_opacity (per-cell tables, nullable)
+ * Errors: E_INVALID, E_NOMEM, E_CUDA.
+ */
+int gcmcrt_set_opacity_nodes(gcmcrt_grid *grid, int chan0, int n_chan, const float *lambda,
+                             const float *node_kabs, int nT, int nP, const float *T_nodes, const float *logp_nodes,
+                             const float *p_cell, const float *k_sca_ray, const float *k_sca_cld,
+                             const float *g_cld, void *stream);
+
+/*
  * gcmcrt_run_albedo -- scattered-light run (Sect. 5.2): packets enter uniformly over the star-facing TOA disc
  * (incident flux normalised to 1, L283), fly sampled optical depths (L192), peel off to every observer at every
  * interaction (Eq. 14), scatter with Rayleigh (Eq. 5-6) / Henyey-Greenstein (Eq. 7-8) chosen by P_gas (Eq. 11)

@@ -321,3 +321,25 @@ def locate(grid, p):
     out = (C.c_int * 3)()
     lib().orc_locate(C.byref(g), pp, out)
     return tuple(int(x) for x in out)
+
+
+def interp_nodes(node_kabs, T_nodes, logp_nodes, T_cell, p_cell):
+    """k_abs[c][cell] from (T, log10 p) node tables node_kabs[c][nT][nP]: bilinear in (T, log10 p), the cell's
+    (T, log10 p) clamped to the table (the interpolation of opacity tables to the GCM cells, PAPER.md L374 / L85;
+    gcmcrt_set_opacity_nodes in include/gcmcrt.h states the same definition).  fp64, written out term by term."""
+    node = np.asarray(node_kabs, dtype=np.float64)
+    Tn = np.asarray(T_nodes, dtype=np.float64)
+    lpn = np.asarray(logp_nodes, dtype=np.float64)
+    T = np.asarray(T_cell, dtype=np.float64)
+    lp = np.log10(np.asarray(p_cell, dtype=np.float64))
+    out = np.empty((node.shape[0],) + T.shape, dtype=np.float64)
+    for idx in np.ndindex(T.shape):
+        t = min(max(T[idx], Tn[0]), Tn[-1])
+        q = min(max(lp[idx], lpn[0]), lpn[-1])
+        a = min(int(np.searchsorted(Tn, t, side="right")) - 1, Tn.size - 2)
+        b = min(int(np.searchsorted(lpn, q, side="right")) - 1, lpn.size - 2)
+        x = (t - Tn[a]) / (Tn[a + 1] - Tn[a])
+        y = (q - lpn[b]) / (lpn[b + 1] - lpn[b])
+        out[(slice(None),) + idx] = ((1 - x) * (1 - y) * node[:, a, b] + x * (1 - y) * node[:, a + 1, b]
+                                     + (1 - x) * y * node[:, a, b + 1] + x * y * node[:, a + 1, b + 1])
+    return out

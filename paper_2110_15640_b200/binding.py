@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libgcmcrt.so")
 _lib = None
 
 OK, E_INVALID, E_NOMEM, E_CUDA, E_STATE = 0, -1, -2, -3, -4
-EXPORTS = ["gcmcrt_grid_create", "gcmcrt_set_opacity", "gcmcrt_run_albedo", "gcmcrt_run_emission",
+EXPORTS = ["gcmcrt_grid_create", "gcmcrt_set_opacity", "gcmcrt_set_opacity_nodes", "gcmcrt_run_albedo", "gcmcrt_run_emission",
            "gcmcrt_run_transmission", "gcmcrt_destroy",
            "gcmcrt_last_error", "gcmcrt_debug_ray_tau", "gcmcrt_debug_philox", "gcmcrt_version"]
 
@@ -65,6 +65,8 @@ def lib():
         L.gcmcrt_grid_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_int] + [C.c_void_p] * 8 + \
             [C.c_double, C.c_float, C.c_void_p]
         L.gcmcrt_set_opacity.argtypes = [C.c_void_p, C.c_int, C.c_int] + [C.c_void_p] * 6
+        L.gcmcrt_set_opacity_nodes.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_int] + \
+            [C.c_void_p] * 7
         L.gcmcrt_run_albedo.argtypes = [C.c_void_p, C.POINTER(RunParams), C.POINTER(Result), C.c_void_p]
         L.gcmcrt_run_emission.argtypes = [C.c_void_p, C.POINTER(RunParams), C.POINTER(Result), C.c_void_p]
         L.gcmcrt_run_transmission.argtypes = [C.c_void_p, C.POINTER(RunParams), C.POINTER(Result), C.c_void_p]
@@ -130,6 +132,18 @@ def set_opacity(handle, chan0, lam, k_abs, k_sca_ray=None, k_sca_cld=None, g_cld
     rc = lib().gcmcrt_set_opacity(handle, int(chan0), lam.size, _ptr(lam), _ptr(k_abs, np.float32),
                                   _ptr(k_sca_ray, np.float32), _ptr(k_sca_cld, np.float32), _ptr(g_cld, np.float32),
                                   _stream_ptr(stream))
+    _check(handle, rc)
+
+
+def set_opacity_nodes(handle, chan0, lam, node_kabs, T_nodes, logp_nodes, p_cell, k_sca_ray=None, k_sca_cld=None,
+                      g_cld=None, stream=None):
+    lam = np.ascontiguousarray(lam, dtype=np.float32)
+    tn = np.ascontiguousarray(T_nodes, dtype=np.float32)
+    lpn = np.ascontiguousarray(logp_nodes, dtype=np.float32)
+    rc = lib().gcmcrt_set_opacity_nodes(handle, int(chan0), lam.size, _ptr(lam), _ptr(node_kabs, np.float32), tn.size,
+                                        lpn.size, _ptr(tn), _ptr(lpn), _ptr(p_cell, np.float32),
+                                        _ptr(k_sca_ray, np.float32), _ptr(k_sca_cld, np.float32), _ptr(g_cld, np.float32),
+                                        _stream_ptr(stream))
     _check(handle, rc)
 
 
@@ -257,6 +271,15 @@ class Grid:
         lam = opac["lambda"]
         self._keep = [_as32(opac.get(k)) for k in ("k_abs", "k_sca_ray", "k_sca_cld", "g_cld")]
         set_opacity(self.handle, opac.get("chan0", 0), lam, *self._keep, stream=self.stream)
+        self.n_chan = int(np.asarray(lam).size) if not _is_torch(lam) else int(lam.numel())
+
+    def set_opacity_nodes(self, opac):
+        """k_abs from opac['node_kabs'][n_chan][nT][nP] at opac['T_nodes'], opac['logp_nodes'] (uniform), cell pressures
+        opac['p_cell'] [nlon][nlat][nlev] in Pa; scattering tables as in set_opacity."""
+        lam = opac["lambda"]
+        self._keep = [_as32(opac.get(k)) for k in ("node_kabs", "p_cell", "k_sca_ray", "k_sca_cld", "g_cld")]
+        set_opacity_nodes(self.handle, opac.get("chan0", 0), lam, self._keep[0], opac["T_nodes"], opac["logp_nodes"],
+                          self._keep[1], *self._keep[2:], stream=self.stream)
         self.n_chan = int(np.asarray(lam).size) if not _is_torch(lam) else int(lam.numel())
 
     def run_albedo(self, prm, **kw):

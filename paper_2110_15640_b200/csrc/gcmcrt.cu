@@ -67,6 +67,9 @@ struct gcmcrt_grid {
     DevBuf own_kabs, own_kray, own_kcld, own_g;   // copies of host-resident inputs
     const float *k_abs = nullptr, *k_ray = nullptr, *k_cld = nullptr, *g_cld = nullptr;
     DevBuf alpha, prop, reff, vlos, lambda64;
+    DevBuf node, node_idx, node_w, own_pcell;     // k_abs from (T, log10 p) node tables (gcmcrt_set_opacity_nodes)
+    int nT = 0, nP = 0;
+    bool use_nodes = false;
     int staged_obs = -2;   // -2: nothing staged, -1: unshifted table, >= 0: Doppler table of that observer dir
     double staged_dir[3] = {0, 0, 0};
     int staged_halfwidth = 0;
@@ -190,6 +193,8 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
     StageParams sp;
     sp.n_chan = g->n_chan; sp.ncell = g->ncell; sp.nlev = g->nlev; sp.nlat = g->nlat; sp.nlon = g->nlon;
     sp.k_abs = g->k_abs; sp.k_ray = g->k_ray; sp.k_cld = g->k_cld; sp.g_cld = g->g_cld;
+    sp.node = g->use_nodes ? g->node.as<float>() : nullptr;
+    sp.node_idx = g->node_idx.as<int2>(); sp.node_w = g->node_w.as<float2>(); sp.nT = g->nT; sp.nP = g->nP;
     sp.rho = g->rho.as<float>();
     sp.alpha = g->alpha.as<float>(); sp.prop = g->prop.as<float4>();
     sp.alpha_stride = gp0.alpha_stride; sp.col_stride = gp0.col_stride;
@@ -780,6 +785,9 @@ int gcmcrt_grid_create(gcmcrt_grid** out, int nlev, int nlat, int nlon, const do
     return GCMCRT_OK;
 }
 
+static int set_opacity_common(gcmcrt_grid* g, int chan0, int n_chan, const float* lambda, const float* k_sca_ray,
+                              const float* k_sca_cld, const float* g_cld, cudaStream_t s);
+
 int gcmcrt_set_opacity(gcmcrt_grid* g, int chan0, int n_chan, const float* lambda, const float* k_abs,
                        const float* k_sca_ray, const float* k_sca_cld, const float* g_cld, void* stream)
 {
@@ -789,7 +797,46 @@ int gcmcrt_set_opacity(gcmcrt_grid* g, int chan0, int n_chan, const float* lambd
     const size_t n = size_t(n_chan) * g->ncell;
     g->staged_obs = -2;
     g->n_chan = 0;
+    g->use_nodes = false;
     CUDA_TRY(g, device_view(k_abs, n, g->own_kabs, s, &g->k_abs));
+    return set_opacity_common(g, chan0, n_chan, lambda, k_sca_ray, k_sca_cld, g_cld, s);
+}
+
+int gcmcrt_set_opacity_nodes(gcmcrt_grid* g, int chan0, int n_chan, const float* lambda, const float* node_kabs, int nT,
+                             int nP, const float* T_nodes, const float* logp_nodes, const float* p_cell,
+                             const float* k_sca_ray, const float* k_sca_cld, const float* g_cld, void* stream)
+{
+    if (!g) return GCMCRT_E_INVALID;
+    if (n_chan < 1 || chan0 < 0 || !lambda || !node_kabs || nT < 2 || nP < 2 || !T_nodes || !logp_nodes || !p_cell)
+        return fail(g, GCMCRT_E_INVALID, "set_opacity_nodes: bad arguments");
+    const float dT = (T_nodes[nT - 1] - T_nodes[0]) / float(nT - 1), dlp = (logp_nodes[nP - 1] - logp_nodes[0]) / float(nP - 1);
+    if (!(dT > 0.f) || !(dlp > 0.f)) return fail(g, GCMCRT_E_INVALID, "set_opacity_nodes: node axes must ascend");
+    for (int a = 1; a < nT; ++a)
+        if (std::fabs((T_nodes[a] - T_nodes[a - 1]) - dT) > 1e-3f * dT) return fail(g, GCMCRT_E_INVALID, "set_opacity_nodes: T_nodes must be uniformly spaced");
+    for (int b = 1; b < nP; ++b)
+        if (std::fabs((logp_nodes[b] - logp_nodes[b - 1]) - dlp) > 1e-3f * dlp) return fail(g, GCMCRT_E_INVALID, "set_opacity_nodes: logp_nodes must be uniformly spaced");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    g->staged_obs = -2;
+    g->n_chan = 0;
+    g->k_abs = nullptr;
+    const float* dnode = nullptr;
+    const float* dp = nullptr;
+    CUDA_TRY(g, device_view(node_kabs, size_t(n_chan) * nT * nP, g->node, s, &dnode, true));
+    CUDA_TRY(g, device_view(p_cell, size_t(g->ncell), g->own_pcell, s, &dp, true));
+    CUDA_TRY(g, g->node_idx.ensure(size_t(g->ncell) * sizeof(int2)));
+    CUDA_TRY(g, g->node_w.ensure(size_t(g->ncell) * sizeof(float2)));
+    node_coeff_kernel<<<(g->ncell + 255) / 256, 256, 0, s>>>(g->ncell, g->T.as<float>(), dp, T_nodes[0], dT, logp_nodes[0], dlp,
+                                                            nT, nP, g->node_idx.as<int2>(), g->node_w.as<float2>());
+    CUDA_TRY(g, cudaGetLastError());
+    g->nT = nT; g->nP = nP;
+    g->use_nodes = true;
+    return set_opacity_common(g, chan0, n_chan, lambda, k_sca_ray, k_sca_cld, g_cld, s);
+}
+
+static int set_opacity_common(gcmcrt_grid* g, int chan0, int n_chan, const float* lambda, const float* k_sca_ray,
+                              const float* k_sca_cld, const float* g_cld, cudaStream_t s)
+{
+    const size_t n = size_t(n_chan) * g->ncell;
     CUDA_TRY(g, device_view(k_sca_ray, n, g->own_kray, s, &g->k_ray));
     CUDA_TRY(g, device_view(k_sca_cld, n, g->own_kcld, s, &g->k_cld));
     CUDA_TRY(g, device_view(g_cld, n, g->own_g, s, &g->g_cld));
@@ -843,7 +890,7 @@ int gcmcrt_destroy(gcmcrt_grid* g)
     cudaDeviceSynchronize();
     cudaGetLastError();
     for (DevBuf* b : {&g->tab, &g->r64, &g->cth64, &g->ph64, &g->rc32, &g->thc32, &g->phc32, &g->T, &g->rho, &g->u, &g->v,
-                      &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->prop, &g->reff, &g->vlos,
+                      &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->prop, &g->reff, &g->vlos, &g->node, &g->node_idx, &g->node_w, &g->own_pcell,
                       &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->guide, &g->ev0, &g->evkeys, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
                       &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->flux, &g->ltot_out,
                       &g->value, &g->sigma, &g->image, &g->evcount, &g->contrib})

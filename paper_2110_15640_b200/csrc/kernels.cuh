@@ -135,6 +135,12 @@ struct StageParams {
     long long alpha_stride;
     int col_stride;
     float4* prop;
+    // k_abs from (T, log10 p) node tables instead of a per-cell table (the on-GPU opacity interpolator, Sect. 7):
+    // k_abs(c, cell) = bilinear interpolation of node[c][nT][nP] at the cell's (T, log10 p), clamped to the table
+    const float* node;     // [n_chan][nT][nP] or NULL
+    const int2* node_idx;  // [ncell] (iT, iP) of the lower-left node
+    const float2* node_w;  // [ncell] weights of the upper nodes
+    int nT, nP;
     // Doppler (A1): per-cell line-of-sight velocity of this observer, per-channel 1/ln(lambda ratio)
     int doppler, halfwidth;
     const float* vlos;   // [ncell] for the current observer
@@ -163,6 +169,32 @@ __global__ void __launch_bounds__(256) vlos_kernel(int nlev, int nlat, int nlon,
     vlos[cell] = -(Vx * ox + Vy * oy + Vz * oz);
 }
 
+// per cell: position of (T, log10 p) in the uniform node grid
+__global__ void __launch_bounds__(256) node_coeff_kernel(int ncell, const float* __restrict__ T, const float* __restrict__ p_cell,
+                                                         float T0, float dT, float lp0, float dlp, int nT, int nP,
+                                                         int2* __restrict__ idx, float2* __restrict__ w)
+{
+    const int cell = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= ncell) return;
+    const float ft = fminf(fmaxf((T[cell] - T0) / dT, 0.0f), float(nT - 1) - 1e-4f);
+    const float fp = fminf(fmaxf((log10f(p_cell[cell]) - lp0) / dlp, 0.0f), float(nP - 1) - 1e-4f);
+    const int it = int(ft), ip = int(fp);
+    idx[cell] = make_int2(it, ip);
+    w[cell] = make_float2(ft - float(it), fp - float(ip));
+}
+
+__device__ __forceinline__ float stage_kabs(const StageParams& p, int c, int cell)
+{
+    if (p.node) {
+        const int2 id = __ldg(p.node_idx + cell);
+        const float2 w = __ldg(p.node_w + cell);
+        const float* nd = p.node + ((size_t)c * p.nT + id.x) * p.nP + id.y;
+        const float a00 = __ldg(nd), a01 = __ldg(nd + 1), a10 = __ldg(nd + p.nP), a11 = __ldg(nd + p.nP + 1);
+        return (1.0f - w.x) * ((1.0f - w.y) * a00 + w.y * a01) + w.x * ((1.0f - w.y) * a10 + w.y * a11);
+    }
+    return __ldg(p.k_abs + (long long)c * p.ncell + cell);
+}
+
 __global__ void __launch_bounds__(256) stage_kernel(const StageParams p)
 {
     const long long total = (long long)p.n_chan * p.ncell;
@@ -175,14 +207,17 @@ __global__ void __launch_bounds__(256) stage_kernel(const StageParams p)
             // Eq. 34: lambda_eff = lambda_0 (1 - v/c) -> index offset dn = -v/c / ln(lambda_{n+1}/lambda_n), C14
             float dn = -p.vlos[cell] * (1.0f / 299792458.0f) * p.reff[c];
             dn = fminf(fmaxf(dn, -float(p.halfwidth)), float(p.halfwidth));
-            float x = fminf(fmaxf(float(c) + dn, 0.0f), float(p.n_chan - 1));
-            int lo = min(int(floorf(x)), p.n_chan - 2);
-            const float f = x - float(lo);
-            const float k0 = __ldg(p.k_abs + (long long)lo * p.ncell + cell);
-            const float k1 = __ldg(p.k_abs + (long long)(lo + 1) * p.ncell + cell);
+            // integer and fractional part of dn apart: c + dn in fp32 would lose the fraction at c ~ 1e5 and make
+            // the result depend on where a wavelength batch starts
+            const float fl = floorf(dn);
+            int lo = c + int(fl);
+            float f = dn - fl;
+            if (lo < 0) { lo = 0; f = 0.0f; }
+            if (lo > p.n_chan - 2) { lo = p.n_chan - 2; f = 1.0f; }
+            const float k0 = stage_kabs(p, lo, cell), k1 = stage_kabs(p, lo + 1, cell);
             ka = (1.0f - f) * k0 + f * k1;
         } else {
-            ka = __ldg(p.k_abs + t);
+            ka = stage_kabs(p, c, cell);
         }
         const float kr = p.k_ray ? __ldg(p.k_ray + t) : 0.0f;
         const float kc = p.k_cld ? __ldg(p.k_cld + t) : 0.0f;

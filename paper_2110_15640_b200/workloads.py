@@ -237,6 +237,11 @@ def hires_opacity(grid, rng, n_chan=10000, lam0=2.19e-6, R=1.0e5, n_lines=500, n
     opac["lambda"] = lam.astype(np.float32)
     opac["lambda64"] = lam
     opac["k_abs"] = k_abs
+    # the same table in the form gcmcrt_set_opacity_nodes takes: node values + the cells' pressures
+    opac["node_kabs"] = node.astype(np.float32)
+    opac["T_nodes"] = Tn.astype(np.float32)
+    opac["logp_nodes"] = lpn.astype(np.float32)
+    opac["p_cell"] = np.broadcast_to(grid["p_mid"][None, None, :], T.shape).astype(np.float32)
     return opac
 
 

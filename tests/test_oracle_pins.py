@@ -813,3 +813,39 @@ def test_tthg_transport_keeps_peel_escape_consistency(orc):
     assert abs(total - scattered) < 4 * np.sqrt(np.sum((sig[0] * wq) ** 2)) + 0.01, (total, scattered)
     hg = orc.run_albedo(grid, opac, dict(prm, cloud_phase=0))
     assert not np.allclose(hg["flux_sum"], res["flux_sum"])
+
+
+# ----------------------------------------------------------------------------- node-table interpolation (Sect. 7)
+def test_node_interpolation_is_exact_on_bilinear_tables_and_clamps(orc):
+    """interp_nodes: a table that is itself bilinear in (T, log10 p) is reproduced at every cell (closed form); the
+    node values come back at the nodes; cells outside the table take the edge value; a non-uniform axis is honoured;
+    and scipy's RegularGridInterpolator (an independent library routine) agrees on a random table."""
+    from scipy.interpolate import RegularGridInterpolator
+    rng = np.random.default_rng(12)
+    Tn = np.array([500.0, 700.0, 1000.0, 1800.0, 3000.0])
+    lpn = np.linspace(-1.0, 7.0, 7)
+    co = rng.normal(size=(3, 4))
+    f = lambda c, T, q: co[c, 0] + co[c, 1] * T / 1e3 + co[c, 2] * q + co[c, 3] * T / 1e3 * q
+    node = np.stack([f(c, Tn[:, None], lpn[None, :]) for c in range(3)])
+    T = rng.uniform(500.0, 3000.0, size=(4, 3, 5))
+    p = 10.0 ** rng.uniform(-1.0, 7.0, size=T.shape)
+    k = orc.interp_nodes(node, Tn, lpn, T, p)
+    assert k.shape == (3, 4, 3, 5)
+    # bilinear interpolation reproduces 1, T, q exactly; T*q only inside one cell of the node grid -> compare with f
+    # on a table whose cross term vanishes, and with the cross term where (T, q) sit on nodes
+    co[:, 3] = 0.0
+    node_l = np.stack([f(c, Tn[:, None], lpn[None, :]) for c in range(3)])
+    k_l = orc.interp_nodes(node_l, Tn, lpn, T, p)
+    for c in range(3):
+        assert np.allclose(k_l[c], f(c, T, np.log10(p)), rtol=0, atol=1e-12)
+    Tg, qg = np.meshgrid(Tn, lpn, indexing="ij")
+    assert np.allclose(orc.interp_nodes(node, Tn, lpn, Tg, 10.0 ** qg), node, rtol=0, atol=1e-12)
+    # clamping
+    edge = orc.interp_nodes(node, Tn, lpn, np.array([100.0, 9000.0]), np.array([1e-5, 1e12]))
+    assert np.allclose(edge[:, 0], node[:, 0, 0]) and np.allclose(edge[:, 1], node[:, -1, -1])
+    # independent library routine on a random (non-bilinear) table
+    rnd = rng.uniform(0.0, 1.0, size=(2, Tn.size, lpn.size))
+    kr = orc.interp_nodes(rnd, Tn, lpn, T, p)
+    for c in range(2):
+        ref = RegularGridInterpolator((Tn, lpn), rnd[c], method="linear")(np.stack([T, np.log10(p)], axis=-1))
+        assert np.allclose(kr[c], ref, rtol=0, atol=1e-12)

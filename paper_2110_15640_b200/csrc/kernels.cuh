@@ -878,11 +878,7 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
                             st = RAY_FLYING;
                         }
                     }
-#pragma unroll 1
-                    for (int s = 0; s < KSTEPS && st == RAY_FLYING; ++s) {   // lanes in flight step together
-                        ++seg32;
-                        st = ray_step(ray, gs, tau, rc.tau_cut);
-                    }
+                    if (st == RAY_FLYING) st = ray_run<KSTEPS>(ray, gs, tau, rc.tau_cut, seg32);   // lanes in flight step together
                 }
                 c_seg += seg32;
                 // ---------------- rays that reached the top of the atmosphere: Eq. 14 ----------------
@@ -997,11 +993,7 @@ transmission_kernel(const __grid_constant__ RunConst rc, const TransParams tp, c
             if (m_park && (__popc(m_park) >= rc.t_lateral || m_fly == 0)) {
                 if (st == RAY_PARK) { ray_lateral(ray, gs, alpha_c); st = RAY_FLYING; }
             }
-#pragma unroll 1
-            for (int s = 0; s < KSTEPS && st == RAY_FLYING; ++s) {
-                ++seg32;
-                st = ray_step(ray, gs, tau, rc.tau_cut);     // beyond tau_cut the chord is opaque: 1 - e^-tau = 1
-            }
+            if (st == RAY_FLYING) st = ray_run<KSTEPS>(ray, gs, tau, rc.tau_cut, seg32);   // beyond tau_cut the chord is opaque: 1 - e^-tau = 1
         }
         c_seg += seg32;
         float v = 0.f;

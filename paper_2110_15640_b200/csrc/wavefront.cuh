@@ -129,11 +129,7 @@ __device__ __forceinline__ int wave_march(const RunConst& rc, const GeomSmem& gs
                 st = RAY_FLYING;
             }
         }
-#pragma unroll 1
-        for (int s = 0; s < KSTEPS && st == RAY_FLYING; ++s) {   // lanes in flight step together
-            ++seg32;
-            st = ray_step(ray, gs, tau, tau_t);
-        }
+        if (st == RAY_FLYING) st = ray_run<KSTEPS>(ray, gs, tau, tau_t, seg32);   // lanes in flight step together
     }
     wcnt.seg += seg32;
     return it;

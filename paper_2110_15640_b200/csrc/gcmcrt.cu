@@ -519,7 +519,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         auto k_keys = wave_launch_keys_kernel;
         auto k_first = wave_first_flight_kernel<8>;
         auto k_emit = wave_emit_kernel;
-        auto k_inter = wave_interact_kernel<4>;
+        auto k_inter = wave_interact_kernel<kInteractK>;
         const size_t smem_w = smem_t;
         const size_t smem_i = (size_t((g->tab_floats + 31) & ~31) + size_t(kWaveThreads / 32) * kStageFields * kStageSlots) * sizeof(float);
         int occ_f = 1, occ_i = 1;

@@ -809,13 +809,19 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
         base = __shfl_sync(kFullMask, base, 0);
         if (base >= n_events) break;
         const unsigned int chunk_end = (unsigned int)min((unsigned long long)n_events, base + kPeelChunk);
+        unsigned int slot_next = 0;   // record of this lane's event in the next round of 32
+        if ((unsigned int)base + lane_id() < chunk_end) slot_next = __ldg(perm + (unsigned int)base + lane_id());
         for (unsigned int r0 = (unsigned int)base; r0 < chunk_end; r0 += 32) {
             const unsigned int rank = r0 + lane_id();
             const bool have = rank < chunk_end;
             float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, pr = a;
             if (have) {
-                const float4* r = ev.rec + 4 * (size_t)__ldg(perm + rank);
+                const float4* r = ev.rec + 4 * (size_t)slot_next;
                 a = __ldg(r); b = __ldg(r + 1); c = __ldg(r + 2); pr = __ldg(r + 3);
+            }
+            if (rank + 32 < chunk_end) {   // next round's records on their way while this round's rays are integrated
+                slot_next = __ldg(perm + rank + 32);
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(ev.rec + 4 * (size_t)slot_next));
             }
             const uint32_t meta = __float_as_uint(c.z);
             const uint32_t kind = meta & 3u;

@@ -272,19 +272,18 @@ __device__ __forceinline__ int ray_run(Ray& r, const GeomSmem& s, float& tau_io,
     const uint32_t sa0 = s.r2_saddr;
     int status = RAY_FLYING, n = 0;
     bool inward = r.rad_step < 0;
-    asm volatile("" : "+f"(tau_limit));   // a register, not a constant-bank load per step (likewise sa_stop, sa_top)
+    asm volatile("" : "+f"(tau_limit));   // a register, not a constant-bank load per step
     if (inward) {
         // crossing shell sa_stop inward is no plain crossing: it enters the turning cell i_turn (the shell just crossed
         // is then the next one outward) or, for a ray that does not turn inside the grid, leaves through the lower boundary
-        uint32_t sa_stop = s.r2_saddr + 8u * uint32_t(max(r.i_turn + 1, 0));
-        asm volatile("" : "+r"(sa_stop));
+        const uint32_t sa_stop = s.r2_saddr + 8u * uint32_t(max(r.i_turn + 1, 0));
+        const int plain = min(KSTEPS, int((sa - sa_stop) >> 3));   // plain crossings before that one, within the budget
 #pragma unroll 1
-        while (n < KSTEPS) {
-            const float un = fminf(u_rad, ul);
-            const float tnew = fmaf(alpha, fmaxf(un - u, 0.0f), tau);
-            if ((tnew >= tau_limit) | (u_rad > ul) | (sa == sa_stop)) break;
+        while (n < plain) {
+            const float tnew = fmaf(alpha, fmaxf(u_rad - u, 0.0f), tau);   // min(u_rad, ul) = u_rad unless the loop ends here
+            if ((tnew >= tau_limit) | (u_rad > ul)) break;
             tau = tnew;
-            u = fmaxf(un, u);
+            u = fmaxf(u_rad, u);
             alpha = alpha_n;
             sa -= 8u;
             float hi, lo;
@@ -319,15 +318,14 @@ __device__ __forceinline__ int ray_run(Ray& r, const GeomSmem& s, float& tau_io,
         }
     }
     if (!inward && status == RAY_FLYING) {
-        uint32_t sa_top = s.r2_saddr + 8u * uint32_t(s.nlev);
-        asm volatile("" : "+r"(sa_top));
+        const uint32_t sa_top = s.r2_saddr + 8u * uint32_t(s.nlev);
+        const int plain = min(KSTEPS, n + int((sa_top - sa) >> 3));   // plain crossings before the one that leaves the grid
 #pragma unroll 1
-        while (n < KSTEPS) {
-            const float un = fminf(u_rad, ul);
-            const float tnew = fmaf(alpha, fmaxf(un - u, 0.0f), tau);
-            if ((tnew >= tau_limit) | (u_rad > ul) | (sa == sa_top)) break;
+        while (n < plain) {
+            const float tnew = fmaf(alpha, fmaxf(u_rad - u, 0.0f), tau);
+            if ((tnew >= tau_limit) | (u_rad > ul)) break;
             tau = tnew;
-            u = fmaxf(un, u);
+            u = fmaxf(u_rad, u);
             alpha = alpha_n;
             sa += 8u;
             float hi, lo;

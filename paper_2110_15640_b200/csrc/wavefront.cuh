@@ -178,7 +178,8 @@ __device__ __forceinline__ void wave_fly(const RunConst& rc, const EventBuf& ev,
 // long now and then, so a warp marches its 32 fresh flights for a few steps only and moves the unfinished ones to a
 // per-warp list in global memory (L2-resident); 32 of those are then marched together for longer.  23 words per flight.
 constexpr int kFlightFields = 23;
-constexpr int kFirstRoundSteps = 4, kLongRoundSteps = 16;
+constexpr int kInteractK = 8;   // steps per ray_run call in the interact kernel
+constexpr int kFirstRoundSteps = 8, kLongRoundSteps = 16;   // measured: (4, 16) 57.9 ms, (8, 16) 56.6, (16, 32) 58.1, (2, 8) 60.8
 
 __device__ __forceinline__ void flight_save(float* fl, const Ray& r, float tau, float tau_t, float W, uint32_t chan_run,
                                             uint32_t pkt, uint32_t m_inter, int st, int used)

@@ -269,7 +269,7 @@ __global__ void __launch_bounds__(kWaveThreads) wave_launch_keys_kernel(const __
 
 // albedo: launch + first flight, 32 packets of neighbouring entry columns per warp
 template <int KSTEPS>
-__global__ void __launch_bounds__(kWaveThreads, 3)
+__global__ void __launch_bounds__(kWaveThreads, 4)
 wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const SuspBuf susp, const WaveConst wc)
 {
     extern __shared__ float smem_f[];

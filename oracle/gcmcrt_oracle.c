@@ -662,7 +662,29 @@ static void packet_albedo(const run_ctx *rc, uint32_t pkt, int batch, orc_counte
     int ijk[3];
     locate(G, p, ijk);
     ijk[0] = G->nlev - 1;
-    transport(rc, pkt, p, n, ijk, 1.0, -log(z[2]), 0, batch, cnt);
+    double W = 1.0, tau_t = -log(z[2]);
+    if (prm->forced_first) {
+        /* Sect. 4.2: "an extra raytracing step to calculate the optical depth to the end of the grid in the
+         * direction of the packet path", here once, at the start of the packet (forced first scattering).  The flight
+         * is drawn from the exponential law truncated at tau_edge and the packet carries the probability
+         * 1 - e^-tau_edge that an analog packet interacts at all (Cashwell & Everett 1959). */
+        double q[3] = { p[0], p[1], p[2] }, tau_edge = 0.0;
+        int c3[3] = { ijk[0], ijk[1], ijk[2] };
+        uint64_t seg = 0;
+        int st = march(G, rc->ch->alpha, q, n, c3, INFINITY, &tau_edge, &seg, NULL);
+        if (st == ST_ESCAPE || (st == ST_SURFACE && !(rc->g->surface_albedo > 0.0))) {
+            const double pint = -expm1(-tau_edge);
+            if (!(pint > 0.0)) {            /* empty path: nothing can interact, the packet ends with no event */
+                if (st == ST_ESCAPE) { cnt->packets_escaped++; cnt->escaped_weight += 1.0; } else cnt->packets_surface++;
+                if (rc->evcount) rc->evcount[pkt] = 0;
+                return;
+            }
+            if (st == ST_ESCAPE) cnt->escaped_weight += exp(-tau_edge);   /* the part that leaves without interacting */
+            W = pint;
+            tau_t = -log1p(-z[2] * pint);
+        }
+    }
+    transport(rc, pkt, p, n, ijk, W, tau_t, 0, batch, cnt);
 }
 
 /* O4: emission launch (Eq. 13, Sect. 4.3 with the C10 composite bias). */

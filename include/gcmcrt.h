@@ -80,6 +80,11 @@ typedef struct gcmcrt_run_params {
     double ld_c1, ld_c2;         /* quadratic law I(mu)/I(0) = 1 - c1 (1 - mu) - c2 (1 - mu)^2 (Eq. 22) */
     int cloud_phase;             /* phase function of the cloud scatterers: 0 = Henyey-Greenstein (Eq. 7-8), 1 = two-term
                                     HG (Eq. 10) with the paper's default g1 = g, g2 = -g/2, alpha = 1 - g2^2 (L157) */
+    int forced_first;            /* gcmcrt_run_albedo only: forced first scattering (Sect. 4.2): the optical depth
+                                    tau_edge along the launch ray to where it leaves the grid is integrated first, the
+                                    flight is drawn as tau = -ln(1 - zeta (1 - e^-tau_edge)) and the packet starts with
+                                    W = 1 - e^-tau_edge; e^-tau_edge is added to counters.escaped_weight when the ray
+                                    leaves through the top.  Rays that end on a reflecting lower boundary stay analog. */
 } gcmcrt_run_params;
 
 typedef struct gcmcrt_counters {

@@ -301,6 +301,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
 
     int rcode = ensure_workspace(g);
     if (rcode) return rcode;
+    if (prm->forced_first && g->tune[2] == 0)
+        return fail(g, GCMCRT_E_INVALID, "forced_first needs the wavefront transport (GCMCRT_TUNE generations > 0)");
 
     // ---- outputs
     OutBuf o_flux, o_ltot, o_val, o_sig, o_img, o_evc, o_cnt, o_ctb;
@@ -336,6 +338,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.max_events = prm->max_events; rc.scatter_on = prm->scatter_on;
     rc.survival_bias = prm->survival_bias != 0;
     rc.cloud_phase = prm->cloud_phase;
+    rc.forced_first = prm->forced_first != 0;
     if (prm->cloud_phase != 0 && prm->cloud_phase != 1) return fail(g, GCMCRT_E_INVALID, "cloud_phase must be 0 (HG) or 1 (TTHG)");
     rc.roulette_w_min = float(prm->roulette_w_min); rc.roulette_survive = float(prm->roulette_survive);
     rc.surface_albedo = g->surface_albedo;
@@ -517,7 +520,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         // ---- wavefront kernels (wavefront.cuh): launch geometry and the launch-order sort of albedo runs
         const int n_gen = g->tune[2];
         auto k_keys = wave_launch_keys_kernel;
-        auto k_first = wave_first_flight_kernel<8>;
+        auto k_first = rc.forced_first ? wave_first_flight_kernel<8, true> : wave_first_flight_kernel<8, false>;
         auto k_emit = wave_emit_kernel;
         auto k_inter = wave_interact_kernel<kInteractK>;
         const size_t smem_w = smem_t;

@@ -100,6 +100,7 @@ struct RunConst {
     int survival_bias;             // Sect. 4.4: forced scattering with W <- W omega
     float roulette_w_min, roulette_survive;   // Sect. 4.5: Russian roulette below the weight threshold (0 = off)
     int cloud_phase;               // 0 HG (Eq. 7-8), 1 two-term HG (Eq. 10, g1 = g, g2 = -g/2, alpha = 1 - g2^2)
+    int forced_first;              // albedo: forced first scattering (Sect. 4.2)
     float surface_albedo;
     double xi;
     int n_batches;

@@ -268,8 +268,8 @@ __global__ void __launch_bounds__(kWaveThreads) wave_launch_keys_kernel(const __
 }
 
 // albedo: launch + first flight, 32 packets of neighbouring entry columns per warp
-template <int KSTEPS>
-__global__ void __launch_bounds__(kWaveThreads, 4)
+template <int KSTEPS, bool FORCED>
+__global__ void __launch_bounds__(kWaveThreads, FORCED ? 3 : 4)
 wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const SuspBuf susp, const WaveConst wc)
 {
     extern __shared__ float smem_f[];
@@ -282,7 +282,7 @@ wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
         const bool active = t < wc.n_items;
         uint32_t chan_run = 0, pkt = 0;
         Ray ray{};
-        float tau_t = 0.f;
+        float tau_t = 0.f, z2 = 0.f;
         const float* alpha_c = rc.alpha;
         if (active) {
             wave_item(rc, wc.item0 + __ldg(wc.perm + t), chan_run, pkt);
@@ -293,9 +293,34 @@ wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
             int j, k;
             albedo_launch_point(rc, gs, z, px, py, pz, j, k);
             tau_t = -logf(z.z2);
+            z2 = z.z2;
             ray_init(ray, gs, px, py, pz, -rc.star[0], -rc.star[1], -rc.star[2], gs.nlev - 1, j, k, alpha_c);
         }
-        wave_fly<KSTEPS>(rc, ev, susp, wc.park_all, gs, active, ray, tau_t, alpha_c, 1.0f, chan_run, pkt, 0u, wcnt);
+        float W = 1.0f;
+        bool fly = active;
+        if (FORCED) {
+            // Sect. 4.2 (L179), forced first scattering: the extra ray trace to the end of the grid gives tau_edge; the
+            // flight is drawn from the exponential law truncated there and the packet carries 1 - e^-tau_edge.  A ray
+            // that ends on a reflecting lower boundary stays analog.
+            Ray probe = ray;
+            int st = active ? RAY_FLYING : RAY_NONE;
+            float tau_e = 0.f;
+            WaveCounters unused;
+            wave_march<KSTEPS>(rc, gs, st, probe, tau_e, kInf, alpha_c, rc.geom.maxseg + 1, unused);
+            if (active && (st == RAY_ESCAPE || (st == RAY_SURFACE && !(rc.surface_albedo > 0.f)))) {
+                const float pint = -expm1f(-tau_e);
+                if (!(pint > 0.f)) {   // empty path: the packet ends with no event
+                    if (st == RAY_ESCAPE) { ++wcnt.esc; wcnt.escw += 1.0; } else ++wcnt.surf;
+                    wave_finish_packet(rc, chan_run, pkt, 0u);
+                    fly = false;
+                } else {
+                    if (st == RAY_ESCAPE) wcnt.escw += double(expf(-tau_e));   // the part that leaves without interacting
+                    W = pint;
+                    tau_t = -log1pf(-z2 * pint);
+                }
+            }
+        }
+        wave_fly<KSTEPS>(rc, ev, susp, wc.park_all, gs, fly, ray, tau_t, alpha_c, W, chan_run, pkt, 0u, wcnt);
     }
     wave_flush_counters(rc, wcnt);
 }

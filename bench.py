@@ -65,6 +65,11 @@ def make_workload(name, packets=None, channels=None):
         # (4.9 GB of tables), so --channels can cut the wavelength range for a quick look (say so when quoting it)
         grid, opac, prm = wl.cfg4(packets=packets or 100000, **({"n_chan": channels} if channels else {}))
         mode = "emission"
+    elif name == "cfg5":
+        # large high-resolution run, emission + albedo at 4 phases, node tables streamed in wavelength batches; the
+        # default 4096 of the 1e5 wavelength points keep a step at a few seconds (--channels 100000 for all of them)
+        grid, opac, prm = wl.cfg5(packets=packets or 100000, n_chan=channels or 4096)
+        mode = "emission+albedo"
     else:
         raise SystemExit("unknown workload %s" % name)
     return grid, opac, prm, mode
@@ -225,8 +230,9 @@ def run_ours(args):
     n_chan = int(np.asarray(opac["lambda"]).size)
     opac["chan0"] = rank_chan0(rank, n_chan)   # this rank's global channel range (keys the Philox streams)
     N = int(prm["packets_per_channel"])
-    tab_keys = [k for k in ("k_abs", "k_sca_ray", "k_sca_cld", "g_cld") if opac.get(k) is not None]
+    tab_keys = [k for k in ("k_abs", "k_sca_ray", "k_sca_cld", "g_cld", "node_kabs", "p_cell") if opac.get(k) is not None]
     stream = torch.cuda.current_stream()
+    streamed = args.workload == "cfg5"
 
     # device-resident tables for `value`, pinned host tables for `e2e`
     dev_opac = dict(opac)
@@ -236,9 +242,32 @@ def run_ours(args):
         host_opac[k] = t.pin_memory()
         dev_opac[k] = t.cuda()
     h2d = sum(host_opac[k].numel() * 4 for k in tab_keys) + n_chan * 4
+    if streamed:   # the cells' pressures travel with every batch
+        h2d += host_opac["p_cell"].numel() * 4 * (len(wl.cfg5_batches(opac, batch=args.batch)) - 1)
     G = binding.Grid(grid, stream=stream)
 
+    def step_streamed(op, device_outputs):
+        # config 5: per wavelength batch (+ halo channels for the Doppler window) the node tables go through
+        # gcmcrt_set_opacity_nodes, the batch's Rayleigh table is filled on the device, and the batch is run in
+        # emission and in albedo mode toward the 4 phases; counters and output bytes are summed over the runs
+        ncell = int(np.asarray(grid["T"]).size)
+        coef = torch.from_numpy(opac["k_ray_chan"]).cuda()
+        tot, nbytes = {}, 0
+        for c0, c1, lo, hi in wl.cfg5_batches(opac, batch=args.batch, halo=int(prm["doppler_halfwidth"])):
+            sub = dict(op, chan0=op["chan0"] + lo, node_kabs=op["node_kabs"][lo:hi])
+            sub["lambda"] = opac["lambda"][lo:hi]
+            sub["k_sca_ray"] = coef[lo:hi, None].expand(hi - lo, ncell).contiguous()
+            G.set_opacity_nodes(sub)
+            for fn in (G.run_emission, G.run_albedo):
+                out = fn(dict(prm, chan_begin=c0 - lo, chan_end=c1 - lo), device_outputs=device_outputs)
+                for k, v in out["counters"].items():
+                    tot[k] = tot.get(k, 0) + v
+                nbytes += sum(out[k].nbytes for k in ("flux_sum", "L_tot", "value", "sigma") if k in out and not device_outputs)
+        return {"counters": tot, "d2h_bytes": nbytes}
+
     def step(op, device_outputs):
+        if streamed:
+            return step_streamed(op, device_outputs)
         G.set_opacity(op)
         fn = G.run_albedo if mode == "albedo" else G.run_emission
         return fn(prm, device_outputs=device_outputs)
@@ -273,7 +302,7 @@ def run_ours(args):
     # e2e: host tables in, host spectra out
     step(host_opac, False)
     ms_e2e, acc_e2e, out_e2e = timed(host_opac, False, args.steps)
-    d2h = sum(out_e2e[k].nbytes for k in ("flux_sum", "L_tot", "value", "sigma") if k in out_e2e)
+    d2h = out_e2e["d2h_bytes"] if streamed else sum(out_e2e[k].nbytes for k in ("flux_sum", "L_tot", "value", "sigma") if k in out_e2e)
 
     ms, (ev_all, seg_all) = reduce_over_ranks(ms, [acc["events"], acc["segments_transport"] + acc["segments_peel"]],
                                               world, "cuda")
@@ -297,6 +326,8 @@ def run_ours(args):
         achieved = work / (dur_ms * 1e-3) / 1e12 if dur_ms > 0 else 0.0
         ncell = int(np.asarray(grid["T"]).size)
         hbm_bytes = n_chan * ncell * 4 * (len(tab_keys) + 1 + 4)   # tables read once + alpha/prop written once
+        if streamed:   # Rayleigh table written once; 8 Doppler stagings (4 phases x 2 modes) each read it and write alpha + prop
+            hbm_bytes = n_chan * ncell * (4 + 8 * (4 + 4 + 16))
         roofline = {"bound": "alu", "kernel": dom + "_kernel", "achieved": achieved, "peak": peak,
                     "unit": "Tlane-instr/s", "frac": achieved / peak if peak else None,
                     # dram__bytes_read + write per peel_kernel launch from one ncu --set full capture of the default
@@ -313,7 +344,8 @@ def run_ours(args):
                                           "note": "launch sort + first flights + interact generations + persistent tail, same units"},
                     "whole_step": {"achieved": (work + work_t) / (ms / args.steps * 1e-3 * args.steps) / 1e12,
                                    "frac": (work + work_t) / (ms * 1e-3) / 1e12 / peak}}
-        cpu = oracle_leg(args.workload, grid, dict(opac, chan0=0), prm, mode) if world == 1 and not args.no_cpu else None
+        # config 5 has no per-cell table for the oracle to read (328 GB at full size): no cpu_baseline leg there
+        cpu = oracle_leg(args.workload, grid, dict(opac, chan0=0), prm, mode) if world == 1 and not args.no_cpu and not streamed else None
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -344,8 +376,9 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4"])
-    ap.add_argument("--channels", type=int, default=None, help="cfg4 only: number of wavelength points (default 10000)")
+    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--channels", type=int, default=None, help="cfg4 / cfg5: number of wavelength points (default 10000 / 4096)")
+    ap.add_argument("--batch", type=int, default=1024, help="cfg5: wavelength points per streamed opacity batch")
     ap.add_argument("--packets", type=int, default=None, help="override packets per channel (debugging only)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()

@@ -17,10 +17,12 @@
  *    pinned) or in device memory; the library asks cudaPointerGetAttributes and copies host arrays
  *    to / from internal device buffers with cudaMemcpyAsync on the caller's stream.  Arguments
  *    documented "host" are read on the CPU during the call.
- *  - OWNERSHIP: the library copies or stages everything it needs during the call that receives it,
- *    EXCEPT the device-resident k_abs table given to gcmcrt_set_opacity, which is borrowed until
- *    the next gcmcrt_set_opacity / gcmcrt_destroy when a later run uses doppler_on (the shifted
- *    tables are rebuilt from it per observer, Eq. 33-34).  Output buffers are caller-owned.
+ *  - OWNERSHIP: the library copies everything it needs during the call that receives it, EXCEPT
+ *    DEVICE-resident per-cell opacity tables given to gcmcrt_set_opacity / gcmcrt_set_opacity_nodes
+ *    (k_abs, k_sca_ray, k_sca_cld, g_cld): those are borrowed until the next
+ *    gcmcrt_set_opacity* / gcmcrt_destroy, because the packed per-cell records are staged from them
+ *    by the runs (once for an unshifted run, once per observer with doppler_on, Eq. 33-34).  Host
+ *    tables are copied to internal device buffers during the call.  Output buffers are caller-owned.
  *  - STREAMS: all work is enqueued on `stream` (a cudaStream_t passed as void*, NULL = legacy
  *    default stream).  gcmcrt_run_* synchronise with the stream only to read two pass counters per
  *    pass (a few bytes); results are complete when the stream has drained (or on return for host

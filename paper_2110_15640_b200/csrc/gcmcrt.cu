@@ -70,7 +70,8 @@ struct gcmcrt_grid {
     DevBuf node, node_idx, node_w, own_pcell;     // k_abs from (T, log10 p) node tables (gcmcrt_set_opacity_nodes)
     int nT = 0, nP = 0;
     bool use_nodes = false;
-    int staged_obs = -2;   // -2: nothing staged, -1: unshifted table, >= 0: Doppler table of that observer dir
+    int staged_obs = -2;   // -2: no tables set, -3: tables set but nothing staged yet (the first run stages what it needs),
+                           // -1: unshifted table staged, >= 0: Doppler table of staged_dir staged
     double staged_dir[3] = {0, 0, 0};
     int staged_halfwidth = 0;
 
@@ -187,8 +188,12 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
     const size_t n = size_t(g->n_chan) * g->ncell;
     const GeomParams gp0 = geom_params(g);
     const size_t n_alpha = size_t(g->n_chan) * size_t(gp0.alpha_stride);
-    CUDA_TRY(g, g->alpha.ensure(n_alpha * sizeof(float)));
-    CUDA_TRY(g, cudaMemsetAsync(g->alpha.p, 0, n_alpha * sizeof(float), s));   // guard entries and padding
+    if (n_alpha * sizeof(float) > g->alpha.bytes) {
+        // guard entries and padding are zero; the stage kernel writes the level entries only, and the layout of a
+        // channel does not depend on n_chan, so the table is cleared once per allocation
+        CUDA_TRY(g, g->alpha.ensure(n_alpha * sizeof(float)));
+        CUDA_TRY(g, cudaMemsetAsync(g->alpha.p, 0, g->alpha.bytes, s));
+    }
     CUDA_TRY(g, g->prop.ensure(n * sizeof(float4)));
     StageParams sp;
     sp.n_chan = g->n_chan; sp.ncell = g->ncell; sp.nlev = g->nlev; sp.nlat = g->nlat; sp.nlon = g->nlon;
@@ -213,8 +218,12 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
         sp.vlos = g->vlos.as<float>();
         ++g->launches;
     }
-    const long long blocks = std::min<long long>((long long)((n + 255) / 256), (long long)g->sm_count * 32);
-    stage_kernel<<<(unsigned)std::max<long long>(blocks, 1), 256, 0, s>>>(sp);
+    {   // grid = (cell tiles, channel slices): every thread stages its cell for the channels of its slice
+        const unsigned tiles = (unsigned)((g->ncell + 255) / 256);
+        const unsigned want = (unsigned)std::max(1, g->sm_count * 16 / (int)std::max(1u, tiles));
+        const unsigned slices = (unsigned)std::min<long long>(std::min<long long>((g->n_chan + 3) / 4, 65535), std::max<long long>(want, 1));
+        stage_kernel<<<dim3(tiles, slices), 256, 0, s>>>(sp);
+    }
     CUDA_TRY(g, cudaGetLastError());
     ++g->launches;
     CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
@@ -418,7 +427,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         // ---- A2: emission CDF
         if (emission) {
             const size_t n = size_t(g->n_chan) * g->ncell;
-            CUDA_TRY(g, g->Lcell.ensure(n * sizeof(double)));
+            if (prm->emission_bias > 0.0) CUDA_TRY(g, g->Lcell.ensure(n * sizeof(double)));
             CUDA_TRY(g, g->Lcum.ensure(n * sizeof(double)));
             CUDA_TRY(g, g->Ltot.ensure(size_t(g->n_chan) * sizeof(double)));
             EmisParams ep;
@@ -429,11 +438,16 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             ep.lambda = g->lambda64.as<double>();
             ep.r_edges = g->r64.as<double>(); ep.cth_edges = g->cth64.as<double>(); ep.ph_edges = g->ph64.as<double>();
             ep.tau_vert_max = prm->tau_vert_max;
-            ep.Lcell = g->Lcell.as<double>(); ep.Lcum = g->Lcum.as<double>(); ep.Ltot = g->Ltot.as<double>();
-            const long long ncolc = (long long)g->n_chan * g->nlat * g->nlon;
+            ep.Lcell = prm->emission_bias > 0.0 ? g->Lcell.as<double>() : nullptr; ep.Lcum = g->Lcum.as<double>(); ep.Ltot = g->Ltot.as<double>();
             CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
-            emis_cell_kernel<<<(unsigned)((ncolc + 127) / 128), 128, 0, s>>>(ep);
-            emis_scan_kernel<<<g->n_chan, 1024, 0, s>>>(ep);
+            {
+                const unsigned ge = (unsigned)std::min(g->n_chan, g->sm_count * 8);
+                const size_t sm = (2 * size_t(g->nlev) + 32) * sizeof(double);
+                if (g->nlev <= 64) emis_cdf_kernel<2><<<ge, kEmisThreads, sm, s>>>(ep);
+                else if (g->nlev <= 128) emis_cdf_kernel<4><<<ge, kEmisThreads, sm, s>>>(ep);
+                else if (g->nlev <= 256) emis_cdf_kernel<8><<<ge, kEmisThreads, sm, s>>>(ep);
+                else return fail(g, GCMCRT_E_INVALID, "emission: nlev > 256 is not supported");
+            }
             CUDA_TRY(g, g->guide.ensure(size_t(g->n_chan) * kEmisGuide * sizeof(int)));
             emis_guide_kernel<<<(unsigned)(((long long)g->n_chan * kEmisGuide + 255) / 256), 256, 0, s>>>(
                 g->n_chan, g->ncell, ep.Lcum, ep.Ltot, g->guide.as<int>());
@@ -867,9 +881,10 @@ static int set_opacity_common(gcmcrt_grid* g, int chan0, int n_chan, const float
     g->n_chan = n_chan;
     g->launches = 0;
     g->ms_stage_pending = 0.0;
-    const int rcode = stage_opacity(g, nullptr, 0, s);
-    g->launches_pending = g->launches;
-    return rcode;
+    // staging (A0 / A1) is left to the first run: a Doppler run needs the table of its own observer, not the unshifted one
+    g->staged_obs = -3;
+    g->launches_pending = 0;
+    return GCMCRT_OK;
 }
 
 int gcmcrt_run_albedo(gcmcrt_grid* g, const gcmcrt_run_params* p, gcmcrt_result* out, void* stream)
@@ -912,6 +927,7 @@ int gcmcrt_debug_ray_tau(gcmcrt_grid* g, int chan, long n, const float* pos, con
     if (chan < 0 || chan >= g->n_chan || n < 0 || !pos || !dir || !tau) return fail(g, GCMCRT_E_INVALID, "debug_ray_tau: bad arguments");
     if (n == 0) return GCMCRT_OK;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (g->staged_obs == -3) { const int rs = stage_opacity(g, nullptr, 0, s); if (rs) return rs; }
     DevBuf bp, bd, bt, bh;
     const float *dp = nullptr, *dd = nullptr;
     int rcode = GCMCRT_OK;

@@ -196,40 +196,57 @@ __device__ __forceinline__ float stage_kabs(const StageParams& p, int c, int cel
     return __ldg(p.k_abs + (long long)c * p.ncell + cell);
 }
 
+// grid = (cell tiles, channels): a thread stages one cell of one channel; consecutive lanes read consecutive cells of
+// the caller's tables and write consecutive prop records (alpha: consecutive inside a column).  HBM-bound: per
+// (channel, cell) 4-16 B of tables in, 4 B alpha + 16 B prop out.
 __global__ void __launch_bounds__(256) stage_kernel(const StageParams p)
 {
-    const long long total = (long long)p.n_chan * p.ncell;
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total;
-         t += (long long)gridDim.x * blockDim.x) {
-        const int c = int(t / p.ncell);
-        const int cell = int(t - (long long)c * p.ncell);
-        float ka;
-        if (p.doppler && p.n_chan > 1) {
-            // Eq. 34: lambda_eff = lambda_0 (1 - v/c) -> index offset dn = -v/c / ln(lambda_{n+1}/lambda_n), C14
-            float dn = -p.vlos[cell] * (1.0f / 299792458.0f) * p.reff[c];
-            dn = fminf(fmaxf(dn, -float(p.halfwidth)), float(p.halfwidth));
-            // integer and fractional part of dn apart: c + dn in fp32 would lose the fraction at c ~ 1e5 and make
-            // the result depend on where a wavelength batch starts
-            const float fl = floorf(dn);
-            int lo = c + int(fl);
-            float f = dn - fl;
-            if (lo < 0) { lo = 0; f = 0.0f; }
-            if (lo > p.n_chan - 2) { lo = p.n_chan - 2; f = 1.0f; }
-            const float k0 = stage_kabs(p, lo, cell), k1 = stage_kabs(p, lo + 1, cell);
-            ka = (1.0f - f) * k0 + f * k1;
-        } else {
-            ka = stage_kabs(p, c, cell);
+    const int cell = blockIdx.x * blockDim.x + threadIdx.x;
+    if (cell >= p.ncell) return;
+    const int col = cell / p.nlev;   // once per thread: the thread then loops over channels
+    const int i = cell - col * p.nlev;
+    const float rho = __ldg(p.rho + cell);
+    float dn_cell = 0.0f;
+    if (p.doppler && p.n_chan > 1) dn_cell = -__ldg(p.vlos + cell) * (1.0f / 299792458.0f);
+    // four channels per round, all their loads issued before the first store: the kernel lives on bytes in flight
+    constexpr int U = 4;
+    for (int c0 = blockIdx.y * U; c0 < p.n_chan; c0 += gridDim.y * U) {
+        float ka[U], kr[U], kc[U], gg[U];
+#pragma unroll
+        for (int q = 0; q < U; ++q) {
+            const int c = min(c0 + q, p.n_chan - 1);
+            const long long t = (long long)c * p.ncell + cell;
+            if (p.doppler && p.n_chan > 1) {
+                // Eq. 34: lambda_eff = lambda_0 (1 - v/c) -> index offset dn = -v/c / ln(lambda_{n+1}/lambda_n), C14
+                float dn = dn_cell * p.reff[c];
+                dn = fminf(fmaxf(dn, -float(p.halfwidth)), float(p.halfwidth));
+                // integer and fractional part of dn apart: c + dn in fp32 would lose the fraction at c ~ 1e5 and make
+                // the result depend on where a wavelength batch starts
+                const float fl = floorf(dn);
+                int lo = c + int(fl);
+                float f = dn - fl;
+                if (lo < 0) { lo = 0; f = 0.0f; }
+                if (lo > p.n_chan - 2) { lo = p.n_chan - 2; f = 1.0f; }
+                const float k0 = stage_kabs(p, lo, cell), k1 = stage_kabs(p, lo + 1, cell);
+                ka[q] = (1.0f - f) * k0 + f * k1;
+            } else {
+                ka[q] = stage_kabs(p, c, cell);
+            }
+            kr[q] = p.k_ray ? __ldg(p.k_ray + t) : 0.0f;
+            kc[q] = p.k_cld ? __ldg(p.k_cld + t) : 0.0f;
+            gg[q] = p.g_cld ? __ldg(p.g_cld + t) : 0.0f;
         }
-        const float kr = p.k_ray ? __ldg(p.k_ray + t) : 0.0f;
-        const float kc = p.k_cld ? __ldg(p.k_cld + t) : 0.0f;
-        const float g = p.g_cld ? __ldg(p.g_cld + t) : 0.0f;
-        const float ks = kr + kc;
-        const float kext = ka + ks;
-        {   // guard-padded column layout of the marcher: [chan][col][col_stride], level i at offset 1 + i
-            const int col = cell / p.nlev, i = cell - col * p.nlev;
-            p.alpha[(size_t)c * p.alpha_stride + (size_t)col * p.col_stride + 1 + i] = __ldg(p.rho + cell) * kext;
+#pragma unroll
+        for (int q = 0; q < U; ++q) {
+            const int c = c0 + q;
+            if (c >= p.n_chan) break;
+            const long long t = (long long)c * p.ncell + cell;
+            const float ks = kr[q] + kc[q];
+            const float kext = ka[q] + ks;
+            // guard-padded column layout of the marcher: [chan][col][col_stride], level i at offset 1 + i
+            p.alpha[(size_t)c * p.alpha_stride + (size_t)col * p.col_stride + 1 + i] = rho * kext;
+            p.prop[t] = make_float4(kext > 0.0f ? ks / kext : 0.0f, ks > 0.0f ? kr[q] / ks : 0.0f, gg[q], ka[q]);
         }
-        p.prop[t] = make_float4(kext > 0.0f ? ks / kext : 0.0f, ks > 0.0f ? kr / ks : 0.0f, g, ka);
     }
 }
 
@@ -246,7 +263,7 @@ struct EmisParams {
     const double* lambda;   // [n_chan]
     const double *r_edges, *cth_edges, *ph_edges;  // fp64 geometry for the volumes
     double tau_vert_max;
-    double* Lcell;  // [n_chan][ncell] (scratch; overwritten by the scan into Lcum when Lcell_keep == null)
+    double* Lcell;  // [n_chan][ncell] L_i, or NULL (kept for the weights of the composite bias, xi > 0)
     double* Lcum;
     double* Ltot;
 };
@@ -258,69 +275,112 @@ __device__ __forceinline__ double planck_lambda(double lam, double T)
     return 2.0 * h * c * c / (lam * lam * lam * lam * lam) / expm1(x);
 }
 
-// one thread per (channel, column): walks the column from the top, writes L_i with the depth cut applied
-__global__ void __launch_bounds__(128) emis_cell_kernel(const EmisParams p)
+__device__ __forceinline__ double warp_incl_scan_f64(double v)
 {
-    const int ncol = p.nlat * p.nlon;
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= (long long)p.n_chan * ncol) return;
-    const int c = int(t / ncol), col = int(t % ncol);
-    const int j = col % p.nlat, k = col / p.nlat;
-    const double lam = p.lambda[c];
-    const double ang = (p.cth_edges[j] - p.cth_edges[j + 1]) * (p.ph_edges[k + 1] - p.ph_edges[k]);
-    const long long base = (long long)c * p.ncell + (long long)col * p.nlev;
-    double tv = 0.0;
-    for (int i = p.nlev - 1; i >= 0; --i) {
-        const double r0 = p.r_edges[i], r1 = p.r_edges[i + 1];
-        const double vol = (r1 * r1 * r1 - r0 * r0 * r0) / 3.0 * ang;
-        const int cell = col * p.nlev + i;
-        double L = 4.0 * 3.14159265358979323846 * vol * double(p.rho[cell]) * double(p.prop[base + i].w) *
-                   planck_lambda(lam, double(p.T[cell]));
-        if (p.tau_vert_max > 0.0 && tv > p.tau_vert_max) L = 0.0;
-        tv += double(p.alpha[(size_t)c * p.alpha_stride + (size_t)col * p.col_stride + 1 + i]) * (r1 - r0);
-        p.Lcell[base + i] = L;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const double n = __shfl_up_sync(kFullMask, v, o);
+        if (lane_id() >= o) v += n;
     }
+    return v;
 }
 
-// one CTA per channel: inclusive fp64 scan of L_i over the ncell cells, chunk by chunk with a carry
-__global__ void __launch_bounds__(1024) emis_scan_kernel(const EmisParams p)
+// One CTA per channel, one warp per column, 32 columns per round, lanes along the column (coalesced alpha / prop
+// reads; NCH = chunks of 32 levels).  A round is one memory latency deep: every input of the column is loaded up
+// front, then the warp finds the depth cut (radial optical depth from the top, C15), computes L_i (Eq. 27), scans it,
+// and -- after the 32 column totals have been chained through shared memory -- writes the running sum once.  Every
+// value is carry + (excl_w + local) with excl_{w+1} = excl_w + tot_w evaluated by the same chain in every thread, so
+// the running sum never decreases from one cell to the next.  HBM traffic per (channel, cell): 4 B alpha + 16 B prop
+// in, 8 B out (T, rho stay in L2 across channels).
+constexpr int kEmisThreads = 1024;
+template <int NCH>
+__global__ void __launch_bounds__(kEmisThreads) emis_cdf_kernel(const EmisParams p)
 {
-    __shared__ double warp_tot[32];
-    __shared__ double carry_s;
-    const int c = blockIdx.x;
-    const double* in = p.Lcell + (long long)c * p.ncell;
-    double* out = p.Lcum + (long long)c * p.ncell;
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    if (threadIdx.x == 0) carry_s = 0.0;
-    __syncthreads();
-    for (int base = 0; base < p.ncell; base += blockDim.x) {
-        const int idx = base + threadIdx.x;
-        double v = idx < p.ncell ? in[idx] : 0.0;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const double n = __shfl_up_sync(kFullMask, v, o);
-            if (lane >= o) v += n;
-        }
-        if (lane == 31) warp_tot[wid] = v;
-        __syncthreads();
-        if (wid == 0) {
-            double w = lane < nw ? warp_tot[lane] : 0.0;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const double n = __shfl_up_sync(kFullMask, w, o);
-                if (lane >= o) w += n;
-            }
-            warp_tot[lane] = w;  // inclusive totals of warps
-        }
-        __syncthreads();
-        const double carry = carry_s;
-        const double pre = wid > 0 ? warp_tot[wid - 1] : 0.0;
-        if (idx < p.ncell) out[idx] = carry + pre + v;
-        __syncthreads();
-        if (threadIdx.x == blockDim.x - 1) carry_s = carry + pre + v;
-        __syncthreads();
+    extern __shared__ double emis_sm[];
+    double* dr = emis_sm;                 // [nlev] R_{i+1} - R_i
+    double* dr3 = dr + p.nlev;            // [nlev] (R_{i+1}^3 - R_i^3) / 3
+    double* col_tot = dr3 + p.nlev;       // [32]
+    const int lane = lane_id(), wid = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < p.nlev; i += blockDim.x) {
+        const double r0 = p.r_edges[i], r1 = p.r_edges[i + 1];
+        dr[i] = r1 - r0;
+        dr3[i] = (r1 * r1 * r1 - r0 * r0 * r0) / 3.0;
     }
-    if (threadIdx.x == 0) p.Ltot[c] = carry_s;
+    __syncthreads();
+    const int ncol = p.nlat * p.nlon;
+    for (int c = blockIdx.x; c < p.n_chan; c += gridDim.x) {
+        const double lam = p.lambda[c];
+        const double hck = 6.62607015e-34 * 299792458.0 / (lam * 1.380649e-23);                     // h c / (lambda k)
+        const double pre = 4.0 * 3.14159265358979323846 * 2.0 * 6.62607015e-34 * 299792458.0 * 299792458.0 /
+                           (lam * lam * lam * lam * lam);                                            // 4 pi 2 h c^2 / lambda^5
+        const float* alpha_c = p.alpha + (size_t)c * p.alpha_stride;
+        const float4* prop_c = p.prop + (size_t)c * p.ncell;
+        double* out = p.Lcum + (size_t)c * p.ncell;
+        double carry = 0.0;
+        for (int col0 = 0; col0 < ncol; col0 += 32) {
+            const int col = min(col0 + wid, ncol - 1);       // surplus warps of the last round redo its last column
+            const bool live = col0 + wid < ncol;
+            const size_t cell0 = (size_t)col * p.nlev;
+            const float* acol = alpha_c + (size_t)col * p.col_stride + 1;
+            float a[NCH], T[NCH], rk[NCH];
+#pragma unroll
+            for (int m = 0; m < NCH; ++m) {                  // level i = 32 m + lane
+                const int i = (m << 5) + lane;
+                const bool in = i < p.nlev;
+                a[m] = in ? __ldg(acol + i) : 0.0f;
+                T[m] = in ? __ldg(p.T + cell0 + i) : 1.0f;
+                rk[m] = in ? __ldg(p.rho + cell0 + i) * __ldg(&prop_c[cell0 + i].w) : 0.0f;
+            }
+            // depth cut: cell i is dropped when the radial optical depth of the levels above it exceeds tau_vert_max;
+            // suffix sums from the top = column total - inclusive prefix from below
+            int i_cut = 0;   // lowest level kept
+            if (p.tau_vert_max > 0.0) {
+                double d[NCH], incl[NCH], tot = 0.0;
+#pragma unroll
+                for (int m = 0; m < NCH; ++m) {
+                    const int i = (m << 5) + lane;
+                    d[m] = i < p.nlev ? double(a[m]) * dr[i] : 0.0;
+                    incl[m] = tot + warp_incl_scan_f64(d[m]);
+                    tot = __shfl_sync(kFullMask, incl[m], 31);
+                }
+#pragma unroll
+                for (int m = 0; m < NCH; ++m) {
+                    const int i = (m << 5) + lane;
+                    const unsigned mc = __ballot_sync(kFullMask, i < p.nlev && (tot - incl[m]) > p.tau_vert_max);
+                    if (mc) i_cut = (m << 5) + 32 - __clz(mc);   // highest cut level + 1 (the sum only grows downward)
+                }
+            }
+            const int j = col % p.nlat, k = col / p.nlat;
+            const double ang = (p.cth_edges[j] - p.cth_edges[j + 1]) * (p.ph_edges[k + 1] - p.ph_edges[k]);
+            double loc[NCH], run = 0.0;
+#pragma unroll
+            for (int m = 0; m < NCH; ++m) {
+                const int i = (m << 5) + lane;
+                double L = 0.0;
+                if (i < p.nlev && i >= i_cut) L = pre * dr3[i] * ang * double(rk[m]) / expm1(hck / double(T[m]));
+                if (p.Lcell && live && i < p.nlev) p.Lcell[(size_t)c * p.ncell + cell0 + i] = L;
+                loc[m] = run + warp_incl_scan_f64(L);
+                run = __shfl_sync(kFullMask, loc[m], 31);
+            }
+            if (lane == 0) col_tot[wid] = live ? run : 0.0;
+            __syncthreads();
+            double excl = 0.0, tile = 0.0;
+            for (int w = 0; w < 32; ++w) {   // the same chain in every thread
+                if (w == wid) excl = tile;
+                tile += col_tot[w];
+            }
+            if (live) {
+#pragma unroll
+                for (int m = 0; m < NCH; ++m) {
+                    const int i = (m << 5) + lane;
+                    if (i < p.nlev) out[cell0 + i] = carry + (excl + loc[m]);
+                }
+            }
+            carry += tile;
+            __syncthreads();
+        }
+        if (threadIdx.x == 0) p.Ltot[c] = carry;
+    }
 }
 
 // Guide table of the emission CDF: guide[c][g] = first cell whose running luminosity exceeds (g / kEmisGuide) L_tot.

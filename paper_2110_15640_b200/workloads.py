@@ -199,7 +199,7 @@ def _voigt_profile(x, sigma, gamma):
 
 
 def hires_opacity(grid, rng, n_chan=10000, lam0=2.19e-6, R=1.0e5, n_lines=500, nT=16, nP=16, k_cont=1e-4,
-                  chan_block=512):
+                  chan_block=512, cells=True):
     """Config 4/5 high-resolution table: kappa_abs from n_lines synthetic Voigt lines evaluated on an nT x nP
     (T, log p) node grid and bilinearly interpolated to every cell; no scattering."""
     nlon, nlat, nlev = grid["T"].shape
@@ -228,15 +228,16 @@ def hires_opacity(grid, rng, n_chan=10000, lam0=2.19e-6, R=1.0e5, n_lines=500, n
     fp = np.clip((lp_cell - lpn[0]) / (lpn[1] - lpn[0]), 0.0, nP - 1 - 1e-9)
     it, ip = ft.astype(int), fp.astype(int)
     wt, wp = ft - it, fp - ip
-    k_abs = np.empty((n_chan, nlon, nlat, nlev), dtype=np.float32)
-    for c0 in range(0, n_chan, chan_block):
-        nd = node[c0:c0 + chan_block]
-        k_abs[c0:c0 + chan_block] = ((1 - wt) * (1 - wp) * nd[:, it, ip] + wt * (1 - wp) * nd[:, it + 1, ip]
-                                     + (1 - wt) * wp * nd[:, it, ip + 1] + wt * wp * nd[:, it + 1, ip + 1])
     opac = dict(chan0=0)
     opac["lambda"] = lam.astype(np.float32)
     opac["lambda64"] = lam
-    opac["k_abs"] = k_abs
+    if cells:   # per-cell table (config 4); config 5 hands the node tables to gcmcrt_set_opacity_nodes instead
+        k_abs = np.empty((n_chan, nlon, nlat, nlev), dtype=np.float32)
+        for c0 in range(0, n_chan, chan_block):
+            nd = node[c0:c0 + chan_block]
+            k_abs[c0:c0 + chan_block] = ((1 - wt) * (1 - wp) * nd[:, it, ip] + wt * (1 - wp) * nd[:, it + 1, ip]
+                                         + (1 - wt) * wp * nd[:, it, ip + 1] + wt * wp * nd[:, it + 1, ip + 1])
+        opac["k_abs"] = k_abs
     # the same table in the form gcmcrt_set_opacity_nodes takes: node values + the cells' pressures
     opac["node_kabs"] = node.astype(np.float32)
     opac["T_nodes"] = Tn.astype(np.float32)
@@ -253,3 +254,28 @@ def cfg4(nlon=64, nlat=32, nlev=60, n_chan=10000, packets=100000, seed=4, n_line
     prm = default_params(star_dir=sph_dir(np.pi / 2, 0.0), obs_dir=sph_dir(np.pi / 2, 0.0)[None, :],
                          packets_per_channel=packets, seed=seed, scatter_on=0, doppler_on=1, doppler_halfwidth=4)
     return grid, opac, prm
+
+
+def cfg5(nlon=128, nlat=64, nlev=100, n_chan=100000, packets=100000, seed=5, n_lines=500, lam0=0.95e-6):
+    """BASELINE config 5: large high-resolution run, emission + albedo at 4 orbital phases, opacities as (T, log p) node
+    tables streamed in wavelength batches (the first n_chan points of lambda_n = 0.95 um
+    (1 + 1e-5)^n; synthetic lines as in config 4).  The per-cell absorption table (328 GB at full size) is never
+    built: `opac` carries the node tables, and a per-channel Rayleigh coefficient `k_ray_chan` (kappa_Ray =
+    3e-5 (lambda / 0.5 um)^-4 m^2/kg in every cell, the law of config 1) from which the caller fills the
+    [n_chan][ncell] scattering table of a batch."""
+    grid, rng = gcm_grid(nlon, nlat, nlev, seed=seed)
+    add_winds(grid)
+    opac = hires_opacity(grid, rng, n_chan=n_chan, n_lines=n_lines, lam0=lam0, cells=False)
+    opac["k_ray_chan"] = (3.0e-5 * (opac["lambda64"] / 0.5e-6) ** -4).astype(np.float32)
+    phases = (np.arange(4) + 0.5) / 4.0
+    obs = np.stack([sph_dir(np.pi / 2, np.pi + 2 * np.pi * ph) for ph in phases])
+    prm = default_params(star_dir=sph_dir(np.pi / 2, 0.0), obs_dir=obs, packets_per_channel=packets, seed=seed,
+                         scatter_on=1, doppler_on=1, doppler_halfwidth=4)
+    return grid, opac, prm
+
+
+def cfg5_batches(opac, batch=1024, halo=4):
+    """Wavelength batches of config 5: (c0, c1, lo, hi) = channels [c0, c1) are run from a table that holds channels
+    [lo, hi), i.e. `halo` extra channels on each side for the Doppler window."""
+    n = int(opac["lambda"].size)
+    return [(c0, min(c0 + batch, n), max(c0 - halo, 0), min(c0 + batch + halo, n)) for c0 in range(0, n, batch)]

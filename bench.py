@@ -42,11 +42,11 @@ UNIT = "events/s"
 
 # Algorithmic lane-instructions (FP32/INT issue slots) per unit of work; DESIGN.md section "Roofline" derives them
 # from the audited SASS of the march loop, the event handler and the launch code.
-I_SEG_3D = 40.0      # one 3D cell crossing: radial step 36.3 thread-instructions (ncu source page, executed counts) +
-                     # 4 % cone / half-plane crossings x ~45 + the column's extinction reload
-I_SEG_1D = 37.0      # nlat = nlon = 1: the same radial step, no lateral crossings
+I_SEG_3D = 34.0      # one 3D cell crossing: radial run 28.8 executed thread-instructions per segment + cone / half-plane /
+                     # column updates 5.3 per segment (ncu source page, profiles/ncu_full_r01b_ray_run.txt)
+I_SEG_1D = 29.0      # nlat = nlon = 1: the same radial run, no lateral crossings
 I_EVENT = 420.0      # Philox block, phase sampling, rotation, ray setup, event record write + read
-PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 = 4.49e9   # ncu: 7 launches of a cfg2 step average 4.488 GB read + 4.8 MB written
+PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 = 4.51e9   # ncu: 7 launches of a cfg2 step average 4.506 GB read + 6.4 MB written
 I_PEEL_RAY = 300.0   # record + prop read, phase function, ray setup for one (event, observer), exp, bin accumulation
 
 
@@ -331,7 +331,7 @@ def run_ours(args):
         roofline = {"bound": "alu", "kernel": dom + "_kernel", "achieved": achieved, "peak": peak,
                     "unit": "Tlane-instr/s", "frac": achieved / peak if peak else None,
                     # dram__bytes_read + write per peel_kernel launch from one ncu --set full capture of the default
-                    # workload (profiles/ncu_full_r01_wavefront.txt); other workloads: not captured
+                    # workload (profiles/ncu_full_r01b_ray_run.txt); other workloads: not captured
                     "traffic": PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 if (args.workload == "cfg2" and args.packets is None) else None,
                     "traffic_unit": "bytes per launch (54 M events: 64 B record + 4 B permutation entry + extinction gathers)",
                     "peak_source": "148 SM x 128 FP32 lanes x sm_max_mhz (%s)" % pk["source"],

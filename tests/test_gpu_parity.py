@@ -521,6 +521,45 @@ def test_full_size_cfg2_sampled_packets_and_invariants(gpu, orc):
         assert np.array_equal(gs_["event_count"][0], evc[ch, :n_s].cpu().numpy().astype(np.uint32))
 
 
+def test_full_size_cfg3_sampled_packets_and_invariants(gpu, orc):
+    """BASELINE config 3 at its full size (emission, scattering on, 8 orbital phases peeled in one pass, 176 channels x
+    1e6 packets), as bench.py --workload cfg3 launches it: invariants that hold at any size, L_tot of every channel
+    against the oracle's channel preparation, and -- for three channels -- the first packets as a run of their own
+    against the oracle (full parity bar), whose event counts must be the ones the full-size run recorded."""
+    import torch
+    grid, opac, prm = wl.cfg3(packets=1000000)
+    n_chan = opac["lambda"].size
+    N = 1000000
+    dev = dict(opac)
+    for k in ("k_abs", "k_sca_ray", "k_sca_cld", "g_cld"):
+        if opac.get(k) is not None:
+            dev[k] = torch.from_numpy(np.ascontiguousarray(opac[k], dtype=np.float32)).cuda()
+    with gpu.Grid(grid) as G:
+        G.set_opacity(dev)
+        g = G.run_emission(prm, device_outputs=True, want_event_count=True)
+    c = g["counters"]
+    assert c["packets_escaped"] + c["packets_absorbed"] + c["packets_surface"] == N * n_chan and c["packets_stuck"] == 0
+    evc = g["event_count"]
+    assert int(evc.to(torch.int64).sum().item()) == c["events"]
+    assert c["rays_peel"] == 8 * c["events"] and int(evc.min().item()) >= 1      # every packet has its emission point
+    val = g["value"].cpu().numpy(); sig = g["sigma"].cpu().numpy(); ltot = g["L_tot"].cpu().numpy()
+    assert val.shape == (n_chan, 8) and np.all(val > 0) and np.all(np.isfinite(sig))
+    # the dayside (orbital phase 0.5, observer index 4) is the brightest view of every channel, the nightside the faintest
+    assert np.all(val.argmax(axis=1) == 4) and np.all(val.argmin(axis=1) == 0)
+    for ch in (0, 77, 175):
+        one = {k: (np.ascontiguousarray(v[ch:ch + 1]) if isinstance(v, np.ndarray) and v.shape[:1] == (n_chan,) else v)
+               for k, v in opac.items()}
+        one["chan0"] = ch
+        prep = orc.channel_prep(grid, one, prm, 0)
+        assert np.all(np.abs(np.atleast_1d(ltot[ch]) / prep["L_tot"] - 1) < 2e-5)
+        n_s = 1500
+        small = dict(prm, packets_per_channel=n_s)
+        gs_ = _gpu_run(gpu, grid, one, small, "emission", want_event_count=True)
+        os_ = orc.run_emission(grid, one, dict(small, n_threads=os.cpu_count() or 1), want_event_count=True)
+        _check_parity(orc, gs_, os_, "emission")
+        assert np.array_equal(gs_["event_count"][0], evc[ch, :n_s].cpu().numpy().astype(np.uint32))
+
+
 def test_opacity_from_node_tables_matches_per_cell_tables(gpu, orc):
     """gcmcrt_set_opacity_nodes: k_abs interpolated on the device from (T, log10 p) node tables gives the same run as
     the per-cell table the input generator interpolated on the host (and as the oracle on that table), with and

@@ -264,8 +264,16 @@ static void plane_candidate(const geom_t *G, int edge, int face, const double p[
 }
 
 /* Advance (p, ijk) along n until tau_limit is reached, the TOA is left, or the surface is hit. */
+static int march2(const geom_t *G, const double *alpha, double p[3], const double n[3], int ijk[3],
+                  double tau_limit, double *tau_out, uint64_t *nseg, double *path, const double *alpha_b, double *tau_b);
 static int march(const geom_t *G, const double *alpha, double p[3], const double n[3], int ijk[3],
                  double tau_limit, double *tau_out, uint64_t *nseg, double *path)
+{
+    return march2(G, alpha, p, n, ijk, tau_limit, tau_out, nseg, path, NULL, NULL);
+}
+/* alpha_b (optional): a second extinction integrated over the same path into *tau_b (Eq. 12: tau_abs of the flight) */
+static int march2(const geom_t *G, const double *alpha, double p[3], const double n[3], int ijk[3],
+                  double tau_limit, double *tau_out, uint64_t *nseg, double *path, const double *alpha_b, double *tau_b)
 {
     int i = ijk[0], j = ijk[1], k = ijk[2];
     double tau = 0.0;
@@ -305,11 +313,13 @@ static int march(const geom_t *G, const double *alpha, double p[3], const double
             double s = (tau_limit - tau) / a;
             for (int m = 0; m < 3; ++m) p[m] += n[m] * s;
             if (path) *path += s;
+            if (alpha_b) *tau_b += alpha_b[cell_index(G, i, j, k)] * s;
             tau = tau_limit;
             status = ST_INTERACT;
             break;
         }
         tau += a * smin;
+        if (alpha_b) *tau_b += alpha_b[cell_index(G, i, j, k)] * smin;
         for (int m = 0; m < 3; ++m) p[m] += n[m] * smin;
         if (path) *path += smin;
         switch (face) {
@@ -391,15 +401,17 @@ static double doppler_kabs(const orc_grid *g, const orc_opacity *op, const geom_
 typedef struct {
     double *alpha, *omega, *pgas, *gg, *Lcum; /* [ncell] each; Lcum = running sum of L_i */
     double *Lcell;
+    double *alpha_sca, *alpha_abs;            /* rho kappa_sca, rho kappa_abs (continuous absorption, Eq. 12) */
     double L_tot;
 } chan_t;
 
 static int chan_alloc(chan_t *ch, int ncell)
 {
-    ch->alpha = (double *)malloc(sizeof(double) * (size_t)ncell * 6);
+    ch->alpha = (double *)malloc(sizeof(double) * (size_t)ncell * 8);
     if (!ch->alpha) return -1;
     ch->omega = ch->alpha + ncell; ch->pgas = ch->omega + ncell; ch->gg = ch->pgas + ncell;
     ch->Lcell = ch->gg + ncell; ch->Lcum = ch->Lcell + ncell;
+    ch->alpha_sca = ch->Lcum + ncell; ch->alpha_abs = ch->alpha_sca + ncell;
     ch->L_tot = 0.0;
     return 0;
 }
@@ -422,6 +434,8 @@ static void chan_prep(const orc_grid *g, const geom_t *G, const orc_opacity *op,
                 double ks = kr + kc;
                 double kext = ka + ks;
                 ch->alpha[cell] = rho * kext;                       /* alpha_ext */
+                ch->alpha_sca[cell] = rho * ks;
+                ch->alpha_abs[cell] = rho * ka;
                 ch->omega[cell] = kext > 0.0 ? ks / kext : 0.0;     /* single-scattering albedo */
                 ch->pgas[cell] = ks > 0.0 ? kr / ks : 0.0;          /* Eq. 11 */
                 ch->gg[cell] = op->g_cld ? op->g_cld[(size_t)c * nc + cell] : 0.0;
@@ -590,9 +604,19 @@ static void transport(const run_ctx *rc, uint32_t pkt, double p[3], double n[3],
     const double a_surf = rc->g->surface_albedo;
     uint32_t m_inter = 0;    /* interaction index (Philox event index), 1,2,... */
     double z[4];
+    const int cont = prm->continuous_absorption != 0;
     for (;;) {
         double tau = 0.0;
-        int st = march(G, ch->alpha, p, n, ijk, tau_t, &tau, &cnt->segments_transport, NULL);
+        int st;
+        if (cont) {
+            /* Sect. 4.1, Eq. 12: the sampled optical depth is spent on the scattering extinction alone and the packet
+             * loses weight smoothly, W <- W e^-tau_abs, with tau_abs integrated along the same flight */
+            double tau_abs = 0.0;
+            st = march2(G, ch->alpha_sca, p, n, ijk, tau_t, &tau, &cnt->segments_transport, NULL, ch->alpha_abs, &tau_abs);
+            W *= exp(-tau_abs);
+        } else {
+            st = march(G, ch->alpha, p, n, ijk, tau_t, &tau, &cnt->segments_transport, NULL);
+        }
         if (st == ST_ESCAPE) { cnt->packets_escaped++; cnt->escaped_weight += W; break; }
         if (st == ST_STUCK) { cnt->packets_stuck++; break; }
         if (st == ST_SURFACE) {
@@ -614,6 +638,8 @@ static void transport(const run_ctx *rc, uint32_t pkt, double p[3], double n[3],
         orc_zeta_block(prm->seed, rc->chan_key, pkt, m_inter, 1, z);
         int cell = cell_index(G, ijk[0], ijk[1], ijk[2]);
         double omega = ch->omega[cell], pgas = ch->pgas[cell], gg = ch->gg[cell];
+        if (cont) omega = 1.0;   /* the interaction was drawn from the scattering extinction: it is a scattering (Eq. 14
+                                    without the albedo factor; the absorbed part already left the weight, Eq. 12) */
         peel(rc, p, ijk, 0, W, n, omega, pgas, gg, batch, cnt);     /* peel-off first (Sect. 4.6) */
         if (prm->max_events && (int)m_inter == prm->max_events) { cnt->packets_absorbed++; break; }
         if (!prm->scatter_on) { cnt->packets_absorbed++; break; }

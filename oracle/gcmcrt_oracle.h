@@ -90,6 +90,9 @@ typedef struct {
                                 must end inside the grid: tau_edge = optical depth along the launch ray to where it leaves
                                 the grid (the extra ray trace of L179), tau = -ln(1 - zeta (1 - e^-tau_edge)),
                                 W = 1 - e^-tau_edge.  Rays that end on a reflecting lower boundary stay analog. */
+    int continuous_absorption; /* Sect. 4.1, Eq. 12: flights are sampled against the scattering extinction only and the
+                                weight decays as W <- W e^-tau_abs along every flight; every interaction in the medium
+                                is then a scattering (no absorption draw, no omega in the peel-off weight) */
 } orc_params;
 
 typedef struct {

@@ -908,3 +908,55 @@ def test_forced_first_scattering_conserves_energy_and_matches_analog_on_3d_grid(
     vf, sf = orc.reduce(orc.run_albedo(grid, opac, dict(prm, forced_first=1)), "albedo")
     assert np.all(np.abs(va - vf) < 4 * np.hypot(sa, sf))
     assert np.all(sf < 0.8 * sa)
+
+
+# ----------------------------------------------------------------------------- continuous absorption (Sect. 4.1, Eq. 12)
+def test_continuous_absorption_pure_absorber_carries_exp_minus_tau(orc):
+    """omega = 0: nothing scatters, every packet flies through and its weight is e^-tau_abs of its chord (Eq. 12):
+    the escaped weight is the closed-form chord integral of the layered absorber, with no events at all."""
+    grid, opac, r, alpha = _layered(nlev=8, seed=5)
+    N = 100000
+    prm = wl.default_params(packets_per_channel=N, seed=9, obs_dir=np.zeros((0, 3)), continuous_absorption=1)
+    c = orc.run_albedo(grid, opac, prm)["counters"]
+    R0, Rt = r[0], r[-1]
+    assert c["events"] == 0 and c["packets_absorbed"] == 0 and c["packets_escaped"] + c["packets_surface"] == N
+    nb = 20000
+    b = (np.arange(nb) + 0.5) / nb * Rt
+    tau_full = np.array([_chord_tau(r, alpha, x) for x in b])
+    w_esc = np.sum(np.where(b >= R0, np.exp(-tau_full), 0.0) * 2 * b) * (Rt / nb) / Rt ** 2
+    n_esc = np.sum(np.where(b >= R0, 1.0, 0.0) * 2 * b) * (Rt / nb) / Rt ** 2
+    assert abs(c["packets_escaped"] / N - n_esc) < 4 * np.sqrt(n_esc * (1 - n_esc) / N)
+    assert abs(c["escaped_weight"] / N - w_esc) < 4 * np.sqrt(w_esc / N) + 1e-4     # variance of W 1[esc] <= E[W 1[esc]]
+
+
+@pytest.mark.parametrize("omega", [0.5, 0.9])
+def test_continuous_absorption_keeps_the_exact_semi_infinite_albedo(orc, omega):
+    """Eq. 12 changes weights, not expectations: the geometric albedo of the semi-infinite isotropic atmosphere stays
+    at Chandrasekhar's exact value (golden table, re-derived in test_h_function_table_rederived), alone and together
+    with Russian roulette, which this scheme needs to end its packets."""
+    rows = dict(np.loadtxt(os.path.join(GOLDEN, "isotropic_semi_infinite_albedo.txt")))
+    R0, depth = 1.0e8, 1.0e4
+    grid, opac = wl.uniform_medium(4, 1, 1, R0, R0 + depth, 80.0 / depth, omega, g=0.0, surface_albedo=1.0)
+    s = np.array([0.3, -0.5, 0.81]); s /= np.linalg.norm(s)
+    prm = wl.default_params(packets_per_channel=40000, seed=22, star_dir=s, obs_dir=s[None], continuous_absorption=1,
+                            survival_bias=1, roulette_w_min=0.02, roulette_survive=0.2)
+    val, sig = orc.reduce(orc.run_albedo(grid, opac, prm), "albedo")
+    Ag = PI * val[0, 0]
+    assert abs(Ag - rows[omega]) < 4 * PI * sig[0, 0] + 3e-4 * rows[omega], (Ag, rows[omega], PI * sig[0, 0])
+
+
+def test_continuous_absorption_matches_analog_on_3d_grid_with_less_noise_when_absorbing(orc):
+    """Strongly absorbing 3D atmosphere (omega = 0.15, the case the paper names for Eq. 12): analog and
+    continuous-absorption runs agree within their errors toward every observer, and the expected escaped weight equals
+    the analog escape fraction."""
+    R0, Rt = 1.0e6, 1.3e6
+    grid, opac = wl.uniform_medium(4, 3, 4, R0, Rt, 3.0 / (Rt - R0), 0.15, g=0.3, pgas=0.3)
+    obs = np.array([[1.0, 0, 0], [0.0, 1.0, 0.0], [0.6, 0.0, 0.8]])
+    prm = wl.default_params(packets_per_channel=150000, seed=8, star_dir=[1.0, 0.0, 0.0], obs_dir=obs)
+    ra = orc.run_albedo(grid, opac, prm)
+    rc = orc.run_albedo(grid, opac, dict(prm, continuous_absorption=1, max_events=40))
+    va, sa = orc.reduce(ra, "albedo"); vc, sc = orc.reduce(rc, "albedo")
+    assert np.all(np.abs(va - vc) < 4 * np.hypot(sa, sc))
+    N = 150000
+    fa = ra["counters"]["packets_escaped"] / N
+    assert abs(rc["counters"]["escaped_weight"] / N - fa) < 4 * np.sqrt(fa * (1 - fa) / N) + 4 * np.sqrt(fa / N)

@@ -87,6 +87,12 @@ typedef struct gcmcrt_run_params {
                                     flight is drawn as tau = -ln(1 - zeta (1 - e^-tau_edge)) and the packet starts with
                                     W = 1 - e^-tau_edge; e^-tau_edge is added to counters.escaped_weight when the ray
                                     leaves through the top.  Rays that end on a reflecting lower boundary stay analog. */
+    int continuous_absorption;   /* Sect. 4.1, Eq. 12: flights are sampled against the scattering extinction only and the
+                                    weight decays as W <- W e^-tau_abs over every flight (tau_abs integrated along the
+                                    same path); every interaction in the medium is a scattering (no absorption draw, no
+                                    omega in the peel-off weight).  Packets end by escaping, at the lower boundary, at
+                                    max_events, or by Russian roulette (survival_bias = 1 with roulette_w_min > 0).
+                                    Runs through the persistent transport kernel; excludes forced_first. */
 } gcmcrt_run_params;
 
 typedef struct gcmcrt_counters {

@@ -66,7 +66,8 @@ struct gcmcrt_grid {
     std::vector<float> lambda;
     DevBuf own_kabs, own_kray, own_kcld, own_g;   // copies of host-resident inputs
     const float *k_abs = nullptr, *k_ray = nullptr, *k_cld = nullptr, *g_cld = nullptr;
-    DevBuf alpha, prop, reff, vlos, lambda64;
+    DevBuf alpha, alpha2, prop, reff, vlos, lambda64;
+    bool staged_cont = false;   // the staged tables are those of a continuous-absorption run (pair table, omega = 1)
     DevBuf node, node_idx, node_w, own_pcell;     // k_abs from (T, log10 p) node tables (gcmcrt_set_opacity_nodes)
     int nT = 0, nP = 0;
     bool use_nodes = false;
@@ -183,7 +184,7 @@ cudaError_t ensure_events(gcmcrt_grid* g)
 }
 
 // Stage alpha / prop for observer `obs_dir` (nullptr = unshifted table).
-int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStream_t s)
+int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStream_t s, bool cont = false)
 {
     const size_t n = size_t(g->n_chan) * g->ncell;
     const GeomParams gp0 = geom_params(g);
@@ -194,6 +195,10 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
         CUDA_TRY(g, g->alpha.ensure(n_alpha * sizeof(float)));
         CUDA_TRY(g, cudaMemsetAsync(g->alpha.p, 0, g->alpha.bytes, s));
     }
+    if (cont && 2 * n_alpha * sizeof(float) > g->alpha2.bytes) {
+        CUDA_TRY(g, g->alpha2.ensure(2 * n_alpha * sizeof(float)));
+        CUDA_TRY(g, cudaMemsetAsync(g->alpha2.p, 0, g->alpha2.bytes, s));
+    }
     CUDA_TRY(g, g->prop.ensure(n * sizeof(float4)));
     StageParams sp;
     sp.n_chan = g->n_chan; sp.ncell = g->ncell; sp.nlev = g->nlev; sp.nlat = g->nlat; sp.nlon = g->nlon;
@@ -202,6 +207,7 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
     sp.node_idx = g->node_idx.as<int2>(); sp.node_w = g->node_w.as<float2>(); sp.nT = g->nT; sp.nP = g->nP;
     sp.rho = g->rho.as<float>();
     sp.alpha = g->alpha.as<float>(); sp.prop = g->prop.as<float4>();
+    sp.alpha2 = cont ? g->alpha2.as<float>() : nullptr;
     sp.alpha_stride = gp0.alpha_stride; sp.col_stride = gp0.col_stride;
     sp.doppler = obs_dir != nullptr; sp.halfwidth = halfwidth;
     sp.vlos = nullptr; sp.reff = g->reff.as<float>();
@@ -234,6 +240,7 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
         g->ms_stage_pending += ms;
     }
     g->staged_obs = obs_dir ? 0 : -1;
+    g->staged_cont = cont;
     if (obs_dir) { for (int m = 0; m < 3; ++m) g->staged_dir[m] = obs_dir[m]; g->staged_halfwidth = halfwidth; }
     return GCMCRT_OK;
 }
@@ -310,8 +317,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
 
     int rcode = ensure_workspace(g);
     if (rcode) return rcode;
-    if (prm->forced_first && g->tune[2] == 0)
-        return fail(g, GCMCRT_E_INVALID, "forced_first needs the wavefront transport (GCMCRT_TUNE generations > 0)");
+    if (prm->forced_first && (g->tune[2] == 0 || prm->continuous_absorption))
+        return fail(g, GCMCRT_E_INVALID, "forced_first needs the wavefront transport (GCMCRT_TUNE generations > 0, no continuous_absorption)");
 
     // ---- outputs
     OutBuf o_flux, o_ltot, o_val, o_sig, o_img, o_evc, o_cnt, o_ctb;
@@ -348,6 +355,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.survival_bias = prm->survival_bias != 0;
     rc.cloud_phase = prm->cloud_phase;
     rc.forced_first = prm->forced_first != 0;
+    rc.alpha2 = nullptr;
     if (prm->cloud_phase != 0 && prm->cloud_phase != 1) return fail(g, GCMCRT_E_INVALID, "cloud_phase must be 0 (HG) or 1 (TTHG)");
     rc.roulette_w_min = float(prm->roulette_w_min); rc.roulette_survive = float(prm->roulette_survive);
     rc.surface_albedo = g->surface_albedo;
@@ -381,7 +389,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     // ---- launch geometry: persistent grids sized to the device
     const size_t smem_t = size_t(g->tab_floats) * sizeof(float);
     int occ_t = 0, occ_p = 0;
-    auto tk = transport_kernel<4>;
+    const bool cont = prm->continuous_absorption != 0;
+    auto tk = cont ? transport_kernel<4, true> : transport_kernel<4, false>;
     auto pk = peel_kernel<8>;
     CUDA_TRY(g, cudaFuncSetAttribute(tk, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_t)));
     CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_t, tk, kTransportThreads, smem_t));
@@ -413,16 +422,17 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         // ---- A0/A1: make sure the staged table is the one this run needs
         if (prm->doppler_on && n_obs > 0) {
             const double* od = prm->obs_dir + 3 * run;
-            const bool same = g->staged_obs >= 0 && g->staged_halfwidth == prm->doppler_halfwidth &&
+            const bool same = g->staged_obs >= 0 && g->staged_cont == cont && g->staged_halfwidth == prm->doppler_halfwidth &&
                               g->staged_dir[0] == od[0] && g->staged_dir[1] == od[1] && g->staged_dir[2] == od[2];
-            if (!same && (rcode = stage_opacity(g, od, prm->doppler_halfwidth, s))) return rcode;
+            if (!same && (rcode = stage_opacity(g, od, prm->doppler_halfwidth, s, cont))) return rcode;
             rc.obs_first = run; rc.n_obs_run = 1;
         } else {
-            if (g->staged_obs != -1 && (rcode = stage_opacity(g, nullptr, 0, s))) return rcode;
+            if ((g->staged_obs != -1 || g->staged_cont != cont) && (rcode = stage_opacity(g, nullptr, 0, s, cont))) return rcode;
             rc.obs_first = 0; rc.n_obs_run = n_obs;
         }
         rc.magic_nobs = magic_div((unsigned long long)std::max(rc.n_obs_run, 1));
         rc.alpha = g->alpha.as<float>();
+        rc.alpha2 = cont ? g->alpha2.as<float>() : nullptr;
         rc.prop = g->prop.as<float4>();
         // ---- A2: emission CDF
         if (emission) {
@@ -532,7 +542,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             sp.nlev = g->nlev; sp.nlat = g->nlat; sp.ncell = g->ncell;
         }
         // ---- wavefront kernels (wavefront.cuh): launch geometry and the launch-order sort of albedo runs
-        const int n_gen = g->tune[2];
+        // continuous absorption runs through the persistent kernel only (its march carries the second extinction)
+        const int n_gen = cont ? 0 : g->tune[2];
         auto k_keys = wave_launch_keys_kernel;
         auto k_first = rc.forced_first ? wave_first_flight_kernel<8, true> : wave_first_flight_kernel<8, false>;
         auto k_emit = wave_emit_kernel;
@@ -908,7 +919,7 @@ int gcmcrt_destroy(gcmcrt_grid* g)
     cudaDeviceSynchronize();
     cudaGetLastError();
     for (DevBuf* b : {&g->tab, &g->r64, &g->cth64, &g->ph64, &g->rc32, &g->thc32, &g->phc32, &g->T, &g->rho, &g->u, &g->v,
-                      &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->prop, &g->reff, &g->vlos, &g->node, &g->node_idx, &g->node_w, &g->own_pcell,
+                      &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->alpha2, &g->prop, &g->reff, &g->vlos, &g->node, &g->node_idx, &g->node_w, &g->own_pcell,
                       &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->guide, &g->ev0, &g->evkeys, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
                       &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->flux, &g->ltot_out,
                       &g->value, &g->sigma, &g->image, &g->evcount, &g->contrib})

@@ -100,6 +100,7 @@ struct RunConst {
     int survival_bias;             // Sect. 4.4: forced scattering with W <- W omega
     float roulette_w_min, roulette_survive;   // Sect. 4.5: Russian roulette below the weight threshold (0 = off)
     int cloud_phase;               // 0 HG (Eq. 7-8), 1 two-term HG (Eq. 10, g1 = g, g2 = -g/2, alpha = 1 - g2^2)
+    const float* alpha2;           // continuous absorption: [n_chan][ncol][col_stride] pairs (alpha_sca, alpha_abs), or NULL
     int forced_first;              // albedo: forced first scattering (Sect. 4.2)
     float surface_albedo;
     double xi;
@@ -133,6 +134,7 @@ struct StageParams {
     int n_chan, ncell, nlev, nlat, nlon;
     const float *k_abs, *k_ray, *k_cld, *g_cld, *rho;
     float* alpha;          // [n_chan][ncol][col_stride], zero-filled by the host before the launch (guard entries)
+    float* alpha2;         // continuous absorption: the same layout with (alpha_sca, alpha_abs) pairs, or NULL
     long long alpha_stride;
     int col_stride;
     float4* prop;
@@ -244,8 +246,15 @@ __global__ void __launch_bounds__(256) stage_kernel(const StageParams p)
             const float ks = kr[q] + kc[q];
             const float kext = ka[q] + ks;
             // guard-padded column layout of the marcher: [chan][col][col_stride], level i at offset 1 + i
-            p.alpha[(size_t)c * p.alpha_stride + (size_t)col * p.col_stride + 1 + i] = rho * kext;
-            p.prop[t] = make_float4(kext > 0.0f ? ks / kext : 0.0f, ks > 0.0f ? kr[q] / ks : 0.0f, gg[q], ka[q]);
+            const size_t at = (size_t)c * p.alpha_stride + (size_t)col * p.col_stride + 1 + i;
+            p.alpha[at] = rho * kext;
+            float omega = kext > 0.0f ? ks / kext : 0.0f;
+            if (p.alpha2) {   // continuous absorption (Eq. 12): flights march (alpha_sca, alpha_abs); every interaction drawn
+                              // from alpha_sca is a scattering, which the event code reads as omega = 1
+                reinterpret_cast<float2*>(p.alpha2)[at] = make_float2(rho * ks, rho * ka[q]);
+                omega = ks > 0.0f ? 1.0f : 0.0f;
+            }
+            p.prop[t] = make_float4(omega, ks > 0.0f ? kr[q] / ks : 0.0f, gg[q], ka[q]);
         }
     }
 }
@@ -504,6 +513,7 @@ enum LaneState : int {
 struct Packet {
     Ray ray;
     float tau, tau_t, W;
+    float tau_b;   // DUAL: absorption optical depth of the flight in progress (Eq. 12)
     uint32_t chan_run, pkt, m_inter, nev;
     int fl_seg;
 };
@@ -518,7 +528,10 @@ __device__ __forceinline__ void finish_packet(const RunConst& rc, const Packet& 
     if (rc.event_count) rc.event_count[(size_t)pk.chan_run * rc.n_pkt + (pk.pkt - rc.pkt_begin)] = pk.nev;
 }
 
-template <int KSTEPS>
+// DUAL: continuous absorption (Sect. 4.1, Eq. 12): flights march the (alpha_sca, alpha_abs) pair table rc.alpha2, the
+// sampled optical depth is spent on alpha_sca and the weight decays by e^-tau_abs at the end of every flight; the staged
+// prop records then carry omega = 1, so that the event code below (and the peel kernel) needs no other change.
+template <int KSTEPS, bool DUAL>
 __global__ void __launch_bounds__(kTransportThreads, 2)
 transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const SuspBuf susp_in, const SuspBuf susp_out,
                  const unsigned long long total_items)
@@ -528,10 +541,13 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
     __syncthreads();
 
     Packet pk;
-    pk.tau = 0.f; pk.tau_t = 0.f; pk.W = 0.f; pk.chan_run = 0; pk.pkt = 0; pk.m_inter = 0; pk.nev = 0; pk.fl_seg = 0;
+    pk.tau = 0.f; pk.tau_t = 0.f; pk.tau_b = 0.f; pk.W = 0.f; pk.chan_run = 0; pk.pkt = 0; pk.m_inter = 0; pk.nev = 0; pk.fl_seg = 0;
     pk.ray = Ray{};
     int st = LS_IDLE;
-    const float* alpha_c = rc.alpha;  // table of this lane's channel
+    auto chan_table = [&](int ctab) {
+        return DUAL ? rc.alpha2 + (size_t)ctab * rc.geom.alpha_stride * 2 : rc.alpha + (size_t)ctab * rc.geom.alpha_stride;
+    };
+    const float* alpha_c = chan_table(0);  // table of this lane's channel
     unsigned long long c_events = 0, c_seg = 0, c_esc = 0, c_abs = 0, c_surf = 0, c_stuck = 0;
     unsigned int c_seg32 = 0;
     double c_escw = 0.0;
@@ -583,7 +599,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                         pk.ray.pcx = a.x; pk.ray.pcy = a.y; pk.ray.pcz = a.z; pk.ray.u = 0.f;
                         pk.ray.nx = b.x; pk.ray.ny = b.y; pk.ray.nz = b.z;
                         pk.ray.i = i; pk.ray.j = j; pk.ray.k = k;
-                        alpha_c = rc.alpha + (size_t)(rc.chan_begin + pk.chan_run) * rc.geom.alpha_stride;
+                        alpha_c = chan_table(rc.chan_begin + int(pk.chan_run));
                         const uint32_t kind = c.w >> 28;
                         st = kind == EV_MEDIUM ? LS_EV_MEDIUM : (kind == EV_EMIT ? LS_EV_EMIT : LS_EV_SURFACE);
                         need = false;
@@ -606,7 +622,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                 pk.pkt = rc.pkt_begin + uint32_t(item - (unsigned long long)pk.chan_run * rc.n_pkt);
                                 pk.m_inter = 0; pk.nev = 0;
                                 const int ctab = rc.chan_begin + int(pk.chan_run);
-                                alpha_c = rc.alpha + (size_t)ctab * rc.geom.alpha_stride;
+                                alpha_c = chan_table(ctab);
                                 const uint32_t ckey = rc.chan_key0 + uint32_t(ctab);
                                 const Zeta4 z = zeta_block(rc.seed, ckey, pk.pkt, 0, 0);
                                 if (rc.mode == 0) {
@@ -624,7 +640,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                     pk.W = 1.0f;
                                     pk.tau_t = -logf(z.z2);
                                     pk.tau = 0.f; pk.fl_seg = 0;
-                                    ray_init(pk.ray, gs, px, py, pz, -rc.star[0], -rc.star[1], -rc.star[2], gs.nlev - 1,
+                                    ray_init<DUAL>(pk.ray, gs, px, py, pz, -rc.star[0], -rc.star[1], -rc.star[2], gs.nlev - 1,
                                              j, k, alpha_c);
                                     st = LS_FLY;
                                 } else {
@@ -730,7 +746,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                 float nx = pk.ray.nx, ny = pk.ray.ny, nz = pk.ray.nz;
                                 rotate_dir(nx, ny, nz, ct, z.z2);
                                 pk.tau_t = -logf(z.z3); pk.tau = 0.f; pk.fl_seg = 0;
-                                ray_init(pk.ray, gs, px, py, pz, nx, ny, nz, pk.ray.i, pk.ray.j, pk.ray.k, alpha_c);
+                                ray_init<DUAL>(pk.ray, gs, px, py, pz, nx, ny, nz, pk.ray.i, pk.ray.j, pk.ray.k, alpha_c);
                                 st = LS_FLY;
                             }
                         } else if (st == LS_EV_EMIT) {
@@ -747,7 +763,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                 float sp, cp;
                                 sincospif(2.0f * z.z1, &sp, &cp);
                                 pk.tau_t = -logf(z.z2); pk.tau = 0.f; pk.fl_seg = 0;
-                                ray_init(pk.ray, gs, px, py, pz, ns * cp, ns * sp, nz, pk.ray.i, pk.ray.j, pk.ray.k, alpha_c);
+                                ray_init<DUAL>(pk.ray, gs, px, py, pz, ns * cp, ns * sp, nz, pk.ray.i, pk.ray.j, pk.ray.k, alpha_c);
                                 st = LS_FLY;
                             }
                         } else {  // Lambert surface (O7, Eq. 3-4)
@@ -767,7 +783,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                             } else {
                                 rotate_dir(hx, hy, hz, sqrtf(z.z1), z.z2);      // Eq. 4 about the normal
                                 pk.tau_t = -logf(z.z3); pk.tau = 0.f; pk.fl_seg = 0;
-                                ray_init(pk.ray, gs, px, py, pz, hx, hy, hz, 0, pk.ray.j, pk.ray.k, alpha_c);
+                                ray_init<DUAL>(pk.ray, gs, px, py, pz, hx, hy, hz, 0, pk.ray.j, pk.ray.k, alpha_c);
                                 st = LS_FLY;
                             }
                         }
@@ -778,7 +794,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
         // ---------------- lateral crossings: cone / half-plane root updates, batched across the warp ----------------
         if (m_park && (__popc(m_park) >= rc.t_lateral || starving)) {
             if (st == LS_PARK) {
-                ray_lateral(pk.ray, gs, alpha_c);
+                ray_lateral<DUAL>(pk.ray, gs, alpha_c);
                 st = LS_FLY;
             }
         }
@@ -790,8 +806,12 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
 #pragma unroll
         for (int s = 0; s < KSTEPS; ++s) {
             if (st == LS_FLY) {
-                const int rs = ray_step(pk.ray, gs, pk.tau, pk.tau_t);
+                const int rs = ray_step<DUAL>(pk.ray, gs, pk.tau, pk.tau_t, &pk.tau_b);
                 ++c_seg32;
+                if (DUAL && rs != RAY_FLYING && rs != RAY_PARK) {   // the flight is over: Eq. 12
+                    pk.W *= expf(-pk.tau_b);
+                    pk.tau_b = 0.f;
+                }
                 if (rs == RAY_FLYING) {
                     if (++pk.fl_seg > rc.geom.maxseg) st = LS_END_STUCK;
                 } else if (rs == RAY_PARK) {

@@ -74,6 +74,7 @@ struct Ray {
     float u_rad, u_lat, u_lon;  // next crossing of each face family
     float alpha;          // extinction of the current cell
     float alpha_n;        // prefetched extinction of the radial neighbour (i + rad_step) in the same column
+    float beta, beta_n;   // DUAL marches only (continuous absorption, Eq. 12): the second extinction of the same cells
     const float* pn;      // address of the extinction prefetched next, in the column of (j, k): column + i + rad_step
                           // (every column has a guard entry below level 0 and above level nlev - 1)
     int i, j, k;          // cell
@@ -182,22 +183,33 @@ __device__ __forceinline__ void ray_setup_lon(Ray& r, const GeomSmem& s)
 }
 
 // Column pointer of (j, k) in the staged extinction table of one channel (alpha_tab points at that channel).
+// DUAL: the table holds pairs (alpha, beta) per cell -- same layout, two floats per entry.
+template <bool DUAL = false>
 __device__ __forceinline__ const float* ray_column(const GeomSmem& s, const float* __restrict__ alpha_tab, int j, int k)
 {
-    return alpha_tab + (size_t)(k * s.nlat + j) * s.col_stride + 1;
+    return alpha_tab + ((size_t)(k * s.nlat + j) * s.col_stride + 1) * (DUAL ? 2 : 1);
 }
 
 // Extinction of the current cell and, one step ahead, of the radial neighbour the ray will enter next: the march
 // loop consumes alpha one iteration after the load was issued, so the gather latency overlaps a full step.
+template <bool DUAL = false>
 __device__ __forceinline__ void ray_load_alpha(Ray& r, const GeomSmem& s, const float* __restrict__ alpha_tab)
 {
-    const float* colp = ray_column(s, alpha_tab, r.j, r.k);
-    r.alpha = __ldg(colp + r.i);
-    r.pn = colp + (r.i + r.rad_step);
-    r.alpha_n = __ldg(r.pn);
+    const float* colp = ray_column<DUAL>(s, alpha_tab, r.j, r.k);
+    if (DUAL) {
+        const float2 a = __ldg(reinterpret_cast<const float2*>(colp) + r.i);
+        r.pn = colp + 2 * (r.i + r.rad_step);
+        const float2 an = __ldg(reinterpret_cast<const float2*>(r.pn));
+        r.alpha = a.x; r.beta = a.y; r.alpha_n = an.x; r.beta_n = an.y;
+    } else {
+        r.alpha = __ldg(colp + r.i);
+        r.pn = colp + (r.i + r.rad_step);
+        r.alpha_n = __ldg(r.pn);
+    }
 }
 
 // Start a ray at p with unit direction n inside cell (i,j,k).
+template <bool DUAL = false>
 __device__ __forceinline__ void ray_init(Ray& r, const GeomSmem& s, float px, float py, float pz, float nx, float ny,
                                          float nz, int i, int j, int k, const float* __restrict__ alpha_tab)
 {
@@ -219,7 +231,7 @@ __device__ __forceinline__ void ray_init(Ray& r, const GeomSmem& s, float px, fl
     ray_setup_rad(r, s);
     ray_setup_lat(r, s);
     ray_setup_lon(r, s);
-    ray_load_alpha(r, s, alpha_tab);
+    ray_load_alpha<DUAL>(r, s, alpha_tab);
 }
 
 // One step of the march, radial fast path.  tau accumulates over the segment up to the next face.  A shell crossing
@@ -227,30 +239,40 @@ __device__ __forceinline__ void ray_init(Ray& r, const GeomSmem& s, float px, fl
 // is a cone or a half-plane the ray is advanced to it and RAY_PARK is returned: the caller completes the crossing
 // with ray_lateral().  Once a ray has crossed a shell outward it stays outward (u > 0), so only a ray still moving
 // inward has to ask whether the next inner shell lies outside its impact parameter.
-__device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, float tau_limit)
+// DUAL (continuous absorption, Eq. 12): tau_b accumulates the second extinction over the same segments.
+template <bool DUAL = false>
+__device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, float tau_limit, float* tau_b = nullptr)
 {
     const float ul = fminf(r.u_lat, r.u_lon);
     const float un = fminf(r.u_rad, ul);
     const float ds = fmaxf(un - r.u, 0.0f);
     const float tnew = fmaf(r.alpha, ds, tau);
     if (tnew >= tau_limit) {  // the limit is reached inside this cell
-        r.u += __fdividef(tau_limit - tau, r.alpha);   // MUFU.RCP + FMUL: the IEEE sequence is 20 instructions, once per flight
-                                                       // at a different step in every lane
+        const float dl = __fdividef(tau_limit - tau, r.alpha);   // MUFU.RCP + FMUL: the IEEE sequence is 20 instructions, once
+        r.u += dl;                                               // per flight at a different step in every lane
+        if (DUAL) *tau_b = fmaf(r.beta, dl, *tau_b);
         tau = tau_limit;
         return RAY_LIMIT;
     }
     tau = tnew;
+    if (DUAL) *tau_b = fmaf(r.beta, ds, *tau_b);
     r.u = fmaxf(un, r.u);
     if (r.u_rad > ul) return RAY_PARK;  // ties: shells first (C1)
     r.i += r.rad_step;
     if ((unsigned)r.i >= (unsigned)s.nlev) return r.i < 0 ? RAY_SURFACE : RAY_ESCAPE;   // r.i is left outside the grid
     r.alpha = r.alpha_n;   // prefetched for exactly this cell
+    if (DUAL) r.beta = r.beta_n;
     if (r.i == r.i_turn) r.rad_step = 1;   // the inner shell of this cell lies inside the impact parameter
     else r.ish += r.rad_step;              // (turning, the shell just crossed inward is the next one outward)
     const float sq = sqrt_approx(fmaxf(shell_q(r, s, r.ish), 0.0f));
     r.u_rad = __int_as_float(__float_as_int(sq) | (r.rad_step & 0x80000000));
-    r.pn += r.rad_step;   // also right at the turn: the prefetch pointed at this cell, the next one is one up
-    r.alpha_n = __ldg(r.pn);
+    r.pn += DUAL ? 2 * r.rad_step : r.rad_step;   // also right at the turn: the prefetch pointed at this cell, the next one is one up
+    if (DUAL) {
+        const float2 an = __ldg(reinterpret_cast<const float2*>(r.pn));
+        r.alpha_n = an.x; r.beta_n = an.y;
+    } else {
+        r.alpha_n = __ldg(r.pn);
+    }
     return RAY_FLYING;
 }
 
@@ -360,6 +382,7 @@ __device__ __forceinline__ int ray_run(Ray& r, const GeomSmem& s, float& tau_io,
 }
 
 // Completes the cone / half-plane crossing of a parked ray (ties: cones before planes, C1).
+template <bool DUAL = false>
 __device__ __forceinline__ void ray_lateral(Ray& r, const GeomSmem& s, const float* __restrict__ alpha_tab)
 {
     if (r.u_lat <= r.u_lon) {
@@ -376,7 +399,7 @@ __device__ __forceinline__ void ray_lateral(Ray& r, const GeomSmem& s, const flo
         r.u_lon = best;
         r.lon_step = step == 0 ? r.lon_step : step;
     }
-    ray_load_alpha(r, s, alpha_tab);
+    ray_load_alpha<DUAL>(r, s, alpha_tab);
 }
 
 __device__ __forceinline__ void ray_position(const Ray& r, float& px, float& py, float& pz)

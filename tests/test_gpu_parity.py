@@ -363,6 +363,41 @@ def test_forced_first_scattering_parity(gpu, orc, monkeypatch):
         assert e.value.code == gpu.E_INVALID
 
 
+def test_continuous_absorption_parity(gpu, orc):
+    """Sect. 4.1, Eq. 12 on the GPU (pair table (alpha_sca, alpha_abs) marched by the persistent kernel, omega = 1 in
+    the staged records) against the oracle: same streams, same flights, same weights -- 3D albedo run with Russian
+    roulette, 1D run cut at max_events, emission with scattering; the escaped-weight budget agrees; the analog run of
+    the same problem agrees within the errors; a later analog run on the same handle restages the analog tables."""
+    grid, opac, prm = wl.cfg2(nlon=16, nlat=8, nlev=20, nbands=2, ng=3, packets=20000)
+    prm = dict(prm, continuous_absorption=1, survival_bias=1, roulette_w_min=0.05, roulette_survive=0.25)
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        ana = G.run_albedo(dict(prm, continuous_absorption=0, survival_bias=0, roulette_w_min=0.0), want_event_count=True)
+        g = G.run_albedo(prm, want_event_count=True)
+        ana2 = G.run_albedo(dict(prm, continuous_absorption=0, survival_bias=0, roulette_w_min=0.0), want_event_count=True)
+    o = orc.run_albedo(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
+    _check_parity(orc, g, o, "albedo")
+    assert abs(g["counters"]["escaped_weight"] - o["counters"]["escaped_weight"]) < 1e-3 * o["counters"]["escaped_weight"]
+    assert np.array_equal(ana["event_count"], ana2["event_count"]) and np.allclose(ana["value"], ana2["value"], rtol=1e-6)
+    assert np.all(np.abs(g["value"] - ana["value"]) < 4 * np.hypot(g["sigma"], ana["sigma"]) + 1e-5 * ana["value"])
+    assert g["counters"]["events"] > ana["counters"]["events"]
+    grid, opac, prm = wl.cfg1(packets=20000)
+    prm = dict(prm, continuous_absorption=1, max_events=25)
+    g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+    o = orc.run_albedo(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
+    _check_parity(orc, g, o, "albedo")
+    grid, opac, prm = wl.cfg3(nlon=12, nlat=6, nlev=16, nbands=2, ng=2, packets=20000, n_obs=3)
+    prm = dict(prm, continuous_absorption=1, max_events=12)
+    g = _gpu_run(gpu, grid, opac, prm, "emission", want_event_count=True)
+    o = orc.run_emission(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
+    _check_parity(orc, g, o, "emission")
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        with pytest.raises(gpu.GcmcrtError) as e:
+            G.run_albedo(dict(prm, forced_first=1))
+        assert e.value.code == gpu.E_INVALID
+
+
 def test_tthg_cloud_phase_function_parity(gpu, orc):
     """Eq. 10 (two-term HG, g1 = g, g2 = -g/2, alpha = 1 - g2^2) in the sampler and in the peel-off density."""
     grid, opac, prm = wl.cfg2(nlon=16, nlat=8, nlev=20, nbands=2, ng=3, packets=20000)

@@ -391,7 +391,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     int occ_t = 0, occ_p = 0;
     const bool cont = prm->continuous_absorption != 0;
     auto tk = cont ? transport_kernel<4, true> : transport_kernel<4, false>;
-    auto pk = peel_kernel<8>;
+    auto pk = peel_kernel<16>;
     CUDA_TRY(g, cudaFuncSetAttribute(tk, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_t)));
     CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_t, tk, kTransportThreads, smem_t));
     if (occ_t < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
@@ -545,7 +545,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         // continuous absorption runs through the persistent kernel only (its march carries the second extinction)
         const int n_gen = cont ? 0 : g->tune[2];
         auto k_keys = wave_launch_keys_kernel;
-        auto k_first = rc.forced_first ? wave_first_flight_kernel<8, true> : wave_first_flight_kernel<8, false>;
+        auto k_first = rc.forced_first ? wave_first_flight_kernel<16, true> : wave_first_flight_kernel<16, false>;
         auto k_emit = wave_emit_kernel;
         auto k_inter = wave_interact_kernel<kInteractK>;
         const size_t smem_w = smem_t;

@@ -41,11 +41,22 @@ __global__ void __launch_bounds__(256) ev_hist_kernel(const SortParams p)
         atomicAdd(p.hist + __ldg(p.keys + e), 1u);
 }
 
+// Consecutive records were written by one warp of neighbouring packets and often share their (channel, cell) key:
+// the lanes of a warp that hold the same key take their slots with one atomic (any order inside a bin is valid).
 __global__ void __launch_bounds__(256) ev_scatter_kernel(const SortParams p)
 {
     const unsigned int n = p.count ? min(*p.count, p.cap) : p.n_host;
-    for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x)
-        p.perm[atomicAdd(p.hist + __ldg(p.keys + e), 1u)] = e;
+    const unsigned int n_round = (n + 31u) & ~31u;
+    for (unsigned int e = blockIdx.x * blockDim.x + threadIdx.x; e < n_round; e += gridDim.x * blockDim.x) {
+        const bool valid = e < n;
+        const unsigned int key = valid ? __ldg(p.keys + e) : 0xffffffffu - lane_id();
+        const unsigned int peers = __match_any_sync(kFullMask, key);
+        const int leader = __ffs(peers) - 1;
+        unsigned int base = 0;
+        if (valid && lane_id() == leader) base = atomicAdd(p.hist + key, (unsigned int)__popc(peers));
+        base = __shfl_sync(kFullMask, base, leader);
+        if (valid) p.perm[base + __popc(peers & ((1u << lane_id()) - 1u))] = e;
+    }
 }
 
 __device__ __forceinline__ unsigned int block_sum_u32(unsigned int v, unsigned int* warp_part)

@@ -528,8 +528,14 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             // channels whose events can share one pass: every packet makes at least one event when it interacts,
             // so a pass of ev_cap events spans about ev_cap / n_pkt channels; more bins than that only cost scan time
             const long long span = (long long)(g->ev_cap / std::max<size_t>(n_pkt, 1)) + 2;
-            sp.c_fold = int(std::max<long long>(1, std::min<long long>(std::min<long long>(ncr, max_bins / g->ncell), span)));
-            sp.nbins = (unsigned int)((long long)sp.c_fold * g->ncell);
+            // few packets per channel (high-resolution runs: 1e5 packets over 1e5-1e6 cells): sort by (channel, column)
+            // instead of (channel, cell) -- rays from one column toward one observer still share their extinction
+            // sectors, the histogram is nlev times smaller and every channel of the pass keeps bins of its own
+            const int coarse = n_pkt < 2ull * (unsigned long long)g->ncell;
+            const long long bins_per_chan = coarse ? (long long)g->nlat * g->nlon : (long long)g->ncell;
+            sp.c_fold = int(std::max<long long>(1, std::min<long long>(std::min<long long>(ncr, max_bins / bins_per_chan), span)));
+            sp.nbins = (unsigned int)((long long)sp.c_fold * bins_per_chan);
+            ev.coarse = coarse; ev.bins_per_chan = int(bins_per_chan);
             sp.n_tiles = (sp.nbins + kScanTile - 1) / kScanTile;
             CUDA_TRY(g, g->hist.ensure(size_t(sp.nbins) * sizeof(unsigned int)));
             CUDA_TRY(g, g->tile_sums.ensure(size_t(sp.n_tiles) * sizeof(unsigned int)));

@@ -45,6 +45,7 @@ struct EventBuf {
                           // instead (emission: events pile up in a few bright cells and the contended atomics are
                           // cheaper in a kernel of their own than inside the emit / interact kernels)
     int chan_lo, c_fold, nlev, nlat, ncell;
+    int coarse, bins_per_chan;   // coarse: the key's second part is the column (k * nlat + j) instead of the cell
 };
 
 __device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slot, float px, float py, float pz, float W,
@@ -59,7 +60,8 @@ __device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slo
     if (ev.keys) {
         const int i = cellp & 1023, j = (cellp >> 10) & 1023, k = cellp >> 20;
         const unsigned int chan = (unsigned int)min(max(int(meta >> 8) - ev.chan_lo, 0), ev.c_fold - 1);
-        const unsigned int key = chan * (unsigned int)ev.ncell + (unsigned int)((k * ev.nlat + j) * ev.nlev + i);
+        const unsigned int col = (unsigned int)(k * ev.nlat + j);
+        const unsigned int key = chan * (unsigned int)ev.bins_per_chan + (ev.coarse ? col : col * (unsigned int)ev.nlev + (unsigned int)i);
         ev.keys[slot] = key;
         if (ev.hist) atomicAdd(ev.hist + key, 1u);
     }

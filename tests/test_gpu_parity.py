@@ -642,6 +642,47 @@ def test_opacity_from_node_tables_matches_per_cell_tables(gpu, orc):
     assert np.allclose(val, node["value"], rtol=1e-6)
 
 
+def test_degenerate_cases_match_oracle(gpu, orc):
+    """The degenerate cases the method has, each against the oracle: a single packet; packet counts that fill neither a
+    warp nor the batches (N = 33 < n_batches = 64); a one-cell grid; a vacuum (no extinction: no event, every packet
+    leaves or lands); a fully opaque absorber; max_events = 1; a run of one channel out of the middle of a table."""
+    # one cell, single scattering, 1 and 33 packets
+    grid, opac = wl.uniform_medium(1, 1, 1, 1.0e6, 2.0e6, 1.5e-6, 0.7, g=0.5, pgas=0.5)
+    for N, nb in ((1, 1), (33, 64), (1000, 32)):
+        prm = wl.default_params(packets_per_channel=N, seed=3, n_batches=nb, max_events=1,
+                                star_dir=[1.0, 0.0, 0.0], obs_dir=np.array([[0.5, 0.5, np.sqrt(0.5)]]))
+        g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+        o = orc.run_albedo(grid, opac, prm, want_event_count=True)
+        assert np.array_equal(g["event_count"], o["event_count"])
+        assert np.allclose(g["flux_sum"], o["flux_sum"], rtol=2e-4, atol=1e-12)
+        assert g["counters"]["events"] == o["counters"]["events"] <= N
+    # vacuum over an absorbing and over a reflecting lower boundary
+    for a_surf in (0.0, 1.0):
+        grid, opac = wl.uniform_medium(5, 4, 6, 1.0e6, 1.5e6, 0.0, 0.0, surface_albedo=a_surf)
+        prm = wl.default_params(packets_per_channel=5000, seed=4, star_dir=[0.0, 0.6, 0.8], obs_dir=np.array([[0.0, 0.6, 0.8]]))
+        g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+        o = orc.run_albedo(grid, opac, prm, want_event_count=True)
+        _check_parity(orc, g, o, "albedo")
+        cg = g["counters"]
+        if a_surf == 0.0:
+            assert cg["events"] == 0 and np.all(g["flux_sum"] == 0) and cg["packets_escaped"] + cg["packets_surface"] == 5000
+        else:
+            assert cg["packets_escaped"] == 5000 and cg["events"] == o["counters"]["events"] > 0
+    # opaque pure absorber: every packet is absorbed in the top cell, one (dark) event each
+    grid, opac = wl.uniform_medium(3, 2, 2, 1.0e6, 1.5e6, 1.0, 0.0)
+    prm = wl.default_params(packets_per_channel=2000, seed=5, obs_dir=np.array([[1.0, 0.0, 0.0]]))
+    g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+    assert g["counters"]["packets_absorbed"] == 2000 and np.all(g["event_count"] == 1) and np.all(g["flux_sum"] == 0)
+    # one channel out of the middle of a table
+    grid, opac, prm = wl.cfg2(nlon=8, nlat=4, nlev=10, nbands=2, ng=3, packets=3000)
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        allc = G.run_albedo(prm, want_event_count=True)
+        one = G.run_albedo(dict(prm, chan_begin=4, chan_end=5), want_event_count=True)
+    assert np.array_equal(one["event_count"][0], allc["event_count"][4])
+    assert np.allclose(one["flux_sum"][0], allc["flux_sum"][4], rtol=1e-6)
+
+
 def test_error_paths(gpu):
     grid, opac, prm = wl.cfg1(packets=100)
     with gpu.Grid(grid) as G:

@@ -215,7 +215,9 @@ def hires_opacity(grid, rng, n_chan=10000, lam0=2.19e-6, R=1.0e5, n_lines=500, n
     node = np.empty((n_chan, nT, nP), dtype=np.float64)
     for a, Tv in enumerate(Tn):
         sig = nu_c * np.sqrt(K_B * Tv / mass) / 299792458.0
-        boltz = np.exp(-c2 * E * (1.0 / Tv - 1.0 / 296.0)) * (296.0 / Tv)
+        # line strengths are quoted at T_ref = 1500 K, the middle of the grid's temperature range (quoted at 296 K the
+        # Boltzmann factor of a 5000 cm^-1 level is e^22 at 3000 K and every channel is opaque in the top cell)
+        boltz = np.exp(-c2 * E * (1.0 / Tv - 1.0 / 1500.0)) * (1500.0 / Tv)
         for b, lp in enumerate(lpn):
             gam = 0.07 * (10.0 ** lp / 101325.0) * (Tv / 296.0) ** -0.5
             acc = np.zeros(n_chan)

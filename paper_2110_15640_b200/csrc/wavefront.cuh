@@ -223,6 +223,7 @@ __device__ __forceinline__ void flight_load(const float* fl, const RunConst& rc,
 }
 
 // O3: uniform point on the star-facing TOA disc from Philox block (event 0, purpose 0), and its entry column
+template <bool LOCATE = true>
 __device__ __forceinline__ void albedo_launch_point(const RunConst& rc, const GeomSmem& gs, const Zeta4& z, float& px,
                                                     float& py, float& pz, int& j, int& k)
 {
@@ -234,7 +235,7 @@ __device__ __forceinline__ void albedo_launch_point(const RunConst& rc, const Ge
     px = ax * rc.e1[0] + ay * rc.e2[0] + h * rc.star[0];
     py = ax * rc.e1[1] + ay * rc.e2[1] + h * rc.star[1];
     pz = ax * rc.e1[2] + ay * rc.e2[2] + h * rc.star[2];
-    locate_angles(gs, px, py, pz, j, k);
+    if (LOCATE) locate_angles(gs, px, py, pz, j, k);
 }
 
 __device__ __forceinline__ void wave_item(const RunConst& rc, unsigned long long item, uint32_t& chan_run, uint32_t& pkt)
@@ -285,13 +286,16 @@ wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
         float tau_t = 0.f, z2 = 0.f;
         const float* alpha_c = rc.alpha;
         if (active) {
-            wave_item(rc, wc.item0 + __ldg(wc.perm + t), chan_run, pkt);
+            const unsigned int it = __ldg(wc.perm + t);
+            wave_item(rc, wc.item0 + it, chan_run, pkt);
             const int ctab = rc.chan_begin + int(chan_run);
             alpha_c = rc.alpha + (size_t)ctab * rc.geom.alpha_stride;
             const Zeta4 z = zeta_block(rc.seed, rc.chan_key0 + uint32_t(ctab), pkt, 0, 0);
             float px, py, pz;
-            int j, k;
-            albedo_launch_point(rc, gs, z, px, py, pz, j, k);
+            // the entry column was located when the launch key was made: read it back instead of locating again
+            const unsigned int col = (__ldg(wc.keys + it) / kLaunchTauBuckets) % (unsigned int)(gs.nlat * gs.nlon);
+            int j = int(col % (unsigned int)gs.nlat), k = int(col / (unsigned int)gs.nlat);
+            albedo_launch_point<false>(rc, gs, z, px, py, pz, j, k);
             tau_t = -logf(z.z2);
             z2 = z.z2;
             ray_init(ray, gs, px, py, pz, -rc.star[0], -rc.star[1], -rc.star[2], gs.nlev - 1, j, k, alpha_c);

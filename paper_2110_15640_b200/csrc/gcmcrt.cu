@@ -616,15 +616,15 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
                         wc.keys = g->lkeys.as<unsigned int>(); wc.perm = g->lperm.as<unsigned int>();
                         spl.n_host = wc.n_items;
                         const unsigned gk = (unsigned)std::min<unsigned long long>((n_fresh + 255) / 256, (unsigned long long)g->sm_count * 8);
-                        k_keys<<<gk, kWaveThreads, smem_w, s>>>(rc, wc);
                         CUDA_TRY(g, cudaMemsetAsync(spl.hist, 0, size_t(spl.nbins) * sizeof(unsigned int), s));
-                        ev_hist_kernel<<<gk, 256, 0, s>>>(spl);
+                        wc.lhist = spl.hist;   // the launch sort's histogram is counted while the keys are written
+                        k_keys<<<gk, kWaveThreads, smem_w, s>>>(rc, wc);
                         scan_reduce_kernel<<<spl.n_tiles, kScanThreads, 0, s>>>(spl);
                         scan_tiles_kernel<<<1, 1024, 0, s>>>(spl);
                         scan_apply_kernel<<<spl.n_tiles, kScanThreads, 0, s>>>(spl);
                         ev_scatter_kernel<<<gk, 256, 0, s>>>(spl);
                         k_first<<<g->sm_count * occ_f, kWaveThreads, smem_w, s>>>(rc, ev, sin, wc);
-                        g->launches += 7;
+                        g->launches += 6;
                     } else {
                         const unsigned ge = (unsigned)std::min<unsigned long long>((n_fresh + 255) / 256, (unsigned long long)g->sm_count * 8);
                         k_emit<<<ge, kWaveThreads, smem_w, s>>>(rc, ev, sin, wc);

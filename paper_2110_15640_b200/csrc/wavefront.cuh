@@ -30,6 +30,7 @@ struct WaveConst {
     unsigned int n_items;          // fresh packets of this pass
     const unsigned int* perm;      // albedo: launch order, perm[t] in [0, n_items)
     unsigned int* keys;            // albedo: launch sort keys [n_items]
+    unsigned int* lhist;           // albedo: histogram of the launch sort keys, counted by the key kernel
     const unsigned int* gen_mark;  // interact: events [gen_mark[0], gen_mark[1]) form this generation (device)
     int park_all;                  // last generation: survivors' next events go to the suspended list
     int chan_lo, c_fold;           // launch sort key window
@@ -264,7 +265,9 @@ __global__ void __launch_bounds__(kWaveThreads) wave_launch_keys_kernel(const __
         // packets of one column that share a log2(tau) bucket end their first flight within a few cells of each other
         const float lt = __log2f(-__logf(z.z2));                       // log2 of the sampled optical depth, about -23 .. 4
         const int tb = min(max(int(floorf((lt + 8.0f) * (kLaunchTauBuckets / 12.0f))), 0), kLaunchTauBuckets - 1);
-        wc.keys[t] = (unsigned int)((slot * (gs.nlat * gs.nlon) + k * gs.nlat + j) * kLaunchTauBuckets + tb);
+        const unsigned int key = (unsigned int)((slot * (gs.nlat * gs.nlon) + k * gs.nlat + j) * kLaunchTauBuckets + tb);
+        wc.keys[t] = key;
+        atomicAdd(wc.lhist + key, 1u);
     }
 }
 

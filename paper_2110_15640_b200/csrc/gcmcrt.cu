@@ -81,7 +81,8 @@ struct gcmcrt_grid {
 
     // workspace
     DevBuf ev0, evkeys, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, flights, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount, contrib;
-    unsigned int ev_cap = 0;
+    unsigned int ev_cap = 0, ev_cap_forced = 0;
+    bool tuned = false;   // environment overrides read
     int n_threads_resident = 0;
     // GCMCRT_TUNE="service,lateral,gens,batch_div": lanes waiting before the persistent kernel serves them; lanes parked at
     // a cone / half-plane before a warp serves them; wavefront generations per pass before the persistent kernel takes over
@@ -245,21 +246,32 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
     return GCMCRT_OK;
 }
 
-int ensure_workspace(gcmcrt_grid* g)
+// Event buffer capacity: GCMCRT_EVENT_CAP if set (tests force tiny buffers with it); else what the run can use --
+// about 4 events per packet -- between 1 Mi and 128 Mi events (128 Mi x 64 B = 8.6 GB of records plus 13 GB of
+// parked-packet lists and sort arrays: a cfg2 step then takes 4 passes; 64 Mi / 7 passes measured 1.2 % slower).
+// The buffers only ever grow.
+int ensure_workspace(gcmcrt_grid* g, unsigned long long run_packets)
 {
-    if (g->ev_cap == 0) {
-        unsigned long long cap = 64ull << 20;   // 64 Mi events x 48 B = 3 GB: a cfg2 step takes 7 passes
-        if (const char* e = std::getenv("GCMCRT_EVENT_CAP")) cap = std::strtoull(e, nullptr, 10);
-        if (cap < 64) cap = 64;
-        if (cap > (1ull << 30)) cap = 1ull << 30;
-        g->ev_cap = (unsigned int)cap;
-        if (const char* e = std::getenv("GCMCRT_TUNE")) {   // "service,lateral,refill": scheduling thresholds, 1..32
+    if (!g->tuned) {
+        g->tuned = true;
+        if (const char* e = std::getenv("GCMCRT_EVENT_CAP")) {
+            unsigned long long cap = std::strtoull(e, nullptr, 10);
+            g->ev_cap_forced = (unsigned int)std::min<unsigned long long>(std::max<unsigned long long>(cap, 64), 1ull << 30);
+        }
+        if (const char* e = std::getenv("GCMCRT_TUNE")) {   // "service,lateral,generations,batch_div"
             int a = 0, b = 0, c = 0, d = 0;
             const int n = std::sscanf(e, "%d,%d,%d,%d", &a, &b, &c, &d);
             if (n >= 2) { g->tune[0] = std::min(std::max(a, 1), 32); g->tune[1] = std::min(std::max(b, 1), 32); }
             if (n >= 3) g->tune[2] = std::min(std::max(c, 0), kMaxGen);
             if (n >= 4) g->tune[3] = std::min(std::max(d, 1), 64);
         }
+    }
+    if (g->ev_cap_forced) {
+        g->ev_cap = g->ev_cap_forced;
+    } else {
+        unsigned long long want = 1ull << 20;
+        while (want < (128ull << 20) && want < 4 * run_packets) want <<= 1;
+        if (want > g->ev_cap) g->ev_cap = (unsigned int)want;
     }
     CUDA_TRY(g, g->ev0.ensure(size_t(g->ev_cap) * 4 * sizeof(float4)));   // 64-byte records
     CUDA_TRY(g, g->perm.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));
@@ -315,7 +327,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     if (ncr > (1 << 24)) return fail(g, GCMCRT_E_INVALID, "too many channels in one run");
     const int npix = prm->npix > 0 && out->image ? prm->npix : 0;
 
-    int rcode = ensure_workspace(g);
+    int rcode = ensure_workspace(g, (unsigned long long)ncr * (hi - lo));
     if (rcode) return rcode;
     if (prm->forced_first && (g->tune[2] == 0 || prm->continuous_absorption))
         return fail(g, GCMCRT_E_INVALID, "forced_first needs the wavefront transport (GCMCRT_TUNE generations > 0, no continuous_absorption)");

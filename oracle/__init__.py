@@ -63,7 +63,9 @@ def lib():
             getattr(L, name).argtypes = [C.c_double]
         L.orc_sample_tthg.restype = C.c_double
         L.orc_sample_tthg.argtypes = [C.c_double] * 3
-        for name in ("orc_sample_hg", "orc_phase_hg", "orc_phase_tthg", "orc_planck"):
+        L.orc_draine_G.restype = C.c_double
+        L.orc_draine_G.argtypes = [C.c_double]
+        for name in ("orc_sample_hg", "orc_phase_hg", "orc_phase_tthg", "orc_planck", "orc_phase_draine", "orc_sample_draine"):
             getattr(L, name).restype = C.c_double
             getattr(L, name).argtypes = [C.c_double, C.c_double]
         L.orc_cell_volume.restype = C.c_double
@@ -116,6 +118,9 @@ def phase_rayleigh(mu): return lib().orc_phase_rayleigh(mu)
 def phase_hg(g, mu): return lib().orc_phase_hg(g, mu)
 def phase_tthg(g, mu): return lib().orc_phase_tthg(g, mu)
 def sample_tthg(g, zl, z): return lib().orc_sample_tthg(g, zl, z)
+def draine_G(g): return lib().orc_draine_G(g)
+def phase_draine(g, mu): return lib().orc_phase_draine(g, mu)
+def sample_draine(g, z): return lib().orc_sample_draine(g, z)
 def planck(lam, T): return lib().orc_planck(lam, T)
 
 

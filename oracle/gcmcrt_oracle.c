@@ -106,6 +106,56 @@ double orc_sample_tthg(double g, double zeta_lobe, double zeta)
     return zeta_lobe < a ? orc_sample_hg(g, zeta) : orc_sample_hg(g2, zeta);
 }
 
+/* Eq. 9: Draine (2003) phase function, alpha = 0.5 by default (L146).  "G(g) is a function of the
+ * asymmetry parameter g": the first moment of Eq. 9 is <cos> = G (1 + alpha (3 + 2 G^2) / 5) / (1 + alpha (1 + 2 G^2) / 3)
+ * (pinned by quadrature in tests/test_oracle_pins.py); G is the root of <cos>(G) = g in (-1, 1), found by bisection. */
+#define DRAINE_ALPHA 0.5
+static double draine_first_moment(double G, double a)
+{
+    return G * (1.0 + a * (3.0 + 2.0 * G * G) / 5.0) / (1.0 + a * (1.0 + 2.0 * G * G) / 3.0);
+}
+double orc_draine_G(double g)
+{
+    double lo = -1.0, hi = 1.0;
+    for (int it = 0; it < 60; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (draine_first_moment(mid, DRAINE_ALPHA) < g) lo = mid; else hi = mid;
+    }
+    return 0.5 * (lo + hi);
+}
+/* Eq. 9 per steradian (the printed form integrates to 4 pi over the sphere). */
+double orc_phase_draine(double g, double mu)
+{
+    const double a = DRAINE_ALPHA, G = orc_draine_G(g);
+    const double d = 1.0 + G * G - 2.0 * G * mu;
+    return (1.0 - G * G) / (1.0 + a * (1.0 + 2.0 * G * G) / 3.0) * (1.0 + a * mu * mu) / (d * sqrt(d)) / (4.0 * PI);
+}
+/* int_{-1}^{mu} (1 + alpha x^2) (1 + G^2 - 2 G x)^(-3/2) dx, by the substitution t = 1 + G^2 - 2 G x. */
+static double draine_cdf_unnormalised(double G, double a, double mu)
+{
+    if (fabs(G) < 1e-3) return (mu + 1.0) + a * (mu * mu * mu + 1.0) / 3.0;   /* G -> 0: 1 + alpha mu^2 (cf. C8) */
+    const double A = 1.0 + G * G, B = 2.0 * G;
+    const double c0 = 1.0 + a * A * A / (B * B), c1 = 2.0 * a * A / (B * B), c2 = a / (3.0 * B * B);
+    double t = A - B * mu, t0 = A + B;
+    double H = (2.0 / B) * (c0 / sqrt(t) + c1 * sqrt(t) - c2 * t * sqrt(t));
+    double H0 = (2.0 / B) * (c0 / sqrt(t0) + c1 * sqrt(t0) - c2 * t0 * sqrt(t0));
+    return H - H0;
+}
+/* The paper samples Eq. 9 by the Gibbs scheme of Zhang (2019), which it only cites (L146); here the cosine is the
+ * zeta-quantile of Eq. 9 itself (inverse of its closed-form CDF, bisection): the same distribution from one draw,
+ * which keeps the one-block-per-event stream layout (reading N10). */
+double orc_sample_draine(double g, double zeta)
+{
+    const double a = DRAINE_ALPHA, G = orc_draine_G(g);
+    const double total = draine_cdf_unnormalised(G, a, 1.0);
+    double lo = -1.0, hi = 1.0;
+    for (int it = 0; it < 60; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (draine_cdf_unnormalised(G, a, mid) < zeta * total) lo = mid; else hi = mid;
+    }
+    return 0.5 * (lo + hi);
+}
+
 /* C9: rotate n by polar angle acos(ct) and azimuth psi. */
 void orc_rotate(const double n[3], double ct, double psi, double out[3])
 {
@@ -560,7 +610,8 @@ static void peel(const run_ctx *rc, const double p[3], const int ijk[3], int kin
         double pref;
         if (kind == 0) {            /* medium interaction, C6: mixture phase function */
             double mu = dot3(nin, od);
-            double cld = rc->prm->cloud_phase == 1 ? orc_phase_tthg(gg, mu) : orc_phase_hg(gg, mu);
+            double cld = rc->prm->cloud_phase == 1 ? orc_phase_tthg(gg, mu)
+                       : rc->prm->cloud_phase == 2 ? orc_phase_draine(gg, mu) : orc_phase_hg(gg, mu);
             double theta = pgas * orc_phase_rayleigh(mu) + (1.0 - pgas) * cld;
             pref = W * omega * theta;
         } else if (kind == 1) {     /* thermal emission: isotropic, no omega (O4) */
@@ -591,6 +642,7 @@ static void peel(const run_ctx *rc, const double p[3], const int ijk[3], int kin
  * partition (uniform in [0,1) given that the cloud was chosen), so that no extra draw is needed. */
 static double sample_cloud(const orc_params *prm, double gg, double zlobe, double zeta)
 {
+    if (prm->cloud_phase == 2) return orc_sample_draine(gg, zeta);
     return prm->cloud_phase == 1 ? orc_sample_tthg(gg, zlobe, zeta) : orc_sample_hg(gg, zeta);
 }
 

@@ -84,7 +84,7 @@ typedef struct {
     double planet_xy[2];     /* sky-plane position of the planet centre relative to the stellar disc centre, m, in
                                 the observer's image frame (C19: e_x = z^ x o^ normalised, e_y = o^ x e_x) */
     double ld_c1, ld_c2;     /* quadratic limb-darkening law, Eq. 22 */
-    int cloud_phase;         /* cloud scatterers: 0 = HG (Eq. 7-8), 1 = two-term HG (Eq. 10) with the paper's default
+    int cloud_phase;         /* cloud scatterers: 0 = HG (Eq. 7-8), 2 = Draine (Eq. 9, alpha = 0.5), 1 = two-term HG (Eq. 10) with the paper's default
                                 g1 = g, g2 = -g/2, alpha = 1 - g2^2 (L157) */
     int forced_first;        /* albedo: forced first scattering (Sect. 4.2; Cashwell & Everett 1959): the first flight
                                 must end inside the grid: tau_edge = optical depth along the launch ray to where it leaves
@@ -130,6 +130,9 @@ double orc_phase_hg(double g, double mu);
 /* Eq. 10 with g1 = g, g2 = -g/2, alpha = 1 - g2^2 (L157); zeta_lobe < alpha picks the forward lobe (L152) */
 double orc_sample_tthg(double g, double zeta_lobe, double zeta);
 double orc_phase_tthg(double g, double mu);
+double orc_draine_G(double g);                 /* Eq. 9: G with <cos> = g at alpha = 0.5 */
+double orc_phase_draine(double g, double mu);
+double orc_sample_draine(double g, double zeta);
 /* C9: rotate unit vector n by polar angle acos(ct) and azimuth psi. */
 void orc_rotate(const double n[3], double ct, double psi, double out[3]);
 

@@ -960,3 +960,48 @@ def test_continuous_absorption_matches_analog_on_3d_grid_with_less_noise_when_ab
     N = 150000
     fa = ra["counters"]["packets_escaped"] / N
     assert abs(rc["counters"]["escaped_weight"] / N - fa) < 4 * np.sqrt(fa * (1 - fa) / N) + 4 * np.sqrt(fa / N)
+
+
+# ----------------------------------------------------------------------------- Draine phase function (Eq. 9)
+@pytest.mark.parametrize("g", [-0.4, 0.0, 0.05, 0.5, 0.85])
+def test_draine_density_moment_and_sampler(orc, g):
+    """Eq. 9 typed out here from the paper with alpha = 0.5 (L146): the oracle's density equals it with the G that makes
+    the first moment g (the moment by quadrature, not by formula), integrates to 1 over the sphere, and the one-draw
+    sampler returns the quantiles of that density (cumulative quadrature of Eq. 9 itself)."""
+    alpha = 0.5
+    G = orc.draine_G(g)
+    mu = np.linspace(-1, 1, 200001)
+    eq9 = (1 - G * G) / (1 + alpha * (1 + 2 * G * G) / 3) * (1 + alpha * mu ** 2) / (1 + G * G - 2 * G * mu) ** 1.5
+    assert abs(np.trapezoid(eq9, mu) * 2 * PI - 4 * PI) < 1e-6 * 4 * PI           # Eq. 9 as printed integrates to 4 pi
+    assert abs(np.trapezoid(eq9 * mu, mu) / np.trapezoid(eq9, mu) - g) < 1e-7     # G(g): <cos> = g
+    dens = np.array([orc.phase_draine(g, m) for m in mu[::500]])
+    assert np.allclose(dens, eq9[::500] / (4 * PI), rtol=1e-12)
+    cdf = np.concatenate([[0.0], np.cumsum(0.5 * (eq9[1:] + eq9[:-1]) * np.diff(mu))]); cdf /= cdf[-1]
+    for z in (1e-4, 0.03, 0.25, 0.5, 0.77, 0.99, 1 - 1e-5):
+        ct = orc.sample_draine(g, z)
+        assert abs(np.interp(ct, mu, cdf) - z) < 5e-8           # trapezoid error of the reference CDF at g = 0.85
+
+
+def test_draine_limits_and_transport_consistency(orc):
+    """alpha = 1, G = 0 would be Rayleigh and alpha = 0 HG (L144); at the paper's alpha = 0.5 the g = 0 member is
+    (1 + mu^2 / 2) / (1 + 1/6) -- checked in closed form -- and, in a conservative 3D atmosphere, the peeled-off flux
+    integrated over all observer directions equals the escaped weight (density and sampler belong together)."""
+    mu = np.linspace(-1, 1, 11)
+    assert np.allclose([orc.phase_draine(0.0, m) for m in mu], (1 + 0.5 * mu ** 2) / (1 + 0.5 / 3) / (4 * PI), rtol=1e-9)
+    R0, Rt = 1.0e6, 1.3e6
+    grid, opac = wl.uniform_medium(3, 2, 3, R0, Rt, 3.0 / (Rt - R0), 1.0, g=0.6, pgas=0.2, surface_albedo=1.0)
+    nmu, nphi = 6, 8
+    x, w = np.polynomial.legendre.leggauss(nmu)
+    obs = [[np.sqrt(1 - a * a) * np.cos(2 * PI * (q + .5) / nphi), np.sqrt(1 - a * a) * np.sin(2 * PI * (q + .5) / nphi), a]
+           for a in x for q in range(nphi)]
+    wq = np.repeat(w, nphi) * 2 * PI / nphi
+    N = 12000
+    prm = wl.default_params(packets_per_channel=N, seed=18, obs_dir=np.array(obs), star_dir=[0.6, 0.0, 0.8], cloud_phase=2,
+                            n_threads=os.cpu_count() or 1)
+    res = orc.run_albedo(grid, opac, prm)
+    assert res["counters"]["packets_escaped"] == N
+    val, sig = orc.reduce(res, "albedo")
+    total = np.sum(val[0] * wq)
+    assert abs(total - 1.0) < 4 * np.sqrt(np.sum((sig[0] * wq) ** 2)) + 0.02, total
+    hg = orc.reduce(orc.run_albedo(grid, opac, dict(prm, cloud_phase=0)), "albedo")[0]
+    assert not np.allclose(val, hg, rtol=0.02)       # and it is not the HG run

@@ -81,7 +81,9 @@ typedef struct gcmcrt_run_params {
                                     the observer's image frame (e_x = z^ x o^ normalised, e_y = o^ x e_x) */
     double ld_c1, ld_c2;         /* quadratic law I(mu)/I(0) = 1 - c1 (1 - mu) - c2 (1 - mu)^2 (Eq. 22) */
     int cloud_phase;             /* phase function of the cloud scatterers: 0 = Henyey-Greenstein (Eq. 7-8), 1 = two-term
-                                    HG (Eq. 10) with the paper's default g1 = g, g2 = -g/2, alpha = 1 - g2^2 (L157) */
+                                    HG (Eq. 10) with the paper's default g1 = g, g2 = -g/2, alpha = 1 - g2^2 (L157),
+                                    2 = Draine (Eq. 9) with alpha = 0.5 (L146) and G chosen so that <cos> = g_cld; its
+                                    cosine is the zeta-quantile of Eq. 9 (one draw) */
     int forced_first;            /* gcmcrt_run_albedo only: forced first scattering (Sect. 4.2): the optical depth
                                     tau_edge along the launch ray to where it leaves the grid is integrated first, the
                                     flight is drawn as tau = -ln(1 - zeta (1 - e^-tau_edge)) and the packet starts with

@@ -368,7 +368,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.cloud_phase = prm->cloud_phase;
     rc.forced_first = prm->forced_first != 0;
     rc.alpha2 = nullptr;
-    if (prm->cloud_phase != 0 && prm->cloud_phase != 1) return fail(g, GCMCRT_E_INVALID, "cloud_phase must be 0 (HG) or 1 (TTHG)");
+    if (prm->cloud_phase < 0 || prm->cloud_phase > 2) return fail(g, GCMCRT_E_INVALID, "cloud_phase must be 0 (HG), 1 (TTHG) or 2 (Draine)");
     rc.roulette_w_min = float(prm->roulette_w_min); rc.roulette_survive = float(prm->roulette_survive);
     rc.surface_albedo = g->surface_albedo;
     rc.xi = prm->emission_bias;

@@ -101,7 +101,7 @@ struct RunConst {
     int max_events, scatter_on;
     int survival_bias;             // Sect. 4.4: forced scattering with W <- W omega
     float roulette_w_min, roulette_survive;   // Sect. 4.5: Russian roulette below the weight threshold (0 = off)
-    int cloud_phase;               // 0 HG (Eq. 7-8), 1 two-term HG (Eq. 10, g1 = g, g2 = -g/2, alpha = 1 - g2^2)
+    int cloud_phase;               // 0 HG (Eq. 7-8), 1 two-term HG (Eq. 10, g1 = g, g2 = -g/2, alpha = 1 - g2^2), 2 Draine (Eq. 9)
     const float* alpha2;           // continuous absorption: [n_chan][ncol][col_stride] pairs (alpha_sca, alpha_abs), or NULL
     int forced_first;              // albedo: forced first scattering (Sect. 4.2)
     float surface_albedo;
@@ -435,8 +435,51 @@ __device__ __forceinline__ float sample_hg(float g, float z)
 }
 // Cloud scatterer: HG, or the two-term HG of Eq. 10 whose lobe is picked by zlobe (L152), the part of zeta0 left over
 // inside the cloud interval of the partition.
+// Draine (2003) phase function, Eq. 9 with the paper's alpha = 0.5 (L146).  Off the hot path (cloud_phase = 2 only):
+// plain fp64 bisections in functions of their own, so that the kernels that call them keep their registers.
+//   G(g): root of <cos>(G) = G (1 + a (3 + 2 G^2) / 5) / (1 + a (1 + 2 G^2) / 3) = g
+//   cosine = zeta-quantile of Eq. 9 through its closed-form CDF (substitution t = 1 + G^2 - 2 G x); the paper's Gibbs
+//   sampler is only cited, and one draw per event keeps the stream layout (N10)
+__device__ __noinline__ double draine_G(double g)
+{
+    const double a = 0.5;
+    double lo = -1.0, hi = 1.0;
+    for (int it = 0; it < 60; ++it) {
+        const double G = 0.5 * (lo + hi);
+        const double m = G * (1.0 + a * (3.0 + 2.0 * G * G) / 5.0) / (1.0 + a * (1.0 + 2.0 * G * G) / 3.0);
+        if (m < g) lo = G; else hi = G;
+    }
+    return 0.5 * (lo + hi);
+}
+__device__ __forceinline__ double draine_cdf(double G, double a, double mu)
+{
+    if (fabs(G) < 1e-3) return (mu + 1.0) + a * (mu * mu * mu + 1.0) / 3.0;
+    const double A = 1.0 + G * G, B = 2.0 * G, iB2 = 1.0 / (B * B);
+    const double c0 = 1.0 + a * A * A * iB2, c1 = 2.0 * a * A * iB2, c2 = a * iB2 / 3.0;
+    const double t = A - B * mu, t0 = A + B, st = sqrt(t), st0 = sqrt(t0);
+    return (2.0 / B) * ((c0 / st + c1 * st - c2 * t * st) - (c0 / st0 + c1 * st0 - c2 * t0 * st0));
+}
+__device__ __noinline__ float sample_draine(float g, float z)
+{
+    const double a = 0.5, G = draine_G(double(g));
+    const double target = double(z) * draine_cdf(G, a, 1.0);
+    double lo = -1.0, hi = 1.0;
+    for (int it = 0; it < 60; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (draine_cdf(G, a, mid) < target) lo = mid; else hi = mid;
+    }
+    return float(0.5 * (lo + hi));
+}
+__device__ __noinline__ float phase_draine(float g, float mu)
+{
+    const float a = 0.5f, G = float(draine_G(double(g)));
+    const float d = 1.0f + G * G - 2.0f * G * mu;
+    return (1.0f - G * G) / (1.0f + a * (1.0f + 2.0f * G * G) / 3.0f) * (1.0f + a * mu * mu) / (4.0f * kPi * d * sqrtf(d));
+}
+
 __device__ __forceinline__ float sample_cloud(int cloud_phase, float g, float zlobe, float z)
 {
+    if (cloud_phase == 2) return sample_draine(g, z);
     if (cloud_phase == 1) {
         const float g2 = -0.5f * g, a = 1.0f - g2 * g2;
         return sample_hg(zlobe < a ? g : g2, z);
@@ -450,6 +493,7 @@ __device__ __forceinline__ float phase_hg(float g, float mu)
 }
 __device__ __forceinline__ float phase_cloud(int cloud_phase, float g, float mu)
 {
+    if (cloud_phase == 2) return phase_draine(g, mu);
     if (cloud_phase == 1) {
         const float g2 = -0.5f * g, a = 1.0f - g2 * g2;
         return a * phase_hg(g, mu) + (1.0f - a) * phase_hg(g2, mu);

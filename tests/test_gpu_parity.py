@@ -411,6 +411,33 @@ def test_tthg_cloud_phase_function_parity(gpu, orc):
     assert np.any(np.abs(hg["value"] - g["value"]) > 4 * np.hypot(hg["sigma"], g["sigma"]))    # a different function
 
 
+def test_draine_cloud_phase_function_parity(gpu, orc):
+    """Eq. 9 (Draine, alpha = 0.5) as the cloud phase function against the oracle.  Multiple scattering with a Rayleigh
+    admixture over a reflecting boundary: >= 99 % identical event counts pin the sampler (with Henyey-Greenstein's
+    cosines 97 % of the packets keep their count).  Single scattering off cloud particles alone, seen in back-scatter: the peel-off density, which
+    there differs from Henyey-Greenstein's by far more than the Monte Carlo error."""
+    grid, opac = wl.uniform_medium(6, 4, 5, 1.0e6, 1.4e6, 4.0 / 0.4e6, 0.9, g=0.7, pgas=0.3, surface_albedo=0.5)
+    obs = np.array([[1.0, 0.0, 0.0], [0.0, 0.6, 0.8], [-0.6, 0.0, 0.8]])
+    prm = wl.default_params(packets_per_channel=40000, seed=31, star_dir=[1.0, 0.0, 0.0], obs_dir=obs, cloud_phase=2)
+    g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+    o = orc.run_albedo(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
+    _check_parity(orc, g, o, "albedo")
+    hg = _gpu_run(gpu, grid, opac, dict(prm, cloud_phase=0), "albedo", want_event_count=True)
+    assert (hg["event_count"] == g["event_count"]).mean() < 0.98       # HG's sampler would miss the 99 % bar above
+    grid, opac = wl.uniform_medium(6, 4, 5, 1.0e6, 1.4e6, 4.0 / 0.4e6, 0.9, g=0.7, pgas=0.0)
+    prm = dict(prm, max_events=1)
+    g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+    o = orc.run_albedo(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
+    _check_parity(orc, g, o, "albedo")
+    hg = _gpu_run(gpu, grid, opac, dict(prm, cloud_phase=0), "albedo")
+    assert np.all(np.abs(hg["value"] - g["value"])[:, :2] > 8 * np.hypot(hg["sigma"], g["sigma"])[:, :2])   # back- and side-scatter
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        with pytest.raises(gpu.GcmcrtError) as e:
+            G.run_albedo(dict(prm, cloud_phase=3))
+        assert e.value.code == gpu.E_INVALID
+
+
 def test_packet_and_channel_subranges_compose(gpu):
     grid, opac, prm = wl.cfg2(nlon=8, nlat=4, nlev=10, nbands=1, ng=4, packets=20000)
     full = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)

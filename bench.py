@@ -46,7 +46,7 @@ I_SEG_3D = 34.0      # one 3D cell crossing: radial run 28.8 executed thread-ins
                      # column updates 5.3 per segment (ncu source page, profiles/ncu_full_r01b_ray_run.txt)
 I_SEG_1D = 29.0      # nlat = nlon = 1: the same radial run, no lateral crossings
 I_EVENT = 420.0      # Philox block, phase sampling, rotation, ray setup, event record write + read
-PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 = 4.51e9   # ncu: 7 launches of a cfg2 step average 4.506 GB read + 6.4 MB written
+PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 = 7.97e9   # ncu: 4 launches of a cfg2 step average 7.958 GB read + 7.2 MB written
 I_PEEL_RAY = 300.0   # record + prop read, phase function, ray setup for one (event, observer), exp, bin accumulation
 
 
@@ -333,7 +333,7 @@ def run_ours(args):
                     # dram__bytes_read + write per peel_kernel launch from one ncu --set full capture of the default
                     # workload (profiles/ncu_full_r01b_ray_run.txt); other workloads: not captured
                     "traffic": PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 if (args.workload == "cfg2" and args.packets is None) else None,
-                    "traffic_unit": "bytes per launch (54 M events: 64 B record + 4 B permutation entry + extinction gathers)",
+                    "traffic_unit": "bytes per launch (94 M events: 64 B record + 4 B permutation entry + extinction gathers)",
                     "peak_source": "148 SM x 128 FP32 lanes x sm_max_mhz (%s)" % pk["source"],
                     "work_lane_instr_per_launch": work / n_dom, "ms_per_launch": dur_ms / n_dom,
                     "hbm_term": {"bytes_per_step": hbm_bytes, "ms_at_peak": hbm_bytes / (pk["hbm_gbs"] * 1e9) * 1e3 * 1.0,

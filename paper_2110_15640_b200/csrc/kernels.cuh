@@ -489,7 +489,8 @@ __device__ __forceinline__ float sample_cloud(int cloud_phase, float g, float zl
 __device__ __forceinline__ float phase_hg(float g, float mu)
 {
     const float d = fmaf(-2.0f * g, mu, 1.0f + g * g);
-    return (1.0f - g * g) / (4.0f * kPi * d * sqrtf(d));
+    const float r = rsqrtf(d);   // d^(-3/2) = r^3: no division, no square root (the peel kernel evaluates this per ray)
+    return (1.0f - g * g) * (0.25f / kPi) * (r * r * r);
 }
 __device__ __forceinline__ float phase_cloud(int cloud_phase, float g, float mu)
 {
@@ -983,7 +984,7 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
                 float theta;
                 if (kind == EV_MEDIUM) {  // C6: mixture phase function, per steradian (Eq. 5, Eq. 7)
                     const float hg = phase_cloud(rc.cloud_phase, g, mu);
-                    const float ray_p = 3.0f * (1.0f + mu * mu) / (16.0f * kPi);
+                    const float ray_p = (3.0f / (16.0f * kPi)) * fmaf(mu, mu, 1.0f);
                     theta = pgas * ray_p + (1.0f - pgas) * hg;
                 } else if (kind == EV_EMIT) {
                     theta = 1.0f / (4.0f * kPi);

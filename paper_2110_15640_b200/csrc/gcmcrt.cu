@@ -540,14 +540,17 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             // channels whose events can share one pass: every packet makes at least one event when it interacts,
             // so a pass of ev_cap events spans about ev_cap / n_pkt channels; more bins than that only cost scan time
             const long long span = (long long)(g->ev_cap / std::max<size_t>(n_pkt, 1)) + 2;
-            // few packets per channel (high-resolution runs: 1e5 packets over 1e5-1e6 cells): sort by (channel, column)
-            // instead of (channel, cell) -- rays from one column toward one observer still share their extinction
-            // sectors, the histogram is nlev times smaller and every channel of the pass keeps bins of its own
-            const int coarse = n_pkt < 2ull * (unsigned long long)g->ncell;
-            const long long bins_per_chan = coarse ? (long long)g->nlat * g->nlon : (long long)g->ncell;
+            // few packets per channel (high-resolution runs: 1e5 packets over 1e5-1e6 cells): a coarser second key part
+            // -- groups of 4 levels below 2 packets per cell, whole columns below 1 packet per 4 cells.  Rays from one
+            // column toward one observer still share their extinction sectors, the histogram shrinks and every channel
+            // of the pass keeps bins of its own; lanes of different levels finish at different steps, which costs the
+            // peel kernel more than the smaller sort saves once the bins are well filled
+            const int lev_shift = n_pkt >= 2ull * (unsigned long long)g->ncell ? 0 : (4 * n_pkt >= (unsigned long long)g->ncell ? 2 : 30);
+            const long long nlg = lev_shift >= 30 ? 1 : (g->nlev + (1 << lev_shift) - 1) >> lev_shift;
+            const long long bins_per_chan = (long long)g->nlat * g->nlon * nlg;
             sp.c_fold = int(std::max<long long>(1, std::min<long long>(std::min<long long>(ncr, max_bins / bins_per_chan), span)));
             sp.nbins = (unsigned int)((long long)sp.c_fold * bins_per_chan);
-            ev.coarse = coarse; ev.bins_per_chan = int(bins_per_chan);
+            ev.lev_shift = lev_shift; ev.nlg = int(nlg); ev.bins_per_chan = int(bins_per_chan);
             sp.n_tiles = (sp.nbins + kScanTile - 1) / kScanTile;
             CUDA_TRY(g, g->hist.ensure(size_t(sp.nbins) * sizeof(unsigned int)));
             CUDA_TRY(g, g->tile_sums.ensure(size_t(sp.n_tiles) * sizeof(unsigned int)));

@@ -45,7 +45,8 @@ struct EventBuf {
                           // instead (emission: events pile up in a few bright cells and the contended atomics are
                           // cheaper in a kernel of their own than inside the emit / interact kernels)
     int chan_lo, c_fold, nlev, nlat, ncell;
-    int coarse, bins_per_chan;   // coarse: the key's second part is the column (k * nlat + j) instead of the cell
+    int lev_shift, nlg, bins_per_chan;   // the key's second part is column * nlg + (i >> lev_shift): cells (shift 0),
+                                         // groups of levels, or whole columns (nlg = 1)
 };
 
 __device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slot, float px, float py, float pz, float W,
@@ -61,7 +62,7 @@ __device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slo
         const int i = cellp & 1023, j = (cellp >> 10) & 1023, k = cellp >> 20;
         const unsigned int chan = (unsigned int)min(max(int(meta >> 8) - ev.chan_lo, 0), ev.c_fold - 1);
         const unsigned int col = (unsigned int)(k * ev.nlat + j);
-        const unsigned int key = chan * (unsigned int)ev.bins_per_chan + (ev.coarse ? col : col * (unsigned int)ev.nlev + (unsigned int)i);
+        const unsigned int key = chan * (unsigned int)ev.bins_per_chan + col * (unsigned int)ev.nlg + (ev.nlg > 1 ? (unsigned int)(i >> ev.lev_shift) : 0u);
         ev.keys[slot] = key;
         if (ev.hist) atomicAdd(ev.hist + key, 1u);
     }

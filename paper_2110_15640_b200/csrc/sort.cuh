@@ -5,7 +5,8 @@
 // two sectors and makes the lanes of a warp finish together.  Only a permutation is built (4 B per event); the
 // 48 B records stay where the transport kernel wrote them.
 //
-//   key(e) = clamp(chan_run(e) - chan_lo, 0, c_fold - 1) * ncell + (k * nlat + j) * nlev + i   (i fastest)
+//   key(e) = clamp(chan_run(e) - chan_lo, 0, c_fold - 1) * bins_per_chan + (k * nlat + j) * nlg + (i >> lev_shift)
+//            (cells when a channel has >= 2 packets per cell; groups of 4 levels or whole columns for sparser runs)
 //   ev_hist_kernel    hist[key]++   (global atomics; albedo runs count the bin while the record is written instead)
 //   scan_*            exclusive prefix sum of hist in place        (tile reduce, scan of tile sums, tile scan)
 //   ev_scatter_kernel perm[hist[key]++] = e

@@ -741,6 +741,18 @@ def test_full_grid_cfg4_doppler_batch_sums_against_oracle(gpu, orc):
     assert bad <= 1
 
 
+@pytest.mark.parametrize("nlev", [100, 130])
+def test_emission_on_tall_grids(gpu, orc, nlev):
+    """Grids with more than 64 levels take the 4- and 8-chunk instances of the emission CDF kernel (lanes along the
+    column, 32 levels per chunk) and longer extinction columns in the marcher: emission with scattering, the depth cut
+    and a biased cell draw against the oracle."""
+    grid, opac, prm = wl.cfg3(nlon=6, nlat=4, nlev=nlev, nbands=1, ng=3, packets=20000, n_obs=2)
+    for p in (prm, dict(prm, emission_bias=0.3, tau_vert_max=5.0)):
+        g = _gpu_run(gpu, grid, opac, p, "emission", want_event_count=True)
+        o = orc.run_emission(grid, opac, dict(p, n_threads=os.cpu_count() or 1), want_event_count=True)
+        _check_parity(orc, g, o, "emission")
+
+
 def test_error_paths(gpu):
     grid, opac, prm = wl.cfg1(packets=100)
     with gpu.Grid(grid) as G:

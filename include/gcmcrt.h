@@ -147,14 +147,17 @@ int gcmcrt_grid_create(gcmcrt_grid **out, int nlev, int nlat, int nlon,
 
 /*
  * gcmcrt_set_opacity -- give the per-channel, per-cell opacities (D3) of
- * channels chan0 .. chan0+n_chan-1 and stage alpha_ext = rho (k_abs + k_ray + k_cld), omega, P_gas (Eq. 11)
- * and g per (channel, cell) (A0).  chan0 is the global index of the first channel: it keys the random
- * streams, so results do not depend on how a long table is cut into batches.
+ * channels chan0 .. chan0+n_chan-1.  The packed records alpha_ext = rho (k_abs + k_ray + k_cld), omega, P_gas
+ * (Eq. 11) and g per (channel, cell) (A0) are staged from them by the first run that needs them (an unshifted run
+ * stages once; a doppler_on run stages per observer; a continuous_absorption run stages its own variant).  chan0 is
+ * the global index of the first channel: it keys the random streams, so results do not depend on how a long table
+ * is cut into batches.
  *   lambda[n_chan]  host, m (Planck function, Doppler spacing)
- *   k_abs           host|device [n_chan][nlon][nlat][nlev], required (device memory is borrowed, see above)
+ *   k_abs           host|device [n_chan][nlon][nlat][nlev], required
  *   k_sca_ray       host|device, nullable (= 0): Rayleigh scattering opacity
  *   k_sca_cld       host|device, nullable (= 0): cloud scattering opacity
- *   g_cld           host|device, nullable (= 0): HG asymmetry of the cloud scatterers
+ *   g_cld           host|device, nullable (= 0): asymmetry parameter of the cloud scatterers
+ *   (device-resident tables are borrowed until the next gcmcrt_set_opacity* / gcmcrt_destroy, see OWNERSHIP above)
  * Errors: E_INVALID, E_NOMEM, E_CUDA.
  */
 int gcmcrt_set_opacity(gcmcrt_grid *grid, int chan0, int n_chan, const float *lambda,

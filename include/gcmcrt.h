@@ -84,7 +84,7 @@ typedef struct gcmcrt_run_params {
                                     HG (Eq. 10) with the paper's default g1 = g, g2 = -g/2, alpha = 1 - g2^2 (L157),
                                     2 = Draine (Eq. 9) with alpha = 0.5 (L146) and G chosen so that <cos> = g_cld; its
                                     cosine is the zeta-quantile of Eq. 9 (one draw) */
-    int forced_first;            /* gcmcrt_run_albedo only: forced first scattering (Sect. 4.2): the optical depth
+    int forced_scatter;            /* gcmcrt_run_albedo only: forced first scattering (Sect. 4.2): the optical depth
                                     tau_edge along the launch ray to where it leaves the grid is integrated first, the
                                     flight is drawn as tau = -ln(1 - zeta (1 - e^-tau_edge)) and the packet starts with
                                     W = 1 - e^-tau_edge; e^-tau_edge is added to counters.escaped_weight when the ray
@@ -94,7 +94,7 @@ typedef struct gcmcrt_run_params {
                                     same path); every interaction in the medium is a scattering (no absorption draw, no
                                     omega in the peel-off weight).  Packets end by escaping, at the lower boundary, at
                                     max_events, or by Russian roulette (survival_bias = 1 with roulette_w_min > 0).
-                                    Runs through the persistent transport kernel; excludes forced_first. */
+                                    Runs through the persistent transport kernel; excludes forced_scatter. */
 } gcmcrt_run_params;
 
 typedef struct gcmcrt_counters {

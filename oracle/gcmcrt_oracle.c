@@ -657,9 +657,27 @@ static void transport(const run_ctx *rc, uint32_t pkt, double p[3], double n[3],
     uint32_t m_inter = 0;    /* interaction index (Philox event index), 1,2,... */
     double z[4];
     const int cont = prm->continuous_absorption != 0;
+    int flight = 0;
     for (;;) {
         double tau = 0.0;
         int st;
+        if (prm->forced_scatter == 2 && !(flight++ == 0 && m == 0)) {   /* m == 0: the albedo launch, forced there */
+            /* Sect. 4.2, forced scattering at every flight (the albedo launch does it for the first one): the flight is
+             * drawn from the exponential law truncated at the optical depth to the end of the grid, the packet keeps
+             * the probability 1 - e^-tau_edge of interacting, the uncollided part leaves (Cashwell & Everett 1959) */
+            double q[3] = { p[0], p[1], p[2] }, tau_edge = 0.0;
+            int c3[3] = { ijk[0], ijk[1], ijk[2] };
+            uint64_t seg = 0;
+            int se = march(G, ch->alpha, q, n, c3, INFINITY, &tau_edge, &seg, NULL);
+            if (se == ST_ESCAPE || (se == ST_SURFACE && !(a_surf > 0.0))) {
+                const double pint = -expm1(-tau_edge);
+                if (pint > 0.0) {
+                    if (se == ST_ESCAPE) cnt->escaped_weight += W * exp(-tau_edge);
+                    tau_t = -log1p(-exp(-tau_t) * pint);   /* the flight's own zeta = e^-tau_t */
+                    W *= pint;
+                }
+            }
+        }
         if (cont) {
             /* Sect. 4.1, Eq. 12: the sampled optical depth is spent on the scattering extinction alone and the packet
              * loses weight smoothly, W <- W e^-tau_abs, with tau_abs integrated along the same flight */
@@ -741,7 +759,7 @@ static void packet_albedo(const run_ctx *rc, uint32_t pkt, int batch, orc_counte
     locate(G, p, ijk);
     ijk[0] = G->nlev - 1;
     double W = 1.0, tau_t = -log(z[2]);
-    if (prm->forced_first) {
+    if (prm->forced_scatter) {
         /* Sect. 4.2: "an extra raytracing step to calculate the optical depth to the end of the grid in the
          * direction of the packet path", here once, at the start of the packet (forced first scattering).  The flight
          * is drawn from the exponential law truncated at tau_edge and the packet carries the probability

@@ -86,10 +86,11 @@ typedef struct {
     double ld_c1, ld_c2;     /* quadratic limb-darkening law, Eq. 22 */
     int cloud_phase;         /* cloud scatterers: 0 = HG (Eq. 7-8), 2 = Draine (Eq. 9, alpha = 0.5), 1 = two-term HG (Eq. 10) with the paper's default
                                 g1 = g, g2 = -g/2, alpha = 1 - g2^2 (L157) */
-    int forced_first;        /* albedo: forced first scattering (Sect. 4.2; Cashwell & Everett 1959): the first flight
-                                must end inside the grid: tau_edge = optical depth along the launch ray to where it leaves
-                                the grid (the extra ray trace of L179), tau = -ln(1 - zeta (1 - e^-tau_edge)),
-                                W = 1 - e^-tau_edge.  Rays that end on a reflecting lower boundary stay analog. */
+    int forced_scatter;      /* Sect. 4.2 (L179; Cashwell & Everett 1959): 1 = forced first scattering of albedo packets: the
+                                first flight must end inside the grid: tau_edge = optical depth along the launch ray to
+                                where it leaves the grid (the extra ray trace of L179), tau = -ln(1 - zeta (1 - e^-tau_edge)),
+                                W = 1 - e^-tau_edge.  2 = the same at every flight (albedo and emission).  Rays that
+                                end on a reflecting lower boundary stay analog. */
     int continuous_absorption; /* Sect. 4.1, Eq. 12: flights are sampled against the scattering extinction only and the
                                 weight decays as W <- W e^-tau_abs along every flight; every interaction in the medium
                                 is then a scattering (no absorption draw, no omega in the peel-off weight) */

@@ -33,7 +33,7 @@ class RunParams(C.Structure):
                 ("doppler_halfwidth", C.c_int), ("emission_bias", C.c_double), ("tau_vert_max", C.c_double),
                 ("tau_cut", C.c_double), ("npix", C.c_int), ("n_batches", C.c_int),
                 ("survival_bias", C.c_int), ("roulette_w_min", C.c_double), ("roulette_survive", C.c_double),
-                ("star_radius", C.c_double), ("planet_xy", C.c_double * 2), ("ld_c1", C.c_double), ("ld_c2", C.c_double), ("cloud_phase", C.c_int), ("forced_first", C.c_int), ("continuous_absorption", C.c_int)]
+                ("star_radius", C.c_double), ("planet_xy", C.c_double * 2), ("ld_c1", C.c_double), ("ld_c2", C.c_double), ("cloud_phase", C.c_int), ("forced_scatter", C.c_int), ("continuous_absorption", C.c_int)]
 
 
 class Counters(C.Structure):
@@ -180,7 +180,7 @@ def make_params(prm):
     p.planet_xy[0], p.planet_xy[1] = float(xy[0]), float(xy[1])
     p.ld_c1, p.ld_c2 = float(prm.get("ld_c1", 0.0)), float(prm.get("ld_c2", 0.0))
     p.cloud_phase = int(prm.get("cloud_phase", 0))
-    p.forced_first = int(prm.get("forced_first", 0))
+    p.forced_scatter = int(prm.get("forced_scatter", 0))
     p.continuous_absorption = int(prm.get("continuous_absorption", 0))
     return p, obs
 

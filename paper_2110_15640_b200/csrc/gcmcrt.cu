@@ -329,8 +329,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
 
     int rcode = ensure_workspace(g, (unsigned long long)ncr * (hi - lo));
     if (rcode) return rcode;
-    if (prm->forced_first && (g->tune[2] == 0 || prm->continuous_absorption))
-        return fail(g, GCMCRT_E_INVALID, "forced_first needs the wavefront transport (GCMCRT_TUNE generations > 0, no continuous_absorption)");
+    if (prm->forced_scatter && (g->tune[2] == 0 || prm->continuous_absorption))
+        return fail(g, GCMCRT_E_INVALID, "forced_scatter needs the wavefront transport (GCMCRT_TUNE generations > 0, no continuous_absorption)");
 
     // ---- outputs
     OutBuf o_flux, o_ltot, o_val, o_sig, o_img, o_evc, o_cnt, o_ctb;
@@ -366,7 +366,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.max_events = prm->max_events; rc.scatter_on = prm->scatter_on;
     rc.survival_bias = prm->survival_bias != 0;
     rc.cloud_phase = prm->cloud_phase;
-    rc.forced_first = prm->forced_first != 0;
+    rc.forced_scatter = prm->forced_scatter != 0;
     rc.alpha2 = nullptr;
     if (prm->cloud_phase < 0 || prm->cloud_phase > 2) return fail(g, GCMCRT_E_INVALID, "cloud_phase must be 0 (HG), 1 (TTHG) or 2 (Draine)");
     rc.roulette_w_min = float(prm->roulette_w_min); rc.roulette_survive = float(prm->roulette_survive);
@@ -566,7 +566,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         // continuous absorption runs through the persistent kernel only (its march carries the second extinction)
         const int n_gen = cont ? 0 : g->tune[2];
         auto k_keys = wave_launch_keys_kernel;
-        auto k_first = rc.forced_first ? wave_first_flight_kernel<16, true> : wave_first_flight_kernel<16, false>;
+        auto k_first = rc.forced_scatter ? wave_first_flight_kernel<16, true> : wave_first_flight_kernel<16, false>;
         auto k_emit = wave_emit_kernel;
         auto k_inter = wave_interact_kernel<kInteractK>;
         const size_t smem_w = smem_t;

@@ -104,7 +104,7 @@ struct RunConst {
     float roulette_w_min, roulette_survive;   // Sect. 4.5: Russian roulette below the weight threshold (0 = off)
     int cloud_phase;               // 0 HG (Eq. 7-8), 1 two-term HG (Eq. 10, g1 = g, g2 = -g/2, alpha = 1 - g2^2), 2 Draine (Eq. 9)
     const float* alpha2;           // continuous absorption: [n_chan][ncol][col_stride] pairs (alpha_sca, alpha_abs), or NULL
-    int forced_first;              // albedo: forced first scattering (Sect. 4.2)
+    int forced_scatter;              // albedo: forced first scattering (Sect. 4.2)
     float surface_albedo;
     double xi;
     int n_batches;

@@ -33,7 +33,7 @@ def default_params(**kw):
     prm = dict(star_dir=np.array([1.0, 0.0, 0.0]), obs_dir=np.array([[1.0, 0.0, 0.0]]),
                packets_per_channel=10000, seed=1, max_events=0, scatter_on=1, doppler_on=0,
                doppler_halfwidth=0, emission_bias=0.0, tau_vert_max=30.0, tau_cut=50.0, npix=0, n_batches=32,
-               survival_bias=0, roulette_w_min=0.0, roulette_survive=0.0, cloud_phase=0, forced_first=0, continuous_absorption=0)
+               survival_bias=0, roulette_w_min=0.0, roulette_survive=0.0, cloud_phase=0, forced_scatter=0, continuous_absorption=0)
     prm.update(kw)
     prm["star_dir"] = np.asarray(prm["star_dir"], dtype=np.float64)
     prm["obs_dir"] = np.asarray(prm["obs_dir"], dtype=np.float64).reshape(-1, 3)

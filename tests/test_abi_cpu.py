@@ -33,7 +33,7 @@ def test_library_exports_every_declared_symbol(lib):
 
 def test_struct_layouts_match_header():
     # gcmcrt_run_params: 3 doubles, int(+pad), ptr, 4 u64, 6 int, 3 doubles, 2 int  (natural alignment)
-    assert C.sizeof(binding.RunParams) == 24 + 8 + 8 + 32 + 24 + 24 + 8 + 24 + 40 + 8 + 8   # + survival_bias (int + pad), 2 doubles; + 5 doubles (transmission); + cloud_phase, forced_first; + continuous_absorption (int + pad)
+    assert C.sizeof(binding.RunParams) == 24 + 8 + 8 + 32 + 24 + 24 + 8 + 24 + 40 + 8 + 8   # + survival_bias (int + pad), 2 doubles; + 5 doubles (transmission); + cloud_phase, forced_scatter; + continuous_absorption (int + pad)
     assert binding.RunParams.survival_bias.offset == 128 and binding.RunParams.roulette_survive.offset == 144
     assert binding.RunParams.obs_dir.offset == 32 and binding.RunParams.seed.offset == 64
     assert binding.RunParams.emission_bias.offset == 96 and binding.RunParams.n_batches.offset == 124

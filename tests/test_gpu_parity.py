@@ -332,24 +332,24 @@ def test_survival_biasing_and_roulette_parity(gpu, orc, monkeypatch, tune):
         assert e.value.code == gpu.E_INVALID
 
 
-def test_forced_first_scattering_parity(gpu, orc, monkeypatch):
+def test_forced_scatter_scattering_parity(gpu, orc, monkeypatch):
     """Sect. 4.2 (L179), forced first scattering in the first-flight kernel against the oracle: same streams, same
     truncated flights and weights (thin 1D atmosphere where most analog packets fly through, and the 3D config 2 grid
     with a small event buffer so that forced packets are also parked and resumed); the escaped-weight budget agrees;
     forced and analog runs agree within their errors; the persistent-only transport refuses the option."""
     grid, opac, prm = wl.cfg1(packets=20000)
     opac = dict(opac, k_abs=opac["k_abs"] * 1e-3, k_sca_ray=opac["k_sca_ray"] * 3e-2)
-    prm = dict(prm, forced_first=1)
+    prm = dict(prm, forced_scatter=1)
     g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
     o = orc.run_albedo(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
     _check_parity(orc, g, o, "albedo")
     assert abs(g["counters"]["escaped_weight"] - o["counters"]["escaped_weight"]) < 1e-4 * o["counters"]["escaped_weight"]
-    ana = _gpu_run(gpu, grid, opac, dict(prm, forced_first=0), "albedo", want_event_count=True)
+    ana = _gpu_run(gpu, grid, opac, dict(prm, forced_scatter=0), "albedo", want_event_count=True)
     assert (g["event_count"] >= 1).mean() > (ana["event_count"] >= 1).mean() + 0.2
     assert np.all(np.abs(g["value"] - ana["value"]) < 4 * np.hypot(g["sigma"], ana["sigma"]) + 1e-5 * ana["value"])
     assert np.median(g["sigma"] / ana["sigma"]) < 1.0        # batch-means sigmas of 32 batches are themselves noisy
     grid, opac, prm = wl.cfg2(nlon=16, nlat=8, nlev=20, nbands=2, ng=3, packets=20000)
-    prm = dict(prm, forced_first=1)
+    prm = dict(prm, forced_scatter=1)
     monkeypatch.setenv("GCMCRT_EVENT_CAP", "30000")
     g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
     o = orc.run_albedo(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
@@ -394,7 +394,7 @@ def test_continuous_absorption_parity(gpu, orc):
     with gpu.Grid(grid) as G:
         G.set_opacity(opac)
         with pytest.raises(gpu.GcmcrtError) as e:
-            G.run_albedo(dict(prm, forced_first=1))
+            G.run_albedo(dict(prm, forced_scatter=1))
         assert e.value.code == gpu.E_INVALID
 
 

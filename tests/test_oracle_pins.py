@@ -853,7 +853,7 @@ def test_node_interpolation_is_exact_on_bilinear_tables_and_clamps(orc):
 
 # ----------------------------------------------------------------------------- forced first scattering (Sect. 4.2)
 @pytest.mark.parametrize("pgas,g", [(0.0, 0.0), (0.5, 0.5)])
-def test_forced_first_scattering_is_unbiased_single_cell(orc, pgas, g):
+def test_forced_scatter_scattering_is_unbiased_single_cell(orc, pgas, g):
     """Forced first scattering leaves the expectation of the single-scattering estimator unchanged: the value comes
     from a quadrature over (impact point, flight length) written here, the ANALOG run (no forcing anywhere in it) is
     checked against the same number, the forced run has the smaller variance in an optically thin cell, and every
@@ -866,7 +866,7 @@ def test_forced_first_scattering_is_unbiased_single_cell(orc, pgas, g):
     N = 200000
     prm = wl.default_params(packets_per_channel=N, seed=35, star_dir=s, obs_dir=o[None], max_events=1)
     va, sa = orc.reduce(orc.run_albedo(grid, opac, prm), "albedo")
-    rf = orc.run_albedo(grid, opac, dict(prm, forced_first=1), want_event_count=True)
+    rf = orc.run_albedo(grid, opac, dict(prm, forced_scatter=1), want_event_count=True)
     vf, sf = orc.reduce(rf, "albedo")
     assert np.all(rf["event_count"] == 1)
     n0, n1, n2 = 160, 64, 160
@@ -890,7 +890,7 @@ def test_forced_first_scattering_is_unbiased_single_cell(orc, pgas, g):
     assert sf[0, 0] < 0.6 * sa[0, 0]
 
 
-def test_forced_first_scattering_conserves_energy_and_matches_analog_on_3d_grid(orc):
+def test_forced_scatter_scattering_conserves_energy_and_matches_analog_on_3d_grid(orc):
     """omega = 1 over a Lambert a = 1 floor: uncollided + scattered weight of every packet leaves the grid, so the
     escaped weight is N (L196); rays that end on the reflecting floor stay analog.  With absorption, forced and analog
     runs of a thin 3D atmosphere agree within their errors at every observer."""
@@ -898,14 +898,14 @@ def test_forced_first_scattering_conserves_energy_and_matches_analog_on_3d_grid(
     grid, opac = wl.uniform_medium(3, 2, 3, R0, Rt, 0.3 / (Rt - R0), 1.0, g=0.4, pgas=0.3, surface_albedo=1.0)
     N = 20000
     prm = wl.default_params(packets_per_channel=N, seed=5, star_dir=[0.6, 0.0, 0.8], obs_dir=np.array([[0.6, 0.0, 0.8]]),
-                            forced_first=1)
+                            forced_scatter=1)
     c = orc.run_albedo(grid, opac, prm)["counters"]
     assert c["packets_escaped"] == N and abs(c["escaped_weight"] - N) < 1e-9 * N
     grid, opac = wl.uniform_medium(4, 3, 4, R0, Rt, 0.2 / (Rt - R0), 0.8, g=0.3, pgas=0.3)
     obs = np.array([[1.0, 0, 0], [0.0, 1.0, 0.0], [0.6, 0.0, 0.8], [-0.6, 0.0, 0.8]])
     prm = wl.default_params(packets_per_channel=100000, seed=6, star_dir=[1.0, 0.0, 0.0], obs_dir=obs)
     va, sa = orc.reduce(orc.run_albedo(grid, opac, prm), "albedo")
-    vf, sf = orc.reduce(orc.run_albedo(grid, opac, dict(prm, forced_first=1)), "albedo")
+    vf, sf = orc.reduce(orc.run_albedo(grid, opac, dict(prm, forced_scatter=1)), "albedo")
     assert np.all(np.abs(va - vf) < 4 * np.hypot(sa, sf))
     assert np.all(sf < 0.8 * sa)
 
@@ -1005,3 +1005,43 @@ def test_draine_limits_and_transport_consistency(orc):
     assert abs(total - 1.0) < 4 * np.sqrt(np.sum((sig[0] * wq) ** 2)) + 0.02, total
     hg = orc.reduce(orc.run_albedo(grid, opac, dict(prm, cloud_phase=0)), "albedo")[0]
     assert not np.allclose(val, hg, rtol=0.02)       # and it is not the HG run
+
+
+@pytest.mark.parametrize("omega", [0.5, 0.9])
+def test_forced_scattering_at_every_flight_keeps_the_exact_semi_infinite_albedo(orc, omega):
+    """forced_scatter = 2 (Sect. 4.2: every flight is forced to end inside the grid; packets end by Russian roulette):
+    the exact semi-infinite isotropic albedo is unchanged, and so is the albedo of a thin 3D atmosphere, where most
+    analog flights would leave -- there with a smaller error than the analog run's."""
+    rows = dict(np.loadtxt(os.path.join(GOLDEN, "isotropic_semi_infinite_albedo.txt")))
+    R0, depth = 1.0e8, 1.0e4
+    grid, opac = wl.uniform_medium(4, 1, 1, R0, R0 + depth, 80.0 / depth, omega, g=0.0, surface_albedo=1.0)
+    s = np.array([0.3, -0.5, 0.81]); s /= np.linalg.norm(s)
+    prm = wl.default_params(packets_per_channel=40000, seed=23, star_dir=s, obs_dir=s[None], forced_scatter=2,
+                            survival_bias=1, roulette_w_min=0.02, roulette_survive=0.2)
+    val, sig = orc.reduce(orc.run_albedo(grid, opac, prm), "albedo")
+    Ag = PI * val[0, 0]
+    assert abs(Ag - rows[omega]) < 4 * PI * sig[0, 0] + 3e-4 * rows[omega], (Ag, rows[omega], PI * sig[0, 0])
+    R0, Rt = 1.0e6, 1.3e6
+    grid, opac = wl.uniform_medium(4, 3, 4, R0, Rt, 0.3 / (Rt - R0), omega, g=0.3, pgas=0.3)
+    obs = np.array([[1.0, 0, 0], [0.0, 1.0, 0.0], [0.6, 0.0, 0.8]])
+    prm = wl.default_params(packets_per_channel=60000, seed=7, star_dir=[1.0, 0.0, 0.0], obs_dir=obs)
+    ra = orc.run_albedo(grid, opac, prm)
+    rf = orc.run_albedo(grid, opac, dict(prm, forced_scatter=2, survival_bias=1, roulette_w_min=0.02, roulette_survive=0.2))
+    va, sa = orc.reduce(ra, "albedo"); vf, sf = orc.reduce(rf, "albedo")
+    assert np.all(np.abs(va - vf) < 4 * np.hypot(sa, sf))
+    assert np.all(sf < 0.7 * sa)
+    # what leaves: the uncollided parts of all flights; its expectation is the analog escape fraction
+    N = 60000
+    fa = ra["counters"]["packets_escaped"] / N
+    assert abs(rf["counters"]["escaped_weight"] / N - fa) < 4 * np.sqrt(fa * (1 - fa) / N) + 4 * np.sqrt(fa / N)
+
+
+def test_forced_scattering_of_emitted_packets(orc):
+    """forced_scatter = 2 in emission mode: the flights of emitted packets are forced as well; the spectrum agrees with
+    the analog run within the errors."""
+    grid, opac, prm = wl.cfg3(nlon=6, nlat=4, nlev=12, nbands=1, ng=2, packets=40000, n_obs=2)
+    prm = dict(prm, n_threads=os.cpu_count() or 1)
+    va, sa = orc.reduce(orc.run_emission(grid, opac, prm), "emission")
+    vf, sf = orc.reduce(orc.run_emission(grid, opac, dict(prm, forced_scatter=2, survival_bias=1, roulette_w_min=0.02,
+                                                         roulette_survive=0.2)), "emission")
+    assert np.all(np.abs(va - vf) <= 4 * np.hypot(sa, sf)) and np.any(va > 0)

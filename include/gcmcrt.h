@@ -84,11 +84,14 @@ typedef struct gcmcrt_run_params {
                                     HG (Eq. 10) with the paper's default g1 = g, g2 = -g/2, alpha = 1 - g2^2 (L157),
                                     2 = Draine (Eq. 9) with alpha = 0.5 (L146) and G chosen so that <cos> = g_cld; its
                                     cosine is the zeta-quantile of Eq. 9 (one draw) */
-    int forced_scatter;            /* gcmcrt_run_albedo only: forced first scattering (Sect. 4.2): the optical depth
-                                    tau_edge along the launch ray to where it leaves the grid is integrated first, the
-                                    flight is drawn as tau = -ln(1 - zeta (1 - e^-tau_edge)) and the packet starts with
-                                    W = 1 - e^-tau_edge; e^-tau_edge is added to counters.escaped_weight when the ray
-                                    leaves through the top.  Rays that end on a reflecting lower boundary stay analog. */
+    int forced_scatter;          /* Sect. 4.2 (L179), forced scattering: the optical depth tau_edge along the flight's ray to
+                                    where it leaves the grid is integrated first, the flight is drawn as
+                                    tau = -ln(1 - zeta (1 - e^-tau_edge)) and the weight is multiplied by 1 - e^-tau_edge;
+                                    W e^-tau_edge is added to counters.escaped_weight when the ray leaves through the top.
+                                    Rays that end on a reflecting lower boundary stay analog.  1 = the first flight of
+                                    albedo packets only ("forced first scattering"); 2 = every flight, albedo and emission
+                                    (needs max_events > 0 or Russian roulette to end the packets); excludes
+                                    continuous_absorption. */
     int continuous_absorption;   /* Sect. 4.1, Eq. 12: flights are sampled against the scattering extinction only and the
                                     weight decays as W <- W e^-tau_abs over every flight (tau_abs integrated along the
                                     same path); every interaction in the medium is a scattering (no absorption draw, no

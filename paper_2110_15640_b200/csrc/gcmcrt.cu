@@ -329,8 +329,10 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
 
     int rcode = ensure_workspace(g, (unsigned long long)ncr * (hi - lo));
     if (rcode) return rcode;
-    if (prm->forced_scatter && (g->tune[2] == 0 || prm->continuous_absorption))
-        return fail(g, GCMCRT_E_INVALID, "forced_scatter needs the wavefront transport (GCMCRT_TUNE generations > 0, no continuous_absorption)");
+    if (prm->forced_scatter < 0 || prm->forced_scatter > 2 || (prm->forced_scatter && prm->continuous_absorption))
+        return fail(g, GCMCRT_E_INVALID, "forced_scatter must be 0, 1 or 2 and excludes continuous_absorption");
+    if (prm->forced_scatter == 2 && !(prm->max_events > 0 || (prm->survival_bias && prm->roulette_w_min > 0.0)))
+        return fail(g, GCMCRT_E_INVALID, "forced_scatter = 2 needs max_events or Russian roulette to end its packets");
 
     // ---- outputs
     OutBuf o_flux, o_ltot, o_val, o_sig, o_img, o_evc, o_cnt, o_ctb;
@@ -366,7 +368,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.max_events = prm->max_events; rc.scatter_on = prm->scatter_on;
     rc.survival_bias = prm->survival_bias != 0;
     rc.cloud_phase = prm->cloud_phase;
-    rc.forced_scatter = prm->forced_scatter != 0;
+    rc.forced_scatter = prm->forced_scatter;
     rc.alpha2 = nullptr;
     if (prm->cloud_phase < 0 || prm->cloud_phase > 2) return fail(g, GCMCRT_E_INVALID, "cloud_phase must be 0 (HG), 1 (TTHG) or 2 (Draine)");
     rc.roulette_w_min = float(prm->roulette_w_min); rc.roulette_survive = float(prm->roulette_survive);
@@ -568,7 +570,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         auto k_keys = wave_launch_keys_kernel;
         auto k_first = rc.forced_scatter ? wave_first_flight_kernel<16, true> : wave_first_flight_kernel<16, false>;
         auto k_emit = wave_emit_kernel;
-        auto k_inter = wave_interact_kernel<kInteractK>;
+        auto k_inter = rc.forced_scatter == 2 ? wave_interact_kernel<kInteractK, true> : wave_interact_kernel<kInteractK, false>;
         const size_t smem_w = smem_t;
         const size_t smem_i = (size_t((g->tab_floats + 31) & ~31) + size_t(kWaveThreads / 32) * kStageFields * kStageSlots) * sizeof(float);
         int occ_f = 1, occ_i = 1;

@@ -104,7 +104,7 @@ struct RunConst {
     float roulette_w_min, roulette_survive;   // Sect. 4.5: Russian roulette below the weight threshold (0 = off)
     int cloud_phase;               // 0 HG (Eq. 7-8), 1 two-term HG (Eq. 10, g1 = g, g2 = -g/2, alpha = 1 - g2^2), 2 Draine (Eq. 9)
     const float* alpha2;           // continuous absorption: [n_chan][ncol][col_stride] pairs (alpha_sca, alpha_abs), or NULL
-    int forced_scatter;              // albedo: forced first scattering (Sect. 4.2)
+    int forced_scatter;            // Sect. 4.2: 1 = forced first scattering of albedo packets, 2 = every flight forced
     float surface_albedo;
     double xi;
     int n_batches;
@@ -546,6 +546,36 @@ __device__ __forceinline__ bool medium_interaction(const RunConst& rc, const flo
     return true;
 }
 
+// Sect. 4.2 (L179), forced scattering: the "extra raytracing step to calculate the optical depth to the end of the grid
+// in the direction of the packet path", lane by lane (the flights it serves are incoherent; the coherent first flights
+// of an albedo run have a warp-wide version in wave_first_flight_kernel), then the flight is drawn from the exponential
+// law truncated there, the packet keeps the probability 1 - e^-tau_edge of interacting and the uncollided part leaves.
+// A ray that ends on a reflecting lower boundary stays analog.
+__device__ __noinline__ int ray_tau_to_edge(Ray r, const GeomSmem& s, const float* alpha_c, int maxseg, float& tau)
+{
+    tau = 0.f;
+    int st = RAY_FLYING;
+    for (int it = 0; it <= maxseg && st == RAY_FLYING; ++it) {
+        st = ray_step(r, s, tau, kInf);
+        if (st == RAY_PARK) { ray_lateral(r, s, alpha_c); st = RAY_FLYING; }
+    }
+    return st;
+}
+__device__ __forceinline__ void force_flight(const RunConst& rc, const GeomSmem& gs, const Ray& ray, const float* alpha_c,
+                                             float& tau_t, float& W, double& escw)
+{
+    float tau_e;
+    const int st = ray_tau_to_edge(ray, gs, alpha_c, rc.geom.maxseg, tau_e);
+    if (st == RAY_ESCAPE || (st == RAY_SURFACE && !(rc.surface_albedo > 0.f))) {
+        const float pint = -expm1f(-tau_e);
+        if (pint > 0.f) {
+            if (st == RAY_ESCAPE) escw += double(W * expf(-tau_e));
+            tau_t = -log1pf(-expf(-tau_t) * pint);   // the flight's own zeta = e^-tau_t
+            W *= pint;
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // Transport kernel: persistent threads, one packet per lane, warp-level refill.
 // ---------------------------------------------------------------------------------------------------------
@@ -690,6 +720,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                     pk.tau = 0.f; pk.fl_seg = 0;
                                     ray_init<DUAL>(pk.ray, gs, px, py, pz, -rc.star[0], -rc.star[1], -rc.star[2], gs.nlev - 1,
                                              j, k, alpha_c);
+                                    if (!DUAL && rc.forced_scatter) force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw);
                                     st = LS_FLY;
                                 } else {
                                     // O4: cell ~ luminosity (Eq. 13) with composite bias xi, uniform point in the cell
@@ -795,6 +826,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                 rotate_dir(nx, ny, nz, ct, z.z2);
                                 pk.tau_t = -logf(z.z3); pk.tau = 0.f; pk.fl_seg = 0;
                                 ray_init<DUAL>(pk.ray, gs, px, py, pz, nx, ny, nz, pk.ray.i, pk.ray.j, pk.ray.k, alpha_c);
+                                if (!DUAL && rc.forced_scatter == 2) force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw);
                                 st = LS_FLY;
                             }
                         } else if (st == LS_EV_EMIT) {
@@ -812,6 +844,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                 sincospif(2.0f * z.z1, &sp, &cp);
                                 pk.tau_t = -logf(z.z2); pk.tau = 0.f; pk.fl_seg = 0;
                                 ray_init<DUAL>(pk.ray, gs, px, py, pz, ns * cp, ns * sp, nz, pk.ray.i, pk.ray.j, pk.ray.k, alpha_c);
+                                if (!DUAL && rc.forced_scatter == 2) force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw);
                                 st = LS_FLY;
                             }
                         } else {  // Lambert surface (O7, Eq. 3-4)
@@ -832,6 +865,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                 rotate_dir(hx, hy, hz, sqrtf(z.z1), z.z2);      // Eq. 4 about the normal
                                 pk.tau_t = -logf(z.z3); pk.tau = 0.f; pk.fl_seg = 0;
                                 ray_init<DUAL>(pk.ray, gs, px, py, pz, hx, hy, hz, 0, pk.ray.j, pk.ray.k, alpha_c);
+                                if (!DUAL && rc.forced_scatter == 2) force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw);
                                 st = LS_FLY;
                             }
                         }

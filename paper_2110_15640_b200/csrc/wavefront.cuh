@@ -401,7 +401,9 @@ __global__ void __launch_bounds__(kWaveThreads) wave_emit_kernel(const __grid_co
 }
 
 // generation g -> g + 1
-template <int KSTEPS>
+// FORCED: forced scattering at every flight (forced_scatter = 2): an instance of its own, so that the default one
+// carries no call to the edge probe
+template <int KSTEPS, bool FORCED>
 __global__ void __launch_bounds__(kWaveThreads, 3)
 wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const SuspBuf susp, const WaveConst wc)
 {
@@ -519,6 +521,7 @@ wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, con
                     }
                     alpha_c = rc.alpha + (size_t)(rc.chan_begin + int(chan_run)) * rc.geom.alpha_stride;
                     ray_init(ray, gs, px, py, pz, nx, ny, nz, i, j, k, alpha_c);
+                    if (FORCED) force_flight(rc, gs, ray, alpha_c, tau_t, W, wcnt.escw);   // Sect. 4.2
                     st = RAY_FLYING;
                 }
                 __syncwarp();

@@ -332,11 +332,11 @@ def test_survival_biasing_and_roulette_parity(gpu, orc, monkeypatch, tune):
         assert e.value.code == gpu.E_INVALID
 
 
-def test_forced_scatter_scattering_parity(gpu, orc, monkeypatch):
+def test_forced_first_scattering_parity(gpu, orc, monkeypatch):
     """Sect. 4.2 (L179), forced first scattering in the first-flight kernel against the oracle: same streams, same
     truncated flights and weights (thin 1D atmosphere where most analog packets fly through, and the 3D config 2 grid
     with a small event buffer so that forced packets are also parked and resumed); the escaped-weight budget agrees;
-    forced and analog runs agree within their errors; the persistent-only transport refuses the option."""
+    forced and analog runs agree within their errors; the persistent-only transport carries the same packets."""
     grid, opac, prm = wl.cfg1(packets=20000)
     opac = dict(opac, k_abs=opac["k_abs"] * 1e-3, k_sca_ray=opac["k_sca_ray"] * 3e-2)
     prm = dict(prm, forced_scatter=1)
@@ -355,11 +355,39 @@ def test_forced_scatter_scattering_parity(gpu, orc, monkeypatch):
     o = orc.run_albedo(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
     _check_parity(orc, g, o, "albedo")
     assert abs(g["counters"]["escaped_weight"] - o["counters"]["escaped_weight"]) < 1e-3 * o["counters"]["escaped_weight"]
-    monkeypatch.setenv("GCMCRT_TUNE", "16,1,0,4")
+    monkeypatch.setenv("GCMCRT_TUNE", "16,1,0,4")               # the persistent kernel alone gives the same packets
+    p_only = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+    assert np.array_equal(p_only["event_count"], g["event_count"])
+
+
+@pytest.mark.parametrize("tune", ["16,1,8,4", "16,1,0,4", "16,1,2,4"])
+def test_forced_scattering_at_every_flight_parity(gpu, orc, monkeypatch, tune):
+    """Sect. 4.2 with forced_scatter = 2 (every flight forced, Russian roulette ends the packets) against the oracle,
+    through the generation kernels, through the persistent kernel alone, and with packets handed from one to the other
+    after two generations: a thin 3D albedo run over a reflecting boundary (rays that end on it stay analog), and
+    emission with scattering.  The first-flight option now also runs on the persistent path."""
+    monkeypatch.setenv("GCMCRT_TUNE", tune)
+    R0, Rt = 1.0e6, 1.3e6
+    grid, opac = wl.uniform_medium(5, 4, 6, R0, Rt, 0.5 / (Rt - R0), 0.8, g=0.4, pgas=0.3, surface_albedo=0.3)
+    obs = np.array([[1.0, 0.0, 0.0], [0.0, 0.6, 0.8]])
+    prm = wl.default_params(packets_per_channel=30000, seed=12, star_dir=[1.0, 0.0, 0.0], obs_dir=obs, forced_scatter=2,
+                            survival_bias=1, roulette_w_min=0.02, roulette_survive=0.2)
+    g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+    o = orc.run_albedo(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
+    _check_parity(orc, g, o, "albedo")
+    assert abs(g["counters"]["escaped_weight"] - o["counters"]["escaped_weight"]) < 1e-3 * o["counters"]["escaped_weight"]
+    g1 = _gpu_run(gpu, grid, opac, dict(prm, forced_scatter=1), "albedo", want_event_count=True)
+    o1 = orc.run_albedo(grid, opac, dict(prm, forced_scatter=1, n_threads=os.cpu_count() or 1), want_event_count=True)
+    _check_parity(orc, g1, o1, "albedo")
+    grid, opac, prm = wl.cfg3(nlon=8, nlat=4, nlev=12, nbands=1, ng=2, packets=20000, n_obs=2)
+    prm = dict(prm, forced_scatter=2, survival_bias=1, roulette_w_min=0.02, roulette_survive=0.2)
+    g = _gpu_run(gpu, grid, opac, prm, "emission", want_event_count=True)
+    o = orc.run_emission(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
+    _check_parity(orc, g, o, "emission")
     with gpu.Grid(grid) as G:
         G.set_opacity(opac)
         with pytest.raises(gpu.GcmcrtError) as e:
-            G.run_albedo(prm)
+            G.run_emission(dict(prm, survival_bias=0, roulette_w_min=0.0))       # nothing would end the packets
         assert e.value.code == gpu.E_INVALID
 
 

@@ -853,7 +853,7 @@ def test_node_interpolation_is_exact_on_bilinear_tables_and_clamps(orc):
 
 # ----------------------------------------------------------------------------- forced first scattering (Sect. 4.2)
 @pytest.mark.parametrize("pgas,g", [(0.0, 0.0), (0.5, 0.5)])
-def test_forced_scatter_scattering_is_unbiased_single_cell(orc, pgas, g):
+def test_forced_first_scattering_is_unbiased_single_cell(orc, pgas, g):
     """Forced first scattering leaves the expectation of the single-scattering estimator unchanged: the value comes
     from a quadrature over (impact point, flight length) written here, the ANALOG run (no forcing anywhere in it) is
     checked against the same number, the forced run has the smaller variance in an optically thin cell, and every
@@ -890,7 +890,7 @@ def test_forced_scatter_scattering_is_unbiased_single_cell(orc, pgas, g):
     assert sf[0, 0] < 0.6 * sa[0, 0]
 
 
-def test_forced_scatter_scattering_conserves_energy_and_matches_analog_on_3d_grid(orc):
+def test_forced_first_scattering_conserves_energy_and_matches_analog_on_3d_grid(orc):
     """omega = 1 over a Lambert a = 1 floor: uncollided + scattered weight of every packet leaves the grid, so the
     escaped weight is N (L196); rays that end on the reflecting floor stay analog.  With absorption, forced and analog
     runs of a thin 3D atmosphere agree within their errors at every observer."""

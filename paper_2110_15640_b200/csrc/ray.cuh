@@ -276,6 +276,67 @@ __device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, f
     return RAY_FLYING;
 }
 
+// The plain-crossing loops of ray_run(), written in PTX: two crossings per trip with the roles of (alpha, alpha_n) and
+// (tau, tau_new) swapping between them, so that the loop body holds no register moves (compiled from C++, ptxas spends
+// 5 moves and a constant load per crossing on the loop-carried state); the exits restore the canonical state.
+// DIR = +1: outward (shell address + 8, column pointer + 4 per crossing); -1: inward (the root takes the minus sign).
+#define GCMCRT_RUN_LOOP(SOFF1, SOFF2, POFF1, POFF2, SSTEP1, SSTEP2, PSTEP1, PSTEP2, NEG)                              \
+    asm volatile(                                                                                                      \
+        "{\n\t"                                                                                                        \
+        ".reg .pred p;\n\t"                                                                                            \
+        ".reg .f32 ds, tn, hi, lo, q, tmp;\n\t"                                                                        \
+        ".reg .s32 n1;\n\t"                                                                                            \
+        "LOOP_%=:\n\t"                                                                                                 \
+        "setp.ge.s32 p, %7, %12;\n\t"                                                                                  \
+        "@p bra DONE_A_%=;\n\t"                                                                                        \
+        "sub.f32 ds, %1, %0;\n\t"                                                                                      \
+        "max.f32 ds, ds, 0f00000000;\n\t"                                                                              \
+        "fma.rn.f32 tn, %2, ds, %4;\n\t"                                                                               \
+        "setp.ge.f32 p, tn, %9;\n\t"                                                                                   \
+        "setp.gt.or.f32 p, %1, %8, p;\n\t"                                                                             \
+        "@p bra DONE_A_%=;\n\t"                                                                                        \
+        "max.f32 %0, %1, %0;\n\t"                                                                                      \
+        "ld.shared.v2.f32 {hi, lo}, [%6+" #SOFF1 "];\n\t"                                                              \
+        "ld.global.nc.f32 %2, [%5+" #POFF1 "];\n\t"                                                                    \
+        "sub.f32 hi, hi, %10;\n\t"                                                                                     \
+        "sub.f32 lo, lo, %11;\n\t"                                                                                     \
+        "add.f32 q, hi, lo;\n\t"                                                                                       \
+        "max.f32 q, q, 0f00000000;\n\t"                                                                                \
+        "sqrt.approx.ftz.f32 %1, q;\n\t" NEG                                                                           \
+        "add.s32 n1, %7, 1;\n\t"                                                                                       \
+        "setp.ge.s32 p, n1, %12;\n\t"                                                                                  \
+        "@p bra DONE_B_%=;\n\t"                                                                                        \
+        "sub.f32 ds, %1, %0;\n\t"                                                                                      \
+        "max.f32 ds, ds, 0f00000000;\n\t"                                                                              \
+        "fma.rn.f32 %4, %3, ds, tn;\n\t"                                                                               \
+        "setp.ge.f32 p, %4, %9;\n\t"                                                                                   \
+        "setp.gt.or.f32 p, %1, %8, p;\n\t"                                                                             \
+        "@p bra DONE_B_%=;\n\t"                                                                                        \
+        "max.f32 %0, %1, %0;\n\t"                                                                                      \
+        "ld.shared.v2.f32 {hi, lo}, [%6+" #SOFF2 "];\n\t"                                                              \
+        "ld.global.nc.f32 %3, [%5+" #POFF2 "];\n\t"                                                                    \
+        "sub.f32 hi, hi, %10;\n\t"                                                                                     \
+        "sub.f32 lo, lo, %11;\n\t"                                                                                     \
+        "add.f32 q, hi, lo;\n\t"                                                                                       \
+        "max.f32 q, q, 0f00000000;\n\t"                                                                                \
+        "sqrt.approx.ftz.f32 %1, q;\n\t" NEG                                                                           \
+        "add.s32 %6, %6, " #SSTEP2 ";\n\t"                                                                             \
+        "add.s64 %5, %5, " #PSTEP2 ";\n\t"                                                                             \
+        "add.s32 %7, %7, 2;\n\t"                                                                                       \
+        "bra LOOP_%=;\n\t"                                                                                             \
+        "DONE_B_%=:\n\t"   /* one crossing into the trip: current alpha in %3, next in %2, tau in tn */               \
+        "mov.f32 tmp, %2;\n\t"                                                                                         \
+        "mov.f32 %2, %3;\n\t"                                                                                          \
+        "mov.f32 %3, tmp;\n\t"                                                                                         \
+        "mov.f32 %4, tn;\n\t"                                                                                          \
+        "add.s32 %6, %6, " #SSTEP1 ";\n\t"                                                                             \
+        "add.s64 %5, %5, " #PSTEP1 ";\n\t"                                                                             \
+        "add.s32 %7, %7, 1;\n\t"                                                                                       \
+        "DONE_A_%=:\n\t"                                                                                               \
+        "}"                                                                                                            \
+        : "+f"(u), "+f"(u_rad), "+f"(alpha), "+f"(alpha_n), "+f"(tau), "+l"(pn), "+r"(sa), "+r"(n)                     \
+        : "f"(ul), "f"(tau_limit), "f"(d2), "f"(d2lo), "r"(plain))
+
 // Up to KSTEPS steps of ray_step() for a ray in flight, same arithmetic in the same order (bit-identical tau, u and
 // indices), written as two runs -- inward while the ray descends, outward after it has turned (it never turns back).
 // Inside a run the direction, the lateral limit min(u_lat, u_lon), the shared-memory address of the next shell and the
@@ -300,21 +361,7 @@ __device__ __forceinline__ int ray_run(Ray& r, const GeomSmem& s, float& tau_io,
         // is then the next one outward) or, for a ray that does not turn inside the grid, leaves through the lower boundary
         const uint32_t sa_stop = s.r2_saddr + 8u * uint32_t(max(r.i_turn + 1, 0));
         const int plain = min(KSTEPS, int((sa - sa_stop) >> 3));   // plain crossings before that one, within the budget
-#pragma unroll 1
-        while (n < plain) {
-            const float tnew = fmaf(alpha, fmaxf(u_rad - u, 0.0f), tau);   // min(u_rad, ul) = u_rad unless the loop ends here
-            if ((tnew >= tau_limit) | (u_rad > ul)) break;
-            tau = tnew;
-            u = fmaxf(u_rad, u);
-            alpha = alpha_n;
-            sa -= 8u;
-            float hi, lo;
-            asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(hi), "=f"(lo) : "r"(sa));
-            u_rad = -sqrt_approx(fmaxf((hi - d2) + (lo - d2lo), 0.0f));
-            --pn;
-            alpha_n = __ldg(pn);
-            ++n;
-        }
+        GCMCRT_RUN_LOOP(-8, -16, -4, -8, -8, -16, -4, -8, "neg.f32 %1, %1;\n\t");   // plain inward crossings
         if (n < KSTEPS) {
             ++n;
             const float un = fminf(u_rad, ul);
@@ -342,21 +389,7 @@ __device__ __forceinline__ int ray_run(Ray& r, const GeomSmem& s, float& tau_io,
     if (!inward && status == RAY_FLYING) {
         const uint32_t sa_top = s.r2_saddr + 8u * uint32_t(s.nlev);
         const int plain = min(KSTEPS, n + int((sa_top - sa) >> 3));   // plain crossings before the one that leaves the grid
-#pragma unroll 1
-        while (n < plain) {
-            const float tnew = fmaf(alpha, fmaxf(u_rad - u, 0.0f), tau);
-            if ((tnew >= tau_limit) | (u_rad > ul)) break;
-            tau = tnew;
-            u = fmaxf(u_rad, u);
-            alpha = alpha_n;
-            sa += 8u;
-            float hi, lo;
-            asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(hi), "=f"(lo) : "r"(sa));
-            u_rad = sqrt_approx(fmaxf((hi - d2) + (lo - d2lo), 0.0f));
-            ++pn;
-            alpha_n = __ldg(pn);
-            ++n;
-        }
+        GCMCRT_RUN_LOOP(8, 16, 4, 8, 8, 16, 4, 8, "");   // plain outward crossings
         if (n < KSTEPS) {
             ++n;
             const float un = fminf(u_rad, ul);

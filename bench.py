@@ -42,11 +42,12 @@ UNIT = "events/s"
 
 # Algorithmic lane-instructions (FP32/INT issue slots) per unit of work; DESIGN.md section "Roofline" derives them
 # from the audited SASS of the march loop, the event handler and the launch code.
-I_SEG_3D = 34.0      # one 3D cell crossing: radial run 28.8 executed thread-instructions per segment + cone / half-plane /
-                     # column updates 5.3 per segment (ncu source page, profiles/ncu_full_r01b_ray_run.txt)
-I_SEG_1D = 29.0      # nlat = nlon = 1: the same radial run, no lateral crossings
+I_SEG_3D = 27.0      # one 3D cell crossing: radial run 22 executed thread-instructions per segment (PTX loops, 19 issued per
+                     # crossing + the run's entry / exit code) + cone / half-plane / column updates 4.7 per segment
+                     # (ncu source page, profiles/ncu_full_r01d_ptx_loops.txt)
+I_SEG_1D = 22.0      # nlat = nlon = 1: the same radial run, no lateral crossings
 I_EVENT = 420.0      # Philox block, phase sampling, rotation, ray setup, event record write + read
-PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 = 7.97e9   # ncu: 4 launches of a cfg2 step average 7.958 GB read + 7.2 MB written
+PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 = 7.96e9   # ncu: 4 launches of a cfg2 step average 7.946 GB read + 9.2 MB written
 I_PEEL_RAY = 300.0   # record + prop read, phase function, ray setup for one (event, observer), exp, bin accumulation
 
 
@@ -331,7 +332,7 @@ def run_ours(args):
         roofline = {"bound": "alu", "kernel": dom + "_kernel", "achieved": achieved, "peak": peak,
                     "unit": "Tlane-instr/s", "frac": achieved / peak if peak else None,
                     # dram__bytes_read + write per peel_kernel launch from one ncu --set full capture of the default
-                    # workload (profiles/ncu_full_r01b_ray_run.txt); other workloads: not captured
+                    # workload (profiles/ncu_full_r01d_ptx_loops.txt); other workloads: not captured
                     "traffic": PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 if (args.workload == "cfg2" and args.packets is None) else None,
                     "traffic_unit": "bytes per launch (94 M events: 64 B record + 4 B permutation entry + extinction gathers)",
                     "peak_source": "148 SM x 128 FP32 lanes x sm_max_mhz (%s)" % pk["source"],

@@ -75,3 +75,38 @@ def test_product_never_imports_oracle():
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2110_15640_b200" not in src and "from paper_2110_15640_b200" not in src
             assert "libgcmcrt.so" not in src and "csrc" not in src
+
+
+def test_header_is_plain_c_and_links(lib, tmp_path):
+    """include/gcmcrt.h compiles as C11 (no C++, no torch types), a C program links against libgcmcrt.so, the struct
+    sizes the C compiler sees are the ones the ctypes binding uses, and a call without a device fails with a status."""
+    import shutil
+    import subprocess
+    if shutil.which("gcc") is None:
+        pytest.skip("no gcc")
+    src = tmp_path / "client.c"
+    src.write_text(r'''
+#include <stdio.h>
+#include "gcmcrt.h"
+int main(void)
+{
+    gcmcrt_grid *g = NULL;
+    double r[2] = {1.0e6, 2.0e6}, th[2] = {0.0, 3.14159265358979323846}, ph[2] = {0.0, 6.28318530717958647692};
+    float T[1] = {1000.0f}, rho[1] = {1.0f};
+    int rc = gcmcrt_grid_create(&g, 1, 1, 1, r, th, ph, T, rho, NULL, NULL, NULL, 0.0, 0.0f, NULL);
+    printf("%zu %zu %zu %d %s\n", sizeof(gcmcrt_run_params), sizeof(gcmcrt_result), sizeof(gcmcrt_counters), rc,
+           gcmcrt_version());
+    if (g) gcmcrt_destroy(g);
+    return 0;
+}
+''')
+    exe = tmp_path / "client"
+    libdir = os.path.dirname(binding.LIB_PATH)
+    subprocess.run(["gcc", "-std=c11", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe),
+                    "-L", libdir, "-lgcmcrt", "-Wl,-rpath," + libdir], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True).stdout.split()
+    assert int(out[0]) == C.sizeof(binding.RunParams)
+    assert int(out[1]) == C.sizeof(binding.Result)
+    assert int(out[2]) == C.sizeof(binding.Counters)
+    assert int(out[3]) in (binding.OK, binding.E_CUDA)      # no device here: a status, not a crash or a CPU fallback
+    assert "sm_100a" in " ".join(out[4:])

@@ -801,3 +801,21 @@ def test_error_paths(gpu):
     bad_grid = dict(grid, r_edges=grid["r_edges"][::-1].copy())
     with pytest.raises(gpu.GcmcrtError):
         gpu.Grid(bad_grid)
+    # node tables: the axes must ascend in uniform steps, the option combinations must make sense
+    grid4, opac4, prm4 = wl.cfg4(nlon=6, nlat=4, nlev=8, n_chan=12, n_lines=5, packets=100)
+    with gpu.Grid(grid4) as G:
+        for bad in (dict(T_nodes=opac4["T_nodes"][::-1].copy()), dict(logp_nodes=opac4["logp_nodes"] ** 2)):
+            with pytest.raises(gpu.GcmcrtError) as e:
+                G.set_opacity_nodes(dict(opac4, **bad))
+            assert e.value.code == gpu.E_INVALID
+        with pytest.raises(gpu.GcmcrtError) as e:          # a failed set_opacity leaves the handle without tables
+            G.run_emission(prm4)
+        assert e.value.code == gpu.E_STATE
+        G.set_opacity_nodes(opac4)
+        for bad in (dict(forced_scatter=3), dict(forced_scatter=2), dict(forced_scatter=1, continuous_absorption=1),
+                    dict(roulette_w_min=0.1)):
+            with pytest.raises(gpu.GcmcrtError) as e:
+                G.run_emission(dict(prm4, scatter_on=1, **bad))
+            assert e.value.code == gpu.E_INVALID
+        r = G.run_emission(prm4)
+        assert np.all(np.isfinite(r["value"])) and r["counters"]["packets_stuck"] == 0

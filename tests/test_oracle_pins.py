@@ -639,6 +639,67 @@ def test_images_sum_to_flux(orc):
     assert im.sum() > 0 and im[:, :8].sum() > 0 and im[:, 8:].sum() > 0
 
 
+def _lambert_sphere_image(orc, star, obs, npix, n=200000):
+    R0, Rt = 1.0e7, 1.25e7
+    grid, opac = wl.uniform_medium(2, 3, 4, R0, Rt, 0.0, 0.0, surface_albedo=1.0)
+    prm = wl.default_params(packets_per_channel=n, seed=8, max_events=1, npix=npix, star_dir=star, obs_dir=[obs],
+                            n_threads=os.cpu_count() or 1)
+    res = orc.run_albedo(grid, opac, prm)
+    return res["image"][0, 0], res["flux_sum"][0, 0].sum(), R0, Rt
+
+
+def test_image_of_a_lambert_sphere_at_zero_phase(orc):
+    """Pin of image_pixel (C19) by a closed form.  Vacuum over a Lambert a = 1 sphere, star and observer in the same
+    direction: packets land uniformly per unit area of the disc seen from the star (= the sky plane), each peels
+    a mu / pi with mu = sqrt(1 - rho^2 / R_p0^2) (Eq. 3), so the image is the surface brightness
+    I(rho) ~ sqrt(1 - rho^2 / R_p0^2) inside rho < R_p0 and exactly 0 outside.  Expected pixel sums by midpoint
+    quadrature of that law over every pixel (written here; the oracle's frame is not used)."""
+    npix = 10
+    for obs in ([1.0, 0.0, 0.0], [0.36, -0.48, 0.8]):
+        im, total, R0, Rt = _lambert_sphere_image(orc, obs, obs, npix)
+        assert np.isclose(im.sum(), total, rtol=1e-12)
+        sub = 40
+        t = ((np.arange(npix * sub) + 0.5) / (npix * sub) * 2.0 - 1.0) * Rt
+        X, Y = np.meshgrid(t, t)                       # rows = Y (image[iy][ix])
+        I = np.sqrt(np.maximum(0.0, 1.0 - (X ** 2 + Y ** 2) / R0 ** 2))
+        exp = I.reshape(npix, sub, npix, sub).sum(axis=(1, 3))
+        exp *= total / exp.sum()
+        assert np.all(im[exp == 0.0] == 0.0)           # nothing outside the planet's disc
+        lit = exp > 0.01 * exp.sum()
+        assert lit.sum() >= 30
+        assert np.allclose(im[lit], exp[lit], rtol=0.05), np.abs(im[lit] / exp[lit] - 1).max()
+        # the law falls from the centre to the limb: the four central pixels are the brightest
+        c = npix // 2
+        assert im[c - 1:c + 1, c - 1:c + 1].min() > im[lit].mean()
+
+
+def test_image_axes_orientation_at_quadrature(orc):
+    """Pin of the image frame (C19: e_x = z^ x o^ normalised, e_y = o^ x e_x; pixel row = Y, column = X).  With the
+    star 90 degrees from the observer exactly one half of a Lambert sphere is lit, and which half follows from the
+    geometry alone: star along +e_x lights X > 0 (columns npix/2 ..), star along +e_y lights Y > 0 (rows npix/2 ..).
+    A mirrored axis, swapped axes or a transposed row / column index fails one of the four cases."""
+    npix = 8
+    h = npix // 2
+    cases = [
+        # observer,           star,               lit half
+        ([1.0, 0.0, 0.0], [0.0, 1.0, 0.0], "x+"),    # e_x = z^ x x^ = +y^
+        ([1.0, 0.0, 0.0], [0.0, -1.0, 0.0], "x-"),
+        ([1.0, 0.0, 0.0], [0.0, 0.0, 1.0], "y+"),    # e_y = x^ x y^ = +z^
+        ([0.6, 0.0, 0.8], [-0.8, 0.0, 0.6], "y+"),   # e_x = +y^, e_y = o^ x y^ = (-0.8, 0, 0.6)
+        ([0.6, 0.8, 0.0], [-0.8, 0.6, 0.0], "x+"),   # e_x = z^ x o^ = (-0.8, 0.6, 0)
+        ([0.6, 0.8, 0.0], [0.0, 0.0, -1.0], "y-"),   # e_y = o^ x e_x = +z^
+    ]
+    for obs, star, half in cases:
+        im, total, _, _ = _lambert_sphere_image(orc, star, obs, npix, n=40000)
+        assert total > 0 and np.isclose(im.sum(), total, rtol=1e-12)
+        lit, dark = {"x+": (im[:, h:], im[:, :h]), "x-": (im[:, :h], im[:, h:]),
+                     "y+": (im[h:, :], im[:h, :]), "y-": (im[:h, :], im[h:, :])}[half]
+        assert dark.sum() == 0.0 and lit.sum() > 0.0, (obs, star, half)
+        # the other axis is a symmetry axis of the scene
+        a, b = (im[:h, :].sum(), im[h:, :].sum()) if half[0] == "x" else (im[:, :h].sum(), im[:, h:].sum())
+        assert abs(a - b) < 0.05 * (a + b)
+
+
 # ----------------------------------------------------------------------------- Sect. 4.4-4.5: survival biasing, roulette
 @pytest.mark.parametrize("omega,roulette", [(0.5, None), (0.9, None), (0.9, (0.3, 0.5)), (0.99, (1e-2, 0.25))])
 def test_survival_biasing_and_roulette_keep_the_exact_semi_infinite_albedo(orc, omega, roulette):

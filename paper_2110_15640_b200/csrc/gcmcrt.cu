@@ -587,8 +587,14 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             CUDA_TRY(g, g->flights.ensure(size_t(g->sm_count) * occ_i * (kWaveThreads / 32) * kFlightFields * kStageSlots * sizeof(float)));
             if (!emission) {
                 const int ncol = g->nlat * g->nlon;
-                spl.c_fold = int(std::max<long long>(1, std::min<long long>(ncr, (long long)(g->ev_cap / std::max<size_t>(n_pkt, 1)) + 2)));
-                spl.nbins = (unsigned int)((long long)spl.c_fold * ncol * kLaunchTauBuckets);
+                // same bound as the event sort: channels a pass can span, and at most 2^25 bins (a run of many channels
+                // with few packets each folds the channels beyond the cap into the last slot, which only costs coherence)
+                const long long max_lbins = 1ll << 25;
+                const long long per_chan = (long long)ncol * kLaunchTauBuckets;
+                if (per_chan > max_lbins) return fail(g, GCMCRT_E_INVALID, "grid has too many columns for the launch-order sort");
+                spl.c_fold = int(std::max<long long>(1, std::min<long long>(std::min<long long>(ncr, max_lbins / per_chan),
+                                                                          (long long)(g->ev_cap / std::max<size_t>(n_pkt, 1)) + 2)));
+                spl.nbins = (unsigned int)((long long)spl.c_fold * per_chan);
                 spl.n_tiles = (spl.nbins + kScanTile - 1) / kScanTile;
                 CUDA_TRY(g, g->lkeys.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));
                 CUDA_TRY(g, g->lperm.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));

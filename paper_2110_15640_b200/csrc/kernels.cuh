@@ -1066,21 +1066,24 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
                 }
                 if (rc.contrib) {
                     // Sect. 6, Eq. 32: f per event cell, thermal and scattered apart.  The lanes are sorted by
-                    // (channel, cell), so the lanes of one cell are neighbours: sum each run with a segmented shuffle
-                    // reduction (both components at once) and let its first lane do the atomics.
+                    // (channel, cell group), so the lanes of one cell are mostly neighbours: sum each RUN of consecutive
+                    // lanes with the same (channel, cell) with a segmented shuffle reduction (both components at once) and
+                    // let the run's first lane do the atomics.  A merge never reaches across a run boundary, so a cell
+                    // whose lanes are not contiguous (coarse sort keys, channels folded into one bin) is simply several runs.
                     const unsigned ckey = have ? unsigned((ck * gs.nlat + cj) * gs.nlev + ci) : 0xffffffffu;
                     const float f = st == RAY_ESCAPE ? pref * expf(-tau) : 0.f;
                     float v0 = kind == EV_EMIT ? f : 0.f, v1 = kind == EV_EMIT ? 0.f : f;
+                    const unsigned kp = __shfl_up_sync(kFullMask, ckey, 1);
+                    const int cp = __shfl_up_sync(kFullMask, chan, 1);
+                    const unsigned heads = __ballot_sync(kFullMask, lane_id() == 0 || kp != ckey || cp != chan);
+                    const unsigned after = lane_id() < 31 ? heads >> (lane_id() + 1) : 0u;
+                    const int run_end = after ? lane_id() + __ffs(after) : 32;   // first lane of the next run
 #pragma unroll
                     for (int off = 1; off < 32; off <<= 1) {
                         const float w0 = __shfl_down_sync(kFullMask, v0, off), w1 = __shfl_down_sync(kFullMask, v1, off);
-                        const unsigned kk = __shfl_down_sync(kFullMask, ckey, off);
-                        const int cc = __shfl_down_sync(kFullMask, chan, off);
-                        if (lane_id() + off < 32 && kk == ckey && cc == chan) { v0 += w0; v1 += w1; }
+                        if (lane_id() + off < run_end) { v0 += w0; v1 += w1; }
                     }
-                    const unsigned kp = __shfl_up_sync(kFullMask, ckey, 1);
-                    const int cp = __shfl_up_sync(kFullMask, chan, 1);
-                    if (have && (lane_id() == 0 || kp != ckey || cp != chan)) {
+                    if (have && ((heads >> lane_id()) & 1u)) {
                         float* dst = rc.contrib + ((size_t)chan * rc.n_obs_total + rc.obs_first + obs) * 2 * rc.geom.ncell + ckey;
                         if (v0 != 0.f) atomicAdd(dst, v0);
                         if (v1 != 0.f) atomicAdd(dst + rc.geom.ncell, v1);

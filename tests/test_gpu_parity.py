@@ -116,10 +116,68 @@ def test_ray_tau_matches_oracle(gpu, orc, shape):
             # the fp32 running distance u (<= 1.1e8 m) is quantised to 4-8 m, so one chord
             # of length L carries a relative error of ~4 m / L; tau is dominated by one high-kappa cell whose chord
             # is < 4e4 m for ~1 % and < 4e3 m for ~0.1 % of random rays (layers are 1.75e5 m thick)
+            # (test_ray_tau_radial_grid_within_the_fp32_bound_of_every_ray checks the same error model ray by ray)
             q = np.quantile(rel, [0.5, 0.99, 0.999, 1.0])
-            assert q[1] < 1e-4 and q[2] < 1e-3, q
-            assert q[0] < 5e-6, q
-            assert rel.max() < 5e-2
+            assert q[1] < 1e-4 and q[2] < 6e-4, q
+            assert q[0] < 3e-6, q
+            assert rel.max() < 5e-2                  # a ray that leaves the grid after a few hundred metres: 8 m of it
+            # what the flux sees: e^-tau of a peel-off ray
+            assert np.abs(np.exp(-tg[m]) - np.exp(-to[m])).max() < 1e-3
+
+
+def test_ray_tau_radial_grid_within_the_fp32_bound_of_every_ray(gpu):
+    """The marcher's error model, checked ray by ray against the closed form on a radial grid
+    (SURVEY.md P3): with d^2 = |p x n|^2 the shells are crossed at u_k = -/+ sqrt(R_k^2 - d^2), and
+    tau = sum alpha_cell (u_next - u_prev).  The GPU carries u in fp32, so every crossing (and the start p.n) sits within
+    delta = 2^-22 max|u| (two ulps: 26 m at 1.1e8 m) of its exact place; moving a crossing by delta changes tau by
+    delta |alpha_after - alpha_before|, so  |tau_gpu - tau| <= delta (alpha_first + alpha_last + sum |d alpha|) +
+    2^-22 n_seg tau.  Every one of 20000 random rays must satisfy its own bound (a skipped or repeated cell misses it by
+    four orders of magnitude); rays that graze a shell within delta are compared on the hit flag only."""
+    grid, opac, _ = wl.cfg1(packets=10)
+    R = grid["r_edges"]
+    nlev = R.size - 1
+    rng = np.random.default_rng(8)
+    pos, d = _rays(rng, 20000, R[0], R[-1])
+    pos32, d32 = pos.astype(np.float32), d.astype(np.float32)
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        chan = 3
+        tg, hg = G.ray_tau(chan, pos32, d32)
+    kext = (opac["k_abs"][chan] + opac["k_sca_ray"][chan]).reshape(nlev).astype(np.float64)
+    alpha = (grid["rho"].reshape(nlev) * kext.astype(np.float32)).astype(np.float64)   # the staged fp32 product
+    p = pos32.astype(np.float64)
+    n = d32.astype(np.float64)
+    n /= np.linalg.norm(n, axis=1)[:, None]
+    u0 = (p * n).sum(axis=1)
+    d2 = (np.cross(p, n) ** 2).sum(axis=1)
+    q = R[None, :] ** 2 - d2[:, None]                                   # [ray][shell]
+    root = np.sqrt(np.maximum(q, 0.0))
+    cross = np.concatenate([np.where(q > 0, -root, np.inf), np.where(q > 0, root, np.inf)], axis=1)
+    cross = np.where(cross > u0[:, None], cross, np.inf)              # crossings ahead of the start
+    hit = np.isfinite(cross[:, 0])                                      # shell 0 is met moving inward: the lower boundary
+    u_end = np.where(hit, cross[:, 0], root[:, nlev])
+    cross = np.where(cross < u_end[:, None], cross, np.inf)
+    cross.sort(axis=1)
+    pts = np.concatenate([u0[:, None], cross], axis=1)                  # start, crossings, then +inf
+    nxt = np.minimum(np.concatenate([cross, np.full((cross.shape[0], 1), np.inf)], axis=1), u_end[:, None])
+    live = np.isfinite(pts) & (pts < u_end[:, None])
+    mid = 0.5 * (np.where(live, pts, 0.0) + np.where(live, nxt, 0.0))
+    cell = np.clip(np.searchsorted(R, np.sqrt(d2[:, None] + mid ** 2), side="right") - 1, 0, nlev - 1)
+    a_seg = np.where(live, alpha[cell], 0.0)
+    tau = (a_seg * np.where(live, nxt - pts, 0.0)).sum(axis=1)
+    nseg = live.sum(axis=1)
+    jump = np.abs(np.diff(a_seg, axis=1)) * live[:, 1:]
+    a_last = np.take_along_axis(a_seg, np.maximum(nseg - 1, 0)[:, None], axis=1)[:, 0]
+    delta = 2.0 ** -22 * np.maximum(np.abs(u0), np.abs(u_end))
+    bound = delta * (a_seg[:, 0] + a_last + jump.sum(axis=1)) + 2.0 ** -22 * nseg * tau + 1e-30
+    # a ray that passes a shell closer than delta may or may not cross it in fp32: compare those on nothing but the flag
+    graze = (np.abs(np.sqrt(d2)[:, None] - R[None, :]) < 64.0).any(axis=1)
+    assert graze.mean() < 0.01
+    ok = ~graze
+    assert np.array_equal(hg[ok] == 1, hit[ok])
+    err = np.abs(tg.astype(np.float64) - tau)
+    assert np.all(err[ok] <= bound[ok]), (err[ok] / bound[ok]).max()
+    assert np.median(err[ok] / bound[ok]) > 1e-3                        # the bound is of the size of the error, not loose
 
 
 def test_ray_tau_edge_rays(gpu, orc):
@@ -162,7 +220,7 @@ def test_albedo_mixed_rayleigh_hg_and_surface(gpu, orc):
                             obs_dir=[[0.8, 0.0, 0.6], [0.0, 0.0, 1.0]])
     g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
     o = orc.run_albedo(grid, opac, dict(prm, n_threads=8), want_event_count=True)
-    _check_parity(orc, g, o, "albedo", min_same=0.97)   # ~7 events per packet: fp32/fp64 paths part more often
+    _check_parity(orc, g, o, "albedo")
     assert g["counters"]["packets_surface"] > 0
 
 
@@ -241,8 +299,8 @@ def test_doppler_parity_and_zero_wind_identity(gpu, orc):
     for k in ("flux_sum", "L_tot", "event_count"):
         o[k] = o[k][4:20]
     vo, so = orc.reduce(o, "emission")
-    assert np.all(np.abs(g["value"] - vo) <= 4 * so + 1e-4 * np.abs(vo))
-    assert np.allclose(g["L_tot"], o["L_tot"], rtol=1e-4)
+    assert np.all(np.abs(g["value"] - vo) <= 4 * so + 1e-5 * np.abs(vo))
+    assert np.allclose(g["L_tot"], o["L_tot"], rtol=1e-5)
     # zero winds + zero rotation: doppler_on changes nothing at all
     for k in ("u", "v", "w"):
         grid[k] = np.zeros_like(grid["T"])
@@ -504,7 +562,24 @@ def test_images_sum_to_flux_and_match_oracle(gpu, orc):
     g = _gpu_run(gpu, grid, opac, prm, "albedo")
     o = orc.run_albedo(grid, opac, prm)
     assert np.allclose(g["image"].sum(axis=(2, 3)), g["flux_sum"].sum(axis=2), rtol=1e-4)
-    assert np.allclose(g["image"], o["image"], rtol=0.05, atol=0.02 * o["image"].max())
+    # the same packets peel the same f into the same pixels: per pixel the bar is 4 sigma + 1e-5 relative with sigma the
+    # oracle's own Monte Carlo error of that pixel, estimated from 32 packet batches run one by one
+    nb = 32
+    per_batch = np.stack([orc.run_albedo(grid, opac, dict(prm, pkt_begin=b * 625, pkt_end=(b + 1) * 625))["image"]
+                          for b in range(nb)])
+    assert np.allclose(per_batch.sum(axis=0), o["image"], rtol=1e-9, atol=1e-12 * o["image"].max())
+    sig_pix = per_batch.std(axis=0, ddof=1) * np.sqrt(nb)
+    assert np.all(np.abs(g["image"] - o["image"]) <= 4 * sig_pix + 1e-5 * np.abs(o["image"]) + 1e-6 * o["image"].max())
+    assert np.abs(g["image"] - o["image"]).max() < 2e-3 * o["image"].max()     # and in fact far closer than the noise
+
+
+def _oracle_cell_sigma(orc, grid, opac, prm, nb):
+    """Monte Carlo error of the oracle's per-cell Eq. 32 sums: the packets run as nb sub-ranges, sigma = std * sqrt(nb)."""
+    N = int(prm["packets_per_channel"])
+    edges = [b * N // nb for b in range(nb + 1)]
+    parts = np.stack([orc.run_emission(grid, opac, dict(prm, pkt_begin=edges[b], pkt_end=edges[b + 1], n_threads=os.cpu_count() or 1),
+                                       want_contrib=True)["contrib"] for b in range(nb)])
+    return parts.std(axis=0, ddof=1) * np.sqrt(nb)
 
 
 def test_contribution_functions_match_oracle(gpu, orc):
@@ -516,11 +591,12 @@ def test_contribution_functions_match_oracle(gpu, orc):
         g = G.run_emission(prm, want_contrib=ncell)
     o = orc.run_emission(grid, opac, dict(prm, n_threads=1), want_contrib=True)
     assert np.allclose(g["contrib"].sum(axis=(2, 3)), g["flux_sum"].sum(axis=2), rtol=2e-4)
+    sig_cell = _oracle_cell_sigma(orc, grid, opac, prm, 16)
+    # every cell of every (channel, observer, component) on the stated bar, sigma the oracle's own error of that cell
+    assert np.all(np.abs(g["contrib"] - o["contrib"]) <= 4 * sig_cell + 1e-5 * o["contrib"] + 1e-7 * o["contrib"].max())
     for comp in (0, 1):
         cg, co = g["contrib"][:, :, comp], o["contrib"][:, :, comp]
         assert np.allclose(cg.sum(axis=2), co.sum(axis=2), rtol=2e-3, atol=1e-4 * co.sum(axis=2).max())
-        big = co > 0.02 * co.max()                 # cells that carry the signal: same packets, same streams
-        assert np.allclose(cg[big], co[big], rtol=2e-2)
         cf_g, cf_o = cg / cg.sum(axis=2, keepdims=True), co / co.sum(axis=2, keepdims=True)      # Eq. 32
         assert np.abs(cf_g - cf_o).max() < 2e-3
     grid, opac, prm = wl.cfg2(nlon=8, nlat=4, nlev=12, nbands=1, ng=3, packets=20000)
@@ -529,6 +605,35 @@ def test_contribution_functions_match_oracle(gpu, orc):
         a = G.run_albedo(prm, want_contrib=ncell)
     assert a["contrib"][:, :, 0].sum() == 0.0
     assert np.allclose(a["contrib"][:, :, 1].sum(axis=2), a["flux_sum"].sum(axis=2), rtol=2e-4)
+
+
+@pytest.mark.parametrize("case", ["multi_pass", "sparse", "sparse_multi_pass"])
+def test_contribution_functions_partition_the_flux_when_cells_are_not_contiguous(gpu, orc, monkeypatch, case):
+    """Eq. 32 sums are taken per run of equal (channel, cell) lanes in the sorted event order.  Two situations make the
+    lanes of one cell non-contiguous: a small event buffer (many passes: resumed packets of earlier channels share the
+    first channel's bins) and fewer than two packets per cell (the sort key is then a group of levels or a whole
+    column).  In both the per-cell sums must still partition the flux and match the oracle's cell by cell."""
+    if case == "multi_pass":
+        grid, opac, prm = wl.cfg3(nlon=8, nlat=4, nlev=12, nbands=2, ng=3, packets=20000, n_obs=2)
+        monkeypatch.setenv("GCMCRT_EVENT_CAP", "9000")
+    else:
+        grid, opac, prm = wl.cfg3(nlon=16, nlat=8, nlev=24, nbands=1, ng=3, packets=3000 if case == "sparse" else 1500, n_obs=2)
+        if case == "sparse_multi_pass":
+            monkeypatch.setenv("GCMCRT_EVENT_CAP", "1500")
+    ncell = grid["T"].size
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        g = G.run_emission(prm, want_contrib=ncell)
+        a = G.run_albedo(dict(prm, obs_dir=prm["obs_dir"][:1]), want_contrib=ncell)
+    if "multi_pass" in case:
+        assert g["counters"]["passes"] > 3
+    o = orc.run_emission(grid, opac, dict(prm, n_threads=os.cpu_count() or 1), want_contrib=True)
+    tot_g = g["contrib"].sum(axis=(2, 3))
+    assert np.allclose(tot_g, g["flux_sum"].sum(axis=2), rtol=2e-4)          # the double count would break this
+    assert np.allclose(a["contrib"][:, :, 1].sum(axis=2), a["flux_sum"].sum(axis=2), rtol=2e-4)
+    sig_cell = _oracle_cell_sigma(orc, grid, opac, prm, 16)
+    assert np.all(np.abs(g["contrib"] - o["contrib"]) <= 4 * sig_cell + 1e-5 * o["contrib"] + 1e-7 * o["contrib"].max())
+    assert (o["contrib"] > 0).sum() > 100
 
 
 def test_transmission_matches_oracle(gpu, orc):
@@ -563,7 +668,7 @@ def test_transmission_matches_oracle(gpu, orc):
         g4 = G.run_transmission(prm4)
     o4 = orc.run_transmission(grid4, opac4, prm4)
     v4, s4 = orc.reduce(o4, "transmission")
-    assert np.all(np.abs(g4["value"] - v4) <= 4 * s4 + 1e-4 * np.abs(v4))
+    assert np.all(np.abs(g4["value"] - v4) <= 4 * s4 + 1e-5 * np.abs(v4))
 
 
 def test_full_size_cfg2_sampled_packets_and_invariants(gpu, orc):
@@ -594,6 +699,18 @@ def test_full_size_cfg2_sampled_packets_and_invariants(gpu, orc):
     # cell), so less light reaches the absorbing lower boundary and more is reflected
     band0 = val[:16, 0]
     assert band0[-1] > band0[0]
+    # one whole band (16 g-ordinates) at the full packet count against the oracle: the stated bar on the spectrum and on
+    # the per-packet event counts of all 1.6e7 packets
+    b0, b1 = 80, 96
+    band = {k: (np.ascontiguousarray(v[b0:b1]) if isinstance(v, np.ndarray) and v.shape[:1] == (n_chan,) else v)
+            for k, v in opac.items()}
+    band["chan0"] = b0
+    ob = orc.run_albedo(grid, band, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
+    vb, sb = orc.reduce(ob, "albedo")
+    assert np.all(np.abs(val[b0:b1] - vb) <= 4 * sb + 1e-5 * np.abs(vb)), (np.abs(val[b0:b1] - vb) / (4 * sb + 1e-5 * np.abs(vb))).max()
+    assert np.allclose(sig[b0:b1], sb, rtol=0.1)
+    same = (evc[b0:b1].cpu().numpy().astype(np.uint32) == ob["event_count"]).mean()
+    assert same >= 0.99, same
     chans, n_s = [0, 77, 175], 1500
     for ch in chans:
         one = {k: (np.ascontiguousarray(v[ch:ch + 1]) if isinstance(v, np.ndarray) and v.shape[:1] == (n_chan,) else v)
@@ -636,6 +753,21 @@ def test_full_size_cfg3_sampled_packets_and_invariants(gpu, orc):
     assert val.shape == (n_chan, 8) and np.all(val > 0) and np.all(np.isfinite(sig))
     # the dayside (orbital phase 0.5, observer index 4) is the brightest view of every channel, the nightside the faintest
     assert np.all(val.argmax(axis=1) == 4) and np.all(val.argmin(axis=1) == 0)
+    # one whole band (16 g-ordinates) at the full packet count against the oracle, all 8 phases
+    b0, b1 = 32, 48
+    band = {k: (np.ascontiguousarray(v[b0:b1]) if isinstance(v, np.ndarray) and v.shape[:1] == (n_chan,) else v)
+            for k, v in opac.items()}
+    band["chan0"] = b0
+    ob = orc.run_emission(grid, band, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
+    vb, sb = orc.reduce(ob, "emission")
+    assert np.all(np.abs(val[b0:b1] - vb) <= 4 * sb + 1e-5 * np.abs(vb)), (np.abs(val[b0:b1] - vb) / (4 * sb + 1e-5 * np.abs(vb))).max()
+    # batch-means sigma: the same batches of the same packets; where a few bright packets make the variance (night side,
+    # opaque g-ordinates) one packet whose emission cell differs on the two sides moves it
+    ratio = sig[b0:b1] / sb
+    assert np.median(np.abs(ratio - 1)) < 0.02 and np.all((ratio > 0.5) & (ratio < 2.0)), (ratio.min(), ratio.max())
+    assert np.allclose(ltot[b0:b1], ob["L_tot"], rtol=1e-5)
+    same = (evc[b0:b1].cpu().numpy().astype(np.uint32) == ob["event_count"]).mean()
+    assert same >= 0.99, same
     for ch in (0, 77, 175):
         one = {k: (np.ascontiguousarray(v[ch:ch + 1]) if isinstance(v, np.ndarray) and v.shape[:1] == (n_chan,) else v)
                for k, v in opac.items()}
@@ -664,21 +796,32 @@ def test_opacity_from_node_tables_matches_per_cell_tables(gpu, orc):
         node0 = G.run_emission(dict(prm, doppler_on=0), want_event_count=True)
     assert (cell["event_count"] == node["event_count"]).mean() > 0.999
     assert np.allclose(cell["L_tot"], node["L_tot"], rtol=2e-5)
-    assert (np.abs(cell["value"] / node["value"] - 1) > 1e-4).sum() <= 8     # of 80; see the comment on `bad` below
     # the oracle runs on its own fp64 interpolation of the node tables (oracle.interp_nodes, rounded to the fp32 ABI)
     k_orc = orc.interp_nodes(opac["node_kabs"], opac["T_nodes"], opac["logp_nodes"], grid["T"], opac["p_cell"])
     assert np.allclose(k_orc, opac["k_abs"], rtol=1e-5)
-    o = orc.run_emission(grid, dict(opac, k_abs=k_orc.astype(np.float32)), dict(prm, n_threads=os.cpu_count() or 1),
-                         want_event_count=True)
-    vo, so = orc.reduce(o, "emission")
-    # the device interpolates in fp32: k_abs differs from the oracle's in the last bits, which can move the CDF draw of
-    # a few packets in 1e6 to the neighbouring cell (2 of 480 000 here); in a line core a single packet can carry most
-    # of a channel's flux (DESIGN.md Tolerances), so a few of the 80 values may sit outside the bar
-    bad = np.abs(node["value"] - vo) > 4 * so + 1e-5 * np.abs(vo)
-    assert bad.sum() <= 4
-    assert np.median(np.abs(node["value"] - vo) / np.abs(vo)) < 1e-3
+    opac_o = dict(opac, k_abs=k_orc.astype(np.float32))
+    o = orc.run_emission(grid, opac_o, dict(prm, n_threads=os.cpu_count() or 1), want_event_count=True)
     assert (node["event_count"] == o["event_count"]).mean() >= 0.99
     assert np.allclose(node["L_tot"], o["L_tot"], rtol=2e-5)
+    vo, so = orc.reduce(o, "emission")
+    assert np.median(np.abs(node["value"] - vo) / np.abs(vo)) < 1e-3
+    # The flux bar.  The device interpolates k_abs in fp32, the oracle in fp64: the last bits of L_i differ, which moves
+    # the CDF draw (Eq. 13) of a few packets in 1e6 to the neighbouring cell.  Under the unbiased draw a line-core
+    # channel gets nearly all its flux from a handful of packets emitted in the thin upper cells, so one moved packet
+    # can shift the channel by more than a batch-means sigma that never saw such a packet -- the situation the paper's
+    # composite emission bias (Sect. 4.3) exists for.  With xi = 0.5 half of the packets are drawn uniformly over the
+    # cells, sigma is a valid error estimate, and every one of the 80 (channel, observer) values must meet the bar,
+    # device node tables against device per-cell tables and against the oracle.
+    pb = dict(prm, emission_bias=0.5)
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        cell_b = G.run_emission(pb)
+        G.set_opacity_nodes(opac)
+        node_b = G.run_emission(pb)
+    ob = orc.run_emission(grid, opac_o, dict(pb, n_threads=os.cpu_count() or 1))
+    vb, sb = orc.reduce(ob, "emission")
+    assert np.all(np.abs(node_b["value"] - vb) <= 4 * sb + 1e-5 * np.abs(vb)), (np.abs(node_b["value"] - vb) / (4 * sb + 1e-5 * np.abs(vb))).max()
+    assert np.all(np.abs(cell_b["value"] - node_b["value"]) <= 4 * sb + 1e-5 * np.abs(vb))
     assert not np.allclose(node0["value"], node["value"], rtol=1e-3)          # the winds do shift the lines
     # streaming in wavelength batches (config 5): a batch carries W halo channels on each side for the Doppler window
     W, nb_ = 3, 16
@@ -738,11 +881,11 @@ def test_degenerate_cases_match_oracle(gpu, orc):
     assert np.allclose(one["flux_sum"][0], allc["flux_sum"][4], rtol=1e-6)
 
 
-def test_full_grid_cfg4_doppler_batch_sums_against_oracle(gpu, orc):
+def test_full_grid_cfg4_doppler_against_oracle(gpu, orc):
     """BASELINE config 4 on its full grid with its packet count (64 of the 1e4 wavelength points; 1e5 packets each;
-    Doppler-shifted emission, no scattering), launched as bench.py --workload cfg4 does: L_tot of every channel and the
-    flux of the first packet batch (packets 0..3124: the same packets on both sides, by the counter-based streams) of
-    five channels against oracle runs on the channel's Doppler window."""
+    Doppler-shifted emission, no scattering), launched as bench.py --workload cfg4 does: L_tot of every compared channel
+    and the spectrum of six channels at the full packet count against oracle runs on each channel's Doppler window --
+    |delta| <= 4 sigma + 1e-5 relative, no exceptions."""
     import torch
     grid, opac, prm = wl.cfg4(n_chan=64, packets=100000)
     n_chan, N, W = 64, 100000, int(prm["doppler_halfwidth"])
@@ -750,23 +893,63 @@ def test_full_grid_cfg4_doppler_batch_sums_against_oracle(gpu, orc):
     with gpu.Grid(grid) as G:
         G.set_opacity(dev)
         g = G.run_emission(prm, device_outputs=True)
-    flux = g["flux_sum"].cpu().numpy(); ltot = g["L_tot"].cpu().numpy().reshape(n_chan, -1)
+    val = g["value"].cpu().numpy().reshape(n_chan); ltot = g["L_tot"].cpu().numpy().reshape(n_chan)
     c = g["counters"]
     assert c["events"] == c["rays_peel"] and c["events"] <= n_chan * N and c["packets_stuck"] == 0
-    n_b0 = N // 32
-    bad = 0
-    for ch in (5, 20, 33, 47, 58):
+    for ch in (5, 12, 20, 33, 47, 58):
         lo, hi = ch - W, ch + W + 1
         sub = dict(opac, chan0=lo, k_abs=np.ascontiguousarray(opac["k_abs"][lo:hi]))
         sub["lambda"] = opac["lambda"][lo:hi]
-        o = orc.run_emission(grid, sub, dict(prm, pkt_begin=0, pkt_end=n_b0, n_threads=os.cpu_count() or 1))
-        assert abs(ltot[ch, 0] / o["L_tot"][W] - 1) < 2e-5
-        ref = o["flux_sum"][W, 0, 0]
-        # fp32 ray integrals against fp64: a few 1e-4; a packet whose CDF draw lands in the neighbouring cell on one
-        # side can move a batch sum by more (DESIGN.md Tolerances), so one of the five may
-        if abs(flux[ch, 0, 0] / ref - 1) > 2e-3:
-            bad += 1
-    assert bad <= 1
+        o = orc.run_emission(grid, sub, dict(prm, n_threads=os.cpu_count() or 1))
+        vo, so = orc.reduce(o, "emission")
+        assert abs(ltot[ch] / o["L_tot"][W, 0] - 1) < 1e-5
+        assert abs(val[ch] - vo[W, 0]) <= 4 * so[W, 0] + 1e-5 * abs(vo[W, 0]), (ch, val[ch], vo[W, 0], so[W, 0])
+
+
+def test_cfg5_at_size_streamed_node_batch_against_oracle(gpu, orc):
+    """BASELINE config 5 at its size (configs[4]): the 128 x 64 x 100 grid, one streamed wavelength
+    batch -- 8 wavelength points plus the 4 halo points of the Doppler window on each side, handed over as (T, log p) node
+    tables through gcmcrt_set_opacity_nodes with the batch's first global channel index as chan0 -- Doppler shifts and
+    Rayleigh scattering on, emission and albedo toward the 4 orbital phases, 1e5 packets per wavelength: the option
+    combination and launch sequence of bench.py --workload cfg5.  Every (wavelength, phase) value of both modes against
+    the oracle (which is given the per-cell table of the same 16 points) on the stated bar, L_tot, and the per-packet
+    event counts of the first phase's run."""
+    W, n_run = 4, 8
+    n_tab = n_run + 2 * W
+    grid, opac, prm = wl.cfg5(n_chan=n_tab, packets=100000, n_lines=12)
+    ncell = grid["T"].size
+    assert grid["T"].shape == (128, 64, 100) and prm["obs_dir"].shape == (4, 3) and prm["doppler_on"] == 1 and prm["scatter_on"] == 1
+    chan0 = 2044                                     # the batch that runs global channels 2048 .. 2055
+    k_ray = np.ascontiguousarray(np.broadcast_to(opac["k_ray_chan"][:, None], (n_tab, ncell))).reshape((n_tab,) + grid["T"].shape)
+    sub = dict(opac, chan0=chan0, k_sca_ray=k_ray)
+    rng_c = dict(chan_begin=W, chan_end=W + n_run)
+    with gpu.Grid(grid) as G:
+        G.set_opacity_nodes(sub)
+        ge = G.run_emission(dict(prm, **rng_c), want_event_count=True)
+        ga = G.run_albedo(dict(prm, **rng_c), want_event_count=True)
+    assert ge["counters"]["packets_stuck"] == 0 and ga["counters"]["packets_stuck"] == 0
+    k_orc = orc.interp_nodes(opac["node_kabs"], opac["T_nodes"], opac["logp_nodes"], grid["T"], opac["p_cell"]).astype(np.float32)
+    oo = dict(chan0=chan0, k_abs=k_orc, k_sca_ray=k_ray)
+    oo["lambda"] = opac["lambda"]
+    ncpu = os.cpu_count() or 1
+    for mode, g, run in (("emission", ge, orc.run_emission), ("albedo", ga, orc.run_albedo)):
+        o = run(grid, oo, dict(prm, n_threads=ncpu), want_event_count=True)
+        for k in ("flux_sum", "L_tot", "event_count"):
+            o[k] = o[k][W:W + n_run]
+        vo, so = orc.reduce(o, mode)
+        tol = 4 * so + 1e-5 * np.abs(vo)
+        assert g["value"].shape == (n_run, 4)
+        assert np.all(np.abs(g["value"] - vo) <= tol), (mode, (np.abs(g["value"] - vo) / tol).max())
+        if mode == "emission":
+            assert np.allclose(g["L_tot"], o["L_tot"], rtol=2e-5)
+        same = (g["event_count"] == o["event_count"]).mean()
+        assert same >= 0.99, (mode, same)
+    # the Doppler shifts and the scattering do act at this size
+    with gpu.Grid(grid) as G:
+        G.set_opacity_nodes(sub)
+        g0 = G.run_emission(dict(prm, doppler_on=0, **rng_c))
+    assert not np.allclose(g0["value"], ge["value"], rtol=1e-3)
+    assert ge["counters"]["events"] > 4 * n_run * 100000
 
 
 @pytest.mark.parametrize("nlev", [100, 130])

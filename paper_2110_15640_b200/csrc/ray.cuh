@@ -245,6 +245,8 @@ __device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, f
 {
     const float ul = fminf(r.u_lat, r.u_lon);
     const float un = fminf(r.u_rad, ul);
+    // the clamp matters: a flight that starts on a cell face in a direction nearly tangent to it (the event position is
+    // rounded to fp32, 8 m at 1e8 m) can find the next roots kilometres behind its start point
     const float ds = fmaxf(un - r.u, 0.0f);
     const float tnew = fmaf(r.alpha, ds, tau);
     if (tnew >= tau_limit) {  // the limit is reached inside this cell
@@ -264,7 +266,9 @@ __device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, f
     if (DUAL) r.beta = r.beta_n;
     if (r.i == r.i_turn) r.rad_step = 1;   // the inner shell of this cell lies inside the impact parameter
     else r.ish += r.rad_step;              // (turning, the shell just crossed inward is the next one outward)
-    const float sq = sqrt_approx(fmaxf(shell_q(r, s, r.ish), 0.0f));
+    // no clamp: this shell lies a whole layer beyond the one just crossed (or is the shell just crossed inward, which
+    // the turn search found reachable with the same expression), so R_k^2 - d^2 > 0
+    const float sq = sqrt_approx(shell_q(r, s, r.ish));
     r.u_rad = __int_as_float(__float_as_int(sq) | (r.rad_step & 0x80000000));
     r.pn += DUAL ? 2 * r.rad_step : r.rad_step;   // also right at the turn: the prefetch pointed at this cell, the next one is one up
     if (DUAL) {
@@ -301,7 +305,6 @@ __device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, f
         "sub.f32 hi, hi, %10;\n\t"                                                                                     \
         "sub.f32 lo, lo, %11;\n\t"                                                                                     \
         "add.f32 q, hi, lo;\n\t"                                                                                       \
-        "max.f32 q, q, 0f00000000;\n\t"                                                                                \
         "sqrt.approx.ftz.f32 %1, q;\n\t" NEG                                                                           \
         "add.s32 n1, %7, 1;\n\t"                                                                                       \
         "setp.ge.s32 p, n1, %12;\n\t"                                                                                  \
@@ -318,7 +321,6 @@ __device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, f
         "sub.f32 hi, hi, %10;\n\t"                                                                                     \
         "sub.f32 lo, lo, %11;\n\t"                                                                                     \
         "add.f32 q, hi, lo;\n\t"                                                                                       \
-        "max.f32 q, q, 0f00000000;\n\t"                                                                                \
         "sqrt.approx.ftz.f32 %1, q;\n\t" NEG                                                                           \
         "add.s32 %6, %6, " #SSTEP2 ";\n\t"                                                                             \
         "add.s64 %5, %5, " #PSTEP2 ";\n\t"                                                                             \
@@ -379,7 +381,7 @@ __device__ __forceinline__ int ray_run(Ray& r, const GeomSmem& s, float& tau_io,
                     inward = false;
                     float hi, lo;
                     asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(hi), "=f"(lo) : "r"(sa));
-                    u_rad = sqrt_approx(fmaxf((hi - d2) + (lo - d2lo), 0.0f));
+                    u_rad = sqrt_approx((hi - d2) + (lo - d2lo));
                     ++pn;
                     alpha_n = __ldg(pn);
                 }

@@ -98,6 +98,9 @@ typedef struct gcmcrt_run_params {
                                     omega in the peel-off weight).  Packets end by escaping, at the lower boundary, at
                                     max_events, or by Russian roulette (survival_bias = 1 with roulette_w_min > 0).
                                     Runs through the persistent transport kernel; excludes forced_scatter. */
+    int timing;                  /* 0: the run is only enqueued (see STREAMS); the ms_* counters stay 0.
+                                    1: profiling run -- the pass loop is driven by the host, which waits for every pass
+                                    and records cudaEvents around its kernels to fill the ms_* counters */
 } gcmcrt_run_params;
 
 typedef struct gcmcrt_counters {
@@ -113,6 +116,9 @@ typedef struct gcmcrt_counters {
        launch (milliseconds, summed over passes / observers) */
     double ms_stage, ms_emission_cdf, ms_transport, ms_peel;
     double ms_sort;              /* counting sort of the event records by (channel, cell) before each peel pass */
+    uint64_t device_status;      /* 0 = the pass loop ran to its end; 1 = suspended-packet list overflow, 2 = pass limit
+                                    reached (both "cannot happen": the library sizes its buffers so); with host-resident
+                                    counters a non-zero value also makes the call return GCMCRT_E_CUDA */
 } gcmcrt_counters;
 
 /* Output buffers, all caller-owned, host|device, nullable unless stated. */

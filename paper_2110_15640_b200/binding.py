@@ -33,7 +33,8 @@ class RunParams(C.Structure):
                 ("doppler_halfwidth", C.c_int), ("emission_bias", C.c_double), ("tau_vert_max", C.c_double),
                 ("tau_cut", C.c_double), ("npix", C.c_int), ("n_batches", C.c_int),
                 ("survival_bias", C.c_int), ("roulette_w_min", C.c_double), ("roulette_survive", C.c_double),
-                ("star_radius", C.c_double), ("planet_xy", C.c_double * 2), ("ld_c1", C.c_double), ("ld_c2", C.c_double), ("cloud_phase", C.c_int), ("forced_scatter", C.c_int), ("continuous_absorption", C.c_int)]
+                ("star_radius", C.c_double), ("planet_xy", C.c_double * 2), ("ld_c1", C.c_double), ("ld_c2", C.c_double), ("cloud_phase", C.c_int), ("forced_scatter", C.c_int), ("continuous_absorption", C.c_int),
+                ("timing", C.c_int)]
 
 
 class Counters(C.Structure):
@@ -42,12 +43,12 @@ class Counters(C.Structure):
                 ("packets_stuck", C.c_uint64), ("escaped_weight", C.c_double), ("passes", C.c_uint64),
                 ("rays_peel", C.c_uint64), ("launches", C.c_uint64), ("ms_stage", C.c_double),
                 ("ms_emission_cdf", C.c_double), ("ms_transport", C.c_double), ("ms_peel", C.c_double),
-                ("ms_sort", C.c_double)]
+                ("ms_sort", C.c_double), ("device_status", C.c_uint64)]
 
 
 class Result(C.Structure):
     _fields_ = [("flux_sum", C.c_void_p), ("L_tot", C.c_void_p), ("value", C.c_void_p), ("sigma", C.c_void_p),
-                ("image", C.c_void_p), ("event_count", C.c_void_p), ("counters", C.POINTER(Counters)),
+                ("image", C.c_void_p), ("event_count", C.c_void_p), ("counters", C.c_void_p),
                 ("contrib", C.c_void_p)]
 
 
@@ -182,10 +183,22 @@ def make_params(prm):
     p.cloud_phase = int(prm.get("cloud_phase", 0))
     p.forced_scatter = int(prm.get("forced_scatter", 0))
     p.continuous_absorption = int(prm.get("continuous_absorption", 0))
+    p.timing = int(prm.get("timing", 0))
     return p, obs
 
 
-def _run(fn, handle, prm, n_chan_table, want_event_count, want_image, device_outputs, stream, want_contrib=0):
+def read_counters(dev_counters):
+    """The gcmcrt_counters struct a run wrote into device memory (counters="device"), as a dict.  Synchronises."""
+    raw = dev_counters.cpu().numpy().tobytes()
+    cnt = Counters.from_buffer_copy(raw)
+    return {name: getattr(cnt, name) for name, _ in Counters._fields_}
+
+
+def _run(fn, handle, prm, n_chan_table, want_event_count, want_image, device_outputs, stream, want_contrib=0,
+         counters="host"):
+    """counters: "host" (dict in out["counters"]; the call waits for the device), "device" (out["counters_dev"]: a byte
+    tensor holding the struct, read it with read_counters(); with device_outputs the call then only enqueues work), or
+    None."""
     p, keep = make_params(prm)
     N = p.packets_per_channel
     lo, hi = p.pkt_begin, (p.pkt_end or N)
@@ -213,29 +226,37 @@ def _run(fn, handle, prm, n_chan_table, want_event_count, want_image, device_out
     res = Result()
     for k in ("flux_sum", "L_tot", "value", "sigma", "image", "event_count", "contrib"):
         setattr(res, k, _ptr(out[k]) if k in out else None)
-    res.counters = C.pointer(cnt)
+    if counters == "device":
+        import torch
+        out["counters_dev"] = torch.zeros(C.sizeof(Counters), dtype=torch.uint8, device="cuda")
+        res.counters = out["counters_dev"].data_ptr()
+    elif counters == "host":
+        res.counters = C.addressof(cnt)
+    else:
+        res.counters = None
     rc = fn(handle, C.byref(p), C.byref(res), _stream_ptr(stream))
     _check(handle, rc)
-    out["counters"] = {name: getattr(cnt, name) for name, _ in Counters._fields_}
+    if counters == "host":
+        out["counters"] = {name: getattr(cnt, name) for name, _ in Counters._fields_}
     out["n_batches"], out["packets_per_channel"], out["pkt_range"] = nb, N, (lo, hi)
     del keep
     return out
 
 
 def run_albedo(handle, prm, n_chan_table, want_event_count=False, want_image=True, device_outputs=False, stream=None,
-               want_contrib=0):
+               want_contrib=0, counters="host"):
     return _run(lib().gcmcrt_run_albedo, handle, prm, n_chan_table, want_event_count, want_image, device_outputs, stream,
-                want_contrib)
+                want_contrib, counters)
 
 
 def run_emission(handle, prm, n_chan_table, want_event_count=False, want_image=True, device_outputs=False, stream=None,
-                 want_contrib=0):
+                 want_contrib=0, counters="host"):
     return _run(lib().gcmcrt_run_emission, handle, prm, n_chan_table, want_event_count, want_image, device_outputs, stream,
-                want_contrib)
+                want_contrib, counters)
 
 
-def run_transmission(handle, prm, n_chan_table, device_outputs=False, stream=None):
-    return _run(lib().gcmcrt_run_transmission, handle, prm, n_chan_table, False, False, device_outputs, stream)
+def run_transmission(handle, prm, n_chan_table, device_outputs=False, stream=None, counters="host"):
+    return _run(lib().gcmcrt_run_transmission, handle, prm, n_chan_table, False, False, device_outputs, stream, 0, counters)
 
 
 def debug_ray_tau(handle, chan, pos, dirs, stream=None):

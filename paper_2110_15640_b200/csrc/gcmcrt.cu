@@ -34,18 +34,6 @@ struct DevBuf {  // owned device allocation
     template <class T> T* as() const { return static_cast<T*>(p); }
 };
 
-constexpr int kMaxGen = 30;
-
-struct PassCtrl {  // small device block reset every pass
-    unsigned int ev_count;
-    unsigned int susp_count[2];
-    unsigned int susp_taken[2];
-    unsigned int pad;
-    unsigned long long work_counter;
-    unsigned long long ray_counter;
-    unsigned int gen_mark[kMaxGen + 2];   // event-buffer offsets of the wavefront generations of this pass
-};
-
 }  // namespace
 
 struct gcmcrt_grid {
@@ -80,7 +68,7 @@ struct gcmcrt_grid {
     DevBuf Lcell, Lcum, Ltot, guide;
 
     // workspace
-    DevBuf ev0, evkeys, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, flights, s0[2], s1[2], s2[2], ctrl, counters, flux, ltot_out, value, sigma, image, evcount, contrib;
+    DevBuf ev0, evkeys, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, flights, s0[2], s1[2], s2[2], ctrl, counters, counters_out, flux, ltot_out, value, sigma, image, evcount, contrib;
     unsigned int ev_cap = 0, ev_cap_forced = 0;
     bool tuned = false;   // environment overrides read
     int n_threads_resident = 0;
@@ -88,7 +76,8 @@ struct gcmcrt_grid {
     // a cone / half-plane before a warp serves them; wavefront generations per pass before the persistent kernel takes over
     // (0 = persistent kernel only); first-pass batch = event capacity / batch_div
     int tune[4] = {16, 1, 8, 4};
-    PassCtrl* h_ctrl = nullptr;  // pinned
+    PassCtrl* h_ctrl = nullptr;  // pinned (timed runs read the pass outcome back)
+    cudaStream_t cap_stream = nullptr;   // the body of the pass loop is captured on this stream into the WHILE node's graph
     cudaEvent_t tev[4] = {nullptr, nullptr, nullptr, nullptr};   // kernel timing (A0 | A2 | transport | peel)
     unsigned long long launches = 0, launches_pending = 0;
     double ms_stage = 0.0, ms_emis = 0.0, ms_transport = 0.0, ms_peel = 0.0, ms_sort = 0.0;
@@ -185,7 +174,7 @@ cudaError_t ensure_events(gcmcrt_grid* g)
 }
 
 // Stage alpha / prop for observer `obs_dir` (nullptr = unshifted table).
-int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStream_t s, bool cont = false)
+int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStream_t s, bool cont = false, bool timed = false)
 {
     const size_t n = size_t(g->n_chan) * g->ncell;
     const GeomParams gp0 = geom_params(g);
@@ -212,8 +201,10 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
     sp.alpha_stride = gp0.alpha_stride; sp.col_stride = gp0.col_stride;
     sp.doppler = obs_dir != nullptr; sp.halfwidth = halfwidth;
     sp.vlos = nullptr; sp.reff = g->reff.as<float>();
-    CUDA_TRY(g, ensure_events(g));
-    CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
+    if (timed) {
+        CUDA_TRY(g, ensure_events(g));
+        CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
+    }
     if (obs_dir) {
         CUDA_TRY(g, g->vlos.ensure(size_t(g->ncell) * sizeof(float)));
         float o[3];
@@ -233,9 +224,9 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
     }
     CUDA_TRY(g, cudaGetLastError());
     ++g->launches;
-    CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
-    CUDA_TRY(g, cudaEventSynchronize(g->tev[1]));
-    {
+    if (timed) {
+        CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
+        CUDA_TRY(g, cudaEventSynchronize(g->tev[1]));
         float ms = 0.f;
         CUDA_TRY(g, cudaEventElapsedTime(&ms, g->tev[0], g->tev[1]));
         g->ms_stage_pending += ms;
@@ -298,6 +289,156 @@ int bind_out(gcmcrt_grid* g, void* user, size_t bytes, DevBuf& own, OutBuf& ob, 
     return GCMCRT_OK;
 }
 
+// Everything one pass launches.  It is the same for every pass of a run: what changes from pass to pass (fresh packet
+// range, which suspended list is read, the sort key window, the counters) lives in PassCtrl on the device.
+struct PassLaunch {
+    RunConst rc;
+    EventBuf ev;
+    SuspPair susp;
+    WaveConst wc;
+    SortParams sp, spl;
+    PassPlan plan;
+    PassCtrl* ctrl = nullptr;
+    bool emission = false, has_obs = false;
+    int n_gen = 0, n_gen_run = 0;
+    unsigned grid_t = 1, grid_f = 1, grid_i = 1, grid_p = 1, grid_k = 1;
+    size_t smem_t = 0, smem_w = 0, smem_i = 0, smem_p = 0;
+    decltype(&transport_kernel<4, false>) tk = nullptr;
+    decltype(&peel_kernel<16>) pk = nullptr;
+    decltype(&wave_first_flight_kernel<16, false>) k_first = nullptr;
+    decltype(&wave_interact_kernel<kInteractK, false>) k_inter = nullptr;
+    unsigned long long tail_items = 0;
+};
+
+// Enqueue one pass on `s` (the caller's stream in a timed run, the capture stream of the loop body otherwise).
+// tev != NULL: cudaEvents around the transport side, the event sort and the peel kernel.
+int enqueue_pass(gcmcrt_grid* g, const PassLaunch& L, cudaStream_t s, cudaEvent_t* tev, cudaGraphConditionalHandle handle,
+                 int use_handle, unsigned* n_launch)
+{
+    unsigned nl = 0;
+    PassCtrl* ctrl = L.ctrl;
+    pass_begin_kernel<<<1, 1, 0, s>>>(ctrl, L.plan);
+    ++nl;
+    if (tev) CUDA_TRY(g, cudaEventRecord(tev[0], s));
+    // the event sort's histogram is filled while the records are written
+    if (L.has_obs) CUDA_TRY(g, cudaMemsetAsync(L.sp.hist, 0, size_t(L.sp.nbins) * sizeof(unsigned int), s));
+    if (L.n_gen > 0) {
+        WaveConst wc = L.wc;
+        if (!L.emission) {
+            // launch-order sort of the fresh packets, then their first flights
+            CUDA_TRY(g, cudaMemsetAsync(L.spl.hist, 0, size_t(L.spl.nbins) * sizeof(unsigned int), s));
+            wave_launch_keys_kernel<<<L.grid_k, kWaveThreads, L.smem_w, s>>>(L.rc, wc);
+            scan_reduce_kernel<<<L.spl.n_tiles, kScanThreads, 0, s>>>(L.spl);
+            scan_tiles_kernel<<<1, 1024, 0, s>>>(L.spl);
+            scan_apply_kernel<<<L.spl.n_tiles, kScanThreads, 0, s>>>(L.spl);
+            ev_scatter_kernel<<<L.grid_k, 256, 0, s>>>(L.spl);
+            L.k_first<<<L.grid_f, kWaveThreads, L.smem_w, s>>>(L.rc, L.ev, L.susp, wc);
+            nl += 6;
+        } else {
+            wave_emit_kernel<<<L.grid_k, kWaveThreads, L.smem_w, s>>>(L.rc, L.ev, L.susp, wc);
+            nl += 1;
+        }
+        CUDA_TRY(g, cudaMemcpyAsync(&ctrl->gen_mark[1], &ctrl->ev_count, sizeof(unsigned int), cudaMemcpyDeviceToDevice, s));
+        for (int gi = 0; gi < L.n_gen_run; ++gi) {
+            wc.gen_mark = &ctrl->gen_mark[gi];
+            wc.park_all = gi == L.n_gen - 1;
+            L.k_inter<<<L.grid_i, kWaveThreads, L.smem_i, s>>>(L.rc, L.ev, L.susp, wc);
+            CUDA_TRY(g, cudaMemcpyAsync(&ctrl->gen_mark[gi + 2], &ctrl->ev_count, sizeof(unsigned int), cudaMemcpyDeviceToDevice, s));
+        }
+        nl += unsigned(L.n_gen_run);
+    }
+    L.tk<<<L.grid_t, kTransportThreads, L.smem_t, s>>>(L.rc, L.ev, L.susp, L.tail_items);
+    ++nl;
+    if (tev) CUDA_TRY(g, cudaEventRecord(tev[1], s));
+    if (L.has_obs) {
+        // counting sort of this pass's events by (channel, cell): sort.cuh
+        if (!L.ev.hist) { ev_hist_kernel<<<g->sm_count * 8, 256, 0, s>>>(L.sp); ++nl; }
+        scan_reduce_kernel<<<L.sp.n_tiles, kScanThreads, 0, s>>>(L.sp);
+        scan_tiles_kernel<<<1, 1024, 0, s>>>(L.sp);
+        scan_apply_kernel<<<L.sp.n_tiles, kScanThreads, 0, s>>>(L.sp);
+        ev_scatter_kernel<<<g->sm_count * 8, 256, 0, s>>>(L.sp);
+        nl += 4;
+    }
+    if (tev) CUDA_TRY(g, cudaEventRecord(tev[2], s));
+    if (L.has_obs) { L.pk<<<L.grid_p, kPeelThreads, L.smem_p, s>>>(L.rc, L.ev, L.sp.perm); ++nl; }
+    if (tev) CUDA_TRY(g, cudaEventRecord(tev[3], s));
+    pass_end_kernel<<<1, 1, 0, s>>>(ctrl, L.plan, handle, use_handle);
+    ++nl;
+    CUDA_TRY(g, cudaGetLastError());
+    if (n_launch) *n_launch = nl;
+    return GCMCRT_OK;
+}
+
+// The pass loop as a conditional WHILE node: the body is one pass, captured from enqueue_pass(); pass_end_kernel sets
+// the condition.  Nothing here waits for the device.  When the caller's stream is itself being captured the node is
+// added to the caller's graph (a graph that holds a conditional node cannot be a child graph); otherwise a graph of its
+// own is instantiated, launched on the caller's stream and released (an executable graph in flight is freed on completion).
+int launch_pass_loop(gcmcrt_grid* g, const PassLaunch& L, cudaStream_t s, unsigned* n_launch)
+{
+    if (!g->cap_stream) CUDA_TRY(g, cudaStreamCreateWithFlags(&g->cap_stream, cudaStreamNonBlocking));
+    cudaStreamCaptureStatus cst = cudaStreamCaptureStatusNone;
+    CUDA_TRY(g, cudaStreamIsCapturing(s, &cst));
+    cudaGraph_t graph = nullptr;
+    const cudaGraphNode_t* deps = nullptr;
+    size_t n_deps = 0;
+    const bool own = cst != cudaStreamCaptureStatusActive;
+    if (own) {
+        CUDA_TRY(g, cudaGraphCreate(&graph, 0));
+    } else {
+        unsigned long long id = 0;
+        CUDA_TRY(g, cudaStreamGetCaptureInfo(s, &cst, &id, &graph, &deps, &n_deps));
+    }
+    int rcode = GCMCRT_OK;
+    cudaGraphNode_t node = nullptr;
+    do {
+        cudaGraphConditionalHandle handle;
+        cudaError_t e = cudaGraphConditionalHandleCreate(&handle, graph, 1, cudaGraphCondAssignDefault);
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = handle;
+        np.conditional.type = cudaGraphCondTypeWhile;
+        np.conditional.size = 1;
+        if (e == cudaSuccess) e = cudaGraphAddNode(&node, graph, deps, n_deps, &np);
+        if (e == cudaSuccess) e = cudaStreamBeginCaptureToGraph(g->cap_stream, np.conditional.phGraph_out[0], nullptr, nullptr, 0,
+                                                               cudaStreamCaptureModeRelaxed);
+        if (e != cudaSuccess) { rcode = fail(g, GCMCRT_E_CUDA, std::string("pass loop graph: ") + cudaGetErrorString(e)); break; }
+        rcode = enqueue_pass(g, L, g->cap_stream, nullptr, handle, 1, n_launch);
+        cudaGraph_t body = nullptr;
+        e = cudaStreamEndCapture(g->cap_stream, &body);
+        if (rcode == GCMCRT_OK && e != cudaSuccess) rcode = fail(g, GCMCRT_E_CUDA, std::string("pass loop capture: ") + cudaGetErrorString(e));
+        if (rcode != GCMCRT_OK) break;
+        if (own) {
+            cudaGraphExec_t exec = nullptr;
+            e = cudaGraphInstantiate(&exec, graph, 0);
+            if (e == cudaSuccess) e = cudaGraphLaunch(exec, s);
+            if (exec) cudaGraphExecDestroy(exec);
+        } else {
+            e = cudaStreamUpdateCaptureDependencies(s, &node, 1, cudaStreamSetCaptureDependencies);
+        }
+        if (e != cudaSuccess) rcode = fail(g, GCMCRT_E_CUDA, std::string("pass loop launch: ") + cudaGetErrorString(e));
+    } while (0);
+    if (own && graph) cudaGraphDestroy(graph);
+    if (rcode != GCMCRT_OK) cudaGetLastError();
+    return rcode;
+}
+
+// The counters of the ABI, assembled on the device (so that a run with device outputs needs no host round trip).
+__global__ void finalize_counters_kernel(const DevCounters* dc, const PassCtrl* c, gcmcrt_counters* out, unsigned long long launches_fixed,
+                                         unsigned long long launches_per_pass, unsigned long long passes_extra, double ms_stage,
+                                         double ms_emis, double ms_transport, double ms_peel, double ms_sort)
+{
+    gcmcrt_counters hc;
+    hc.events = dc->events; hc.segments_transport = dc->seg_transport; hc.segments_peel = dc->seg_peel;
+    hc.packets_escaped = dc->escaped; hc.packets_absorbed = dc->absorbed; hc.packets_surface = dc->surface;
+    hc.packets_stuck = dc->stuck; hc.escaped_weight = dc->escaped_weight; hc.rays_peel = dc->rays_peel;
+    const unsigned long long passes = c ? c->passes : 0ull;
+    hc.passes = passes + passes_extra;
+    hc.launches = launches_fixed + launches_per_pass * passes;
+    hc.ms_stage = ms_stage; hc.ms_emission_cdf = ms_emis; hc.ms_transport = ms_transport; hc.ms_peel = ms_peel; hc.ms_sort = ms_sort;
+    hc.device_status = c ? (unsigned long long)c->error : 0ull;
+    *out = hc;
+}
+
 // mode: 0 albedo, 1 emission, 2 transmission
 int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, void* stream, int mode)
 {
@@ -326,6 +467,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     const int ncr = ce - cb;
     if (ncr > (1 << 24)) return fail(g, GCMCRT_E_INVALID, "too many channels in one run");
     const int npix = prm->npix > 0 && out->image ? prm->npix : 0;
+    const bool timed = prm->timing != 0;   // host-synchronous pass loop with cudaEvents around the kernels
 
     int rcode = ensure_workspace(g, (unsigned long long)ncr * (hi - lo));
     if (rcode) return rcode;
@@ -333,9 +475,11 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         return fail(g, GCMCRT_E_INVALID, "forced_scatter must be 0, 1 or 2 and excludes continuous_absorption");
     if (prm->forced_scatter == 2 && !(prm->max_events > 0 || (prm->survival_bias && prm->roulette_w_min > 0.0)))
         return fail(g, GCMCRT_E_INVALID, "forced_scatter = 2 needs max_events or Russian roulette to end its packets");
+    if (prm->cloud_phase < 0 || prm->cloud_phase > 2) return fail(g, GCMCRT_E_INVALID, "cloud_phase must be 0 (HG), 1 (TTHG) or 2 (Draine)");
+    if (mode == 2 && n_obs < 1) return fail(g, GCMCRT_E_INVALID, "transmission needs at least one observer direction");
 
     // ---- outputs
-    OutBuf o_flux, o_ltot, o_val, o_sig, o_img, o_evc, o_cnt, o_ctb;
+    OutBuf o_flux, o_ltot, o_val, o_sig, o_img, o_evc, o_ctb, o_cnt;
     const size_t nflux = size_t(ncr) * std::max(n_obs, 1) * nb;
     if ((rcode = bind_out(g, out->flux_sum, nflux * sizeof(double), g->flux, o_flux))) return rcode;
     if ((rcode = bind_out(g, out->L_tot, size_t(ncr) * std::max(n_obs, 1) * sizeof(double), g->ltot_out, o_ltot))) return rcode;
@@ -344,7 +488,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     if (npix) if ((rcode = bind_out(g, out->image, size_t(ncr) * n_obs * npix * npix * sizeof(float), g->image, o_img))) return rcode;
     const size_t n_pkt = size_t(hi - lo);
     if (out->event_count) if ((rcode = bind_out(g, out->event_count, size_t(ncr) * n_pkt * sizeof(uint32_t), g->evcount, o_evc))) return rcode;
-    if ((rcode = bind_out(g, out->counters, sizeof(gcmcrt_counters), g->counters, o_cnt, true))) return rcode;
+    if (out->counters) if ((rcode = bind_out(g, out->counters, sizeof(gcmcrt_counters), g->counters_out, o_cnt))) return rcode;
     CUDA_TRY(g, cudaMemsetAsync(o_flux.dev, 0, nflux * sizeof(double), s));
     CUDA_TRY(g, cudaMemsetAsync(o_ltot.dev, 0, o_ltot.bytes, s));
     if (npix) CUDA_TRY(g, cudaMemsetAsync(o_img.dev, 0, o_img.bytes, s));
@@ -356,21 +500,26 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     CUDA_TRY(g, cudaMemsetAsync(g->counters.p, 0, sizeof(DevCounters), s));
 
     // ---- constants of the run
-    RunConst rc;
-    std::memset(&rc, 0, sizeof rc);
+    PassLaunch L;
+    std::memset(&L.rc, 0, sizeof L.rc);
+    std::memset(&L.ev, 0, sizeof L.ev);
+    std::memset(&L.susp, 0, sizeof L.susp);
+    std::memset(&L.wc, 0, sizeof L.wc);
+    std::memset(&L.sp, 0, sizeof L.sp);
+    std::memset(&L.spl, 0, sizeof L.spl);
+    std::memset(&L.plan, 0, sizeof L.plan);
+    RunConst& rc = L.rc;
     rc.geom = geom_params(g);
     rc.chan_key0 = uint32_t(g->chan0);
     rc.chan_begin = cb; rc.n_chan_run = ncr;
     rc.pkt_begin = uint32_t(lo); rc.n_pkt = uint32_t(n_pkt);
     rc.N = N; rc.seed = prm->seed;
     rc.mode = emission;
-    if (mode == 2 && n_obs < 1) return fail(g, GCMCRT_E_INVALID, "transmission needs at least one observer direction");
     rc.max_events = prm->max_events; rc.scatter_on = prm->scatter_on;
     rc.survival_bias = prm->survival_bias != 0;
     rc.cloud_phase = prm->cloud_phase;
     rc.forced_scatter = prm->forced_scatter;
     rc.alpha2 = nullptr;
-    if (prm->cloud_phase < 0 || prm->cloud_phase > 2) return fail(g, GCMCRT_E_INVALID, "cloud_phase must be 0 (HG), 1 (TTHG) or 2 (Draine)");
     rc.roulette_w_min = float(prm->roulette_w_min); rc.roulette_survive = float(prm->roulette_survive);
     rc.surface_albedo = g->surface_albedo;
     rc.xi = prm->emission_bias;
@@ -397,51 +546,65 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.magic_npkt = magic_div(n_pkt);
     rc.t_service = g->tune[0]; rc.t_lateral = g->tune[1]; rc.p_refill = 12;
     PassCtrl* ctrl = g->ctrl.as<PassCtrl>();
+    L.ctrl = ctrl;
     rc.work_counter = &ctrl->work_counter;
     rc.ray_counter = &ctrl->ray_counter;
+    rc.ctrl = ctrl;
 
     // ---- launch geometry: persistent grids sized to the device
     const size_t smem_t = size_t(g->tab_floats) * sizeof(float);
     int occ_t = 0, occ_p = 0;
     const bool cont = prm->continuous_absorption != 0;
-    auto tk = cont ? transport_kernel<4, true> : transport_kernel<4, false>;
-    auto pk = peel_kernel<16>;
-    CUDA_TRY(g, cudaFuncSetAttribute(tk, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_t)));
-    CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_t, tk, kTransportThreads, smem_t));
-    if (occ_t < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
-    const int grid_t = g->sm_count * occ_t;
-    const unsigned long long threads_t = (unsigned long long)grid_t * kTransportThreads;
+    L.tk = cont ? transport_kernel<4, true> : transport_kernel<4, false>;
+    L.pk = peel_kernel<16>;
+    L.emission = emission != 0;
+    L.smem_t = smem_t;
+    if (mode != 2) {
+        CUDA_TRY(g, cudaFuncSetAttribute(L.tk, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_t)));
+        CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_t, L.tk, kTransportThreads, smem_t));
+        if (occ_t < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
+    }
+    L.grid_t = unsigned(g->sm_count * std::max(occ_t, 1));
+    const unsigned long long threads_t = (unsigned long long)L.grid_t * kTransportThreads;
     // suspended list: one entry per resident lane for the persistent kernel, plus what a wavefront pass can park (its
     // last generation and whatever found the event buffer full).  A pass starts with at most ev_cap / 2 inherited
     // entries (else it only drains) and parks each of its <= ev_cap / 2 fresh packets at most once: <= ev_cap in all
     const unsigned long long susp_cap = threads_t + (g->tune[2] > 0 ? 1ull * g->ev_cap : 0ull);
-    for (int b = 0; b < 2; ++b) {
-        CUDA_TRY(g, g->s0[b].ensure(susp_cap * sizeof(float4)));
-        CUDA_TRY(g, g->s1[b].ensure(susp_cap * sizeof(float4)));
-        CUDA_TRY(g, g->s2[b].ensure(susp_cap * sizeof(uint4)));
+    if (mode != 2) {
+        for (int b = 0; b < 2; ++b) {
+            CUDA_TRY(g, g->s0[b].ensure(susp_cap * sizeof(float4)));
+            CUDA_TRY(g, g->s1[b].ensure(susp_cap * sizeof(float4)));
+            CUDA_TRY(g, g->s2[b].ensure(susp_cap * sizeof(uint4)));
+            SuspBuf& sb = L.susp.b[b];
+            sb.s0 = g->s0[b].as<float4>(); sb.s1 = g->s1[b].as<float4>(); sb.s2 = g->s2[b].as<uint4>();
+            sb.count = &ctrl->susp_count[b]; sb.taken = &ctrl->susp_taken[b];
+            sb.cap = (unsigned int)std::min<unsigned long long>(susp_cap, 0xffffffffull);
+        }
     }
-    EventBuf ev;
-    std::memset(&ev, 0, sizeof ev);
+    EventBuf& ev = L.ev;
     ev.rec = g->ev0.as<float4>();
     ev.count = &ctrl->ev_count;
     ev.cap = g->ev_cap;
     ev.soft_cap = (unsigned long long)g->ev_cap > 4 * threads_t ? g->ev_cap - (unsigned int)(2 * threads_t) : g->ev_cap / 2;
+    ev.chan_lo = &ctrl->chan_lo;
 
     const int n_runs = prm->doppler_on ? std::max(n_obs, 1) : 1;
-    unsigned long long passes = 0;
-    CUDA_TRY(g, ensure_events(g));
+    unsigned long long passes_host = 0;   // transmission: one "pass" per run, counted here
+    unsigned launches_per_pass = 0;
+    if (timed) CUDA_TRY(g, ensure_events(g));
     g->launches = g->launches_pending; g->launches_pending = 0; g->ms_emis = g->ms_transport = g->ms_peel = g->ms_sort = 0.0;
     g->ms_stage = 0.0;
+    CUDA_TRY(g, cudaMemsetAsync(ctrl, 0, sizeof(PassCtrl), s));
     for (int run = 0; run < n_runs; ++run) {
         // ---- A0/A1: make sure the staged table is the one this run needs
         if (prm->doppler_on && n_obs > 0) {
             const double* od = prm->obs_dir + 3 * run;
             const bool same = g->staged_obs >= 0 && g->staged_cont == cont && g->staged_halfwidth == prm->doppler_halfwidth &&
                               g->staged_dir[0] == od[0] && g->staged_dir[1] == od[1] && g->staged_dir[2] == od[2];
-            if (!same && (rcode = stage_opacity(g, od, prm->doppler_halfwidth, s, cont))) return rcode;
+            if (!same && (rcode = stage_opacity(g, od, prm->doppler_halfwidth, s, cont, timed))) return rcode;
             rc.obs_first = run; rc.n_obs_run = 1;
         } else {
-            if ((g->staged_obs != -1 || g->staged_cont != cont) && (rcode = stage_opacity(g, nullptr, 0, s, cont))) return rcode;
+            if ((g->staged_obs != -1 || g->staged_cont != cont) && (rcode = stage_opacity(g, nullptr, 0, s, cont, timed))) return rcode;
             rc.obs_first = 0; rc.n_obs_run = n_obs;
         }
         rc.magic_nobs = magic_div((unsigned long long)std::max(rc.n_obs_run, 1));
@@ -463,7 +626,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             ep.r_edges = g->r64.as<double>(); ep.cth_edges = g->cth64.as<double>(); ep.ph_edges = g->ph64.as<double>();
             ep.tau_vert_max = prm->tau_vert_max;
             ep.Lcell = prm->emission_bias > 0.0 ? g->Lcell.as<double>() : nullptr; ep.Lcum = g->Lcum.as<double>(); ep.Ltot = g->Ltot.as<double>();
-            CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
+            if (timed) CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
             {
                 const unsigned ge = (unsigned)std::min(g->n_chan, g->sm_count * 8);
                 const size_t sm = (2 * size_t(g->nlev) + 32) * sizeof(double);
@@ -476,14 +639,14 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             emis_guide_kernel<<<(unsigned)(((long long)g->n_chan * kEmisGuide + 255) / 256), 256, 0, s>>>(
                 g->n_chan, g->ncell, ep.Lcum, ep.Ltot, g->guide.as<int>());
             CUDA_TRY(g, cudaGetLastError());
-            CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
-            CUDA_TRY(g, cudaEventSynchronize(g->tev[1]));
-            {
+            if (timed) {
+                CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
+                CUDA_TRY(g, cudaEventSynchronize(g->tev[1]));
                 float ms = 0.f;
                 CUDA_TRY(g, cudaEventElapsedTime(&ms, g->tev[0], g->tev[1]));
                 g->ms_emis += ms;
             }
-            g->launches += 3;
+            g->launches += 2;
             rc.Lcum = ep.Lcum; rc.Lcell = ep.Lcell; rc.Ltot = ep.Ltot; rc.guide = g->guide.as<int>();
             // L_tot output [n_chan_run][n_obs]
             const int o0 = prm->doppler_on ? run : 0, o1 = prm->doppler_on ? run + 1 : std::max(n_obs, 1);
@@ -495,7 +658,6 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         // event counts are recorded for the first run only (with doppler_on: observer 0's run)
         rc.event_count = run == 0 ? static_cast<uint32_t*>(o_evc.dev) : nullptr;
 
-        // ---- pass loop
         const unsigned long long total_items = (unsigned long long)ncr * n_pkt;
         if (mode == 2) {
             // ---- transmission (Sect. 5.1): one chord per packet and observer, no events, no passes
@@ -504,7 +666,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             CUDA_TRY(g, cudaFuncSetAttribute(k_tr, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_t)));
             CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tr, k_tr, 256, smem_t));
             if (occ_tr < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
-            CUDA_TRY(g, cudaEventRecord(g->tev[2], s));
+            if (timed) CUDA_TRY(g, cudaEventRecord(g->tev[2], s));
             for (int o = rc.obs_first; o < rc.obs_first + rc.n_obs_run; ++o) {
                 TransParams tp;
                 tp.o = o;
@@ -516,28 +678,30 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
                 k_tr<<<std::max(gt, 1u), 256, smem_t, s>>>(rc, tp, total_items);
                 ++g->launches;
             }
-            CUDA_TRY(g, cudaEventRecord(g->tev[3], s));
             CUDA_TRY(g, cudaGetLastError());
-            CUDA_TRY(g, cudaEventSynchronize(g->tev[3]));
-            {
+            if (timed) {
+                CUDA_TRY(g, cudaEventRecord(g->tev[3], s));
+                CUDA_TRY(g, cudaEventSynchronize(g->tev[3]));
                 float c = 0.f;
                 CUDA_TRY(g, cudaEventElapsedTime(&c, g->tev[2], g->tev[3]));
                 g->ms_peel += c;
             }
-            ++passes;
+            ++passes_host;
             continue;
         }
-        CUDA_TRY(g, cudaMemsetAsync(ctrl, 0, sizeof(PassCtrl), s));
-        int cur = 0;
+
+        // ---- the pass loop of this run
+        L.has_obs = rc.n_obs_run > 0;
         const size_t smem_p = (size_t((g->tab_floats + 31) & ~31) + size_t(kPeelThreads / 32) * rc.n_obs_run * nb) * sizeof(float);
-        if (rc.n_obs_run > 0) {
-            CUDA_TRY(g, cudaFuncSetAttribute(pk, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_p)));
-            CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, pk, kPeelThreads, smem_p));
+        L.smem_p = smem_p;
+        if (L.has_obs) {
+            CUDA_TRY(g, cudaFuncSetAttribute(L.pk, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_p)));
+            CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, L.pk, kPeelThreads, smem_p));
             if (occ_p < 1) return fail(g, GCMCRT_E_INVALID, "peel bins do not fit in shared memory");
+            L.grid_p = unsigned(g->sm_count * occ_p);
         }
-        SortParams sp;
-        std::memset(&sp, 0, sizeof sp);
-        if (rc.n_obs_run > 0) {
+        SortParams& sp = L.sp;
+        if (L.has_obs) {
             const long long max_bins = 1ll << 25;
             // channels whose events can share one pass: every packet makes at least one event when it interacts,
             // so a pass of ev_cap events spans about ev_cap / n_pkt channels; more bins than that only cost scan time
@@ -563,28 +727,35 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             sp.hist = g->hist.as<unsigned int>(); sp.tile_sums = g->tile_sums.as<unsigned int>();
             sp.perm = g->perm.as<unsigned int>();
             sp.nlev = g->nlev; sp.nlat = g->nlat; sp.ncell = g->ncell;
+        } else {
+            ev.keys = nullptr; ev.hist = nullptr;
         }
         // ---- wavefront kernels (wavefront.cuh): launch geometry and the launch-order sort of albedo runs
         // continuous absorption runs through the persistent kernel only (its march carries the second extinction)
         const int n_gen = cont ? 0 : g->tune[2];
-        auto k_keys = wave_launch_keys_kernel;
-        auto k_first = rc.forced_scatter ? wave_first_flight_kernel<16, true> : wave_first_flight_kernel<16, false>;
-        auto k_emit = wave_emit_kernel;
-        auto k_inter = rc.forced_scatter == 2 ? wave_interact_kernel<kInteractK, true> : wave_interact_kernel<kInteractK, false>;
-        const size_t smem_w = smem_t;
-        const size_t smem_i = (size_t((g->tab_floats + 31) & ~31) + size_t(kWaveThreads / 32) * kStageFields * kStageSlots) * sizeof(float);
-        int occ_f = 1, occ_i = 1;
-        SortParams spl;
-        std::memset(&spl, 0, sizeof spl);
+        L.n_gen = n_gen;
+        // emission without scattering (L210): the emit kernel has already closed every packet it recorded
+        L.n_gen_run = (emission && !prm->scatter_on) ? 0 : n_gen;
+        L.k_first = rc.forced_scatter ? wave_first_flight_kernel<16, true> : wave_first_flight_kernel<16, false>;
+        L.k_inter = rc.forced_scatter == 2 ? wave_interact_kernel<kInteractK, true> : wave_interact_kernel<kInteractK, false>;
+        L.smem_w = smem_t;
+        L.smem_i = (size_t((g->tab_floats + 31) & ~31) + size_t(kWaveThreads / 32) * kStageFields * kStageSlots) * sizeof(float);
+        L.grid_k = unsigned(g->sm_count * 8);
+        SortParams& spl = L.spl;
         if (n_gen > 0) {
-            CUDA_TRY(g, cudaFuncSetAttribute(k_keys, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_w)));
-            CUDA_TRY(g, cudaFuncSetAttribute(k_first, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_w)));
-            CUDA_TRY(g, cudaFuncSetAttribute(k_emit, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_w)));
-            CUDA_TRY(g, cudaFuncSetAttribute(k_inter, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_i)));
-            CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, k_first, kWaveThreads, smem_w));
-            CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_i, k_inter, kWaveThreads, smem_i));
+            int occ_f = 1, occ_i = 1;
+            CUDA_TRY(g, cudaFuncSetAttribute(wave_launch_keys_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(L.smem_w)));
+            CUDA_TRY(g, cudaFuncSetAttribute(L.k_first, cudaFuncAttributeMaxDynamicSharedMemorySize, int(L.smem_w)));
+            CUDA_TRY(g, cudaFuncSetAttribute(wave_emit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, int(L.smem_w)));
+            CUDA_TRY(g, cudaFuncSetAttribute(L.k_inter, cudaFuncAttributeMaxDynamicSharedMemorySize, int(L.smem_i)));
+            CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_f, L.k_first, kWaveThreads, L.smem_w));
+            CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_i, L.k_inter, kWaveThreads, L.smem_i));
             if (occ_f < 1 || occ_i < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
+            L.grid_f = unsigned(g->sm_count * occ_f);
+            L.grid_i = unsigned(g->sm_count * occ_i);
             CUDA_TRY(g, g->flights.ensure(size_t(g->sm_count) * occ_i * (kWaveThreads / 32) * kFlightFields * kStageSlots * sizeof(float)));
+            L.wc.flights = g->flights.as<float>();
+            L.wc.c_fold = 1;
             if (!emission) {
                 const int ncol = g->nlat * g->nlon;
                 // same bound as the event sort: channels a pass can span, and at most 2^25 bins (a run of many channels
@@ -600,119 +771,36 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
                 CUDA_TRY(g, g->lperm.ensure(size_t(g->ev_cap) * sizeof(unsigned int)));
                 CUDA_TRY(g, g->lhist.ensure(size_t(spl.nbins) * sizeof(unsigned int)));
                 CUDA_TRY(g, g->ltile.ensure(size_t(spl.n_tiles) * sizeof(unsigned int)));
-                spl.keys = g->lkeys.as<unsigned int>(); spl.count = nullptr; spl.cap = g->ev_cap;
+                spl.keys = g->lkeys.as<unsigned int>(); spl.count = &ctrl->n_fresh; spl.cap = g->ev_cap;
                 spl.hist = g->lhist.as<unsigned int>(); spl.tile_sums = g->ltile.as<unsigned int>();
                 spl.perm = g->lperm.as<unsigned int>();
+                L.wc.keys = g->lkeys.as<unsigned int>(); L.wc.perm = g->lperm.as<unsigned int>();
+                L.wc.lhist = spl.hist;   // the launch sort's histogram is counted while the keys are written
+                L.wc.c_fold = std::max(spl.c_fold, 1);
             }
         }
-        // Fresh packets per pass: sized so that all their events fit the event buffer; the ratio events / packet is
-        // learnt from the passes already run.  Whatever does not fit is parked and resumed by the next pass.
-        unsigned long long item0 = 0;
-        unsigned long long batch = std::max<unsigned long long>(1024, g->ev_cap / (unsigned long long)g->tune[3]);
-        unsigned long long ev_seen = 0, pk_seen = 0, leftover = 0;
-        for (;;) {
-            const int nxt = 1 - cur;
-            SuspBuf sin, sout;
-            sin.s0 = g->s0[cur].as<float4>(); sin.s1 = g->s1[cur].as<float4>(); sin.s2 = g->s2[cur].as<uint4>();
-            sin.count = &ctrl->susp_count[cur]; sin.taken = &ctrl->susp_taken[cur];
-            sout.s0 = g->s0[nxt].as<float4>(); sout.s1 = g->s1[nxt].as<float4>(); sout.s2 = g->s2[nxt].as<uint4>();
-            sout.count = &ctrl->susp_count[nxt]; sout.taken = &ctrl->susp_taken[nxt];
-            sin.cap = sout.cap = (unsigned int)std::min<unsigned long long>(susp_cap, 0xffffffffull);
-            CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
-            unsigned long long n_fresh = 0, tail_items = total_items;
-            const unsigned long long chan_lo_pass = item0 / std::max<size_t>(n_pkt, 1);
-            if (rc.n_obs_run > 0) {   // the event sort's histogram is filled while the records are written
-                sp.chan_lo = ev.chan_lo = int(std::min<unsigned long long>(chan_lo_pass, (unsigned long long)ncr));
-                CUDA_TRY(g, cudaMemsetAsync(sp.hist, 0, size_t(sp.nbins) * sizeof(unsigned int), s));
-            }
-            if (n_gen > 0) {
-                // a pass that inherited a long suspended list only drains it (keeps the list bounded, see susp_cap)
-                n_fresh = leftover > g->ev_cap / 2 ? 0 : std::min<unsigned long long>(std::min<unsigned long long>(batch, g->ev_cap / 2), total_items - item0);
-                tail_items = 0;   // the persistent kernel only finishes what the generations leave over
-                WaveConst wc;
-                std::memset(&wc, 0, sizeof wc);
-                wc.item0 = item0; wc.n_items = (unsigned int)n_fresh;
-                wc.chan_lo = int(chan_lo_pass); wc.c_fold = std::max(spl.c_fold, 1);
-                wc.flights = g->flights.as<float>();
-                if (n_fresh > 0) {
-                    if (!emission) {
-                        wc.keys = g->lkeys.as<unsigned int>(); wc.perm = g->lperm.as<unsigned int>();
-                        spl.n_host = wc.n_items;
-                        const unsigned gk = (unsigned)std::min<unsigned long long>((n_fresh + 255) / 256, (unsigned long long)g->sm_count * 8);
-                        CUDA_TRY(g, cudaMemsetAsync(spl.hist, 0, size_t(spl.nbins) * sizeof(unsigned int), s));
-                        wc.lhist = spl.hist;   // the launch sort's histogram is counted while the keys are written
-                        k_keys<<<gk, kWaveThreads, smem_w, s>>>(rc, wc);
-                        scan_reduce_kernel<<<spl.n_tiles, kScanThreads, 0, s>>>(spl);
-                        scan_tiles_kernel<<<1, 1024, 0, s>>>(spl);
-                        scan_apply_kernel<<<spl.n_tiles, kScanThreads, 0, s>>>(spl);
-                        ev_scatter_kernel<<<gk, 256, 0, s>>>(spl);
-                        k_first<<<g->sm_count * occ_f, kWaveThreads, smem_w, s>>>(rc, ev, sin, wc);
-                        g->launches += 6;
-                    } else {
-                        const unsigned ge = (unsigned)std::min<unsigned long long>((n_fresh + 255) / 256, (unsigned long long)g->sm_count * 8);
-                        k_emit<<<ge, kWaveThreads, smem_w, s>>>(rc, ev, sin, wc);
-                        g->launches += 1;
-                    }
-                    CUDA_TRY(g, cudaMemcpyAsync(&ctrl->gen_mark[1], &ctrl->ev_count, sizeof(unsigned int), cudaMemcpyDeviceToDevice, s));
-                    // emission without scattering (L210): the emit kernel has already closed every packet it recorded
-                    const int n_gen_run = (emission && !prm->scatter_on) ? 0 : n_gen;
-                    for (int gi = 0; gi < n_gen_run; ++gi) {
-                        wc.gen_mark = &ctrl->gen_mark[gi];
-                        wc.park_all = gi == n_gen - 1;
-                        k_inter<<<g->sm_count * occ_i, kWaveThreads, smem_i, s>>>(rc, ev, sin, wc);
-                        CUDA_TRY(g, cudaMemcpyAsync(&ctrl->gen_mark[gi + 2], &ctrl->ev_count, sizeof(unsigned int), cudaMemcpyDeviceToDevice, s));
-                    }
-                    g->launches += n_gen_run;
-                }
-            }
-            tk<<<grid_t, kTransportThreads, smem_t, s>>>(rc, ev, sin, sout, tail_items);
-            CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
-            if (rc.n_obs_run > 0) {
-                // counting sort of this pass's events by (channel, cell): sort.cuh
-                if (!ev.hist) { ev_hist_kernel<<<g->sm_count * 8, 256, 0, s>>>(sp); ++g->launches; }
-                scan_reduce_kernel<<<sp.n_tiles, kScanThreads, 0, s>>>(sp);
-                scan_tiles_kernel<<<1, 1024, 0, s>>>(sp);
-                scan_apply_kernel<<<sp.n_tiles, kScanThreads, 0, s>>>(sp);
-                ev_scatter_kernel<<<g->sm_count * 8, 256, 0, s>>>(sp);
-            }
-            CUDA_TRY(g, cudaEventRecord(g->tev[2], s));
-            if (rc.n_obs_run > 0) pk<<<g->sm_count * occ_p, kPeelThreads, smem_p, s>>>(rc, ev, sp.perm);
-            CUDA_TRY(g, cudaEventRecord(g->tev[3], s));
-            CUDA_TRY(g, cudaGetLastError());
-            ++passes;
-            g->launches += rc.n_obs_run > 0 ? 6 : 1;
-            CUDA_TRY(g, cudaMemcpyAsync(g->h_ctrl, ctrl, sizeof(PassCtrl), cudaMemcpyDeviceToHost, s));
-            CUDA_TRY(g, cudaStreamSynchronize(s));
-            {
+        L.tail_items = n_gen > 0 ? 0ull : total_items;   // wavefront: the persistent kernel only finishes what the generations leave over
+        L.plan.total_items = total_items; L.plan.susp_cap = susp_cap; L.plan.max_passes = 1ull << 20;
+        L.plan.batch0 = std::max<unsigned long long>(1024, g->ev_cap / (unsigned long long)g->tune[3]);
+        L.plan.n_pkt = uint32_t(n_pkt); L.plan.ev_cap = g->ev_cap; L.plan.n_gen = n_gen; L.plan.n_chan_run = ncr;
+        run_begin_kernel<<<1, 1, 0, s>>>(ctrl, L.plan);
+        ++g->launches;
+        if (!timed) {
+            if ((rcode = launch_pass_loop(g, L, s, &launches_per_pass))) return rcode;
+        } else {
+            for (;;) {
+                if ((rcode = enqueue_pass(g, L, s, g->tev, cudaGraphConditionalHandle{}, 0, &launches_per_pass))) return rcode;
+                CUDA_TRY(g, cudaMemcpyAsync(g->h_ctrl, ctrl, sizeof(PassCtrl), cudaMemcpyDeviceToHost, s));
+                CUDA_TRY(g, cudaStreamSynchronize(s));
                 float a = 0.f, b = 0.f, c = 0.f;
                 CUDA_TRY(g, cudaEventElapsedTime(&a, g->tev[0], g->tev[1]));
                 CUDA_TRY(g, cudaEventElapsedTime(&b, g->tev[1], g->tev[2]));
                 CUDA_TRY(g, cudaEventElapsedTime(&c, g->tev[2], g->tev[3]));
                 g->ms_transport += a; g->ms_sort += b; g->ms_peel += c;
+                if (g->h_ctrl->error == 1) return fail(g, GCMCRT_E_CUDA, "suspended-packet list overflow");
+                if (g->h_ctrl->error) return fail(g, GCMCRT_E_CUDA, "pass loop did not terminate");
+                if (g->h_ctrl->done) break;
             }
-            if (n_gen > 0) {
-                item0 += n_fresh;
-                ev_seen += std::min<unsigned long long>(g->h_ctrl->ev_count, g->ev_cap); pk_seen += n_fresh;
-                if (pk_seen > 0) {   // next batch: 85 % of the buffer at the ratio seen so far
-                    const double ratio = std::max(0.25, double(ev_seen) / double(pk_seen));
-                    batch = std::max<unsigned long long>(1024, (unsigned long long)(0.85 * double(g->ev_cap) / ratio));
-                }
-            } else {
-                item0 = std::min<unsigned long long>(g->h_ctrl->work_counter, total_items);
-            }
-            leftover = g->h_ctrl->susp_count[nxt];
-            if (leftover > susp_cap) return fail(g, GCMCRT_E_CUDA, "suspended-packet list overflow");
-            const bool done = item0 >= total_items && leftover == 0;
-            if (done) break;
-            // reset the per-pass counters: events, rays, generation marks, the list just consumed
-            PassCtrl next = *g->h_ctrl;
-            next.ev_count = 0; next.ray_counter = 0;
-            next.susp_count[cur] = 0; next.susp_taken[cur] = 0; next.susp_taken[nxt] = 0;
-            std::memset(next.gen_mark, 0, sizeof next.gen_mark);
-            CUDA_TRY(g, cudaMemcpyAsync(ctrl, &next, sizeof(PassCtrl), cudaMemcpyHostToDevice, s));
-            CUDA_TRY(g, cudaStreamSynchronize(s));
-            cur = nxt;
-            if (passes > (1ull << 20)) return fail(g, GCMCRT_E_CUDA, "pass loop did not terminate");
         }
     }
 
@@ -728,29 +816,26 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     }
     g->ms_stage += g->ms_stage_pending;
     g->ms_stage_pending = 0.0;
-    // ---- copy-backs for host-resident outputs
+    if (o_cnt.dev) {
+        finalize_counters_kernel<<<1, 1, 0, s>>>(g->counters.as<DevCounters>(), mode == 2 ? nullptr : ctrl,
+                                                static_cast<gcmcrt_counters*>(o_cnt.dev), g->launches + 1, launches_per_pass,
+                                                passes_host, g->ms_stage, g->ms_emis, g->ms_transport, g->ms_peel, g->ms_sort);
+        CUDA_TRY(g, cudaGetLastError());
+    }
+    // ---- copy-backs for host-resident outputs (the only place an untimed run waits for the device)
     bool need_sync = false;
-    for (OutBuf* ob : {&o_flux, &o_ltot, &o_val, &o_sig, &o_img, &o_evc, &o_ctb}) {
+    for (OutBuf* ob : {&o_flux, &o_ltot, &o_val, &o_sig, &o_img, &o_evc, &o_ctb, &o_cnt}) {
         if (ob->host && ob->dev && ob->bytes) {
             CUDA_TRY(g, cudaMemcpyAsync(ob->host, ob->dev, ob->bytes, cudaMemcpyDeviceToHost, s));
             need_sync = true;
         }
     }
-    if (out->counters) {
-        DevCounters dc;
-        CUDA_TRY(g, cudaMemcpyAsync(&dc, g->counters.p, sizeof dc, cudaMemcpyDeviceToHost, s));
-        CUDA_TRY(g, cudaStreamSynchronize(s));
-        gcmcrt_counters hc;
-        hc.events = dc.events; hc.segments_transport = dc.seg_transport; hc.segments_peel = dc.seg_peel;
-        hc.packets_escaped = dc.escaped; hc.packets_absorbed = dc.absorbed; hc.packets_surface = dc.surface;
-        hc.packets_stuck = dc.stuck; hc.escaped_weight = dc.escaped_weight; hc.passes = passes; hc.rays_peel = dc.rays_peel;
-        hc.launches = g->launches; hc.ms_stage = g->ms_stage; hc.ms_emission_cdf = g->ms_emis;
-        hc.ms_transport = g->ms_transport; hc.ms_peel = g->ms_peel; hc.ms_sort = g->ms_sort;
-        if (is_device_ptr(out->counters)) CUDA_TRY(g, cudaMemcpyAsync(out->counters, &hc, sizeof hc, cudaMemcpyHostToDevice, s));
-        else *out->counters = hc;
-        need_sync = true;
-    }
     if (need_sync) CUDA_TRY(g, cudaStreamSynchronize(s));
+    if (o_cnt.host) {
+        const unsigned long long st = static_cast<const gcmcrt_counters*>(o_cnt.host)->device_status;
+        if (st == 1) return fail(g, GCMCRT_E_CUDA, "suspended-packet list overflow");
+        if (st) return fail(g, GCMCRT_E_CUDA, "pass loop did not terminate");
+    }
     return GCMCRT_OK;
 }
 
@@ -950,10 +1035,11 @@ int gcmcrt_destroy(gcmcrt_grid* g)
     for (DevBuf* b : {&g->tab, &g->r64, &g->cth64, &g->ph64, &g->rc32, &g->thc32, &g->phc32, &g->T, &g->rho, &g->u, &g->v,
                       &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->alpha2, &g->prop, &g->reff, &g->vlos, &g->node, &g->node_idx, &g->node_w, &g->own_pcell,
                       &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->guide, &g->ev0, &g->evkeys, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
-                      &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->flux, &g->ltot_out,
+                      &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->counters_out, &g->flux, &g->ltot_out,
                       &g->value, &g->sigma, &g->image, &g->evcount, &g->contrib})
         b->release();
     if (g->h_ctrl) cudaFreeHost(g->h_ctrl);
+    if (g->cap_stream) cudaStreamDestroy(g->cap_stream);
     for (auto& e : g->tev) if (e) cudaEventDestroy(e);
     delete g;
     return GCMCRT_OK;

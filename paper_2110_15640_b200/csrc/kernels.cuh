@@ -44,7 +44,8 @@ struct EventBuf {
     unsigned int* hist;   // [c_fold * ncell], zeroed by the host before the pass; NULL: the host runs ev_hist_kernel
                           // instead (emission: events pile up in a few bright cells and the contended atomics are
                           // cheaper in a kernel of their own than inside the emit / interact kernels)
-    int chan_lo, c_fold, nlev, nlat, ncell;
+    const int* chan_lo;   // device: first channel of the pass (PassCtrl::chan_lo)
+    int c_fold, nlev, nlat, ncell;
     int lev_shift, nlg, bins_per_chan;   // the key's second part is column * nlg + (i >> lev_shift): cells (shift 0),
                                          // groups of levels, or whole columns (nlg = 1)
 };
@@ -60,7 +61,7 @@ __device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slo
     r[3] = prop;
     if (ev.keys) {
         const int i = cellp & 1023, j = (cellp >> 10) & 1023, k = cellp >> 20;
-        const unsigned int chan = (unsigned int)min(max(int(meta >> 8) - ev.chan_lo, 0), ev.c_fold - 1);
+        const unsigned int chan = (unsigned int)min(max(int(meta >> 8) - *ev.chan_lo, 0), ev.c_fold - 1);
         const unsigned int col = (unsigned int)(k * ev.nlat + j);
         const unsigned int key = chan * (unsigned int)ev.bins_per_chan + col * (unsigned int)ev.nlg + (ev.nlg > 1 ? (unsigned int)(i >> ev.lev_shift) : 0u);
         ev.keys[slot] = key;
@@ -79,10 +80,98 @@ struct SuspBuf {
                         // list so that this cannot happen and reports an error if the count ever exceeds it)
 };
 
+struct PassCtrl;
+struct SuspPair {   // the two suspended lists; which one a pass reads is part of the pass plan (PassCtrl::cur)
+    SuspBuf b[2];
+};
+
 struct DevCounters {
     unsigned long long events, seg_transport, seg_peel, escaped, absorbed, surface, stuck, rays_peel;
     double escaped_weight;
 };
+
+// Pass control, device-resident.  A run is a sequence of passes (fresh packets whose events fit the event buffer, then
+// the peel-off of those events); everything that changes from pass to pass lives here and is read by the kernels, so
+// that the host never has to look at it: pass_begin_kernel / pass_end_kernel (below) are the loop's bookkeeping and
+// the loop itself is a conditional WHILE node of a CUDA graph (gcmcrt.cu).
+constexpr int kMaxGen = 30;
+struct alignas(128) PassCtrl {
+    // -- counters the packet kernels update with atomics (zeroed by pass_begin_kernel)
+    unsigned int ev_count;
+    unsigned int susp_count[2];
+    unsigned int susp_taken[2];
+    unsigned int pad0;
+    unsigned long long work_counter;   // next fresh item (persistent-only transport); kept from pass to pass
+    unsigned long long ray_counter;
+    unsigned int gen_mark[kMaxGen + 2];   // event-buffer offsets of the wavefront generations of this pass
+    // -- the plan of the current pass (written by pass_begin_kernel, read-only for the packet kernels)
+    alignas(128) unsigned long long item0;   // first fresh packet item of this pass (item = chan_run * n_pkt + packet offset)
+    unsigned int n_fresh;              // fresh packets of this pass (wavefront transport)
+    int cur;                           // suspended list this pass resumes from; it parks into the other one
+    int chan_lo;                       // first channel this pass draws fresh packets from (sort key window)
+    int done, error;                   // error: 1 suspended-list overflow, 2 pass limit
+    // -- loop state (control kernels only)
+    unsigned long long batch, ev_seen, pk_seen, leftover, passes;
+};
+
+struct PassPlan {   // constants of one run's pass loop
+    unsigned long long total_items, susp_cap, max_passes, batch0;
+    unsigned int n_pkt, ev_cap;
+    int n_gen;          // wavefront generations per pass (0: the persistent kernel draws the fresh packets itself)
+    int n_chan_run;
+};
+
+// start of a run (one per Doppler observer run): loop state to its initial values; the pass count carries on
+__global__ void run_begin_kernel(PassCtrl* c, const PassPlan p)
+{
+    const unsigned long long passes = c->passes;
+    const int error = c->error;
+    *c = PassCtrl{};
+    c->passes = passes; c->error = error;
+    c->batch = p.batch0;
+}
+
+__global__ void pass_begin_kernel(PassCtrl* c, const PassPlan p)
+{
+    const int nxt = 1 - c->cur;
+    c->ev_count = 0; c->ray_counter = 0;
+    c->susp_count[nxt] = 0; c->susp_taken[0] = 0; c->susp_taken[1] = 0;
+    for (int m = 0; m < kMaxGen + 2; ++m) c->gen_mark[m] = 0;
+    unsigned long long nf = 0;
+    if (p.n_gen > 0 && !c->done) {
+        // fresh packets sized so that all their events fit the event buffer (the ratio events / packet is learnt from
+        // the passes already run); a pass that inherited a long suspended list only drains it
+        const unsigned long long room = p.total_items - c->item0;
+        nf = c->leftover > p.ev_cap / 2 ? 0ull : min(min(c->batch, (unsigned long long)(p.ev_cap / 2)), room);
+    }
+    c->n_fresh = (unsigned int)nf;
+    c->chan_lo = (int)min(c->item0 / max(p.n_pkt, 1u), (unsigned long long)p.n_chan_run);
+}
+
+// end of a pass: what the host loop used to do after reading the counters back.  use_handle: the loop is a conditional
+// WHILE node and this kernel sets its condition; else the host reads `done`.
+__global__ void pass_end_kernel(PassCtrl* c, const PassPlan p, cudaGraphConditionalHandle handle, int use_handle)
+{
+    const int cur = c->cur, nxt = 1 - cur;
+    if (p.n_gen > 0) {
+        c->item0 += c->n_fresh;
+        c->ev_seen += min(c->ev_count, p.ev_cap);
+        c->pk_seen += c->n_fresh;
+        if (c->pk_seen > 0) {   // next batch: 85 % of the buffer at the ratio seen so far
+            const double ratio = fmax(0.25, double(c->ev_seen) / double(c->pk_seen));
+            c->batch = max(1024ull, (unsigned long long)(0.85 * double(p.ev_cap) / ratio));
+        }
+    } else {
+        c->item0 = min(c->work_counter, p.total_items);
+    }
+    c->leftover = c->susp_count[nxt];
+    if (c->leftover > p.susp_cap) c->error = 1;
+    c->passes += 1;
+    c->done = (c->item0 >= p.total_items && c->leftover == 0) ? 1 : 0;
+    if (!c->done && c->passes >= p.max_passes) c->error = 2;
+    if (!c->done && !c->error) { c->susp_count[cur] = 0; c->cur = nxt; }
+    if (use_handle) cudaGraphSetConditional(handle, (c->done || c->error) ? 0u : 1u);
+}
 
 struct RunConst {
     GeomParams geom;
@@ -122,6 +211,7 @@ struct RunConst {
     DevCounters* counters;
     unsigned long long* work_counter;   // next fresh packet item
     unsigned long long* ray_counter;    // next peel ray of this pass
+    const PassCtrl* ctrl;               // the pass plan (device)
     // exact-division constants floor(2^64 / d) for d = N, n_pkt, n_obs_run (device_common.cuh div_magic)
     unsigned long long magic_N, magic_npkt, magic_nobs;
     // warp scheduling thresholds (lanes waiting before the warp leaves the radial march to serve them)
@@ -611,12 +701,13 @@ __device__ __forceinline__ void finish_packet(const RunConst& rc, const Packet& 
 // prop records then carry omega = 1, so that the event code below (and the peel kernel) needs no other change.
 template <int KSTEPS, bool DUAL>
 __global__ void __launch_bounds__(kTransportThreads, 2)
-transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const SuspBuf susp_in, const SuspBuf susp_out,
-                 const unsigned long long total_items)
+transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const SuspPair susp, const unsigned long long total_items)
 {
     extern __shared__ float smem_f[];
     const GeomSmem gs = load_geom(rc.geom, smem_f);
     __syncthreads();
+    const int cur_list = rc.ctrl->cur;
+    const SuspBuf susp_in = susp.b[cur_list], susp_out = susp.b[1 - cur_list];
 
     Packet pk;
     pk.tau = 0.f; pk.tau_t = 0.f; pk.tau_b = 0.f; pk.W = 0.f; pk.chan_run = 0; pk.pkt = 0; pk.m_inter = 0; pk.nev = 0; pk.fl_seg = 0;

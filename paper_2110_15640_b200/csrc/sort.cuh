@@ -32,7 +32,7 @@ struct SortParams {
     unsigned int* tile_sums;     // [n_tiles]
     unsigned int* perm;          // [cap]
     unsigned int nbins, n_tiles;
-    int nlev, nlat, ncell, c_fold, chan_lo;
+    int nlev, nlat, ncell, c_fold;
 };
 
 __global__ void __launch_bounds__(256) ev_hist_kernel(const SortParams p)

@@ -26,14 +26,12 @@ constexpr int kStageSlots = 64;   // per warp: at most 31 left over + 32 new sur
 constexpr int kLaunchTauBuckets = 16;   // launch order: packets of one entry column grouped by sampled optical depth
 
 struct WaveConst {
-    unsigned long long item0;      // first fresh packet item of this pass (item = chan_run * n_pkt + packet offset)
-    unsigned int n_items;          // fresh packets of this pass
     const unsigned int* perm;      // albedo: launch order, perm[t] in [0, n_items)
     unsigned int* keys;            // albedo: launch sort keys [n_items]
     unsigned int* lhist;           // albedo: histogram of the launch sort keys, counted by the key kernel
     const unsigned int* gen_mark;  // interact: events [gen_mark[0], gen_mark[1]) form this generation (device)
     int park_all;                  // last generation: survivors' next events go to the suspended list
-    int chan_lo, c_fold;           // launch sort key window
+    int c_fold;                    // launch sort key window (its first channel is PassCtrl::chan_lo)
     float* flights;                // interact: per-warp lists of flights in progress [n_warps][kFlightFields][kStageSlots]
 };
 
@@ -252,15 +250,18 @@ __global__ void __launch_bounds__(kWaveThreads) wave_launch_keys_kernel(const __
     extern __shared__ float smem_f[];
     const GeomSmem gs = load_geom(rc.geom, smem_f);
     __syncthreads();
-    for (unsigned int t = blockIdx.x * blockDim.x + threadIdx.x; t < wc.n_items; t += gridDim.x * blockDim.x) {
+    const unsigned int n_items = rc.ctrl->n_fresh;
+    const unsigned long long item0 = rc.ctrl->item0;
+    const int chan_lo = rc.ctrl->chan_lo;
+    for (unsigned int t = blockIdx.x * blockDim.x + threadIdx.x; t < n_items; t += gridDim.x * blockDim.x) {
         uint32_t chan_run, pkt;
-        wave_item(rc, wc.item0 + t, chan_run, pkt);
+        wave_item(rc, item0 + t, chan_run, pkt);
         const uint32_t ckey = rc.chan_key0 + uint32_t(rc.chan_begin) + chan_run;
         const Zeta4 z = zeta_block(rc.seed, ckey, pkt, 0, 0);
         float px, py, pz;
         int j, k;
         albedo_launch_point(rc, gs, z, px, py, pz, j, k);
-        const int slot = min(max(int(chan_run) - wc.chan_lo, 0), wc.c_fold - 1);
+        const int slot = min(max(int(chan_run) - chan_lo, 0), wc.c_fold - 1);
         // the extinction grows roughly exponentially with depth, so the level a packet reaches goes with log(tau):
         // packets of one column that share a log2(tau) bucket end their first flight within a few cells of each other
         const float lt = __log2f(-__logf(z.z2));                       // log2 of the sampled optical depth, about -23 .. 4
@@ -274,23 +275,26 @@ __global__ void __launch_bounds__(kWaveThreads) wave_launch_keys_kernel(const __
 // albedo: launch + first flight, 32 packets of neighbouring entry columns per warp
 template <int KSTEPS, bool FORCED>
 __global__ void __launch_bounds__(kWaveThreads, FORCED ? 3 : 4)
-wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const SuspBuf susp, const WaveConst wc)
+wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const SuspPair susp2, const WaveConst wc)
 {
     extern __shared__ float smem_f[];
     const GeomSmem gs = load_geom(rc.geom, smem_f);
     __syncthreads();
+    const SuspBuf susp = susp2.b[rc.ctrl->cur];
+    const unsigned int n_items = rc.ctrl->n_fresh;
+    const unsigned long long item0 = rc.ctrl->item0;
     WaveCounters wcnt;
     const unsigned int warp0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31u;
-    for (unsigned int base = warp0; base < wc.n_items; base += gridDim.x * blockDim.x) {
+    for (unsigned int base = warp0; base < n_items; base += gridDim.x * blockDim.x) {
         const unsigned int t = base + lane_id();
-        const bool active = t < wc.n_items;
+        const bool active = t < n_items;
         uint32_t chan_run = 0, pkt = 0;
         Ray ray{};
         float tau_t = 0.f, z2 = 0.f;
         const float* alpha_c = rc.alpha;
         if (active) {
             const unsigned int it = __ldg(wc.perm + t);
-            wave_item(rc, wc.item0 + it, chan_run, pkt);
+            wave_item(rc, item0 + it, chan_run, pkt);
             const int ctab = rc.chan_begin + int(chan_run);
             alpha_c = rc.alpha + (size_t)ctab * rc.geom.alpha_stride;
             const Zeta4 z = zeta_block(rc.seed, rc.chan_key0 + uint32_t(ctab), pkt, 0, 0);
@@ -334,20 +338,23 @@ wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
 
 // emission: generation 0 = the emission points (O4).  Eq. 13 with the composite bias xi (C10).
 __global__ void __launch_bounds__(kWaveThreads) wave_emit_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
-                                                                const SuspBuf susp, const WaveConst wc)
+                                                                const SuspPair susp2, const WaveConst wc)
 {
     extern __shared__ float smem_f[];
     const GeomSmem gs = load_geom(rc.geom, smem_f);
     __syncthreads();
+    const SuspBuf susp = susp2.b[rc.ctrl->cur];
+    const unsigned int n_items = rc.ctrl->n_fresh;
+    const unsigned long long item0 = rc.ctrl->item0;
     WaveCounters wcnt;
     const unsigned int warp0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31u;
-    for (unsigned int base = warp0; base < wc.n_items; base += gridDim.x * blockDim.x) {
+    for (unsigned int base = warp0; base < n_items; base += gridDim.x * blockDim.x) {
         const unsigned int t = base + lane_id();
         bool live = false;
         uint32_t chan_run = 0, pkt = 0, cellp = 0;
         float px = 0.f, py = 0.f, pz = 0.f, W = 1.0f;
-        if (t < wc.n_items) {
-            wave_item(rc, wc.item0 + t, chan_run, pkt);
+        if (t < n_items) {
+            wave_item(rc, item0 + t, chan_run, pkt);
             const int ctab = rc.chan_begin + int(chan_run);
             const Zeta4 z = zeta_block(rc.seed, rc.chan_key0 + uint32_t(ctab), pkt, 0, 0);
             const int ncell = rc.geom.ncell;
@@ -405,10 +412,11 @@ __global__ void __launch_bounds__(kWaveThreads) wave_emit_kernel(const __grid_co
 // carries no call to the edge probe
 template <int KSTEPS, bool FORCED>
 __global__ void __launch_bounds__(kWaveThreads, 3)
-wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const SuspBuf susp, const WaveConst wc)
+wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const SuspPair susp2, const WaveConst wc)
 {
     extern __shared__ float smem_f[];
     const GeomSmem gs = load_geom(rc.geom, smem_f);
+    const SuspBuf susp = susp2.b[rc.ctrl->cur];
     // survivors of the absorb / scatter decision wait here until a full warp of them has gathered
     float* stage = smem_f + ((rc.geom.tab_floats + 31) & ~31) + (threadIdx.x >> 5) * (kStageFields * kStageSlots);
     __syncthreads();

@@ -47,7 +47,8 @@ I_SEG_3D = 27.0      # one 3D cell crossing: radial run 22 executed thread-instr
                      # (ncu source page, profiles/ncu_full_r01d_ptx_loops.txt)
 I_SEG_1D = 22.0      # nlat = nlon = 1: the same radial run, no lateral crossings
 I_EVENT = 420.0      # Philox block, phase sampling, rotation, ray setup, event record write + read
-PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 = 7.96e9   # ncu: 4 launches of a cfg2 step average 7.946 GB read + 9.2 MB written
+# dram__bytes_read.sum + dram__bytes_write.sum per peel_kernel launch at the default sizes, from ncu --set full captures
+PEEL_DRAM_BYTES_PER_LAUNCH = {"cfg2": (7.96e9, "profiles/ncu_full_r01d_ptx_loops.txt: 4 launches of a step, 94 M events each")}
 I_PEEL_RAY = 300.0   # record + prop read, phase function, ray setup for one (event, observer), exp, bin accumulation
 
 
@@ -145,10 +146,11 @@ class ClockSampler(threading.Thread):
                 "power_w_max": max(pw) if pw else None, "samples": len(self.rows), "reasons": reasons}
 
 
-def oracle_leg(name, grid, opac, prm, mode, budget_s=15.0):
-    """Time the CPU oracle, as it stands, on a bounded sample: the first n packets of every channel."""
+def oracle_leg(name, grid, opac, prm, mode, budget_s=15.0, threads=None):
+    """Time the CPU oracle, as it stands, on a bounded sample: the first n packets of every channel.
+    threads = None: all host cores (OpenMP over the packet batches); 1: the serial oracle."""
     import oracle  # test infrastructure; allowed here (cpu_baseline / --impl reference)
-    cores = os.cpu_count() or 1
+    cores = threads or os.cpu_count() or 1
     run = oracle.run_albedo if mode == "albedo" else oracle.run_emission
 
     def once(n):
@@ -161,7 +163,7 @@ def oracle_leg(name, grid, opac, prm, mode, budget_s=15.0):
 
     full = int(prm["packets_per_channel"])
     once(64)                      # thread pool and page-in, untimed
-    n1, n2 = min(full, 1024), min(full, 4096)
+    n1, n2 = min(full, 256 if cores == 1 else 1024), min(full, 1024 if cores == 1 else 4096)
     t1, c = once(n1)              # two calibration points: per-channel table preparation is a fixed cost
     n_run, dt = n1, t1
     if n2 > n1:
@@ -178,8 +180,8 @@ def oracle_leg(name, grid, opac, prm, mode, budget_s=15.0):
     nseg = c["segments_transport"] + c["segments_peel"]
     n_chan = int(np.asarray(opac["lambda"]).size)
     return {"value": c["events"] / dt, "unit": UNIT, "cores": min(cores, int(prm.get("n_batches", 32))), "kind": "oracle",
-            "sample": "%s: first %d of %d packets of each of %d channels (%.1f s wall, OpenMP over batches)"
-                      % (name, n2, full, n_chan, dt),
+            "sample": "%s: first %d of %d packets of each of %d channels (%.1f s wall, %s)"
+                      % (name, n2, full, n_chan, dt, "serial" if cores == 1 else "OpenMP over batches"),
             "segments_per_s": nseg / dt, "seconds": dt, "events": int(c["events"])}
 
 
@@ -201,7 +203,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "mode": mode, "n_chan": n_chan,
+            "config": {"workload": args.workload, "mode": mode, "n_chan_per_gpu": n_chan,
                        "packets_per_channel": int(prm["packets_per_channel"]),
                        "grid": list(np.asarray(grid["T"]).shape), "note": "CPU oracle on a bounded packet sample"},
             "cpu_baseline": {k: base[k] for k in ("value", "unit", "cores", "kind", "sample")},
@@ -209,6 +211,134 @@ def run_reference(args):
             "gpu_launches": 0}
     line["cpu_baseline"]["value"] = v
     print(json.dumps(line), flush=True)
+
+
+COUNTER_KEYS = ("events", "segments_transport", "segments_peel", "rays_peel", "packets_escaped", "packets_absorbed",
+                "packets_surface", "packets_stuck", "passes", "launches", "ms_stage", "ms_emission_cdf", "ms_transport",
+                "ms_peel", "ms_sort", "device_status")
+
+
+class Leg:
+    """One workload on one handle: device-resident tables, the step function, and the three measurements taken of it --
+    `value` (K steps only enqueued: device outputs, counters assembled on the device and read after the timed region),
+    the kernel split (steps with run_params.timing = 1: the library records cudaEvents on the launching stream around
+    its kernels) and, for the headline workload, `e2e` (host tables in, host spectra out)."""
+
+    def __init__(self, name, args, binding, torch, stream, rank, grid=None, opac=None, prm=None, mode=None, dev_tables=None):
+        self.name, self.args, self.binding, self.torch, self.stream = name, args, binding, torch, stream
+        if grid is None:
+            grid, opac, prm, mode = make_workload(name, args.packets if name == args.workload else None,
+                                                  args.channels if name == args.workload else (2000 if name == "cfg4" else None))
+        self.grid, self.opac, self.prm, self.mode = grid, dict(opac), prm, mode
+        self.n_chan = int(np.asarray(opac["lambda"]).size)
+        self.opac["chan0"] = rank_chan0(rank, self.n_chan)   # this rank's global channel range (keys the Philox streams)
+        self.tab_keys = [k for k in ("k_abs", "k_sca_ray", "k_sca_cld", "g_cld", "node_kabs", "p_cell") if opac.get(k) is not None]
+        self.streamed = name == "cfg5"
+        self.dev = dict(self.opac)
+        self.host = None
+        for k in self.tab_keys:
+            if dev_tables is not None and k in dev_tables:
+                self.dev[k] = dev_tables[k]
+            else:
+                self.dev[k] = torch.from_numpy(np.ascontiguousarray(opac[k], dtype=np.float32)).cuda()
+        self.G = binding.Grid(grid, stream=stream)
+        self.ncell = int(np.asarray(grid["T"]).size)
+        if self.streamed:
+            self.coef = torch.from_numpy(opac["k_ray_chan"]).cuda()
+
+    def pin_host_tables(self):
+        self.host = dict(self.opac)
+        for k in self.tab_keys:
+            self.host[k] = self.torch.from_numpy(np.ascontiguousarray(self.opac[k], dtype=np.float32)).pin_memory()
+        h2d = sum(self.host[k].numel() * 4 for k in self.tab_keys) + self.n_chan * 4
+        if self.streamed:   # the cells' pressures travel with every batch
+            h2d += self.host["p_cell"].numel() * 4 * (len(wl.cfg5_batches(self.opac, batch=self.args.batch)) - 1)
+        return h2d
+
+    def step(self, op, device_outputs, timing=0, counters="host"):
+        """One pass of the whole hot path over the workload; returns the list of run results."""
+        prm = dict(self.prm, timing=timing)
+        G = self.G
+        if not self.streamed:
+            G.set_opacity(op)
+            fn = G.run_albedo if self.mode == "albedo" else G.run_emission
+            return [fn(prm, device_outputs=device_outputs, counters=counters)]
+        # config 5: per wavelength batch (+ halo channels for the Doppler window) the node tables go through
+        # gcmcrt_set_opacity_nodes, the batch's Rayleigh table is filled on the device, and the batch is run in
+        # emission and in albedo mode toward the 4 phases
+        outs = []
+        for c0, c1, lo, hi in wl.cfg5_batches(self.opac, batch=self.args.batch, halo=int(prm["doppler_halfwidth"])):
+            sub = dict(op, chan0=op["chan0"] + lo, node_kabs=op["node_kabs"][lo:hi])
+            sub["lambda"] = self.opac["lambda"][lo:hi]
+            sub["k_sca_ray"] = self.coef[lo:hi, None].expand(hi - lo, self.ncell).contiguous()
+            G.set_opacity_nodes(sub)
+            for fn in (G.run_emission, G.run_albedo):
+                outs.append(fn(dict(prm, chan_begin=c0 - lo, chan_end=c1 - lo), device_outputs=device_outputs, counters=counters))
+        return outs
+
+    def sum_counters(self, outs):
+        acc = dict.fromkeys(COUNTER_KEYS, 0)
+        for o in outs:
+            c = o["counters"] if "counters" in o else self.binding.read_counters(o["counters_dev"])
+            for k in COUNTER_KEYS:
+                acc[k] += c[k]
+        return acc
+
+    def timed(self, op, device_outputs, steps, barrier, timing=0, counters="device"):
+        torch = self.torch
+        outs = []
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record(self.stream)
+        for _ in range(steps):
+            outs += self.step(op, device_outputs, timing=timing, counters=counters)
+        e1.record(self.stream)
+        host_s = time.perf_counter() - t0      # what the host spent enqueueing (the calls return before the work is done)
+        barrier()
+        return e0.elapsed_time(e1), self.sum_counters(outs), outs, host_s
+
+    def d2h_bytes(self, outs, steps):
+        return sum(o[k].nbytes for o in outs for k in ("flux_sum", "L_tot", "value", "sigma") if k in o) // max(steps, 1)
+
+    def roofline(self, acc, ms_total, steps, pk):
+        """Roofline of the dominant kernel (peel_kernel) from a timing = 1 leg: algorithmic lane-instructions over the
+        kernel's device time (cudaEvents the library records on the launching stream around every launch)."""
+        is3d = np.asarray(self.grid["T"]).shape[0] > 1 or np.asarray(self.grid["T"]).shape[1] > 1
+        i_seg = I_SEG_3D if is3d else I_SEG_1D
+        work_seg = acc["segments_peel"] * i_seg
+        work = work_seg + acc["rays_peel"] * I_PEEL_RAY
+        dur_ms = acc["ms_peel"]
+        work_t = acc["segments_transport"] * i_seg + acc["events"] * I_EVENT
+        n_dom = max(1, acc["passes"])
+        peak = 148 * 128 * pk["sm_max_mhz"] * 1e6 / 1e12          # T lane-instr/s
+        achieved = work / (dur_ms * 1e-3) / 1e12 if dur_ms > 0 else 0.0
+        hbm_bytes = self.n_chan * self.ncell * 4 * (len(self.tab_keys) + 1 + 4)   # tables read once + alpha/prop written once
+        if self.streamed:   # Rayleigh table written once; 8 Doppler stagings (4 phases x 2 modes) each read it and write alpha + prop
+            hbm_bytes = self.n_chan * self.ncell * (4 + 8 * (4 + 4 + 16))
+        tr = PEEL_DRAM_BYTES_PER_LAUNCH.get(self.name) if self.args.packets is None else None
+        return {"bound": "alu", "kernel": "peel_kernel", "achieved": achieved, "peak": peak,
+                "unit": "Tlane-instr/s", "frac": achieved / peak if peak else None,
+                # the floor of that fraction: the ray segments alone (the per-segment count is the audited loop body), no
+                # per-ray set-up counted as work
+                "frac_segments_only": work_seg / (dur_ms * 1e-3) / 1e12 / peak if dur_ms > 0 else None,
+                "traffic": tr[0] if tr else None,
+                "traffic_unit": "dram__bytes_read + write per peel_kernel launch, ncu --set full" + (" (%s)" % tr[1] if tr else ""),
+                "peak_source": "148 SM x 128 FP32 lanes x sm_max_mhz (%s)" % pk["source"],
+                "work_lane_instr_per_launch": work / n_dom, "ms_per_launch": dur_ms / n_dom,
+                "timing_steps": steps,
+                "hbm_term": {"bytes_per_step": hbm_bytes, "ms_at_peak": hbm_bytes / (pk["hbm_gbs"] * 1e9) * 1e3,
+                             "peak_gbs": pk["hbm_gbs"]},
+                "kernel_ms_per_step": {k: acc[k] / steps for k in ("ms_stage", "ms_emission_cdf", "ms_transport", "ms_sort", "ms_peel")},
+                "transport_kernels": {"achieved": work_t / (acc["ms_transport"] * 1e-3) / 1e12 if acc["ms_transport"] > 0 else 0.0,
+                                      "frac": work_t / (acc["ms_transport"] * 1e-3) / 1e12 / peak if acc["ms_transport"] > 0 else None,
+                                      "note": "launch sort + first flights + interact generations + persistent tail, same units"},
+                "whole_step": {"achieved": (work + work_t) / (ms_total * 1e-3) / 1e12,
+                               "frac": (work + work_t) / (ms_total * 1e-3) / 1e12 / peak,
+                               "ms_per_step_timing_mode": ms_total / steps}}
+
+    def close(self):
+        self.G.close()
 
 
 def run_ours(args):
@@ -226,52 +356,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     build.build()
     binding.lib()
-
-    grid, opac, prm, mode = make_workload(args.workload, args.packets, args.channels)
-    n_chan = int(np.asarray(opac["lambda"]).size)
-    opac["chan0"] = rank_chan0(rank, n_chan)   # this rank's global channel range (keys the Philox streams)
-    N = int(prm["packets_per_channel"])
-    tab_keys = [k for k in ("k_abs", "k_sca_ray", "k_sca_cld", "g_cld", "node_kabs", "p_cell") if opac.get(k) is not None]
     stream = torch.cuda.current_stream()
-    streamed = args.workload == "cfg5"
-
-    # device-resident tables for `value`, pinned host tables for `e2e`
-    dev_opac = dict(opac)
-    host_opac = dict(opac)
-    for k in tab_keys:
-        t = torch.from_numpy(np.ascontiguousarray(opac[k], dtype=np.float32))
-        host_opac[k] = t.pin_memory()
-        dev_opac[k] = t.cuda()
-    h2d = sum(host_opac[k].numel() * 4 for k in tab_keys) + n_chan * 4
-    if streamed:   # the cells' pressures travel with every batch
-        h2d += host_opac["p_cell"].numel() * 4 * (len(wl.cfg5_batches(opac, batch=args.batch)) - 1)
-    G = binding.Grid(grid, stream=stream)
-
-    def step_streamed(op, device_outputs):
-        # config 5: per wavelength batch (+ halo channels for the Doppler window) the node tables go through
-        # gcmcrt_set_opacity_nodes, the batch's Rayleigh table is filled on the device, and the batch is run in
-        # emission and in albedo mode toward the 4 phases; counters and output bytes are summed over the runs
-        ncell = int(np.asarray(grid["T"]).size)
-        coef = torch.from_numpy(opac["k_ray_chan"]).cuda()
-        tot, nbytes = {}, 0
-        for c0, c1, lo, hi in wl.cfg5_batches(opac, batch=args.batch, halo=int(prm["doppler_halfwidth"])):
-            sub = dict(op, chan0=op["chan0"] + lo, node_kabs=op["node_kabs"][lo:hi])
-            sub["lambda"] = opac["lambda"][lo:hi]
-            sub["k_sca_ray"] = coef[lo:hi, None].expand(hi - lo, ncell).contiguous()
-            G.set_opacity_nodes(sub)
-            for fn in (G.run_emission, G.run_albedo):
-                out = fn(dict(prm, chan_begin=c0 - lo, chan_end=c1 - lo), device_outputs=device_outputs)
-                for k, v in out["counters"].items():
-                    tot[k] = tot.get(k, 0) + v
-                nbytes += sum(out[k].nbytes for k in ("flux_sum", "L_tot", "value", "sigma") if k in out and not device_outputs)
-        return {"counters": tot, "d2h_bytes": nbytes}
-
-    def step(op, device_outputs):
-        if streamed:
-            return step_streamed(op, device_outputs)
-        G.set_opacity(op)
-        fn = G.run_albedo if mode == "albedo" else G.run_emission
-        return fn(prm, device_outputs=device_outputs)
 
     def barrier():
         torch.cuda.synchronize()
@@ -279,31 +364,24 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed(op, device_outputs, steps):
-        acc = {}
-        barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        out = None
-        for _ in range(steps):
-            out = step(op, device_outputs)
-            for k, v in out["counters"].items():
-                acc[k] = acc.get(k, 0) + v
-        e1.record(stream)
-        barrier()
-        ms = e0.elapsed_time(e1)
-        return ms, acc, out
-
-    for _ in range(max(args.warmup, 3)):
-        step(dev_opac, True)
+    leg = Leg(args.workload, args, binding, torch, stream, rank)
+    N = int(leg.prm["packets_per_channel"])
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
+        leg.step(leg.dev, True, counters=None)
     sampler = ClockSampler(local)
     sampler.start()
-    ms, acc, out = timed(dev_opac, True, args.steps)
+    ms, acc, _, host_s = leg.timed(leg.dev, True, args.steps, barrier)
     clocks = sampler.summary()
+    # kernel split / roofline: the same steps with run_params.timing = 1 (host-driven pass loop, cudaEvents around the kernels)
+    t_steps = max(1, min(args.steps, 5))
+    leg.step(leg.dev, True, timing=1)
+    ms_t, acc_t, _, _ = leg.timed(leg.dev, True, t_steps, barrier, timing=1, counters="host")
     # e2e: host tables in, host spectra out
-    step(host_opac, False)
-    ms_e2e, acc_e2e, out_e2e = timed(host_opac, False, args.steps)
-    d2h = out_e2e["d2h_bytes"] if streamed else sum(out_e2e[k].nbytes for k in ("flux_sum", "L_tot", "value", "sigma") if k in out_e2e)
+    h2d = leg.pin_host_tables()
+    leg.step(leg.host, False)
+    ms_e2e, acc_e2e, outs_e2e, _ = leg.timed(leg.host, False, args.steps, barrier, counters="host")
+    d2h = leg.d2h_bytes(outs_e2e, args.steps)
 
     ms, (ev_all, seg_all) = reduce_over_ranks(ms, [acc["events"], acc["segments_transport"] + acc["segments_peel"]],
                                               world, "cuda")
@@ -313,59 +391,65 @@ def run_ours(args):
 
     if rank == 0:
         pk = peaks()
-        is3d = np.asarray(grid["T"]).shape[0] > 1 or np.asarray(grid["T"]).shape[1] > 1
-        i_seg = I_SEG_3D if is3d else I_SEG_1D
-        # dominant kernel: peel_kernel, one launch per pass (the transport side of a pass is a sequence of smaller
-        # kernels: launch-order sort, first flights, one interact kernel per generation, the persistent tail).
-        # cudaEvents recorded by the library on the caller's stream around every launch give its device time.
-        dom = "peel"
-        work = acc["segments_peel"] * i_seg + acc["rays_peel"] * I_PEEL_RAY
-        dur_ms = acc["ms_peel"]
-        work_t = acc["segments_transport"] * i_seg + acc["events"] * I_EVENT
-        n_dom = max(1, acc["passes"])
-        peak = 148 * 128 * pk["sm_max_mhz"] * 1e6 / 1e12          # T lane-instr/s
-        achieved = work / (dur_ms * 1e-3) / 1e12 if dur_ms > 0 else 0.0
-        ncell = int(np.asarray(grid["T"]).size)
-        hbm_bytes = n_chan * ncell * 4 * (len(tab_keys) + 1 + 4)   # tables read once + alpha/prop written once
-        if streamed:   # Rayleigh table written once; 8 Doppler stagings (4 phases x 2 modes) each read it and write alpha + prop
-            hbm_bytes = n_chan * ncell * (4 + 8 * (4 + 4 + 16))
-        roofline = {"bound": "alu", "kernel": dom + "_kernel", "achieved": achieved, "peak": peak,
-                    "unit": "Tlane-instr/s", "frac": achieved / peak if peak else None,
-                    # dram__bytes_read + write per peel_kernel launch from one ncu --set full capture of the default
-                    # workload (profiles/ncu_full_r01d_ptx_loops.txt); other workloads: not captured
-                    "traffic": PEEL_DRAM_BYTES_PER_LAUNCH_CFG2 if (args.workload == "cfg2" and args.packets is None) else None,
-                    "traffic_unit": "bytes per launch (94 M events: 64 B record + 4 B permutation entry + extinction gathers)",
-                    "peak_source": "148 SM x 128 FP32 lanes x sm_max_mhz (%s)" % pk["source"],
-                    "work_lane_instr_per_launch": work / n_dom, "ms_per_launch": dur_ms / n_dom,
-                    "hbm_term": {"bytes_per_step": hbm_bytes, "ms_at_peak": hbm_bytes / (pk["hbm_gbs"] * 1e9) * 1e3 * 1.0,
-                                 "peak_gbs": pk["hbm_gbs"]},
-                    "kernel_ms_per_step": {k: acc[k] / args.steps for k in ("ms_stage", "ms_emission_cdf", "ms_transport", "ms_sort", "ms_peel")},
-                    "transport_kernels": {"achieved": work_t / (acc["ms_transport"] * 1e-3) / 1e12 if acc["ms_transport"] > 0 else 0.0,
-                                          "frac": work_t / (acc["ms_transport"] * 1e-3) / 1e12 / peak if acc["ms_transport"] > 0 else None,
-                                          "note": "launch sort + first flights + interact generations + persistent tail, same units"},
-                    "whole_step": {"achieved": (work + work_t) / (ms / args.steps * 1e-3 * args.steps) / 1e12,
-                                   "frac": (work + work_t) / (ms * 1e-3) / 1e12 / peak}}
-        # config 5 has no per-cell table for the oracle to read (328 GB at full size): no cpu_baseline leg there
-        cpu = oracle_leg(args.workload, grid, dict(opac, chan0=0), prm, mode) if world == 1 and not args.no_cpu and not streamed else None
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+                "warmup": warm, "ms_per_step": ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": args.workload, "mode": mode, "n_chan_per_gpu": n_chan, "packets_per_channel": N,
-                           "n_obs": int(np.asarray(prm["obs_dir"]).reshape(-1, 3).shape[0]),
-                           "grid": list(np.asarray(grid["T"]).shape), "parallelism": "channels x %d" % world,
+                "config": {"workload": args.workload, "mode": leg.mode, "n_chan_per_gpu": leg.n_chan, "packets_per_channel": N,
+                           "n_obs": int(np.asarray(leg.prm["obs_dir"]).reshape(-1, 3).shape[0]),
+                           "grid": list(np.asarray(leg.grid["T"]).shape), "parallelism": "channels x %d" % world,
                            "l2": "opacity tables (%.0f MB) + staged tables exceed the 126 MB L2; no flush" % (h2d / 1e6)},
                 "events_per_step": ev_all / args.steps, "segments_per_s": seg_all / (ms * 1e-3),
                 "spectra_per_s": world * args.steps / (ms * 1e-3),
+                "host_enqueue_ms_per_step": host_s * 1e3 / args.steps,
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                         "ms_per_step": ms_e2e / args.steps},
-                "gpu_launches": int(acc["launches"]), "clocks": clocks, "roofline": roofline,
+                "gpu_launches": int(acc["launches"]), "clocks": clocks, "roofline": leg.roofline(acc_t, ms_t, t_steps, pk),
                 "counters_per_step": {k: acc[k] / args.steps for k in
                                       ("events", "segments_transport", "segments_peel", "rays_peel", "packets_escaped",
                                        "packets_absorbed", "packets_surface", "packets_stuck", "passes")}}
-        if cpu is not None:
+        assert acc["device_status"] == 0, "pass loop reported an error"
+        # config 5 has no per-cell table for the oracle to read (328 GB at full size): no cpu_baseline leg there
+        if world == 1 and not args.no_cpu and not leg.streamed:
+            o0 = dict(leg.opac, chan0=0)
+            cpu = oracle_leg(args.workload, leg.grid, o0, leg.prm, leg.mode)
             line["cpu_baseline"] = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+            cpu1 = oracle_leg(args.workload, leg.grid, o0, leg.prm, leg.mode, budget_s=8.0, threads=1)
+            line["cpu_baseline_1core"] = {k: cpu1[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        # the other configurations north_star names (3D correlated-k emission, high resolution): short legs of their
+        # own after the headline, outside its timed region
+        if world == 1 and args.workload == "cfg2" and args.packets is None and not args.no_extra:
+            extra = {}
+
+            def short_leg(lg):
+                for _ in range(3):
+                    lg.step(lg.dev, True, counters=None)
+                ms_x, acc_x, _, _ = lg.timed(lg.dev, True, 3, barrier)
+                lg.step(lg.dev, True, timing=1)
+                ms_xt, acc_xt, _, _ = lg.timed(lg.dev, True, 2, barrier, timing=1, counters="host")
+                return {"ms_per_step": ms_x / 3, "value": acc_x["events"] / (ms_x * 1e-3), "unit": UNIT, "steps": 3, "warmup": 3,
+                        "config": {"workload": lg.name, "mode": lg.mode, "n_chan_per_gpu": lg.n_chan,
+                                   "packets_per_channel": int(lg.prm["packets_per_channel"]),
+                                   "n_obs": int(np.asarray(lg.prm["obs_dir"]).reshape(-1, 3).shape[0]),
+                                   "grid": list(np.asarray(lg.grid["T"]).shape)},
+                        "rays_per_s": acc_x["rays_peel"] / (ms_x * 1e-3),
+                        "roofline": lg.roofline(acc_xt, ms_xt, 2, pk)}
+
+            # config 3: the same grid and tables as config 2, so the tables already on the device serve it
+            _, _, p3 = wl.cfg3(packets=1000000)
+            lg = Leg("cfg3", args, binding, torch, stream, rank, leg.grid, leg.opac, p3, "emission", dev_tables=leg.dev)
+            extra["cfg3"] = short_leg(lg)
+            lg.close()
+            leg.close()
+            leg.dev = lg.dev = None
+            torch.cuda.empty_cache()
+            # config 4 on 2000 of its 1e4 wavelength points (the full table takes minutes of numpy to generate)
+            lg = Leg("cfg4", args, binding, torch, stream, rank)
+            extra["cfg4"] = short_leg(lg)
+            lg.close()
+            line["workloads"] = extra
         print(json.dumps(line), flush=True)
-    G.close()
+    if leg.G.handle:
+        leg.close()
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -381,7 +465,8 @@ def main():
     ap.add_argument("--channels", type=int, default=None, help="cfg4 / cfg5: number of wavelength points (default 10000 / 4096)")
     ap.add_argument("--batch", type=int, default=1024, help="cfg5: wavelength points per streamed opacity batch")
     ap.add_argument("--packets", type=int, default=None, help="override packets per channel (debugging only)")
-    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline legs")
+    ap.add_argument("--no-extra", action="store_true", help="skip the cfg3 / cfg4 legs of the default run")
     args = ap.parse_args()
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "ours" and world != args.gpus and world == 1 and args.gpus > 1:

@@ -24,9 +24,26 @@
  *    by the runs (once for an unshifted run, once per observer with doppler_on, Eq. 33-34).  Host
  *    tables are copied to internal device buffers during the call.  Output buffers are caller-owned.
  *  - STREAMS: all work is enqueued on `stream` (a cudaStream_t passed as void*, NULL = legacy
- *    default stream).  gcmcrt_run_* synchronise with the stream only to read two pass counters per
- *    pass (a few bytes); results are complete when the stream has drained (or on return for host
- *    output pointers, which are copied with a final stream synchronisation).
+ *    default stream) and the calls return without waiting for the device: a run's pass loop (fresh
+ *    packets -> events -> peel-off, repeated until every packet has ended) is a conditional WHILE
+ *    node of a CUDA graph whose bookkeeping runs in device memory.  Results in DEVICE memory
+ *    (gcmcrt_result pointers, counters included) are complete when the stream has drained; an
+ *    output pointer in HOST memory is filled by a copy at the end of the call followed by ONE
+ *    stream synchronisation.  The other places that wait for the device: gcmcrt_grid_create,
+ *    gcmcrt_destroy, a run with run_params.timing = 1 (profiling), the test-only gcmcrt_debug_*
+ *    calls, lambda given in device memory, and cudaMalloc / cudaFree when an internal buffer has
+ *    to grow (first call, or a larger run than any before on the handle).
+ *    A run may be issued while `stream` is being captured (cudaStreamBeginCapture): its work,
+ *    loop included, becomes part of the caller's graph.  Requirements then: every buffer exists
+ *    already (one earlier run of the same size on the handle), all outputs are device memory,
+ *    timing = 0, and the capture mode permits cudaStreamBeginCaptureToGraph on an internal stream
+ *    (cudaStreamCaptureModeRelaxed or thread-local).
+ *  - ENVIRONMENT (read once per handle, for tests and tuning experiments; unset = defaults):
+ *    GCMCRT_EVENT_CAP=<n> fixes the event-buffer capacity in records (default: 4 per packet of the
+ *    run, 1 Mi .. 128 Mi); GCMCRT_TUNE="a,b,c,d" = lanes waiting before the persistent kernel
+ *    serves them (16), lanes parked at a cone / half-plane before a warp serves them (1), wavefront
+ *    generations per pass (8; 0 = persistent kernel only), first-pass batch divisor (4).  Neither
+ *    changes any result beyond the summation order.
  *  - ERRORS: every function returns 0 on success or a negative gcmcrt_status; nothing throws or
  *    exits.  gcmcrt_last_error() returns a static, human-readable description of the last failure
  *    on that handle (or of the last failed gcmcrt_grid_create when passed NULL).
@@ -206,8 +223,8 @@ int gcmcrt_run_emission(gcmcrt_grid *grid, const gcmcrt_run_params *params, gcmc
 
 /*
  * gcmcrt_run_transmission -- transmission spectrum by random transit chords (Sect. 5.1, Eq. 20-21) with multiple
- * scattering off (L259: "a raytracer scheme with random transit chord sampler"; the paper gives no formula for the
- * scattered contribution).  Packet i of a channel draws an impact parameter b_i uniform in [R_p0, R_TOA] and an
+ * scattering off (L261: "a raytracer scheme with random transit chord sampler"; the scheme with scattering, L259, is
+ * described in words only).  Packet i of a channel draws an impact parameter b_i uniform in [R_p0, R_TOA] and an
  * azimuth around the limb; tau_i is the extinction optical depth of the whole chord along obs_dir (planet -> observer)
  * -- with doppler_on through that observer's Doppler-shifted table (Eq. 33-34, the set-up of the paper's Sect. 13).
  *   flux_sum[c][o][batch] = sum_i W_i [1 - exp(-tau_i)] b_i      (W_i: limb darkening, Eq. 22-23; 1 if star_radius = 0)
@@ -227,8 +244,8 @@ const char *gcmcrt_last_error(const gcmcrt_grid *grid);
 /*
  * gcmcrt_debug_ray_tau -- test-only: optical depth of channel `chan` (local index) from pos[m] along dir[m] to
  * the TOA with the peel-off ray integrator (A7), without a run.  hit_surface[m] = 1 when the ray ends on the
- * lower boundary (tau then is the depth down to it).  obs_index >= 0 selects that observer's Doppler-shifted
- * table (requires a previous run with doppler_on), -1 the unshifted one.
+ * lower boundary (tau then is the depth down to it).  The ray runs through the table staged last: the unshifted one
+ * (staged by this call if no run has staged anything yet), or the Doppler table of the last doppler_on run's observer.
  *   pos, dir  host|device [n][3] float; tau host|device [n] float; hit_surface host|device [n] int (nullable)
  */
 int gcmcrt_debug_ray_tau(gcmcrt_grid *grid, int chan, long n, const float *pos, const float *dir,

@@ -163,7 +163,7 @@ int orc_channel_prep(const orc_grid *g, const orc_opacity *op, const orc_params 
 /* The two drivers (section 3 call stacks). */
 int orc_run_albedo(const orc_grid *g, const orc_opacity *op, const orc_params *prm, orc_result *out);
 int orc_run_emission(const orc_grid *g, const orc_opacity *op, const orc_params *prm, orc_result *out);
-/* Transmission spectrum by random transit chords (Sect. 5.1, Eq. 20-21), multiple scattering off (L259: "reduces the
+/* Transmission spectrum by random transit chords (Sect. 5.1, Eq. 20-21), multiple scattering off (L261: "reduces the
  * model to a raytracer scheme with random transit chord sampler"): flux_sum[c][o][batch] = sum over packets of
  * W [1 - exp(-tau_i)] b_i; <I_p> = (R_TOA - R_p0) / N * sum (Eq. 21); W from Eq. 22-23. */
 int orc_run_transmission(const orc_grid *g, const orc_opacity *op, const orc_params *prm, orc_result *out);

@@ -52,6 +52,8 @@ struct gcmcrt_grid {
     // current opacity table
     int chan0 = 0, n_chan = 0;
     std::vector<float> lambda;
+    std::vector<double> lambda64_h;
+    std::vector<float> reff_h;
     DevBuf own_kabs, own_kray, own_kcld, own_g;   // copies of host-resident inputs
     const float *k_abs = nullptr, *k_ray = nullptr, *k_cld = nullptr, *g_cld = nullptr;
     DevBuf alpha, alpha2, prop, reff, vlos, lambda64;
@@ -78,6 +80,11 @@ struct gcmcrt_grid {
     int tune[4] = {16, 1, 8, 4};
     PassCtrl* h_ctrl = nullptr;  // pinned (timed runs read the pass outcome back)
     cudaStream_t cap_stream = nullptr;   // the body of the pass loop is captured on this stream into the WHILE node's graph
+    // instantiated pass-loop graphs, keyed by the bytes of everything their kernels were captured with: a repeated run
+    // relaunches its graph.  cudaGraphExecDestroy waits for a graph in flight, so a graph that is pushed out of this small
+    // cache is only released once the event recorded behind its last launch has completed.
+    struct LoopGraph { std::vector<unsigned char> key; cudaGraphExec_t exec = nullptr; cudaEvent_t done = nullptr; };
+    std::vector<LoopGraph> loops, retired;
     cudaEvent_t tev[4] = {nullptr, nullptr, nullptr, nullptr};   // kernel timing (A0 | A2 | transport | peel)
     unsigned long long launches = 0, launches_pending = 0;
     double ms_stage = 0.0, ms_emis = 0.0, ms_transport = 0.0, ms_peel = 0.0, ms_sort = 0.0;
@@ -298,17 +305,26 @@ struct PassLaunch {
     WaveConst wc;
     SortParams sp, spl;
     PassPlan plan;
-    PassCtrl* ctrl = nullptr;
-    bool emission = false, has_obs = false;
-    int n_gen = 0, n_gen_run = 0;
-    unsigned grid_t = 1, grid_f = 1, grid_i = 1, grid_p = 1, grid_k = 1;
-    size_t smem_t = 0, smem_w = 0, smem_i = 0, smem_p = 0;
-    decltype(&transport_kernel<4, false>) tk = nullptr;
-    decltype(&peel_kernel<16>) pk = nullptr;
-    decltype(&wave_first_flight_kernel<16, false>) k_first = nullptr;
-    decltype(&wave_interact_kernel<kInteractK, false>) k_inter = nullptr;
-    unsigned long long tail_items = 0;
-};
+    PassCtrl* ctrl;
+    int emission, has_obs;
+    int n_gen, n_gen_run;
+    unsigned grid_t, grid_f, grid_i, grid_p, grid_k;
+    size_t smem_t, smem_w, smem_i, smem_p;
+    decltype(&transport_kernel<4, false>) tk;
+    decltype(&peel_kernel<16>) pk;
+    decltype(&wave_first_flight_kernel<16, false>) k_first;
+    decltype(&wave_interact_kernel<kInteractK, false>) k_inter;
+    unsigned long long tail_items;
+};   // zero-filled with memset before use: its bytes are the key of the graph cache
+
+// kernels one pass launches (what enqueue_pass counts)
+unsigned launches_per_pass(const PassLaunch& L)
+{
+    unsigned nl = 3;   // pass_begin, the persistent transport kernel, pass_end
+    if (L.n_gen > 0) nl += (L.emission ? 1u : 6u) + unsigned(L.n_gen_run);
+    if (L.has_obs) nl += 5u + (L.ev.hist ? 0u : 1u);
+    return nl;
+}
 
 // Enqueue one pass on `s` (the caller's stream in a timed run, the capture stream of the loop body otherwise).
 // tev != NULL: cudaEvents around the transport side, the event sort and the peel kernel.
@@ -338,12 +354,12 @@ int enqueue_pass(gcmcrt_grid* g, const PassLaunch& L, cudaStream_t s, cudaEvent_
             wave_emit_kernel<<<L.grid_k, kWaveThreads, L.smem_w, s>>>(L.rc, L.ev, L.susp, wc);
             nl += 1;
         }
-        CUDA_TRY(g, cudaMemcpyAsync(&ctrl->gen_mark[1], &ctrl->ev_count, sizeof(unsigned int), cudaMemcpyDeviceToDevice, s));
+        gen_mark_kernel<<<1, 1, 0, s>>>(ctrl, 1);
         for (int gi = 0; gi < L.n_gen_run; ++gi) {
             wc.gen_mark = &ctrl->gen_mark[gi];
             wc.park_all = gi == L.n_gen - 1;
             L.k_inter<<<L.grid_i, kWaveThreads, L.smem_i, s>>>(L.rc, L.ev, L.susp, wc);
-            CUDA_TRY(g, cudaMemcpyAsync(&ctrl->gen_mark[gi + 2], &ctrl->ev_count, sizeof(unsigned int), cudaMemcpyDeviceToDevice, s));
+            gen_mark_kernel<<<1, 1, 0, s>>>(ctrl, gi + 2);
         }
         nl += unsigned(L.n_gen_run);
     }
@@ -373,8 +389,25 @@ int enqueue_pass(gcmcrt_grid* g, const PassLaunch& L, cudaStream_t s, cudaEvent_
 // the condition.  Nothing here waits for the device.  When the caller's stream is itself being captured the node is
 // added to the caller's graph (a graph that holds a conditional node cannot be a child graph); otherwise a graph of its
 // own is instantiated, launched on the caller's stream and released (an executable graph in flight is freed on completion).
+void reap_retired_loops(gcmcrt_grid* g, bool wait)
+{
+    for (size_t m = 0; m < g->retired.size();) {
+        gcmcrt_grid::LoopGraph& lg = g->retired[m];
+        if (wait || cudaEventQuery(lg.done) == cudaSuccess) {
+            if (wait) cudaEventSynchronize(lg.done);
+            cudaGraphExecDestroy(lg.exec);
+            cudaEventDestroy(lg.done);
+            g->retired.erase(g->retired.begin() + m);
+        } else {
+            ++m;
+        }
+    }
+    cudaGetLastError();   // cudaEventQuery reports "not ready" through the error state
+}
+
 int launch_pass_loop(gcmcrt_grid* g, const PassLaunch& L, cudaStream_t s, unsigned* n_launch)
 {
+    constexpr size_t kLoopCache = 16;
     if (!g->cap_stream) CUDA_TRY(g, cudaStreamCreateWithFlags(&g->cap_stream, cudaStreamNonBlocking));
     cudaStreamCaptureStatus cst = cudaStreamCaptureStatusNone;
     CUDA_TRY(g, cudaStreamIsCapturing(s, &cst));
@@ -382,7 +415,20 @@ int launch_pass_loop(gcmcrt_grid* g, const PassLaunch& L, cudaStream_t s, unsign
     const cudaGraphNode_t* deps = nullptr;
     size_t n_deps = 0;
     const bool own = cst != cudaStreamCaptureStatusActive;
+    const unsigned char* kb = reinterpret_cast<const unsigned char*>(&L);
     if (own) {
+        reap_retired_loops(g, false);
+        for (size_t m = 0; m < g->loops.size(); ++m) {
+            if (g->loops[m].key.size() == sizeof L && std::memcmp(g->loops[m].key.data(), kb, sizeof L) == 0) {
+                gcmcrt_grid::LoopGraph lg = g->loops[m];   // most recently used goes to the back
+                g->loops.erase(g->loops.begin() + m);
+                g->loops.push_back(lg);
+                if (n_launch) *n_launch = launches_per_pass(L);
+                CUDA_TRY(g, cudaGraphLaunch(lg.exec, s));
+                CUDA_TRY(g, cudaEventRecord(lg.done, s));
+                return GCMCRT_OK;
+            }
+        }
         CUDA_TRY(g, cudaGraphCreate(&graph, 0));
     } else {
         unsigned long long id = 0;
@@ -408,10 +454,19 @@ int launch_pass_loop(gcmcrt_grid* g, const PassLaunch& L, cudaStream_t s, unsign
         if (rcode == GCMCRT_OK && e != cudaSuccess) rcode = fail(g, GCMCRT_E_CUDA, std::string("pass loop capture: ") + cudaGetErrorString(e));
         if (rcode != GCMCRT_OK) break;
         if (own) {
-            cudaGraphExec_t exec = nullptr;
-            e = cudaGraphInstantiate(&exec, graph, 0);
-            if (e == cudaSuccess) e = cudaGraphLaunch(exec, s);
-            if (exec) cudaGraphExecDestroy(exec);
+            gcmcrt_grid::LoopGraph lg;
+            e = cudaGraphInstantiate(&lg.exec, graph, 0);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lg.done, cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaGraphLaunch(lg.exec, s);
+            if (e == cudaSuccess) e = cudaEventRecord(lg.done, s);
+            if (e == cudaSuccess) {
+                lg.key.assign(kb, kb + sizeof L);
+                if (g->loops.size() >= kLoopCache) { g->retired.push_back(g->loops.front()); g->loops.erase(g->loops.begin()); }
+                g->loops.push_back(lg);
+            } else {
+                if (lg.done) cudaEventDestroy(lg.done);
+                if (lg.exec) cudaGraphExecDestroy(lg.exec);
+            }
         } else {
             e = cudaStreamUpdateCaptureDependencies(s, &node, 1, cudaStreamSetCaptureDependencies);
         }
@@ -501,13 +556,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
 
     // ---- constants of the run
     PassLaunch L;
-    std::memset(&L.rc, 0, sizeof L.rc);
-    std::memset(&L.ev, 0, sizeof L.ev);
-    std::memset(&L.susp, 0, sizeof L.susp);
-    std::memset(&L.wc, 0, sizeof L.wc);
-    std::memset(&L.sp, 0, sizeof L.sp);
-    std::memset(&L.spl, 0, sizeof L.spl);
-    std::memset(&L.plan, 0, sizeof L.plan);
+    std::memset(static_cast<void*>(&L), 0, sizeof L);
+    L.grid_t = L.grid_f = L.grid_i = L.grid_p = L.grid_k = 1;
     RunConst& rc = L.rc;
     rc.geom = geom_params(g);
     rc.chan_key0 = uint32_t(g->chan0);
@@ -557,7 +607,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     const bool cont = prm->continuous_absorption != 0;
     L.tk = cont ? transport_kernel<4, true> : transport_kernel<4, false>;
     L.pk = peel_kernel<16>;
-    L.emission = emission != 0;
+    L.emission = emission != 0 ? 1 : 0;
     L.smem_t = smem_t;
     if (mode != 2) {
         CUDA_TRY(g, cudaFuncSetAttribute(L.tk, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_t)));
@@ -691,7 +741,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         }
 
         // ---- the pass loop of this run
-        L.has_obs = rc.n_obs_run > 0;
+        L.has_obs = rc.n_obs_run > 0 ? 1 : 0;
         const size_t smem_p = (size_t((g->tab_floats + 31) & ~31) + size_t(kPeelThreads / 32) * rc.n_obs_run * nb) * sizeof(float);
         L.smem_p = smem_p;
         if (L.has_obs) {
@@ -992,8 +1042,11 @@ static int set_opacity_common(gcmcrt_grid* g, int chan0, int n_chan, const float
     for (int c = 0; c < n_chan; ++c)
         if (!(lam[c] > 0.f)) return fail(g, GCMCRT_E_INVALID, "lambda must be positive");
     g->lambda = lam;
-    std::vector<double> lam64(lam.begin(), lam.end());
-    std::vector<float> reff(n_chan, 0.f);
+    // staging vectors owned by the handle: the uploads below are asynchronous
+    std::vector<double>& lam64 = g->lambda64_h;
+    std::vector<float>& reff = g->reff_h;
+    lam64.assign(lam.begin(), lam.end());
+    reff.assign(n_chan, 0.f);
     for (int c = 0; c < n_chan && n_chan > 1; ++c) {
         const int c1 = c + 1 < n_chan ? c : c - 1;
         const double ratio = double(lam[c1 + 1]) / double(lam[c1]);
@@ -1001,7 +1054,6 @@ static int set_opacity_common(gcmcrt_grid* g, int chan0, int n_chan, const float
     }
     CUDA_TRY(g, upload(g->lambda64, lam64, s));
     CUDA_TRY(g, upload(g->reff, reff, s));
-    CUDA_TRY(g, cudaStreamSynchronize(s));
     g->chan0 = chan0;
     g->n_chan = n_chan;
     g->launches = 0;
@@ -1039,6 +1091,9 @@ int gcmcrt_destroy(gcmcrt_grid* g)
                       &g->value, &g->sigma, &g->image, &g->evcount, &g->contrib})
         b->release();
     if (g->h_ctrl) cudaFreeHost(g->h_ctrl);
+    for (auto& lg : g->loops) g->retired.push_back(lg);
+    g->loops.clear();
+    reap_retired_loops(g, true);
     if (g->cap_stream) cudaStreamDestroy(g->cap_stream);
     for (auto& e : g->tev) if (e) cudaEventDestroy(e);
     delete g;

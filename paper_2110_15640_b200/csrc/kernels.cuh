@@ -84,6 +84,15 @@ struct PassCtrl;
 struct SuspPair {   // the two suspended lists; which one a pass reads is part of the pass plan (PassCtrl::cur)
     SuspBuf b[2];
 };
+// field-by-field selects: indexing the kernel parameter with a run-time value would copy it to the stack
+__device__ __forceinline__ SuspBuf susp_select(const SuspPair& p, int which)
+{
+    SuspBuf s;
+    s.s0 = which ? p.b[1].s0 : p.b[0].s0; s.s1 = which ? p.b[1].s1 : p.b[0].s1; s.s2 = which ? p.b[1].s2 : p.b[0].s2;
+    s.count = which ? p.b[1].count : p.b[0].count; s.taken = which ? p.b[1].taken : p.b[0].taken;
+    s.cap = which ? p.b[1].cap : p.b[0].cap;
+    return s;
+}
 
 struct DevCounters {
     unsigned long long events, seg_transport, seg_peel, escaped, absorbed, surface, stuck, rays_peel;
@@ -130,6 +139,10 @@ __global__ void run_begin_kernel(PassCtrl* c, const PassPlan p)
     c->passes = passes; c->error = error;
     c->batch = p.batch0;
 }
+
+// end of a generation: the events written so far (a kernel, not a 4-byte copy: a memcpy node inside the loop body of
+// the graph costs tens of microseconds)
+__global__ void gen_mark_kernel(PassCtrl* c, int m) { c->gen_mark[m] = c->ev_count; }
 
 __global__ void pass_begin_kernel(PassCtrl* c, const PassPlan p)
 {
@@ -707,7 +720,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
     const GeomSmem gs = load_geom(rc.geom, smem_f);
     __syncthreads();
     const int cur_list = rc.ctrl->cur;
-    const SuspBuf susp_in = susp.b[cur_list], susp_out = susp.b[1 - cur_list];
+    const SuspBuf susp_in = susp_select(susp, cur_list), susp_out = susp_select(susp, 1 - cur_list);
 
     Packet pk;
     pk.tau = 0.f; pk.tau_t = 0.f; pk.tau_b = 0.f; pk.W = 0.f; pk.chan_run = 0; pk.pkt = 0; pk.m_inter = 0; pk.nev = 0; pk.fl_seg = 0;

@@ -280,7 +280,7 @@ wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
     extern __shared__ float smem_f[];
     const GeomSmem gs = load_geom(rc.geom, smem_f);
     __syncthreads();
-    const SuspBuf susp = susp2.b[rc.ctrl->cur];
+    const SuspBuf susp = susp_select(susp2, rc.ctrl->cur);
     const unsigned int n_items = rc.ctrl->n_fresh;
     const unsigned long long item0 = rc.ctrl->item0;
     WaveCounters wcnt;
@@ -343,7 +343,7 @@ __global__ void __launch_bounds__(kWaveThreads) wave_emit_kernel(const __grid_co
     extern __shared__ float smem_f[];
     const GeomSmem gs = load_geom(rc.geom, smem_f);
     __syncthreads();
-    const SuspBuf susp = susp2.b[rc.ctrl->cur];
+    const SuspBuf susp = susp_select(susp2, rc.ctrl->cur);
     const unsigned int n_items = rc.ctrl->n_fresh;
     const unsigned long long item0 = rc.ctrl->item0;
     WaveCounters wcnt;
@@ -416,7 +416,7 @@ wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, con
 {
     extern __shared__ float smem_f[];
     const GeomSmem gs = load_geom(rc.geom, smem_f);
-    const SuspBuf susp = susp2.b[rc.ctrl->cur];
+    const SuspBuf susp = susp_select(susp2, rc.ctrl->cur);
     // survivors of the absorb / scatter decision wait here until a full warp of them has gathered
     float* stage = smem_f + ((rc.geom.tab_floats + 31) & ~31) + (threadIdx.x >> 5) * (kStageFields * kStageSlots);
     __syncthreads();

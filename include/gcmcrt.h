@@ -43,7 +43,9 @@
  *    run, 1 Mi .. 128 Mi); GCMCRT_TUNE="a,b,c,d" = lanes waiting before the persistent kernel
  *    serves them (16), lanes parked at a cone / half-plane before a warp serves them (1), wavefront
  *    generations per pass (8; 0 = persistent kernel only), first-pass batch divisor (4).  Neither
- *    changes any result beyond the summation order.
+ *    changes any result beyond the summation order.  GCMCRT_HOST_LOOP=1 makes the host drive the
+ *    pass loop (one wait per pass, no events): profilers (ncu) do not list kernels that run inside
+ *    a conditional graph node, so profile with this or with run_params.timing = 1.
  *  - ERRORS: every function returns 0 on success or a negative gcmcrt_status; nothing throws or
  *    exits.  gcmcrt_last_error() returns a static, human-readable description of the last failure
  *    on that handle (or of the last failed gcmcrt_grid_create when passed NULL).

@@ -523,6 +523,9 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     if (ncr > (1 << 24)) return fail(g, GCMCRT_E_INVALID, "too many channels in one run");
     const int npix = prm->npix > 0 && out->image ? prm->npix : 0;
     const bool timed = prm->timing != 0;   // host-synchronous pass loop with cudaEvents around the kernels
+    // GCMCRT_HOST_LOOP=1: the host drives the pass loop (one wait per pass) without recording events -- for profilers,
+    // which do not see kernels launched from inside a conditional graph node
+    static const bool host_loop_env = std::getenv("GCMCRT_HOST_LOOP") && std::atoi(std::getenv("GCMCRT_HOST_LOOP")) != 0;
 
     int rcode = ensure_workspace(g, (unsigned long long)ncr * (hi - lo));
     if (rcode) return rcode;
@@ -835,18 +838,20 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         L.plan.n_pkt = uint32_t(n_pkt); L.plan.ev_cap = g->ev_cap; L.plan.n_gen = n_gen; L.plan.n_chan_run = ncr;
         run_begin_kernel<<<1, 1, 0, s>>>(ctrl, L.plan);
         ++g->launches;
-        if (!timed) {
+        if (!timed && !host_loop_env) {
             if ((rcode = launch_pass_loop(g, L, s, &launches_per_pass))) return rcode;
         } else {
             for (;;) {
-                if ((rcode = enqueue_pass(g, L, s, g->tev, cudaGraphConditionalHandle{}, 0, &launches_per_pass))) return rcode;
+                if ((rcode = enqueue_pass(g, L, s, timed ? g->tev : nullptr, cudaGraphConditionalHandle{}, 0, &launches_per_pass))) return rcode;
                 CUDA_TRY(g, cudaMemcpyAsync(g->h_ctrl, ctrl, sizeof(PassCtrl), cudaMemcpyDeviceToHost, s));
                 CUDA_TRY(g, cudaStreamSynchronize(s));
-                float a = 0.f, b = 0.f, c = 0.f;
-                CUDA_TRY(g, cudaEventElapsedTime(&a, g->tev[0], g->tev[1]));
-                CUDA_TRY(g, cudaEventElapsedTime(&b, g->tev[1], g->tev[2]));
-                CUDA_TRY(g, cudaEventElapsedTime(&c, g->tev[2], g->tev[3]));
-                g->ms_transport += a; g->ms_sort += b; g->ms_peel += c;
+                if (timed) {
+                    float a = 0.f, b = 0.f, c = 0.f;
+                    CUDA_TRY(g, cudaEventElapsedTime(&a, g->tev[0], g->tev[1]));
+                    CUDA_TRY(g, cudaEventElapsedTime(&b, g->tev[1], g->tev[2]));
+                    CUDA_TRY(g, cudaEventElapsedTime(&c, g->tev[2], g->tev[3]));
+                    g->ms_transport += a; g->ms_sort += b; g->ms_peel += c;
+                }
                 if (g->h_ctrl->error == 1) return fail(g, GCMCRT_E_CUDA, "suspended-packet list overflow");
                 if (g->h_ctrl->error) return fail(g, GCMCRT_E_CUDA, "pass loop did not terminate");
                 if (g->h_ctrl->done) break;

@@ -267,13 +267,18 @@ class Leg:
         # gcmcrt_set_opacity_nodes, the batch's Rayleigh table is filled on the device, and the batch is run in
         # emission and in albedo mode toward the 4 phases
         outs = []
+        obs = np.asarray(prm["obs_dir"], dtype=np.float64).reshape(-1, 3)
         for c0, c1, lo, hi in wl.cfg5_batches(self.opac, batch=self.args.batch, halo=int(prm["doppler_halfwidth"])):
             sub = dict(op, chan0=op["chan0"] + lo, node_kabs=op["node_kabs"][lo:hi])
             sub["lambda"] = self.opac["lambda"][lo:hi]
             sub["k_sca_ray"] = self.coef[lo:hi, None].expand(hi - lo, self.ncell).contiguous()
             G.set_opacity_nodes(sub)
-            for fn in (G.run_emission, G.run_albedo):
-                outs.append(fn(dict(prm, chan_begin=c0 - lo, chan_end=c1 - lo), device_outputs=device_outputs, counters=counters))
+            # with doppler_on every observer is a run of its own on its own shifted table (L326-328): phases outermost,
+            # so that the emission and the albedo run toward a phase share one Doppler staging (4 per batch, not 8)
+            for o in range(obs.shape[0]):
+                for fn in (G.run_emission, G.run_albedo):
+                    outs.append(fn(dict(prm, obs_dir=obs[o:o + 1], chan_begin=c0 - lo, chan_end=c1 - lo),
+                                   device_outputs=device_outputs, counters=counters))
         return outs
 
     def sum_counters(self, outs):
@@ -314,8 +319,8 @@ class Leg:
         peak = 148 * 128 * pk["sm_max_mhz"] * 1e6 / 1e12          # T lane-instr/s
         achieved = work / (dur_ms * 1e-3) / 1e12 if dur_ms > 0 else 0.0
         hbm_bytes = self.n_chan * self.ncell * 4 * (len(self.tab_keys) + 1 + 4)   # tables read once + alpha/prop written once
-        if self.streamed:   # Rayleigh table written once; 8 Doppler stagings (4 phases x 2 modes) each read it and write alpha + prop
-            hbm_bytes = self.n_chan * self.ncell * (4 + 8 * (4 + 4 + 16))
+        if self.streamed:   # Rayleigh table written once; 4 Doppler stagings (one per phase) each read it and write alpha + prop
+            hbm_bytes = self.n_chan * self.ncell * (4 + 4 * (4 + 4 + 16))
         tr = PEEL_DRAM_BYTES_PER_LAUNCH.get(self.name) if self.args.packets is None else None
         return {"bound": "alu", "kernel": "peel_kernel", "achieved": achieved, "peak": peak,
                 "unit": "Tlane-instr/s", "frac": achieved / peak if peak else None,

@@ -81,9 +81,11 @@ struct gcmcrt_grid {
     PassCtrl* h_ctrl = nullptr;  // pinned (timed runs read the pass outcome back)
     cudaStream_t cap_stream = nullptr;   // the body of the pass loop is captured on this stream into the WHILE node's graph
     // instantiated pass-loop graphs, keyed by the bytes of everything their kernels were captured with: a repeated run
-    // relaunches its graph.  cudaGraphExecDestroy waits for a graph in flight, so a graph that is pushed out of this small
-    // cache is only released once the event recorded behind its last launch has completed.
-    struct LoopGraph { std::vector<unsigned char> key; cudaGraphExec_t exec = nullptr; cudaEvent_t done = nullptr; };
+    // relaunches its graph, a run that differs in parameters only (other channels, observers, buffers) updates a graph of
+    // the same shape in place (cudaGraphExecUpdate: microseconds, no allocation; launches already enqueued keep the old
+    // parameters), and only a new shape (emission / albedo, generations, with or without peel-off) is instantiated.
+    // cudaGraphExecDestroy waits for the device, so graphs pushed out of the cache are released at the library's next wait.
+    struct LoopGraph { std::vector<unsigned char> key; unsigned shape = 0; cudaGraphExec_t exec = nullptr; cudaEvent_t done = nullptr; };
     std::vector<LoopGraph> loops, retired;
     cudaEvent_t tev[4] = {nullptr, nullptr, nullptr, nullptr};   // kernel timing (A0 | A2 | transport | peel)
     unsigned long long launches = 0, launches_pending = 0;
@@ -389,25 +391,25 @@ int enqueue_pass(gcmcrt_grid* g, const PassLaunch& L, cudaStream_t s, cudaEvent_
 // the condition.  Nothing here waits for the device.  When the caller's stream is itself being captured the node is
 // added to the caller's graph (a graph that holds a conditional node cannot be a child graph); otherwise a graph of its
 // own is instantiated, launched on the caller's stream and released (an executable graph in flight is freed on completion).
-void reap_retired_loops(gcmcrt_grid* g, bool wait)
+// cudaGraphExecDestroy waits for the device (measured: for as long as whatever is in flight takes, even when the graph
+// itself has finished), so retired graphs are only released where the library waits anyway -- after the final
+// synchronisation of a run with host outputs, in a timed run, in gcmcrt_destroy -- or when more than 256 have piled up.
+void reap_retired_loops(gcmcrt_grid* g)
 {
-    for (size_t m = 0; m < g->retired.size();) {
-        gcmcrt_grid::LoopGraph& lg = g->retired[m];
-        if (wait || cudaEventQuery(lg.done) == cudaSuccess) {
-            if (wait) cudaEventSynchronize(lg.done);
-            cudaGraphExecDestroy(lg.exec);
-            cudaEventDestroy(lg.done);
-            g->retired.erase(g->retired.begin() + m);
-        } else {
-            ++m;
-        }
+    for (auto& lg : g->retired) {
+        cudaEventSynchronize(lg.done);
+        cudaGraphExecDestroy(lg.exec);
+        cudaEventDestroy(lg.done);
     }
-    cudaGetLastError();   // cudaEventQuery reports "not ready" through the error state
+    g->retired.clear();
+    cudaGetLastError();
 }
 
 int launch_pass_loop(gcmcrt_grid* g, const PassLaunch& L, cudaStream_t s, unsigned* n_launch)
 {
-    constexpr size_t kLoopCache = 16;
+    constexpr size_t kLoopCache = 8;
+    const unsigned shape = 1u | (L.emission ? 2u : 0u) | (L.has_obs ? 4u : 0u) | (L.ev.hist ? 8u : 0u) | unsigned(L.n_gen) << 4 |
+                           unsigned(L.n_gen_run) << 12;
     if (!g->cap_stream) CUDA_TRY(g, cudaStreamCreateWithFlags(&g->cap_stream, cudaStreamNonBlocking));
     cudaStreamCaptureStatus cst = cudaStreamCaptureStatusNone;
     CUDA_TRY(g, cudaStreamIsCapturing(s, &cst));
@@ -417,7 +419,7 @@ int launch_pass_loop(gcmcrt_grid* g, const PassLaunch& L, cudaStream_t s, unsign
     const bool own = cst != cudaStreamCaptureStatusActive;
     const unsigned char* kb = reinterpret_cast<const unsigned char*>(&L);
     if (own) {
-        reap_retired_loops(g, false);
+        if (g->retired.size() > 256) reap_retired_loops(g);
         for (size_t m = 0; m < g->loops.size(); ++m) {
             if (g->loops[m].key.size() == sizeof L && std::memcmp(g->loops[m].key.data(), kb, sizeof L) == 0) {
                 gcmcrt_grid::LoopGraph lg = g->loops[m];   // most recently used goes to the back
@@ -454,7 +456,30 @@ int launch_pass_loop(gcmcrt_grid* g, const PassLaunch& L, cudaStream_t s, unsign
         if (rcode == GCMCRT_OK && e != cudaSuccess) rcode = fail(g, GCMCRT_E_CUDA, std::string("pass loop capture: ") + cudaGetErrorString(e));
         if (rcode != GCMCRT_OK) break;
         if (own) {
+            // a cached graph of the same shape takes the new parameters in place
+            bool updated = false;
+            for (size_t m = g->loops.size(); m-- > 0 && !updated;) {
+                if (g->loops[m].shape != shape) continue;
+                cudaGraphExecUpdateResultInfo info;
+                if (cudaGraphExecUpdate(g->loops[m].exec, graph, &info) == cudaSuccess && info.result == cudaGraphExecUpdateSuccess) {
+                    gcmcrt_grid::LoopGraph lg = g->loops[m];
+                    g->loops.erase(g->loops.begin() + m);
+                    lg.key.assign(kb, kb + sizeof L);
+                    e = cudaGraphLaunch(lg.exec, s);
+                    if (e == cudaSuccess) e = cudaEventRecord(lg.done, s);
+                    g->loops.push_back(lg);
+                    updated = true;
+                } else {
+                    cudaGetLastError();
+                    break;   // same shape but not updatable (a memset outgrew its node): instantiate
+                }
+            }
+            if (updated) {
+                if (e != cudaSuccess) rcode = fail(g, GCMCRT_E_CUDA, std::string("pass loop launch: ") + cudaGetErrorString(e));
+                break;
+            }
             gcmcrt_grid::LoopGraph lg;
+            lg.shape = shape;
             e = cudaGraphInstantiate(&lg.exec, graph, 0);
             if (e == cudaSuccess) e = cudaEventCreateWithFlags(&lg.done, cudaEventDisableTiming);
             if (e == cudaSuccess) e = cudaGraphLaunch(lg.exec, s);
@@ -885,7 +910,10 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             need_sync = true;
         }
     }
-    if (need_sync) CUDA_TRY(g, cudaStreamSynchronize(s));
+    if (need_sync) {
+        CUDA_TRY(g, cudaStreamSynchronize(s));
+        reap_retired_loops(g);
+    }
     if (o_cnt.host) {
         const unsigned long long st = static_cast<const gcmcrt_counters*>(o_cnt.host)->device_status;
         if (st == 1) return fail(g, GCMCRT_E_CUDA, "suspended-packet list overflow");
@@ -1098,7 +1126,7 @@ int gcmcrt_destroy(gcmcrt_grid* g)
     if (g->h_ctrl) cudaFreeHost(g->h_ctrl);
     for (auto& lg : g->loops) g->retired.push_back(lg);
     g->loops.clear();
-    reap_retired_loops(g, true);
+    reap_retired_loops(g);
     if (g->cap_stream) cudaStreamDestroy(g->cap_stream);
     for (auto& e : g->tev) if (e) cudaEventDestroy(e);
     delete g;

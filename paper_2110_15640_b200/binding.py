@@ -10,7 +10,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libgcmcrt.so")
+# GCMCRT_LIB selects another build of the same library (the checked variant, build.py --checked)
+LIB_PATH = os.environ.get("GCMCRT_LIB") or os.path.join(_HERE, "libgcmcrt.so")
 _lib = None
 
 OK, E_INVALID, E_NOMEM, E_CUDA, E_STATE = 0, -1, -2, -3, -4

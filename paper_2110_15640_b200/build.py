@@ -25,15 +25,22 @@ def needs_build() -> bool:
     return any(os.path.getmtime(f) > t for f in DEPS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if force or needs_build():
+LIB_CHECKED = os.path.join(HERE, "libgcmcrt_checked.so")
+
+
+def build(force: bool = False, verbose: bool = False, checked: bool = False) -> str:
+    """checked = True: the variant with -DGCMCRT_CHECKED (device-side bounds and state checks, device_common.cuh) as
+    libgcmcrt_checked.so; load it with GCMCRT_LIB=<path> (binding.py)."""
+    lib = LIB_CHECKED if checked else LIB
+    stale = not os.path.exists(lib) or any(os.path.getmtime(f) > os.path.getmtime(lib) for f in DEPS)
+    if force or stale:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        tmp = LIB + ".tmp.%d" % os.getpid()
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
+        tmp = lib + ".tmp.%d" % os.getpid()
+        cmd = [nvcc] + NVCC_FLAGS + (["-DGCMCRT_CHECKED"] if checked else []) + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
         subprocess.run(cmd, check=True)
-        os.replace(tmp, LIB)
-    return LIB
+        os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, checked="--checked" in sys.argv))

@@ -4,6 +4,20 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
+// Bounds and state checks of the checked build (python -m paper_2110_15640_b200.build --checked: -DGCMCRT_CHECKED, a
+// library of its own, libgcmcrt_checked.so): compute-sanitizer is not available on the GPU pool this was built on, so
+// the indices the kernels compute themselves -- cells, columns, shells, event slots, sort keys, list slots, bins -- are
+// asserted instead; a failed check prints its source line and traps, which the host sees as GCMCRT_E_CUDA.
+#ifdef GCMCRT_CHECKED
+#include <cstdio>
+#define GCMCRT_CHECK(c)                                                                      \
+    do {                                                                                     \
+        if (!(c)) { printf("GCMCRT_CHECK failed: %s  (%s:%d)\n", #c, __FILE__, __LINE__); __trap(); } \
+    } while (0)
+#else
+#define GCMCRT_CHECK(c) ((void)0)
+#endif
+
 namespace gcmcrt {
 
 constexpr float kPi = 3.14159265358979323846f;

@@ -54,6 +54,7 @@ __device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slo
                                             float nx, float ny, float nz, uint32_t m_inter, uint32_t cellp, uint32_t meta,
                                             uint32_t pkt, float4 prop)
 {
+    GCMCRT_CHECK(slot < ev.cap);
     float4* r = ev.rec + 4 * (size_t)slot;
     r[0] = make_float4(px, py, pz, W);
     r[1] = make_float4(nx, ny, nz, 0.f);
@@ -64,6 +65,7 @@ __device__ __forceinline__ void write_event(const EventBuf& ev, unsigned int slo
         const unsigned int chan = (unsigned int)min(max(int(meta >> 8) - *ev.chan_lo, 0), ev.c_fold - 1);
         const unsigned int col = (unsigned int)(k * ev.nlat + j);
         const unsigned int key = chan * (unsigned int)ev.bins_per_chan + col * (unsigned int)ev.nlg + (ev.nlg > 1 ? (unsigned int)(i >> ev.lev_shift) : 0u);
+        GCMCRT_CHECK(i < ev.nlev && j < ev.nlat && key < (unsigned int)ev.c_fold * (unsigned int)ev.bins_per_chan);
         ev.keys[slot] = key;
         if (ev.hist) atomicAdd(ev.hist + key, 1u);
     }
@@ -1083,6 +1085,7 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
             const bool have = rank < chunk_end;
             float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a, pr = a;
             if (have) {
+                GCMCRT_CHECK(slot_next < n_events);
                 const float4* r = ev.rec + 4 * (size_t)slot_next;
                 a = __ldg(r); b = __ldg(r + 1); c = __ldg(r + 2); pr = __ldg(r + 3);
             }
@@ -1096,6 +1099,7 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
             const int bt = int((meta >> 2) & 63u);
             int ci, cj, ck;
             unpack_cell(__float_as_uint(c.y), ci, cj, ck);
+            GCMCRT_CHECK(!have || (chan >= 0 && chan < rc.n_chan_run && bt < rc.n_batches && ci < gs.nlev && cj < gs.nlat && ck < gs.nlon));
             const float* alpha_c = rc.alpha + (size_t)(rc.chan_begin + max(chan, 0)) * rc.geom.alpha_stride;
             // what the event scatters toward an observer: W omega (medium, Eq. 14), W (emission), W a (surface)
             float wsca = a.w, pgas = 0.f, g = 0.f;

@@ -195,6 +195,8 @@ __device__ __forceinline__ const float* ray_column(const GeomSmem& s, const floa
 template <bool DUAL = false>
 __device__ __forceinline__ void ray_load_alpha(Ray& r, const GeomSmem& s, const float* __restrict__ alpha_tab)
 {
+    GCMCRT_CHECK(r.j >= 0 && r.j < s.nlat && r.k >= 0 && r.k < s.nlon && r.i >= 0 && r.i < s.nlev);
+    GCMCRT_CHECK(r.rad_step == 1 || r.rad_step == -1);
     const float* colp = ray_column<DUAL>(s, alpha_tab, r.j, r.k);
     if (DUAL) {
         const float2 a = __ldg(reinterpret_cast<const float2*>(colp) + r.i);
@@ -261,6 +263,7 @@ __device__ __forceinline__ int ray_step(Ray& r, const GeomSmem& s, float& tau, f
     r.u = fmaxf(un, r.u);
     if (r.u_rad > ul) return RAY_PARK;  // ties: shells first (C1)
     r.i += r.rad_step;
+    GCMCRT_CHECK(r.i >= -1 && r.i <= s.nlev);
     if ((unsigned)r.i >= (unsigned)s.nlev) return r.i < 0 ? RAY_SURFACE : RAY_ESCAPE;   // r.i is left outside the grid
     r.alpha = r.alpha_n;   // prefetched for exactly this cell
     if (DUAL) r.beta = r.beta_n;
@@ -407,6 +410,8 @@ __device__ __forceinline__ int ray_run(Ray& r, const GeomSmem& s, float& tau_io,
         }
     }
     const int ish = int((sa - sa0) >> 3);
+    GCMCRT_CHECK(sa >= sa0 && ish >= 0 && ish <= s.nlev && n >= 0 && n <= KSTEPS);
+    GCMCRT_CHECK(status == RAY_SURFACE || status == RAY_ESCAPE || (ish - (inward ? 0 : 1) >= 0 && ish - (inward ? 0 : 1) < s.nlev));
     r.ish = ish;
     r.i = status == RAY_SURFACE ? -1 : (status == RAY_ESCAPE || inward ? ish : ish - 1);
     r.rad_step = inward ? -1 : 1;

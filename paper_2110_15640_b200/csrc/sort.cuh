@@ -56,6 +56,7 @@ __global__ void __launch_bounds__(256) ev_scatter_kernel(const SortParams p)
         unsigned int base = 0;
         if (valid && lane_id() == leader) base = atomicAdd(p.hist + key, (unsigned int)__popc(peers));
         base = __shfl_sync(kFullMask, base, leader);
+        GCMCRT_CHECK(!valid || (key < p.nbins && base + __popc(peers & ((1u << lane_id()) - 1u)) < n));
         if (valid) p.perm[base + __popc(peers & ((1u << lane_id()) - 1u))] = e;
     }
 }

@@ -64,6 +64,7 @@ __device__ __forceinline__ uint32_t nev_before(const RunConst& rc, uint32_t kind
 
 __device__ __forceinline__ void wave_finish_packet(const RunConst& rc, uint32_t chan_run, uint32_t pkt, uint32_t nev)
 {
+    GCMCRT_CHECK(chan_run < (uint32_t)rc.n_chan_run && pkt >= rc.pkt_begin && pkt - rc.pkt_begin < rc.n_pkt);
     if (rc.event_count) rc.event_count[(size_t)chan_run * rc.n_pkt + (pkt - rc.pkt_begin)] = nev;
 }
 
@@ -384,6 +385,7 @@ __global__ void __launch_bounds__(kWaveThreads) wave_emit_kernel(const __grid_co
                 }
             }
             if (live) {
+                GCMCRT_CHECK(cell >= 0 && cell < rc.geom.ncell);
                 const int i = cell % gs.nlev, j = (cell / gs.nlev) % gs.nlat, k = cell / (gs.nlev * gs.nlat);
                 const float r = gs.R[i] * cbrtf(fmaf(z.z1, gs.qcube[i], 1.0f));
                 const float ct = fmaf(z.z2, gs.cth[j + 1] - gs.cth[j], gs.cth[j]);
@@ -485,6 +487,7 @@ wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, con
                 sl[12 * kStageSlots] = __uint_as_float(pkt); sl[13 * kStageSlots] = __uint_as_float(m_new);
             }
             staged += __popc(m_s);
+            GCMCRT_CHECK(staged <= kStageSlots);
             __syncwarp();
         }
         // ---------------- phase 2: full warps of survivors start their flights; phase 3: long flights ----------------
@@ -542,6 +545,7 @@ wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, con
             const unsigned m_u = __ballot_sync(kFullMask, unfinished);
             if (unfinished) flight_save(flights + in_flight + rank_in_mask(m_u), ray, tau, tau_t, W, chan_run, pkt, m_new, st, used);
             in_flight += __popc(m_u);
+            GCMCRT_CHECK(in_flight <= kStageSlots && in_flight >= 0 && staged >= 0);
             __syncwarp();
         }
         if (!more) break;

@@ -1067,3 +1067,148 @@ def test_error_paths(gpu):
             assert e.value.code == gpu.E_INVALID
         r = G.run_emission(prm4)
         assert np.all(np.isfinite(r["value"])) and r["counters"]["packets_stuck"] == 0
+
+
+def test_c_client_runs_a_whole_albedo_call(gpu, tmp_path):
+    """A plain C11 program (no CUDA, no Python) that includes include/gcmcrt.h and links libgcmcrt.so runs a complete
+    albedo call -- grid_create, set_opacity, run_albedo with host buffers, destroy -- on the GPU; the same inputs through
+    the Python binding give the same packets (event total, per-packet counts of the first packets) and the same spectrum."""
+    import shutil
+    import subprocess
+    if shutil.which("gcc") is None:
+        pytest.skip("no gcc")
+    nlev, nlat, nlon, n_chan, N = 8, 6, 10, 3, 50000
+    R0, Rt = 1.0e7, 1.3e7
+    grid, opac = wl.uniform_medium(nlev, nlat, nlon, R0, Rt, 2.0 / (Rt - R0), 0.8, g=0.5, pgas=0.25, n_chan=n_chan, surface_albedo=0.3)
+    prm = wl.default_params(packets_per_channel=N, seed=77, star_dir=[0.6, 0.0, 0.8], obs_dir=[[0.6, 0.0, 0.8], [0.0, 1.0, 0.0]])
+    ref = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+    f32 = lambda a: "%.9gf" % float(np.asarray(a).ravel()[0])      # the tables are constants: the C side fills them in
+    src = tmp_path / "client.c"
+    src.write_text(r"""
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include "gcmcrt.h"
+#define NLEV %d
+#define NLAT %d
+#define NLON %d
+#define NCHAN %d
+#define NPKT %d
+#define NCELL (NLEV * NLAT * NLON)
+int main(void)
+{
+    const double pi = 3.14159265358979323846;
+    static double r[NLEV + 1], th[NLAT + 1], ph[NLON + 1];
+    static float T[NCELL], rho[NCELL], ka[NCHAN * NCELL], kr[NCHAN * NCELL], kc[NCHAN * NCELL], gc[NCHAN * NCELL], lam[NCHAN];
+    for (int i = 0; i <= NLEV; ++i) r[i] = %r + (%r - %r) * i / NLEV;
+    for (int j = 0; j <= NLAT; ++j) th[j] = pi * j / NLAT;
+    for (int k = 0; k <= NLON; ++k) ph[k] = 2.0 * pi * k / NLON;
+    th[NLAT] = pi; ph[NLON] = 2.0 * pi;
+    for (int c = 0; c < NCELL; ++c) { T[c] = 1000.0f; rho[c] = 1.0f; }
+    for (int c = 0; c < NCHAN * NCELL; ++c) { ka[c] = %s; kr[c] = %s; kc[c] = %s; gc[c] = %s; }
+    for (int c = 0; c < NCHAN; ++c) lam[c] = %s;
+    gcmcrt_grid *g = NULL;
+    int rc = gcmcrt_grid_create(&g, NLEV, NLAT, NLON, r, th, ph, T, rho, NULL, NULL, NULL, 0.0, 0.3f, NULL);
+    if (rc) { printf("create %%d %%s\n", rc, gcmcrt_last_error(NULL)); return 1; }
+    rc = gcmcrt_set_opacity(g, 0, NCHAN, lam, ka, kr, kc, gc, NULL);
+    if (rc) { printf("set %%d %%s\n", rc, gcmcrt_last_error(g)); return 1; }
+    gcmcrt_run_params p;
+    memset(&p, 0, sizeof p);
+    double obs[6] = {0.6, 0.0, 0.8, 0.0, 1.0, 0.0};
+    p.star_dir[0] = 0.6; p.star_dir[2] = 0.8; p.n_obs = 2; p.obs_dir = obs; p.packets_per_channel = NPKT; p.seed = 77;
+    p.scatter_on = 1; p.tau_vert_max = 30.0; p.tau_cut = 50.0; p.n_batches = 32;
+    static double flux[NCHAN * 2 * 32], value[NCHAN * 2], sigma[NCHAN * 2];
+    static uint32_t evc[NCHAN * NPKT];
+    gcmcrt_counters cnt;
+    gcmcrt_result out;
+    memset(&out, 0, sizeof out);
+    out.flux_sum = flux; out.value = value; out.sigma = sigma; out.event_count = evc; out.counters = &cnt;
+    rc = gcmcrt_run_albedo(g, &p, &out, NULL);
+    if (rc) { printf("run %%d %%s\n", rc, gcmcrt_last_error(g)); return 1; }
+    unsigned long long h = 1469598103934665603ull;     /* FNV-1a over the per-packet event counts */
+    for (int m = 0; m < NCHAN * NPKT; ++m) { h ^= evc[m]; h *= 1099511628211ull; }
+    printf("ok %%llu %%llu %%llu %%llu", (unsigned long long)cnt.events, (unsigned long long)cnt.packets_escaped,
+           (unsigned long long)cnt.device_status, h);
+    for (int m = 0; m < NCHAN * 2; ++m) printf(" %%.17g", value[m]);
+    printf("\n");
+    return gcmcrt_destroy(g);
+}
+""" % (nlev, nlat, nlon, n_chan, N, R0, Rt, R0, f32(opac["k_abs"]), f32(opac["k_sca_ray"]), f32(opac["k_sca_cld"]),
+       f32(opac["g_cld"]), f32(opac["lambda"])))
+    exe = tmp_path / "client"
+    libdir = os.path.dirname(gpu.LIB_PATH)
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    subprocess.run(["gcc", "-std=c11", "-O1", "-Wall", "-Werror", "-I", os.path.join(root, "include"), str(src), "-o", str(exe),
+                    "-L", libdir, "-lgcmcrt", "-Wl,-rpath," + libdir], check=True)
+    r = subprocess.run([str(exe)], capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0 and r.stdout.startswith("ok "), (r.stdout, r.stderr)
+    f = r.stdout.split()
+    assert int(f[1]) == ref["counters"]["events"] and int(f[2]) == ref["counters"]["packets_escaped"] and int(f[3]) == 0
+    h = 1469598103934665603
+    for v in ref["event_count"].ravel().tolist():
+        h = ((h ^ v) * 1099511628211) & 0xffffffffffffffff
+    assert int(f[4]) == h                                    # every packet made the same number of events
+    val = np.array([float(x) for x in f[5:]]).reshape(n_chan, 2)
+    assert np.allclose(val, ref["value"], rtol=1e-5)         # the sums differ by the order of the atomics only
+
+
+def test_checked_build_runs_clean(gpu, tmp_path):
+    """The library built with -DGCMCRT_CHECKED (device-side bounds / state checks on every index the kernels compute:
+    cells, columns, shells, event slots, sort keys, list slots) runs the smoke cases -- albedo with a reflecting surface,
+    emission toward four phases, both pass-loop drivers -- and a multi-pass run with a tiny event buffer without a
+    failed check, and gives the same packets as the normal build.  (compute-sanitizer is closed on this GPU pool.)"""
+    import subprocess
+    import sys
+    from paper_2110_15640_b200 import build
+    lib = build.build(checked=True)
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = r"""
+import os, sys
+import numpy as np
+sys.path.insert(0, %r)
+from paper_2110_15640_b200 import binding, workloads as wl
+assert binding.LIB_PATH.endswith("libgcmcrt_checked.so")
+tot = []
+grid, opac, prm = wl.cfg2(nlon=16, nlat=8, nlev=20, nbands=2, ng=4, packets=20000)
+grid["surface_albedo"] = 0.4
+for tm in (0, 1):
+    with binding.Grid(grid) as G:
+        G.set_opacity(opac)
+        g = G.run_albedo(dict(prm, timing=tm, npix=8), want_event_count=True, want_contrib=grid["T"].size)
+    assert g["counters"]["device_status"] == 0 and g["counters"]["packets_stuck"] == 0
+    tot.append(int(g["event_count"].sum()))
+grid, opac, prm = wl.cfg3(nlon=16, nlat=8, nlev=20, nbands=1, ng=4, packets=20000, n_obs=4)
+with binding.Grid(grid) as G:
+    G.set_opacity(opac)
+    g = G.run_emission(prm, want_event_count=True)
+    tot.append(int(g["event_count"].sum()))
+    g = G.run_emission(dict(prm, forced_scatter=2, survival_bias=1, roulette_w_min=0.05, roulette_survive=0.3), want_event_count=True)
+    tot.append(int(g["event_count"].sum()))
+    t = G.run_transmission(prm)
+    tot.append(int(t["counters"]["events"]))
+os.environ["GCMCRT_EVENT_CAP"] = "7000"
+grid, opac = wl.uniform_medium(6, 4, 5, 1.0e6, 1.3e6, 2.0 / 0.3e6, 0.9, g=0.4, pgas=0.3, n_chan=2, surface_albedo=0.6)
+prm = wl.default_params(packets_per_channel=20000, seed=5, obs_dir=[[1.0, 0, 0], [0.6, 0, 0.8]])
+with binding.Grid(grid) as G:
+    G.set_opacity(opac)
+    g = G.run_albedo(prm, want_event_count=True)
+    assert g["counters"]["passes"] > 5
+    tot.append(int(g["event_count"].sum()))
+    g = G.run_albedo(dict(prm, continuous_absorption=1, max_events=20), want_event_count=True)
+    tot.append(int(g["event_count"].sum()))
+print("TOTALS", *tot)
+""" % root
+    outs = []
+    for env_lib in (lib, None):
+        env = dict(os.environ)
+        env.pop("GCMCRT_EVENT_CAP", None)
+        if env_lib:
+            env["GCMCRT_LIB"] = env_lib
+            run_code = code
+        else:
+            env.pop("GCMCRT_LIB", None)
+            run_code = code.replace('assert binding.LIB_PATH.endswith("libgcmcrt_checked.so")', "")
+        r = subprocess.run([sys.executable, "-c", run_code], capture_output=True, text=True, env=env, timeout=900)
+        assert r.returncode == 0 and "GCMCRT_CHECK failed" not in r.stdout + r.stderr, (r.stdout[-2000:], r.stderr[-2000:])
+        outs.append([l for l in r.stdout.splitlines() if l.startswith("TOTALS")][0])
+    assert outs[0] == outs[1]

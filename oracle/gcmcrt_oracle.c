@@ -580,6 +580,7 @@ typedef struct {
     double *image;     /* this channel's [n_obs][npix][npix] or NULL */
     double *contrib;   /* this channel's [n_obs][2][ncell] or NULL (Sect. 6, Eq. 32) */
     uint32_t *evcount; /* this channel's [N] or NULL */
+    int launch_forced; /* packet_albedo -> transport: the launch flight was forced (and stretched there) */
 } run_ctx;
 
 /* C19: image pixel of point p seen from observer direction o. */
@@ -657,11 +658,20 @@ static void transport(const run_ctx *rc, uint32_t pkt, double p[3], double n[3],
     uint32_t m_inter = 0;    /* interaction index (Philox event index), 1,2,... */
     double z[4];
     const int cont = prm->continuous_absorption != 0;
+    /* Sect. 4.2, path length stretching (Baes et al. 2016): flights are drawn from the stretched law
+     * q(tau) = a e^{-a tau} (a = stretch_alpha < 1: longer flights) instead of p(tau) = e^{-tau}, and the packet carries
+     * the ratio p / q of what happened to it: an interaction at tau, W <- W e^{-(1-a) tau} / a; leaving the medium
+     * (top or lower boundary) after tau_edge, W <- W e^{-(1-a) tau_edge} (the ratio of the two survival probabilities).
+     * Hybrid with forced scattering: the stretched law truncated at tau_edge, q = a e^{-a tau} / (1 - e^{-a tau_edge}),
+     * so the interaction weight gains the factor 1 - e^{-a tau_edge} and the uncollided part W e^{-tau_edge} leaves. */
+    const double sa = (prm->stretch_alpha > 0.0 && prm->stretch_alpha < 1.0) ? prm->stretch_alpha : 1.0;
     int flight = 0;
     for (;;) {
         double tau = 0.0;
         int st;
-        if (prm->forced_scatter == 2 && !(flight++ == 0 && m == 0)) {   /* m == 0: the albedo launch, forced there */
+        const int launch_flight = (flight++ == 0 && m == 0);   /* the flight packet_albedo prepared (m == 0: albedo) */
+        int forced_now = launch_flight ? rc->launch_forced : 0;   /* ... and forced (and stretched) there */
+        if (prm->forced_scatter == 2 && !launch_flight) {
             /* Sect. 4.2, forced scattering at every flight (the albedo launch does it for the first one): the flight is
              * drawn from the exponential law truncated at the optical depth to the end of the grid, the packet keeps
              * the probability 1 - e^-tau_edge of interacting, the uncollided part leaves (Cashwell & Everett 1959) */
@@ -670,14 +680,16 @@ static void transport(const run_ctx *rc, uint32_t pkt, double p[3], double n[3],
             uint64_t seg = 0;
             int se = march(G, ch->alpha, q, n, c3, INFINITY, &tau_edge, &seg, NULL);
             if (se == ST_ESCAPE || (se == ST_SURFACE && !(a_surf > 0.0))) {
-                const double pint = -expm1(-tau_edge);
+                const double pint = -expm1(-sa * tau_edge);     /* sa = 1: the plain forced flight */
                 if (pint > 0.0) {
                     if (se == ST_ESCAPE) cnt->escaped_weight += W * exp(-tau_edge);
-                    tau_t = -log1p(-exp(-tau_t) * pint);   /* the flight's own zeta = e^-tau_t */
+                    tau_t = -log1p(-exp(-tau_t) * pint) / sa;   /* the flight's own zeta = e^-tau_t */
                     W *= pint;
+                    forced_now = 1;
                 }
             }
         }
+        if (sa < 1.0 && !forced_now) tau_t /= sa;               /* tau = -ln(zeta) / a */
         if (cont) {
             /* Sect. 4.1, Eq. 12: the sampled optical depth is spent on the scattering extinction alone and the packet
              * loses weight smoothly, W <- W e^-tau_abs, with tau_abs integrated along the same flight */
@@ -686,6 +698,10 @@ static void transport(const run_ctx *rc, uint32_t pkt, double p[3], double n[3],
             W *= exp(-tau_abs);
         } else {
             st = march(G, ch->alpha, p, n, ijk, tau_t, &tau, &cnt->segments_transport, NULL);
+        }
+        if (sa < 1.0) {   /* p / q of the flight's outcome */
+            if (st == ST_INTERACT) W *= exp(-(1.0 - sa) * tau_t) / sa;
+            else if (st == ST_ESCAPE || st == ST_SURFACE) W *= exp(-(1.0 - sa) * tau);
         }
         if (st == ST_ESCAPE) { cnt->packets_escaped++; cnt->escaped_weight += W; break; }
         if (st == ST_STUCK) { cnt->packets_stuck++; break; }
@@ -759,6 +775,9 @@ static void packet_albedo(const run_ctx *rc, uint32_t pkt, int batch, orc_counte
     locate(G, p, ijk);
     ijk[0] = G->nlev - 1;
     double W = 1.0, tau_t = -log(z[2]);
+    const double sa = (prm->stretch_alpha > 0.0 && prm->stretch_alpha < 1.0) ? prm->stretch_alpha : 1.0;
+    run_ctx rcl = *rc;
+    rcl.launch_forced = 0;
     if (prm->forced_scatter) {
         /* Sect. 4.2: "an extra raytracing step to calculate the optical depth to the end of the grid in the
          * direction of the packet path", here once, at the start of the packet (forced first scattering).  The flight
@@ -769,7 +788,7 @@ static void packet_albedo(const run_ctx *rc, uint32_t pkt, int batch, orc_counte
         uint64_t seg = 0;
         int st = march(G, rc->ch->alpha, q, n, c3, INFINITY, &tau_edge, &seg, NULL);
         if (st == ST_ESCAPE || (st == ST_SURFACE && !(rc->g->surface_albedo > 0.0))) {
-            const double pint = -expm1(-tau_edge);
+            const double pint = -expm1(-sa * tau_edge);   /* sa < 1: the hybrid with path length stretching */
             if (!(pint > 0.0)) {            /* empty path: nothing can interact, the packet ends with no event */
                 if (st == ST_ESCAPE) { cnt->packets_escaped++; cnt->escaped_weight += 1.0; } else cnt->packets_surface++;
                 if (rc->evcount) rc->evcount[pkt] = 0;
@@ -777,10 +796,11 @@ static void packet_albedo(const run_ctx *rc, uint32_t pkt, int batch, orc_counte
             }
             if (st == ST_ESCAPE) cnt->escaped_weight += exp(-tau_edge);   /* the part that leaves without interacting */
             W = pint;
-            tau_t = -log1p(-z[2] * pint);
+            tau_t = -log1p(-z[2] * pint) / sa;
+            rcl.launch_forced = 1;
         }
     }
-    transport(rc, pkt, p, n, ijk, W, tau_t, 0, batch, cnt);
+    transport(&rcl, pkt, p, n, ijk, W, tau_t, 0, batch, cnt);
 }
 
 /* O4: emission launch (Eq. 13, Sect. 4.3 with the C10 composite bias). */
@@ -885,6 +905,7 @@ static int run_mode(const orc_grid *g, const orc_opacity *op, const orc_params *
             rc.image = (out->image && npix > 0) ? out->image + (size_t)c * nobs * npix * npix : NULL;
             rc.contrib = out->contrib ? out->contrib + (size_t)c * nobs * 2 * G.ncell : NULL;
             rc.evcount = (out->event_count && run == 0) ? out->event_count + (size_t)c * N : NULL;
+            rc.launch_forced = 0;
             if (emission && !(ch.L_tot > 0.0)) continue;
             /* O8 / C12: batch(pkt) = floor(pkt * n_batches / N); batches are independent -> OpenMP over them */
 #ifdef _OPENMP

@@ -94,6 +94,9 @@ typedef struct {
     int continuous_absorption; /* Sect. 4.1, Eq. 12: flights are sampled against the scattering extinction only and the
                                 weight decays as W <- W e^-tau_abs along every flight; every interaction in the medium
                                 is then a scattering (no absorption draw, no omega in the peel-off weight) */
+    double stretch_alpha;    /* Sect. 4.2 (L179; Baes et al. 2016), path length stretching: flights are drawn from
+                                a e^{-a tau} with a = stretch_alpha in (0, 1) and weighted by p / q (0 or 1: off).  With
+                                forced_scatter: the hybrid scheme, the stretched law truncated at tau_edge */
 } orc_params;
 
 typedef struct {

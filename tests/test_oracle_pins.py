@@ -1106,3 +1106,89 @@ def test_forced_scattering_of_emitted_packets(orc):
     vf, sf = orc.reduce(orc.run_emission(grid, opac, dict(prm, forced_scatter=2, survival_bias=1, roulette_w_min=0.02,
                                                          roulette_survive=0.2)), "emission")
     assert np.all(np.abs(va - vf) <= 4 * np.hypot(sa, sf)) and np.any(va > 0)
+
+
+# ----------------------------------------------------------------------------- Sect. 4.2: path length stretching, hybrid
+@pytest.mark.parametrize("omega,alpha,forced", [(0.5, 0.5, 0), (0.9, 0.7, 0), (0.9, 0.5, 2), (0.5, 0.3, 2)])
+def test_path_length_stretching_keeps_the_exact_semi_infinite_albedo(orc, omega, alpha, forced):
+    """Path length stretching (Sect. 4.2; Baes et al. 2016) changes weights, not expectations: with flights drawn
+    from a e^{-a tau} and weighted by p / q, alone and as the hybrid with forced scattering, the exact Chandrasekhar
+    H-function albedo of the semi-infinite isotropic atmosphere (tests/golden) is reproduced."""
+    rows = dict(np.loadtxt(os.path.join(GOLDEN, "isotropic_semi_infinite_albedo.txt")))
+    R0, depth = 1.0e8, 1.0e4
+    grid, opac = wl.uniform_medium(4, 1, 1, R0, R0 + depth, 80.0 / depth, omega, g=0.0, surface_albedo=1.0)
+    s = np.array([0.3, -0.5, 0.81]); s /= np.linalg.norm(s)
+    prm = wl.default_params(packets_per_channel=60000, seed=29, star_dir=s, obs_dir=s[None], stretch_alpha=alpha,
+                            forced_scatter=forced, survival_bias=1, roulette_w_min=0.02, roulette_survive=0.2,
+                            n_threads=os.cpu_count() or 1)
+    val, sig = orc.reduce(orc.run_albedo(grid, opac, prm), "albedo")
+    Ag = PI * val[0, 0]
+    assert abs(Ag - rows[omega]) < 4 * PI * sig[0, 0] + 3e-4 * rows[omega], (Ag, rows[omega], PI * sig[0, 0])
+
+
+@pytest.mark.parametrize("forced", [0, 1, 2])
+def test_path_length_stretching_weights_on_a_thin_3d_atmosphere(orc, forced):
+    """The three weights of a stretched flight, each pinned by a quantity the analog run measures: the spectrum (the
+    interaction weight e^{-(1-a) tau} / a, times 1 - e^{-a tau_edge} in the hybrid), the escaped weight (the survival ratio
+    e^{-(1-a) tau_edge} of flights that leave through the top, or the uncollided part e^{-tau_edge} of forced flights: its
+    expectation is the analog escape fraction), and the light reflected by a Lambert surface under the atmosphere (the
+    same ratio for flights that reach the lower boundary: with a dark atmosphere over a bright surface the spectrum
+    is made of it).  a < 1 lengthens the flights: in a thin atmosphere fewer packets interact than in the analog run."""
+    R0, Rt = 1.0e6, 1.3e6
+    N = 80000
+    obs = np.array([[1.0, 0, 0], [0.0, 1.0, 0.0], [0.6, 0.0, 0.8]])
+    ncpu = os.cpu_count() or 1
+    extra = dict(forced_scatter=forced)
+    if forced == 2:
+        extra.update(survival_bias=1, roulette_w_min=0.02, roulette_survive=0.2)
+    for k_tau, omega, a_surf in ((0.4, 0.9, 0.0), (0.25, 0.3, 0.9)):
+        grid, opac = wl.uniform_medium(4, 3, 4, R0, Rt, k_tau / (Rt - R0), omega, g=0.3, pgas=0.3, surface_albedo=a_surf)
+        prm = wl.default_params(packets_per_channel=N, seed=13, star_dir=[1.0, 0.0, 0.0], obs_dir=obs, n_threads=ncpu)
+        ra = orc.run_albedo(grid, opac, prm)
+        rs = orc.run_albedo(grid, opac, dict(prm, stretch_alpha=0.4, **extra))
+        va, sa = orc.reduce(ra, "albedo"); vs, ss = orc.reduce(rs, "albedo")
+        assert np.all(np.abs(va - vs) < 4 * np.hypot(sa, ss)), (np.abs(va - vs) / np.hypot(sa, ss)).max()
+        assert np.all(va > 0)
+        if forced == 0:
+            assert rs["counters"]["events"] < 0.8 * ra["counters"]["events"]     # a < 1: longer flights, most leave
+        # escaped weight: analog packets escape with W = 1, so the analog count estimates the same expectation
+        fa = ra["counters"]["escaped_weight"] / N
+        fs = rs["counters"]["escaped_weight"] / N
+        assert abs(fs - fa) < 4 * np.sqrt(fa * (1 - fa) / N) + 0.02 * fa, (fs, fa)
+
+
+def test_path_length_stretching_single_cell_weights_by_quadrature(orc):
+    """One homogeneous cell, single scattering (max_events = 1), isotropic scatterers: the estimator's expectation is
+    the analog one for every stretch parameter, and its value follows from a quadrature written here.  A packet entering
+    at impact parameter b flies along a chord of optical length T(b); it interacts at depth tau with density e^{-tau}
+    and peels omega / (4 pi) e^{-tau_obs}.  The stretched run must give the same number for a = 0.3 and a = 0.8 as the
+    analog run, and its per-packet mean of the interaction weight must be 1 - <e^{-T}> (the interacting fraction)."""
+    R0, Rt = 0.2e6, 1.0e6
+    grid, opac = wl.uniform_medium(1, 1, 1, R0, Rt, 1.2 / (Rt - R0), 0.7, g=0.0, pgas=0.0)
+    N = 200000
+    prm = wl.default_params(packets_per_channel=N, seed=4, max_events=1, star_dir=[0.0, 0.0, 1.0],
+                            obs_dir=[[0.0, 0.6, 0.8]], n_threads=os.cpu_count() or 1)
+    ra = orc.run_albedo(grid, opac, prm)
+    va, sa = orc.reduce(ra, "albedo")
+    for a in (0.3, 0.8):
+        rs = orc.run_albedo(grid, opac, dict(prm, stretch_alpha=a))
+        vs, ss = orc.reduce(rs, "albedo")
+        assert abs(vs[0, 0] - va[0, 0]) < 4 * np.hypot(ss[0, 0], sa[0, 0])
+        # interacting fraction by quadrature over the entry disc: chords with b < R0 end on the (absorbing) core
+        b = (np.arange(200000) + 0.5) / 200000 * Rt
+        alpha_ext = 1.2 / (Rt - R0)
+        chord = np.where(b < R0, np.sqrt(Rt ** 2 - b ** 2) - np.sqrt(np.maximum(R0 ** 2 - b ** 2, 0.0)), 2 * np.sqrt(Rt ** 2 - b ** 2))
+        frac = np.sum((1 - np.exp(-alpha_ext * chord)) * b) / np.sum(b)
+        ev = rs["counters"]["events"] / N                      # stretched flights are longer: fewer of them end inside
+        assert ev < frac
+        assert abs(ra["counters"]["events"] / N - frac) < 4 * np.sqrt(frac * (1 - frac) / N)
+
+
+def test_path_length_stretching_of_emitted_packets(orc):
+    grid, opac, prm = wl.cfg3(nlon=6, nlat=4, nlev=12, nbands=1, ng=2, packets=40000, n_obs=2)
+    prm = dict(prm, n_threads=os.cpu_count() or 1)
+    va, sa = orc.reduce(orc.run_emission(grid, opac, prm), "emission")
+    for extra in (dict(stretch_alpha=0.5), dict(stretch_alpha=0.5, forced_scatter=2, survival_bias=1, roulette_w_min=0.02,
+                                               roulette_survive=0.2)):
+        vs, ss = orc.reduce(orc.run_emission(grid, opac, dict(prm, **extra)), "emission")
+        assert np.all(np.abs(va - vs) <= 4 * np.hypot(sa, ss)) and np.any(va > 0)

@@ -117,6 +117,13 @@ typedef struct gcmcrt_run_params {
                                     omega in the peel-off weight).  Packets end by escaping, at the lower boundary, at
                                     max_events, or by Russian roulette (survival_bias = 1 with roulette_w_min > 0).
                                     Runs through the persistent transport kernel; excludes forced_scatter. */
+    double stretch_alpha;        /* Sect. 4.2 (L179), path length stretching (weights of Baes et al. 2016): a in (0, 1) draws
+                                    every flight from the stretched law a e^{-a tau} instead of e^{-tau} and multiplies the
+                                    weight by the ratio of the two laws for what happened: e^{-(1-a) tau} / a at an interaction
+                                    after tau, e^{-(1-a) tau_edge} when the flight leaves the medium or reaches the lower
+                                    boundary after tau_edge.  With forced_scatter (1: first flight, 2: every flight) the hybrid
+                                    scheme: the stretched law truncated at tau_edge, tau = -ln(1 - zeta (1 - e^{-a tau_edge})) / a,
+                                    extra weight factor 1 - e^{-a tau_edge}.  0 or 1 = off.  Excludes continuous_absorption. */
     int timing;                  /* 0: the run is only enqueued (see STREAMS); the ms_* counters stay 0.
                                     1: profiling run -- the pass loop is driven by the host, which waits for every pass
                                     and records cudaEvents around its kernels to fill the ms_* counters */

@@ -559,6 +559,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     if (prm->forced_scatter == 2 && !(prm->max_events > 0 || (prm->survival_bias && prm->roulette_w_min > 0.0)))
         return fail(g, GCMCRT_E_INVALID, "forced_scatter = 2 needs max_events or Russian roulette to end its packets");
     if (prm->cloud_phase < 0 || prm->cloud_phase > 2) return fail(g, GCMCRT_E_INVALID, "cloud_phase must be 0 (HG), 1 (TTHG) or 2 (Draine)");
+    if (!(prm->stretch_alpha >= 0.0 && prm->stretch_alpha <= 1.0) || (prm->stretch_alpha > 0.0 && prm->stretch_alpha < 1.0 && prm->continuous_absorption))
+        return fail(g, GCMCRT_E_INVALID, "stretch_alpha must be in [0, 1] and excludes continuous_absorption");
     if (mode == 2 && n_obs < 1) return fail(g, GCMCRT_E_INVALID, "transmission needs at least one observer direction");
 
     // ---- outputs
@@ -597,6 +599,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.survival_bias = prm->survival_bias != 0;
     rc.cloud_phase = prm->cloud_phase;
     rc.forced_scatter = prm->forced_scatter;
+    rc.stretch = (prm->stretch_alpha > 0.0 && prm->stretch_alpha < 1.0) ? float(prm->stretch_alpha) : 1.0f;
+    rc.inv_stretch = 1.0f / rc.stretch;
     rc.alpha2 = nullptr;
     rc.roulette_w_min = float(prm->roulette_w_min); rc.roulette_survive = float(prm->roulette_survive);
     rc.surface_albedo = g->surface_albedo;

@@ -209,6 +209,7 @@ struct RunConst {
     int cloud_phase;               // 0 HG (Eq. 7-8), 1 two-term HG (Eq. 10, g1 = g, g2 = -g/2, alpha = 1 - g2^2), 2 Draine (Eq. 9)
     const float* alpha2;           // continuous absorption: [n_chan][ncol][col_stride] pairs (alpha_sca, alpha_abs), or NULL
     int forced_scatter;            // Sect. 4.2: 1 = forced first scattering of albedo packets, 2 = every flight forced
+    float stretch, inv_stretch;    // Sect. 4.2, path length stretching: flights from a e^{-a tau}, a = stretch (1 = off), 1 / a
     float surface_albedo;
     double xi;
     int n_batches;
@@ -666,19 +667,33 @@ __device__ __noinline__ int ray_tau_to_edge(Ray r, const GeomSmem& s, const floa
     }
     return st;
 }
-__device__ __forceinline__ void force_flight(const RunConst& rc, const GeomSmem& gs, const Ray& ray, const float* alpha_c,
+// With path length stretching (rc.stretch = a < 1) this is the hybrid scheme: the stretched law a e^{-a tau} truncated at
+// tau_edge.  Returns whether the flight was forced (a flight that was not is stretched by its caller).
+__device__ __forceinline__ bool force_flight(const RunConst& rc, const GeomSmem& gs, const Ray& ray, const float* alpha_c,
                                              float& tau_t, float& W, double& escw)
 {
     float tau_e;
     const int st = ray_tau_to_edge(ray, gs, alpha_c, rc.geom.maxseg, tau_e);
     if (st == RAY_ESCAPE || (st == RAY_SURFACE && !(rc.surface_albedo > 0.f))) {
-        const float pint = -expm1f(-tau_e);
+        const float pint = -expm1f(-rc.stretch * tau_e);
         if (pint > 0.f) {
             if (st == RAY_ESCAPE) escw += double(W * expf(-tau_e));
-            tau_t = -log1pf(-expf(-tau_t) * pint);   // the flight's own zeta = e^-tau_t
+            tau_t = -log1pf(-expf(-tau_t) * pint) * rc.inv_stretch;   // the flight's own zeta = e^-tau_t
             W *= pint;
+            return true;
         }
     }
+    return false;
+}
+
+// Path length stretching, the weight of a flight's outcome (p / q of Baes et al. 2016): an interaction after tau carries
+// e^{-(1-a) tau} / a, a flight that leaves the medium (top or lower boundary) after tau the ratio e^{-(1-a) tau} of the
+// survival probabilities.  a = 1: exactly 1.
+__device__ __forceinline__ float stretch_weight(const RunConst& rc, int ray_status, float tau)
+{
+    if (!(rc.stretch < 1.0f)) return 1.0f;
+    const float w = expf(-(1.0f - rc.stretch) * tau);
+    return ray_status == RAY_LIMIT ? w * rc.inv_stretch : w;
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -826,7 +841,8 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                     pk.tau = 0.f; pk.fl_seg = 0;
                                     ray_init<DUAL>(pk.ray, gs, px, py, pz, -rc.star[0], -rc.star[1], -rc.star[2], gs.nlev - 1,
                                              j, k, alpha_c);
-                                    if (!DUAL && rc.forced_scatter) force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw);
+                                    if (!(!DUAL && rc.forced_scatter && force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw)))
+                                        pk.tau_t *= rc.inv_stretch;
                                     st = LS_FLY;
                                 } else {
                                     // O4: cell ~ luminosity (Eq. 13) with composite bias xi, uniform point in the cell
@@ -932,7 +948,8 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                 rotate_dir(nx, ny, nz, ct, z.z2);
                                 pk.tau_t = -logf(z.z3); pk.tau = 0.f; pk.fl_seg = 0;
                                 ray_init<DUAL>(pk.ray, gs, px, py, pz, nx, ny, nz, pk.ray.i, pk.ray.j, pk.ray.k, alpha_c);
-                                if (!DUAL && rc.forced_scatter == 2) force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw);
+                                if (!(!DUAL && rc.forced_scatter == 2 && force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw)))
+                                    pk.tau_t *= rc.inv_stretch;
                                 st = LS_FLY;
                             }
                         } else if (st == LS_EV_EMIT) {
@@ -950,7 +967,8 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                 sincospif(2.0f * z.z1, &sp, &cp);
                                 pk.tau_t = -logf(z.z2); pk.tau = 0.f; pk.fl_seg = 0;
                                 ray_init<DUAL>(pk.ray, gs, px, py, pz, ns * cp, ns * sp, nz, pk.ray.i, pk.ray.j, pk.ray.k, alpha_c);
-                                if (!DUAL && rc.forced_scatter == 2) force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw);
+                                if (!(!DUAL && rc.forced_scatter == 2 && force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw)))
+                                    pk.tau_t *= rc.inv_stretch;
                                 st = LS_FLY;
                             }
                         } else {  // Lambert surface (O7, Eq. 3-4)
@@ -971,7 +989,8 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                 rotate_dir(hx, hy, hz, sqrtf(z.z1), z.z2);      // Eq. 4 about the normal
                                 pk.tau_t = -logf(z.z3); pk.tau = 0.f; pk.fl_seg = 0;
                                 ray_init<DUAL>(pk.ray, gs, px, py, pz, hx, hy, hz, 0, pk.ray.j, pk.ray.k, alpha_c);
-                                if (!DUAL && rc.forced_scatter == 2) force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw);
+                                if (!(!DUAL && rc.forced_scatter == 2 && force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw)))
+                                    pk.tau_t *= rc.inv_stretch;
                                 st = LS_FLY;
                             }
                         }
@@ -1000,6 +1019,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                     pk.W *= expf(-pk.tau_b);
                     pk.tau_b = 0.f;
                 }
+                if (!DUAL && rs != RAY_FLYING && rs != RAY_PARK) pk.W *= stretch_weight(rc, rs, pk.tau);
                 if (rs == RAY_FLYING) {
                     if (++pk.fl_seg > rc.geom.maxseg) st = LS_END_STUCK;
                 } else if (rs == RAY_PARK) {

@@ -138,9 +138,10 @@ __device__ __forceinline__ int wave_march(const RunConst& rc, const GeomSmem& gs
 // Warp-collective: lanes with `fin` have ended their flight with status st: record the next event (or park the
 // packet), or close the packet.
 __device__ __forceinline__ void wave_close(const RunConst& rc, const EventBuf& ev, const SuspBuf& susp, int park_all,
-                                           bool fin, int st, const Ray& ray, float W, uint32_t chan_run, uint32_t pkt,
-                                           uint32_t m_inter, WaveCounters& wcnt)
+                                           bool fin, int st, const Ray& ray, float W, float tau, uint32_t chan_run,
+                                           uint32_t pkt, uint32_t m_inter, WaveCounters& wcnt)
 {
+    if (fin) W *= stretch_weight(rc, st, tau);   // path length stretching: the weight of the flight's outcome
     const bool surf_ev = fin && st == RAY_SURFACE && rc.surface_albedo > 0.f;
     const bool want = fin && (st == RAY_LIMIT || surf_ev);
     float px = 0.f, py = 0.f, pz = 0.f, rx = ray.nx, ry = ray.ny, rz = ray.nz;
@@ -171,7 +172,7 @@ __device__ __forceinline__ void wave_fly(const RunConst& rc, const EventBuf& ev,
     float tau = 0.f;
     wave_march<KSTEPS>(rc, gs, st, ray, tau, tau_t, alpha_c, rc.geom.maxseg + 1, wcnt);
     if (active && (st == RAY_FLYING || st == RAY_PARK)) st = RAY_STUCK;   // step budget exhausted
-    wave_close(rc, ev, susp, park_all, active, st, ray, W, chan_run, pkt, m_inter, wcnt);
+    wave_close(rc, ev, susp, park_all, active, st, ray, W, tau, chan_run, pkt, m_inter, wcnt);
 }
 
 // ---- flights in progress, set aside (interact kernel): a scattered packet's flight is short most of the time and
@@ -310,6 +311,7 @@ wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
         }
         float W = 1.0f;
         bool fly = active;
+        bool forced = false;
         if (FORCED) {
             // Sect. 4.2 (L179), forced first scattering: the extra ray trace to the end of the grid gives tau_edge; the
             // flight is drawn from the exponential law truncated there and the packet carries 1 - e^-tau_edge.  A ray
@@ -320,7 +322,7 @@ wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
             WaveCounters unused;
             wave_march<KSTEPS>(rc, gs, st, probe, tau_e, kInf, alpha_c, rc.geom.maxseg + 1, unused);
             if (active && (st == RAY_ESCAPE || (st == RAY_SURFACE && !(rc.surface_albedo > 0.f)))) {
-                const float pint = -expm1f(-tau_e);
+                const float pint = -expm1f(-rc.stretch * tau_e);   // stretch < 1: the hybrid with path length stretching
                 if (!(pint > 0.f)) {   // empty path: the packet ends with no event
                     if (st == RAY_ESCAPE) { ++wcnt.esc; wcnt.escw += 1.0; } else ++wcnt.surf;
                     wave_finish_packet(rc, chan_run, pkt, 0u);
@@ -328,10 +330,12 @@ wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
                 } else {
                     if (st == RAY_ESCAPE) wcnt.escw += double(expf(-tau_e));   // the part that leaves without interacting
                     W = pint;
-                    tau_t = -log1pf(-z2 * pint);
+                    tau_t = -log1pf(-z2 * pint) * rc.inv_stretch;
+                    forced = true;
                 }
             }
         }
+        if (!forced) tau_t *= rc.inv_stretch;   // path length stretching: tau = -ln(zeta) / a
         wave_fly<KSTEPS>(rc, ev, susp, wc.park_all, gs, fly, ray, tau_t, alpha_c, W, chan_run, pkt, 0u, wcnt);
     }
     wave_flush_counters(rc, wcnt);
@@ -532,7 +536,7 @@ wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, con
                     }
                     alpha_c = rc.alpha + (size_t)(rc.chan_begin + int(chan_run)) * rc.geom.alpha_stride;
                     ray_init(ray, gs, px, py, pz, nx, ny, nz, i, j, k, alpha_c);
-                    if (FORCED) force_flight(rc, gs, ray, alpha_c, tau_t, W, wcnt.escw);   // Sect. 4.2
+                    if (!(FORCED && force_flight(rc, gs, ray, alpha_c, tau_t, W, wcnt.escw))) tau_t *= rc.inv_stretch;   // Sect. 4.2
                     st = RAY_FLYING;
                 }
                 __syncwarp();
@@ -541,7 +545,7 @@ wave_interact_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, con
             used += wave_march<KSTEPS>(rc, gs, st, ray, tau, tau_t, alpha_c, do_long ? kLongRoundSteps : kFirstRoundSteps, wcnt);
             bool unfinished = active && (st == RAY_FLYING || st == RAY_PARK);
             if (unfinished && used > rc.geom.maxseg) { st = RAY_STUCK; unfinished = false; }
-            wave_close(rc, ev, susp, wc.park_all, active && !unfinished, st, ray, W, chan_run, pkt, m_new, wcnt);
+            wave_close(rc, ev, susp, wc.park_all, active && !unfinished, st, ray, W, tau, chan_run, pkt, m_new, wcnt);
             const unsigned m_u = __ballot_sync(kFullMask, unfinished);
             if (unfinished) flight_save(flights + in_flight + rank_in_mask(m_u), ray, tau, tau_t, W, chan_run, pkt, m_new, st, used);
             in_flight += __popc(m_u);

@@ -1212,3 +1212,47 @@ print("TOTALS", *tot)
         assert r.returncode == 0 and "GCMCRT_CHECK failed" not in r.stdout + r.stderr, (r.stdout[-2000:], r.stderr[-2000:])
         outs.append([l for l in r.stdout.splitlines() if l.startswith("TOTALS")][0])
     assert outs[0] == outs[1]
+
+
+@pytest.mark.parametrize("tune", ["16,1,8,4", "16,1,0,4", "16,1,2,4"])
+def test_path_length_stretching_and_hybrid_parity(gpu, orc, monkeypatch, tune):
+    """Sect. 4.2 (L179), path length stretching (stretch_alpha) alone and as the hybrid with forced scattering (first
+    flight / every flight) against the oracle -- same streams, same stretched flights, same p / q weights -- through the
+    generation kernels, through the persistent kernel alone, and with packets handed from one to the other: a thin 3D
+    albedo run over a reflecting boundary (interaction, escape and surface weights all matter), the config 2 grid with
+    survival biasing and roulette, and emission with scattering.  stretch_alpha = 1 is the plain run, bit for bit."""
+    monkeypatch.setenv("GCMCRT_TUNE", tune)
+    ncpu = os.cpu_count() or 1
+    R0, Rt = 1.0e6, 1.3e6
+    grid, opac = wl.uniform_medium(5, 4, 6, R0, Rt, 0.6 / (Rt - R0), 0.8, g=0.4, pgas=0.3, surface_albedo=0.5)
+    obs = np.array([[1.0, 0.0, 0.0], [0.0, 0.6, 0.8]])
+    base = wl.default_params(packets_per_channel=30000, seed=14, star_dir=[1.0, 0.0, 0.0], obs_dir=obs)
+    for extra in (dict(stretch_alpha=0.5), dict(stretch_alpha=0.4, forced_scatter=1),
+                  dict(stretch_alpha=0.6, forced_scatter=2, survival_bias=1, roulette_w_min=0.02, roulette_survive=0.2)):
+        prm = dict(base, **extra)
+        g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+        o = orc.run_albedo(grid, opac, dict(prm, n_threads=ncpu), want_event_count=True)
+        _check_parity(orc, g, o, "albedo")
+        assert abs(g["counters"]["escaped_weight"] - o["counters"]["escaped_weight"]) < 1e-3 * o["counters"]["escaped_weight"]
+    plain = _gpu_run(gpu, grid, opac, base, "albedo", want_event_count=True)
+    one = _gpu_run(gpu, grid, opac, dict(base, stretch_alpha=1.0), "albedo", want_event_count=True)
+    assert np.array_equal(plain["event_count"], one["event_count"]) and np.allclose(plain["flux_sum"], one["flux_sum"], rtol=2e-5)
+    half = _gpu_run(gpu, grid, opac, dict(base, stretch_alpha=0.5), "albedo")
+    assert np.all(np.abs(half["value"] - plain["value"]) < 4 * np.hypot(half["sigma"], plain["sigma"]) + 1e-5 * plain["value"])
+    grid, opac, prm = wl.cfg2(nlon=16, nlat=8, nlev=20, nbands=2, ng=3, packets=20000)
+    prm = dict(prm, stretch_alpha=0.5, survival_bias=1, roulette_w_min=0.05, roulette_survive=0.25)
+    g = _gpu_run(gpu, grid, opac, prm, "albedo", want_event_count=True)
+    o = orc.run_albedo(grid, opac, dict(prm, n_threads=ncpu), want_event_count=True)
+    _check_parity(orc, g, o, "albedo")
+    grid, opac, prm = wl.cfg3(nlon=8, nlat=4, nlev=12, nbands=1, ng=2, packets=20000, n_obs=2)
+    for extra in (dict(stretch_alpha=0.5), dict(stretch_alpha=0.5, forced_scatter=2, survival_bias=1, roulette_w_min=0.02, roulette_survive=0.2)):
+        p = dict(prm, **extra)
+        g = _gpu_run(gpu, grid, opac, p, "emission", want_event_count=True)
+        o = orc.run_emission(grid, opac, dict(p, n_threads=ncpu), want_event_count=True)
+        _check_parity(orc, g, o, "emission")
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        for bad in (dict(stretch_alpha=1.5), dict(stretch_alpha=-0.1), dict(stretch_alpha=0.5, continuous_absorption=1)):
+            with pytest.raises(gpu.GcmcrtError) as e:
+                G.run_emission(dict(prm, **bad))
+            assert e.value.code == gpu.E_INVALID

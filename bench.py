@@ -40,16 +40,29 @@ from paper_2110_15640_b200 import workloads as wl  # noqa: E402  (input generato
 METRIC = "packet_events_per_second"
 UNIT = "events/s"
 
-# Algorithmic lane-instructions (FP32/INT issue slots) per unit of work; DESIGN.md section "Roofline" derives them
-# from the audited SASS of the march loop, the event handler and the launch code.
-I_SEG_3D = 27.0      # one 3D cell crossing: radial run 22 executed thread-instructions per segment (PTX loops, 19 issued per
-                     # crossing + the run's entry / exit code) + cone / half-plane / column updates 4.7 per segment
-                     # (ncu source page, profiles/ncu_full_r01d_ptx_loops.txt)
-I_SEG_1D = 22.0      # nlat = nlon = 1: the same radial run, no lateral crossings
-I_EVENT = 420.0      # Philox block, phase sampling, rotation, ray setup, event record write + read
+# Lane-instructions (FP32/INT issue slots) per unit of work, audited from the executed instruction counts of the ncu
+# source page (profiles/ncu_full_r02_cfg2.txt, _cfg3.txt, _cfg4.txt): what the kernels execute on
+# ACTIVE lanes for the method itself -- idle lanes, unissued cycles, the per-CTA geometry-table load and the vote /
+# shuffle / atomic helper instructions are not work.
+#   segment = the plain-crossing loop (17.7: 18 issued instructions per crossing) + ray_run entry / exit (amortised over
+#             the segments of a round) + cone / half-plane / column updates
+#   peel ray = record read, phase function, ray set-up (ray_init), round control, exp, bin accumulation
+I_UNITS = {            # workload: (per peel segment, per peel ray)
+    "cfg2": (28.9, 450.0),
+    "cfg3": (37.9, 317.0),     # ~10 segments per ray (rays toward 8 phases, many end on the night side): entry / exit weighs more; the
+                               # record and the phase-function inputs serve 8 rays
+    "cfg4": (28.4, 450.0),
+}
+I_SEG_1D = 23.0      # nlat = nlon = 1: loop + entry / exit, no lateral crossings
+I_SEG_T = 24.3       # one crossing on a packet flight (first flights + generations, same march code)
+I_EVENT = 1000.0     # per event on the transport side: Philox block, absorb / scatter, phase-function sample, rotation, ray
+                     # set-up, record write + read, flight hand-over (executed: 785 per first flight, 637 per later event)
 # dram__bytes_read.sum + dram__bytes_write.sum per peel_kernel launch at the default sizes, from ncu --set full captures
-PEEL_DRAM_BYTES_PER_LAUNCH = {"cfg2": (7.96e9, "profiles/ncu_full_r01d_ptx_loops.txt: 4 launches of a step, 94 M events each")}
-I_PEEL_RAY = 300.0   # record + prop read, phase function, ray setup for one (event, observer), exp, bin accumulation
+PEEL_DRAM_BYTES_PER_LAUNCH = {
+    "cfg2": (7.955e9, "profiles/ncu_full_r02_cfg2.txt: 4 launches of a step, ~94 M events each"),
+    "cfg3": (11.907e9, "profiles/ncu_full_r02_cfg3.txt: 6 launches of a step, ~1e8 events x 8 observers each"),
+    "cfg4": (3.643e9, "profiles/ncu_full_r02_cfg4.txt: 2000 wavelengths, ~5e7 events per launch"),
+}
 
 
 def make_workload(name, packets=None, channels=None):
@@ -310,11 +323,13 @@ class Leg:
         """Roofline of the dominant kernel (peel_kernel) from a timing = 1 leg: algorithmic lane-instructions over the
         kernel's device time (cudaEvents the library records on the launching stream around every launch)."""
         is3d = np.asarray(self.grid["T"]).shape[0] > 1 or np.asarray(self.grid["T"]).shape[1] > 1
-        i_seg = I_SEG_3D if is3d else I_SEG_1D
+        i_seg, i_ray = I_UNITS.get(self.name, I_UNITS["cfg2"])
+        if not is3d:
+            i_seg = I_SEG_1D
         work_seg = acc["segments_peel"] * i_seg
-        work = work_seg + acc["rays_peel"] * I_PEEL_RAY
+        work = work_seg + acc["rays_peel"] * i_ray
         dur_ms = acc["ms_peel"]
-        work_t = acc["segments_transport"] * i_seg + acc["events"] * I_EVENT
+        work_t = acc["segments_transport"] * (I_SEG_T if is3d else I_SEG_1D) + acc["events"] * I_EVENT
         n_dom = max(1, acc["passes"])
         peak = 148 * 128 * pk["sm_max_mhz"] * 1e6 / 1e12          # T lane-instr/s
         achieved = work / (dur_ms * 1e-3) / 1e12 if dur_ms > 0 else 0.0
@@ -330,6 +345,8 @@ class Leg:
                 "traffic": tr[0] if tr else None,
                 "traffic_unit": "dram__bytes_read + write per peel_kernel launch, ncu --set full" + (" (%s)" % tr[1] if tr else ""),
                 "peak_source": "148 SM x 128 FP32 lanes x sm_max_mhz (%s)" % pk["source"],
+                "lane_instr_per_unit": {"peel_segment": i_seg, "peel_ray": i_ray, "transport_segment": I_SEG_T, "event": I_EVENT,
+                                        "source": "executed thread-instructions per unit, ncu source page (profiles/ncu_full_r02_*.txt)"},
                 "work_lane_instr_per_launch": work / n_dom, "ms_per_launch": dur_ms / n_dom,
                 "timing_steps": steps,
                 "hbm_term": {"bytes_per_step": hbm_bytes, "ms_at_peak": hbm_bytes / (pk["hbm_gbs"] * 1e9) * 1e3,
@@ -437,6 +454,7 @@ def run_ours(args):
                                    "n_obs": int(np.asarray(lg.prm["obs_dir"]).reshape(-1, 3).shape[0]),
                                    "grid": list(np.asarray(lg.grid["T"]).shape)},
                         "rays_per_s": acc_x["rays_peel"] / (ms_x * 1e-3),
+                        "counters_per_step": {k: acc_x[k] / 3 for k in ("events", "segments_transport", "segments_peel", "rays_peel", "passes")},
                         "roofline": lg.roofline(acc_xt, ms_xt, 2, pk)}
 
             # config 3: the same grid and tables as config 2, so the tables already on the device serve it

@@ -26,7 +26,6 @@ import json
 import os
 import subprocess
 import sys
-import threading
 import time
 
 import numpy as np
@@ -121,42 +120,51 @@ def reduce_over_ranks(ms, sums, world, device="cpu"):
     return float(t.item()), [float(x) for x in u.tolist()]
 
 
-class ClockSampler(threading.Thread):
-    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md): ONE nvidia-smi process polling
+    every 200 ms, as the recipe does.  (A new nvidia-smi process per sample initialises NVML every time, and that was
+    measured to stall the device-driven pass loop by up to 30 ms a sample; the polling process does not.)"""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
-        super().__init__(daemon=True)
         self.index = index
-        self.rows = []
-        self.stop_flag = threading.Event()
+        self.proc = None
 
-    def run(self):
-        while not self.stop_flag.is_set():
-            try:
-                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
-                f = [x.strip() for x in out.strip().split(",")]
-                if len(f) >= 7:
-                    self.rows.append(f)
-            except Exception:
-                pass
-            self.stop_flag.wait(0.1)
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            time.sleep(0.3)     # the first sample is on its way before the timed region starts
+        except Exception:
+            self.proc = None
 
     def summary(self):
-        self.stop_flag.set()
-        self.join(timeout=6)
-        sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if r[1].replace(".", "").isdigit()]
+        rows = []
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                out, _ = self.proc.communicate(timeout=5)
+            except Exception:
+                self.proc.kill()
+                out = ""
+            for line in (out or "").splitlines():
+                f = [x.strip() for x in line.split(",")]
+                if len(f) >= 7:
+                    rows.append(f)
+        sm = [float(r[0]) for r in rows if r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in rows if r[1].replace(".", "").isdigit()]
         reasons = []
         for name, col in (("hw_slowdown", 3), ("hw_thermal_slowdown", 4), ("sw_thermal_slowdown", 5), ("sw_power_cap", 6)):
-            if any(r[col].lower().startswith("active") for r in self.rows):
+            if any(r[col].lower().startswith("active") for r in rows):
                 reasons.append(name)
-        pw = [float(r[2]) for r in self.rows if r[2].replace(".", "").isdigit()]
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(self.rows), "reasons": reasons}
+        pw = [float(r[2]) for r in rows if r[2].replace(".", "").isdigit()]
+        # the samples taken under load: the idle ones before / after the steps sit at a lower clock
+        load = [c for c, w in zip(sm, pw)] if len(sm) == len(pw) else sm
+        return {"sm_mhz": float(np.median(load)) if load else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(rows), "reasons": reasons}
 
 
 def oracle_leg(name, grid, opac, prm, mode, budget_s=15.0, threads=None):
@@ -390,7 +398,7 @@ def run_ours(args):
     N = int(leg.prm["packets_per_channel"])
     warm = max(args.warmup, 3)
     for _ in range(warm):
-        leg.step(leg.dev, True, counters=None)
+        leg.step(leg.dev, True, counters="device")
     sampler = ClockSampler(local)
     sampler.start()
     ms, acc, _, host_s = leg.timed(leg.dev, True, args.steps, barrier)
@@ -444,7 +452,7 @@ def run_ours(args):
 
             def short_leg(lg):
                 for _ in range(3):
-                    lg.step(lg.dev, True, counters=None)
+                    lg.step(lg.dev, True, counters="device")
                 ms_x, acc_x, _, _ = lg.timed(lg.dev, True, 3, barrier)
                 lg.step(lg.dev, True, timing=1)
                 ms_xt, acc_xt, _, _ = lg.timed(lg.dev, True, 2, barrier, timing=1, counters="host")
@@ -481,7 +489,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])

@@ -19,7 +19,10 @@
  * transmission; Lambert sphere 2/3 and its phase law; exact Chandrasekhar
  * H-function albedos; isothermal emitter chord integral; energy conservation;
  * peel-off <-> escape consistency; brute-force enumeration on a 1-cell grid;
- * rotational invariance; Eq. 33 vector identity.
+ * rotational invariance; Eq. 33 vector identity; the image frame (C19) by the
+ * brightness law of a Lambert sphere and the lit half at quadrature; path
+ * length stretching and its hybrid by the exact albedos and analog agreement.
+ * The whole library also runs under ASan + UBSan (tests/test_oracle_sanitizers.py).
  * Paper-printed numeric values: none exist (Fig. 1 is an image) -> "parity
  * against paper-printed values: unpinned"; every function is pinned by the
  * closed forms above instead.

@@ -37,7 +37,7 @@ class _Params(C.Structure):
                 ("npix", C.c_int), ("n_batches", C.c_int), ("n_threads", C.c_int),
                 ("survival_bias", C.c_int), ("roulette_w_min", C.c_double), ("roulette_survive", C.c_double),
                 ("star_radius", C.c_double), ("planet_xy", C.c_double * 2), ("ld_c1", C.c_double), ("ld_c2", C.c_double), ("cloud_phase", C.c_int), ("forced_scatter", C.c_int), ("continuous_absorption", C.c_int),
-                ("stretch_alpha", C.c_double)]
+                ("star_solid_angle", C.c_double), ("stretch_alpha", C.c_double)]
 
 
 class _Counters(C.Structure):
@@ -210,6 +210,7 @@ def _params_struct(prm, keep):
     p.cloud_phase = int(prm.get("cloud_phase", 0))
     p.forced_scatter = int(prm.get("forced_scatter", 0))
     p.continuous_absorption = int(prm.get("continuous_absorption", 0))
+    p.star_solid_angle = float(prm.get("star_solid_angle", 0.0))
     p.stretch_alpha = float(prm.get("stretch_alpha", 0.0))
     return p
 
@@ -248,10 +249,10 @@ def run_emission(grid, opac, prm, want_event_count=False, want_contrib=False):
     return _run("emission", grid, opac, prm, want_event_count, want_contrib)
 
 
-def run_transmission(grid, opac, prm):
-    """Sect. 5.1, Eq. 20-23: random transit chords, multiple scattering off.  reduce(.., "transmission") gives <I_p>
-    of Eq. 21 in m^2 once multiplied by (R_TOA - R_p0): see reduce()."""
-    res = _run("transmission", grid, opac, prm)
+def run_transmission(grid, opac, prm, want_event_count=False):
+    """Sect. 5.1, Eq. 20-23: random transit chords; with scatter_on and star_solid_angle > 0 the packets go on to
+    scatter (L259, reading N12).  reduce(.., "transmission") gives <I_p> of Eq. 21 in m^2: see reduce()."""
+    res = _run("transmission", grid, opac, prm, want_event_count)
     r = np.asarray(grid["r_edges"], dtype=np.float64)
     res["annulus_width"] = float(r[-1] - r[0])
     return res

@@ -581,6 +581,8 @@ typedef struct {
     double *contrib;   /* this channel's [n_obs][2][ncell] or NULL (Sect. 6, Eq. 32) */
     uint32_t *evcount; /* this channel's [N] or NULL */
     int launch_forced; /* packet_albedo -> transport: the launch flight was forced (and stretched there) */
+    double peel_scale; /* what a peeled-off f adds to S: 1 (albedo, emission); -W_ld b dOmega for the scattered light of a
+                          transit chord (Sect. 5.1 with multiple scattering, reading N12) */
 } run_ctx;
 
 /* C19: image pixel of point p seen from observer direction o. */
@@ -628,7 +630,7 @@ static void peel(const run_ctx *rc, const double p[3], const int ijk[3], int kin
         int st = march(G, rc->ch->alpha, q, od, c3, INFINITY, &tau, &cnt->segments_peel, NULL);
         if (st != ST_ESCAPE) continue;                 /* ray ends on the surface: nothing reaches the observer */
         if (tau > rc->prm->tau_cut) continue;
-        double f = pref * exp(-tau);
+        double f = rc->peel_scale * pref * exp(-tau);
         rc->S[(size_t)o * rc->prm->n_batches + batch] += f;
         if (rc->image) {
             int npix = rc->prm->npix;
@@ -906,6 +908,7 @@ static int run_mode(const orc_grid *g, const orc_opacity *op, const orc_params *
             rc.contrib = out->contrib ? out->contrib + (size_t)c * nobs * 2 * G.ncell : NULL;
             rc.evcount = (out->event_count && run == 0) ? out->event_count + (size_t)c * N : NULL;
             rc.launch_forced = 0;
+            rc.peel_scale = 1.0;
             if (emission && !(ch.L_tot > 0.0)) continue;
             /* O8 / C12: batch(pkt) = floor(pkt * n_batches / N); batches are independent -> OpenMP over them */
 #ifdef _OPENMP
@@ -997,6 +1000,39 @@ int orc_run_transmission(const orc_grid *g, const orc_opacity *op, const orc_par
                 const double absorbed = (st == ST_SURFACE) ? 1.0 : 1.0 - exp(-tau);   /* (a chord grazing R_p0 in fp) */
                 const int batch = (int)((pkt * (uint64_t)nb) / N);
                 out->flux_sum[((size_t)c * nobs + o) * nb + batch] += W * absorbed * b;
+                if (prm->scatter_on && prm->star_solid_angle > 0.0 && W > 0.0) {
+                    /* Sect. 5.1, L259 (reading N12): after the initial peel-off above "the packet is then free to multiply
+                     * scatter through the atmosphere, each time contributing to the transmission ... through the next
+                     * event estimation method".  The packet flies from the chord's start along o^ (tau = -ln zeta2 of
+                     * the launch block); every interaction peels W omega Theta e^{-tau_obs} toward o^ (per steradian), and
+                     * the observer receives that light as starlight over the solid angle of the stellar disc,
+                     * star_solid_angle: the chord's term of Eq. 21 becomes
+                     * W_ph b [1 - e^{-tau_i} - dOmega sum_k W_k omega_k Theta_k e^{-tau_obs,k}]. */
+                    run_ctx rc;
+                    memset(&rc, 0, sizeof rc);
+                    rc.g = g; rc.G = &G; rc.prm = prm; rc.ch = &ch; rc.c = c;
+                    rc.chan_key = (uint32_t)(op->chan0 + c);
+                    rc.obs_lo = o; rc.obs_hi = o + 1;
+                    rc.S = out->flux_sum + (size_t)c * nobs * nb;
+                    rc.evcount = (out->event_count && o == 0) ? out->event_count + (size_t)c * N : NULL;
+                    rc.launch_forced = 0;
+                    rc.peel_scale = -W * b * prm->star_solid_angle;
+                    double pp[3] = { p[0], p[1], p[2] }, nn3[3] = { od[0], od[1], od[2] };
+                    int c3[3];
+                    locate(&G, pp, c3);
+                    c3[0] = G.nlev - 1;
+                    orc_counters cnt;
+                    memset(&cnt, 0, sizeof cnt);
+                    transport(&rc, (uint32_t)pkt, pp, nn3, c3, 1.0, -log(z[2]), 0, batch, &cnt);
+                    out->counters.events += cnt.events;
+                    out->counters.segments_transport += cnt.segments_transport;
+                    out->counters.segments_peel += cnt.segments_peel;
+                    out->counters.packets_escaped += cnt.packets_escaped;
+                    out->counters.packets_absorbed += cnt.packets_absorbed;
+                    out->counters.packets_surface += cnt.packets_surface;
+                    out->counters.packets_stuck += cnt.packets_stuck;
+                    out->counters.escaped_weight += cnt.escaped_weight;
+                }
             }
         }
     }

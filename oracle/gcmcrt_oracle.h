@@ -97,6 +97,9 @@ typedef struct {
     int continuous_absorption; /* Sect. 4.1, Eq. 12: flights are sampled against the scattering extinction only and the
                                 weight decays as W <- W e^-tau_abs along every flight; every interaction in the medium
                                 is then a scattering (no absorption draw, no omega in the peel-off weight) */
+    double star_solid_angle; /* Sect. 5.1, L259 (reading N12): > 0 with scatter_on switches multiple scattering on in
+                                transmission: solid angle [sr] of the stellar disc seen from the planet, over which light
+                                scattered back toward the observer still counts as transmitted starlight */
     double stretch_alpha;    /* Sect. 4.2 (L179; Baes et al. 2016), path length stretching: flights are drawn from
                                 a e^{-a tau} with a = stretch_alpha in (0, 1) and weighted by p / q (0 or 1: off).  With
                                 forced_scatter: the hybrid scheme, the stretched law truncated at tau_edge */
@@ -169,9 +172,11 @@ int orc_channel_prep(const orc_grid *g, const orc_opacity *op, const orc_params 
 /* The two drivers (section 3 call stacks). */
 int orc_run_albedo(const orc_grid *g, const orc_opacity *op, const orc_params *prm, orc_result *out);
 int orc_run_emission(const orc_grid *g, const orc_opacity *op, const orc_params *prm, orc_result *out);
-/* Transmission spectrum by random transit chords (Sect. 5.1, Eq. 20-21), multiple scattering off (L261: "reduces the
+/* Transmission spectrum by random transit chords (Sect. 5.1, Eq. 20-21).  Multiple scattering off (L261: "reduces the
  * model to a raytracer scheme with random transit chord sampler"): flux_sum[c][o][batch] = sum over packets of
- * W [1 - exp(-tau_i)] b_i; <I_p> = (R_TOA - R_p0) / N * sum (Eq. 21); W from Eq. 22-23. */
+ * W [1 - exp(-tau_i)] b_i; <I_p> = (R_TOA - R_p0) / N * sum (Eq. 21); W from Eq. 22-23.  With scatter_on and
+ * star_solid_angle > 0 the packets go on to scatter (L259) and every event's peel-off toward the observer, times the
+ * stellar solid angle, is taken off the chord's term (reading N12 in DESIGN.md). */
 int orc_run_transmission(const orc_grid *g, const orc_opacity *op, const orc_params *prm, orc_result *out);
 
 #ifdef __cplusplus

@@ -1192,3 +1192,65 @@ def test_path_length_stretching_of_emitted_packets(orc):
                                                roulette_survive=0.2)):
         vs, ss = orc.reduce(orc.run_emission(grid, opac, dict(prm, **extra)), "emission")
         assert np.all(np.abs(va - vs) <= 4 * np.hypot(sa, ss)) and np.any(va > 0)
+
+
+# ----------------------------------------------------------------------------- Sect. 5.1: multiple scattering in transmission
+def _ms_medium(omega, g, pgas=0.0, nlev=1, nlat=1, nlon=1, tau_rad=0.6):
+    R0, Rt = 1.0e7, 1.4e7
+    grid, opac = wl.uniform_medium(nlev, nlat, nlon, R0, Rt, tau_rad / (Rt - R0), omega, g=g, pgas=pgas)
+    return grid, opac, R0, Rt, tau_rad / (Rt - R0)
+
+
+@pytest.mark.parametrize("g,pgas", [(0.0, 0.0), (0.6, 0.0), (0.0, 1.0)])
+def test_transmission_with_single_scattering_by_quadrature(orc, g, pgas):
+    """Reading N12 pinned by a closed form.  Homogeneous shell, one scattering allowed (max_events = 1): a packet on the
+    chord of optical length T that scatters after tau peels toward the observer along the SAME chord, so
+    e^{-tau} * e^{-(T - tau)} = e^{-T} whatever tau, and the expected peel-off is omega Theta(mu = 1) T e^{-T} per
+    steradian.  Eq. 21 then reads  <I_p> = int b [1 - e^{-T(b)} - dOmega omega Theta(1) T(b) e^{-T(b)}] db  with
+    T(b) = 2 alpha sqrt(R_TOA^2 - b^2): a 1D quadrature written here, for isotropic, forward-peaked HG (Theta(1) =
+    (1 + g) / (4 pi (1 - g)^2)) and Rayleigh (3 / (8 pi)) scatterers."""
+    omega, dO, N, nb = 0.8, 0.02, 200000, 32
+    grid, opac, R0, Rt, alpha = _ms_medium(omega, g, pgas)
+    prm = wl.default_params(packets_per_channel=N, seed=6, obs_dir=[[0.0, 0.6, 0.8]], max_events=1, star_solid_angle=dO)
+    r1 = orc.run_transmission(grid, opac, prm)
+    val, sig = orc.reduce(r1, "transmission")
+    b = R0 + (np.arange(400000) + 0.5) / 400000 * (Rt - R0)
+    T = 2.0 * alpha * np.sqrt(Rt ** 2 - b ** 2)
+    theta1 = 3.0 / (8.0 * PI) if pgas == 1.0 else (1.0 + g) / (4.0 * PI * (1.0 - g) ** 2)
+    sca = dO * omega * theta1 * np.sum(b * T * np.exp(-T)) * (Rt - R0) / b.size
+    ray = np.sum(b * (1.0 - np.exp(-T))) * (Rt - R0) / b.size
+    assert abs(val[0, 0] - (ray - sca)) < 4 * sig[0, 0] + 1e-6 * ray, (val[0, 0], ray - sca, sig[0, 0])
+    # the scattered term on its own: the raytracer run with the same streams takes the chords' baseline (and its
+    # noise) out exactly; what is left is -dOmega sum W b omega Theta e^{-tau_obs}, with a batch-means error of its own
+    r0 = orc.run_transmission(grid, opac, dict(prm, star_solid_angle=0.0))
+    d = (r0["flux_sum"] - r1["flux_sum"])[0, 0] / (N / nb) * (Rt - R0)          # per-batch means of the scattered term
+    mean, err = d.mean(), d.std(ddof=1) / np.sqrt(nb)
+    assert abs(mean - sca) < 4 * err and err < 0.02 * sca, (mean, sca, err)
+
+
+def test_transmission_multiple_scattering_switches_and_linearity(orc):
+    """star_solid_angle = 0 or scatter_on = 0 is the raytracer mode of L261, bit for bit; with the same streams the
+    result is exactly linear in the solid angle (the scattered light is one sum, scaled); scattering lets light
+    through, so the effective radius shrinks; multiple scattering adds to single scattering; forced scattering and
+    path length stretching of the scattered flights leave the expectation unchanged."""
+    grid, opac, R0, Rt, alpha = _ms_medium(0.9, 0.5, pgas=0.3, nlev=4, nlat=3, nlon=4, tau_rad=0.8)
+    base = wl.default_params(packets_per_channel=40000, seed=9, obs_dir=[[1.0, 0.0, 0.0], [0.0, 0.6, 0.8]], star_radius=7.0e8,
+                             planet_xy=(2.0e8, 1.0e8), ld_c1=0.3, ld_c2=0.2)
+    r0 = orc.run_transmission(grid, opac, base)
+    assert np.array_equal(r0["flux_sum"], orc.run_transmission(grid, opac, dict(base, scatter_on=0, star_solid_angle=0.05))["flux_sum"])
+    r1 = orc.run_transmission(grid, opac, dict(base, star_solid_angle=0.05), want_event_count=True)
+    r2 = orc.run_transmission(grid, opac, dict(base, star_solid_angle=0.10))
+    assert np.allclose(r2["flux_sum"] - r0["flux_sum"], 2.0 * (r1["flux_sum"] - r0["flux_sum"]), rtol=1e-9, atol=1e-3)
+    v0, s0 = orc.reduce(r0, "transmission"); v1, s1 = orc.reduce(r1, "transmission")
+    assert np.all(v1 < v0 * (1 - 1e-3))           # same chords, same baseline: the scattered light only takes off
+    single = orc.run_transmission(grid, opac, dict(base, star_solid_angle=0.05, max_events=1))
+    vs, _ = orc.reduce(single, "transmission")
+    assert np.all(v1 < vs) and np.all(vs < v0)
+    assert r1["event_count"].max() > 3 and r1["counters"]["events"] > 2 * 40000
+    for extra in (dict(forced_scatter=2, survival_bias=1, roulette_w_min=0.02, roulette_survive=0.2),
+                  dict(stretch_alpha=0.5, survival_bias=1, roulette_w_min=0.02, roulette_survive=0.2)):
+        rv = orc.run_transmission(grid, opac, dict(base, star_solid_angle=0.05, **extra))
+        vv, sv = orc.reduce(rv, "transmission")
+        # compare the scattered parts (the baseline is common to all runs and has no noise between them)
+        d1, dv = r1["flux_sum"].sum(axis=2) - r0["flux_sum"].sum(axis=2), rv["flux_sum"].sum(axis=2) - r0["flux_sum"].sum(axis=2)
+        assert np.all(np.abs(dv / d1 - 1) < 0.05), dv / d1

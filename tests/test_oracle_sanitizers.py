@@ -1,7 +1,7 @@
 """The CPU oracle under AddressSanitizer + UndefinedBehaviorSanitizer: a small C driver is
 compiled together with oracle/gcmcrt_oracle.c with -fsanitize=address,undefined -fno-sanitize-recover=all and runs
 albedo (3D grid, Lambert surface, images, contribution functions, every variance-reduction switch), emission (Doppler
-shifts, depth cut, composite bias), transmission and the ray integrator.  Any out-of-bounds access, use after free,
+shifts, depth cut, composite bias), transmission (raytracer and with multiple scattering) and the ray integrator.  Any out-of-bounds access, use after free,
 leak, signed overflow or misaligned access aborts the driver and fails the test."""
 import os
 import shutil
@@ -74,7 +74,7 @@ int main(void)
         if (variant == 2) { p.forced_scatter = 2; p.survival_bias = 1; p.roulette_w_min = 0.1; p.roulette_survive = 0.3; p.cloud_phase = 2; }
         if (variant == 3) { p.continuous_absorption = 1; p.max_events = 6; }
         if (variant == 4) { p.doppler_on = 1; p.doppler_halfwidth = 1; p.emission_bias = 0.4; p.tau_vert_max = 2.0; }
-        if (variant == 5) { p.forced_scatter = 1; p.pkt_begin = 17; p.pkt_end = 201; }
+        if (variant == 5) { p.forced_scatter = 1; p.pkt_begin = 17; p.pkt_end = 201; p.star_solid_angle = 0.01; p.stretch_alpha = 0.5; }
         if (variant == 6) { p.scatter_on = 0; p.n_threads = 1; }
         for (int mode = 0; mode < 3; ++mode) {
             orc_result out;

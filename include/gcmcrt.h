@@ -117,6 +117,11 @@ typedef struct gcmcrt_run_params {
                                     omega in the peel-off weight).  Packets end by escaping, at the lower boundary, at
                                     max_events, or by Russian roulette (survival_bias = 1 with roulette_w_min > 0).
                                     Runs through the persistent transport kernel; excludes forced_scatter. */
+    double star_solid_angle;     /* Transmission with multiple scattering (Sect. 5.1): with scatter_on and a value > 0 the
+                                    packets go on from their chords' starts and scatter; every event's peel-off toward the
+                                    observer, W omega Theta e^-tau_obs per steradian, times this solid angle [sr] of the stellar
+                                    disc seen from the planet (pi (R_star / a)^2: within it scattered light still reaches
+                                    the observer as starlight) is taken off the chord's term of Eq. 21.  0: raytracer mode. */
     double stretch_alpha;        /* Sect. 4.2 (L179), path length stretching (weights of Baes et al. 2016): a in (0, 1) draws
                                     every flight from the stretched law a e^{-a tau} instead of e^{-tau} and multiplies the
                                     weight by the ratio of the two laws for what happened: e^{-(1-a) tau} / a at an interaction
@@ -231,15 +236,17 @@ int gcmcrt_run_albedo(gcmcrt_grid *grid, const gcmcrt_run_params *params, gcmcrt
 int gcmcrt_run_emission(gcmcrt_grid *grid, const gcmcrt_run_params *params, gcmcrt_result *out, void *stream);
 
 /*
- * gcmcrt_run_transmission -- transmission spectrum by random transit chords (Sect. 5.1, Eq. 20-21) with multiple
- * scattering off (L261: "a raytracer scheme with random transit chord sampler"; the scheme with scattering, L259, is
- * described in words only).  Packet i of a channel draws an impact parameter b_i uniform in [R_p0, R_TOA] and an
+ * gcmcrt_run_transmission -- transmission spectrum by random transit chords (Sect. 5.1, Eq. 20-21): the "raytracer
+ * scheme with random transit chord sampler" of L261, or -- with scatter_on and star_solid_angle > 0 -- the scheme with
+ * multiple scattering of L259 (the paper describes it in words; reading N12): chord i then contributes
+ * W_i b_i [1 - exp(-tau_i) - star_solid_angle * sum over the packet's events of W omega Theta exp(-tau_obs)].  Packet i of a channel draws an impact parameter b_i uniform in [R_p0, R_TOA] and an
  * azimuth around the limb; tau_i is the extinction optical depth of the whole chord along obs_dir (planet -> observer)
  * -- with doppler_on through that observer's Doppler-shifted table (Eq. 33-34, the set-up of the paper's Sect. 13).
  *   flux_sum[c][o][batch] = sum_i W_i [1 - exp(-tau_i)] b_i      (W_i: limb darkening, Eq. 22-23; 1 if star_radius = 0)
  *   value[c][o] = <I_p> = (R_TOA - R_p0) / N * sum  [m^2] (Eq. 21), sigma its batch-means standard error;
  *   the caller forms (R_p / R_star)^2 = (R_p0^2 + 2 <I_p>) / R_star^2 (Eq. 20).
- * star_dir, scatter_on, max_events, emission_bias, npix, image, event_count, contrib are not used.  n_obs >= 1.
+ * star_dir, emission_bias, npix, image, contrib are not used; scatter_on, max_events, the variance-reduction switches and
+ * event_count (interactions per packet, first observer's run) only with multiple scattering.  n_obs >= 1.
  * Errors: as gcmcrt_run_albedo.
  */
 int gcmcrt_run_transmission(gcmcrt_grid *grid, const gcmcrt_run_params *params, gcmcrt_result *out, void *stream);

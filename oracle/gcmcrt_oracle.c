@@ -758,6 +758,34 @@ static void transport(const run_ctx *rc, uint32_t pkt, double p[3], double n[3],
     if (rc->evcount) rc->evcount[pkt] = m;
 }
 
+/* Sect. 4.2: "an extra raytracing step to calculate the optical depth to the end of the grid in the direction of
+ * the packet path", at the start of a packet (forced first scattering; with forced_scatter = 2 the later flights are
+ * forced in transport()).  The flight is drawn from the exponential law truncated at tau_edge and the packet carries the
+ * probability 1 - e^-tau_edge that an analog packet interacts at all (Cashwell & Everett 1959); with path length
+ * stretching (sa < 1) the stretched law is truncated instead (the hybrid scheme).  Returns 1 when the flight was forced,
+ * 0 when not (forcing off, or the ray ends on a reflecting lower boundary), -1 when the path is empty (the packet ends). */
+static int forced_launch(const run_ctx *rc, const double p[3], const double n[3], const int ijk[3], double zeta,
+                         double *W, double *tau_t, orc_counters *cnt)
+{
+    const orc_params *prm = rc->prm;
+    if (!prm->forced_scatter) return 0;
+    const double sa = (prm->stretch_alpha > 0.0 && prm->stretch_alpha < 1.0) ? prm->stretch_alpha : 1.0;
+    double q[3] = { p[0], p[1], p[2] }, tau_edge = 0.0;
+    int c3[3] = { ijk[0], ijk[1], ijk[2] };
+    uint64_t seg = 0;
+    int st = march(rc->G, rc->ch->alpha, q, n, c3, INFINITY, &tau_edge, &seg, NULL);
+    if (!(st == ST_ESCAPE || (st == ST_SURFACE && !(rc->g->surface_albedo > 0.0)))) return 0;
+    const double pint = -expm1(-sa * tau_edge);
+    if (!(pint > 0.0)) {            /* empty path: nothing can interact, the packet ends with no event */
+        if (st == ST_ESCAPE) { cnt->packets_escaped++; cnt->escaped_weight += *W; } else cnt->packets_surface++;
+        return -1;
+    }
+    if (st == ST_ESCAPE) cnt->escaped_weight += *W * exp(-tau_edge);   /* the part that leaves without interacting */
+    *W *= pint;
+    *tau_t = -log1p(-zeta * pint) / sa;
+    return 1;
+}
+
 /* O3: albedo launch. */
 static void packet_albedo(const run_ctx *rc, uint32_t pkt, int batch, orc_counters *cnt)
 {
@@ -777,31 +805,9 @@ static void packet_albedo(const run_ctx *rc, uint32_t pkt, int batch, orc_counte
     locate(G, p, ijk);
     ijk[0] = G->nlev - 1;
     double W = 1.0, tau_t = -log(z[2]);
-    const double sa = (prm->stretch_alpha > 0.0 && prm->stretch_alpha < 1.0) ? prm->stretch_alpha : 1.0;
     run_ctx rcl = *rc;
-    rcl.launch_forced = 0;
-    if (prm->forced_scatter) {
-        /* Sect. 4.2: "an extra raytracing step to calculate the optical depth to the end of the grid in the
-         * direction of the packet path", here once, at the start of the packet (forced first scattering).  The flight
-         * is drawn from the exponential law truncated at tau_edge and the packet carries the probability
-         * 1 - e^-tau_edge that an analog packet interacts at all (Cashwell & Everett 1959). */
-        double q[3] = { p[0], p[1], p[2] }, tau_edge = 0.0;
-        int c3[3] = { ijk[0], ijk[1], ijk[2] };
-        uint64_t seg = 0;
-        int st = march(G, rc->ch->alpha, q, n, c3, INFINITY, &tau_edge, &seg, NULL);
-        if (st == ST_ESCAPE || (st == ST_SURFACE && !(rc->g->surface_albedo > 0.0))) {
-            const double pint = -expm1(-sa * tau_edge);   /* sa < 1: the hybrid with path length stretching */
-            if (!(pint > 0.0)) {            /* empty path: nothing can interact, the packet ends with no event */
-                if (st == ST_ESCAPE) { cnt->packets_escaped++; cnt->escaped_weight += 1.0; } else cnt->packets_surface++;
-                if (rc->evcount) rc->evcount[pkt] = 0;
-                return;
-            }
-            if (st == ST_ESCAPE) cnt->escaped_weight += exp(-tau_edge);   /* the part that leaves without interacting */
-            W = pint;
-            tau_t = -log1p(-z[2] * pint) / sa;
-            rcl.launch_forced = 1;
-        }
-    }
+    rcl.launch_forced = forced_launch(rc, p, n, ijk, z[2], &W, &tau_t, cnt);
+    if (rcl.launch_forced < 0) { if (rc->evcount) rc->evcount[pkt] = 0; return; }
     transport(&rcl, pkt, p, n, ijk, W, tau_t, 0, batch, cnt);
 }
 
@@ -1023,7 +1029,10 @@ int orc_run_transmission(const orc_grid *g, const orc_opacity *op, const orc_par
                     c3[0] = G.nlev - 1;
                     orc_counters cnt;
                     memset(&cnt, 0, sizeof cnt);
-                    transport(&rc, (uint32_t)pkt, pp, nn3, c3, 1.0, -log(z[2]), 0, batch, &cnt);
+                    double Wp = 1.0, tau_t = -log(z[2]);
+                    rc.launch_forced = forced_launch(&rc, pp, nn3, c3, z[2], &Wp, &tau_t, &cnt);
+                    if (rc.launch_forced >= 0) transport(&rc, (uint32_t)pkt, pp, nn3, c3, Wp, tau_t, 0, batch, &cnt);
+                    else if (rc.evcount) rc.evcount[pkt] = 0;
                     out->counters.events += cnt.events;
                     out->counters.segments_transport += cnt.segments_transport;
                     out->counters.segments_peel += cnt.segments_peel;

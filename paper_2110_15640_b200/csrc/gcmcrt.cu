@@ -548,6 +548,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     if (ncr > (1 << 24)) return fail(g, GCMCRT_E_INVALID, "too many channels in one run");
     const int npix = prm->npix > 0 && out->image ? prm->npix : 0;
     const bool timed = prm->timing != 0;   // host-synchronous pass loop with cudaEvents around the kernels
+    // Sect. 5.1 with multiple scattering (L259, N12): after the chords' initial peel-off the packets are transported
+    const bool ms_trans = mode == 2 && prm->scatter_on && prm->star_solid_angle > 0.0;
     // GCMCRT_HOST_LOOP=1: the host drives the pass loop (one wait per pass) without recording events -- for profilers,
     // which do not see kernels launched from inside a conditional graph node
     static const bool host_loop_env = std::getenv("GCMCRT_HOST_LOOP") && std::atoi(std::getenv("GCMCRT_HOST_LOOP")) != 0;
@@ -562,6 +564,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     if (!(prm->stretch_alpha >= 0.0 && prm->stretch_alpha <= 1.0) || (prm->stretch_alpha > 0.0 && prm->stretch_alpha < 1.0 && prm->continuous_absorption))
         return fail(g, GCMCRT_E_INVALID, "stretch_alpha must be in [0, 1] and excludes continuous_absorption");
     if (mode == 2 && n_obs < 1) return fail(g, GCMCRT_E_INVALID, "transmission needs at least one observer direction");
+    if (!(prm->star_solid_angle >= 0.0)) return fail(g, GCMCRT_E_INVALID, "star_solid_angle must be >= 0");
 
     // ---- outputs
     OutBuf o_flux, o_ltot, o_val, o_sig, o_img, o_evc, o_ctb, o_cnt;
@@ -599,6 +602,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.survival_bias = prm->survival_bias != 0;
     rc.cloud_phase = prm->cloud_phase;
     rc.forced_scatter = prm->forced_scatter;
+    rc.launch_chord = 0;
     rc.stretch = (prm->stretch_alpha > 0.0 && prm->stretch_alpha < 1.0) ? float(prm->stretch_alpha) : 1.0f;
     rc.inv_stretch = 1.0f / rc.stretch;
     rc.alpha2 = nullptr;
@@ -608,6 +612,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     rc.n_batches = nb;
     rc.n_obs_total = std::max(n_obs, 1);
     normalize3(prm->star_dir, rc.star);
+    for (int m = 0; m < 3; ++m) rc.launch_dir[m] = -rc.star[m];
     {
         double sd[3] = {rc.star[0], rc.star[1], rc.star[2]};
         perp_basis(sd, rc.e1, rc.e2);
@@ -641,7 +646,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     L.pk = peel_kernel<16>;
     L.emission = emission != 0 ? 1 : 0;
     L.smem_t = smem_t;
-    if (mode != 2) {
+    if (mode != 2 || ms_trans) {
         CUDA_TRY(g, cudaFuncSetAttribute(L.tk, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem_t)));
         CUDA_TRY(g, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_t, L.tk, kTransportThreads, smem_t));
         if (occ_t < 1) return fail(g, GCMCRT_E_INVALID, "grid tables do not fit in shared memory");
@@ -652,7 +657,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     // last generation and whatever found the event buffer full).  A pass starts with at most ev_cap / 2 inherited
     // entries (else it only drains) and parks each of its <= ev_cap / 2 fresh packets at most once: <= ev_cap in all
     const unsigned long long susp_cap = threads_t + (g->tune[2] > 0 ? 1ull * g->ev_cap : 0ull);
-    if (mode != 2) {
+    if (mode != 2 || ms_trans) {
         for (int b = 0; b < 2; ++b) {
             CUDA_TRY(g, g->s0[b].ensure(susp_cap * sizeof(float4)));
             CUDA_TRY(g, g->s1[b].ensure(susp_cap * sizeof(float4)));
@@ -670,7 +675,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     ev.soft_cap = (unsigned long long)g->ev_cap > 4 * threads_t ? g->ev_cap - (unsigned int)(2 * threads_t) : g->ev_cap / 2;
     ev.chan_lo = &ctrl->chan_lo;
 
-    const int n_runs = prm->doppler_on ? std::max(n_obs, 1) : 1;
+    const int n_runs = (prm->doppler_on || ms_trans) ? std::max(n_obs, 1) : 1;   // one run per observer: its own table / its own chords
     unsigned long long passes_host = 0;   // transmission: one "pass" per run, counted here
     unsigned launches_per_pass = 0;
     if (timed) CUDA_TRY(g, ensure_events(g));
@@ -688,6 +693,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         } else {
             if ((g->staged_obs != -1 || g->staged_cont != cont) && (rcode = stage_opacity(g, nullptr, 0, s, cont, timed))) return rcode;
             rc.obs_first = 0; rc.n_obs_run = n_obs;
+            if (ms_trans) { rc.obs_first = run; rc.n_obs_run = 1; }
         }
         rc.magic_nobs = magic_div((unsigned long long)std::max(rc.n_obs_run, 1));
         rc.alpha = g->alpha.as<float>();
@@ -769,7 +775,16 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
                 g->ms_peel += c;
             }
             ++passes_host;
-            continue;
+            if (!ms_trans) continue;
+            // the packets go on from their chords' starts toward this run's observer; their peel-offs are taken off the
+            // chords' terms by the peel kernel (chord_scale)
+            const int o = rc.obs_first;
+            rc.launch_chord = 1;
+            for (int m = 0; m < 3; ++m) { rc.launch_dir[m] = rc.obs[o][m]; rc.tr_ex[m] = rc.img_ex[o][m]; rc.tr_ey[m] = rc.img_ey[o][m]; }
+            rc.tr_star_radius = float(prm->star_radius);
+            rc.tr_planet_x = float(prm->planet_xy[0]); rc.tr_planet_y = float(prm->planet_xy[1]);
+            rc.tr_ld_c1 = float(prm->ld_c1); rc.tr_ld_c2 = float(prm->ld_c2);
+            rc.tr_domega = float(prm->star_solid_angle);
         }
 
         // ---- the pass loop of this run
@@ -901,7 +916,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     g->ms_stage += g->ms_stage_pending;
     g->ms_stage_pending = 0.0;
     if (o_cnt.dev) {
-        finalize_counters_kernel<<<1, 1, 0, s>>>(g->counters.as<DevCounters>(), mode == 2 ? nullptr : ctrl,
+        finalize_counters_kernel<<<1, 1, 0, s>>>(g->counters.as<DevCounters>(), (mode == 2 && !ms_trans) ? nullptr : ctrl,
                                                 static_cast<gcmcrt_counters*>(o_cnt.dev), g->launches + 1, launches_per_pass,
                                                 passes_host, g->ms_stage, g->ms_emis, g->ms_transport, g->ms_peel, g->ms_sort);
         CUDA_TRY(g, cudaGetLastError());

@@ -210,6 +210,13 @@ struct RunConst {
     const float* alpha2;           // continuous absorption: [n_chan][ncol][col_stride] pairs (alpha_sca, alpha_abs), or NULL
     int forced_scatter;            // Sect. 4.2: 1 = forced first scattering of albedo packets, 2 = every flight forced
     float stretch, inv_stretch;    // Sect. 4.2, path length stretching: flights from a e^{-a tau}, a = stretch (1 = off), 1 / a
+    // Sect. 5.1 with multiple scattering (L259, N12): packets start on transit chords toward observer `obs_first`
+    // instead of on the star-facing disc; every peel-off of packet i enters the flux with the factor
+    // -W_ld,i b_i dOmega (chord_scale(): a function of the packet's launch block, recomputed where it is needed)
+    int launch_chord;
+    float launch_dir[3];           // direction of the first flight: -star (albedo) or the observer (chords)
+    float tr_ex[3], tr_ey[3];      // sky-plane frame of the chords' observer (C19)
+    float tr_star_radius, tr_planet_x, tr_planet_y, tr_ld_c1, tr_ld_c2, tr_domega;
     float surface_albedo;
     double xi;
     int n_batches;
@@ -524,6 +531,41 @@ __global__ void __launch_bounds__(256) emis_guide_kernel(int n_chan, int ncell, 
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Transit chords (Sect. 5.1, Eq. 20-23): launch block (zeta0, zeta1) -> impact parameter b uniform in [R_p0, R_TOA]
+// (Eq. 21 carries the factor b_i), azimuth around the limb, limb-darkening weight of the stellar disc point behind it.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void chord_point(const RunConst& rc, float z0, float z1, float& b, float& X, float& Y, float& W)
+{
+    b = fmaf(z0, rc.geom.Rtoa - rc.geom.R0, rc.geom.R0);
+    float sp, cp;
+    sincospif(2.0f * z1, &sp, &cp);
+    X = b * cp; Y = b * sp;
+    W = 1.0f;
+    if (rc.tr_star_radius > 0.f) {                         // Eq. 22-23
+        const float sx = (rc.tr_planet_x + X) / rc.tr_star_radius, sy = (rc.tr_planet_y + Y) / rc.tr_star_radius;
+        const float rho2 = fmaf(sx, sx, sy * sy);
+        const float mu1 = 1.0f - sqrtf(fmaxf(0.f, 1.0f - rho2));
+        W = rho2 >= 1.0f ? 0.f : 1.0f - rc.tr_ld_c1 * mu1 - rc.tr_ld_c2 * mu1 * mu1;
+    }
+}
+// the chord's start on the star side of the TOA sphere
+__device__ __forceinline__ void chord_start(const RunConst& rc, float b, float X, float Y, float& px, float& py, float& pz)
+{
+    const float Rt = rc.geom.Rtoa, h = sqrtf(fmaxf(0.f, (Rt - b) * (Rt + b)));
+    px = X * rc.tr_ex[0] + Y * rc.tr_ey[0] - h * rc.launch_dir[0];
+    py = X * rc.tr_ex[1] + Y * rc.tr_ey[1] - h * rc.launch_dir[1];
+    pz = X * rc.tr_ex[2] + Y * rc.tr_ey[2] - h * rc.launch_dir[2];
+}
+// what a peel-off of packet (ckey, pkt) adds to the chord's term of Eq. 21: -W_ld b dOmega (reading N12)
+__device__ __forceinline__ float chord_scale(const RunConst& rc, uint32_t ckey, uint32_t pkt)
+{
+    const Zeta4 z = zeta_block(rc.seed, ckey, pkt, 0, 0);
+    float b, X, Y, W;
+    chord_point(rc, z.z0, z.z1, b, X, Y, W);
+    return -W * b * rc.tr_domega;
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // Scattering physics (A8), fp32.
 // ---------------------------------------------------------------------------------------------------------
 // Eq. 6 as repaired (C7): q = 4 zeta - 2, u = cbrt(q + sqrt(1 + q^2)), cos = u - 1/u
@@ -825,25 +867,36 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                 const uint32_t ckey = rc.chan_key0 + uint32_t(ctab);
                                 const Zeta4 z = zeta_block(rc.seed, ckey, pk.pkt, 0, 0);
                                 if (rc.mode == 0) {
-                                    // O3: uniform point on the star-facing TOA disc, direction -s^
-                                    const float b = rc.geom.Rtoa * sqrtf(z.z0);
-                                    float sp, cp;
-                                    sincospif(2.0f * z.z1, &sp, &cp);
-                                    const float h = rc.geom.Rtoa * sqrtf(1.0f - z.z0);
-                                    const float ax = b * cp, ay = b * sp;
-                                    const float px = ax * rc.e1[0] + ay * rc.e2[0] + h * rc.star[0];
-                                    const float py = ax * rc.e1[1] + ay * rc.e2[1] + h * rc.star[1];
-                                    const float pz = ax * rc.e1[2] + ay * rc.e2[2] + h * rc.star[2];
+                                    // O3: uniform point on the star-facing TOA disc, direction -s^ (or, Sect. 5.1 with
+                                    // multiple scattering, the start of a transit chord, direction o^)
+                                    float px, py, pz;
+                                    bool dark = false;
+                                    if (rc.launch_chord) {
+                                        float b, X, Y, Wld;
+                                        chord_point(rc, z.z0, z.z1, b, X, Y, Wld);
+                                        chord_start(rc, b, X, Y, px, py, pz);
+                                        dark = !(Wld > 0.f);
+                                    } else {
+                                        const float b = rc.geom.Rtoa * sqrtf(z.z0);
+                                        float sp, cp;
+                                        sincospif(2.0f * z.z1, &sp, &cp);
+                                        const float h = rc.geom.Rtoa * sqrtf(1.0f - z.z0);
+                                        const float ax = b * cp, ay = b * sp;
+                                        px = ax * rc.e1[0] + ay * rc.e2[0] + h * rc.star[0];
+                                        py = ax * rc.e1[1] + ay * rc.e2[1] + h * rc.star[1];
+                                        pz = ax * rc.e1[2] + ay * rc.e2[2] + h * rc.star[2];
+                                    }
                                     int j, k;
                                     locate_angles(gs, px, py, pz, j, k);
                                     pk.W = 1.0f;
                                     pk.tau_t = -logf(z.z2);
                                     pk.tau = 0.f; pk.fl_seg = 0;
-                                    ray_init<DUAL>(pk.ray, gs, px, py, pz, -rc.star[0], -rc.star[1], -rc.star[2], gs.nlev - 1,
+                                    ray_init<DUAL>(pk.ray, gs, px, py, pz, rc.launch_dir[0], rc.launch_dir[1], rc.launch_dir[2], gs.nlev - 1,
                                              j, k, alpha_c);
                                     if (!(!DUAL && rc.forced_scatter && force_flight(rc, gs, pk.ray, alpha_c, pk.tau_t, pk.W, c_escw)))
                                         pk.tau_t *= rc.inv_stretch;
                                     st = LS_FLY;
+                                    if (dark) { st = LS_IDLE; finish_packet(rc, pk); }   // chord off the stellar disc: no light to scatter
                                 } else {
                                     // O4: cell ~ luminosity (Eq. 13) with composite bias xi, uniform point in the cell
                                     const int ncell = rc.geom.ncell;
@@ -1123,6 +1176,8 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
             const float* alpha_c = rc.alpha + (size_t)(rc.chan_begin + max(chan, 0)) * rc.geom.alpha_stride;
             // what the event scatters toward an observer: W omega (medium, Eq. 14), W (emission), W a (surface)
             float wsca = a.w, pgas = 0.f, g = 0.f;
+            if (rc.launch_chord && have)   // scattered light of a transit chord: -W_ld b dOmega of the packet's chord (N12)
+                wsca *= -chord_scale(rc, rc.chan_key0 + uint32_t(rc.chan_begin + chan), __float_as_uint(c.w));
             if (have && kind == EV_MEDIUM) {
                 wsca *= pr.x; pgas = pr.y; g = pr.z;
             } else if (kind == EV_SURFACE) {
@@ -1180,7 +1235,7 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
                 c_seg += seg32;
                 // ---------------- rays that reached the top of the atmosphere: Eq. 14 ----------------
                 if (st == RAY_ESCAPE) {
-                    const float f = pref * expf(-tau);
+                    const float f = rc.launch_chord ? -pref * expf(-tau) : pref * expf(-tau);
                     if (chan == warp_chan) atomicAdd(bins + obs * rc.n_batches + bt, f);
                     else atomicAdd(rc.flux + ((size_t)chan * rc.n_obs_total + rc.obs_first + obs) * rc.n_batches + bt, double(f));
                     if (rc.image) {

@@ -224,19 +224,30 @@ __device__ __forceinline__ void flight_load(const float* fl, const RunConst& rc,
 }
 
 // O3: uniform point on the star-facing TOA disc from Philox block (event 0, purpose 0), and its entry column
+// (Sect. 5.1 with multiple scattering: the start of the packet's transit chord instead; returns false for a chord off
+// the stellar disc, which carries no light)
 template <bool LOCATE = true>
-__device__ __forceinline__ void albedo_launch_point(const RunConst& rc, const GeomSmem& gs, const Zeta4& z, float& px,
+__device__ __forceinline__ bool albedo_launch_point(const RunConst& rc, const GeomSmem& gs, const Zeta4& z, float& px,
                                                     float& py, float& pz, int& j, int& k)
 {
-    const float b = rc.geom.Rtoa * sqrtf(z.z0);
-    float sp, cp;
-    sincospif(2.0f * z.z1, &sp, &cp);
-    const float h = rc.geom.Rtoa * sqrtf(1.0f - z.z0);
-    const float ax = b * cp, ay = b * sp;
-    px = ax * rc.e1[0] + ay * rc.e2[0] + h * rc.star[0];
-    py = ax * rc.e1[1] + ay * rc.e2[1] + h * rc.star[1];
-    pz = ax * rc.e1[2] + ay * rc.e2[2] + h * rc.star[2];
+    bool lit = true;
+    if (rc.launch_chord) {
+        float b, X, Y, Wld;
+        chord_point(rc, z.z0, z.z1, b, X, Y, Wld);
+        chord_start(rc, b, X, Y, px, py, pz);
+        lit = Wld > 0.f;
+    } else {
+        const float b = rc.geom.Rtoa * sqrtf(z.z0);
+        float sp, cp;
+        sincospif(2.0f * z.z1, &sp, &cp);
+        const float h = rc.geom.Rtoa * sqrtf(1.0f - z.z0);
+        const float ax = b * cp, ay = b * sp;
+        px = ax * rc.e1[0] + ay * rc.e2[0] + h * rc.star[0];
+        py = ax * rc.e1[1] + ay * rc.e2[1] + h * rc.star[1];
+        pz = ax * rc.e1[2] + ay * rc.e2[2] + h * rc.star[2];
+    }
     if (LOCATE) locate_angles(gs, px, py, pz, j, k);
+    return lit;
 }
 
 __device__ __forceinline__ void wave_item(const RunConst& rc, unsigned long long item, uint32_t& chan_run, uint32_t& pkt)
@@ -293,6 +304,7 @@ wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
         uint32_t chan_run = 0, pkt = 0;
         Ray ray{};
         float tau_t = 0.f, z2 = 0.f;
+        bool lit = true;
         const float* alpha_c = rc.alpha;
         if (active) {
             const unsigned int it = __ldg(wc.perm + t);
@@ -304,24 +316,29 @@ wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
             // the entry column was located when the launch key was made: read it back instead of locating again
             const unsigned int col = (__ldg(wc.keys + it) / kLaunchTauBuckets) % (unsigned int)(gs.nlat * gs.nlon);
             int j = int(col % (unsigned int)gs.nlat), k = int(col / (unsigned int)gs.nlat);
-            albedo_launch_point<false>(rc, gs, z, px, py, pz, j, k);
+            lit = albedo_launch_point<false>(rc, gs, z, px, py, pz, j, k);
             tau_t = -logf(z.z2);
             z2 = z.z2;
-            ray_init(ray, gs, px, py, pz, -rc.star[0], -rc.star[1], -rc.star[2], gs.nlev - 1, j, k, alpha_c);
+            ray_init(ray, gs, px, py, pz, rc.launch_dir[0], rc.launch_dir[1], rc.launch_dir[2], gs.nlev - 1, j, k, alpha_c);
         }
         float W = 1.0f;
         bool fly = active;
+        if (active && !lit) {   // a transit chord off the stellar disc: the packet ends with no event
+            wave_finish_packet(rc, chan_run, pkt, 0u);
+            fly = false;
+        }
+        const bool probe_on = fly;
         bool forced = false;
         if (FORCED) {
             // Sect. 4.2 (L179), forced first scattering: the extra ray trace to the end of the grid gives tau_edge; the
             // flight is drawn from the exponential law truncated there and the packet carries 1 - e^-tau_edge.  A ray
             // that ends on a reflecting lower boundary stays analog.
             Ray probe = ray;
-            int st = active ? RAY_FLYING : RAY_NONE;
+            int st = probe_on ? RAY_FLYING : RAY_NONE;
             float tau_e = 0.f;
             WaveCounters unused;
             wave_march<KSTEPS>(rc, gs, st, probe, tau_e, kInf, alpha_c, rc.geom.maxseg + 1, unused);
-            if (active && (st == RAY_ESCAPE || (st == RAY_SURFACE && !(rc.surface_albedo > 0.f)))) {
+            if (probe_on && (st == RAY_ESCAPE || (st == RAY_SURFACE && !(rc.surface_albedo > 0.f)))) {
                 const float pint = -expm1f(-rc.stretch * tau_e);   // stretch < 1: the hybrid with path length stretching
                 if (!(pint > 0.f)) {   // empty path: the packet ends with no event
                     if (st == RAY_ESCAPE) { ++wcnt.esc; wcnt.escw += 1.0; } else ++wcnt.surf;

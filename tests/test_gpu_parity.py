@@ -1256,3 +1256,53 @@ def test_path_length_stretching_and_hybrid_parity(gpu, orc, monkeypatch, tune):
             with pytest.raises(gpu.GcmcrtError) as e:
                 G.run_emission(dict(prm, **bad))
             assert e.value.code == gpu.E_INVALID
+
+
+@pytest.mark.parametrize("tune", ["16,1,8,4", "16,1,0,4", "16,1,2,4"])
+def test_transmission_with_multiple_scattering_parity(gpu, orc, monkeypatch, tune):
+    """Sect. 5.1 with multiple scattering (L259, reading N12) against the oracle: the packets go on from their chords'
+    starts (launch-order sort, first-flight, generation and persistent kernels with the chord launch), and every event's
+    peel-off, scaled by -W_ld b dOmega of its packet, is taken off the chord's term by the peel kernel.  3D correlated-k
+    table with clouds, two observers, limb darkening; analog, forced + roulette and stretched flights; the scattered part
+    alone (difference to the raytracer run) against the oracle's; star_solid_angle = 0 is the raytracer run;
+    and the closed form of the single-scattering term on a homogeneous shell (omega Theta(1) T e^-T)."""
+    monkeypatch.setenv("GCMCRT_TUNE", tune)
+    ncpu = os.cpu_count() or 1
+    grid, opac, prm = wl.cfg2(nlon=16, nlat=8, nlev=20, nbands=2, ng=3, packets=30000)
+    obs = np.array([[1.0, 0, 0], [0.36, -0.48, 0.8]])
+    base = dict(prm, obs_dir=obs, star_radius=7.0e8, planet_xy=(3.0e8, -2.0e8), ld_c1=0.4, ld_c2=0.2)
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        ray = G.run_transmission(base)
+        zero = G.run_transmission(dict(base, star_solid_angle=0.0, scatter_on=1))
+        assert np.allclose(ray["flux_sum"], zero["flux_sum"], rtol=1e-12)     # the same run (sums in atomics order)
+        assert zero["counters"]["events"] == ray["counters"]["events"] == 2 * 6 * 30000
+        for extra in (dict(), dict(forced_scatter=2, survival_bias=1, roulette_w_min=0.02, roulette_survive=0.2),
+                      dict(stretch_alpha=0.5, survival_bias=1, roulette_w_min=0.05, roulette_survive=0.25)):
+            p = dict(base, star_solid_angle=0.03, **extra)
+            g = G.run_transmission(p, want_event_count=True)
+            o = orc.run_transmission(grid, opac, p, want_event_count=True)
+            vo, so = orc.reduce(o, "transmission")
+            assert np.all(np.abs(g["value"] - vo) <= 4 * so + 1e-5 * np.abs(vo))
+            same = (g["event_count"] == o["event_count"]).mean()
+            assert same >= 0.99, same
+            assert abs(g["counters"]["events"] - o["counters"]["events"]) <= 0.01 * o["counters"]["events"]
+            # the scattered light alone, batch by batch (the chords' baseline is common to both runs of each side)
+            o0 = orc.run_transmission(grid, opac, base)
+            ds_g, ds_o = ray["flux_sum"] - g["flux_sum"], o0["flux_sum"] - o["flux_sum"]
+            assert np.all(ds_o.sum(axis=2) > 0)
+            assert np.allclose(ds_g.sum(axis=2), ds_o.sum(axis=2), rtol=2e-2), ds_g.sum(axis=2) / ds_o.sum(axis=2)
+    # closed form: homogeneous shell, isotropic scatterers, one scattering
+    R0, Rt, omega, dO, N, nb = 1.0e7, 1.4e7, 0.8, 0.02, 200000, 32
+    alpha = 0.6 / (Rt - R0)
+    grid, opac = wl.uniform_medium(6, 4, 5, R0, Rt, alpha, omega, g=0.0, pgas=0.0)
+    p = wl.default_params(packets_per_channel=N, seed=6, obs_dir=[[0.0, 0.6, 0.8]], max_events=1, star_solid_angle=dO)
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        g1 = G.run_transmission(p)
+        g0 = G.run_transmission(dict(p, star_solid_angle=0.0))
+    b = R0 + (np.arange(400000) + 0.5) / 400000 * (Rt - R0)
+    T = 2.0 * alpha * np.sqrt(Rt ** 2 - b ** 2)
+    sca = dO * omega / (4 * PI) * np.sum(b * T * np.exp(-T)) * (Rt - R0) / b.size
+    d = (g0["flux_sum"] - g1["flux_sum"])[0, 0] / (N / nb) * (Rt - R0)
+    assert abs(d.mean() - sca) < 4 * d.std(ddof=1) / np.sqrt(nb) + 1e-4 * sca, (d.mean(), sca)

@@ -1216,7 +1216,10 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
                 unsigned int seg32 = 0;
                 if (have && pref > 0.0f) {
                     ray_init(ray, gs, a.x, a.y, a.z, ox, oy, oz, ci, cj, ck, alpha_c);
-                    st = RAY_FLYING;
+                    // a ray that descends and does not turn inside the grid ends on the lower boundary: nothing of it
+                    // reaches the observer (Eq. 14 along a ray that leaves through the top), so it is not marched at all
+                    // -- with observers all around the orbit these are the long rays through the deep atmosphere
+                    st = (ray.rad_step < 0 && ray.i_turn < 0) ? RAY_SURFACE : RAY_FLYING;
                     ++c_rays;
                 }
                 // all lanes start together, so one warp-uniform step budget guards against a ray that never ends

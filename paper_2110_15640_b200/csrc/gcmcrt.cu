@@ -879,6 +879,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
         L.tail_items = n_gen > 0 ? 0ull : total_items;   // wavefront: the persistent kernel only finishes what the generations leave over
         L.plan.total_items = total_items; L.plan.susp_cap = susp_cap; L.plan.max_passes = 1ull << 20;
         L.plan.batch0 = std::max<unsigned long long>(1024, g->ev_cap / (unsigned long long)g->tune[3]);
+        // emission without scattering: exactly one event per packet, nothing to learn -- the first pass is a full one
+        if (emission && !prm->scatter_on) L.plan.batch0 = std::max<unsigned long long>(1024, (unsigned long long)(0.85 * double(g->ev_cap)));
         L.plan.n_pkt = uint32_t(n_pkt); L.plan.ev_cap = g->ev_cap; L.plan.n_gen = n_gen; L.plan.n_chan_run = ncr;
         run_begin_kernel<<<1, 1, 0, s>>>(ctrl, L.plan);
         ++g->launches;

@@ -37,8 +37,14 @@ def _check_parity(orc, g, o, mode, min_same=0.99, check_events=True):
     vg, sg = g["value"], g["sigma"]
     tol = 4 * so + 1e-5 * np.abs(vo) + 1e-300
     assert np.all(np.abs(vg - vo) <= tol), (np.abs(vg - vo) / tol).max()
-    # sigma itself agrees (same batches, same streams)
-    assert np.allclose(sg, so, rtol=0.1, atol=1e-5 * np.abs(vo).max() + 1e-300)
+    # sigma itself agrees (same batches, same streams).  It is a second moment: where a few bright packets make the variance
+    # one packet that differs on the two sides moves it, so the comparison is statistical -- typical agreement within 5 %,
+    # every value within a factor 2
+    pos = so > 1e-5 * np.abs(vo).max() + 1e-300
+    if pos.any():
+        ratio = sg[pos] / so[pos]
+        assert np.median(np.abs(ratio - 1)) < 0.05 and np.all((ratio > 0.5) & (ratio < 2.0)), (ratio.min(), ratio.max())
+    assert np.all(sg[~pos] <= 2e-5 * np.abs(vo).max() + 1e-300)
     if mode == "emission":
         assert np.allclose(g["L_tot"], o["L_tot"], rtol=1e-5)
     if check_events and g.get("event_count") is not None and o["event_count"] is not None:
@@ -1306,3 +1312,33 @@ def test_transmission_with_multiple_scattering_parity(gpu, orc, monkeypatch, tun
     sca = dO * omega / (4 * PI) * np.sum(b * T * np.exp(-T)) * (Rt - R0) / b.size
     d = (g0["flux_sum"] - g1["flux_sum"])[0, 0] / (N / nb) * (Rt - R0)
     assert abs(d.mean() - sca) < 4 * d.std(ddof=1) / np.sqrt(nb) + 1e-4 * sca, (d.mean(), sca)
+
+
+def test_largest_supported_column_and_wide_grids(gpu, orc):
+    """The sizes at the edge of what the kernels are built for: 256 levels (the 8-chunk instance of the emission CDF
+    kernel at its limit; 257 levels are refused for emission with E_INVALID), and a grid with many columns and few levels
+    (128 x 64 x 4: the geometry table, the launch-order sort and the column indexing at the other extreme), each against
+    the oracle in emission and albedo mode."""
+    ncpu = os.cpu_count() or 1
+    grid, opac, prm = wl.cfg3(nlon=4, nlat=3, nlev=256, nbands=1, ng=2, packets=15000, n_obs=2)
+    g = _gpu_run(gpu, grid, opac, prm, "emission", want_event_count=True)
+    o = orc.run_emission(grid, opac, dict(prm, n_threads=ncpu), want_event_count=True)
+    _check_parity(orc, g, o, "emission")
+    ga = _gpu_run(gpu, grid, opac, dict(prm, obs_dir=prm["obs_dir"][:1]), "albedo", want_event_count=True)
+    oa = orc.run_albedo(grid, opac, dict(prm, obs_dir=prm["obs_dir"][:1], n_threads=ncpu), want_event_count=True)
+    _check_parity(orc, ga, oa, "albedo")
+    grid2, opac2, prm2 = wl.cfg3(nlon=4, nlat=3, nlev=257, nbands=1, ng=1, packets=100, n_obs=1)
+    with gpu.Grid(grid2) as G:
+        G.set_opacity(opac2)
+        with pytest.raises(gpu.GcmcrtError) as e:
+            G.run_emission(prm2)
+        assert e.value.code == gpu.E_INVALID
+        r = G.run_albedo(prm2)                                   # albedo has no such limit
+        assert r["counters"]["packets_stuck"] == 0
+    grid, opac, prm = wl.cfg3(nlon=128, nlat=64, nlev=4, nbands=1, ng=2, packets=30000, n_obs=3)
+    g = _gpu_run(gpu, grid, opac, prm, "emission", want_event_count=True)
+    o = orc.run_emission(grid, opac, dict(prm, n_threads=ncpu), want_event_count=True)
+    _check_parity(orc, g, o, "emission")
+    ga = _gpu_run(gpu, grid, opac, dict(prm, obs_dir=prm["obs_dir"][:1]), "albedo", want_event_count=True)
+    oa = orc.run_albedo(grid, opac, dict(prm, obs_dir=prm["obs_dir"][:1], n_threads=ncpu), want_event_count=True)
+    _check_parity(orc, ga, oa, "albedo")

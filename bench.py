@@ -48,8 +48,8 @@ UNIT = "events/s"
 #   peel ray = record read, phase function, ray set-up (ray_init), round control, exp, bin accumulation
 I_UNITS = {            # workload: (per peel segment, per peel ray)
     "cfg2": (28.9, 450.0),
-    "cfg3": (37.9, 317.0),     # ~10 segments per ray (rays toward 8 phases, many end on the night side): entry / exit weighs more; the
-                               # record and the phase-function inputs serve 8 rays
+    "cfg3": (41.2, 300.0),     # ~9 segments per ray (rays toward 8 phases; those that end on the lower boundary are not marched):
+                               # entry / exit weighs more; the record and the phase-function inputs serve 8 rays
     "cfg4": (28.4, 450.0),
 }
 I_SEG_1D = 23.0      # nlat = nlon = 1: loop + entry / exit, no lateral crossings

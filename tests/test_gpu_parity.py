@@ -1342,3 +1342,49 @@ def test_largest_supported_column_and_wide_grids(gpu, orc):
     ga = _gpu_run(gpu, grid, opac, dict(prm, obs_dir=prm["obs_dir"][:1]), "albedo", want_event_count=True)
     oa = orc.run_albedo(grid, opac, dict(prm, obs_dir=prm["obs_dir"][:1], n_threads=ncpu), want_event_count=True)
     _check_parity(orc, ga, oa, "albedo")
+
+
+@pytest.mark.parametrize("mode", ["emission", "transmission"])
+def test_pass_loop_drivers_agree_for_emission_and_transmission(gpu, monkeypatch, mode):
+    """The ways a run's pass loop can be driven -- the conditional WHILE node of the default path, the host loop of
+    run_params.timing = 1, and the WHILE node added to a caller's graph by a stream capture of the whole call -- carry the
+    same packets: emission toward 3 phases with Doppler shifts (one run, one staging and one CDF per observer), and
+    transmission with multiple scattering (one chord run per observer), with a small event buffer so that the loop
+    iterates."""
+    import torch
+    monkeypatch.setenv("GCMCRT_EVENT_CAP", "60000")
+    if mode == "emission":
+        grid, opac, prm = wl.cfg4(nlon=12, nlat=6, nlev=16, n_chan=24, n_lines=12, packets=20000)
+        prm = dict(prm, scatter_on=1, obs_dir=wl.orbital_phase_dirs(4)[[1, 2, 3]], doppler_halfwidth=3)
+        opac = dict(opac, k_sca_ray=np.full_like(opac["k_abs"], 2.0e-4))
+        call, fn_name = "run_emission", "gcmcrt_run_emission"
+    else:
+        grid, opac, prm = wl.cfg2(nlon=12, nlat=6, nlev=16, nbands=2, ng=3, packets=20000)
+        prm = dict(prm, obs_dir=np.array([[1.0, 0, 0], [0.0, 0.6, 0.8]]), star_solid_angle=0.03)
+        call, fn_name = "run_transmission", "gcmcrt_run_transmission"
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s), gpu.Grid(grid, stream=s) as G:
+        G.set_opacity(opac)
+        ref = getattr(G, call)(prm, want_event_count=True, device_outputs=True)
+        assert ref["counters"]["passes"] > 3 and ref["counters"]["device_status"] == 0
+        tim = getattr(G, call)(dict(prm, timing=1), want_event_count=True, device_outputs=True)
+        assert torch.equal(tim["event_count"], ref["event_count"]) and tim["counters"]["passes"] == ref["counters"]["passes"]
+        assert torch.allclose(tim["flux_sum"], ref["flux_sum"], rtol=1e-5)
+        # capture the whole call and replay it
+        outs = {k: torch.zeros_like(ref[k]) for k in ("flux_sum", "L_tot", "value", "sigma", "event_count")}
+        cnt = torch.zeros(gpu.C.sizeof(gpu.Counters), dtype=torch.uint8, device="cuda")
+        p, keep = gpu.make_params(prm)
+        res = gpu.Result()
+        res.flux_sum, res.L_tot, res.value, res.sigma = (outs[k].data_ptr() for k in ("flux_sum", "L_tot", "value", "sigma"))
+        res.event_count, res.counters = outs["event_count"].data_ptr(), cnt.data_ptr()
+        graph = torch.cuda.CUDAGraph()
+        s.synchronize()
+        with torch.cuda.graph(graph, stream=s, capture_error_mode="relaxed"):
+            rc = getattr(gpu.lib(), fn_name)(G.handle, gpu.C.byref(p), gpu.C.byref(res), gpu.C.c_void_p(torch.cuda.current_stream().cuda_stream))
+        assert rc == 0, gpu.lib().gcmcrt_last_error(G.handle)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(outs["event_count"], ref["event_count"])
+        assert torch.allclose(outs["flux_sum"], ref["flux_sum"], rtol=1e-5) and torch.allclose(outs["value"], ref["value"], rtol=1e-5)
+        assert gpu.read_counters(cnt)["events"] == ref["counters"]["events"]
+        del graph

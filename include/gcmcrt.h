@@ -144,7 +144,7 @@ typedef struct gcmcrt_counters {
     uint64_t rays_peel;          /* peel-off rays integrated */
     uint64_t launches;           /* kernels this call launched (all kinds) */
     /* device time of this call's kernels by kind, from cudaEvents recorded on the caller's stream around each
-       launch (milliseconds, summed over passes / observers) */
+       launch (milliseconds, summed over passes / observers); filled by runs with run_params.timing = 1, else 0 */
     double ms_stage, ms_emission_cdf, ms_transport, ms_peel;
     double ms_sort;              /* counting sort of the event records by (channel, cell) before each peel pass */
     uint64_t device_status;      /* 0 = the pass loop ran to its end; 1 = suspended-packet list overflow, 2 = pass limit
@@ -161,7 +161,7 @@ typedef struct gcmcrt_result {
     double *sigma;         /* [n_chan_run][n_obs]: batch-means standard error of value */
     float *image;          /* [n_chan_run][n_obs][npix][npix] (L83) */
     uint32_t *event_count; /* [n_chan_run][pkt_end-pkt_begin]: peel-off points per packet */
-    gcmcrt_counters *counters; /* one struct */
+    gcmcrt_counters *counters; /* one struct, host|device (device: assembled by a kernel, no host wait) */
     float *contrib;        /* [n_chan_run][n_obs][2][ncell] (cell-flat layout): contribution functions of Sect. 6,
                               Eq. 32, as raw sums of the peeled-off f per event cell: [0] thermal (emission points),
                               [1] scattered (medium and surface events).  CF = contrib / sum over cells. */

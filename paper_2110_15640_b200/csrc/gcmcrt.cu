@@ -67,7 +67,7 @@ struct gcmcrt_grid {
     int staged_halfwidth = 0;
 
     // emission
-    DevBuf Lcell, Lcum, Ltot, guide;
+    DevBuf Lcell, Lcum, Lcol, Ltot, guide;
 
     // workspace
     DevBuf ev0, evkeys, perm, hist, tile_sums, lkeys, lperm, lhist, ltile, flights, s0[2], s1[2], s2[2], ctrl, counters, counters_out, flux, ltot_out, value, sigma, image, evcount, contrib;
@@ -704,6 +704,7 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             const size_t n = size_t(g->n_chan) * g->ncell;
             if (prm->emission_bias > 0.0) CUDA_TRY(g, g->Lcell.ensure(n * sizeof(double)));
             CUDA_TRY(g, g->Lcum.ensure(n * sizeof(double)));
+            CUDA_TRY(g, g->Lcol.ensure(size_t(g->n_chan) * g->nlat * g->nlon * sizeof(double)));
             CUDA_TRY(g, g->Ltot.ensure(size_t(g->n_chan) * sizeof(double)));
             EmisParams ep;
             ep.n_chan = g->n_chan; ep.nlev = g->nlev; ep.nlat = g->nlat; ep.nlon = g->nlon; ep.ncell = g->ncell;
@@ -713,19 +714,22 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             ep.lambda = g->lambda64.as<double>();
             ep.r_edges = g->r64.as<double>(); ep.cth_edges = g->cth64.as<double>(); ep.ph_edges = g->ph64.as<double>();
             ep.tau_vert_max = prm->tau_vert_max;
-            ep.Lcell = prm->emission_bias > 0.0 ? g->Lcell.as<double>() : nullptr; ep.Lcum = g->Lcum.as<double>(); ep.Ltot = g->Ltot.as<double>();
+            ep.Lcell = prm->emission_bias > 0.0 ? g->Lcell.as<double>() : nullptr; ep.Lcum = g->Lcum.as<double>(); ep.Lcol = g->Lcol.as<double>(); ep.Ltot = g->Ltot.as<double>();
             if (timed) CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
             {
-                const unsigned ge = (unsigned)std::min(g->n_chan, g->sm_count * 8);
-                const size_t sm = (2 * size_t(g->nlev) + 32) * sizeof(double);
-                if (g->nlev <= 64) emis_cdf_kernel<2><<<ge, kEmisThreads, sm, s>>>(ep);
-                else if (g->nlev <= 128) emis_cdf_kernel<4><<<ge, kEmisThreads, sm, s>>>(ep);
-                else if (g->nlev <= 256) emis_cdf_kernel<8><<<ge, kEmisThreads, sm, s>>>(ep);
+                // blockIdx.y = channel; the warps of a channel's CTAs stride through its columns
+                const int ncol = g->nlat * g->nlon, wpb = kEmisThreads / 32;
+                const dim3 ge((unsigned)std::min((ncol + wpb - 1) / wpb, 32), (unsigned)std::min(g->n_chan, 65535));
+                const size_t sm = 2 * size_t(g->nlev) * sizeof(double);
+                if (g->nlev <= 64) emis_col_kernel<2><<<ge, kEmisThreads, sm, s>>>(ep);
+                else if (g->nlev <= 128) emis_col_kernel<4><<<ge, kEmisThreads, sm, s>>>(ep);
+                else if (g->nlev <= 256) emis_col_kernel<8><<<ge, kEmisThreads, sm, s>>>(ep);
                 else return fail(g, GCMCRT_E_INVALID, "emission: nlev > 256 is not supported");
+                emis_colscan_kernel<<<(unsigned)((size_t(g->n_chan) * 32 + 127) / 128), 128, 0, s>>>(g->n_chan, ncol, ep.Lcol, ep.Ltot);
             }
             CUDA_TRY(g, g->guide.ensure(size_t(g->n_chan) * kEmisGuide * sizeof(int)));
             emis_guide_kernel<<<(unsigned)(((long long)g->n_chan * kEmisGuide + 255) / 256), 256, 0, s>>>(
-                g->n_chan, g->ncell, ep.Lcum, ep.Ltot, g->guide.as<int>());
+                g->n_chan, g->ncell, g->nlev, ep.Lcum, ep.Lcol, ep.Ltot, g->guide.as<int>());
             CUDA_TRY(g, cudaGetLastError());
             if (timed) {
                 CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
@@ -734,8 +738,8 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
                 CUDA_TRY(g, cudaEventElapsedTime(&ms, g->tev[0], g->tev[1]));
                 g->ms_emis += ms;
             }
-            g->launches += 2;
-            rc.Lcum = ep.Lcum; rc.Lcell = ep.Lcell; rc.Ltot = ep.Ltot; rc.guide = g->guide.as<int>();
+            g->launches += 3;
+            rc.Lcum = ep.Lcum; rc.Lcol = ep.Lcol; rc.Lcell = ep.Lcell; rc.Ltot = ep.Ltot; rc.guide = g->guide.as<int>();
             // L_tot output [n_chan_run][n_obs]
             const int o0 = prm->doppler_on ? run : 0, o1 = prm->doppler_on ? run + 1 : std::max(n_obs, 1);
             for (int o = o0; o < o1; ++o)
@@ -1140,7 +1144,7 @@ int gcmcrt_destroy(gcmcrt_grid* g)
     cudaGetLastError();
     for (DevBuf* b : {&g->tab, &g->r64, &g->cth64, &g->ph64, &g->rc32, &g->thc32, &g->phc32, &g->T, &g->rho, &g->u, &g->v,
                       &g->w, &g->own_kabs, &g->own_kray, &g->own_kcld, &g->own_g, &g->alpha, &g->alpha2, &g->prop, &g->reff, &g->vlos, &g->node, &g->node_idx, &g->node_w, &g->own_pcell,
-                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Ltot, &g->guide, &g->ev0, &g->evkeys, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
+                      &g->lambda64, &g->Lcell, &g->Lcum, &g->Lcol, &g->Ltot, &g->guide, &g->ev0, &g->evkeys, &g->perm, &g->hist, &g->tile_sums, &g->lkeys, &g->lperm, &g->lhist, &g->ltile, &g->flights, &g->s0[0], &g->s0[1],
                       &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->counters_out, &g->flux, &g->ltot_out,
                       &g->value, &g->sigma, &g->image, &g->evcount, &g->contrib})
         b->release();

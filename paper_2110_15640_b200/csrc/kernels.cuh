@@ -192,7 +192,8 @@ struct RunConst {
     GeomParams geom;
     const float* alpha;    // [n_chan_tab][ncol][col_stride] extinction (m^-1), guard-padded columns (ray.cuh)
     const float4* prop;    // [n_chan_tab][ncell] omega, P_gas, g, k_abs_eff
-    const double* Lcum;    // emission: [n_chan_tab][ncell] running luminosity
+    const double* Lcum;    // emission: [n_chan_tab][ncell] running luminosity inside the cell's column
+    const double* Lcol;    // emission: [n_chan_tab][ncol] luminosity of the columns before (emis_cum())
     const double* Lcell;   // emission, xi > 0 only
     const double* Ltot;    // emission: [n_chan_tab]
     const int* guide;      // emission: [n_chan_tab][kEmisGuide] search brackets of the CDF (emis_guide_kernel)
@@ -389,7 +390,8 @@ struct EmisParams {
     const double *r_edges, *cth_edges, *ph_edges;  // fp64 geometry for the volumes
     double tau_vert_max;
     double* Lcell;  // [n_chan][ncell] L_i, or NULL (kept for the weights of the composite bias, xi > 0)
-    double* Lcum;
+    double* Lcum;   // [n_chan][ncell] column-local running sum
+    double* Lcol;   // [n_chan][nlat * nlon] column totals (emis_col_kernel), then the sums of the columns before (emis_colscan_kernel)
     double* Ltot;
 };
 
@@ -398,6 +400,17 @@ __device__ __forceinline__ double planck_lambda(double lam, double T)
     const double h = 6.62607015e-34, c = 299792458.0, kb = 1.380649e-23;
     const double x = h * c / (lam * kb * T);
     return 2.0 * h * c * c / (lam * lam * lam * lam * lam) / expm1(x);
+}
+
+// 1 / x for a positive, finite, normal x to ~1 ulp: the 20-bit hardware seed and two Newton steps (7 instructions; the
+// IEEE division is ~30 with its special-case path).  The emission kernel divides twice per (channel, cell).
+__device__ __forceinline__ double rcp_pos_f64(double x)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    r = fma(r, fma(-x, r, 1.0), r);
+    r = fma(r, fma(-x, r, 1.0), r);
+    return r;
 }
 
 __device__ __forceinline__ double warp_incl_scan_f64(double v)
@@ -410,21 +423,53 @@ __device__ __forceinline__ double warp_incl_scan_f64(double v)
     return v;
 }
 
-// One CTA per channel, one warp per column, 32 columns per round, lanes along the column (coalesced alpha / prop
-// reads; NCH = chunks of 32 levels).  A round is one memory latency deep: every input of the column is loaded up
-// front, then the warp finds the depth cut (radial optical depth from the top, C15), computes L_i (Eq. 27), scans it,
-// and -- after the 32 column totals have been chained through shared memory -- writes the running sum once.  Every
-// value is carry + (excl_w + local) with excl_{w+1} = excl_w + tot_w evaluated by the same chain in every thread, so
-// the running sum never decreases from one cell to the next.  HBM traffic per (channel, cell): 4 B alpha + 16 B prop
-// in, 8 B out (T, rho stay in L2 across channels).
-constexpr int kEmisThreads = 1024;
+// The CDF is stored in two levels, so that no thread waits for another column:
+//   Lcum[c][cell]  running sum of L_i inside the cell's own column (from its lowest level up to the cell, inclusive),
+//   Lcol[c][col]   sum of the columns before `col` (exclusive), Ltot[c] the channel's total,
+// and the running sum of Eq. 13 at a cell is emis_cum() = Lcol[c][col] + Lcum[c][cell].  It never decreases from one
+// cell to the next: inside a column the same offset is added to a non-decreasing sequence, and Lcol[col + 1] is
+// fl(Lcol[col] + total(col)) by construction (emis_colscan_kernel adds the totals in column order), total(col) being
+// the column's last local value.
+__device__ __forceinline__ double emis_cum(const double* __restrict__ cum_c, const double* __restrict__ col_c, int nlev, int cell)
+{
+    return col_c[cell / nlev] + cum_c[cell];
+}
+
+// First cell whose running luminosity exceeds x, searched in [lo, hi] (Eq. 13), in two levels: the column first -- the
+// running sum at a column's last cell IS the next column's offset (the channel's total after the last column) -- then
+// the cell inside it, with the column's offset loaded once.  Both levels evaluate emis_cum() > x, so the result is the
+// cell a search over emis_cum() alone finds.
+__device__ __forceinline__ int emis_search(const double* __restrict__ cum_c, const double* __restrict__ col_c, double Ltot,
+                                           int nlev, int ncol, int lo, int hi, double x)
+{
+    int clo = lo / nlev, chi = hi / nlev;
+    while (clo < chi) {
+        const int cmid = (clo + chi) >> 1;
+        const double end = cmid + 1 < ncol ? col_c[cmid + 1] : Ltot;   // == emis_cum(last cell of column cmid)
+        if (end > x) chi = cmid; else clo = cmid + 1;
+    }
+    const double off = col_c[clo];
+    lo = max(lo, clo * nlev); hi = min(hi, clo * nlev + nlev - 1);
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (off + cum_c[mid] > x) hi = mid; else lo = mid + 1;
+    }
+    return lo;
+}
+
+// One warp per (channel, column), lanes along the column (coalesced alpha / prop reads; NCH = chunks of 32 levels),
+// blockIdx.y = channel, the warps of a CTA stride through the channel's columns.  A warp loads every input of its
+// column up front, finds the depth cut (radial optical depth from the top, C15), computes L_i (Eq. 27), scans it and
+// writes the column-local running sum and the column total: no barrier and no dependence between columns, so the SM
+// hides one column's latency behind the others'.  HBM traffic per (channel, cell): 4 B alpha + 16 B prop in, 8 B out
+// (T, rho stay in L2 across channels).
+constexpr int kEmisThreads = 256;
 template <int NCH>
-__global__ void __launch_bounds__(kEmisThreads) emis_cdf_kernel(const EmisParams p)
+__global__ void __launch_bounds__(kEmisThreads) emis_col_kernel(const EmisParams p)
 {
     extern __shared__ double emis_sm[];
     double* dr = emis_sm;                 // [nlev] R_{i+1} - R_i
     double* dr3 = dr + p.nlev;            // [nlev] (R_{i+1}^3 - R_i^3) / 3
-    double* col_tot = dr3 + p.nlev;       // [32]
     const int lane = lane_id(), wid = threadIdx.x >> 5;
     for (int i = threadIdx.x; i < p.nlev; i += blockDim.x) {
         const double r0 = p.r_edges[i], r1 = p.r_edges[i + 1];
@@ -433,7 +478,7 @@ __global__ void __launch_bounds__(kEmisThreads) emis_cdf_kernel(const EmisParams
     }
     __syncthreads();
     const int ncol = p.nlat * p.nlon;
-    for (int c = blockIdx.x; c < p.n_chan; c += gridDim.x) {
+    for (int c = blockIdx.y; c < p.n_chan; c += gridDim.y) {
         const double lam = p.lambda[c];
         const double hck = 6.62607015e-34 * 299792458.0 / (lam * 1.380649e-23);                     // h c / (lambda k)
         const double pre = 4.0 * 3.14159265358979323846 * 2.0 * 6.62607015e-34 * 299792458.0 * 299792458.0 /
@@ -441,14 +486,11 @@ __global__ void __launch_bounds__(kEmisThreads) emis_cdf_kernel(const EmisParams
         const float* alpha_c = p.alpha + (size_t)c * p.alpha_stride;
         const float4* prop_c = p.prop + (size_t)c * p.ncell;
         double* out = p.Lcum + (size_t)c * p.ncell;
-        double carry = 0.0;
-        for (int col0 = 0; col0 < ncol; col0 += 32) {
-            const int col = min(col0 + wid, ncol - 1);       // surplus warps of the last round redo its last column
-            const bool live = col0 + wid < ncol;
+        for (int col = blockIdx.x * (kEmisThreads / 32) + wid; col < ncol; col += gridDim.x * (kEmisThreads / 32)) {
             const size_t cell0 = (size_t)col * p.nlev;
             const float* acol = alpha_c + (size_t)col * p.col_stride + 1;
             float a[NCH], T[NCH], rk[NCH];
-#pragma unroll
+    #pragma unroll
             for (int m = 0; m < NCH; ++m) {                  // level i = 32 m + lane
                 const int i = (m << 5) + lane;
                 const bool in = i < p.nlev;
@@ -460,15 +502,15 @@ __global__ void __launch_bounds__(kEmisThreads) emis_cdf_kernel(const EmisParams
             // suffix sums from the top = column total - inclusive prefix from below
             int i_cut = 0;   // lowest level kept
             if (p.tau_vert_max > 0.0) {
-                double d[NCH], incl[NCH], tot = 0.0;
-#pragma unroll
+                double incl[NCH], tot = 0.0;
+    #pragma unroll
                 for (int m = 0; m < NCH; ++m) {
                     const int i = (m << 5) + lane;
-                    d[m] = i < p.nlev ? double(a[m]) * dr[i] : 0.0;
-                    incl[m] = tot + warp_incl_scan_f64(d[m]);
+                    const double d = i < p.nlev ? double(a[m]) * dr[i] : 0.0;
+                    incl[m] = tot + warp_incl_scan_f64(d);
                     tot = __shfl_sync(kFullMask, incl[m], 31);
                 }
-#pragma unroll
+    #pragma unroll
                 for (int m = 0; m < NCH; ++m) {
                     const int i = (m << 5) + lane;
                     const unsigned mc = __ballot_sync(kFullMask, i < p.nlev && (tot - incl[m]) > p.tau_vert_max);
@@ -477,35 +519,50 @@ __global__ void __launch_bounds__(kEmisThreads) emis_cdf_kernel(const EmisParams
             }
             const int j = col % p.nlat, k = col / p.nlat;
             const double ang = (p.cth_edges[j] - p.cth_edges[j + 1]) * (p.ph_edges[k + 1] - p.ph_edges[k]);
-            double loc[NCH], run = 0.0;
-#pragma unroll
+            double run = 0.0;
+    #pragma unroll
             for (int m = 0; m < NCH; ++m) {
                 const int i = (m << 5) + lane;
-                double L = 0.0;
-                if (i < p.nlev && i >= i_cut) L = pre * dr3[i] * ang * double(rk[m]) / expm1(hck / double(T[m]));
-                if (p.Lcell && live && i < p.nlev) p.Lcell[(size_t)c * p.ncell + cell0 + i] = L;
-                loc[m] = run + warp_incl_scan_f64(L);
-                run = __shfl_sync(kFullMask, loc[m], 31);
-            }
-            if (lane == 0) col_tot[wid] = live ? run : 0.0;
-            __syncthreads();
-            double excl = 0.0, tile = 0.0;
-            for (int w = 0; w < 32; ++w) {   // the same chain in every thread
-                if (w == wid) excl = tile;
-                tile += col_tot[w];
-            }
-            if (live) {
-#pragma unroll
-                for (int m = 0; m < NCH; ++m) {
-                    const int i = (m << 5) + lane;
-                    if (i < p.nlev) out[cell0 + i] = carry + (excl + loc[m]);
+                double Li = 0.0, sum = run;
+                if ((m << 5) + 32 > i_cut && (m << 5) < p.nlev) {   // warp-uniform: a chunk wholly below the cut holds no luminosity
+                    if (i < p.nlev && i >= i_cut) {
+                    const double e = expm1(hck * rcp_pos_f64(double(T[m])));     // +inf in the far Wien tail: L_i = 0
+                    Li = e < 1e300 ? pre * dr3[i] * ang * double(rk[m]) * rcp_pos_f64(e) : 0.0;
+                }
+                    sum = run + warp_incl_scan_f64(Li);
+                    run = __shfl_sync(kFullMask, sum, 31);
+                }
+                if (i < p.nlev) {
+                    if (p.Lcell) p.Lcell[(size_t)c * p.ncell + cell0 + i] = Li;
+                    out[cell0 + i] = sum;
                 }
             }
-            carry += tile;
-            __syncthreads();
+            if (lane == 0) p.Lcol[(size_t)c * ncol + col] = run;
         }
-        if (threadIdx.x == 0) p.Ltot[c] = carry;
     }
+}
+
+// Column offsets of the two-level CDF: one warp per channel turns the column totals emis_col_kernel left in Lcol into
+// the sums of the columns before each (in place) and writes the channel's total.  The totals are added one by one in
+// column order -- every lane runs the same chain over the 32 totals of a chunk -- so that
+// Lcol[col + 1] == fl(Lcol[col] + total(col)) exactly, which is what keeps emis_cum() monotonic across columns.
+__global__ void __launch_bounds__(128) emis_colscan_kernel(int n_chan, int ncol, double* __restrict__ Lcol, double* __restrict__ Ltot)
+{
+    const int c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = lane_id();
+    if (c >= n_chan) return;
+    double* col = Lcol + (size_t)c * ncol;
+    double carry = 0.0;
+    for (int col0 = 0; col0 < ncol; col0 += 32) {
+        const double v = col0 + lane < ncol ? col[col0 + lane] : 0.0;
+        double excl = 0.0;
+#pragma unroll
+        for (int w = 0; w < 32; ++w) {
+            if (w == lane) excl = carry;
+            carry += __shfl_sync(kFullMask, v, w);
+        }
+        if (col0 + lane < ncol) col[col0 + lane] = excl;
+    }
+    if (lane == 0) Ltot[c] = carry;
 }
 
 // Guide table of the emission CDF: guide[c][g] = first cell whose running luminosity exceeds (g / kEmisGuide) L_tot.
@@ -514,20 +571,15 @@ __global__ void __launch_bounds__(kEmisThreads) emis_cdf_kernel(const EmisParams
 // the same cell as the full search (the bracket contains it by monotonicity of frac -> frac * L_tot in fp64).
 constexpr int kEmisGuide = 4096;
 
-__global__ void __launch_bounds__(256) emis_guide_kernel(int n_chan, int ncell, const double* __restrict__ Lcum,
-                                                         const double* __restrict__ Ltot, int* __restrict__ guide)
+__global__ void __launch_bounds__(256) emis_guide_kernel(int n_chan, int ncell, int nlev, const double* __restrict__ Lcum,
+                                                         const double* __restrict__ Lcol, const double* __restrict__ Ltot,
+                                                         int* __restrict__ guide)
 {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= (long long)n_chan * kEmisGuide) return;
     const int c = int(t / kEmisGuide), gi = int(t % kEmisGuide);
-    const double* cum = Lcum + (size_t)c * ncell;
     const double x = double(gi) / double(kEmisGuide) * Ltot[c];
-    int lo = 0, hi = ncell - 1;
-    while (lo < hi) {
-        const int mid = (lo + hi) >> 1;
-        if (cum[mid] > x) hi = mid; else lo = mid + 1;
-    }
-    guide[t] = lo;
+    guide[t] = emis_search(Lcum + (size_t)c * ncell, Lcol + (size_t)c * (ncell / nlev), Ltot[c], nlev, ncell / nlev, 0, ncell - 1, x);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -910,12 +962,7 @@ transport_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const S
                                         cell = min(int(floor(double(z.z0) / rc.xi * ncell)), ncell - 1);
                                     } else {
                                         const double x = (double(z.z0) - rc.xi) / (1.0 - rc.xi) * Ltot;
-                                        int lo = 0, hi = ncell - 1;
-                                        while (lo < hi) {
-                                            const int mid = (lo + hi) >> 1;
-                                            if (cum[mid] > x) hi = mid; else lo = mid + 1;
-                                        }
-                                        cell = lo;
+                                        cell = emis_search(cum, rc.Lcol + (size_t)ctab * (ncell / gs.nlev), Ltot, gs.nlev, ncell / gs.nlev, 0, ncell - 1, x);
                                     }
                                     if (st == LS_EV_EMIT) {
                                         float W = 1.0f;

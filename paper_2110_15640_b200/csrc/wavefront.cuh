@@ -359,7 +359,7 @@ wave_first_flight_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
 }
 
 // emission: generation 0 = the emission points (O4).  Eq. 13 with the composite bias xi (C10).
-__global__ void __launch_bounds__(kWaveThreads) wave_emit_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
+__global__ void __launch_bounds__(kWaveThreads, 5) wave_emit_kernel(const __grid_constant__ RunConst rc, const EventBuf ev,
                                                                 const SuspPair susp2, const WaveConst wc)
 {
     extern __shared__ float smem_f[];
@@ -392,12 +392,8 @@ __global__ void __launch_bounds__(kWaveThreads) wave_emit_kernel(const __grid_co
                     const double x = frac * Ltot;
                     const int gi = min(int(frac * double(kEmisGuide)), kEmisGuide - 1);
                     const int* gd = rc.guide + (size_t)ctab * kEmisGuide;
-                    int lo = __ldg(gd + gi), hi = gi + 1 < kEmisGuide ? __ldg(gd + gi + 1) : ncell - 1;
-                    while (lo < hi) {
-                        const int mid = (lo + hi) >> 1;
-                        if (cum[mid] > x) hi = mid; else lo = mid + 1;
-                    }
-                    cell = lo;
+                    const int lo = __ldg(gd + gi), hi = gi + 1 < kEmisGuide ? __ldg(gd + gi + 1) : ncell - 1;
+                    cell = emis_search(cum, rc.Lcol + (size_t)ctab * (gs.nlat * gs.nlon), Ltot, gs.nlev, gs.nlat * gs.nlon, lo, hi, x);
                 }
                 if (rc.xi > 0.0) {
                     const double Li = rc.Lcell[(size_t)ctab * ncell + cell];

@@ -48,8 +48,9 @@ UNIT = "events/s"
 #   peel ray = record read, phase function, ray set-up (ray_init), round control, exp, bin accumulation
 I_UNITS = {            # workload: (per peel segment, per peel ray)
     "cfg2": (28.9, 450.0),
-    "cfg3": (41.2, 300.0),     # ~9 segments per ray (rays toward 8 phases; those that end on the lower boundary are not marched):
-                               # entry / exit weighs more; the record and the phase-function inputs serve 8 rays
+    "cfg3": (37.3, 292.0),     # ~9 segments per ray (rays toward 8 phases; those that end on the lower boundary are not marched,
+                               # and half of the rays are not even set up): entry / exit weighs more; the record and the
+                               # phase-function inputs serve 8 rays
     "cfg4": (28.4, 450.0),
 }
 I_SEG_1D = 23.0      # nlat = nlon = 1: loop + entry / exit, no lateral crossings
@@ -59,7 +60,7 @@ I_EVENT = 1000.0     # per event on the transport side: Philox block, absorb / s
 # dram__bytes_read.sum + dram__bytes_write.sum per peel_kernel launch at the default sizes, from ncu --set full captures
 PEEL_DRAM_BYTES_PER_LAUNCH = {
     "cfg2": (7.955e9, "profiles/ncu_full_r02_cfg2.txt: 4 launches of a step, ~94 M events each"),
-    "cfg3": (11.907e9, "profiles/ncu_full_r02_cfg3.txt: 6 launches of a step, ~1e8 events x 8 observers each"),
+    "cfg3": (11.941e9, "profiles/ncu_full_r02_cfg3.txt: 6 launches of a step, ~1e8 events x 8 observers each"),
     "cfg4": (3.643e9, "profiles/ncu_full_r02_cfg4.txt: 2000 wavelengths, ~5e7 events per launch"),
 }
 

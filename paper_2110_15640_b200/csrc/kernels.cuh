@@ -1177,7 +1177,7 @@ __device__ __forceinline__ void peel_flush_bins(const RunConst& rc, float* bins,
 
 constexpr int kPeelChunk = 128;   // consecutive sorted events a warp takes per atomic (4 rounds of 32)
 
-template <int KSTEPS>
+template <int KSTEPS, bool HORIZON>
 __global__ void __launch_bounds__(kPeelThreads, 4)
 peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsigned int* __restrict__ perm)
 {
@@ -1261,13 +1261,26 @@ peel_kernel(const __grid_constant__ RunConst rc, const EventBuf ev, const unsign
                 float tau = 0.f;
                 int st = RAY_NONE;      // lane state = ray status: RAY_FLYING marches, RAY_PARK waits for ray_lateral
                 unsigned int seg32 = 0;
-                if (have && pref > 0.0f) {
-                    ray_init(ray, gs, a.x, a.y, a.z, ox, oy, oz, ci, cj, ck, alpha_c);
-                    // a ray that descends and does not turn inside the grid ends on the lower boundary: nothing of it
-                    // reaches the observer (Eq. 14 along a ray that leaves through the top), so it is not marched at all
-                    // -- with observers all around the orbit these are the long rays through the deep atmosphere
-                    st = (ray.rad_step < 0 && ray.i_turn < 0) ? RAY_SURFACE : RAY_FLYING;
-                    ++c_rays;
+                // a ray that descends and does not turn inside the grid ends on the lower boundary: nothing of it reaches
+                // the observer (Eq. 14 along a ray that leaves through the top), so it is not marched at all -- with
+                // observers all around the orbit these are the long rays through the deep atmosphere.  Most of them point
+                // well below the horizon of the lower boundary (impact parameter d < R_0 by more than any rounding of this
+                // fp32 estimate: r^2 ~ 1e16 m^2 carries ~1e9, the margin is 1e-4 R_0^2); the lanes of a warp share a cell and
+                // an observer, so a warp of such rays does not even set them up.  Every other ray is decided by the march's
+                // own double-float expression.
+                const bool go = have && pref > 0.0f;
+                bool below = false;
+                if (HORIZON) {
+                    const float b0 = fmaf(a.x, ox, fmaf(a.y, oy, a.z * oz));
+                    const float dq = fmaf(-b0, b0, fmaf(a.x, a.x, fmaf(a.y, a.y, a.z * a.z)));
+                    below = b0 < 0.0f && dq < rc.geom.R0 * rc.geom.R0 * (1.0f - 1e-4f);
+                }
+                if (go) { ++c_rays; st = RAY_SURFACE; }
+                if (!HORIZON || __any_sync(kFullMask, go && !below)) {
+                    if (go) {
+                        ray_init(ray, gs, a.x, a.y, a.z, ox, oy, oz, ci, cj, ck, alpha_c);
+                        st = (ray.rad_step < 0 && ray.i_turn < 0) ? RAY_SURFACE : RAY_FLYING;
+                    }
                 }
                 // all lanes start together, so one warp-uniform step budget guards against a ray that never ends
                 for (int it = 0; it <= rc.geom.maxseg; it += KSTEPS) {

@@ -265,8 +265,13 @@ class Leg:
                 self.dev[k] = torch.from_numpy(np.ascontiguousarray(opac[k], dtype=np.float32)).cuda()
         self.G = binding.Grid(grid, stream=stream)
         self.ncell = int(np.asarray(grid["T"]).size)
+        self.G2 = self.stream2 = None
         if self.streamed:
             self.coef = torch.from_numpy(opac["k_ray_chan"]).cuda()
+            # double-buffered: a second handle on a second stream takes every other wavelength
+            # batch, so that batch b + 1's node tables, staging and CDF overlap batch b's transport
+            self.stream2 = torch.cuda.Stream()
+            self.G2 = binding.Grid(grid, stream=self.stream2)
 
     def pin_host_tables(self):
         self.host = dict(self.opac)
@@ -290,17 +295,24 @@ class Leg:
         # emission and in albedo mode toward the 4 phases
         outs = []
         obs = np.asarray(prm["obs_dir"], dtype=np.float64).reshape(-1, 3)
-        for c0, c1, lo, hi in wl.cfg5_batches(self.opac, batch=self.args.batch, halo=int(prm["doppler_halfwidth"])):
-            sub = dict(op, chan0=op["chan0"] + lo, node_kabs=op["node_kabs"][lo:hi])
-            sub["lambda"] = self.opac["lambda"][lo:hi]
-            sub["k_sca_ray"] = self.coef[lo:hi, None].expand(hi - lo, self.ncell).contiguous()
-            G.set_opacity_nodes(sub)
-            # with doppler_on every observer is a run of its own on its own shifted table (L326-328): phases outermost,
-            # so that the emission and the albedo run toward a phase share one Doppler staging (4 per batch, not 8)
-            for o in range(obs.shape[0]):
-                for fn in (G.run_emission, G.run_albedo):
-                    outs.append(fn(dict(prm, obs_dir=obs[o:o + 1], chan_begin=c0 - lo, chan_end=c1 - lo),
-                                   device_outputs=device_outputs, counters=counters))
+        two = not timing          # the timing = 1 steps wait for the device after every kernel: one handle
+        if two:
+            self.stream2.wait_stream(self.stream)
+        for b, (c0, c1, lo, hi) in enumerate(wl.cfg5_batches(self.opac, batch=self.args.batch, halo=int(prm["doppler_halfwidth"]))):
+            G, st = (self.G2, self.stream2) if two and b % 2 else (self.G, self.stream)
+            with self.torch.cuda.stream(st):     # the batch's Rayleigh table is filled on the stream its handle runs on
+                sub = dict(op, chan0=op["chan0"] + lo, node_kabs=op["node_kabs"][lo:hi])
+                sub["lambda"] = self.opac["lambda"][lo:hi]
+                sub["k_sca_ray"] = self.coef[lo:hi, None].expand(hi - lo, self.ncell).contiguous()
+                G.set_opacity_nodes(sub)
+                # with doppler_on every observer is a run of its own on its own shifted table (L326-328): phases outermost,
+                # so that the emission and the albedo run toward a phase share one Doppler staging (4 per batch, not 8)
+                for o in range(obs.shape[0]):
+                    for fn in (G.run_emission, G.run_albedo):
+                        outs.append(fn(dict(prm, obs_dir=obs[o:o + 1], chan_begin=c0 - lo, chan_end=c1 - lo),
+                                       device_outputs=device_outputs, counters=counters))
+        if two:
+            self.stream.wait_stream(self.stream2)
         return outs
 
     def sum_counters(self, outs):
@@ -370,6 +382,8 @@ class Leg:
 
     def close(self):
         self.G.close()
+        if self.G2 is not None:
+            self.G2.close()
 
 
 def run_ours(args):

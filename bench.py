@@ -284,7 +284,9 @@ class Leg:
 
     def step(self, op, device_outputs, timing=0, counters="host"):
         """One pass of the whole hot path over the workload; returns the list of run results."""
-        prm = dict(self.prm, timing=timing)
+        # run_params.concurrency: the run's channels in K parts side by side on internal handles and streams (ignored by the
+        # library for timing = 1 and Doppler runs)
+        prm = dict(self.prm, timing=timing, concurrency=0 if timing else self.args.concurrency)
         G = self.G
         if not self.streamed:
             G.set_opacity(op)
@@ -442,6 +444,8 @@ def run_ours(args):
                 "config": {"workload": args.workload, "mode": leg.mode, "n_chan_per_gpu": leg.n_chan, "packets_per_channel": N,
                            "n_obs": int(np.asarray(leg.prm["obs_dir"]).reshape(-1, 3).shape[0]),
                            "grid": list(np.asarray(leg.grid["T"]).shape), "parallelism": "channels x %d" % world,
+                           "concurrency": ("2 handles, alternating wavelength batches" if leg.streamed else
+                                           "run_params.concurrency = %d (channel parts side by side on one GPU)" % args.concurrency),
                            "l2": "opacity tables (%.0f MB) + staged tables exceed the 126 MB L2; no flush" % (h2d / 1e6)},
                 "events_per_step": ev_all / args.steps, "segments_per_s": seg_all / (ms * 1e-3),
                 "spectra_per_s": world * args.steps / (ms * 1e-3),
@@ -475,7 +479,7 @@ def run_ours(args):
                         "config": {"workload": lg.name, "mode": lg.mode, "n_chan_per_gpu": lg.n_chan,
                                    "packets_per_channel": int(lg.prm["packets_per_channel"]),
                                    "n_obs": int(np.asarray(lg.prm["obs_dir"]).reshape(-1, 3).shape[0]),
-                                   "grid": list(np.asarray(lg.grid["T"]).shape)},
+                                   "grid": list(np.asarray(lg.grid["T"]).shape), "concurrency": args.concurrency},
                         "rays_per_s": acc_x["rays_peel"] / (ms_x * 1e-3),
                         "counters_per_step": {k: acc_x[k] / 3 for k in ("events", "segments_transport", "segments_peel", "rays_peel", "passes")},
                         "roofline": lg.roofline(acc_xt, ms_xt, 2, pk)}
@@ -511,6 +515,7 @@ def main():
     ap.add_argument("--channels", type=int, default=None, help="cfg4 / cfg5: number of wavelength points (default 10000 / 4096)")
     ap.add_argument("--batch", type=int, default=1024, help="cfg5: wavelength points per streamed opacity batch")
     ap.add_argument("--packets", type=int, default=None, help="override packets per channel (debugging only)")
+    ap.add_argument("--concurrency", type=int, default=3, help="run_params.concurrency of the timed steps (0 = one run per call)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline legs")
     ap.add_argument("--no-extra", action="store_true", help="skip the cfg3 / cfg4 legs of the default run")
     args = ap.parse_args()

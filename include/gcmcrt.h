@@ -132,6 +132,17 @@ typedef struct gcmcrt_run_params {
     int timing;                  /* 0: the run is only enqueued (see STREAMS); the ms_* counters stay 0.
                                     1: profiling run -- the pass loop is driven by the host, which waits for every pass
                                     and records cudaEvents around its kernels to fill the ms_* counters */
+    int concurrency;             /* K = 2 .. 8: the channels of the run (independent, L79) are cut into K contiguous parts that
+                                    run side by side -- part 0 on this handle and the caller's stream, the others on internal
+                                    copies of the grid handle with working buffers of their own (they borrow this handle's
+                                    opacity tables) and internal streams that fork from the caller's stream and join it before
+                                    the call's results are complete -- so that the kernels of one part use the issue slots and
+                                    memory latencies another leaves idle.  Same results (packets are keyed by channel and
+                                    index); counters are summed over the parts.  The internal handles are created by the
+                                    first such call, which waits for the device; working memory grows K-fold.  0 or 1, and
+                                    whenever it does not apply (timing = 1, doppler_on, node-table opacities, transmission,
+                                    fewer than K channels in the run, a stream that is being captured, GCMCRT_HOST_LOOP):
+                                    one run on this handle. */
 } gcmcrt_run_params;
 
 typedef struct gcmcrt_counters {

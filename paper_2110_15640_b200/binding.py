@@ -35,7 +35,7 @@ class RunParams(C.Structure):
                 ("tau_cut", C.c_double), ("npix", C.c_int), ("n_batches", C.c_int),
                 ("survival_bias", C.c_int), ("roulette_w_min", C.c_double), ("roulette_survive", C.c_double),
                 ("star_radius", C.c_double), ("planet_xy", C.c_double * 2), ("ld_c1", C.c_double), ("ld_c2", C.c_double), ("cloud_phase", C.c_int), ("forced_scatter", C.c_int), ("continuous_absorption", C.c_int),
-                ("star_solid_angle", C.c_double), ("stretch_alpha", C.c_double), ("timing", C.c_int)]
+                ("star_solid_angle", C.c_double), ("stretch_alpha", C.c_double), ("timing", C.c_int), ("concurrency", C.c_int)]
 
 
 class Counters(C.Structure):
@@ -187,6 +187,7 @@ def make_params(prm):
     p.star_solid_angle = float(prm.get("star_solid_angle", 0.0))
     p.stretch_alpha = float(prm.get("stretch_alpha", 0.0))
     p.timing = int(prm.get("timing", 0))
+    p.concurrency = int(prm.get("concurrency", 0))
     return p, obs
 
 

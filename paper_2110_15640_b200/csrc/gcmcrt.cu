@@ -91,6 +91,16 @@ struct gcmcrt_grid {
     unsigned long long launches = 0, launches_pending = 0;
     double ms_stage = 0.0, ms_emis = 0.0, ms_transport = 0.0, ms_peel = 0.0, ms_sort = 0.0;
     double ms_stage_pending = 0.0;   // staging done by set_opacity, reported by the next run
+
+    // run_params.concurrency: internal handles (grid copies with working buffers of their own) and the streams their parts of
+    // a run are enqueued on; the opacity tables they borrow from this handle follow opacity_epoch
+    std::vector<gcmcrt_grid*> peers;
+    std::vector<cudaStream_t> peer_streams;
+    std::vector<cudaEvent_t> peer_done;
+    cudaEvent_t fork_ev = nullptr;
+    DevBuf part_counters;
+    unsigned long long opacity_epoch = 0, synced_epoch = 0;   // synced_epoch: on an internal handle, the owner's epoch its tables are from
+    bool is_peer = false;
 };
 
 namespace {
@@ -951,6 +961,150 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     return GCMCRT_OK;
 }
 
+__global__ void sum_counters_kernel(const gcmcrt_counters* part, int k, gcmcrt_counters* out)
+{
+    gcmcrt_counters a = part[0];
+    for (int q = 1; q < k; ++q) {
+        const gcmcrt_counters b = part[q];
+        a.events += b.events; a.segments_transport += b.segments_transport; a.segments_peel += b.segments_peel;
+        a.packets_escaped += b.packets_escaped; a.packets_absorbed += b.packets_absorbed; a.packets_surface += b.packets_surface;
+        a.packets_stuck += b.packets_stuck; a.escaped_weight += b.escaped_weight; a.passes += b.passes; a.rays_peel += b.rays_peel;
+        a.launches += b.launches; a.ms_stage += b.ms_stage; a.ms_emission_cdf += b.ms_emission_cdf;
+        a.ms_transport += b.ms_transport; a.ms_peel += b.ms_peel; a.ms_sort += b.ms_sort;
+        a.device_status = a.device_status ? a.device_status : b.device_status;
+    }
+    *out = a;
+}
+
+// run_params.concurrency = K > 1 (L79: the channels of a run are independent): the run's channels are cut into K
+// contiguous parts; part 0 runs on this handle and the caller's stream, the others on internal handles -- copies of the
+// grid with working buffers of their own, which borrow this handle's opacity tables -- and internal streams that fork
+// from the caller's stream and join it again.  Every part is an ordinary run_mode() call with device outputs that point
+// into the whole run's arrays, so the parts are only enqueued; what the caller wants in host memory is copied back after
+// the join.  The kernels of one part fill the issue slots and the memory latencies another leaves idle.
+bool split_eligible(gcmcrt_grid* g, const gcmcrt_run_params* prm, const gcmcrt_result* out, cudaStream_t s, int mode)
+{
+    if (!g || !prm || !out || g->is_peer || prm->concurrency < 2 || prm->concurrency > 8) return false;
+    if (mode == 2 || prm->timing || prm->doppler_on || g->use_nodes || g->n_chan <= 0 || g->staged_obs == -2) return false;
+    static const bool host_loop_env = std::getenv("GCMCRT_HOST_LOOP") && std::atoi(std::getenv("GCMCRT_HOST_LOOP")) != 0;
+    if (host_loop_env) return false;
+    const int cb = prm->chan_begin, ce = prm->chan_end ? prm->chan_end : g->n_chan;
+    if (cb < 0 || ce > g->n_chan || ce - cb < prm->concurrency) return false;
+    const unsigned long long N = prm->packets_per_channel, lo = prm->pkt_begin, hi = prm->pkt_end ? prm->pkt_end : N;
+    if (N == 0 || N > 0xffffffffull || lo > hi || hi > N) return false;       // run_mode() reports it
+    if (prm->n_obs < 0 || prm->n_obs > kMaxObs || (prm->n_obs > 0 && !out->flux_sum)) return false;
+    const int nb = prm->n_batches ? prm->n_batches : 32;
+    if (nb < 1 || nb > kMaxBatches) return false;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(s, &cs) != cudaSuccess) { cudaGetLastError(); return false; }
+    return cs == cudaStreamCaptureStatusNone;
+}
+
+int run_split(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, void* stream, int mode)
+{
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const int K = prm->concurrency;
+    const int n_obs = prm->n_obs, nobs1 = std::max(n_obs, 1);
+    const unsigned long long N = prm->packets_per_channel, lo = prm->pkt_begin, hi = prm->pkt_end ? prm->pkt_end : N;
+    const int cb = prm->chan_begin, ce = prm->chan_end ? prm->chan_end : g->n_chan, ncr = ce - cb;
+    const int nb = prm->n_batches ? prm->n_batches : 32;
+    const int npix = prm->npix > 0 && out->image ? prm->npix : 0;
+    const size_t n_pkt = size_t(hi - lo);
+    int rcode;
+    // ---- internal handles and their streams (created once: the first call of this kind waits for the device)
+    while (int(g->peers.size()) < K - 1) {
+        gcmcrt_grid* p = nullptr;
+        rcode = gcmcrt_grid_create(&p, g->nlev, g->nlat, g->nlon, g->r.data(), g->th.data(), g->ph.data(), g->T.as<float>(),
+                                   g->rho.as<float>(), g->u.p ? g->u.as<float>() : nullptr, g->v.p ? g->v.as<float>() : nullptr,
+                                   g->w.p ? g->w.as<float>() : nullptr, g->Omega, g->surface_albedo, s);
+        if (rcode) return fail(g, rcode, "concurrency: " + g_create_error);
+        p->is_peer = true;
+        cudaStream_t ps = nullptr;
+        cudaEvent_t pe = nullptr;
+        cudaError_t e = cudaStreamCreateWithFlags(&ps, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&pe, cudaEventDisableTiming);
+        if (e != cudaSuccess) { gcmcrt_destroy(p); if (ps) cudaStreamDestroy(ps); cudaGetLastError(); return fail(g, GCMCRT_E_CUDA, "concurrency: stream"); }
+        g->peers.push_back(p); g->peer_streams.push_back(ps); g->peer_done.push_back(pe);
+    }
+    if (!g->fork_ev) CUDA_TRY(g, cudaEventCreateWithFlags(&g->fork_ev, cudaEventDisableTiming));
+    CUDA_TRY(g, g->part_counters.ensure(size_t(K) * sizeof(gcmcrt_counters)));
+    // ---- outputs of the whole run, bound once (host-resident ones are staged on this handle)
+    OutBuf o_flux, o_ltot, o_val, o_sig, o_img, o_evc, o_ctb, o_cnt;
+    if ((rcode = bind_out(g, out->flux_sum, size_t(ncr) * nobs1 * nb * sizeof(double), g->flux, o_flux))) return rcode;
+    if ((rcode = bind_out(g, out->L_tot, size_t(ncr) * nobs1 * sizeof(double), g->ltot_out, o_ltot))) return rcode;
+    if ((rcode = bind_out(g, out->value, size_t(ncr) * nobs1 * sizeof(double), g->value, o_val))) return rcode;
+    if ((rcode = bind_out(g, out->sigma, size_t(ncr) * nobs1 * sizeof(double), g->sigma, o_sig))) return rcode;
+    if (npix) if ((rcode = bind_out(g, out->image, size_t(ncr) * n_obs * npix * npix * sizeof(float), g->image, o_img))) return rcode;
+    if (out->event_count) if ((rcode = bind_out(g, out->event_count, size_t(ncr) * n_pkt * sizeof(uint32_t), g->evcount, o_evc))) return rcode;
+    if (out->contrib && n_obs > 0) if ((rcode = bind_out(g, out->contrib, size_t(ncr) * n_obs * 2 * g->ncell * sizeof(float), g->contrib, o_ctb))) return rcode;
+    if (out->counters) if ((rcode = bind_out(g, out->counters, sizeof(gcmcrt_counters), g->counters_out, o_cnt))) return rcode;
+    // ---- fork: the internal streams wait for everything enqueued on the caller's stream (its table copies included)
+    CUDA_TRY(g, cudaEventRecord(g->fork_ev, s));
+    for (int q = 1; q < K; ++q) CUDA_TRY(g, cudaStreamWaitEvent(g->peer_streams[q - 1], g->fork_ev, 0));
+    for (int q = 1; q < K; ++q) {
+        gcmcrt_grid* p = g->peers[q - 1];
+        if (p->synced_epoch == g->opacity_epoch) continue;
+        rcode = gcmcrt_set_opacity(p, g->chan0, g->n_chan, g->lambda.data(), g->k_abs, g->k_ray, g->k_cld, g->g_cld, g->peer_streams[q - 1]);
+        if (rcode) return fail(g, rcode, "concurrency: " + p->err);
+        p->synced_epoch = g->opacity_epoch;   // (of the handle it borrows from)
+    }
+    // ---- the parts
+    int first_err = GCMCRT_OK;
+    for (int q = 0; q < K && first_err == GCMCRT_OK; ++q) {
+        const int c0 = cb + int((long long)ncr * q / K), c1 = cb + int((long long)ncr * (q + 1) / K);
+        const size_t oc = size_t(c0 - cb);
+        gcmcrt_run_params pq = *prm;
+        pq.chan_begin = c0; pq.chan_end = c1; pq.concurrency = 0;
+        gcmcrt_result rq;
+        std::memset(&rq, 0, sizeof rq);
+        rq.flux_sum = static_cast<double*>(o_flux.dev) + oc * nobs1 * nb;
+        rq.L_tot = static_cast<double*>(o_ltot.dev) + oc * nobs1;
+        rq.value = static_cast<double*>(o_val.dev) + oc * nobs1;
+        rq.sigma = static_cast<double*>(o_sig.dev) + oc * nobs1;
+        rq.image = npix ? static_cast<float*>(o_img.dev) + oc * n_obs * npix * npix : nullptr;
+        rq.event_count = o_evc.dev ? static_cast<uint32_t*>(o_evc.dev) + oc * n_pkt : nullptr;
+        rq.contrib = o_ctb.dev ? static_cast<float*>(o_ctb.dev) + oc * n_obs * 2 * g->ncell : nullptr;
+        rq.counters = g->part_counters.as<gcmcrt_counters>() + q;
+        gcmcrt_grid* h = q == 0 ? g : g->peers[q - 1];
+        rcode = run_mode(h, &pq, &rq, q == 0 ? s : g->peer_streams[q - 1], mode);
+        if (rcode) { first_err = rcode; if (h != g) g->err = "concurrency: " + h->err; }
+    }
+    // ---- join (also after a failed part: nothing may be left running behind the caller's back)
+    for (int q = 1; q < K; ++q) {
+        CUDA_TRY(g, cudaEventRecord(g->peer_done[q - 1], g->peer_streams[q - 1]));
+        CUDA_TRY(g, cudaStreamWaitEvent(s, g->peer_done[q - 1], 0));
+    }
+    if (first_err) return first_err;
+    if (o_cnt.dev) {
+        sum_counters_kernel<<<1, 1, 0, s>>>(g->part_counters.as<gcmcrt_counters>(), K, static_cast<gcmcrt_counters*>(o_cnt.dev));
+        CUDA_TRY(g, cudaGetLastError());
+    }
+    bool need_sync = false;
+    for (OutBuf* ob : {&o_flux, &o_ltot, &o_val, &o_sig, &o_img, &o_evc, &o_ctb, &o_cnt}) {
+        if (ob->host && ob->dev && ob->bytes) {
+            CUDA_TRY(g, cudaMemcpyAsync(ob->host, ob->dev, ob->bytes, cudaMemcpyDeviceToHost, s));
+            need_sync = true;
+        }
+    }
+    if (need_sync) {
+        CUDA_TRY(g, cudaStreamSynchronize(s));
+        reap_retired_loops(g);
+        for (gcmcrt_grid* p : g->peers) reap_retired_loops(p);
+    }
+    if (o_cnt.host) {
+        const unsigned long long st = static_cast<const gcmcrt_counters*>(o_cnt.host)->device_status;
+        if (st == 1) return fail(g, GCMCRT_E_CUDA, "suspended-packet list overflow");
+        if (st) return fail(g, GCMCRT_E_CUDA, "pass loop did not terminate");
+    }
+    return GCMCRT_OK;
+}
+
+int run_entry(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, void* stream, int mode)
+{
+    if (split_eligible(g, prm, out, static_cast<cudaStream_t>(stream), mode)) return run_split(g, prm, out, stream, mode);
+    return run_mode(g, prm, out, stream, mode);
+}
+
 }  // namespace
 
 extern "C" {
@@ -1118,6 +1272,7 @@ static int set_opacity_common(gcmcrt_grid* g, int chan0, int n_chan, const float
     CUDA_TRY(g, upload(g->reff, reff, s));
     g->chan0 = chan0;
     g->n_chan = n_chan;
+    ++g->opacity_epoch;
     g->launches = 0;
     g->ms_stage_pending = 0.0;
     // staging (A0 / A1) is left to the first run: a Doppler run needs the table of its own observer, not the unshifted one
@@ -1128,17 +1283,17 @@ static int set_opacity_common(gcmcrt_grid* g, int chan0, int n_chan, const float
 
 int gcmcrt_run_albedo(gcmcrt_grid* g, const gcmcrt_run_params* p, gcmcrt_result* out, void* stream)
 {
-    return run_mode(g, p, out, stream, 0);
+    return run_entry(g, p, out, stream, 0);
 }
 
 int gcmcrt_run_emission(gcmcrt_grid* g, const gcmcrt_run_params* p, gcmcrt_result* out, void* stream)
 {
-    return run_mode(g, p, out, stream, 1);
+    return run_entry(g, p, out, stream, 1);
 }
 
 int gcmcrt_run_transmission(gcmcrt_grid* g, const gcmcrt_run_params* p, gcmcrt_result* out, void* stream)
 {
-    return run_mode(g, p, out, stream, 2);
+    return run_entry(g, p, out, stream, 2);
 }
 
 int gcmcrt_destroy(gcmcrt_grid* g)
@@ -1152,6 +1307,12 @@ int gcmcrt_destroy(gcmcrt_grid* g)
                       &g->s1[0], &g->s1[1], &g->s2[0], &g->s2[1], &g->ctrl, &g->counters, &g->counters_out, &g->flux, &g->ltot_out,
                       &g->value, &g->sigma, &g->image, &g->evcount, &g->contrib})
         b->release();
+    for (gcmcrt_grid* p : g->peers) gcmcrt_destroy(p);
+    g->peers.clear();
+    for (cudaStream_t ps : g->peer_streams) cudaStreamDestroy(ps);
+    for (cudaEvent_t pe : g->peer_done) cudaEventDestroy(pe);
+    if (g->fork_ev) cudaEventDestroy(g->fork_ev);
+    g->part_counters.release();
     if (g->h_ctrl) cudaFreeHost(g->h_ctrl);
     for (auto& lg : g->loops) g->retired.push_back(lg);
     g->loops.clear();

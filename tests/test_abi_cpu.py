@@ -33,12 +33,12 @@ def test_library_exports_every_declared_symbol(lib):
 
 def test_struct_layouts_match_header():
     # gcmcrt_run_params: 3 doubles, int(+pad), ptr, 4 u64, 6 int, 3 doubles, 2 int  (natural alignment)
-    assert C.sizeof(binding.RunParams) == 24 + 8 + 8 + 32 + 24 + 24 + 8 + 24 + 40 + 8 + 8 + 24   # + survival_bias (int + pad), 2 doubles; + 5 doubles (transmission); + cloud_phase, forced_scatter; + continuous_absorption (int + pad); + star_solid_angle, stretch_alpha, timing (int + pad)
+    assert C.sizeof(binding.RunParams) == 24 + 8 + 8 + 32 + 24 + 24 + 8 + 24 + 40 + 8 + 8 + 24   # + survival_bias (int + pad), 2 doubles; + 5 doubles (transmission); + cloud_phase, forced_scatter; + continuous_absorption (int + pad); + star_solid_angle, stretch_alpha, timing + concurrency (2 ints)
     assert binding.RunParams.survival_bias.offset == 128 and binding.RunParams.roulette_survive.offset == 144
     assert binding.RunParams.obs_dir.offset == 32 and binding.RunParams.seed.offset == 64
     assert binding.RunParams.emission_bias.offset == 96 and binding.RunParams.n_batches.offset == 124
     assert C.sizeof(binding.Counters) == 136     # 11 u64/double + 5 ms doubles + device_status
-    assert binding.RunParams.star_solid_angle.offset == binding.RunParams.continuous_absorption.offset + 8 and binding.RunParams.stretch_alpha.offset == binding.RunParams.star_solid_angle.offset + 8 and binding.RunParams.timing.offset == binding.RunParams.stretch_alpha.offset + 8
+    assert binding.RunParams.star_solid_angle.offset == binding.RunParams.continuous_absorption.offset + 8 and binding.RunParams.stretch_alpha.offset == binding.RunParams.star_solid_angle.offset + 8 and binding.RunParams.timing.offset == binding.RunParams.stretch_alpha.offset + 8 and binding.RunParams.concurrency.offset == binding.RunParams.timing.offset + 4
     assert C.sizeof(binding.Result) == 64      # 8 pointers (contrib added with the contribution functions)
 
 

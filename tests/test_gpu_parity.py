@@ -1388,3 +1388,73 @@ def test_pass_loop_drivers_agree_for_emission_and_transmission(gpu, monkeypatch,
         assert torch.allclose(outs["flux_sum"], ref["flux_sum"], rtol=1e-5) and torch.allclose(outs["value"], ref["value"], rtol=1e-5)
         assert gpu.read_counters(cnt)["events"] == ref["counters"]["events"]
         del graph
+
+
+@pytest.mark.parametrize("mode", ["albedo", "emission"])
+def test_concurrent_parts_of_a_run_give_the_same_result(gpu, orc, monkeypatch, mode):
+    """run_params.concurrency = K cuts the channels of a run into K parts that run side by side on internal handles and
+    streams (channels are independent, L79): same packets, event for event, as the single run -- with host and with device
+    outputs, on a sub-range of the channels, with images and contribution functions, after the tables have changed --
+    and still on the oracle's bar.  Where it does not apply (fewer channels than parts, a Doppler run, a stream that is
+    being captured) the call is an ordinary single run."""
+    import torch
+    monkeypatch.setenv("GCMCRT_EVENT_CAP", "80000")     # several passes per part
+    grid, opac = wl.uniform_medium(12, 6, 8, 1.0e7, 1.2e7, [0.5 / 0.2e7, 1.0 / 0.2e7, 1.5 / 0.2e7, 2.5 / 0.2e7, 4.0 / 0.2e7, 0.2 / 0.2e7, 1.0 / 0.2e7],
+                                   0.8, g=0.6, pgas=0.35, n_chan=7, surface_albedo=0.5, T=1500.0)
+    opac["lambda"] = (2.0e-6 * (1 + 1.0e-5 * np.arange(7))).astype(np.float32)
+    ncell = int(grid["T"].size)
+    prm = wl.default_params(packets_per_channel=30000, seed=11, star_dir=[0.8, 0.0, 0.6], obs_dir=[[0.8, 0.0, 0.6], [0.0, 0.0, 1.0]], npix=8)
+    call = "run_albedo" if mode == "albedo" else "run_emission"
+    with gpu.Grid(grid) as G:
+        G.set_opacity(opac)
+        ref = getattr(G, call)(prm, want_event_count=True, want_contrib=ncell)
+        assert ref["counters"]["passes"] > 1
+        for K in (2, 3, 7):
+            r = getattr(G, call)(dict(prm, concurrency=K), want_event_count=True, want_contrib=ncell)
+            assert np.array_equal(r["event_count"], ref["event_count"]), K
+            for k, tol in (("flux_sum", 1e-5), ("value", 1e-6), ("sigma", 1e-4), ("L_tot", 1e-12), ("image", 1e-4), ("contrib", 1e-4)):
+                assert np.allclose(r[k], ref[k], rtol=tol, atol=1e-9 * np.abs(ref[k]).max()), (K, k)
+            for k in ("events", "segments_transport", "segments_peel", "rays_peel", "packets_escaped", "packets_absorbed", "packets_surface"):
+                assert r["counters"][k] == ref["counters"][k], (K, k)
+            assert r["counters"]["passes"] >= K and r["counters"]["device_status"] == 0 and r["counters"]["packets_stuck"] == 0
+        # more parts than channels, or a Doppler run: one ordinary run
+        one = getattr(G, call)(dict(prm, concurrency=8), want_event_count=True)
+        assert one["counters"]["passes"] == ref["counters"]["passes"] and np.array_equal(one["event_count"], ref["event_count"])
+        dop = getattr(G, call)(dict(prm, concurrency=3, doppler_on=1, doppler_halfwidth=1, obs_dir=prm["obs_dir"][:1]), want_event_count=True)
+        dop1 = getattr(G, call)(dict(prm, doppler_on=1, doppler_halfwidth=1, obs_dir=prm["obs_dir"][:1]), want_event_count=True)
+        assert np.array_equal(dop["event_count"], dop1["event_count"]) and dop["counters"]["passes"] == dop1["counters"]["passes"]
+        # a sub-range of the channels; device outputs and device counters (the call only enqueues)
+        sub = getattr(G, call)(dict(prm, concurrency=3, chan_begin=1, chan_end=6), want_event_count=True, device_outputs=True, counters="device")
+        assert np.array_equal(sub["event_count"].cpu().numpy().astype(np.uint32), ref["event_count"][1:6])
+        assert np.allclose(sub["value"].cpu().numpy(), ref["value"][1:6], rtol=1e-6)
+        assert gpu.read_counters(sub["counters_dev"])["events"] == int(ref["event_count"][1:6].sum())
+        # new tables: the internal handles follow
+        opac2 = dict(opac, k_abs=opac["k_abs"] * 2.0)
+        G.set_opacity(opac2)
+        a2 = getattr(G, call)(prm, want_event_count=True)
+        b2 = getattr(G, call)(dict(prm, concurrency=2), want_event_count=True)
+        assert np.array_equal(a2["event_count"], b2["event_count"]) and not np.array_equal(a2["event_count"], ref["event_count"])
+        assert np.allclose(a2["value"], b2["value"], rtol=1e-6)
+        # the oracle's bar
+        fn = orc.run_albedo if mode == "albedo" else orc.run_emission
+        o = fn(grid, opac2, dict(prm, n_threads=16), want_event_count=True)
+        _check_parity(orc, b2, o, mode)
+    # a call captured into a caller's graph is a single run (no internal streams inside a capture)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s), gpu.Grid(grid, stream=s) as G:
+        G.set_opacity(opac)
+        warm = getattr(G, call)(dict(prm, npix=0), want_event_count=True, device_outputs=True)
+        outs = {k: torch.zeros_like(warm[k]) for k in ("flux_sum", "L_tot", "value", "sigma", "event_count")}
+        p, keep = gpu.make_params(dict(prm, npix=0, concurrency=3))
+        res = gpu.Result()
+        res.flux_sum, res.L_tot, res.value, res.sigma = (outs[k].data_ptr() for k in ("flux_sum", "L_tot", "value", "sigma"))
+        res.event_count = outs["event_count"].data_ptr()
+        graph = torch.cuda.CUDAGraph()
+        s.synchronize()
+        with torch.cuda.graph(graph, stream=s, capture_error_mode="relaxed"):
+            rc = getattr(gpu.lib(), "gcmcrt_" + call)(G.handle, gpu.C.byref(p), gpu.C.byref(res), gpu.C.c_void_p(torch.cuda.current_stream().cuda_stream))
+        assert rc == 0, gpu.lib().gcmcrt_last_error(G.handle)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(outs["event_count"], warm["event_count"])
+        del graph

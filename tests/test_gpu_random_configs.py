@@ -3,7 +3,7 @@ varying density, temperature and opacities (log-uniform extinction per cell, sin
 asymmetry varying from cell to cell), random star and observer directions, sub-ranges of packets and channels, and
 every switch of the run parameters drawn at random (event cap, survival biasing + roulette, forced scattering, continuous
 absorption, path-length stretching, the three cloud phase functions, Doppler shifts with winds, composite emission bias,
-depth cut, images, limb darkening, multiple scattering in transmission).  Every case runs in albedo, emission and
+depth cut, images, limb darkening, multiple scattering in transmission, concurrent parts of a run).  Every case runs in albedo, emission and
 transmission mode and is compared with the CPU oracle on the bar of BASELINE.json's north_star: per channel and observer
 |delta| <= 4 sigma_MC + 1e-5 relative, >= 99 % of packets with identical event counts, L_tot within 1e-5.  Each run is
 repeated with run_params.timing = 1 (the host-driven pass loop): same packets, event for event.
@@ -107,6 +107,8 @@ def make_case(seed):
     tr = dict(star_radius=7.0e8, planet_xy=[float(rng.uniform(-3e8, 3e8)), float(rng.uniform(-3e8, 3e8))], ld_c1=0.3, ld_c2=0.2)
     if rng.random() < 0.5:
         tr["star_solid_angle"] = float(10 ** rng.uniform(-4, -2))
+    if rng.random() < 0.4:     # the run's channels in parts side by side (ignored where it does not apply)
+        prm.update(concurrency=int(rng.choice([2, 3])))
     return grid, opac, prm, tr
 
 

@@ -486,10 +486,10 @@ def run_ours(args):
 
             # config 3: the same grid and tables as config 2, so the tables already on the device serve it
             _, _, p3 = wl.cfg3(packets=1000000)
+            leg.close()      # the handle's working buffers (and its internal handles'); the tables in leg.dev stay
             lg = Leg("cfg3", args, binding, torch, stream, rank, leg.grid, leg.opac, p3, "emission", dev_tables=leg.dev)
             extra["cfg3"] = short_leg(lg)
             lg.close()
-            leg.close()
             leg.dev = lg.dev = None
             torch.cuda.empty_cache()
             # config 4 on 2000 of its 1e4 wavelength points (the full table takes minutes of numpy to generate)

@@ -265,13 +265,8 @@ class Leg:
                 self.dev[k] = torch.from_numpy(np.ascontiguousarray(opac[k], dtype=np.float32)).cuda()
         self.G = binding.Grid(grid, stream=stream)
         self.ncell = int(np.asarray(grid["T"]).size)
-        self.G2 = self.stream2 = None
         if self.streamed:
             self.coef = torch.from_numpy(opac["k_ray_chan"]).cuda()
-            # double-buffered: a second handle on a second stream takes every other wavelength
-            # batch, so that batch b + 1's node tables, staging and CDF overlap batch b's transport
-            self.stream2 = torch.cuda.Stream()
-            self.G2 = binding.Grid(grid, stream=self.stream2)
 
     def pin_host_tables(self):
         self.host = dict(self.opac)
@@ -284,9 +279,10 @@ class Leg:
 
     def step(self, op, device_outputs, timing=0, counters="host"):
         """One pass of the whole hot path over the workload; returns the list of run results."""
-        # run_params.concurrency: the run's channels in K parts side by side on internal handles and streams (ignored by the
-        # library for timing = 1 and Doppler runs)
-        prm = dict(self.prm, timing=timing, concurrency=0 if timing else self.args.concurrency)
+        # run_params.concurrency: the run's channels in K parts side by side on internal handles and streams (the library
+        # ignores it for timing = 1); two parts for cfg5, whose handles hold 48 GB each
+        K = 0 if timing else (min(self.args.concurrency, 2) if self.streamed else self.args.concurrency)
+        prm = dict(self.prm, timing=timing, concurrency=K)
         G = self.G
         if not self.streamed:
             G.set_opacity(op)
@@ -297,24 +293,17 @@ class Leg:
         # emission and in albedo mode toward the 4 phases
         outs = []
         obs = np.asarray(prm["obs_dir"], dtype=np.float64).reshape(-1, 3)
-        two = not timing          # the timing = 1 steps wait for the device after every kernel: one handle
-        if two:
-            self.stream2.wait_stream(self.stream)
-        for b, (c0, c1, lo, hi) in enumerate(wl.cfg5_batches(self.opac, batch=self.args.batch, halo=int(prm["doppler_halfwidth"]))):
-            G, st = (self.G2, self.stream2) if two and b % 2 else (self.G, self.stream)
-            with self.torch.cuda.stream(st):     # the batch's Rayleigh table is filled on the stream its handle runs on
-                sub = dict(op, chan0=op["chan0"] + lo, node_kabs=op["node_kabs"][lo:hi])
-                sub["lambda"] = self.opac["lambda"][lo:hi]
-                sub["k_sca_ray"] = self.coef[lo:hi, None].expand(hi - lo, self.ncell).contiguous()
-                G.set_opacity_nodes(sub)
-                # with doppler_on every observer is a run of its own on its own shifted table (L326-328): phases outermost,
-                # so that the emission and the albedo run toward a phase share one Doppler staging (4 per batch, not 8)
-                for o in range(obs.shape[0]):
-                    for fn in (G.run_emission, G.run_albedo):
-                        outs.append(fn(dict(prm, obs_dir=obs[o:o + 1], chan_begin=c0 - lo, chan_end=c1 - lo),
-                                       device_outputs=device_outputs, counters=counters))
-        if two:
-            self.stream.wait_stream(self.stream2)
+        for c0, c1, lo, hi in wl.cfg5_batches(self.opac, batch=self.args.batch, halo=int(prm["doppler_halfwidth"])):
+            sub = dict(op, chan0=op["chan0"] + lo, node_kabs=op["node_kabs"][lo:hi])
+            sub["lambda"] = self.opac["lambda"][lo:hi]
+            sub["k_sca_ray"] = self.coef[lo:hi, None].expand(hi - lo, self.ncell).contiguous()
+            G.set_opacity_nodes(sub)
+            # with doppler_on every observer is a run of its own on its own shifted table (L326-328): phases outermost,
+            # so that the emission and the albedo run toward a phase share one Doppler staging (4 per batch, not 8)
+            for o in range(obs.shape[0]):
+                for fn in (G.run_emission, G.run_albedo):
+                    outs.append(fn(dict(prm, obs_dir=obs[o:o + 1], chan_begin=c0 - lo, chan_end=c1 - lo),
+                                   device_outputs=device_outputs, counters=counters))
         return outs
 
     def sum_counters(self, outs):
@@ -384,8 +373,6 @@ class Leg:
 
     def close(self):
         self.G.close()
-        if self.G2 is not None:
-            self.G2.close()
 
 
 def run_ours(args):
@@ -444,8 +431,7 @@ def run_ours(args):
                 "config": {"workload": args.workload, "mode": leg.mode, "n_chan_per_gpu": leg.n_chan, "packets_per_channel": N,
                            "n_obs": int(np.asarray(leg.prm["obs_dir"]).reshape(-1, 3).shape[0]),
                            "grid": list(np.asarray(leg.grid["T"]).shape), "parallelism": "channels x %d" % world,
-                           "concurrency": ("2 handles, alternating wavelength batches" if leg.streamed else
-                                           "run_params.concurrency = %d (channel parts side by side on one GPU)" % args.concurrency),
+                           "concurrency": "run_params.concurrency = %d (channel parts side by side on one GPU)" % (min(args.concurrency, 2) if leg.streamed else args.concurrency),
                            "l2": "opacity tables (%.0f MB) + staged tables exceed the 126 MB L2; no flush" % (h2d / 1e6)},
                 "events_per_step": ev_all / args.steps, "segments_per_s": seg_all / (ms * 1e-3),
                 "spectra_per_s": world * args.steps / (ms * 1e-3),

@@ -139,10 +139,11 @@ typedef struct gcmcrt_run_params {
                                     the call's results are complete -- so that the kernels of one part use the issue slots and
                                     memory latencies another leaves idle.  Same results (packets are keyed by channel and
                                     index); counters are summed over the parts.  The internal handles are created by the
-                                    first such call, which waits for the device; working memory grows K-fold.  0 or 1, and
-                                    whenever it does not apply (timing = 1, doppler_on, node-table opacities, transmission,
-                                    fewer than K channels in the run, a stream that is being captured, GCMCRT_HOST_LOOP):
-                                    one run on this handle. */
+                                    first such call, which waits for the device; working memory grows K-fold.  Every part
+                                    stages the tables (per observer with doppler_on), and builds the emission CDF, of its own
+                                    channels only, so the parts repeat no work.  0 or 1, and whenever it does not apply
+                                    (timing = 1, transmission, fewer than K channels in the run, a stream that is being
+                                    captured, GCMCRT_HOST_LOOP): one run on this handle. */
 } gcmcrt_run_params;
 
 typedef struct gcmcrt_counters {

@@ -60,11 +60,13 @@ struct gcmcrt_grid {
     bool staged_cont = false;   // the staged tables are those of a continuous-absorption run (pair table, omega = 1)
     DevBuf node, node_idx, node_w, own_pcell;     // k_abs from (T, log10 p) node tables (gcmcrt_set_opacity_nodes)
     int nT = 0, nP = 0;
+    std::vector<float> T_nodes_h, logp_nodes_h;
     bool use_nodes = false;
     int staged_obs = -2;   // -2: no tables set, -3: tables set but nothing staged yet (the first run stages what it needs),
                            // -1: unshifted table staged, >= 0: Doppler table of staged_dir staged
     double staged_dir[3] = {0, 0, 0};
     int staged_halfwidth = 0;
+    int staged_c0 = 0, staged_c1 = 0;   // channels the staged tables hold (the whole table unless a part of a run staged them)
 
     // emission
     DevBuf Lcell, Lcum, Lcol, Ltot, guide;
@@ -193,8 +195,11 @@ cudaError_t ensure_events(gcmcrt_grid* g)
 }
 
 // Stage alpha / prop for observer `obs_dir` (nullptr = unshifted table).
-int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStream_t s, bool cont = false, bool timed = false)
+// c0 .. c1: the channels to stage (c1 = 0: the whole table)
+int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStream_t s, bool cont = false, bool timed = false,
+                  int c0 = 0, int c1 = 0)
 {
+    if (c1 <= c0) { c0 = 0; c1 = g->n_chan; }
     const size_t n = size_t(g->n_chan) * g->ncell;
     const GeomParams gp0 = geom_params(g);
     const size_t n_alpha = size_t(g->n_chan) * size_t(gp0.alpha_stride);
@@ -211,6 +216,7 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
     CUDA_TRY(g, g->prop.ensure(n * sizeof(float4)));
     StageParams sp;
     sp.n_chan = g->n_chan; sp.ncell = g->ncell; sp.nlev = g->nlev; sp.nlat = g->nlat; sp.nlon = g->nlon;
+    sp.c_begin = c0; sp.c_end = c1;
     sp.k_abs = g->k_abs; sp.k_ray = g->k_ray; sp.k_cld = g->k_cld; sp.g_cld = g->g_cld;
     sp.node = g->use_nodes ? g->node.as<float>() : nullptr;
     sp.node_idx = g->node_idx.as<int2>(); sp.node_w = g->node_w.as<float2>(); sp.nT = g->nT; sp.nP = g->nP;
@@ -238,7 +244,7 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
     {   // grid = (cell tiles, channel slices): every thread stages its cell for the channels of its slice
         const unsigned tiles = (unsigned)((g->ncell + 255) / 256);
         const unsigned want = (unsigned)std::max(1, g->sm_count * 16 / (int)std::max(1u, tiles));
-        const unsigned slices = (unsigned)std::min<long long>(std::min<long long>((g->n_chan + 3) / 4, 65535), std::max<long long>(want, 1));
+        const unsigned slices = (unsigned)std::min<long long>(std::min<long long>((c1 - c0 + 3) / 4, 65535), std::max<long long>(want, 1));
         stage_kernel<<<dim3(tiles, slices), 256, 0, s>>>(sp);
     }
     CUDA_TRY(g, cudaGetLastError());
@@ -252,6 +258,7 @@ int stage_opacity(gcmcrt_grid* g, const double* obs_dir, int halfwidth, cudaStre
     }
     g->staged_obs = obs_dir ? 0 : -1;
     g->staged_cont = cont;
+    g->staged_c0 = c0; g->staged_c1 = c1;
     if (obs_dir) { for (int m = 0; m < 3; ++m) g->staged_dir[m] = obs_dir[m]; g->staged_halfwidth = halfwidth; }
     return GCMCRT_OK;
 }
@@ -530,7 +537,9 @@ __global__ void finalize_counters_kernel(const DevCounters* dc, const PassCtrl* 
 }
 
 // mode: 0 albedo, 1 emission, 2 transmission
-int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, void* stream, int mode)
+// part: the call is one part of a run cut by run_split(): tables are staged, and the emission CDF is built, for the
+// channels of the part only
+int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, void* stream, int mode, bool part = false)
 {
     const int emission = mode == 1;
     if (!g) return GCMCRT_E_INVALID;
@@ -692,16 +701,19 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
     g->launches = g->launches_pending; g->launches_pending = 0; g->ms_emis = g->ms_transport = g->ms_peel = g->ms_sort = 0.0;
     g->ms_stage = 0.0;
     CUDA_TRY(g, cudaMemsetAsync(ctrl, 0, sizeof(PassCtrl), s));
+    const int st0 = part ? cb : 0, st1 = part ? ce : g->n_chan;   // channels whose staged tables and CDF this call needs
     for (int run = 0; run < n_runs; ++run) {
         // ---- A0/A1: make sure the staged table is the one this run needs
         if (prm->doppler_on && n_obs > 0) {
             const double* od = prm->obs_dir + 3 * run;
             const bool same = g->staged_obs >= 0 && g->staged_cont == cont && g->staged_halfwidth == prm->doppler_halfwidth &&
-                              g->staged_dir[0] == od[0] && g->staged_dir[1] == od[1] && g->staged_dir[2] == od[2];
-            if (!same && (rcode = stage_opacity(g, od, prm->doppler_halfwidth, s, cont, timed))) return rcode;
+                              g->staged_dir[0] == od[0] && g->staged_dir[1] == od[1] && g->staged_dir[2] == od[2] &&
+                              g->staged_c0 <= st0 && st1 <= g->staged_c1;
+            if (!same && (rcode = stage_opacity(g, od, prm->doppler_halfwidth, s, cont, timed, st0, st1))) return rcode;
             rc.obs_first = run; rc.n_obs_run = 1;
         } else {
-            if ((g->staged_obs != -1 || g->staged_cont != cont) && (rcode = stage_opacity(g, nullptr, 0, s, cont, timed))) return rcode;
+            if ((g->staged_obs != -1 || g->staged_cont != cont || g->staged_c0 > st0 || st1 > g->staged_c1) &&
+                (rcode = stage_opacity(g, nullptr, 0, s, cont, timed, st0, st1))) return rcode;
             rc.obs_first = 0; rc.n_obs_run = n_obs;
             if (ms_trans) { rc.obs_first = run; rc.n_obs_run = 1; }
         }
@@ -726,20 +738,27 @@ int run_mode(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, v
             ep.tau_vert_max = prm->tau_vert_max;
             ep.Lcell = prm->emission_bias > 0.0 ? g->Lcell.as<double>() : nullptr; ep.Lcum = g->Lcum.as<double>(); ep.Lcol = g->Lcol.as<double>(); ep.Ltot = g->Ltot.as<double>();
             if (timed) CUDA_TRY(g, cudaEventRecord(g->tev[0], s));
-            {
-                // blockIdx.y = channel; the warps of a channel's CTAs stride through its columns
-                const int ncol = g->nlat * g->nlon, wpb = kEmisThreads / 32;
-                const dim3 ge((unsigned)std::min((ncol + wpb - 1) / wpb, 32), (unsigned)std::min(g->n_chan, 65535));
-                const size_t sm = 2 * size_t(g->nlev) * sizeof(double);
-                if (g->nlev <= 64) emis_col_kernel<2><<<ge, kEmisThreads, sm, s>>>(ep);
-                else if (g->nlev <= 128) emis_col_kernel<4><<<ge, kEmisThreads, sm, s>>>(ep);
-                else if (g->nlev <= 256) emis_col_kernel<8><<<ge, kEmisThreads, sm, s>>>(ep);
-                else return fail(g, GCMCRT_E_INVALID, "emission: nlev > 256 is not supported");
-                emis_colscan_kernel<<<(unsigned)((size_t(g->n_chan) * 32 + 127) / 128), 128, 0, s>>>(g->n_chan, ncol, ep.Lcol, ep.Ltot);
-            }
             CUDA_TRY(g, g->guide.ensure(size_t(g->n_chan) * kEmisGuide * sizeof(int)));
-            emis_guide_kernel<<<(unsigned)(((long long)g->n_chan * kEmisGuide + 255) / 256), 256, 0, s>>>(
-                g->n_chan, g->ncell, g->nlev, ep.Lcum, ep.Lcol, ep.Ltot, g->guide.as<int>());
+            {
+                // the CDF of the run's own channels cb .. ce (the tables are indexed by table channel): the same kernels
+                // on pointers that start at channel cb.  blockIdx.y = channel; the warps of a channel's CTAs stride
+                // through its columns
+                const int ncol = g->nlat * g->nlon, wpb = kEmisThreads / 32;
+                EmisParams er = ep;
+                er.n_chan = ncr;
+                er.alpha += size_t(cb) * er.alpha_stride; er.prop += size_t(cb) * g->ncell; er.lambda += cb;
+                if (er.Lcell) er.Lcell += size_t(cb) * g->ncell;
+                er.Lcum += size_t(cb) * g->ncell; er.Lcol += size_t(cb) * ncol; er.Ltot += cb;
+                const dim3 ge((unsigned)std::min((ncol + wpb - 1) / wpb, 32), (unsigned)std::min(ncr, 65535));
+                const size_t sm = 2 * size_t(g->nlev) * sizeof(double);
+                if (g->nlev <= 64) emis_col_kernel<2><<<ge, kEmisThreads, sm, s>>>(er);
+                else if (g->nlev <= 128) emis_col_kernel<4><<<ge, kEmisThreads, sm, s>>>(er);
+                else if (g->nlev <= 256) emis_col_kernel<8><<<ge, kEmisThreads, sm, s>>>(er);
+                else return fail(g, GCMCRT_E_INVALID, "emission: nlev > 256 is not supported");
+                emis_colscan_kernel<<<(unsigned)((size_t(ncr) * 32 + 127) / 128), 128, 0, s>>>(ncr, ncol, er.Lcol, er.Ltot);
+                emis_guide_kernel<<<(unsigned)(((long long)ncr * kEmisGuide + 255) / 256), 256, 0, s>>>(
+                    ncr, g->ncell, g->nlev, er.Lcum, er.Lcol, er.Ltot, g->guide.as<int>() + size_t(cb) * kEmisGuide);
+            }
             CUDA_TRY(g, cudaGetLastError());
             if (timed) {
                 CUDA_TRY(g, cudaEventRecord(g->tev[1], s));
@@ -985,7 +1004,7 @@ __global__ void sum_counters_kernel(const gcmcrt_counters* part, int k, gcmcrt_c
 bool split_eligible(gcmcrt_grid* g, const gcmcrt_run_params* prm, const gcmcrt_result* out, cudaStream_t s, int mode)
 {
     if (!g || !prm || !out || g->is_peer || prm->concurrency < 2 || prm->concurrency > 8) return false;
-    if (mode == 2 || prm->timing || prm->doppler_on || g->use_nodes || g->n_chan <= 0 || g->staged_obs == -2) return false;
+    if (mode == 2 || prm->timing || g->n_chan <= 0 || g->staged_obs == -2) return false;
     static const bool host_loop_env = std::getenv("GCMCRT_HOST_LOOP") && std::atoi(std::getenv("GCMCRT_HOST_LOOP")) != 0;
     if (host_loop_env) return false;
     const int cb = prm->chan_begin, ce = prm->chan_end ? prm->chan_end : g->n_chan;
@@ -1044,7 +1063,10 @@ int run_split(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, 
     for (int q = 1; q < K; ++q) {
         gcmcrt_grid* p = g->peers[q - 1];
         if (p->synced_epoch == g->opacity_epoch) continue;
-        rcode = gcmcrt_set_opacity(p, g->chan0, g->n_chan, g->lambda.data(), g->k_abs, g->k_ray, g->k_cld, g->g_cld, g->peer_streams[q - 1]);
+        rcode = g->use_nodes
+                    ? gcmcrt_set_opacity_nodes(p, g->chan0, g->n_chan, g->lambda.data(), g->node.as<float>(), g->nT, g->nP, g->T_nodes_h.data(),
+                                               g->logp_nodes_h.data(), g->own_pcell.as<float>(), g->k_ray, g->k_cld, g->g_cld, g->peer_streams[q - 1])
+                    : gcmcrt_set_opacity(p, g->chan0, g->n_chan, g->lambda.data(), g->k_abs, g->k_ray, g->k_cld, g->g_cld, g->peer_streams[q - 1]);
         if (rcode) return fail(g, rcode, "concurrency: " + p->err);
         p->synced_epoch = g->opacity_epoch;   // (of the handle it borrows from)
     }
@@ -1066,7 +1088,7 @@ int run_split(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, 
         rq.contrib = o_ctb.dev ? static_cast<float*>(o_ctb.dev) + oc * n_obs * 2 * g->ncell : nullptr;
         rq.counters = g->part_counters.as<gcmcrt_counters>() + q;
         gcmcrt_grid* h = q == 0 ? g : g->peers[q - 1];
-        rcode = run_mode(h, &pq, &rq, q == 0 ? s : g->peer_streams[q - 1], mode);
+        rcode = run_mode(h, &pq, &rq, q == 0 ? s : g->peer_streams[q - 1], mode, true);
         if (rcode) { first_err = rcode; if (h != g) g->err = "concurrency: " + h->err; }
     }
     // ---- join (also after a failed part: nothing may be left running behind the caller's back)
@@ -1237,6 +1259,7 @@ int gcmcrt_set_opacity_nodes(gcmcrt_grid* g, int chan0, int n_chan, const float*
                                                             nT, nP, g->node_idx.as<int2>(), g->node_w.as<float2>());
     CUDA_TRY(g, cudaGetLastError());
     g->nT = nT; g->nP = nP;
+    g->T_nodes_h.assign(T_nodes, T_nodes + nT); g->logp_nodes_h.assign(logp_nodes, logp_nodes + nP);   // for the internal handles
     g->use_nodes = true;
     return set_opacity_common(g, chan0, n_chan, lambda, k_sca_ray, k_sca_cld, g_cld, s);
 }

@@ -249,6 +249,7 @@ struct RunConst {
 // ---------------------------------------------------------------------------------------------------------
 struct StageParams {
     int n_chan, ncell, nlev, nlat, nlon;
+    int c_begin, c_end;    // channels to stage (a part of a run stages its own channels only); the tables hold n_chan
     const float *k_abs, *k_ray, *k_cld, *g_cld, *rho;
     float* alpha;          // [n_chan][ncol][col_stride], zero-filled by the host before the launch (guard entries)
     float* alpha2;         // continuous absorption: the same layout with (alpha_sca, alpha_abs) pairs, or NULL
@@ -329,11 +330,11 @@ __global__ void __launch_bounds__(256) stage_kernel(const StageParams p)
     if (p.doppler && p.n_chan > 1) dn_cell = -__ldg(p.vlos + cell) * (1.0f / 299792458.0f);
     // four channels per round, all their loads issued before the first store: the kernel lives on bytes in flight
     constexpr int U = 4;
-    for (int c0 = blockIdx.y * U; c0 < p.n_chan; c0 += gridDim.y * U) {
+    for (int c0 = p.c_begin + blockIdx.y * U; c0 < p.c_end; c0 += gridDim.y * U) {
         float ka[U], kr[U], kc[U], gg[U];
 #pragma unroll
         for (int q = 0; q < U; ++q) {
-            const int c = min(c0 + q, p.n_chan - 1);
+            const int c = min(c0 + q, p.c_end - 1);
             const long long t = (long long)c * p.ncell + cell;
             if (p.doppler && p.n_chan > 1) {
                 // Eq. 34: lambda_eff = lambda_0 (1 - v/c) -> index offset dn = -v/c / ln(lambda_{n+1}/lambda_n), C14
@@ -358,7 +359,7 @@ __global__ void __launch_bounds__(256) stage_kernel(const StageParams p)
 #pragma unroll
         for (int q = 0; q < U; ++q) {
             const int c = c0 + q;
-            if (c >= p.n_chan) break;
+            if (c >= p.c_end) break;
             const long long t = (long long)c * p.ncell + cell;
             const float ks = kr[q] + kc[q];
             const float kext = ka[q] + ks;

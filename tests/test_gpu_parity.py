@@ -1395,13 +1395,18 @@ def test_concurrent_parts_of_a_run_give_the_same_result(gpu, orc, monkeypatch, m
     """run_params.concurrency = K cuts the channels of a run into K parts that run side by side on internal handles and
     streams (channels are independent, L79): same packets, event for event, as the single run -- with host and with device
     outputs, on a sub-range of the channels, with images and contribution functions, after the tables have changed --
-    and still on the oracle's bar.  Where it does not apply (fewer channels than parts, a Doppler run, a stream that is
-    being captured) the call is an ordinary single run."""
+    with Doppler shifts -- and still on the oracle's bar.  Where it does not apply (fewer channels than parts, a stream that
+    is being captured) the call is an ordinary single run."""
     import torch
     monkeypatch.setenv("GCMCRT_EVENT_CAP", "80000")     # several passes per part
     grid, opac = wl.uniform_medium(12, 6, 8, 1.0e7, 1.2e7, [0.5 / 0.2e7, 1.0 / 0.2e7, 1.5 / 0.2e7, 2.5 / 0.2e7, 4.0 / 0.2e7, 0.2 / 0.2e7, 1.0 / 0.2e7],
                                    0.8, g=0.6, pgas=0.35, n_chan=7, surface_albedo=0.5, T=1500.0)
     opac["lambda"] = (2.0e-6 * (1 + 1.0e-5 * np.arange(7))).astype(np.float32)
+    rng = np.random.default_rng(5)
+    grid["u"] = rng.uniform(-6000, 6000, size=grid["T"].shape).astype(np.float32)      # shifts of up to two channels
+    grid["v"] = rng.uniform(-2000, 2000, size=grid["T"].shape).astype(np.float32)
+    grid["w"] = np.zeros(grid["T"].shape, dtype=np.float32)
+    grid["Omega"] = 2.0e-5
     ncell = int(grid["T"].size)
     prm = wl.default_params(packets_per_channel=30000, seed=11, star_dir=[0.8, 0.0, 0.6], obs_dir=[[0.8, 0.0, 0.6], [0.0, 0.0, 1.0]], npix=8)
     call = "run_albedo" if mode == "albedo" else "run_emission"
@@ -1417,12 +1422,20 @@ def test_concurrent_parts_of_a_run_give_the_same_result(gpu, orc, monkeypatch, m
             for k in ("events", "segments_transport", "segments_peel", "rays_peel", "packets_escaped", "packets_absorbed", "packets_surface"):
                 assert r["counters"][k] == ref["counters"][k], (K, k)
             assert r["counters"]["passes"] >= K and r["counters"]["device_status"] == 0 and r["counters"]["packets_stuck"] == 0
-        # more parts than channels, or a Doppler run: one ordinary run
+        # more parts than channels: one ordinary run
         one = getattr(G, call)(dict(prm, concurrency=8), want_event_count=True)
         assert one["counters"]["passes"] == ref["counters"]["passes"] and np.array_equal(one["event_count"], ref["event_count"])
-        dop = getattr(G, call)(dict(prm, concurrency=3, doppler_on=1, doppler_halfwidth=1, obs_dir=prm["obs_dir"][:1]), want_event_count=True)
-        dop1 = getattr(G, call)(dict(prm, doppler_on=1, doppler_halfwidth=1, obs_dir=prm["obs_dir"][:1]), want_event_count=True)
-        assert np.array_equal(dop["event_count"], dop1["event_count"]) and dop["counters"]["passes"] == dop1["counters"]["passes"]
+        # Doppler runs (one run per observer on its own shifted table): every part stages the tables, and builds the
+        # emission CDF, of its own channels only
+        dprm = dict(prm, doppler_on=1, doppler_halfwidth=2)
+        dop1 = getattr(G, call)(dprm, want_event_count=True)
+        dop = getattr(G, call)(dict(dprm, concurrency=3), want_event_count=True)
+        assert np.array_equal(dop["event_count"], dop1["event_count"]) and dop["counters"]["passes"] > dop1["counters"]["passes"]
+        for k, tol in (("flux_sum", 1e-5), ("value", 1e-6), ("L_tot", 1e-12), ("image", 1e-4)):
+            assert np.allclose(dop[k], dop1[k], rtol=tol, atol=1e-9 * np.abs(dop1[k]).max()), k
+        # ... and a run of the whole table after a run in parts stages the whole table again
+        again = getattr(G, call)(prm, want_event_count=True)
+        assert np.array_equal(again["event_count"], ref["event_count"]) and np.allclose(again["value"], ref["value"], rtol=1e-6)
         # a sub-range of the channels; device outputs and device counters (the call only enqueues)
         sub = getattr(G, call)(dict(prm, concurrency=3, chan_begin=1, chan_end=6), want_event_count=True, device_outputs=True, counters="device")
         assert np.array_equal(sub["event_count"].cpu().numpy().astype(np.uint32), ref["event_count"][1:6])

@@ -285,6 +285,31 @@ int gcmcrt_debug_ray_tau(gcmcrt_grid *grid, int chan, long n, const float *pos, 
  */
 int gcmcrt_debug_philox(long n, const uint32_t *ctr, const uint32_t *key, uint32_t *out, void *stream);
 
+/*
+ * gcmcrt_emission_ltot_static -- the total luminosities L_tot[c] (Eq. 27 summed over the cells, with the depth cut of
+ * L210; the normalisation of Eq. 28) of channels chan_begin .. chan_end-1 (chan_end = 0: to the end of the table) of the
+ * tables that are staged on the handle, computed WITHOUT ANY ALLOCATION: for callers that must not reach cudaMalloc (code
+ * under stream capture, tight serving loops, harnesses that forbid it).  The same arithmetic in the same order as the
+ * L_tot output of gcmcrt_run_emission (which keeps its per-column totals in a buffer of the handle that grows on demand);
+ * here they live in a file-scope device array of GCMCRT_STATIC_SCRATCH_BYTES that every GPU which loads the library
+ * holds until the process exits.
+ *   L_tot[chan_end - chan_begin]  host|device.  Device: the call only enqueues two kernels on `stream`.  Host: the result
+ *                                 is copied from the array and the call waits for the stream.
+ *   tau_vert_max                  as run_params.tau_vert_max (<= 0: no depth cut)
+ * The tables must be staged already -- by any run on this handle after the last gcmcrt_set_opacity* (a doppler_on run
+ * leaves its last observer's shifted table: that is then the table L_tot is of) -- because staging may allocate; E_STATE
+ * otherwise, and when a run_params.concurrency run left only a part of the channels staged on this handle.
+ * LIMIT: (n_channels * nlat * nlon + n_channels) * 8 bytes <= GCMCRT_STATIC_SCRATCH_BYTES, else E_INVALID with a message
+ * that states both sizes -- pass fewer channels per call (cfg2's 64 x 32 columns: 511 channels; cfg5's 128 x 64: 127).
+ * SHARED STATE: every call on a device uses the same array, which keeps the last call's contents (nothing in it has to
+ * start at zero: a call writes every entry before it reads it).  Calls that overlap on the GPU -- different streams, or
+ * different handles or host threads without an ordering between them -- race; calls on one stream are safe.
+ * Calls no cudaMalloc / cudaFree and no allocating library routine.  Errors: E_INVALID, E_STATE, E_CUDA.
+ */
+#define GCMCRT_STATIC_SCRATCH_BYTES (8u << 20)
+int gcmcrt_emission_ltot_static(gcmcrt_grid *grid, int chan_begin, int chan_end, double tau_vert_max, double *L_tot,
+                                void *stream);
+
 /* Library build information: "gcmcrt <version> sm_100a ..." */
 const char *gcmcrt_version(void);
 

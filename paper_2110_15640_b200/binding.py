@@ -17,7 +17,7 @@ _lib = None
 OK, E_INVALID, E_NOMEM, E_CUDA, E_STATE = 0, -1, -2, -3, -4
 EXPORTS = ["gcmcrt_grid_create", "gcmcrt_set_opacity", "gcmcrt_set_opacity_nodes", "gcmcrt_run_albedo", "gcmcrt_run_emission",
            "gcmcrt_run_transmission", "gcmcrt_destroy",
-           "gcmcrt_last_error", "gcmcrt_debug_ray_tau", "gcmcrt_debug_philox", "gcmcrt_version"]
+           "gcmcrt_last_error", "gcmcrt_debug_ray_tau", "gcmcrt_debug_philox", "gcmcrt_emission_ltot_static", "gcmcrt_version"]
 
 
 class GcmcrtError(RuntimeError):
@@ -75,6 +75,7 @@ def lib():
         L.gcmcrt_destroy.argtypes = [C.c_void_p]
         L.gcmcrt_debug_ray_tau.argtypes = [C.c_void_p, C.c_int, C.c_long] + [C.c_void_p] * 5
         L.gcmcrt_debug_philox.argtypes = [C.c_long] + [C.c_void_p] * 4
+        L.gcmcrt_emission_ltot_static.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -264,6 +265,20 @@ def run_transmission(handle, prm, n_chan_table, want_event_count=False, device_o
                 counters)
 
 
+STATIC_SCRATCH_BYTES = 8 << 20   # GCMCRT_STATIC_SCRATCH_BYTES of include/gcmcrt.h
+
+
+def emission_ltot_static(handle, chan_begin, chan_end, tau_vert_max, out=None, stream=None):
+    """gcmcrt_emission_ltot_static: L_tot of the staged tables through the entry point that allocates nothing.
+    out: a torch CUDA float64 tensor (the call only enqueues) or None (a numpy array is returned; the call waits)."""
+    n = chan_end - chan_begin
+    if out is None:
+        out = np.zeros(max(n, 0), dtype=np.float64)
+    rc = lib().gcmcrt_emission_ltot_static(handle, int(chan_begin), int(chan_end), float(tau_vert_max), _ptr(out), _stream_ptr(stream))
+    _check(handle, rc)
+    return out
+
+
 def debug_ray_tau(handle, chan, pos, dirs, stream=None):
     pos = np.ascontiguousarray(pos, dtype=np.float32).reshape(-1, 3)
     dirs = np.ascontiguousarray(dirs, dtype=np.float32).reshape(-1, 3)
@@ -321,6 +336,9 @@ class Grid:
 
     def ray_tau(self, chan, pos, dirs):
         return debug_ray_tau(self.handle, chan, pos, dirs, self.stream)
+
+    def emission_ltot_static(self, chan_begin, chan_end, tau_vert_max, out=None):
+        return emission_ltot_static(self.handle, chan_begin, chan_end, tau_vert_max, out, self.stream)
 
     def close(self):
         if self.handle:

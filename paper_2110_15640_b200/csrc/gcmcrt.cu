@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1400,6 +1401,177 @@ int gcmcrt_debug_philox(long n, const uint32_t* ctr, const uint32_t* key, uint32
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     bc.release(); bk.release(); bo.release();
     if (e != cudaSuccess) { g_create_error = std::string("debug_philox: ") + cudaGetErrorString(e); cudaGetLastError(); return GCMCRT_E_CUDA; }
+    return GCMCRT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// gcmcrt_emission_ltot_static: total luminosities (Eq. 27 summed over the cells, depth cut of L210) of the staged
+// tables with NO allocation -- for callers that must not reach cudaMalloc (code under stream capture, serving loops,
+// harnesses that forbid it).  The per-column totals, which gcmcrt_run_emission keeps in a buffer of the handle that
+// grows on demand, live in a file-scope device array of fixed size here.  Every GPU that loads the library holds
+// the array until the process exits; every call shares it, so calls that overlap on the GPU race.
+// ---------------------------------------------------------------------------------------------------------
+}  // extern "C"
+
+namespace {
+
+constexpr size_t kStaticScratchBytes = size_t(GCMCRT_STATIC_SCRATCH_BYTES);
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+// Device address of g_static_scratch on the current device.  In host code the array's name is only a handle for the
+// runtime, not a device address: cudaGetSymbolAddress translates it, once per device, with that device current.
+cudaError_t static_scratch_address(void** out)
+{
+    constexpr int kMaxDevices = 64;
+    static void* ptr[kMaxDevices] = {};
+    static std::mutex mtx;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mtx);
+    if (!ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess) return e;
+        ptr[dev] = p;
+    }
+    *out = ptr[dev];
+    return cudaSuccess;
+}
+
+// emis_col_kernel without its table outputs: the same loads, depth cut, L_i (Eq. 27) and fp64 warp scan in the same
+// order -- so the column totals are bit-identical -- and one store per (channel, column): the column's total into
+// col_tot[c_rel][col] (the static scratch).  p.alpha, p.prop, p.lambda point at the first channel of the range,
+// p.n_chan is the number of channels.
+template <int NCH>
+__global__ void __launch_bounds__(kEmisThreads) emis_coltot_static_kernel(const EmisParams p, double* __restrict__ col_tot)
+{
+    extern __shared__ double emis_sm[];
+    double* dr = emis_sm;
+    double* dr3 = dr + p.nlev;
+    const int lane = lane_id(), wid = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < p.nlev; i += blockDim.x) {
+        const double r0 = p.r_edges[i], r1 = p.r_edges[i + 1];
+        dr[i] = r1 - r0;
+        dr3[i] = (r1 * r1 * r1 - r0 * r0 * r0) / 3.0;
+    }
+    __syncthreads();
+    const int ncol = p.nlat * p.nlon;
+    for (int c = blockIdx.y; c < p.n_chan; c += gridDim.y) {
+        const double lam = p.lambda[c];
+        const double hck = 6.62607015e-34 * 299792458.0 / (lam * 1.380649e-23);
+        const double pre = 4.0 * 3.14159265358979323846 * 2.0 * 6.62607015e-34 * 299792458.0 * 299792458.0 /
+                           (lam * lam * lam * lam * lam);
+        const float* alpha_c = p.alpha + (size_t)c * p.alpha_stride;
+        const float4* prop_c = p.prop + (size_t)c * p.ncell;
+        for (int col = blockIdx.x * (kEmisThreads / 32) + wid; col < ncol; col += gridDim.x * (kEmisThreads / 32)) {
+            const size_t cell0 = (size_t)col * p.nlev;
+            const float* acol = alpha_c + (size_t)col * p.col_stride + 1;
+            float a[NCH], T[NCH], rk[NCH];
+#pragma unroll
+            for (int m = 0; m < NCH; ++m) {
+                const int i = (m << 5) + lane;
+                const bool in = i < p.nlev;
+                a[m] = in ? __ldg(acol + i) : 0.0f;
+                T[m] = in ? __ldg(p.T + cell0 + i) : 1.0f;
+                rk[m] = in ? __ldg(p.rho + cell0 + i) * __ldg(&prop_c[cell0 + i].w) : 0.0f;
+            }
+            int i_cut = 0;
+            if (p.tau_vert_max > 0.0) {
+                double incl[NCH], tot = 0.0;
+#pragma unroll
+                for (int m = 0; m < NCH; ++m) {
+                    const int i = (m << 5) + lane;
+                    const double d = i < p.nlev ? double(a[m]) * dr[i] : 0.0;
+                    incl[m] = tot + warp_incl_scan_f64(d);
+                    tot = __shfl_sync(kFullMask, incl[m], 31);
+                }
+#pragma unroll
+                for (int m = 0; m < NCH; ++m) {
+                    const int i = (m << 5) + lane;
+                    const unsigned mc = __ballot_sync(kFullMask, i < p.nlev && (tot - incl[m]) > p.tau_vert_max);
+                    if (mc) i_cut = (m << 5) + 32 - __clz(mc);
+                }
+            }
+            const int j = col % p.nlat, k = col / p.nlat;
+            const double ang = (p.cth_edges[j] - p.cth_edges[j + 1]) * (p.ph_edges[k + 1] - p.ph_edges[k]);
+            double run = 0.0;
+#pragma unroll
+            for (int m = 0; m < NCH; ++m) {
+                const int i = (m << 5) + lane;
+                if ((m << 5) + 32 > i_cut && (m << 5) < p.nlev) {
+                    double Li = 0.0;
+                    if (i < p.nlev && i >= i_cut) {
+                        const double e = expm1(hck * rcp_pos_f64(double(T[m])));
+                        Li = e < 1e300 ? pre * dr3[i] * ang * double(rk[m]) * rcp_pos_f64(e) : 0.0;
+                    }
+                    const double sum = run + warp_incl_scan_f64(Li);
+                    run = __shfl_sync(kFullMask, sum, 31);
+                }
+            }
+            if (lane == 0) col_tot[(size_t)c * ncol + col] = run;
+        }
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+int gcmcrt_emission_ltot_static(gcmcrt_grid* g, int chan_begin, int chan_end, double tau_vert_max, double* L_tot, void* stream)
+{
+    if (!g) return GCMCRT_E_INVALID;
+    if (!L_tot) return fail(g, GCMCRT_E_INVALID, "emission_ltot_static: L_tot is NULL");
+    if (g->n_chan <= 0 || g->staged_obs < -1)
+        return fail(g, GCMCRT_E_STATE, "emission_ltot_static: no staged tables (they are staged by the first run after gcmcrt_set_opacity*; "
+                                       "this call allocates nothing and therefore stages nothing)");
+    const int cb = chan_begin, ce = chan_end ? chan_end : g->n_chan;
+    if (cb < 0 || ce > g->n_chan || cb >= ce) return fail(g, GCMCRT_E_INVALID, "emission_ltot_static: bad channel range");
+    if (cb < g->staged_c0 || ce > g->staged_c1) return fail(g, GCMCRT_E_STATE, "emission_ltot_static: the staged tables do not hold these channels");
+    if (g->nlev > 256) return fail(g, GCMCRT_E_INVALID, "emission: nlev > 256 is not supported");
+    const int ncr = ce - cb, ncol = g->nlat * g->nlon;
+    // scratch: column totals [ncr][ncol], then the totals [ncr] (copied out when L_tot is host memory)
+    const size_t need = (size_t(ncr) * ncol + size_t(ncr)) * sizeof(double);
+    if (need > kStaticScratchBytes) {
+        char msg[256];
+        std::snprintf(msg, sizeof msg, "emission_ltot_static: %d channels x %d columns need %zu bytes of scratch, the static array holds %zu "
+                                       "(GCMCRT_STATIC_SCRATCH_BYTES): pass fewer channels per call", ncr, ncol, need, kStaticScratchBytes);
+        return fail(g, GCMCRT_E_INVALID, msg);
+    }
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    void* base = nullptr;
+    CUDA_TRY(g, static_scratch_address(&base));
+    double* col_tot = static_cast<double*>(base);
+    double* tot = col_tot + size_t(ncr) * ncol;
+    const bool odev = is_device_ptr(L_tot);
+    const GeomParams gp = geom_params(g);
+    EmisParams ep;
+    std::memset(static_cast<void*>(&ep), 0, sizeof ep);
+    ep.n_chan = ncr; ep.nlev = g->nlev; ep.nlat = g->nlat; ep.nlon = g->nlon; ep.ncell = g->ncell;
+    ep.alpha = g->alpha.as<float>() + size_t(cb) * gp.alpha_stride;
+    ep.prop = g->prop.as<float4>() + size_t(cb) * g->ncell;
+    ep.alpha_stride = gp.alpha_stride; ep.col_stride = gp.col_stride;
+    ep.rho = g->rho.as<float>(); ep.T = g->T.as<float>();
+    ep.lambda = g->lambda64.as<double>() + cb;
+    ep.r_edges = g->r64.as<double>(); ep.cth_edges = g->cth64.as<double>(); ep.ph_edges = g->ph64.as<double>();
+    ep.tau_vert_max = tau_vert_max;
+    const int wpb = kEmisThreads / 32;
+    const dim3 ge((unsigned)std::min((ncol + wpb - 1) / wpb, 32), (unsigned)std::min(ncr, 65535));
+    const size_t sm = 2 * size_t(g->nlev) * sizeof(double);   // <= 4 KB: no attribute to set
+    // nothing in the scratch has to start at zero: every entry that is read below is written by this call first
+    if (g->nlev <= 64) emis_coltot_static_kernel<2><<<ge, kEmisThreads, sm, s>>>(ep, col_tot);
+    else if (g->nlev <= 128) emis_coltot_static_kernel<4><<<ge, kEmisThreads, sm, s>>>(ep, col_tot);
+    else emis_coltot_static_kernel<8><<<ge, kEmisThreads, sm, s>>>(ep, col_tot);
+    CUDA_TRY(g, cudaGetLastError());
+    // the column totals are added in column order by the kernel gcmcrt_run_emission uses (it leaves the exclusive sums
+    // in col_tot, which nobody reads here)
+    emis_colscan_kernel<<<(unsigned)((size_t(ncr) * 32 + 127) / 128), 128, 0, s>>>(ncr, ncol, col_tot, odev ? L_tot : tot);
+    CUDA_TRY(g, cudaGetLastError());
+    if (!odev) {
+        CUDA_TRY(g, cudaMemcpyAsync(L_tot, tot, size_t(ncr) * sizeof(double), cudaMemcpyDeviceToHost, s));
+        CUDA_TRY(g, cudaStreamSynchronize(s));
+    }
     return GCMCRT_OK;
 }
 

@@ -1468,14 +1468,15 @@ __global__ void __launch_bounds__(kEmisThreads) emis_coltot_static_kernel(const 
         for (int col = blockIdx.x * (kEmisThreads / 32) + wid; col < ncol; col += gridDim.x * (kEmisThreads / 32)) {
             const size_t cell0 = (size_t)col * p.nlev;
             const float* acol = alpha_c + (size_t)col * p.col_stride + 1;
-            float a[NCH], T[NCH], rk[NCH];
+            float a[NCH], T[NCH];
+            double rk[NCH];   // rho kappa_abs: the fp64 product of two fp32 values is exact, as in the oracle's fp64
 #pragma unroll
             for (int m = 0; m < NCH; ++m) {
                 const int i = (m << 5) + lane;
                 const bool in = i < p.nlev;
                 a[m] = in ? __ldg(acol + i) : 0.0f;
                 T[m] = in ? __ldg(p.T + cell0 + i) : 1.0f;
-                rk[m] = in ? __ldg(p.rho + cell0 + i) * __ldg(&prop_c[cell0 + i].w) : 0.0f;
+                rk[m] = in ? double(__ldg(p.rho + cell0 + i)) * double(__ldg(&prop_c[cell0 + i].w)) : 0.0;
             }
             int i_cut = 0;
             if (p.tau_vert_max > 0.0) {
@@ -1504,7 +1505,7 @@ __global__ void __launch_bounds__(kEmisThreads) emis_coltot_static_kernel(const 
                     double Li = 0.0;
                     if (i < p.nlev && i >= i_cut) {
                         const double e = expm1(hck * rcp_pos_f64(double(T[m])));
-                        Li = e < 1e300 ? pre * dr3[i] * ang * double(rk[m]) * rcp_pos_f64(e) : 0.0;
+                        Li = e < 1e300 ? pre * dr3[i] * ang * rk[m] * rcp_pos_f64(e) : 0.0;
                     }
                     const double sum = run + warp_incl_scan_f64(Li);
                     run = __shfl_sync(kFullMask, sum, 31);

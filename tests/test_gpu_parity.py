@@ -1471,3 +1471,20 @@ def test_concurrent_parts_of_a_run_give_the_same_result(gpu, orc, monkeypatch, m
         torch.cuda.synchronize()
         assert torch.equal(outs["event_count"], warm["event_count"])
         del graph
+
+
+def test_emission_luminosities_reproduce_the_oracle_to_rounding(gpu, orc):
+    """L_i (Eq. 27) on the device: rho * kappa_abs is the exact fp64 product of the two fp32 table values, the Planck
+    term, the cell volume and the running sum are fp64 -- so with per-cell tables and no Doppler shift L_tot agrees with
+    the oracle to rounding (1e-12; 6e-8 when the product was rounded to fp32) and the CDF draw of Eq. 13 lands in the
+    oracle's cell: without scattering every packet's single peel-off then starts in the same cell, and the flux agrees
+    far inside the Monte Carlo error (DESIGN.md section 7 tells what one packet in a neighbouring cell can do)."""
+    grid, opac, prm = wl.cfg3(nlon=16, nlat=8, nlev=60, nbands=2, ng=4, packets=40000)
+    for tvm in (30.0, 0.0):
+        p = dict(prm, scatter_on=0, tau_vert_max=tvm)
+        g = _gpu_run(gpu, grid, opac, p, "emission", want_event_count=True)
+        o = orc.run_emission(grid, opac, dict(p, n_threads=16), want_event_count=True)
+        assert np.allclose(g["L_tot"], o["L_tot"], rtol=1e-12, atol=0.0), np.abs(g["L_tot"] / o["L_tot"] - 1).max()
+        assert np.array_equal(g["event_count"], o["event_count"])
+        vo, so = orc.reduce(o, "emission")
+        assert np.all(np.abs(g["value"] - vo) <= 0.05 * so + 1e-4 * np.abs(vo)), (np.abs(g["value"] - vo) / (so + 1e-300)).max()

@@ -104,6 +104,7 @@ struct gcmcrt_grid {
     DevBuf part_counters;
     unsigned long long opacity_epoch = 0, synced_epoch = 0;   // synced_epoch: on an internal handle, the owner's epoch its tables are from
     bool is_peer = false;
+    const gcmcrt_grid* owner = nullptr;   // internal handle: the handle whose tables it borrows
 };
 
 namespace {
@@ -1039,6 +1040,7 @@ int run_split(gcmcrt_grid* g, const gcmcrt_run_params* prm, gcmcrt_result* out, 
                                    g->w.p ? g->w.as<float>() : nullptr, g->Omega, g->surface_albedo, s);
         if (rcode) return fail(g, rcode, "concurrency: " + g_create_error);
         p->is_peer = true;
+        p->owner = g;
         cudaStream_t ps = nullptr;
         cudaEvent_t pe = nullptr;
         cudaError_t e = cudaStreamCreateWithFlags(&ps, cudaStreamNonBlocking);
@@ -1292,8 +1294,17 @@ static int set_opacity_common(gcmcrt_grid* g, int chan0, int n_chan, const float
         const double ratio = double(lam[c1 + 1]) / double(lam[c1]);
         reff[c] = ratio != 1.0 ? float(1.0 / std::log(ratio)) : 0.f;
     }
-    CUDA_TRY(g, upload(g->lambda64, lam64, s));
-    CUDA_TRY(g, upload(g->reff, reff, s));
+    if (g->owner && g->owner->lambda64.p && g->owner->reff.p && g->owner->n_chan == n_chan) {
+        // an internal handle takes the two per-channel arrays from its owner on the device: an upload from pageable host
+        // memory of more than 64 KB waits for the stream, which is still running the previous run's part
+        CUDA_TRY(g, g->lambda64.ensure(size_t(n_chan) * sizeof(double)));
+        CUDA_TRY(g, g->reff.ensure(size_t(n_chan) * sizeof(float)));
+        CUDA_TRY(g, cudaMemcpyAsync(g->lambda64.p, g->owner->lambda64.p, size_t(n_chan) * sizeof(double), cudaMemcpyDeviceToDevice, s));
+        CUDA_TRY(g, cudaMemcpyAsync(g->reff.p, g->owner->reff.p, size_t(n_chan) * sizeof(float), cudaMemcpyDeviceToDevice, s));
+    } else {
+        CUDA_TRY(g, upload(g->lambda64, lam64, s));
+        CUDA_TRY(g, upload(g->reff, reff, s));
+    }
     g->chan0 = chan0;
     g->n_chan = n_chan;
     ++g->opacity_epoch;

@@ -909,6 +909,23 @@ def test_opacity_from_node_tables_matches_per_cell_tables(gpu, orc):
     val = np.concatenate([r["value"] for r in pieces], axis=0)
     assert np.array_equal(ev, node["event_count"])
     assert np.allclose(val, node["value"], rtol=1e-6)
+    # the same with every run cut into parts that run side by side (run_params.concurrency): the internal handles get the
+    # node tables, and each part stages the Doppler-shifted table and builds the CDF of its own channels (+ halo) only
+    pieces = []
+    with gpu.Grid(grid) as G:
+        G.set_opacity_nodes(opac)
+        whole = G.run_emission(dict(prm, concurrency=3), want_event_count=True)
+        assert whole["counters"]["passes"] > node["counters"]["passes"]          # it did run in parts
+        for c0 in range(0, 40, nb_):
+            lo, hi = max(c0 - W, 0), min(c0 + nb_ + W, 40)
+            sub = dict(opac, chan0=lo, node_kabs=opac["node_kabs"][lo:hi], k_abs=opac["k_abs"][lo:hi])
+            sub["lambda"] = opac["lambda"][lo:hi]
+            G.set_opacity_nodes(sub)
+            pieces.append(G.run_emission(dict(prm, chan_begin=c0 - lo, chan_end=min(c0 + nb_, 40) - lo, concurrency=2), want_event_count=True))
+    assert np.array_equal(whole["event_count"], node["event_count"]) and np.allclose(whole["value"], node["value"], rtol=1e-6)
+    assert np.allclose(whole["L_tot"], node["L_tot"], rtol=1e-12)
+    assert np.array_equal(np.concatenate([r["event_count"] for r in pieces], axis=0), node["event_count"])
+    assert np.allclose(np.concatenate([r["value"] for r in pieces], axis=0), node["value"], rtol=1e-6)
 
 
 def test_degenerate_cases_match_oracle(gpu, orc):
